@@ -1,0 +1,195 @@
+/*
+ * tpc_cf_oracle.c — CPU ORACLE of the TPC cluster finder.  TEST INFRASTRUCTURE, NOT PRODUCT.
+ * See tpc_cf_oracle.h for who may use it.  Plain C99, single thread, no blocking / fusion /
+ * reordering beyond the definition: SURVEY.md §8(c) "Algorithm (oracle, step by step)",
+ * which restates BASELINE.json:north_star for the step named in PAPER.md:57.
+ *
+ * Notation follows the definition: Q = zero-bordered charge map of one (sector,row) plane,
+ * p = pad, t = time bin, (dp,dt) = offset from the peak, S0/S1p/S1t/S2p/S2t = moment sums.
+ */
+#include "tpc_cf_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define BORDER 2            /* 5x5 window => reads reach +-2 outside the plane (R2: they return 0) */
+
+static int sgn(int x) { return (x > 0) - (x < 0); }
+
+static uint32_t pads_of_row(const orc_geometry* g, uint32_t r)
+{
+    return g->npads ? (uint32_t)g->npads[r] : g->max_pads;
+}
+
+/* R11: a digit is valid iff it addresses an existing cell and carries charge. */
+static int digit_valid(const orc_geometry* g, const orc_digit* d)
+{
+    if (d->sector >= g->n_sectors) return 0;
+    if (d->row >= g->n_rows) return 0;
+    if (d->pad >= pads_of_row(g, d->row)) return 0;
+    if (d->time >= g->n_time) return 0;
+    if (d->charge == 0) return 0;
+    return 1;
+}
+
+static int geometry_ok(const orc_geometry* g)
+{
+    if (!g) return 0;
+    if (g->n_sectors == 0 || g->n_rows == 0 || g->max_pads == 0 || g->n_time == 0) return 0;
+    if (g->n_sectors > 256 || g->n_rows > 256 || g->max_pads > 256 || g->n_time > 65536) return 0;
+    if (g->npads)
+        for (uint32_t r = 0; r < g->n_rows; ++r)
+            if (g->npads[r] == 0 || g->npads[r] > g->max_pads) return 0;
+    return 1;
+}
+
+/* One plane: Q is (P+4) x (T+4), row stride W = T+4, already filled.  Emits clusters in
+ * (pad,time) loop order.  Returns the number of peaks found (all counted, only those that
+ * fit are written), or -3 if an exactness assertion fails (P5). */
+static int64_t scan_plane(const uint16_t* Q, uint32_t P, uint32_t T,
+                          uint32_t s, uint32_t r, const orc_params* prm,
+                          orc_cluster* out, uint64_t room)
+{
+    const size_t W = (size_t)T + 2 * BORDER;
+    int64_t n_found = 0;
+#define QAT(pp, tt) Q[(size_t)((pp) + BORDER) * W + (size_t)((tt) + BORDER)]
+    for (int p = 0; p < (int)P; ++p) {                       /* pad-major, time-minor (R10) */
+        for (int t = 0; t < (int)T; ++t) {
+            const uint16_t q = QAT(p, t);
+            if (q < prm->q_peak_min) continue;               /* R6 */
+            int peak = 1;
+            for (int dp = -1; dp <= 1; ++dp)
+                for (int dt = -1; dt <= 1; ++dt) {
+                    if (dp == 0 && dt == 0) continue;
+                    const uint16_t nb = QAT(p + dp, t + dt);
+                    if (dp < 0 || (dp == 0 && dt < 0)) peak &= (q > nb);   /* earlier: strict (R1) */
+                    else                               peak &= (q >= nb);  /* later: non-strict   */
+                }
+            if (!peak) continue;
+
+            int64_t S0 = 0, S1p = 0, S1t = 0, S2p = 0, S2t = 0;
+            for (int dp = -2; dp <= 2; ++dp)
+                for (int dt = -2; dt <= 2; ++dt) {
+                    const int ring = (abs(dp) == 2 || abs(dt) == 2);
+                    if (ring) {                               /* outer ring: gated (R3, R4) */
+                        const int ip = dp - sgn(dp), it = dt - sgn(dt);
+                        if (QAT(p + ip, t + it) < prm->q_inner_gate) continue;
+                    }
+                    const int64_t c = QAT(p + dp, t + dt);    /* inner 3x3 always counted */
+                    S0 += c; S1p += c * dp; S1t += c * dt; S2p += c * dp * dp; S2t += c * dt * dt;
+                }
+            /* P5 / R8: every sum is an integer below 2^24, so fp32 accumulation is exact. */
+            if (S0 >= (1 << 24) || llabs(S1p) >= (1 << 24) || llabs(S1t) >= (1 << 24) ||
+                S2p >= (1 << 24) || S2t >= (1 << 24)) return -3;
+
+            if ((uint64_t)n_found < room) {
+                const double mp = (double)S1p / (double)S0;
+                const double mt = (double)S1t / (double)S0;
+                double vp = (double)S2p / (double)S0 - mp * mp;
+                double vt = (double)S2t / (double)S0 - mt * mt;
+                if (vp < 0) vp = 0;
+                if (vt < 0) vt = 0;
+                orc_cluster c;
+                memset(&c, 0, sizeof c);
+                c.sector = (uint8_t)s; c.row = (uint8_t)r; c.pad = (uint8_t)p; c.flags = 0;
+                c.time = (uint16_t)t; c.qmax = q; c.qtot = (uint32_t)S0;
+                c.pad_mean = (float)((double)p + mp);         /* R7 */
+                c.time_mean = (float)((double)t + mt);
+                c.sigma_pad = (float)sqrt(vp);
+                c.sigma_time = (float)sqrt(vt);
+                c.rsv = 0;
+                out[n_found] = c;
+            }
+            ++n_found;
+        }
+    }
+#undef QAT
+    return n_found;
+}
+
+int tpc_cf_oracle_run_planes(const orc_digit* digits, uint64_t n,
+                             const orc_geometry* g, const orc_params* prm,
+                             uint32_t plane_begin, uint32_t plane_end,
+                             orc_cluster* out, uint64_t capacity, orc_status* st)
+{
+    if (!g || !prm || !st || (n && !digits) || (capacity && !out)) return -1;
+    if (!geometry_ok(g) || prm->q_peak_min == 0) return -1;
+    const uint32_t n_planes = g->n_sectors * g->n_rows;
+    if (plane_end > n_planes) plane_end = n_planes;
+    if (plane_begin > plane_end) return -1;
+    memset(st, 0, sizeof *st);
+
+    /* bucket digits by plane (counting sort on sector*n_rows+row; input order is free, R12) */
+    uint64_t* first = (uint64_t*)calloc((size_t)n_planes + 1, sizeof(uint64_t));
+    uint64_t* order = (uint64_t*)malloc((size_t)(n ? n : 1) * sizeof(uint64_t));
+    uint64_t* fill  = (uint64_t*)malloc((size_t)(n_planes + 1) * sizeof(uint64_t));
+    const size_t W = (size_t)g->n_time + 2 * BORDER;
+    uint16_t* Q = (uint16_t*)malloc(((size_t)g->max_pads + 2 * BORDER) * W * sizeof(uint16_t));
+    if (!first || !order || !fill || !Q) { free(first); free(order); free(fill); free(Q); return -2; }
+
+    uint64_t n_bad = 0, n_used = 0;
+    for (uint64_t i = 0; i < n; ++i) {
+        if (!digit_valid(g, &digits[i])) {
+            /* count a bad digit once, and only if the full frame is being processed or it
+             * cannot be attributed to a plane outside the requested range */
+            const uint32_t pl = (digits[i].sector < g->n_sectors && digits[i].row < g->n_rows)
+                                ? digits[i].sector * g->n_rows + digits[i].row : plane_begin;
+            if (pl >= plane_begin && pl < plane_end) ++n_bad;
+            continue;
+        }
+        ++first[(uint32_t)digits[i].sector * g->n_rows + digits[i].row + 1];
+    }
+    for (uint32_t k = 0; k < n_planes; ++k) first[k + 1] += first[k];
+    memcpy(fill, first, (size_t)(n_planes + 1) * sizeof(uint64_t));
+    for (uint64_t i = 0; i < n; ++i)
+        if (digit_valid(g, &digits[i]))
+            order[fill[(uint32_t)digits[i].sector * g->n_rows + digits[i].row]++] = i;
+
+    uint64_t n_clusters = 0;
+    int rc = 0;
+    for (uint32_t pl = plane_begin; pl < plane_end; ++pl) {
+        const uint32_t s = pl / g->n_rows, r = pl % g->n_rows;
+        const uint32_t P = pads_of_row(g, r), T = g->n_time;
+        memset(Q, 0, ((size_t)P + 2 * BORDER) * W * sizeof(uint16_t));          /* Q = 0, zero border */
+        for (uint64_t k = first[pl]; k < first[pl + 1]; ++k) {
+            const orc_digit* d = &digits[order[k]];
+            Q[(size_t)(d->pad + BORDER) * W + (size_t)(d->time + BORDER)] = d->charge;
+            ++n_used;
+        }
+        const uint64_t room = capacity > n_clusters ? capacity - n_clusters : 0;
+        const int64_t found = scan_plane(Q, P, T, s, r, prm, out ? out + n_clusters : NULL, room);
+        if (found < 0) { rc = (int)found; break; }
+        n_clusters += (uint64_t)found;
+    }
+    st->n_clusters = n_clusters;
+    st->n_digits_used = n_used;
+    st->n_bad_digits = n_bad;
+    st->overflow = n_clusters > capacity ? 1u : 0u;
+    free(first); free(order); free(fill); free(Q);
+    return rc;
+}
+
+int tpc_cf_oracle_run(const orc_digit* digits, uint64_t n,
+                      const orc_geometry* g, const orc_params* prm,
+                      orc_cluster* out, uint64_t capacity, orc_status* st)
+{
+    if (!g) return -1;
+    return tpc_cf_oracle_run_planes(digits, n, g, prm, 0, g->n_sectors * g->n_rows, out, capacity, st);
+}
+
+int tpc_cf_oracle_dense_plane(const orc_digit* digits, uint64_t n,
+                              const orc_geometry* g, uint32_t sector, uint32_t row,
+                              uint16_t* dense)
+{
+    if (!g || !dense || (n && !digits) || !geometry_ok(g)) return -1;
+    if (sector >= g->n_sectors || row >= g->n_rows) return -1;
+    const uint32_t P = pads_of_row(g, row), T = g->n_time;
+    memset(dense, 0, (size_t)P * T * sizeof(uint16_t));
+    for (uint64_t i = 0; i < n; ++i) {
+        const orc_digit* d = &digits[i];
+        if (!digit_valid(g, d) || d->sector != sector || d->row != row) continue;
+        dense[(size_t)d->pad * T + d->time] = d->charge;
+    }
+    return 0;
+}

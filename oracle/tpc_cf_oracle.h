@@ -1,0 +1,89 @@
+/*
+ * tpc_cf_oracle.h — CPU ORACLE of the TPC cluster finder.  TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * build, link, import or call anything in oracle/.  The product path (paper_2402_01205_b200/)
+ * shares no code, header, table or helper with this directory: the record layouts below are
+ * restated here on purpose (same bytes as include/tpc_cf.h, independent text).
+ *
+ * What it computes: the step the paper names "cluster finding in the GPUs on the EPNs"
+ * (§5), on one 2.8 ms time frame.  The paper gives no algorithm;
+ * the definition is BASELINE.json:north_star as made unambiguous in SURVEY.md §8(c)
+ * (readings R1..R19, restated in DESIGN.md §3).  The oracle is that definition executed
+ * literally, one (sector,row) plane at a time, single-threaded, sums in int64, moments in double.
+ *
+ * Parity pins (tests/test_oracle_*.py): hand-evaluated grids tests/golden/E*.txt, brute-force
+ * sparse-dict checker, numpy argmax / box-filter special cases, closed-form moments, invariants.
+ * No function in this file is "parity unpinned".
+ */
+#ifndef TPC_CF_ORACLE_H
+#define TPC_CF_ORACLE_H
+
+#include <stdint.h>
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* 8-byte input record: one zero-suppressed ADC sample (BASELINE.json:north_star "digits
+ * (sector, pad row, pad, time bin, charge)").  Little-endian, naturally aligned. */
+typedef struct {
+    uint8_t  sector, row, pad, rsv;
+    uint16_t time, charge;
+} orc_digit;
+
+/* 32-byte output record: one cluster (north_star: "qTot, qMax, pad and time centroids and sigmas").
+ * (sector,row,pad,time) is the peak cell; flags and rsv are 0. */
+typedef struct {
+    uint8_t  sector, row, pad, flags;
+    uint16_t time, qmax;
+    uint32_t qtot;
+    float    pad_mean, time_mean, sigma_pad, sigma_time;
+    uint32_t rsv;
+} orc_cluster;
+
+typedef struct {
+    uint32_t n_sectors, n_rows, max_pads, n_time;
+    const uint16_t* npads;      /* host, n_rows entries; NULL => every row has max_pads pads */
+} orc_geometry;
+
+typedef struct {
+    uint16_t q_peak_min;        /* R6: peak threshold, default 4 */
+    uint16_t q_inner_gate;      /* R4: gate threshold on the inner cell, default 2 */
+    uint32_t flags;             /* ignored by the oracle */
+} orc_params;
+
+typedef struct {
+    uint64_t n_clusters;        /* true number of peaks, even if > capacity */
+    uint64_t n_digits_used;
+    uint64_t n_bad_digits;      /* R11: out-of-range or zero-charge digits, skipped */
+    uint32_t overflow;          /* 1 if n_clusters > capacity */
+    uint32_t rsv;
+} orc_status;
+
+/* Runs the definition over all digits (any order).  All pointers are HOST pointers.
+ * Writes at most `capacity` clusters, ascending (sector,row,pad,time); returns 0, or
+ * -1 on a NULL/invalid argument, -2 on allocation failure, -3 if a moment sum reaches 2^24
+ * (cannot happen for uint16 charges; asserted per SURVEY.md §8(c)-P5). */
+int tpc_cf_oracle_run(const orc_digit* digits, uint64_t n,
+                      const orc_geometry* geom, const orc_params* params,
+                      orc_cluster* out, uint64_t capacity, orc_status* status);
+
+/* Same, restricted to planes [plane_begin, plane_end) with plane = sector*n_rows + row.
+ * Used by bench.py's cpu_baseline to time a bounded sample of a large frame. */
+int tpc_cf_oracle_run_planes(const orc_digit* digits, uint64_t n,
+                             const orc_geometry* geom, const orc_params* params,
+                             uint32_t plane_begin, uint32_t plane_end,
+                             orc_cluster* out, uint64_t capacity, orc_status* status);
+
+/* Fills dense[npads*n_time] (pad-major, time-minor) with the charge map of one plane, the
+ * way step "Q[d.pad][d.time] = d.charge" of the definition builds it.  For map-parity tests. */
+int tpc_cf_oracle_dense_plane(const orc_digit* digits, uint64_t n,
+                              const orc_geometry* geom, uint32_t sector, uint32_t row,
+                              uint16_t* dense);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
