@@ -1,0 +1,145 @@
+/*
+ * tpc_cf.h — C ABI of the B200-native TPC cluster finder (product boundary).
+ *
+ * Operation: the step the paper names "cluster finding in the GPUs on the EPNs" (§5), run on one
+ * 2.8 ms time frame: zero-suppressed ADC digits (sector, pad row, pad, time bin, charge) ->
+ * clusters (qTot, qMax, pad/time centroids and sigmas).  The paper gives no algorithm; the definition is
+ * BASELINE.json:north_star, made unambiguous by the readings R1..R19 of SURVEY.md §8(c) (restated in DESIGN.md §3):
+ *   peak      : q >= q_peak_min (4) and 3x3 (pad x time) local maximum, strict '>' against the 4 neighbours that
+ *               are lexicographically earlier in (pad,time), '>=' against the 4 later ones               (R1, R6)
+ *   qTot      : inner 3x3 always + each outer 5x5-ring cell (dp,dt) whose gate cell (dp-sgn dp, dt-sgn dt)
+ *               holds >= q_inner_gate (2) ADC                                                            (R3, R4)
+ *   moments   : charge-weighted mean / population sigma over exactly those cells, offsets taken relative to
+ *               the peak (so the fp32 sums are exact integers < 2^24), zero border outside the plane   (R2, R7, R8)
+ *   order     : one cluster per peak, ascending (sector,row,pad,time) of the peak cell                   (R10)
+ *
+ * All structs are POD, little-endian, naturally aligned.  No C++ or torch type crosses this boundary.
+ * Pointers are marked HOST or DEVICE.  The library never allocates device memory: the caller (PyTorch in the
+ * Python binding) owns digits, clusters, status and workspace.
+ */
+#ifndef TPC_CF_H
+#define TPC_CF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* 8-byte input record (north_star: "digits (sector, pad row, pad, time bin, charge)"). */
+typedef struct {
+    uint8_t  sector, row, pad, rsv;   /* rsv is ignored */
+    uint16_t time, charge;
+} tpc_digit;
+
+/* 32-byte output record (north_star: "clusters (qTot, qMax, pad and time centroids and sigmas)").
+ * (sector,row,pad,time) is the peak cell; flags and rsv are written as 0. */
+typedef struct {
+    uint8_t  sector, row, pad, flags;
+    uint16_t time, qmax;
+    uint32_t qtot;
+    float    pad_mean, time_mean, sigma_pad, sigma_time;
+    uint32_t rsv;
+} tpc_cluster;
+
+/* Detector geometry.  Limits (8/16-bit record fields): n_sectors <= 256, n_rows <= 256, max_pads <= 255,
+ * n_time <= 65535.  npads: HOST pointer to n_rows entries (1..max_pads), or NULL => every row has max_pads
+ * pads (R15, R19).  It is copied at create; it need not outlive the call. */
+typedef struct {
+    uint32_t n_sectors, n_rows, max_pads, n_time;
+    const uint16_t* npads;
+} tpc_cf_geometry;
+
+enum {
+    TPC_CF_DIGITS_SORTED = 1u,  /* hint: digits ascend in (sector,row,pad,time).  Selects the fused shared-memory
+                                   path ("T3").  The hint is verified on the device for free; if it is false (or a
+                                   capacity of the fused path is exceeded) the general path runs instead and
+                                   status.path says so.  The result never depends on the hint. */
+    TPC_CF_FORCE_GENERAL = 2u   /* always run the general (map in HBM, "T1") path, whatever the order */
+};
+
+typedef struct {
+    uint16_t q_peak_min;    /* R6, default 4; 0 is rejected */
+    uint16_t q_inner_gate;  /* R4, default 2 */
+    uint32_t flags;         /* TPC_CF_* bits */
+} tpc_cf_params;
+
+/* Written last on the stream, by the device. */
+typedef struct {
+    uint64_t n_clusters;     /* true number of peaks, even if > capacity */
+    uint64_t n_digits_used;  /* valid digits */
+    uint64_t n_bad_digits;   /* R11: out-of-range or zero-charge digits: skipped and counted */
+    uint32_t overflow;       /* 1 if n_clusters > capacity: the first `capacity` clusters in output order are written */
+    uint32_t path;           /* 1 = general path (T1) produced the output, 3 = fused sorted path (T3) */
+} tpc_cf_status;
+
+typedef struct {
+    tpc_cluster*   clusters;  /* DEVICE, caller-owned, `capacity` entries, 32-byte aligned */
+    uint64_t       capacity;
+    tpc_cf_status* status;    /* DEVICE, caller-owned, 8-byte aligned; valid after the stream is synchronised */
+    void*          stream;    /* cudaStream_t (0 = legacy default stream) */
+} tpc_cf_out;
+
+typedef struct tpc_cf tpc_cf;   /* opaque handle: host state only */
+
+enum {
+    TPC_CF_OK = 0,
+    TPC_CF_E_NULL = -1,       /* a required pointer is NULL */
+    TPC_CF_E_GEOMETRY = -2,   /* zero or out-of-limit dimension, bad npads entry, or differs from create */
+    TPC_CF_E_CAPACITY = -3,   /* n > max_digits */
+    TPC_CF_E_WORKSPACE = -4,  /* workspace too small or not 256-byte aligned */
+    TPC_CF_E_PARAMS = -5,     /* q_peak_min == 0 or unknown flag bits */
+    TPC_CF_E_CUDA = -6,       /* a CUDA call failed; text via tpc_cf_strerror */
+    TPC_CF_E_NOMEM = -7       /* host allocation failed */
+};
+
+/* Bytes of DEVICE workspace `create` needs for this geometry and these capacities (0 on invalid geometry).
+ * Layout: dense uint16 charge map with a 2-cell zero border per plane, line index, unit tables,
+ * cluster staging (32 B per max_clusters), sort scratch for the general path. */
+size_t tpc_cf_workspace_bytes(const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters);
+
+/* Creates a handle bound to a caller-owned DEVICE workspace (256-byte aligned, >= tpc_cf_workspace_bytes).
+ * Enqueues on `stream` the one-time zeroing of the charge map; every run leaves the map zero again (K0 is an
+ * "un-scatter").  Returns TPC_CF_OK or a negative error; *h is set only on success. */
+int tpc_cf_create(tpc_cf** h, const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters,
+                  void* workspace, size_t workspace_bytes, void* stream);
+
+/* Enqueues the whole hot path for `n` digits on out->stream and returns without
+ * synchronising.  digits: DEVICE pointer, 8-byte aligned, any order, at most one digit per cell (R11), must
+ * stay alive until the stream has passed the run.  geom must equal the geometry given to create.
+ * Synchronous errors (nothing enqueued): negative return.  Asynchronous conditions are in out->status.
+ * One handle serves one stream at a time. */
+int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n,
+               const tpc_cf_geometry* geom, const tpc_cf_params* params, tpc_cf_out* out);
+
+/* End-to-end convenience used by bench.py's `e2e` leg: HOST digits in (pinned or pageable), HOST clusters and
+ * status out; copies host->device, runs, copies the status and the clusters back, synchronises the stream.
+ * dev_digits / dev_clusters / dev_status are caller-owned DEVICE staging buffers (max_digits / capacity / 1). */
+int tpc_cf_run_host(tpc_cf* h, const tpc_digit* host_digits, uint64_t n,
+                    const tpc_cf_geometry* geom, const tpc_cf_params* params,
+                    tpc_digit* dev_digits, tpc_cluster* dev_clusters, tpc_cf_status* dev_status,
+                    tpc_cluster* host_clusters, uint64_t capacity, tpc_cf_status* host_status, void* stream);
+
+/* Test hook for the K1 map-parity check: scatters the digits, copies the dense plane
+ * (sector,row) into `dense` (DEVICE, npads(row) x n_time uint16, pad-major), and un-scatters again. */
+int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint64_t n,
+                             uint32_t sector, uint32_t row, uint16_t* dense, void* stream);
+
+/* Number of kernel launches the last run enqueued (for bench.py's gpu_launches). */
+int tpc_cf_last_launch_count(const tpc_cf* h);
+
+/* Device time in ms of kernel class `which` during the last run, measured by CUDA events recorded on the run's
+ * stream when profiling was enabled with tpc_cf_set_profiling(h, 1).  which: 0 = whole run, 1 = fused T3 kernel
+ * (or T1 peak kernel when the general path ran).  Synchronises on the events.  Negative on error. */
+int   tpc_cf_set_profiling(tpc_cf* h, int on);
+float tpc_cf_last_kernel_ms(tpc_cf* h, int which);
+
+int tpc_cf_destroy(tpc_cf* h);
+
+const char* tpc_cf_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPC_CF_H */

@@ -1,0 +1,272 @@
+// tpc_cf_api.cu — the C ABI of include/tpc_cf.h: argument validation, workspace carving, kernel sequencing.
+// The library never allocates device memory; the handle owns host state and a few CUDA events only.
+#include <new>
+#include <stdio.h>
+#include <string.h>
+
+#include "tpc_cf_internal.cuh"
+
+using namespace tpccf;
+
+struct tpc_cf {
+    Geo geo;
+    Workspace ws;
+    uint64_t max_digits, max_clusters;
+    uint32_t n_sort_tiles;
+    size_t map_bytes;
+    int last_launches;
+    int profiling;
+    cudaEvent_t ev[4];          // run begin, dominant kernel begin, dominant kernel end, run end
+    char cuda_msg[256];
+};
+
+static thread_local char g_last_cuda_msg[256] = "";
+
+static bool geometry_to_geo(const tpc_cf_geometry* g, Geo* out)
+{
+    if (g->n_sectors == 0 || g->n_rows == 0 || g->max_pads == 0 || g->n_time == 0) return false;
+    if (g->n_sectors > 256 || g->n_rows > 256 || g->max_pads > 255 || g->n_time > 65535) return false;
+    memset(out, 0, sizeof *out);
+    out->n_sectors = g->n_sectors; out->n_rows = g->n_rows; out->max_pads = g->max_pads; out->n_time = g->n_time;
+    out->n_planes = g->n_sectors * g->n_rows;
+    out->PS = g->max_pads + 4;
+    out->TS = (g->n_time + 4 + 7) & ~7u;
+    out->LS = g->max_pads + 1;
+    for (uint32_t r = 0; r < g->n_rows; ++r) {
+        const uint32_t p = g->npads ? g->npads[r] : g->max_pads;
+        if (p == 0 || p > g->max_pads) return false;
+        out->npads[r] = (uint8_t)p;
+    }
+    return true;
+}
+
+static bool same_geometry(const Geo& a, const Geo& b)
+{
+    return a.n_sectors == b.n_sectors && a.n_rows == b.n_rows && a.max_pads == b.max_pads &&
+           a.n_time == b.n_time && memcmp(a.npads, b.npads, sizeof a.npads) == 0;
+}
+
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// Carves the workspace; base may be NULL to compute the size only.
+static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, char* base, Workspace* ws,
+                    uint32_t* n_sort_tiles, size_t* map_bytes)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) { char* p = base ? base + off : nullptr; off += align256(bytes ? bytes : 1); return p; };
+    const uint64_t nwords = ceil_div_u64(max_digits, 32) + 1;
+    const uint64_t nblk = ceil_div_u64(nwords, 256) + 1;
+    const uint64_t tiles = ceil_div_u64(max_clusters ? max_clusters : 1, 2048);
+    const size_t mapb = (size_t)g.n_planes * g.PS * g.TS * sizeof(uint16_t);
+    Workspace w;
+    w.counters = (Counters*)take(sizeof(Counters));
+    w.map = (uint16_t*)take(mapb);
+    w.peakmask = (uint32_t*)take(nwords * 4);
+    w.blk_cnt = (uint32_t*)take(nblk * 4);
+    w.blk_off = (uint32_t*)take(nblk * 4);
+    w.scan_part = (uint32_t*)take((ceil_div_u64(nblk, 1024) + 1) * 4);
+    w.stage = (tpc_cluster*)take((size_t)max_digits * sizeof(tpc_cluster));
+    w.compact = (tpc_cluster*)take((size_t)max_clusters * sizeof(tpc_cluster));
+    w.keyA = (uint64_t*)take((size_t)max_clusters * 8);
+    w.keyB = (uint64_t*)take((size_t)max_clusters * 8);
+    w.idxA = (uint32_t*)take((size_t)max_clusters * 4);
+    w.idxB = (uint32_t*)take((size_t)max_clusters * 4);
+    w.ghist = (uint32_t*)take((size_t)tiles * 256 * 4);
+    w.ghist_part = (uint32_t*)take((ceil_div_u64(tiles * 256, 1024) + 1) * 4);
+    w.line_start = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
+    if (ws) *ws = w;
+    if (n_sort_tiles) *n_sort_tiles = (uint32_t)tiles;
+    if (map_bytes) *map_bytes = mapb;
+    return off;
+}
+
+static int cuda_fail(tpc_cf* h, cudaError_t e, const char* where)
+{
+    snprintf(g_last_cuda_msg, sizeof g_last_cuda_msg, "%s: %s", where, cudaGetErrorString(e));
+    if (h) memcpy(h->cuda_msg, g_last_cuda_msg, sizeof h->cuda_msg);
+    return TPC_CF_E_CUDA;
+}
+
+extern "C" size_t tpc_cf_workspace_bytes(const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters)
+{
+    Geo g;
+    if (!geom || !geometry_to_geo(geom, &g)) return 0;
+    if (max_digits >= (1ull << 32) || max_clusters >= (1ull << 32)) return 0;
+    return carve(g, max_digits, max_clusters, nullptr, nullptr, nullptr, nullptr);
+}
+
+extern "C" int tpc_cf_create(tpc_cf** hp, const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters,
+                             void* workspace, size_t workspace_bytes, void* stream)
+{
+    if (!hp || !geom || !workspace) return TPC_CF_E_NULL;
+    Geo g;
+    if (!geometry_to_geo(geom, &g)) return TPC_CF_E_GEOMETRY;
+    if (max_digits >= (1ull << 32) || max_clusters >= (1ull << 32)) return TPC_CF_E_CAPACITY;
+    if (((uintptr_t)workspace & 255u) != 0) return TPC_CF_E_WORKSPACE;
+    if (carve(g, max_digits, max_clusters, nullptr, nullptr, nullptr, nullptr) > workspace_bytes)
+        return TPC_CF_E_WORKSPACE;
+    tpc_cf* h = new (std::nothrow) tpc_cf;
+    if (!h) return TPC_CF_E_NOMEM;
+    memset(h, 0, sizeof *h);
+    h->geo = g;
+    h->max_digits = max_digits;
+    h->max_clusters = max_clusters;
+    carve(g, max_digits, max_clusters, (char*)workspace, &h->ws, &h->n_sort_tiles, &h->map_bytes);
+    for (int i = 0; i < 4; ++i) {
+        cudaError_t e = cudaEventCreate(&h->ev[i]);
+        if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaEventCreate"); }
+    }
+    // K0, once: the charge map starts zero; every run restores it (un-scatter).
+    cudaError_t e = cudaMemsetAsync(h->ws.map, 0, h->map_bytes, (cudaStream_t)stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), (cudaStream_t)stream);
+    if (e != cudaSuccess) { for (int i = 0; i < 4; ++i) cudaEventDestroy(h->ev[i]); delete h; return cuda_fail(nullptr, e, "cudaMemsetAsync(map)"); }
+    *hp = h;
+    return TPC_CF_OK;
+}
+
+static int check_run_args(tpc_cf* h, const tpc_digit* digits, uint64_t n, const tpc_cf_geometry* geom,
+                          const tpc_cf_params* params)
+{
+    if (!h || !geom || !params || (n && !digits)) return TPC_CF_E_NULL;
+    Geo g;
+    if (!geometry_to_geo(geom, &g) || !same_geometry(g, h->geo)) return TPC_CF_E_GEOMETRY;
+    if (n > h->max_digits) return TPC_CF_E_CAPACITY;
+    if (params->q_peak_min == 0) return TPC_CF_E_PARAMS;
+    if (params->flags & ~(uint32_t)(TPC_CF_DIGITS_SORTED | TPC_CF_FORCE_GENERAL)) return TPC_CF_E_PARAMS;
+    if (((uintptr_t)digits & 7u) != 0) return TPC_CF_E_NULL;
+    return TPC_CF_OK;
+}
+
+extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const tpc_cf_geometry* geom,
+                          const tpc_cf_params* params, tpc_cf_out* out)
+{
+    int rc = check_run_args(h, digits, n, geom, params);
+    if (rc != TPC_CF_OK) return rc;
+    if (!out || !out->status || (out->capacity && !out->clusters)) return TPC_CF_E_NULL;
+    if (((uintptr_t)out->clusters & 15u) != 0 || ((uintptr_t)out->status & 7u) != 0) return TPC_CF_E_NULL;
+    cudaStream_t st = (cudaStream_t)out->stream;
+    const bool hint = (params->flags & TPC_CF_DIGITS_SORTED) != 0;
+    const bool fused = hint && !(params->flags & TPC_CF_FORCE_GENERAL);
+    const bool prof = h->profiling != 0;
+    int k = 0;
+
+    (void)cudaGetLastError();
+    if (prof) cudaEventRecord(h->ev[0], st);
+    cudaError_t e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), st);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(counters)");
+
+    if (fused) {
+        // T3: line index -> fused smem kernel (scatter into smem lines, peak test, moments) -> compaction
+        int r = launch_fused_sorted(h->geo, h->ws, digits, n, params->q_peak_min, params->q_inner_gate, st,
+                                    prof ? h->ev[1] : nullptr, prof ? h->ev[2] : nullptr);
+        if (r < 0) return r;
+        k += r;
+        k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, 0, st);
+        k += launch_finalize(h->ws, out->status, out->capacity, 3u, 1, st);
+    } else {
+        // T1: K1 scatter -> K2+K4 digit-centric peaks + moments on the HBM map -> K3 compaction -> (K5 key sort)
+        //     -> K0 un-scatter
+        k += launch_general_peaks(h->geo, h->ws, digits, n, params->q_peak_min, params->q_inner_gate, st,
+                                  prof ? h->ev[1] : nullptr, prof ? h->ev[2] : nullptr);
+        k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, hint ? 0 : 1, st);
+        if (!hint) k += launch_key_sort(h->ws, h->max_clusters, h->n_sort_tiles, out->clusters, out->capacity, st);
+        k += launch_unscatter(h->geo, h->ws, digits, n, st);
+        k += launch_finalize(h->ws, out->status, out->capacity, 1u, hint ? 1 : 0, st);
+    }
+    if (prof) cudaEventRecord(h->ev[3], st);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(h, e, "kernel launch");
+    h->last_launches = k;
+    return TPC_CF_OK;
+}
+
+extern "C" int tpc_cf_run_host(tpc_cf* h, const tpc_digit* host_digits, uint64_t n, const tpc_cf_geometry* geom,
+                               const tpc_cf_params* params, tpc_digit* dev_digits, tpc_cluster* dev_clusters,
+                               tpc_cf_status* dev_status, tpc_cluster* host_clusters, uint64_t capacity,
+                               tpc_cf_status* host_status, void* stream)
+{
+    if (!h || !params || !host_status || !dev_status || (n && (!host_digits || !dev_digits))) return TPC_CF_E_NULL;
+    if (capacity && (!dev_clusters || !host_clusters)) return TPC_CF_E_NULL;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaSuccess;
+    if (n) e = cudaMemcpyAsync(dev_digits, host_digits, n * sizeof(tpc_digit), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemcpyAsync(H2D digits)");
+    tpc_cf_params prm = *params;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        tpc_cf_out out = { dev_clusters, capacity, dev_status, stream };
+        int rc = tpc_cf_run(h, dev_digits, n, geom, &prm, &out);
+        if (rc != TPC_CF_OK) return rc;
+        e = cudaMemcpyAsync(host_status, dev_status, sizeof(tpc_cf_status), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(h, e, "status readback");
+        if (host_status->path != 0) break;
+        prm.flags &= ~(uint32_t)TPC_CF_DIGITS_SORTED;   // the promise was false: rerun on the general path
+    }
+    uint64_t m = host_status->n_clusters < capacity ? host_status->n_clusters : capacity;
+    if (m) {
+        e = cudaMemcpyAsync(host_clusters, dev_clusters, m * sizeof(tpc_cluster), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(h, e, "cluster readback");
+    }
+    return TPC_CF_OK;
+}
+
+extern "C" int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint64_t n, uint32_t sector,
+                                        uint32_t row, uint16_t* dense, void* stream)
+{
+    if (!h || !dense || (n && !digits)) return TPC_CF_E_NULL;
+    if (n > h->max_digits) return TPC_CF_E_CAPACITY;
+    if (sector >= h->geo.n_sectors || row >= h->geo.n_rows) return TPC_CF_E_GEOMETRY;
+    cudaStream_t st = (cudaStream_t)stream;
+    (void)cudaGetLastError();
+    cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), st);
+    launch_scatter_only(h->geo, h->ws, digits, n, st);
+    launch_copy_plane(h->geo, h->ws, sector * h->geo.n_rows + row, h->geo.npads[row], dense, st);
+    launch_unscatter(h->geo, h->ws, digits, n, st);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(h, e, "debug_dense_plane");
+    return TPC_CF_OK;
+}
+
+extern "C" int tpc_cf_last_launch_count(const tpc_cf* h) { return h ? h->last_launches : TPC_CF_E_NULL; }
+
+extern "C" int tpc_cf_set_profiling(tpc_cf* h, int on)
+{
+    if (!h) return TPC_CF_E_NULL;
+    h->profiling = on ? 1 : 0;
+    return TPC_CF_OK;
+}
+
+extern "C" float tpc_cf_last_kernel_ms(tpc_cf* h, int which)
+{
+    if (!h || !h->profiling) return -1.f;
+    float ms = -1.f;
+    cudaError_t e;
+    if (which == 0) { e = cudaEventSynchronize(h->ev[3]); if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, h->ev[0], h->ev[3]); }
+    else            { e = cudaEventSynchronize(h->ev[2]); if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, h->ev[1], h->ev[2]); }
+    if (e != cudaSuccess) { cuda_fail(h, e, "event timing"); return -1.f; }
+    return ms;
+}
+
+extern "C" int tpc_cf_destroy(tpc_cf* h)
+{
+    if (!h) return TPC_CF_E_NULL;
+    for (int i = 0; i < 4; ++i) cudaEventDestroy(h->ev[i]);
+    delete h;
+    return TPC_CF_OK;
+}
+
+extern "C" const char* tpc_cf_strerror(int code)
+{
+    switch (code) {
+    case TPC_CF_OK: return "ok";
+    case TPC_CF_E_NULL: return "required pointer is NULL or misaligned";
+    case TPC_CF_E_GEOMETRY: return "invalid geometry, or geometry differs from create";
+    case TPC_CF_E_CAPACITY: return "n exceeds max_digits, or a capacity is >= 2^32";
+    case TPC_CF_E_WORKSPACE: return "workspace too small or not 256-byte aligned";
+    case TPC_CF_E_PARAMS: return "invalid params (q_peak_min == 0 or unknown flag bits)";
+    case TPC_CF_E_CUDA: return g_last_cuda_msg[0] ? g_last_cuda_msg : "CUDA error";
+    case TPC_CF_E_NOMEM: return "host allocation failed";
+    default: return "unknown error";
+    }
+}

@@ -1,0 +1,289 @@
+// tpc_cf_compact.cu — K3 compaction and K5 ordered output, shared by the general and the fused path.
+//   Both paths leave the peak set as one bit per digit (peakmask) and the cluster of peak digit j at stage[j].
+//   k_count_peaks / scan / k_gather : order-preserving compaction (popc + prefix sums) into the output array.
+//     Sorted digits => digit order is (sector,row,pad,time) order => the output is final (R10).
+//   Unsorted digits (general path only): the compacted clusters go to ws.compact and an LSD radix sort on the
+//     40-bit (sector,row,pad,time) key orders them (keys are unique, so exactly one array is correct, R10).
+//   k_finalize writes the status block last.
+#include "tpc_cf_internal.cuh"
+
+namespace tpccf {
+
+// ---- block-wide exclusive scan (blockDim.x <= 1024, multiple of 32) ------------------------------------------
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total)
+{
+    __shared__ uint32_t s_warp[32];
+    const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= (unsigned)o) inc += u;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = lane < nwarp ? s_warp[lane] : 0u;
+        uint32_t winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= (unsigned)o) winc += u;
+        }
+        s_warp[lane] = winc - w;                 // exclusive warp offsets
+        if (lane == 31 && total) *total = winc;  // block total
+    }
+    __syncthreads();
+    const uint32_t r = s_warp[warp] + inc - v;
+    __syncthreads();                             // s_warp may be reused by the next call
+    return r;
+}
+
+// ---- generic exclusive scan over uint32 ----------------------------------------------------------------------
+static constexpr int kScanThreads = 1024;
+
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_reduce(const uint32_t* __restrict__ in, uint64_t n, uint32_t* __restrict__ partial)
+{
+    __shared__ uint32_t s_total;
+    const uint64_t i = (uint64_t)blockIdx.x * kScanThreads + threadIdx.x;
+    const uint32_t v = i < n ? in[i] : 0u;
+    block_exclusive_scan(v, &s_total);
+    __syncthreads();
+    if (threadIdx.x == 0) partial[blockIdx.x] = s_total;
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_partials(uint32_t* partial, uint64_t nb, unsigned long long* total)
+{
+    __shared__ uint32_t s_total;
+    unsigned long long carry = 0;
+    for (uint64_t base = 0; base < nb; base += kScanThreads) {
+        const uint64_t i = base + threadIdx.x;
+        const uint32_t v = i < nb ? partial[i] : 0u;
+        const uint32_t ex = block_exclusive_scan(v, &s_total);
+        __syncthreads();
+        if (i < nb) partial[i] = (uint32_t)(carry + ex);
+        carry += s_total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0 && total) *total = carry;
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_apply(const uint32_t* in, uint32_t* out, uint64_t n, const uint32_t* __restrict__ partial)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * kScanThreads + threadIdx.x;
+    const uint32_t v = i < n ? in[i] : 0u;
+    const uint32_t ex = block_exclusive_scan(v, nullptr);
+    if (i < n) out[i] = partial[blockIdx.x] + ex;
+}
+
+int launch_scan_u32(const uint32_t* in, uint32_t* out, uint64_t n, uint32_t* partials,
+                    unsigned long long* total, cudaStream_t st)
+{
+    if (n == 0) return 0;
+    const uint64_t nb = ceil_div_u64(n, kScanThreads);
+    k_scan_reduce<<<(unsigned)nb, kScanThreads, 0, st>>>(in, n, partials);
+    k_scan_partials<<<1, kScanThreads, 0, st>>>(partials, nb, total);
+    k_scan_apply<<<(unsigned)nb, kScanThreads, 0, st>>>(in, out, n, partials);
+    return 3;
+}
+
+// ---- K3: compaction -------------------------------------------------------------------------------------------
+static constexpr int kCompactThreads = 256;   // one peakmask word (32 digits) per thread
+
+__global__ void __launch_bounds__(kCompactThreads)
+k_count_peaks(const uint32_t* __restrict__ peakmask, uint64_t nwords, uint32_t* __restrict__ blk_cnt)
+{
+    __shared__ uint32_t s_total;
+    const uint64_t w = (uint64_t)blockIdx.x * kCompactThreads + threadIdx.x;
+    const uint32_t c = w < nwords ? (uint32_t)__popc(peakmask[w]) : 0u;
+    block_exclusive_scan(c, &s_total);
+    __syncthreads();
+    if (threadIdx.x == 0) blk_cnt[blockIdx.x] = s_total;
+}
+
+__global__ void __launch_bounds__(kCompactThreads)
+k_gather(const uint32_t* __restrict__ peakmask, uint64_t nwords, const uint32_t* __restrict__ blk_off,
+         const uint4* __restrict__ stage, uint4* out, uint64_t capacity, uint4* compact, uint64_t max_clusters,
+         int sort_if_unsorted, const Counters* cnt)
+{
+    const uint64_t w = (uint64_t)blockIdx.x * kCompactThreads + threadIdx.x;
+    uint32_t m = w < nwords ? peakmask[w] : 0u;
+    const uint32_t ex = block_exclusive_scan((uint32_t)__popc(m), nullptr);
+    uint4* dst = out;
+    uint64_t cap = capacity;
+    if (sort_if_unsorted && cnt->unsorted) { dst = compact; cap = max_clusters; }
+    uint64_t pos = (uint64_t)blk_off[blockIdx.x] + ex;
+    while (m) {
+        const int b = __ffs(m) - 1;
+        m &= m - 1;
+        const uint64_t j = w * 32 + b;
+        if (pos < cap) {
+            const uint4 lo = __ldcs(stage + 2 * j), hi = __ldcs(stage + 2 * j + 1);
+            __stcs(dst + 2 * pos, lo);
+            __stcs(dst + 2 * pos + 1, hi);
+        }
+        ++pos;
+    }
+}
+
+int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t capacity, uint64_t max_clusters,
+                   int sort_if_unsorted, cudaStream_t st)
+{
+    if (n == 0) return 0;
+    const uint64_t nwords = ceil_div_u64(n, 32);
+    const uint64_t nblk = ceil_div_u64(nwords, kCompactThreads);
+    k_count_peaks<<<(unsigned)nblk, kCompactThreads, 0, st>>>(ws.peakmask, nwords, ws.blk_cnt);
+    int k = 1 + launch_scan_u32(ws.blk_cnt, ws.blk_off, nblk, ws.scan_part, &ws.counters->n_clusters, st);
+    k_gather<<<(unsigned)nblk, kCompactThreads, 0, st>>>(ws.peakmask, nwords, ws.blk_off, (const uint4*)ws.stage,
+                                                         (uint4*)out, capacity, (uint4*)ws.compact, max_clusters,
+                                                         sort_if_unsorted, ws.counters);
+    return k + 1;
+}
+
+// ---- K5 for unsorted input: LSD radix sort of (key40, index), 8 bits per pass, warp-private tiles -------------
+static constexpr int kSortTile = 2048;     // elements per warp
+static constexpr int kSortWarps = 8;
+
+__device__ __forceinline__ uint64_t sort_count(const Counters* cnt, uint64_t max_clusters)
+{
+    const uint64_t c = cnt->n_clusters;
+    return c < max_clusters ? c : max_clusters;
+}
+
+__global__ void k_sort_init(const uint4* __restrict__ compact, const Counters* cnt, uint64_t max_clusters,
+                            uint64_t* __restrict__ key, uint32_t* __restrict__ idx)
+{
+    if (!cnt->unsorted) return;
+    const uint64_t N = sort_count(cnt, max_clusters);
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const uint4 lo = compact[2 * i];
+    key[i] = key40(lo.x, lo.y);
+    idx[i] = (uint32_t)i;
+}
+
+__global__ void __launch_bounds__(kSortWarps * 32)
+k_radix_hist(const uint64_t* __restrict__ key, const Counters* cnt, uint64_t max_clusters, int shift,
+             uint32_t* __restrict__ ghist, uint32_t n_tiles)
+{
+    if (!cnt->unsorted) return;
+    __shared__ uint32_t s_hist[kSortWarps][256];
+    const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t tile = blockIdx.x * kSortWarps + warp;
+    const uint64_t N = sort_count(cnt, max_clusters);
+    for (int d = lane; d < 256; d += 32) s_hist[warp][d] = 0;
+    __syncwarp();
+    if (tile < n_tiles) {
+        const uint64_t b = (uint64_t)tile * kSortTile;
+        for (int it = 0; it < kSortTile / 32; ++it) {
+            const uint64_t i = b + (uint64_t)it * 32 + lane;
+            if (i < N) atomicAdd(&s_hist[warp][(key[i] >> shift) & 0xffu], 1u);
+        }
+        __syncwarp();
+        for (int d = lane; d < 256; d += 32) ghist[(size_t)d * n_tiles + tile] = s_hist[warp][d];
+    }
+}
+
+__global__ void __launch_bounds__(kSortWarps * 32)
+k_radix_scatter(const uint64_t* __restrict__ key_in, const uint32_t* __restrict__ idx_in,
+                uint64_t* __restrict__ key_out, uint32_t* __restrict__ idx_out, const Counters* cnt,
+                uint64_t max_clusters, int shift, const uint32_t* __restrict__ goff, uint32_t n_tiles)
+{
+    if (!cnt->unsorted) return;
+    __shared__ uint32_t s_base[kSortWarps][256];
+    const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t tile = blockIdx.x * kSortWarps + warp;
+    if (tile >= n_tiles) return;
+    const uint64_t N = sort_count(cnt, max_clusters);
+    for (int d = lane; d < 256; d += 32) s_base[warp][d] = goff[(size_t)d * n_tiles + tile];
+    __syncwarp();
+    const uint64_t b = (uint64_t)tile * kSortTile;
+    for (int it = 0; it < kSortTile / 32; ++it) {
+        const uint64_t i = b + (uint64_t)it * 32 + lane;
+        const bool act = i < N;
+        const unsigned am = __ballot_sync(0xffffffffu, act);
+        if (am == 0) break;
+        if (act) {
+            const uint64_t k = key_in[i];
+            const uint32_t d = (uint32_t)(k >> shift) & 0xffu;
+            const unsigned peers = __match_any_sync(am, d);
+            const uint32_t rank = (uint32_t)__popc(peers & ((1u << lane) - 1u));
+            const uint32_t pos = s_base[warp][d] + rank;
+            key_out[pos] = k;
+            idx_out[pos] = idx_in[i];
+            __syncwarp(am);
+            if (rank == 0) s_base[warp][d] += (uint32_t)__popc(peers);
+        }
+        __syncwarp();
+    }
+}
+
+__global__ void k_sort_gather(const uint4* __restrict__ compact, const uint32_t* __restrict__ idx,
+                              const Counters* cnt, uint64_t max_clusters, uint4* __restrict__ out, uint64_t capacity)
+{
+    if (!cnt->unsorted) return;
+    uint64_t N = sort_count(cnt, max_clusters);
+    if (N > capacity) N = capacity;
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const uint32_t j = idx[i];
+    out[2 * i] = compact[2 * (uint64_t)j];
+    out[2 * i + 1] = compact[2 * (uint64_t)j + 1];
+}
+
+int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_tiles, tpc_cluster* out,
+                    uint64_t capacity, cudaStream_t st)
+{
+    if (max_clusters == 0) return 0;
+    int k = 0;
+    const unsigned g256 = (unsigned)ceil_div_u64(max_clusters, 256);
+    k_sort_init<<<g256, 256, 0, st>>>((const uint4*)ws.compact, ws.counters, max_clusters, ws.keyA, ws.idxA);
+    ++k;
+    uint64_t* kin = ws.keyA; uint64_t* kout = ws.keyB;
+    uint32_t* iin = ws.idxA; uint32_t* iout = ws.idxB;
+    const unsigned gt = (unsigned)ceil_div_u64(n_sort_tiles, kSortWarps);
+    for (int pass = 0; pass < 5; ++pass) {
+        const int shift = pass * 8;
+        k_radix_hist<<<gt, kSortWarps * 32, 0, st>>>(kin, ws.counters, max_clusters, shift, ws.ghist, n_sort_tiles);
+        k += 1 + launch_scan_u32(ws.ghist, ws.ghist, (uint64_t)256 * n_sort_tiles, ws.ghist_part, nullptr, st);
+        k_radix_scatter<<<gt, kSortWarps * 32, 0, st>>>(kin, iin, kout, iout, ws.counters, max_clusters, shift,
+                                                        ws.ghist, n_sort_tiles);
+        ++k;
+        uint64_t* tk = kin; kin = kout; kout = tk;
+        uint32_t* ti = iin; iin = iout; iout = ti;
+    }
+    k_sort_gather<<<g256, 256, 0, st>>>((const uint4*)ws.compact, iin, ws.counters, max_clusters, (uint4*)out,
+                                        capacity);
+    return k + 1;
+}
+
+// ---- status ---------------------------------------------------------------------------------------------------
+__global__ void k_finalize(const Counters* cnt, tpc_cf_status* status, uint64_t capacity, uint32_t path,
+                           int hint_sorted)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    tpc_cf_status s;
+    s.n_clusters = cnt->n_clusters;
+    s.n_digits_used = cnt->n_used;
+    s.n_bad_digits = cnt->n_bad;
+    s.overflow = s.n_clusters > capacity ? 1u : 0u;
+    s.path = path;
+    if (hint_sorted && cnt->unsorted) {   // false DIGITS_SORTED promise: detected, no output (include/tpc_cf.h)
+        s.n_clusters = 0;
+        s.overflow = 0;
+        s.path = 0;
+    }
+    *status = s;
+}
+
+int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,
+                    int hint_sorted, cudaStream_t st)
+{
+    k_finalize<<<1, 32, 0, st>>>(ws.counters, status, capacity, path, hint_sorted);
+    return 1;
+}
+
+}  // namespace tpccf

@@ -1,0 +1,143 @@
+// tpc_cf_internal.cuh — internal declarations of the B200 TPC cluster finder (product code, sm_100a).
+// Nothing here is shared with oracle/.  Definition implemented: include/tpc_cf.h (BASELINE.json:north_star,
+// readings R1..R19 of SURVEY.md §8(c) / DESIGN.md §3; step named in PAPER.md:57).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tpc_cf.h"
+
+namespace tpccf {
+
+// Geometry as the kernels see it (passed by value as a kernel parameter; 256 + 32 bytes).
+struct Geo {
+    uint32_t n_sectors, n_rows, max_pads, n_time;
+    uint32_t n_planes;   // n_sectors * n_rows
+    uint32_t PS;         // map pad stride  = max_pads + 4 (2-cell zero border each side, R2)
+    uint32_t TS;         // map time stride = roundup(n_time + 4, 8) uint16 (16-byte multiple)
+    uint32_t LS;         // line-index stride per plane = max_pads + 1
+    uint8_t  npads[256]; // pads of each row (R19)
+};
+
+// Device-side counters of one run (zeroed by a memset node at the start of every run).
+struct Counters {
+    unsigned long long n_bad;       // R11
+    unsigned long long n_used;
+    unsigned long long n_clusters;  // total peaks
+    unsigned int unsorted;          // 1 if digits[i-1] > digits[i] for some i (key = sector,row,pad,time)
+    unsigned int rsv;
+};
+
+// Pointers into the caller-owned workspace.
+struct Workspace {
+    Counters* counters;
+    uint16_t* map;        // [n_planes][PS][TS], zero between runs
+    uint32_t* peakmask;   // bit j%32 of word j/32: digit j is a peak
+    uint32_t* blk_cnt;    // peaks per 256-word block of peakmask
+    uint32_t* blk_off;    // exclusive scan of blk_cnt
+    uint32_t* scan_part;  // scan partials
+    tpc_cluster* stage;   // [max_digits] sparse: cluster of peak digit j at stage[j]
+    tpc_cluster* compact; // [max_clusters] digit-order clusters awaiting the key sort (unsorted input only)
+    uint64_t* keyA; uint64_t* keyB;   // [max_clusters] radix sort ping-pong
+    uint32_t* idxA; uint32_t* idxB;
+    uint32_t* ghist;      // [256][n_sort_tiles]
+    uint32_t* ghist_part;
+    uint32_t* line_start; // [n_planes*LS + 1] first digit of each (plane,pad) line (fused path)
+};
+
+struct Handle;
+
+// ---- shared device arithmetic -------------------------------------------------------------------------------
+
+__host__ __device__ inline uint32_t npads_of(const Geo& g, uint32_t row) { return g.npads[row]; }
+
+// R11: a digit is valid iff it addresses an existing cell and carries charge.
+__device__ __forceinline__ bool digit_valid(const Geo& g, uint32_t w0, uint32_t w1)
+{
+    const uint32_t s = w0 & 0xffu, r = (w0 >> 8) & 0xffu, p = (w0 >> 16) & 0xffu;
+    const uint32_t t = w1 & 0xffffu, q = w1 >> 16;
+    return s < g.n_sectors && r < g.n_rows && p < (uint32_t)g.npads[r < 256u ? r : 0u] && t < g.n_time && q != 0u;
+}
+
+// Sort key of a digit / cluster: (sector,row,pad,time) big-endian in 40 bits (R10).
+__device__ __forceinline__ uint64_t key40(uint32_t w0, uint32_t w1)
+{
+    return ((uint64_t)(w0 & 0xffu) << 32) | ((uint64_t)((w0 >> 8) & 0xffu) << 24) |
+           ((uint64_t)((w0 >> 16) & 0xffu) << 16) | (uint64_t)(w1 & 0xffffu);
+}
+
+// K4: from the 5x5 window c[dp+2][dt+2] around a peak, the gated sums and the 32-byte record.
+// Gate of outer cell (dp,dt) is (dp - sgn dp, dt - sgn dt) (R3); compared raw against q_inner_gate (R4).
+// Sums are integers taken relative to the peak, |S| <= 25*65535*4 < 2^24 (R8), so any order is exact;
+// the variance numerator S0*S2 - S1^2 is formed in int64 and rounded once.
+struct ClusterWords { uint4 lo, hi; };
+
+__device__ __forceinline__ ClusterWords cluster_from_window(const int (&c)[5][5], uint32_t w0, uint32_t time,
+                                                            uint32_t gate)
+{
+    int S0 = 0, S1p = 0, S1t = 0, S2p = 0, S2t = 0;
+#pragma unroll
+    for (int a = 0; a < 5; ++a) {
+#pragma unroll
+        for (int b = 0; b < 5; ++b) {
+            const int dp = a - 2, dt = b - 2;
+            const bool ring = (dp == 2 || dp == -2 || dt == 2 || dt == -2);
+            int v = c[a][b];
+            if (ring) {
+                const int ga = a - (dp > 0) + (dp < 0), gb = b - (dt > 0) + (dt < 0);
+                v = ((uint32_t)c[ga][gb] >= gate) ? v : 0;
+            }
+            S0 += v; S1p += v * dp; S1t += v * dt; S2p += v * dp * dp; S2t += v * dt * dt;
+        }
+    }
+    const uint32_t pad = (w0 >> 16) & 0xffu;
+    const float f0 = (float)S0;
+    const float den = f0 * f0;
+    const long long np = (long long)S0 * S2p - (long long)S1p * S1p;
+    const long long nt = (long long)S0 * S2t - (long long)S1t * S1t;
+    const float pad_mean = (float)pad + (float)S1p / f0;      // R7
+    const float time_mean = (float)time + (float)S1t / f0;
+    const float sp = sqrtf(fmaxf((float)np, 0.f) / den);
+    const float st = sqrtf(fmaxf((float)nt, 0.f) / den);
+    ClusterWords r;
+    r.lo.x = w0 & 0x00ffffffu;                                // sector,row,pad,flags=0
+    r.lo.y = time | ((uint32_t)c[2][2] << 16);                // time,qmax
+    r.lo.z = (uint32_t)S0;                                    // qtot
+    r.lo.w = __float_as_uint(pad_mean);
+    r.hi.x = __float_as_uint(time_mean);
+    r.hi.y = __float_as_uint(sp);
+    r.hi.z = __float_as_uint(st);
+    r.hi.w = 0u;
+    return r;
+}
+
+// ---- launchers (each returns the number of kernels it enqueued, or a negative tpc_cf error) -----------------
+
+int launch_general_peaks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
+                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
+                         cudaEvent_t ev_k0, cudaEvent_t ev_k1);
+int launch_unscatter(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, cudaStream_t st);
+int launch_scatter_only(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, cudaStream_t st);
+int launch_copy_plane(const Geo& g, const Workspace& ws, uint32_t plane, uint32_t P, uint16_t* dense,
+                      cudaStream_t st);
+
+int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
+                        uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
+                        cudaEvent_t ev_k0, cudaEvent_t ev_k1);
+
+// compaction of stage[j] by peakmask into dst (= out, or ws.compact when a key sort must follow)
+int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t capacity, uint64_t max_clusters,
+                   int sort_if_unsorted, cudaStream_t st);
+int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_tiles, tpc_cluster* out,
+                    uint64_t capacity, cudaStream_t st);
+int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,
+                    int hint_sorted, cudaStream_t st);
+
+// exclusive scan of n uint32 (in -> out, may alias); total (optional) receives the sum as 64-bit.
+int launch_scan_u32(const uint32_t* in, uint32_t* out, uint64_t n, uint32_t* partials,
+                    unsigned long long* total, cudaStream_t st);
+
+static inline uint64_t ceil_div_u64(uint64_t a, uint64_t b) { return (a + b - 1) / b; }
+
+}  // namespace tpccf

@@ -1,0 +1,281 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Bar: tests/parity.py.  Paths: "general" (T1, map in HBM, any order) and "fused" (T3, sorted).
+Citations: SURVEY.md §8(a) K0..K5, §8(b) boundary, §8(c) readings; definition BASELINE.json:north_star.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from datagen import gen
+from oracle import oracle as orc
+from parity import assert_clusters_equal, key
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "worked_examples.txt")
+
+
+def _cf():
+    import paper_2402_01205_b200 as cf
+    return cf
+
+
+def parse_golden(path=GOLDEN):
+    ex, cur = [], None
+    for line in open(path):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        tag, rest = line[0], line[1:].split()
+        if tag == "E":
+            cur = {"name": rest[0], "digits": []}
+            ex.append(cur)
+        elif tag == "D":
+            cur["digits"].append(tuple(int(x) for x in rest))
+    return ex
+
+
+PATHS = {"general": 0, "general_hint": 3, "fused": 1}   # flags: DIGITS_SORTED=1, FORCE_GENERAL=2
+
+
+def gpu_run(digits, geom, flags, max_clusters=None, capacity=None, q_peak_min=4, q_inner_gate=2, finder=None):
+    cf = _cf()
+    n_sectors, n_rows, max_pads, n_time, npads = geom
+    n = int(digits.shape[0])
+    own = finder is None
+    if own:
+        finder = cf.ClusterFinder(n_sectors, n_rows, max_pads, n_time, npads=npads, max_digits=max(n, 1),
+                                  max_clusters=max_clusters if max_clusters is not None else max(n, 1),
+                                  q_peak_min=q_peak_min, q_inner_gate=q_inner_gate)
+    d = cf.to_device(digits)
+    finder.run(d, n, flags=flags, capacity=capacity)
+    cl, st = finder.result()
+    if capacity is not None:
+        cl = cl[:capacity]
+    if own:
+        finder.close()
+    return cl, st
+
+
+def sort_digits(d):
+    k = ((d["sector"].astype(np.uint64) << 32) | (d["row"].astype(np.uint64) << 24) |
+         (d["pad"].astype(np.uint64) << 16) | d["time"].astype(np.uint64))
+    return d[np.argsort(k, kind="stable")]
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_worked_examples(path):
+    """E1..E15 (tests/golden/worked_examples.txt) placed on distinct rows of one 12x12 sector, all at once."""
+    ex = parse_golden()
+    digits = np.concatenate([orc.make_digits(e["digits"], sector=0, row=i) for i, e in enumerate(ex)])
+    geom = (1, len(ex), 12, 12, None)
+    if PATHS[path] & 1:
+        digits = sort_digits(digits)       # the golden file lists each example's digits in no particular order
+    ora, ost = orc.run(digits, *geom[:4])
+    cl, st = gpu_run(digits, geom, PATHS[path])
+    assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == 0 and st["overflow"] == 0
+    assert st["path"] == (3 if path == "fused" else 1)
+    assert_clusters_equal(cl, ora, "worked examples/" + path)
+
+
+def test_map_parity_config1():
+    """K1 scatter: dense planes equal the oracle's (SURVEY.md §7.2 minimum slice), and the map is clean after."""
+    cf = _cf()
+    digits = gen.generate(1)
+    geom = gen.geometry(1)
+    f = cf.ClusterFinder(*geom[:4], max_digits=digits.shape[0])
+    d = cf.to_device(digits)
+    for row in (0, 1, 77, 151):
+        got = f.dense_plane(d, digits.shape[0], 0, row, geom[2])
+        want = orc.dense_plane(digits, *geom[:4], 0, row)
+        assert np.array_equal(got, want), "plane row %d differs" % row
+    empty = f.dense_plane(d, 0, 0, 5, geom[2])
+    assert not empty.any(), "map not restored to zero by the un-scatter"
+    f.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_config_full_parity(cfg, path):
+    digits = gen.generate(cfg)
+    geom = gen.geometry(cfg)
+    ora, ost = orc.run(digits, *geom[:4], npads=geom[4])
+    cl, st = gpu_run(digits, geom, PATHS[path], max_clusters=ost["n_clusters"] + 16)
+    assert st["n_clusters"] == ost["n_clusters"] and st["n_digits_used"] == ost["n_digits_used"]
+    assert_clusters_equal(cl, ora, "config %d/%s" % (cfg, path))
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_shuffled_input_general(cfg):
+    """Any-order contract (R12, I1): a random permutation of the digits gives the identical output array."""
+    digits = gen.generate(cfg)
+    geom = gen.geometry(cfg)
+    ora, ost = orc.run(digits, *geom[:4])
+    rng = np.random.default_rng(100 + cfg)
+    sh = digits[rng.permutation(digits.shape[0])]
+    cl, st = gpu_run(sh, geom, 0, max_clusters=ost["n_clusters"] + 16)
+    assert st["path"] == 1 and st["n_clusters"] == ost["n_clusters"]
+    assert_clusters_equal(cl, ora, "config %d shuffled" % cfg)
+
+
+@pytest.mark.parametrize("flags", [1, 3])
+def test_false_sorted_promise_is_detected(flags):
+    """include/tpc_cf.h: a false DIGITS_SORTED promise is detected on the device and reported as path 0."""
+    digits = gen.generate(1)
+    geom = gen.geometry(1)
+    sh = digits[np.random.default_rng(7).permutation(digits.shape[0])]
+    cl, st = gpu_run(sh, geom, flags)
+    assert st["path"] == 0 and st["n_clusters"] == 0
+
+
+def test_run_host_retries_on_false_promise():
+    cf = _cf()
+    digits = gen.generate(1)
+    geom = gen.geometry(1)
+    ora, _ = orc.run(digits, *geom[:4])
+    sh = digits[np.random.default_rng(8).permutation(digits.shape[0])]
+    f = cf.ClusterFinder(*geom[:4], max_digits=digits.shape[0], max_clusters=ora.shape[0] + 8)
+    cl, st = f.run_host(sh, flags=cf.DIGITS_SORTED)
+    assert st["path"] == 1
+    assert_clusters_equal(cl.copy(), ora, "run_host retry")
+    cl, st = f.run_host(digits, flags=cf.DIGITS_SORTED)
+    assert st["path"] == 3
+    assert_clusters_equal(cl.copy(), ora, "run_host sorted")
+    f.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_empty_and_single(path):
+    geom = (2, 3, 20, 40, None)
+    cl, st = gpu_run(np.zeros(0, dtype=orc.DIGIT), geom, PATHS[path])
+    assert st["n_clusters"] == 0 and cl.shape[0] == 0 and st["n_bad_digits"] == 0
+    one = orc.make_digits([(19, 39, 9)], sector=1, row=2)      # last cell of the last plane
+    ora, _ = orc.run(one, *geom[:4])
+    cl, st = gpu_run(one, geom, PATHS[path])
+    assert_clusters_equal(cl, ora, "single digit/" + path)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_bad_digits_are_skipped_and_counted(path):
+    """R11: out-of-range (sector,row,pad for that row,time) and zero-charge digits are skipped and counted."""
+    npads = np.array([10, 12, 16], dtype=np.uint16)
+    geom = (2, 3, 16, 64, npads)
+    good = [(0, 0, 5, 10, 9), (0, 0, 5, 11, 4), (0, 1, 11, 63, 7), (1, 2, 15, 0, 30), (1, 2, 14, 0, 6)]
+    bad = [(0, 0, 10, 5, 50),    # pad 10 does not exist in row 0
+           (0, 1, 12, 5, 50),    # pad 12 does not exist in row 1
+           (0, 1, 3, 64, 50),    # time out of range
+           (1, 1, 3, 3, 0),      # zero charge
+           (2, 0, 1, 1, 50),     # sector out of range
+           (1, 3, 1, 1, 50)]     # row out of range
+    d = np.zeros(len(good) + len(bad), dtype=orc.DIGIT)
+    for i, (s, r, p, t, q) in enumerate(good + bad):
+        d[i] = (s, r, p, 0, t, q)
+    d = sort_digits(d)
+    ora, ost = orc.run(d, *geom[:4], npads=npads)
+    assert ost["n_bad_digits"] == len(bad)
+    cl, st = gpu_run(d, geom, PATHS[path])
+    assert st["n_bad_digits"] == len(bad) and st["n_digits_used"] == len(good)
+    assert_clusters_equal(cl, ora, "bad digits/" + path)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_capacity_overflow(path):
+    """§8(b): more peaks than capacity => first `capacity` clusters in output order, true count, overflow = 1."""
+    digits = gen.generate(1)
+    geom = gen.geometry(1)
+    ora, ost = orc.run(digits, *geom[:4])
+    cap = 1000
+    cl, st = gpu_run(digits, geom, PATHS[path], capacity=cap)
+    assert st["overflow"] == 1 and st["n_clusters"] == ost["n_clusters"]
+    assert_clusters_equal(cl[:cap], ora[:cap], "overflow/" + path)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_variable_pads_and_back_to_back_frames(path):
+    """config 5 at 2 sectors: npads 66->138 (R19), 4 frames enqueued back to back on one stream with one
+    workspace (R16): a stale map or stale staging would show up as ghost clusters."""
+    cf = _cf()
+    import torch
+    c = dict(gen.CONFIGS[5]); c["n_sectors"] = 2
+    geom = gen.geometry(c)
+    frames = [gen.generate(c, frame=f) for f in range(4)]
+    nmax = max(f.shape[0] for f in frames)
+    finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=nmax, max_clusters=nmax // 8)
+    devs = [cf.to_device(f) for f in frames]
+    outs = [torch.empty(finder.max_clusters * 32, dtype=torch.uint8, device="cuda:0") for _ in frames]
+    sts = [torch.zeros(32, dtype=torch.uint8, device="cuda:0") for _ in frames]
+    for f, d, o, s in zip(frames, devs, outs, sts):
+        finder.run(d, f.shape[0], flags=PATHS[path], clusters=o, status=s)
+    for i, (f, o, s) in enumerate(zip(frames, outs, sts)):
+        cl, st = finder.result(clusters=o, status=s)
+        ora, ost = orc.run(f, *geom[:4], npads=geom[4])
+        assert st["n_clusters"] == ost["n_clusters"]
+        assert_clusters_equal(cl, ora, "config5 frame %d/%s" % (i, path))
+    finder.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_dense_pairs_plateaus(path):
+    """config 4 at 1 sector: ~10% occupancy, 30% close pairs, flat-top plateaus (R1b, R5)."""
+    c = dict(gen.CONFIGS[4]); c["n_sectors"] = 1
+    geom = gen.geometry(c)
+    digits = gen.generate(c)
+    ora, ost = orc.run(digits, *geom[:4])
+    cl, st = gpu_run(digits, geom, PATHS[path], max_clusters=ost["n_clusters"] + 16)
+    assert st["n_clusters"] == ost["n_clusters"]
+    assert_clusters_equal(cl, ora, "config4x1/" + path)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_thresholds_and_saturated_charges(path):
+    """Non-default thresholds and full-range uint16 charges (R13, P5): random 40x60 planes, values up to 65535."""
+    rng = np.random.default_rng(11)
+    geom = (1, 6, 40, 60, None)
+    cells = []
+    d = []
+    for row in range(6):
+        m = rng.random((40, 60)) < (0.05 + 0.15 * row)
+        p, t = np.nonzero(m)
+        q = rng.choice([1, 2, 3, 4, 5, 9, 200, 65535], size=p.size)
+        for a, b, c_ in zip(p, t, q):
+            d.append((0, row, a, 0, b, c_))
+    digits = sort_digits(np.array(d, dtype=orc.DIGIT))
+    for qmin, gate in ((4, 2), (1, 0), (5, 65535), (200, 3)):
+        ora, ost = orc.run(digits, *geom[:4], q_peak_min=qmin, q_inner_gate=gate)
+        cl, st = gpu_run(digits, geom, PATHS[path], q_peak_min=qmin, q_inner_gate=gate)
+        assert_clusters_equal(cl, ora, "thresholds %d/%d %s" % (qmin, gate, path))
+
+
+def test_full_frame_sampled_planes():
+    """BASELINE.json configs[2] at full size (36 sectors, ~2%), in the launch configuration bench.py times (fused
+    path, DIGITS_SORTED): cluster count and order checked globally, and the clusters of sampled planes compared
+    one by one with the oracle run on exactly those planes."""
+    cf = _cf()
+    geom = gen.geometry(3)
+    digits = gen.generate(3)
+    n = digits.shape[0]
+    f = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=n // 12)
+    d = cf.to_device(digits)
+    f.run(d, n, flags=cf.DIGITS_SORTED)
+    cl, st = f.result()
+    assert st["path"] == 3 and st["overflow"] == 0 and st["n_digits_used"] == n
+    k = key(cl)
+    assert np.all(k[1:] > k[:-1])
+    plane_of = cl["sector"].astype(np.int64) * geom[1] + cl["row"]
+    dplane = digits["sector"].astype(np.int64) * geom[1] + digits["row"]
+    rng = np.random.default_rng(3)
+    total = 0
+    for pl in [0, geom[0] * geom[1] - 1] + list(rng.integers(0, geom[0] * geom[1], size=22)):
+        lo, hi = np.searchsorted(dplane, [pl, pl + 1])
+        ora, ost = orc.run(digits[lo:hi], *geom[:4], planes=(int(pl), int(pl) + 1))
+        a, b = np.searchsorted(plane_of, [pl, pl + 1])
+        assert_clusters_equal(cl[a:b], ora, "config 3 plane %d" % pl)
+        total += ora.shape[0]
+    assert total > 10000
+    # general path on the same frame: identical array
+    f.run(d, n, flags=cf.DIGITS_SORTED | cf.FORCE_GENERAL)
+    cl2, st2 = f.result()
+    assert st2["path"] == 1 and st2["n_clusters"] == st["n_clusters"]
+    assert np.array_equal(cl2.view(np.uint8), cl.view(np.uint8)), "general and fused path differ on config 3"
+    f.close()
