@@ -52,10 +52,11 @@ typedef struct {
 } tpc_cf_geometry;
 
 enum {
-    TPC_CF_DIGITS_SORTED = 1u,  /* hint: digits ascend in (sector,row,pad,time).  Selects the fused shared-memory
-                                   path ("T3").  The hint is verified on the device for free; if it is false (or a
-                                   capacity of the fused path is exceeded) the general path runs instead and
-                                   status.path says so.  The result never depends on the hint. */
+    TPC_CF_DIGITS_SORTED = 1u,  /* promise: digits ascend in (sector,row,pad,time).  Selects the fused shared-memory
+                                   path ("T3") and skips the key sort.  The promise is verified on the device for
+                                   free; if it is false nothing is output and status.path = 0, n_clusters = 0
+                                   (rerun without the flag; tpc_cf_run_host does that by itself).  A wrong result
+                                   is never returned silently. */
     TPC_CF_FORCE_GENERAL = 2u   /* always run the general (map in HBM, "T1") path, whatever the order */
 };
 
@@ -71,7 +72,8 @@ typedef struct {
     uint64_t n_digits_used;  /* valid digits */
     uint64_t n_bad_digits;   /* R11: out-of-range or zero-charge digits: skipped and counted */
     uint32_t overflow;       /* 1 if n_clusters > capacity: the first `capacity` clusters in output order are written */
-    uint32_t path;           /* 1 = general path (T1) produced the output, 3 = fused sorted path (T3) */
+    uint32_t path;           /* 1 = general path (T1) produced the output, 3 = fused sorted path (T3),
+                                0 = no output: DIGITS_SORTED was promised but the digits are not sorted */
 } tpc_cf_status;
 
 typedef struct {
@@ -129,11 +131,13 @@ int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint64_t n,
 /* Number of kernel launches the last run enqueued (for bench.py's gpu_launches). */
 int tpc_cf_last_launch_count(const tpc_cf* h);
 
-/* Device time in ms of kernel class `which` during the last run, measured by CUDA events recorded on the run's
- * stream when profiling was enabled with tpc_cf_set_profiling(h, 1).  which: 0 = whole run, 1 = fused T3 kernel
- * (or T1 peak kernel when the general path ran).  Synchronises on the events.  Negative on error. */
+/* Profiling (bench.py's roofline leg).  After tpc_cf_set_profiling(h, 1) every run records CUDA events on its
+ * stream around the whole run and around its dominant kernel (the fused kernel on the sorted path, the
+ * peak+moment kernel on the general path); the last 64 runs are kept.  tpc_cf_profile_ms(h, run, which) returns
+ * the device time in ms of run number `run` (0 = first run after profiling was switched on): which = 0 whole
+ * run, 1 dominant kernel.  It synchronises on that run's events.  Negative on error / unknown run. */
 int   tpc_cf_set_profiling(tpc_cf* h, int on);
-float tpc_cf_last_kernel_ms(tpc_cf* h, int which);
+float tpc_cf_profile_ms(tpc_cf* h, uint32_t run, int which);
 
 int tpc_cf_destroy(tpc_cf* h);
 

@@ -26,7 +26,7 @@ FORCE_GENERAL = 2
 
 EXPORTS = ["tpc_cf_workspace_bytes", "tpc_cf_create", "tpc_cf_run", "tpc_cf_run_host",
            "tpc_cf_debug_dense_plane", "tpc_cf_last_launch_count", "tpc_cf_set_profiling",
-           "tpc_cf_last_kernel_ms", "tpc_cf_destroy", "tpc_cf_strerror"]
+           "tpc_cf_profile_ms", "tpc_cf_destroy", "tpc_cf_strerror"]
 
 
 class Geometry(ctypes.Structure):
@@ -83,8 +83,8 @@ def load(build_if_missing=True):
     lib.tpc_cf_last_launch_count.argtypes = [ctypes.c_void_p]
     lib.tpc_cf_set_profiling.restype = ctypes.c_int
     lib.tpc_cf_set_profiling.argtypes = [ctypes.c_void_p, ctypes.c_int]
-    lib.tpc_cf_last_kernel_ms.restype = ctypes.c_float
-    lib.tpc_cf_last_kernel_ms.argtypes = [ctypes.c_void_p, ctypes.c_int]
+    lib.tpc_cf_profile_ms.restype = ctypes.c_float
+    lib.tpc_cf_profile_ms.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_int]
     lib.tpc_cf_destroy.restype = ctypes.c_int
     lib.tpc_cf_destroy.argtypes = [ctypes.c_void_p]
     lib.tpc_cf_strerror.restype = ctypes.c_char_p
@@ -213,8 +213,8 @@ class ClusterFinder:
     def set_profiling(self, on):
         _check(self.lib.tpc_cf_set_profiling(self.h, 1 if on else 0))
 
-    def last_kernel_ms(self, which):
-        return float(self.lib.tpc_cf_last_kernel_ms(self.h, which))
+    def profile_ms(self, run, which):
+        return float(self.lib.tpc_cf_profile_ms(self.h, run, which))
 
     def last_launch_count(self):
         return int(self.lib.tpc_cf_last_launch_count(self.h))

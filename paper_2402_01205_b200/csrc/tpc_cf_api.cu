@@ -8,6 +8,8 @@
 
 using namespace tpccf;
 
+static constexpr int kProfSlots = 64;
+
 struct tpc_cf {
     Geo geo;
     Workspace ws;
@@ -16,7 +18,8 @@ struct tpc_cf {
     size_t map_bytes;
     int last_launches;
     int profiling;
-    cudaEvent_t ev[4];          // run begin, dominant kernel begin, dominant kernel end, run end
+    uint32_t run_index;         // runs since profiling was switched on
+    cudaEvent_t ev[kProfSlots][4];   // per slot: run begin, dominant kernel begin, dominant kernel end, run end
     char cuda_msg[256];
 };
 
@@ -112,14 +115,18 @@ extern "C" int tpc_cf_create(tpc_cf** hp, const tpc_cf_geometry* geom, uint64_t 
     h->max_digits = max_digits;
     h->max_clusters = max_clusters;
     carve(g, max_digits, max_clusters, (char*)workspace, &h->ws, &h->n_sort_tiles, &h->map_bytes);
-    for (int i = 0; i < 4; ++i) {
-        cudaError_t e = cudaEventCreate(&h->ev[i]);
+    for (int i = 0; i < kProfSlots * 4; ++i) {
+        cudaError_t e = cudaEventCreate(&h->ev[i / 4][i % 4]);
         if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaEventCreate"); }
     }
     // K0, once: the charge map starts zero; every run restores it (un-scatter).
     cudaError_t e = cudaMemsetAsync(h->ws.map, 0, h->map_bytes, (cudaStream_t)stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), (cudaStream_t)stream);
-    if (e != cudaSuccess) { for (int i = 0; i < 4; ++i) cudaEventDestroy(h->ev[i]); delete h; return cuda_fail(nullptr, e, "cudaMemsetAsync(map)"); }
+    if (e != cudaSuccess) {
+        for (int i = 0; i < kProfSlots * 4; ++i) cudaEventDestroy(h->ev[i / 4][i % 4]);
+        delete h;
+        return cuda_fail(nullptr, e, "cudaMemsetAsync(map)");
+    }
     *hp = h;
     return TPC_CF_OK;
 }
@@ -148,17 +155,18 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     const bool hint = (params->flags & TPC_CF_DIGITS_SORTED) != 0;
     const bool fused = hint && !(params->flags & TPC_CF_FORCE_GENERAL);
     const bool prof = h->profiling != 0;
+    cudaEvent_t* ev = h->ev[h->run_index % kProfSlots];
     int k = 0;
 
     (void)cudaGetLastError();
-    if (prof) cudaEventRecord(h->ev[0], st);
+    if (prof) cudaEventRecord(ev[0], st);
     cudaError_t e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), st);
     if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(counters)");
 
     if (fused) {
         // T3: line index -> fused smem kernel (scatter into smem lines, peak test, moments) -> compaction
         int r = launch_fused_sorted(h->geo, h->ws, digits, n, params->q_peak_min, params->q_inner_gate, st,
-                                    prof ? h->ev[1] : nullptr, prof ? h->ev[2] : nullptr);
+                                    prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
         if (r < 0) return r;
         k += r;
         k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, 0, st);
@@ -167,13 +175,13 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
         // T1: K1 scatter -> K2+K4 digit-centric peaks + moments on the HBM map -> K3 compaction -> (K5 key sort)
         //     -> K0 un-scatter
         k += launch_general_peaks(h->geo, h->ws, digits, n, params->q_peak_min, params->q_inner_gate, st,
-                                  prof ? h->ev[1] : nullptr, prof ? h->ev[2] : nullptr);
+                                  prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
         k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, hint ? 0 : 1, st);
         if (!hint) k += launch_key_sort(h->ws, h->max_clusters, h->n_sort_tiles, out->clusters, out->capacity, st);
         k += launch_unscatter(h->geo, h->ws, digits, n, st);
         k += launch_finalize(h->ws, out->status, out->capacity, 1u, hint ? 1 : 0, st);
     }
-    if (prof) cudaEventRecord(h->ev[3], st);
+    if (prof) { cudaEventRecord(ev[3], st); ++h->run_index; }
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(h, e, "kernel launch");
     h->last_launches = k;
@@ -234,16 +242,18 @@ extern "C" int tpc_cf_set_profiling(tpc_cf* h, int on)
 {
     if (!h) return TPC_CF_E_NULL;
     h->profiling = on ? 1 : 0;
+    h->run_index = 0;
     return TPC_CF_OK;
 }
 
-extern "C" float tpc_cf_last_kernel_ms(tpc_cf* h, int which)
+extern "C" float tpc_cf_profile_ms(tpc_cf* h, uint32_t run, int which)
 {
-    if (!h || !h->profiling) return -1.f;
+    if (!h || !h->profiling || run >= h->run_index || run + kProfSlots < h->run_index) return -1.f;
+    cudaEvent_t* ev = h->ev[run % kProfSlots];
     float ms = -1.f;
     cudaError_t e;
-    if (which == 0) { e = cudaEventSynchronize(h->ev[3]); if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, h->ev[0], h->ev[3]); }
-    else            { e = cudaEventSynchronize(h->ev[2]); if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, h->ev[1], h->ev[2]); }
+    if (which == 0) { e = cudaEventSynchronize(ev[3]); if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ev[0], ev[3]); }
+    else            { e = cudaEventSynchronize(ev[2]); if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ev[1], ev[2]); }
     if (e != cudaSuccess) { cuda_fail(h, e, "event timing"); return -1.f; }
     return ms;
 }
@@ -251,7 +261,7 @@ extern "C" float tpc_cf_last_kernel_ms(tpc_cf* h, int which)
 extern "C" int tpc_cf_destroy(tpc_cf* h)
 {
     if (!h) return TPC_CF_E_NULL;
-    for (int i = 0; i < 4; ++i) cudaEventDestroy(h->ev[i]);
+    for (int i = 0; i < kProfSlots * 4; ++i) cudaEventDestroy(h->ev[i / 4][i % 4]);
     delete h;
     return TPC_CF_OK;
 }
