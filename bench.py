@@ -1,0 +1,331 @@
+#!/usr/bin/env python
+"""bench.py — TPC cluster finder on B200: digits/s (BASELINE.json:metric) on a synthetic time frame.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--path fused|general] [--impl reference]
+
+A step = one pass of the whole hot path (SURVEY.md §8(a) K0..K5 = one tpc_cf_run) over one full time frame that is
+already resident in HBM.  Default workload: BASELINE.json configs[2] (36 sectors x 152 rows x 138 pads x 14336 time
+bins, ~2 % occupancy, seed 3) — the full frame the north_star's target is quoted on; it fits one GPU.
+N > 1 (torchrun): replicas only ("avoiding any GPU intercommunication"): every rank
+processes its own frame (frame index = rank), no data-path collective; value = total digits / max-over-ranks time.
+`--impl reference` times the CPU oracle (oracle/, as it stands, single thread) on a bounded sample of the same
+workload on the host cores.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "tpc_digits_per_second"
+UNIT = "digits/s"
+
+
+def load_peaks():
+    """Measured roofline denominators (driver-written), else the fallback of B200_PROFILING.md."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+def load_traffic(workload, path):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(p) as f:
+            t = json.load(f)
+        e = t.get("%s/%s" % (workload, path))
+        return float(e["dram_bytes_per_launch"]) if e else None
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.rows = []
+        self.stop = False
+        self.th = None
+
+    def _poll(self):
+        while not self.stop:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                if out.returncode == 0 and out.stdout.strip():
+                    self.rows.append([c.strip() for c in out.stdout.strip().split(",")])
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def __enter__(self):
+        self.th = threading.Thread(target=self._poll, daemon=True)
+        self.th.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop = True
+        self.th.join(timeout=6)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def oracle_sample(cfg_id, n_sectors_sample, frame=0):
+    """Bounded sample for the CPU oracle: the first n_sectors_sample sectors of the workload (same bytes as the
+    full frame's slice).  Returns (digits, geometry)."""
+    from datagen import gen
+    geom = gen.geometry(cfg_id)
+    d = gen.generate(cfg_id, frame=frame, sectors=(0, n_sectors_sample))
+    return d, geom
+
+
+def time_oracle(digits, geom, n_sectors_sample):
+    from oracle import oracle as orc
+    t0 = time.perf_counter()
+    cl, st = orc.run(digits, geom[0], geom[1], geom[2], geom[3], npads=geom[4],
+                     planes=(0, n_sectors_sample * geom[1]))
+    dt = time.perf_counter() - t0
+    return dt, st
+
+
+def sample_sectors(cfg_id):
+    # ~8 ms per 138x14336 plane single-threaded => 8 sectors (1216 planes) ~ 10-15 s; config 1/2 have one sector
+    from datagen import gen
+    return min(gen.CONFIGS[cfg_id]["n_sectors"], 8)
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from datagen import gen
+    from oracle import oracle as orc
+    orc.build()
+    ns = sample_sectors(args.config)
+    digits, geom = oracle_sample(args.config, ns)
+    for _ in range(min(args.warmup, 1)):
+        time_oracle(digits, geom, ns)
+    times = []
+    for _ in range(args.steps):
+        dt, st = time_oracle(digits, geom, ns)
+        times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    value = digits.shape[0] / (ms * 1e-3)
+    sample = "first %d of %d sectors of the frame (%d digits, %d clusters) per step" % (
+        ns, geom[0], digits.shape[0], st["n_clusters"])
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u16/i64/f64", "data": "synthetic",
+            "config": {"workload": "config%d: %s" % (args.config, gen.CONFIGS[args.config]["label"]),
+                       "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "clusters_per_s": st["n_clusters"] / (ms * 1e-3)}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--path", default="fused", choices=["fused", "general"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from datagen import gen
+    import paper_2402_01205_b200 as cf
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local_rank)
+    dev = "cuda:%d" % local_rank
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    cfg = gen.CONFIGS[args.config]
+    geom = gen.geometry(args.config)
+    n_frames = cfg["frames"]
+    # replicas: rank r works on its own frames (frame index offset by rank * n_frames)
+    t0 = time.perf_counter()
+    frames = [gen.generate(args.config, frame=rank * n_frames + f) for f in range(n_frames)]
+    gen_s = time.perf_counter() - t0
+    n_digits = [int(f.shape[0]) for f in frames]
+    nmax = max(n_digits)
+    max_clusters = nmax // 10 + 1024
+    finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=nmax, max_clusters=max_clusters, device=dev)
+    flags = cf.DIGITS_SORTED if args.path == "fused" else (cf.DIGITS_SORTED | cf.FORCE_GENERAL)
+
+    pinned = [torch.from_numpy(f.view(np.uint8)).pin_memory() for f in frames]
+    dev_digits = [p.to(dev, non_blocking=True) for p in pinned]
+    outs = [torch.empty(max_clusters * 32, dtype=torch.uint8, device=dev) for _ in frames]
+    stats = [torch.zeros(32, dtype=torch.uint8, device=dev) for _ in frames]
+    torch.cuda.synchronize()
+
+    def step():
+        for d, n, o, s in zip(dev_digits, n_digits, outs, stats):
+            finder.run(d, n, flags=flags, clusters=o, status=s)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    sts = [finder.result(clusters=o, status=s)[1] for o, s in zip(outs, stats)]
+    for st in sts:
+        if st["path"] == 0 or st["overflow"]:
+            raise RuntimeError("bench run invalid: status %r" % (st,))
+    n_clusters = [st["n_clusters"] for st in sts]
+    launches_per_step = finder.last_launch_count() * n_frames
+
+    # ---- timed region: K steps, device-resident inputs (each frame > L2, so no L2 flush is needed) ----
+    finder.set_profiling(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    with ClockSampler(local_rank) as clocks:
+        ev0.record()
+        for _ in range(args.steps):
+            step()
+        ev1.record()
+        torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    total_ms = ev0.elapsed_time(ev1)
+    runs = args.steps * n_frames
+    kern_ms = [finder.profile_ms(r, 1) for r in range(max(0, runs - 64), runs)]
+    kern_ms = [k for k in kern_ms if k > 0]
+    finder.set_profiling(False)
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        c = torch.tensor([sum(n_digits), sum(n_clusters)], dtype=torch.float64, device=dev)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        digits_per_step, clusters_per_step = float(c[0].item()), float(c[1].item())
+    else:
+        digits_per_step, clusters_per_step = float(sum(n_digits)), float(sum(n_clusters))
+    ms_per_step = total_ms / args.steps
+    value = digits_per_step / (ms_per_step * 1e-3)
+
+    # ---- e2e: the public call with HOST buffers (pinned), H2D + run + D2H of status and clusters, every step ----
+    e2e = None
+    if not args.no_e2e:
+        host_out = torch.empty(max_clusters * 32, dtype=torch.uint8, pin_memory=True)
+        e_steps = max(1, min(args.steps, 3))
+        for p, d in zip(pinned, dev_digits):
+            finder.run_host(p, flags=flags, dev_digits=d, host_clusters=host_out)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(e_steps):
+            for p, d in zip(pinned, dev_digits):
+                cl, st = finder.run_host(p, flags=flags, dev_digits=d, host_clusters=host_out)
+        torch.cuda.synchronize()
+        e_ms = (time.perf_counter() - t0) * 1e3 / e_steps
+        if world > 1:
+            t = torch.tensor([e_ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_ms = float(t.item())
+        e2e = {"value": digits_per_step / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms,
+               "h2d_bytes_per_step": int(sum(n_digits) * 8), "d2h_bytes_per_step": int(sum(n_clusters) * 32 + 32 * n_frames),
+               "steps": e_steps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (HBM-bound: stencil/compaction work, no contraction) ----
+    peak, peak_src = load_peaks()
+    nd, nc = n_digits[-1], n_clusters[-1]     # per launch: one frame
+    if args.path == "fused":
+        kname = "k_fused_lines"
+        # algorithmic bytes per launch: 8 B/digit read, 32 B/cluster staged, 1 bit/digit peak mask
+        alg_bytes = 8.0 * nd + 32.0 * nc + nd / 8.0
+    else:
+        kname = "k_peaks_map"
+        # 8 B/digit read + 3x3 neighbourhood of every digit >= threshold is covered by the 2 B/digit map cells of
+        # three lines (each map sector counted once) + 32 B/cluster staged + peak mask
+        alg_bytes = 8.0 * nd + 2.0 * nd + 32.0 * nc + nd / 8.0
+    k_ms = float(np.mean(kern_ms)) if kern_ms else None
+    roof = {"bound": "hbm", "kernel": kname, "achieved": (alg_bytes / (k_ms * 1e-3) / 1e9) if k_ms else None,
+            "peak": peak, "unit": "GB/s", "peak_source": peak_src,
+            "frac": (alg_bytes / (k_ms * 1e-3) / 1e9 / peak) if k_ms else None,
+            "traffic": load_traffic("config%d" % args.config, args.path),
+            "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms,
+            "kernel_share_of_step": (k_ms * n_frames / ms_per_step) if k_ms else None}
+    io_bytes = 8.0 * digits_per_step + 32.0 * clusters_per_step
+    f_io = io_bytes / (ms_per_step * 1e-3) / 1e9 / peak
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import oracle as orc
+        orc.build()
+        ns = sample_sectors(args.config)
+        hi = int(np.searchsorted(frames[0]["sector"], ns))
+        sample = frames[0][:hi]
+        dt, ost = time_oracle(sample, geom, ns)
+        cpu = {"value": sample.shape[0] / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": "first %d of %d sectors of frame 0 (%d digits, %d clusters), %.1f s, single thread" % (
+                   ns, geom[0], sample.shape[0], ost["n_clusters"], dt),
+               "clusters_per_s": ost["n_clusters"] / dt, "host_cores_available": os.cpu_count()}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u16/i32/f32", "data": "synthetic",
+            "config": {"workload": "config%d: %s" % (args.config, cfg["label"]), "path": args.path,
+                       "frames_per_step": n_frames, "digits_per_frame": nd, "clusters_per_frame": nc,
+                       "occupancy": gen.occupancy(frames[0], args.config), "parallelism": "replicas x%d" % world,
+                       "l2": "inputs (%.2f GB digits per frame) larger than the 126 MB L2; no flush" % (nd * 8 / 1e9),
+                       "checksum_frame0": "%016x" % gen.checksum(frames[0]) if nd < 50_000_000 else "skipped (large)",
+                       "gen_seconds": gen_s},
+            "clusters_per_s": clusters_per_step / (ms_per_step * 1e-3),
+            "f_io": {"value": f_io, "bytes_per_step": io_bytes, "note": "compulsory I/O (8 B/digit + 32 B/cluster) / time / peak"},
+            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+            "clocks": clocks.summary()}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
