@@ -21,6 +21,7 @@ namespace tpccf {
 static constexpr int kFThreads = 256;
 static constexpr int kS = 2;                    // lines per step
 static constexpr int kSlots = 3 * kS + 4;       // process window S+4, build S, clear S
+static constexpr int kPeakQ = 512;              // CTA peak queue entries per step
 
 __device__ __forceinline__ uint32_t key24_of(uint32_t w0)
 {
@@ -85,6 +86,9 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_ls[260];       // line starts of this plane: s_ls[p] for p = 0..max_pads, then next plane's start
     __shared__ int s_unsorted;
+    __shared__ uint32_t s_wq[kFThreads / 32][64];   // per-warp survivor queues (stage A -> B)
+    __shared__ uint32_t s_pq[kPeakQ];               // CTA peak queue (stage B -> C)
+    __shared__ uint32_t s_npk[2];                   // its fill count, double-buffered by step parity
 
     const uint32_t plane = blockIdx.x / units_per_plane, unit = blockIdx.x % units_per_plane;
     const uint32_t sector = plane / g.n_rows, row = plane % g.n_rows;
@@ -92,7 +96,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     const int pa = (int)(unit * pads_per_unit);
     const int pb = min(pa + (int)pads_per_unit, P);
     const int T = (int)g.n_time;
-    const int tid = threadIdx.x, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t w0_base = sector | (row << 8);
 
     // slot views
@@ -107,7 +111,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     };
 
     for (int i = tid; i <= (int)g.LS; i += kFThreads) s_ls[i] = line_start[plane * g.LS + i];
-    if (tid == 0) s_unsorted = 0;
+    if (tid == 0) { s_unsorted = 0; s_npk[0] = 0u; s_npk[1] = 0u; }
     for (uint32_t i = tid; i < kSlots * slot_words; i += kFThreads) sm[i] = 0u;
     __syncthreads();
 
@@ -178,71 +182,134 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     };
 
     // ---- K2 + K4: digit-centric peak test and moments for lines [l0,l1) -------------------------------------------
-    auto process = [&](int l0, int l1) {
+    // Peaks are ~1 in 20 digits, so the work is done in three dense stages instead of one divergent pass:
+    //   A (every digit)     own-line test against the adjacent digits of the line; survivors -> per-warp queue
+    //   B (survivors, ~25%) lines p-1 / p+1 through the bitmap windows; peaks -> CTA queue + peakmask bit
+    //   C (peaks, ~5%)      5x5 window from the five slots, gated sums, record -> stage[j]   (after a barrier)
+    auto locate = [&](uint32_t j, int l0, int l1, int& p, uint32_t& jl, uint32_t& len) {
+        p = l0;
+#pragma unroll
+        for (int i = 1; i < kS; ++i) if (l0 + i < l1 && j >= s_ls[l0 + i]) p = l0 + i;
+        const uint32_t lbeg = s_ls[p];
+        jl = j - lbeg;
+        len = s_ls[p + 1] - lbeg;
+    };
+    auto fetch = [&](const SlotView& sv, uint32_t j, uint32_t jl) -> uint32_t {
+        if (jl < cap) return sv.tq[jl];
+        return __ldg(&digits[min(j, n - 1)].y);
+    };
+    auto moments = [&](uint32_t j, int p, int t) {
+        int c[5][5];
+#pragma unroll
+        for (int a = 0; a < 5; ++a) {
+            const int pp = p + a - 2;
+            if (pp >= 0 && pp < P) {
+                window<2>(slot_of(pp), cap, digits, s_ls[pp], n, t, c[a]);
+            } else {
+#pragma unroll
+                for (int b = 0; b < 5; ++b) c[a][b] = 0;
+            }
+        }
+        const ClusterWords r = cluster_from_window(c, w0_base | ((uint32_t)p << 16), (uint32_t)t, q_gate);
+        stage[2 * (size_t)j] = r.lo;
+        stage[2 * (size_t)j + 1] = r.hi;
+    };
+    auto stage_b = [&](bool act, uint32_t j, int l0, int l1, int par) {
+        bool peak = false;
+        int p = l0, t = 0;
+        if (act) {
+            uint32_t jl, len;
+            locate(j, l0, l1, p, jl, len);
+            const uint32_t self = fetch(slot_of(p), j, jl);
+            t = (int)(self & 0xffffu);
+            const uint32_t q = self >> 16;
+            peak = true;
+            if (p > 0) {                                                    // line p-1: earlier, strict (R1)
+                int c[3];
+                window<1>(slot_of(p - 1), cap, digits, s_ls[p - 1], n, t, c);
+                peak = q > (uint32_t)c[0] && q > (uint32_t)c[1] && q > (uint32_t)c[2];
+            }
+            if (peak && p + 1 < P) {                                        // line p+1: later, >=
+                int c[3];
+                window<1>(slot_of(p + 1), cap, digits, s_ls[p + 1], n, t, c);
+                peak = q >= (uint32_t)c[0] && q >= (uint32_t)c[1] && q >= (uint32_t)c[2];
+            }
+        }
+        const unsigned pm = __ballot_sync(0xffffffffu, peak);
+        if (pm == 0) return;
+        const int leader = __ffs(pm) - 1;
+        uint32_t base = 0;
+        if (lane == leader) base = atomicAdd(&s_npk[par], (uint32_t)__popc(pm));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (peak) {
+            atomicOr(&peakmask[j >> 5], 1u << (j & 31u));
+            const uint32_t slot = base + (uint32_t)__popc(pm & ((1u << lane) - 1u));
+            if (slot < kPeakQ) s_pq[slot] = j;
+            else moments(j, p, t);                                          // queue full: do it here (rare)
+        }
+    };
+    auto phase1 = [&](int l0, int l1, int par) {
         l1 = min(l1, pb);
         if (l0 >= l1) return;
         const uint32_t jb = s_ls[l0], je = s_ls[l1];
         if (je <= jb) return;
-        for (uint32_t j0 = (jb & ~31u); j0 < je; j0 += kFThreads) {
-            const uint32_t j = j0 + tid;
-            bool peak = false;
-            int p = l0, t = 0;
-            uint32_t q = 0, jl = 0;
+        uint32_t* wq = s_wq[warp];
+        uint32_t wcount = 0;                                                // warp-uniform
+        for (uint32_t j0 = (jb & ~31u) + 32u * warp; j0 < je; j0 += kFThreads) {
+            const uint32_t j = j0 + lane;
+            bool surv = false;
             if (j >= jb && j < je) {
-#pragma unroll
-                for (int i = 1; i < kS; ++i) if (l0 + i < l1 && j >= s_ls[l0 + i]) p = l0 + i;
-                const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
-                jl = j - lbeg;
+                int p; uint32_t jl, len;
+                locate(j, l0, l1, p, jl, len);
                 const SlotView sv = slot_of(p);
-                uint32_t self;
-                if (jl < cap) self = sv.tq[jl]; else self = __ldg(&digits[j].y);
-                t = (int)(self & 0xffffu); q = self >> 16;
+                const uint32_t self = fetch(sv, j, jl);
+                const int t = (int)(self & 0xffffu);
+                const uint32_t q = self >> 16;
                 if (q >= q_peak_min && t < T) {
-                    // own line: neighbours in time are the adjacent digits of the line
-                    uint32_t prev = 0, next = 0;
-                    if (jl > 0) { if (jl - 1 < cap) prev = sv.tq[jl - 1]; else prev = __ldg(&digits[j - 1].y); }
-                    if (jl + 1 < len) { if (jl + 1 < cap) next = sv.tq[jl + 1]; else next = __ldg(&digits[min(j + 1, n - 1)].y); }
+                    // own line: the neighbours in time are the adjacent digits of the line
+                    const uint32_t prev = jl > 0 ? fetch(sv, j - 1, jl - 1) : 0u;
+                    const uint32_t next = jl + 1 < len ? fetch(sv, j + 1, jl + 1) : 0u;
                     const uint32_t qm = (jl > 0 && (int)(prev & 0xffffu) == t - 1) ? (prev >> 16) : 0u;
                     const uint32_t qp = (jl + 1 < len && (int)(next & 0xffffu) == t + 1 && t + 1 < T) ? (next >> 16) : 0u;
-                    peak = q > qm && q >= qp;                                   // R1: (0,-1) strict, (0,+1) >=
-                    if (peak && p > 0) {                                        // line p-1: earlier, strict
-                        int c[3];
-                        window<1>(slot_of(p - 1), cap, digits, s_ls[p - 1], n, t, c);
-                        peak = q > (uint32_t)c[0] && q > (uint32_t)c[1] && q > (uint32_t)c[2];
-                    }
-                    if (peak && p + 1 < P) {                                    // line p+1: later, >=
-                        int c[3];
-                        window<1>(slot_of(p + 1), cap, digits, s_ls[p + 1], n, t, c);
-                        peak = q >= (uint32_t)c[0] && q >= (uint32_t)c[1] && q >= (uint32_t)c[2];
-                    }
+                    surv = q > qm && q >= qp;                               // R1: (0,-1) strict, (0,+1) >=
                 }
             }
-            const unsigned m = __ballot_sync(0xffffffffu, peak);
-            if (lane == 0 && m) atomicOr(&peakmask[j >> 5], m);
-            if (peak) {
-                int c[5][5];
-#pragma unroll
-                for (int a = 0; a < 5; ++a) {
-                    const int pp = p + a - 2;
-                    if (pp >= 0 && pp < P) {
-                        window<2>(slot_of(pp), cap, digits, s_ls[pp], n, t, c[a]);
-                    } else {
-#pragma unroll
-                        for (int b = 0; b < 5; ++b) c[a][b] = 0;
-                    }
-                }
-                const ClusterWords r = cluster_from_window(c, w0_base | ((uint32_t)p << 16), (uint32_t)t, q_gate);
-                stage[2 * (size_t)j] = r.lo;
-                stage[2 * (size_t)j + 1] = r.hi;
+            const unsigned m = __ballot_sync(0xffffffffu, surv);
+            if (surv) wq[wcount + (uint32_t)__popc(m & ((1u << lane) - 1u))] = j;
+            wcount += (uint32_t)__popc(m);
+            __syncwarp();
+            if (wcount >= 32u) {
+                stage_b(true, wq[lane], l0, l1, par);
+                const uint32_t mv = (lane + 32u < wcount) ? wq[lane + 32u] : 0u;
+                __syncwarp();
+                if (lane + 32u < wcount) wq[lane] = mv;
+                wcount -= 32u;
+                __syncwarp();
             }
         }
+        if (wcount) stage_b((uint32_t)lane < wcount, (uint32_t)lane < wcount ? wq[lane] : 0u, l0, l1, par);
+    };
+    auto phase2 = [&](int l0, int l1, int par) {
+        l1 = min(l1, pb);
+        const uint32_t np = min(s_npk[par], (uint32_t)kPeakQ);
+        for (uint32_t i = tid; i < np; i += kFThreads) {
+            const uint32_t j = s_pq[i];
+            int p; uint32_t jl, len;
+            locate(j, l0, l1, p, jl, len);
+            const uint32_t self = fetch(slot_of(p), j, jl);
+            moments(j, p, (int)(self & 0xffffu));
+        }
+        if (tid == 0) s_npk[par ^ 1] = 0u;
     };
 
     // prologue: lines needed by step 0
     build(pa - 2, pa + kS + 2);
     __syncthreads();
-    for (int l0 = pa; l0 < pb; l0 += kS) {
-        process(l0, l0 + kS);
+    int par = 0;
+    for (int l0 = pa; l0 < pb; l0 += kS, par ^= 1) {
+        phase1(l0, l0 + kS, par);
+        __syncthreads();
+        phase2(l0, l0 + kS, par);
         build(l0 + kS + 2, l0 + 2 * kS + 2);
         clear(l0 - kS - 2, l0 - 2);
         __syncthreads();
