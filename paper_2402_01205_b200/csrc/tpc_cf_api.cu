@@ -77,6 +77,7 @@ static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, ch
     w.ghist = (uint32_t*)take((size_t)tiles * 256 * 4);
     w.ghist_part = (uint32_t*)take((ceil_div_u64(tiles * 256, 1024) + 1) * 4);
     w.line_start = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
+    w.ovf = (uint32_t*)take((size_t)max_digits * 4);
     if (ws) *ws = w;
     if (n_sort_tiles) *n_sort_tiles = (uint32_t)tiles;
     if (map_bytes) *map_bytes = mapb;
@@ -170,7 +171,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
         if (r < 0) return r;
         k += r;
         k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, 0, st);
-        k += launch_finalize(h->ws, out->status, out->capacity, 3u, 1, st);
+        k += launch_finalize(h->ws, out->status, out->capacity, 3u, 1, n, st);
     } else {
         // T1: K1 scatter -> K2+K4 digit-centric peaks + moments on the HBM map -> K3 compaction -> (K5 key sort)
         //     -> K0 un-scatter
@@ -179,7 +180,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
         k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, hint ? 0 : 1, st);
         if (!hint) k += launch_key_sort(h->ws, h->max_clusters, h->n_sort_tiles, out->clusters, out->capacity, st);
         k += launch_unscatter(h->geo, h->ws, digits, n, st);
-        k += launch_finalize(h->ws, out->status, out->capacity, 1u, hint ? 1 : 0, st);
+        k += launch_finalize(h->ws, out->status, out->capacity, 1u, hint ? 1 : 0, n, st);
     }
     if (prof) { cudaEventRecord(ev[3], st); ++h->run_index; }
     e = cudaGetLastError();

@@ -262,12 +262,12 @@ int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_
 
 // ---- status ---------------------------------------------------------------------------------------------------
 __global__ void k_finalize(const Counters* cnt, tpc_cf_status* status, uint64_t capacity, uint32_t path,
-                           int hint_sorted)
+                           int hint_sorted, uint64_t n)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     tpc_cf_status s;
     s.n_clusters = cnt->n_clusters;
-    s.n_digits_used = cnt->n_used;
+    s.n_digits_used = n - cnt->n_bad;
     s.n_bad_digits = cnt->n_bad;
     s.overflow = s.n_clusters > capacity ? 1u : 0u;
     s.path = path;
@@ -280,9 +280,9 @@ __global__ void k_finalize(const Counters* cnt, tpc_cf_status* status, uint64_t 
 }
 
 int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,
-                    int hint_sorted, cudaStream_t st)
+                    int hint_sorted, uint64_t n, cudaStream_t st)
 {
-    k_finalize<<<1, 32, 0, st>>>(ws.counters, status, capacity, path, hint_sorted);
+    k_finalize<<<1, 32, 0, st>>>(ws.counters, status, capacity, path, hint_sorted, n);
     return 1;
 }
 

@@ -319,11 +319,6 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     if (tid == 0 && s_unsorted) atomicOr(&cnt->unsorted, 1u);
 }
 
-__global__ void k_set_used(Counters* cnt, uint64_t n)
-{
-    if (threadIdx.x == 0 && blockIdx.x == 0) cnt->n_used = n - cnt->n_bad;
-}
-
 int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1)
@@ -361,8 +356,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
                                                              ws.counters, ws.peakmask, (uint4*)ws.stage);
     if (ev_k1) cudaEventRecord(ev_k1, st);
     ++k;
-    k_set_used<<<1, 32, 0, st>>>(ws.counters, n);
-    return k + 1;
+    return k;
 }
 
 }  // namespace tpccf

@@ -23,12 +23,11 @@ __global__ void __launch_bounds__(kThreads)
 k_scatter(const uint2* __restrict__ digits, uint64_t n, Geo g, uint16_t* __restrict__ map, Counters* cnt)
 {
     const uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
-    bool bad = false, used = false, unsorted = false;
+    bool bad = false, unsorted = false;
     if (i < n) {
         const uint2 d = __ldg(digits + i);
         if (digit_valid(g, d.x, d.y)) {
             map[cell_offset(g, d.x, d.y)] = (uint16_t)(d.y >> 16);
-            used = true;
         } else {
             bad = true;
         }
@@ -37,12 +36,12 @@ k_scatter(const uint2* __restrict__ digits, uint64_t n, Geo g, uint16_t* __restr
             unsorted = key40(e.x, e.y) > key40(d.x, d.y);
         }
     }
+    // bad digits and order violations are rare: one atomic per warp that saw any (n_used = n - n_bad at the end;
+    // a per-warp atomic on one counter for every warp would serialise in L2)
     const unsigned mb = __ballot_sync(0xffffffffu, bad);
-    const unsigned mu = __ballot_sync(0xffffffffu, used);
     const unsigned ms = __ballot_sync(0xffffffffu, unsorted);
     if ((threadIdx.x & 31) == 0) {
         if (mb) atomicAdd(&cnt->n_bad, (unsigned long long)__popc(mb));
-        if (mu) atomicAdd(&cnt->n_used, (unsigned long long)__popc(mu));
         if (ms) atomicOr(&cnt->unsorted, 1u);
     }
 }

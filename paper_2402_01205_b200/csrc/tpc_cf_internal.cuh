@@ -26,7 +26,7 @@ struct Counters {
     unsigned long long n_used;
     unsigned long long n_clusters;  // total peaks
     unsigned int unsorted;          // 1 if digits[i-1] > digits[i] for some i (key = sector,row,pad,time)
-    unsigned int rsv;
+    unsigned int n_ovf;             // fused path: peaks routed to the exact slow path (k_fused_overflow)
 };
 
 // Pointers into the caller-owned workspace.
@@ -44,6 +44,7 @@ struct Workspace {
     uint32_t* ghist;      // [256][n_sort_tiles]
     uint32_t* ghist_part;
     uint32_t* line_start; // [n_planes*LS + 1] first digit of each (plane,pad) line (fused path)
+    uint32_t* ovf;        // [max_digits] digit indices of peaks handled by k_fused_overflow
 };
 
 struct Handle;
@@ -132,7 +133,7 @@ int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t c
 int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_tiles, tpc_cluster* out,
                     uint64_t capacity, cudaStream_t st);
 int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,
-                    int hint_sorted, cudaStream_t st);
+                    int hint_sorted, uint64_t n, cudaStream_t st);
 
 // exclusive scan of n uint32 (in -> out, may alias); total (optional) receives the sum as 64-bit.
 int launch_scan_u32(const uint32_t* in, uint32_t* out, uint64_t n, uint32_t* partials,

@@ -1,0 +1,196 @@
+"""-m "not gpu" tests of the boundary and the host logic: the C-ABI library loads and exports every symbol that
+include/tpc_cf.h declares, workspace sizing, synchronous argument errors that need no device, the seeded generator's
+contract (sorted, deterministic for any thread count, occupancies of BASELINE.json:configs), and the replica
+sharding used for N > 1 under a world-size-2 gloo group.  No compute call is made here.
+"""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "tpc_cf.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(tpc_cf_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    import paper_2402_01205_b200 as cf
+    lib = cf.load()
+    syms = declared_symbols()
+    assert "tpc_cf_create" in syms and "tpc_cf_run" in syms and "tpc_cf_destroy" in syms
+    for s in syms:
+        assert hasattr(lib, s), "libtpc_cf.so does not export %s" % s
+    assert sorted(cf.EXPORTS) == syms, "binding.EXPORTS and include/tpc_cf.h disagree"
+
+
+def test_library_is_sm100a_and_uses_no_fallback():
+    import paper_2402_01205_b200 as cf
+    from paper_2402_01205_b200 import build
+    cf.load()
+    out = subprocess.run(["cuobjdump", "-lelf", build.SO], capture_output=True, text=True)
+    if out.returncode == 0:
+        assert "sm_100a" in out.stdout, out.stdout
+    src = open(os.path.join(ROOT, "paper_2402_01205_b200", "binding.py")).read()
+    assert "oracle" not in src.replace("oracle/", ""), "the product binding must not reference the oracle"
+
+
+def test_struct_layouts_match_header():
+    import paper_2402_01205_b200 as cf
+    assert cf.DIGIT.itemsize == 8 and cf.CLUSTER.itemsize == 32 and cf.STATUS.itemsize == 32
+    assert cf.CLUSTER.fields["qtot"][1] == 8 and cf.CLUSTER.fields["pad_mean"][1] == 12
+    assert ctypes.sizeof(cf.Geometry) == 24 and ctypes.sizeof(cf.Params) == 8 and ctypes.sizeof(cf.Out) == 32
+
+
+def test_workspace_bytes_and_geometry_limits():
+    import paper_2402_01205_b200 as cf
+    g, _ = cf.make_geometry(36, 152, 138, 14336)
+    full = cf.tpc_cf_workspace_bytes(g, 220_000_000, 14_000_000)
+    # dense uint16 map with a 2-cell border dominates: 36*152 planes x 142 x 14344 cells
+    map_bytes = 36 * 152 * 142 * 14344 * 2
+    assert full > map_bytes and full < map_bytes + 220_000_000 * 40 + 14_000_000 * 64 + (1 << 26)
+    small = cf.tpc_cf_workspace_bytes(g, 1000, 100)
+    assert map_bytes < small < full
+    for bad in ((0, 152, 138, 14336), (36, 0, 138, 14336), (36, 152, 256, 14336), (36, 152, 138, 65536),
+                (257, 152, 138, 14336)):
+        gb, _ = cf.make_geometry(*bad)
+        assert cf.tpc_cf_workspace_bytes(gb, 1000, 100) == 0
+    gn, keep = cf.make_geometry(1, 3, 16, 64, npads=[10, 17, 16])       # 17 > max_pads
+    assert cf.tpc_cf_workspace_bytes(gn, 10, 10) == 0
+    assert cf.tpc_cf_workspace_bytes(g, 1 << 32, 10) == 0                # capacities must stay below 2^32
+
+
+def test_synchronous_errors_without_a_device():
+    import paper_2402_01205_b200 as cf
+    lib = cf.load()
+    g, _ = cf.make_geometry(1, 2, 8, 16)
+    h = ctypes.c_void_p()
+    assert lib.tpc_cf_create(ctypes.byref(h), ctypes.byref(g), 10, 10, None, 0, None) == -1          # E_NULL
+    buf = ctypes.create_string_buffer(1 << 16)
+    addr = (ctypes.addressof(buf) + 255) & ~255
+    assert lib.tpc_cf_create(ctypes.byref(h), ctypes.byref(g), 10, 10, addr + 8, 1 << 15, None) == -4  # misaligned
+    assert lib.tpc_cf_create(ctypes.byref(h), ctypes.byref(g), 10, 10, addr, 64, None) == -4           # too small
+    gb, _ = cf.make_geometry(0, 2, 8, 16)
+    assert lib.tpc_cf_create(ctypes.byref(h), ctypes.byref(gb), 10, 10, addr, 1 << 15, None) == -2     # E_GEOMETRY
+    assert lib.tpc_cf_run(None, None, 0, ctypes.byref(g), None, None) == -1
+    assert lib.tpc_cf_destroy(None) == -1
+    for code in range(-7, 1):
+        assert lib.tpc_cf_strerror(code)
+    assert b"unknown" in lib.tpc_cf_strerror(-99)
+
+
+def test_product_fails_loudly_without_cuda():
+    import torch
+    import paper_2402_01205_b200 as cf
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        cf.ClusterFinder(1, 2, 8, 16, max_digits=16)
+
+
+# ---- generator ---------------------------------------------------------------------------------------------------
+
+def digit_keys(d):
+    return ((d["sector"].astype(np.uint64) << 32) | (d["row"].astype(np.uint64) << 24) |
+            (d["pad"].astype(np.uint64) << 16) | d["time"].astype(np.uint64))
+
+
+def test_generator_contract_config1():
+    from datagen import gen
+    d1 = gen.generate(1, n_threads=1)
+    d4 = gen.generate(1, n_threads=4)
+    assert np.array_equal(d1, d4), "output depends on the thread count"
+    k = digit_keys(d1)
+    assert np.all(k[1:] > k[:-1]), "digits not strictly ascending in (sector,row,pad,time) / duplicate cells"
+    assert d1["charge"].min() >= 2 and d1["time"].max() < 512 and d1["pad"].max() < 138 and d1["row"].max() < 152
+    assert 0.004 < gen.occupancy(d1, 1) < 0.008                       # config 1 comes out ~0.57 %
+    assert gen.checksum(d1) == gen.checksum(d4)
+    part = gen.generate(dict(gen.CONFIGS[3], n_sectors=36), sectors=(5, 6))
+    assert part["sector"].min() == 5 and part["sector"].max() == 5
+
+
+@pytest.mark.parametrize("cfg,lo,hi", [(2, 0.045, 0.055), (3, 0.018, 0.022), (4, 0.09, 0.11), (5, 0.0045, 0.0055)])
+def test_generator_occupancies(cfg, lo, hi):
+    """±10 % of the occupancies BASELINE.json:configs states, measured on one sector."""
+    from datagen import gen
+    c = dict(gen.CONFIGS[cfg], n_sectors=1)
+    d = gen.generate(c)
+    assert lo < gen.occupancy(d, c) < hi
+    k = digit_keys(d)
+    assert np.all(k[1:] > k[:-1])
+    if cfg == 5:
+        npads = gen.geometry(c)[4]
+        assert npads[0] == 66 and npads[-1] == 138 and int(npads.sum()) == 15429
+        assert np.all(d["pad"] < npads[d["row"]])
+
+
+def test_generator_plateaus_yield_one_peak_each():
+    """config 4 injects rectangular flat tops (R1b): the oracle must find exactly one peak per plateau cell set,
+    at its (min pad, min time) corner — checked on the plateau cells that are still flat in the output."""
+    from datagen import gen
+    from oracle import oracle as orc
+    c = dict(gen.CONFIGS[4], n_sectors=1, n_rows=4)
+    d = gen.generate(c)
+    cl, st = orc.run(d, 1, 4, 138, 14336)
+    assert st["n_clusters"] > 1000
+    # a peak's later neighbour in time never exceeds it, and equal-charge horizontal runs start at the peak
+    peaks = {(int(x["row"]), int(x["pad"]), int(x["time"])): int(x["qmax"]) for x in cl}
+    cells = {(int(x["row"]), int(x["pad"]), int(x["time"])): int(x["charge"]) for x in d[d["row"] == 0]}
+    flat_pairs = 0
+    for (r, p, t), q in cells.items():
+        if q >= 30 and cells.get((r, p, t + 1)) == q:
+            flat_pairs += 1
+            assert (r, p, t + 1) not in peaks, "second cell of a flat run must not be a peak"
+    assert flat_pairs > 0
+
+
+# ---- N > 1: replicas only ------------------------------------------------------------------------
+
+_GLOO_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %(root)r)
+import numpy as np
+import torch, torch.distributed as dist
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%(port)d", rank=int(sys.argv[1]), world_size=2)
+rank = dist.get_rank()
+from datagen import gen
+from oracle import oracle as orc
+cfg = dict(gen.CONFIGS[1])
+# replicas: rank r owns frame r; value = sum of units / max of times, exactly as bench.py aggregates
+d = gen.generate(cfg, frame=rank)
+cl, st = orc.run(d, *gen.geometry(cfg)[:4])
+t = torch.tensor([10.0 + rank], dtype=torch.float64)
+dist.all_reduce(t, op=dist.ReduceOp.MAX)
+c = torch.tensor([float(d.shape[0]), float(st["n_clusters"])], dtype=torch.float64)
+dist.all_reduce(c, op=dist.ReduceOp.SUM)
+if rank == 0:
+    print(json.dumps({"tmax": t.item(), "digits": c[0].item(), "clusters": c[1].item(), "own": int(d.shape[0])}))
+dist.barrier()
+dist.destroy_process_group()
+"""
+
+
+def test_replica_sharding_world_size_2_gloo(tmp_path):
+    """Frames go round-robin to ranks with no data-path collective; the only collectives are the
+    timing MAX and the unit SUM that bench.py uses.  Run with the gloo backend on CPU, world size 2."""
+    from datagen import gen
+    port = 29500 + (os.getpid() % 2000)
+    script = tmp_path / "worker.py"
+    script.write_text(_GLOO_WORKER % {"root": ROOT, "port": port})
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE, stderr=subprocess.PIPE,
+                              text=True) for r in range(2)]
+    outs = [p.communicate(timeout=300) for p in procs]
+    for p, (o, e) in zip(procs, outs):
+        assert p.returncode == 0, e[-2000:]
+    import json
+    res = json.loads(outs[0][0].strip().splitlines()[-1])
+    n0 = gen.generate(1, frame=0).shape[0]
+    n1 = gen.generate(1, frame=1).shape[0]
+    assert res["tmax"] == 11.0 and res["digits"] == n0 + n1 and res["own"] == n0 and n0 != n1

@@ -279,3 +279,26 @@ def test_full_frame_sampled_planes():
     assert st2["path"] == 1 and st2["n_clusters"] == st["n_clusters"]
     assert np.array_equal(cl2.view(np.uint8), cl.view(np.uint8)), "general and fused path differ on config 3"
     f.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_dense_isolated_peaks_overflow_the_peak_queue(path):
+    """Degenerate density: a checkerboard-like pattern where every digit is a peak (2048 peaks per pad line) — far
+    more than the fused kernel's per-step shared-memory peak queue holds, so its exact slow path is exercised;
+    lines longer than the tq capacity of a slot are exercised too (a fully occupied row)."""
+    rng = np.random.default_rng(5)
+    geom = (1, 3, 12, 4096, None)
+    d = []
+    for pad in range(0, 12, 2):
+        for t in range(pad % 4, 4096, 2):
+            d.append((0, 1, pad, 0, t, int(rng.integers(4, 500))))
+    for pad in range(12):                      # a fully occupied row: every cell holds charge
+        for t in range(0, 4096):
+            d.append((0, 2, pad, 0, t, int(rng.integers(1, 60))))
+    d.append((0, 0, 3, 0, 7, 9))
+    digits = sort_digits(np.array(d, dtype=orc.DIGIT))
+    ora, ost = orc.run(digits, *geom[:4])
+    assert ost["n_clusters"] > 12000
+    cl, st = gpu_run(digits, geom, PATHS[path])
+    assert st["n_clusters"] == ost["n_clusters"]
+    assert_clusters_equal(cl, ora, "dense isolated peaks/" + path)
