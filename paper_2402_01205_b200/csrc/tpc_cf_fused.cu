@@ -1,15 +1,19 @@
 // tpc_cf_fused.cu — fused path ("T3") for digits sorted by (sector,row,pad,time): the charge map never exists in HBM.
 //
 //   k_line_index   lower_bound of every (plane,pad) line in the digit array -> ws.line_start
-//   k_fused_lines  one CTA per (plane, pad range).  The pad lines of the range stream through a ring of line slots in
-//                  shared memory.  A line slot is the line of the charge map in compressed form:
-//                     bm[w]   presence bitmap over time bins (bit t+32; one guard word each side = zero border, R2)
+//   k_fused_lines  one CTA (8 warps) per (plane, pad range).  The pad lines of the range stream through a ring of line
+//                  slots in shared memory.  A line slot is one line of the charge map in compressed form:
+//                     bm[w]   presence bitmap over time bins (bit t+32; guard words = zero border in time, R2)
 //                     pre[w]  index within the line of the first digit of bitmap word w (rank directory)
 //                     tq[i]   (time | charge << 16) of the i-th digit of the line = upper word of the input record
-//                  K1 (scatter) = building a slot from the line's digits, K2 = digit-centric 3x3 test against the
-//                  slots of lines p-1, p, p+1, K4 = 5x5 window gathered from the five slots p-2..p+2, K0 = clearing
-//                  the bitmap of the slot that leaves the ring.  Per step: S lines are processed, the next S lines
-//                  are built and the S lines retired one step earlier are cleared, with ONE __syncthreads.
+//                  One WARP owns one LINE at a time, so line geometry and slot pointers are warp-uniform:
+//                   K1 build    the warp zeroes its slot's bitmap, then streams the line's digits into bm/pre/tq
+//                               (this is also K0: a slot is cleaned by the warp that reuses it)
+//                   K2 stage A  own-line test of every digit against the adjacent digits of the line (shuffles)
+//                      stage B  survivors (~25 %) against lines p-1 / p+1 through 3-bit bitmap windows
+//                   K4 stage C  peaks (~5 %) gathered into a CTA queue; 5x5 window from the five slots p-2..p+2,
+//                               gated sums, record -> stage[j]
+//                  Step = 8 lines: [A+B on lines l0..l0+7] barrier [C for their peaks | build lines l0+10..l0+17] barrier.
 //                  Peaks are recorded as one bit per digit (peakmask) and their cluster at stage[j]; the shared
 //                  compaction (tpc_cf_compact.cu) turns that into the ordered output (K3, K5).
 //   The DIGITS_SORTED promise is verified here for free: every digit is checked once against the line (or gap) it
@@ -19,9 +23,10 @@
 namespace tpccf {
 
 static constexpr int kFThreads = 256;
-static constexpr int kS = 2;                    // lines per step
-static constexpr int kSlots = 3 * kS + 4;       // process window S+4, build S, clear S
-static constexpr int kPeakQ = 512;              // CTA peak queue entries per step
+static constexpr int kWarps = kFThreads / 32;
+static constexpr int kS = kWarps;               // lines per step: one per warp
+static constexpr int kSlots = 2 * kS + 4;       // lines l0-2 .. l0+S+1 in use, next S being built
+static constexpr int kPeakQ = 1024;             // CTA peak queue entries per step
 
 __device__ __forceinline__ uint32_t key24_of(uint32_t w0)
 {
@@ -46,49 +51,61 @@ k_line_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __re
     line_start[e] = lo;
 }
 
-struct SlotView {
-    uint32_t* bm;
-    uint32_t* tq;
-    uint16_t* pre;
+// Slot layout (warp-uniform).
+struct Ring {
+    uint32_t* sm;          // base of the dynamic shared memory
+    uint32_t slot_words;   // words per slot (multiple of 4)
+    uint32_t wpl;          // bitmap words per line (multiple of 4)
+    uint32_t cap;          // tq entries per slot (lines longer than this read the tail from global memory)
+    __device__ __forceinline__ uint32_t* slot(int v) const { return sm + (uint32_t)v * slot_words; }
 };
 
-// charges of the window t-H..t+H of one line slot (0 where no digit), c[k] for time t-H+k
-template <int H>
-__device__ __forceinline__ void window(const SlotView& sv, uint32_t cap, const uint2* __restrict__ digits,
-                                       uint32_t lbeg, uint32_t n, int t, int (&c)[2 * H + 1])
+// ring index of the line at distance d (|d| < kSlots) from the line whose ring index is v0
+__device__ __forceinline__ int ring_at(int v0, int d)
 {
+    int v = v0 + d;
+    v += (v < 0) ? kSlots : 0;
+    v -= (v >= kSlots) ? kSlots : 0;
+    return v;
+}
+
+// charges of the window t-H..t+H of one line slot (0 where no digit): c[k] is time t-H+k.  Branch-free except for the
+// rare tail of a line longer than cap, read from the digit array (gl = global index of the line's first digit).
+template <int H>
+__device__ __forceinline__ void window(const Ring& rg, const uint32_t* __restrict__ slot,
+                                       const uint2* __restrict__ digits, uint32_t gl, uint32_t n, int t,
+                                       int (&c)[2 * H + 1])
+{
+    const uint32_t* tq = slot + rg.wpl;
+    const uint16_t* pre = reinterpret_cast<const uint16_t*>(slot + rg.wpl + rg.cap);
     const int b = t + 32 - H;
     const int w = b >> 5, s = b & 31;
-    const uint32_t lo = sv.bm[w], hi = sv.bm[w + 1];
-    uint32_t bits = __funnelshift_r(lo, hi, s) & ((1u << (2 * H + 1)) - 1u);
-#pragma unroll
-    for (int k = 0; k < 2 * H + 1; ++k) c[k] = 0;
-    if (!bits) return;
-    uint32_t idx = (lo >> s) ? (uint32_t)sv.pre[w] + (uint32_t)__popc(lo & ((1u << s) - 1u)) : (uint32_t)sv.pre[w + 1];
+    const uint32_t lo = slot[w], hi = slot[w + 1];
+    const uint32_t bits = __funnelshift_r(lo, hi, s) & ((1u << (2 * H + 1)) - 1u);
+    const uint32_t p0 = pre[w], p1 = pre[w + 1];
+    const uint32_t idx = (lo >> s) ? p0 + (uint32_t)__popc(lo & ((1u << s) - 1u)) : p1;
 #pragma unroll
     for (int k = 0; k < 2 * H + 1; ++k) {
-        if (bits & (1u << k)) {
-            uint32_t v;
-            if (idx < cap) v = sv.tq[idx];
-            else { uint32_t gi = lbeg + idx; gi = gi < n ? gi : n - 1; v = __ldg(&digits[gi].y); }
-            c[k] = (int)(v >> 16);
-            ++idx;
-        }
+        const uint32_t ik = idx + (uint32_t)__popc(bits & ((1u << k) - 1u));
+        uint32_t v = tq[min(ik, rg.cap - 1u)];
+        const bool present = (bits >> k) & 1u;
+        if (present && ik >= rg.cap) v = __ldg(&digits[min(gl + ik, n - 1u)].y);
+        c[k] = present ? (int)(v >> 16) : 0;
     }
 }
 
-__global__ void __launch_bounds__(kFThreads, 4)
+__global__ void __launch_bounds__(kFThreads, 2)
 k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
               uint32_t pads_per_unit, uint32_t units_per_plane, uint32_t wpl, uint32_t cap,
               uint32_t q_peak_min, uint32_t q_gate, Counters* cnt, uint32_t* __restrict__ peakmask,
               uint4* __restrict__ stage)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ uint32_t s_ls[260];       // line starts of this plane: s_ls[p] for p = 0..max_pads, then next plane's start
+    __shared__ uint32_t s_ls[260];          // line starts of this plane: s_ls[p], p = 0..max_pads, then next plane's start
+    __shared__ uint32_t s_wq[kWarps][64];   // per-warp survivor queues (stage A -> B): index within the warp's line
+    __shared__ uint32_t s_pq[kPeakQ];       // CTA peak queue (stage B -> C): (line - l0) << 16 | index within the line
+    __shared__ uint32_t s_npk[2];           // its fill count, double-buffered by step parity
     __shared__ int s_unsorted;
-    __shared__ uint32_t s_wq[kFThreads / 32][64];   // per-warp survivor queues (stage A -> B)
-    __shared__ uint32_t s_pq[kPeakQ];               // CTA peak queue (stage B -> C)
-    __shared__ uint32_t s_npk[2];                   // its fill count, double-buffered by step parity
 
     const uint32_t plane = blockIdx.x / units_per_plane, unit = blockIdx.x % units_per_plane;
     const uint32_t sector = plane / g.n_rows, row = plane % g.n_rows;
@@ -99,20 +116,18 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t w0_base = sector | (row << 8);
 
-    // slot views
-    const uint32_t slot_words = wpl + cap + ((wpl + 1) >> 1);
-    uint32_t* sm = reinterpret_cast<uint32_t*>(smem_raw);
-    auto slot_of = [&](int p) -> SlotView {
-        const int v = (p - pa + 2 + kSlots) % kSlots;     // p >= pa - 2 - kSlots always
-        uint32_t* base = sm + (uint32_t)v * slot_words;
-        SlotView sv;
-        sv.bm = base; sv.tq = base + wpl; sv.pre = reinterpret_cast<uint16_t*>(base + wpl + cap);
-        return sv;
-    };
+    Ring rg;
+    rg.sm = reinterpret_cast<uint32_t*>(smem_raw);
+    rg.wpl = wpl; rg.cap = cap;
+    rg.slot_words = wpl + cap + (((wpl >> 1) + 3u) & ~3u);
 
     for (int i = tid; i <= (int)g.LS; i += kFThreads) s_ls[i] = line_start[plane * g.LS + i];
     if (tid == 0) { s_unsorted = 0; s_npk[0] = 0u; s_npk[1] = 0u; }
-    for (uint32_t i = tid; i < kSlots * slot_words; i += kFThreads) sm[i] = 0u;
+    {   // every slot starts as an empty line (lines outside the plane keep this state: zero border in pad, R2)
+        uint4* z = reinterpret_cast<uint4*>(rg.sm);
+        const uint32_t nz = (kSlots * rg.slot_words) >> 2;
+        for (uint32_t i = tid; i < nz; i += kFThreads) z[i] = make_uint4(0, 0, 0, 0);
+    }
     __syncthreads();
 
     if (pa >= P && unit != 0) return;    // nothing in this pad range (rows with fewer pads)
@@ -137,149 +152,150 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         }
     }
 
-    // ---- K1: build the slots of lines [b0,b1) (clipped to existing lines) ---------------------------------------
-    auto build = [&](int b0, int b1) {
-        b0 = max(b0, 0); b1 = min(b1, min(P, pb + 2));
-        if (b0 >= b1) return;
-        const uint32_t jb = s_ls[b0], je = s_ls[b1];
-        if (je <= jb) return;
-        for (uint32_t j0 = jb; j0 < je; j0 += kFThreads) {      // uniform trip count: the shuffles need whole warps
-            const uint32_t j = j0 + tid;
-            const bool act = j < je;
-            uint2 d = make_uint2(0, 0);
-            if (act) d = __ldg(digits + j);
-            // previous digit (lane-1, or a load for lane 0 / first of the range)
-            uint32_t pw0 = __shfl_up_sync(0xffffffffu, d.x, 1), pw1 = __shfl_up_sync(0xffffffffu, d.y, 1);
-            if (act && lane == 0 && j > jb) { const uint2 e = __ldg(digits + j - 1); pw0 = e.x; pw1 = e.y; }
-            if (!act) continue;
-            const int p = (int)((d.x >> 16) & 0xffu);
-            const uint32_t t = d.y & 0xffffu;
-            const bool owner = p >= pa && p < pb;
-            if ((d.x & 0xffffu) != w0_base || p < b0 || p >= b1) { bad_order = true; continue; }
-            const uint32_t lbeg = s_ls[p];
-            if (j < lbeg || j >= s_ls[p + 1]) { bad_order = true; continue; }
-            const uint32_t jl = j - lbeg;
-            const bool first_of_line = (jl == 0);
-            const uint32_t pt = pw1 & 0xffffu;
-            if (!first_of_line && pt >= t) bad_order = true;          // not strictly ascending (or a duplicate cell)
-            if (t >= (uint32_t)T || (d.y >> 16) == 0u) { if (owner) atomicAdd(&cnt->n_bad, 1ull); }
-            if (t >= (uint32_t)T) continue;
-            const SlotView sv = slot_of(p);
-            const uint32_t bw = (t + 32u) >> 5;
-            atomicOr(&sv.bm[bw], 1u << (t & 31u));
-            if (first_of_line || ((pt + 32u) >> 5) != bw) sv.pre[bw] = (uint16_t)jl;
-            if (jl < cap) sv.tq[jl] = d.y;
+    const int blo = max(pa - 2, 0), bhi = min(P, pb + 2);   // lines this unit ever builds
+
+    // tq entry jl of line p (slot given); the tail beyond cap comes from the digit array
+    auto fetch = [&](const uint32_t* slot, uint32_t gl, uint32_t jl) -> uint32_t {
+        if (jl < rg.cap) return slot[rg.wpl + jl];
+        return __ldg(&digits[min(gl + jl, n - 1u)].y);
+    };
+
+    // ---- prefetch for K1: the (time|charge) words of line p go straight into the tq area of slot v with cp.async ----
+    // (issued at the top of a step by the warp that builds the line after the step's first barrier)
+    auto prefetch_line = [&](int p, int v) {
+        if (p < blo || p >= bhi) return;
+        const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
+        const uint32_t m = min(len, rg.cap);
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(rg.slot(v) + rg.wpl);
+        for (uint32_t jl = lane; jl < m; jl += 32)
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + 4u * jl), "l"(&digits[lbeg + jl].y) : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    // ---- K0 + K1: this warp (re)builds the slot v of line p from the line's digits -----------------------------------
+    // staged: the tq words [0, min(len,cap)) were already copied by prefetch_line.
+    auto build_line = [&](int p, int v, bool staged) {
+        uint32_t* slot = rg.slot(v);
+        {
+            uint4* z = reinterpret_cast<uint4*>(slot);
+            for (uint32_t x = lane; x < (rg.wpl >> 2); x += 32) z[x] = make_uint4(0, 0, 0, 0);
+        }
+        if (staged) asm volatile("cp.async.wait_all;" ::: "memory");
+        __syncwarp();
+        if (p < blo || p >= bhi) return;                    // a line outside the plane / the halo: stays empty
+        const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
+        uint16_t* pre = reinterpret_cast<uint16_t*>(slot + rg.wpl + rg.cap);
+        const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
+        const bool owner = p >= pa && p < pb;
+        uint32_t carry = 0;                                 // tq word of the digit before this chunk
+        uint32_t xn = lane < len ? __ldg(&digits[lbeg + lane].x) : 0u;   // key words, loaded one chunk ahead
+        for (uint32_t c0 = 0; c0 < len; c0 += 32) {
+            const uint32_t jl = c0 + lane;
+            const bool act = jl < len;
+            const uint32_t dx = xn;
+            if (jl + 32 < len) xn = __ldg(&digits[lbeg + jl + 32].x);
+            uint32_t dy = 0u;
+            if (act) {
+                if (staged && jl < rg.cap) dy = slot[rg.wpl + jl];
+                else { dy = __ldg(&digits[lbeg + jl].y); if (jl < rg.cap) slot[rg.wpl + jl] = dy; }
+            }
+            uint32_t prevy = __shfl_up_sync(0xffffffffu, dy, 1);
+            if (lane == 0) prevy = carry;
+            carry = __shfl_sync(0xffffffffu, dy, 31);
+            const uint32_t t = dy & 0xffffu, pt = prevy & 0xffffu;
+            const bool first = (jl == 0);
+            const bool ok = act && (dx & 0x00ffffffu) == w0_line;
+            if (act && (!ok || (!first && pt >= t))) bad_order = true;   // wrong line, not ascending, or duplicate cell
+            const bool badd = ok && owner && (t >= (uint32_t)T || (dy >> 16) == 0u);
+            if (__any_sync(0xffffffffu, badd)) {
+                const unsigned mbad = __ballot_sync(0xffffffffu, badd);
+                if (lane == 0) atomicAdd(&cnt->n_bad, (unsigned long long)__popc(mbad));
+            }
+            if (ok && t < (uint32_t)T) {
+                const uint32_t bw = (t + 32u) >> 5;
+                atomicOr(&slot[bw], 1u << (t & 31u));
+                if (first || ((pt + 32u) >> 5) != bw) pre[bw] = (uint16_t)jl;
+            }
         }
     };
 
-    // ---- K0: clear the bitmaps of lines [c0,c1) ------------------------------------------------------------------
-    auto clear = [&](int c0, int c1) {
-        for (int p = c0; p < c1; ++p) {
-            if (p < pa - 2) continue;
-            const SlotView sv = slot_of(p);
-            for (uint32_t i = tid; i < wpl; i += kFThreads) sv.bm[i] = 0u;
-        }
-    };
-
-    // ---- K2 + K4: digit-centric peak test and moments for lines [l0,l1) -------------------------------------------
-    // Peaks are ~1 in 20 digits, so the work is done in three dense stages instead of one divergent pass:
-    //   A (every digit)     own-line test against the adjacent digits of the line; survivors -> per-warp queue
-    //   B (survivors, ~25%) lines p-1 / p+1 through the bitmap windows; peaks -> CTA queue + peakmask bit
-    //   C (peaks, ~5%)      5x5 window from the five slots, gated sums, record -> stage[j]   (after a barrier)
-    auto locate = [&](uint32_t j, int l0, int l1, int& p, uint32_t& jl, uint32_t& len) {
-        p = l0;
-#pragma unroll
-        for (int i = 1; i < kS; ++i) if (l0 + i < l1 && j >= s_ls[l0 + i]) p = l0 + i;
-        const uint32_t lbeg = s_ls[p];
-        jl = j - lbeg;
-        len = s_ls[p + 1] - lbeg;
-    };
-    auto fetch = [&](const SlotView& sv, uint32_t j, uint32_t jl) -> uint32_t {
-        if (jl < cap) return sv.tq[jl];
-        return __ldg(&digits[min(j, n - 1)].y);
-    };
-    auto moments = [&](uint32_t j, int p, int t) {
+    // ---- K4 (stage C): 5x5 window from the slots of lines p-2..p+2, gated sums, record -> stage[j] ----------------
+    // vp = ring index of line p.  Slots of lines outside the plane are empty (R2).
+    auto moments = [&](int p, uint32_t jl, int vp) {
+        const uint32_t gl = s_ls[p];
+        const uint32_t self = fetch(rg.slot(vp), gl, jl);
+        const int t = (int)(self & 0xffffu);
         int c[5][5];
 #pragma unroll
-        for (int a = 0; a < 5; ++a) {
-            const int pp = p + a - 2;
-            if (pp >= 0 && pp < P) {
-                window<2>(slot_of(pp), cap, digits, s_ls[pp], n, t, c[a]);
-            } else {
-#pragma unroll
-                for (int b = 0; b < 5; ++b) c[a][b] = 0;
-            }
-        }
+        for (int a = 0; a < 5; ++a)
+            window<2>(rg, rg.slot(ring_at(vp, a - 2)), digits, s_ls[min(max(p + a - 2, 0), P)], n, t, c[a]);
         const ClusterWords r = cluster_from_window(c, w0_base | ((uint32_t)p << 16), (uint32_t)t, q_gate);
-        stage[2 * (size_t)j] = r.lo;
-        stage[2 * (size_t)j + 1] = r.hi;
+        const size_t j = (size_t)gl + jl;
+        stage[2 * j] = r.lo;
+        stage[2 * j + 1] = r.hi;
     };
-    auto stage_b = [&](bool act, uint32_t j, int l0, int l1, int par) {
-        bool peak = false;
-        int p = l0, t = 0;
-        if (act) {
-            uint32_t jl, len;
-            locate(j, l0, l1, p, jl, len);
-            const uint32_t self = fetch(slot_of(p), j, jl);
-            t = (int)(self & 0xffffu);
-            const uint32_t q = self >> 16;
-            peak = true;
-            if (p > 0) {                                                    // line p-1: earlier, strict (R1)
-                int c[3];
-                window<1>(slot_of(p - 1), cap, digits, s_ls[p - 1], n, t, c);
-                peak = q > (uint32_t)c[0] && q > (uint32_t)c[1] && q > (uint32_t)c[2];
-            }
-            if (peak && p + 1 < P) {                                        // line p+1: later, >=
-                int c[3];
-                window<1>(slot_of(p + 1), cap, digits, s_ls[p + 1], n, t, c);
-                peak = q >= (uint32_t)c[0] && q >= (uint32_t)c[1] && q >= (uint32_t)c[2];
-            }
-        }
-        const unsigned pm = __ballot_sync(0xffffffffu, peak);
-        if (pm == 0) return;
-        const int leader = __ffs(pm) - 1;
-        uint32_t base = 0;
-        if (lane == leader) base = atomicAdd(&s_npk[par], (uint32_t)__popc(pm));
-        base = __shfl_sync(0xffffffffu, base, leader);
-        if (peak) {
-            atomicOr(&peakmask[j >> 5], 1u << (j & 31u));
-            const uint32_t slot = base + (uint32_t)__popc(pm & ((1u << lane) - 1u));
-            if (slot < kPeakQ) s_pq[slot] = j;
-            else moments(j, p, t);                                          // queue full: do it here (rare)
-        }
-    };
-    auto phase1 = [&](int l0, int l1, int par) {
-        l1 = min(l1, pb);
-        if (l0 >= l1) return;
-        const uint32_t jb = s_ls[l0], je = s_ls[l1];
-        if (je <= jb) return;
+
+    // ---- K2: stages A and B for line p (ring index vp), owned by this warp; lo = p - l0 ------------------------------
+    auto stage_ab = [&](int p, int vp, int lo, int par) {
+        const uint32_t gl = s_ls[p], len = s_ls[p + 1] - gl;
+        if (len == 0) return;
+        const uint32_t* sp = rg.slot(vp);
+        const uint32_t* sm1 = rg.slot(ring_at(vp, -1));
+        const uint32_t* sp1 = rg.slot(ring_at(vp, 1));
+        const uint32_t glm = s_ls[max(p - 1, 0)], glp = s_ls[min(p + 1, P)];
         uint32_t* wq = s_wq[warp];
-        uint32_t wcount = 0;                                                // warp-uniform
-        for (uint32_t j0 = (jb & ~31u) + 32u * warp; j0 < je; j0 += kFThreads) {
-            const uint32_t j = j0 + lane;
-            bool surv = false;
-            if (j >= jb && j < je) {
-                int p; uint32_t jl, len;
-                locate(j, l0, l1, p, jl, len);
-                const SlotView sv = slot_of(p);
-                const uint32_t self = fetch(sv, j, jl);
-                const int t = (int)(self & 0xffffu);
+
+        auto stage_b = [&](bool act, uint32_t jl) {
+            bool peak = false;
+            int t = 0;
+            if (act) {
+                const uint32_t self = fetch(sp, gl, jl);
+                t = (int)(self & 0xffffu);
                 const uint32_t q = self >> 16;
-                if (q >= q_peak_min && t < T) {
-                    // own line: the neighbours in time are the adjacent digits of the line
-                    const uint32_t prev = jl > 0 ? fetch(sv, j - 1, jl - 1) : 0u;
-                    const uint32_t next = jl + 1 < len ? fetch(sv, j + 1, jl + 1) : 0u;
-                    const uint32_t qm = (jl > 0 && (int)(prev & 0xffffu) == t - 1) ? (prev >> 16) : 0u;
-                    const uint32_t qp = (jl + 1 < len && (int)(next & 0xffffu) == t + 1 && t + 1 < T) ? (next >> 16) : 0u;
-                    surv = q > qm && q >= qp;                               // R1: (0,-1) strict, (0,+1) >=
-                }
+                int cm[3], cp[3];
+                window<1>(rg, sm1, digits, glm, n, t, cm);      // line p-1: earlier, strict (R1)
+                window<1>(rg, sp1, digits, glp, n, t, cp);      // line p+1: later, >=
+                peak = q > (uint32_t)cm[0] && q > (uint32_t)cm[1] && q > (uint32_t)cm[2] &&
+                       q >= (uint32_t)cp[0] && q >= (uint32_t)cp[1] && q >= (uint32_t)cp[2];
             }
+            const unsigned pm = __ballot_sync(0xffffffffu, peak);
+            if (pm == 0) return;
+            const int leader = __ffs(pm) - 1;
+            uint32_t base = 0;
+            if (lane == leader) base = atomicAdd(&s_npk[par], (uint32_t)__popc(pm));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            if (peak) {
+                const uint32_t j = gl + jl;
+                atomicOr(&peakmask[j >> 5], 1u << (j & 31u));
+                const uint32_t slot = base + (uint32_t)__popc(pm & ((1u << lane) - 1u));
+                if (slot < kPeakQ) s_pq[slot] = ((uint32_t)lo << 16) | jl;
+                else moments(p, jl, vp);                        // queue full (very dense data): do it here
+            }
+        };
+
+        uint32_t wcount = 0;                                    // warp-uniform
+        uint32_t carry = 0;                                     // tq word of the digit before this chunk
+        for (uint32_t c0 = 0; c0 < len; c0 += 32) {
+            const uint32_t jl = c0 + lane;
+            const bool act = jl < len;
+            const uint32_t self = act ? fetch(sp, gl, jl) : 0u;
+            uint32_t prev = __shfl_up_sync(0xffffffffu, self, 1);
+            uint32_t next = __shfl_down_sync(0xffffffffu, self, 1);
+            if (lane == 0) prev = carry;
+            if (lane == 31) next = (jl + 1 < len) ? fetch(sp, gl, jl + 1) : 0u;
+            carry = __shfl_sync(0xffffffffu, self, 31);
+            const int t = (int)(self & 0xffffu);
+            const uint32_t q = self >> 16;
+            // the neighbours in time are the adjacent digits of the line (an absent one reads as charge 0)
+            const uint32_t qm = ((int)(prev & 0xffffu) == t - 1) ? (prev >> 16) : 0u;
+            const uint32_t qp = ((int)(next & 0xffffu) == t + 1 && t + 1 < T) ? (next >> 16) : 0u;
+            const bool surv = act && q >= q_peak_min && t < T && q > qm && q >= qp;   // R1: (0,-1) strict, (0,+1) >=
             const unsigned m = __ballot_sync(0xffffffffu, surv);
-            if (surv) wq[wcount + (uint32_t)__popc(m & ((1u << lane) - 1u))] = j;
+            if (surv) wq[wcount + (uint32_t)__popc(m & ((1u << lane) - 1u))] = jl;
             wcount += (uint32_t)__popc(m);
             __syncwarp();
             if (wcount >= 32u) {
-                stage_b(true, wq[lane], l0, l1, par);
+                stage_b(true, wq[lane]);
                 const uint32_t mv = (lane + 32u < wcount) ? wq[lane + 32u] : 0u;
                 __syncwarp();
                 if (lane + 32u < wcount) wq[lane] = mv;
@@ -287,32 +303,32 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
                 __syncwarp();
             }
         }
-        if (wcount) stage_b((uint32_t)lane < wcount, (uint32_t)lane < wcount ? wq[lane] : 0u, l0, l1, par);
-    };
-    auto phase2 = [&](int l0, int l1, int par) {
-        l1 = min(l1, pb);
-        const uint32_t np = min(s_npk[par], (uint32_t)kPeakQ);
-        for (uint32_t i = tid; i < np; i += kFThreads) {
-            const uint32_t j = s_pq[i];
-            int p; uint32_t jl, len;
-            locate(j, l0, l1, p, jl, len);
-            const uint32_t self = fetch(slot_of(p), j, jl);
-            moments(j, p, (int)(self & 0xffffu));
-        }
-        if (tid == 0) s_npk[par ^ 1] = 0u;
+        if (wcount) stage_b((uint32_t)lane < wcount, (uint32_t)lane < wcount ? wq[lane] : 0u);
     };
 
-    // prologue: lines needed by step 0
-    build(pa - 2, pa + kS + 2);
+    // ---- main loop -------------------------------------------------------------------------------------------------
+    // Ring index of line p is (p - (pa - 2)) mod kSlots.  Prologue: lines pa-2 .. pa+S+1.
+    for (int i = warp; i < kS + 4; i += kWarps) build_line(pa - 2 + i, i, false);
     __syncthreads();
-    int par = 0;
+    int vl0 = 2, par = 0;                                       // ring index of line l0; step parity
     for (int l0 = pa; l0 < pb; l0 += kS, par ^= 1) {
-        phase1(l0, l0 + kS, par);
+        const bool more = l0 + kS < pb;                         // lines l0+S+2 .. l0+2S+1 enter the ring in this step
+        const int pnew = l0 + kS + 2 + warp, vnew = ring_at(vl0, kS + 2 + warp - kSlots);
+        if (more) prefetch_line(pnew, vnew);
+        if (l0 + warp < pb) stage_ab(l0 + warp, ring_at(vl0, warp), warp, par);
         __syncthreads();
-        phase2(l0, l0 + kS, par);
-        build(l0 + kS + 2, l0 + 2 * kS + 2);
-        clear(l0 - kS - 2, l0 - 2);
+        {
+            if (tid == 0) s_npk[par ^ 1] = 0u;
+            const uint32_t np = min(s_npk[par], (uint32_t)kPeakQ);
+            for (uint32_t i = tid; i < np; i += kFThreads) {
+                const uint32_t e = s_pq[i];
+                const int lo = (int)(e >> 16);
+                moments(l0 + lo, e & 0xffffu, ring_at(vl0, lo));
+            }
+        }
+        if (more) build_line(pnew, vnew, true);
         __syncthreads();
+        vl0 = ring_at(vl0, kS);
     }
     if (bad_order) s_unsorted = 1;
     __syncthreads();
@@ -335,14 +351,16 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     for (uint32_t r = 0; r < g.n_rows; ++r) total_pads += g.npads[r];
     total_pads *= g.n_sectors;
     const double mean_len = (double)n / (double)(total_pads ? total_pads : 1);
-    const uint32_t wpl = (g.n_time + 31) / 32 + 3;          // guard word below, >= 2 words above the last bin
-    uint32_t cap = (uint32_t)(mean_len * 1.5) + 64;
-    cap = (cap + 31u) & ~31u;
-    const uint32_t max_smem = 52 * 1024;                     // 4 CTAs per SM (+ ~1 KB static + 1 KB reserved each)
-    const uint32_t fixed = kSlots * (wpl * 4 + ((wpl + 1) / 2) * 4);
-    if (fixed + kSlots * cap * 4 > max_smem) cap = fixed < max_smem ? ((max_smem - fixed) / (kSlots * 4)) & ~31u : 0;
+    const uint32_t wpl = (((g.n_time + 31) / 32 + 3) + 3u) & ~3u;   // guard word below, >= 2 above; multiple of 4
+    const uint32_t pre_words = ((wpl >> 1) + 3u) & ~3u;
+    uint32_t cap = ((uint32_t)(mean_len * 1.5) + 64u + 31u) & ~31u;
+    const uint32_t max_smem = 104 * 1024;                    // 2 CTAs per SM (+ ~8 KB static + 1 KB reserved each)
+    const uint32_t fixed = kSlots * (wpl + pre_words) * 4;
+    if (fixed + kSlots * 32 * 4 > 200 * 1024) return TPC_CF_E_GEOMETRY;   // cannot happen for n_time <= 65535
+    uint32_t limit = fixed + kSlots * 32 * 4 <= max_smem ? max_smem : 200 * 1024;
+    if (fixed + kSlots * cap * 4 > limit) cap = ((limit - fixed) / (kSlots * 4)) & ~31u;
     const uint32_t smem = fixed + kSlots * cap * 4;
-    const uint32_t pads_per_unit = (g.max_pads + 1) / 2;
+    const uint32_t pads_per_unit = 6 * kS;                   // 48 pads: 6 steps per CTA, 4 halo lines
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
     static bool attr_set = false;
     if (!attr_set) {
@@ -355,8 +373,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
                                                              pads_per_unit, upp, wpl, cap, q_peak_min, q_gate,
                                                              ws.counters, ws.peakmask, (uint4*)ws.stage);
     if (ev_k1) cudaEventRecord(ev_k1, st);
-    ++k;
-    return k;
+    return k + 1;
 }
 
 }  // namespace tpccf
