@@ -56,7 +56,8 @@ struct Ring {
     uint32_t* sm;          // base of the dynamic shared memory
     uint32_t slot_words;   // words per slot (multiple of 4)
     uint32_t wpl;          // bitmap words per line (multiple of 4)
-    uint32_t cap;          // tq entries per slot (lines longer than this read the tail from global memory)
+    uint32_t cap;          // tq entries per slot (multiple of 128; longer lines read their tail from global memory)
+    uint32_t pre_words;    // words of the rank directory (wpl uint16, padded to a multiple of 4 words)
     __device__ __forceinline__ uint32_t* slot(int v) const { return sm + (uint32_t)v * slot_words; }
 };
 
@@ -119,7 +120,8 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     Ring rg;
     rg.sm = reinterpret_cast<uint32_t*>(smem_raw);
     rg.wpl = wpl; rg.cap = cap;
-    rg.slot_words = wpl + cap + (((wpl >> 1) + 3u) & ~3u);
+    rg.pre_words = ((wpl >> 1) + 3u) & ~3u;
+    rg.slot_words = wpl + cap + rg.pre_words + (cap >> 5);   // bm | tq | pre | stage-A bits
 
     for (int i = tid; i <= (int)g.LS; i += kFThreads) s_ls[i] = line_start[plane * g.LS + i];
     if (tid == 0) { s_unsorted = 0; s_npk[0] = 0u; s_npk[1] = 0u; }
@@ -187,35 +189,51 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         uint16_t* pre = reinterpret_cast<uint16_t*>(slot + rg.wpl + rg.cap);
         const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
         const bool owner = p >= pa && p < pb;
+        uint32_t* sbm = slot + rg.wpl + rg.cap + rg.pre_words;   // stage-A result: one bit per digit index < cap
+        // (time|charge) word of digit jl: from the staged tq area, else from the digit array (and into tq)
+        auto load_y = [&](uint32_t jl) -> uint32_t {
+            if (jl >= len) return 0u;
+            if (staged && jl < rg.cap) return slot[rg.wpl + jl];
+            const uint32_t y = __ldg(&digits[lbeg + jl].y);
+            if (jl < rg.cap) slot[rg.wpl + jl] = y;
+            return y;
+        };
         uint32_t carry = 0;                                 // tq word of the digit before this chunk
-        uint32_t xn = lane < len ? __ldg(&digits[lbeg + lane].x) : 0u;   // key words, loaded one chunk ahead
+        uint32_t xn = lane < len ? __ldg(&digits[lbeg + lane].x) : 0u;   // both words are loaded one chunk ahead
+        uint32_t yn = load_y(lane);
         for (uint32_t c0 = 0; c0 < len; c0 += 32) {
             const uint32_t jl = c0 + lane;
             const bool act = jl < len;
-            const uint32_t dx = xn;
-            if (jl + 32 < len) xn = __ldg(&digits[lbeg + jl + 32].x);
-            uint32_t dy = 0u;
-            if (act) {
-                if (staged && jl < rg.cap) dy = slot[rg.wpl + jl];
-                else { dy = __ldg(&digits[lbeg + jl].y); if (jl < rg.cap) slot[rg.wpl + jl] = dy; }
-            }
+            const uint32_t dx = xn, dy = yn;
+            xn = (jl + 32 < len) ? __ldg(&digits[lbeg + jl + 32].x) : 0u;
+            yn = load_y(jl + 32);
             uint32_t prevy = __shfl_up_sync(0xffffffffu, dy, 1);
+            uint32_t nexty = __shfl_down_sync(0xffffffffu, dy, 1);
+            const uint32_t ny0 = __shfl_sync(0xffffffffu, yn, 0);
             if (lane == 0) prevy = carry;
+            if (lane == 31) nexty = ny0;
             carry = __shfl_sync(0xffffffffu, dy, 31);
-            const uint32_t t = dy & 0xffffu, pt = prevy & 0xffffu;
+            const uint32_t t = dy & 0xffffu, pt = prevy & 0xffffu, q = dy >> 16;
             const bool first = (jl == 0);
             const bool ok = act && (dx & 0x00ffffffu) == w0_line;
             if (act && (!ok || (!first && pt >= t))) bad_order = true;   // wrong line, not ascending, or duplicate cell
-            const bool badd = ok && owner && (t >= (uint32_t)T || (dy >> 16) == 0u);
+            const bool badd = ok && owner && (t >= (uint32_t)T || q == 0u);
             if (__any_sync(0xffffffffu, badd)) {
                 const unsigned mbad = __ballot_sync(0xffffffffu, badd);
                 if (lane == 0) atomicAdd(&cnt->n_bad, (unsigned long long)__popc(mbad));
             }
-            if (ok && t < (uint32_t)T) {
+            const bool valid = ok && t < (uint32_t)T;
+            if (valid) {
                 const uint32_t bw = (t + 32u) >> 5;
                 atomicOr(&slot[bw], 1u << (t & 31u));
                 if (first || ((pt + 32u) >> 5) != bw) pre[bw] = (uint16_t)jl;
             }
+            // K2 stage A, done here because only the line itself is needed: the neighbours in time are the adjacent
+            // digits of the line (an absent one reads as charge 0).  R1: (0,-1) strict, (0,+1) >=
+            const uint32_t qm = (pt + 1u == t && !first) ? (prevy >> 16) : 0u;
+            const uint32_t qp = ((nexty & 0xffffu) == t + 1u && t + 1u < (uint32_t)T) ? (nexty >> 16) : 0u;
+            const unsigned sm = __ballot_sync(0xffffffffu, valid && q >= q_peak_min && q > qm && q >= qp);
+            if (lane == 0 && c0 < rg.cap) sbm[c0 >> 5] = sm;
         }
     };
 
@@ -274,23 +292,9 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         };
 
         uint32_t wcount = 0;                                    // warp-uniform
-        uint32_t carry = 0;                                     // tq word of the digit before this chunk
-        for (uint32_t c0 = 0; c0 < len; c0 += 32) {
-            const uint32_t jl = c0 + lane;
-            const bool act = jl < len;
-            const uint32_t self = act ? fetch(sp, gl, jl) : 0u;
-            uint32_t prev = __shfl_up_sync(0xffffffffu, self, 1);
-            uint32_t next = __shfl_down_sync(0xffffffffu, self, 1);
-            if (lane == 0) prev = carry;
-            if (lane == 31) next = (jl + 1 < len) ? fetch(sp, gl, jl + 1) : 0u;
-            carry = __shfl_sync(0xffffffffu, self, 31);
-            const int t = (int)(self & 0xffffu);
-            const uint32_t q = self >> 16;
-            // the neighbours in time are the adjacent digits of the line (an absent one reads as charge 0)
-            const uint32_t qm = ((int)(prev & 0xffffu) == t - 1) ? (prev >> 16) : 0u;
-            const uint32_t qp = ((int)(next & 0xffffu) == t + 1 && t + 1 < T) ? (next >> 16) : 0u;
-            const bool surv = act && q >= q_peak_min && t < T && q > qm && q >= qp;   // R1: (0,-1) strict, (0,+1) >=
+        auto enqueue = [&](bool surv, uint32_t jl) {            // survivors -> warp queue; stage B on every full 32
             const unsigned m = __ballot_sync(0xffffffffu, surv);
+            if (m == 0) return;
             if (surv) wq[wcount + (uint32_t)__popc(m & ((1u << lane) - 1u))] = jl;
             wcount += (uint32_t)__popc(m);
             __syncwarp();
@@ -302,6 +306,27 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
                 wcount -= 32u;
                 __syncwarp();
             }
+        };
+        // stage A was done when the line was built: one bit per digit index below cap
+        const uint32_t* sbm = sp + rg.wpl + rg.cap + rg.pre_words;
+        const uint32_t nstaged = min(len, rg.cap);
+        for (uint32_t c0 = 0; c0 < nstaged; c0 += 32) enqueue((sbm[c0 >> 5] >> lane) & 1u, c0 + lane);
+        // tail of a line longer than cap: the own-line test from the digit array
+        uint32_t carry = nstaged < len ? fetch(sp, gl, nstaged - 1) : 0u;
+        for (uint32_t c0 = nstaged; c0 < len; c0 += 32) {
+            const uint32_t jl = c0 + lane;
+            const bool act = jl < len;
+            const uint32_t self = act ? fetch(sp, gl, jl) : 0u;
+            uint32_t prev = __shfl_up_sync(0xffffffffu, self, 1);
+            uint32_t next = __shfl_down_sync(0xffffffffu, self, 1);
+            if (lane == 0) prev = carry;
+            if (lane == 31) next = (jl + 1 < len) ? fetch(sp, gl, jl + 1) : 0u;
+            carry = __shfl_sync(0xffffffffu, self, 31);
+            const int t = (int)(self & 0xffffu);
+            const uint32_t q = self >> 16;
+            const uint32_t qm = ((int)(prev & 0xffffu) == t - 1) ? (prev >> 16) : 0u;
+            const uint32_t qp = ((int)(next & 0xffffu) == t + 1 && t + 1 < T) ? (next >> 16) : 0u;
+            enqueue(act && q >= q_peak_min && t < T && q > qm && q >= qp, jl);   // R1: (0,-1) strict, (0,+1) >=
         }
         if (wcount) stage_b((uint32_t)lane < wcount, (uint32_t)lane < wcount ? wq[lane] : 0u);
     };
@@ -353,13 +378,14 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const double mean_len = (double)n / (double)(total_pads ? total_pads : 1);
     const uint32_t wpl = (((g.n_time + 31) / 32 + 3) + 3u) & ~3u;   // guard word below, >= 2 above; multiple of 4
     const uint32_t pre_words = ((wpl >> 1) + 3u) & ~3u;
-    uint32_t cap = ((uint32_t)(mean_len * 1.5) + 64u + 31u) & ~31u;
+    uint32_t cap = ((uint32_t)(mean_len * 1.5) + 64u + 127u) & ~127u;
     const uint32_t max_smem = 104 * 1024;                    // 2 CTAs per SM (+ ~8 KB static + 1 KB reserved each)
     const uint32_t fixed = kSlots * (wpl + pre_words) * 4;
-    if (fixed + kSlots * 32 * 4 > 200 * 1024) return TPC_CF_E_GEOMETRY;   // cannot happen for n_time <= 65535
-    uint32_t limit = fixed + kSlots * 32 * 4 <= max_smem ? max_smem : 200 * 1024;
-    if (fixed + kSlots * cap * 4 > limit) cap = ((limit - fixed) / (kSlots * 4)) & ~31u;
-    const uint32_t smem = fixed + kSlots * cap * 4;
+    if (fixed + kSlots * 128 * 4 + kSlots * 16 > 200 * 1024) return TPC_CF_E_GEOMETRY;   // cannot happen for n_time <= 65535
+    const uint32_t limit = fixed + kSlots * 128 * 4 + kSlots * 16 <= max_smem ? max_smem : 200 * 1024;
+    const uint32_t per_cap = kSlots * 4 + kSlots / 8 + 1;   // bytes per unit of cap: tq word + stage-A bit
+    if (fixed + per_cap * cap > limit) cap = ((limit - fixed) / per_cap) & ~127u;
+    const uint32_t smem = fixed + kSlots * (cap * 4 + (cap >> 5) * 4);
     const uint32_t pads_per_unit = 6 * kS;                   // 48 pads: 6 steps per CTA, 4 halo lines
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
     static bool attr_set = false;
