@@ -11,9 +11,10 @@
 //                               (this is also K0: a slot is cleaned by the warp that reuses it)
 //                   K2 stage A  own-line test of every digit against the adjacent digits of the line (shuffles)
 //                      stage B  survivors (~25 %) against lines p-1 / p+1 through 3-bit bitmap windows
-//                   K4 stage C  peaks (~5 %) gathered into a CTA queue; 5x5 window from the five slots p-2..p+2,
+//                   K4 stage C  peaks (~5 %) gathered into a per-warp queue; 5x5 window from the five slots p-2..p+2,
 //                               gated sums, record -> stage[j]
-//                  Step = 8 lines: [A+B on lines l0..l0+7] barrier [C for their peaks | build lines l0+10..l0+17] barrier.
+//                  Step = 8 lines, one barrier: each warp prefetches (cp.async) the line it will build, runs A+B+C on
+//                  its current line, then rebuilds the slot of a line that left the ring.
 //                  Peaks are recorded as one bit per digit (peakmask) and their cluster at stage[j]; the shared
 //                  compaction (tpc_cf_compact.cu) turns that into the ordered output (K3, K5).
 //   The DIGITS_SORTED promise is verified here for free: every digit is checked once against the line (or gap) it
@@ -26,7 +27,6 @@ static constexpr int kFThreads = 256;
 static constexpr int kWarps = kFThreads / 32;
 static constexpr int kS = kWarps;               // lines per step: one per warp
 static constexpr int kSlots = 2 * kS + 4;       // lines l0-2 .. l0+S+1 in use, next S being built
-static constexpr int kPeakQ = 1024;             // CTA peak queue entries per step
 
 __device__ __forceinline__ uint32_t key24_of(uint32_t w0)
 {
@@ -104,8 +104,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_ls[260];          // line starts of this plane: s_ls[p], p = 0..max_pads, then next plane's start
     __shared__ uint32_t s_wq[kWarps][64];   // per-warp survivor queues (stage A -> B): index within the warp's line
-    __shared__ uint32_t s_pq[kPeakQ];       // CTA peak queue (stage B -> C): (line - l0) << 16 | index within the line
-    __shared__ uint32_t s_npk[2];           // its fill count, double-buffered by step parity
+    __shared__ uint32_t s_pq[kWarps][64];   // per-warp peak queues (stage B -> C): index within the warp's line
     __shared__ int s_unsorted;
 
     const uint32_t plane = blockIdx.x / units_per_plane, unit = blockIdx.x % units_per_plane;
@@ -124,7 +123,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     rg.slot_words = wpl + cap + rg.pre_words + (cap >> 5);   // bm | tq | pre | stage-A bits
 
     for (int i = tid; i <= (int)g.LS; i += kFThreads) s_ls[i] = line_start[plane * g.LS + i];
-    if (tid == 0) { s_unsorted = 0; s_npk[0] = 0u; s_npk[1] = 0u; }
+    if (tid == 0) s_unsorted = 0;
     {   // every slot starts as an empty line (lines outside the plane keep this state: zero border in pad, R2)
         uint4* z = reinterpret_cast<uint4*>(rg.sm);
         const uint32_t nz = (kSlots * rg.slot_words) >> 2;
@@ -254,7 +253,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     };
 
     // ---- K2: stages A and B for line p (ring index vp), owned by this warp; lo = p - l0 ------------------------------
-    auto stage_ab = [&](int p, int vp, int lo, int par) {
+    auto stage_ab = [&](int p, int vp) {
         const uint32_t gl = s_ls[p], len = s_ls[p + 1] - gl;
         if (len == 0) return;
         const uint32_t* sp = rg.slot(vp);
@@ -262,6 +261,8 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         const uint32_t* sp1 = rg.slot(ring_at(vp, 1));
         const uint32_t glm = s_ls[max(p - 1, 0)], glp = s_ls[min(p + 1, P)];
         uint32_t* wq = s_wq[warp];
+        uint32_t* pq = s_pq[warp];
+        uint32_t pcount = 0;                                    // warp-uniform
 
         auto stage_b = [&](bool act, uint32_t jl) {
             bool peak = false;
@@ -276,18 +277,23 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
                 peak = q > (uint32_t)cm[0] && q > (uint32_t)cm[1] && q > (uint32_t)cm[2] &&
                        q >= (uint32_t)cp[0] && q >= (uint32_t)cp[1] && q >= (uint32_t)cp[2];
             }
+            // peaks -> this warp's peak queue; stage C runs on every full 32 (dense lanes) and once at the end
             const unsigned pm = __ballot_sync(0xffffffffu, peak);
             if (pm == 0) return;
-            const int leader = __ffs(pm) - 1;
-            uint32_t base = 0;
-            if (lane == leader) base = atomicAdd(&s_npk[par], (uint32_t)__popc(pm));
-            base = __shfl_sync(0xffffffffu, base, leader);
             if (peak) {
                 const uint32_t j = gl + jl;
                 atomicOr(&peakmask[j >> 5], 1u << (j & 31u));
-                const uint32_t slot = base + (uint32_t)__popc(pm & ((1u << lane) - 1u));
-                if (slot < kPeakQ) s_pq[slot] = ((uint32_t)lo << 16) | jl;
-                else moments(p, jl, vp);                        // queue full (very dense data): do it here
+                pq[pcount + (uint32_t)__popc(pm & ((1u << lane) - 1u))] = jl;
+            }
+            pcount += (uint32_t)__popc(pm);
+            __syncwarp();
+            if (pcount >= 32u) {
+                moments(p, pq[lane], vp);
+                const uint32_t mv = (lane + 32u < pcount) ? pq[lane + 32u] : 0u;
+                __syncwarp();
+                if (lane + 32u < pcount) pq[lane] = mv;
+                pcount -= 32u;
+                __syncwarp();
             }
         };
 
@@ -329,28 +335,22 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             enqueue(act && q >= q_peak_min && t < T && q > qm && q >= qp, jl);   // R1: (0,-1) strict, (0,+1) >=
         }
         if (wcount) stage_b((uint32_t)lane < wcount, (uint32_t)lane < wcount ? wq[lane] : 0u);
+        if ((uint32_t)lane < pcount) moments(p, pq[lane], vp);
     };
 
     // ---- main loop -------------------------------------------------------------------------------------------------
     // Ring index of line p is (p - (pa - 2)) mod kSlots.  Prologue: lines pa-2 .. pa+S+1.
-    for (int i = warp; i < kS + 4; i += kWarps) build_line(pa - 2 + i, i, false);
+    for (int i = warp; i < kS + 4; i += kWarps) prefetch_line(pa - 2 + i, i);
+    for (int i = warp; i < kS + 4; i += kWarps) build_line(pa - 2 + i, i, true);
     __syncthreads();
-    int vl0 = 2, par = 0;                                       // ring index of line l0; step parity
-    for (int l0 = pa; l0 < pb; l0 += kS, par ^= 1) {
+    // Step (ONE barrier): every warp prefetches the line it will build, runs stages A+B+C on its current line
+    // (lines l0-2 .. l0+S+1 are complete), then rebuilds the slot of a line that left the ring (l0-S-2 .. l0-3).
+    int vl0 = 2;                                                // ring index of line l0
+    for (int l0 = pa; l0 < pb; l0 += kS) {
         const bool more = l0 + kS < pb;                         // lines l0+S+2 .. l0+2S+1 enter the ring in this step
         const int pnew = l0 + kS + 2 + warp, vnew = ring_at(vl0, kS + 2 + warp - kSlots);
         if (more) prefetch_line(pnew, vnew);
-        if (l0 + warp < pb) stage_ab(l0 + warp, ring_at(vl0, warp), warp, par);
-        __syncthreads();
-        {
-            if (tid == 0) s_npk[par ^ 1] = 0u;
-            const uint32_t np = min(s_npk[par], (uint32_t)kPeakQ);
-            for (uint32_t i = tid; i < np; i += kFThreads) {
-                const uint32_t e = s_pq[i];
-                const int lo = (int)(e >> 16);
-                moments(l0 + lo, e & 0xffffu, ring_at(vl0, lo));
-            }
-        }
+        if (l0 + warp < pb) stage_ab(l0 + warp, ring_at(vl0, warp));
         if (more) build_line(pnew, vnew, true);
         __syncthreads();
         vl0 = ring_at(vl0, kS);
