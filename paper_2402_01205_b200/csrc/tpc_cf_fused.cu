@@ -163,19 +163,26 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
 
     // ---- prefetch for K1: the (time|charge) words of line p go straight into the tq area of slot v with cp.async ----
     // (issued at the top of a step by the warp that builds the line after the step's first barrier)
-    auto prefetch_line = [&](int p, int v) {
+    // The key words (sector,row,pad) are staged too, into this warp's own buffer, when with_x is set: the build then
+    // verifies every digit's line without a single exposed global load.
+    uint32_t* xst = rg.sm + kSlots * rg.slot_words + (uint32_t)warp * rg.cap;
+    auto prefetch_line = [&](int p, int v, bool with_x) {
         if (p < blo || p >= bhi) return;
         const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
         const uint32_t m = min(len, rg.cap);
         const uint32_t dst = (uint32_t)__cvta_generic_to_shared(rg.slot(v) + rg.wpl);
-        for (uint32_t jl = lane; jl < m; jl += 32)
+        const uint32_t dsx = (uint32_t)__cvta_generic_to_shared(xst);
+        for (uint32_t jl = lane; jl < m; jl += 32) {
             asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + 4u * jl), "l"(&digits[lbeg + jl].y) : "memory");
+            if (with_x)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dsx + 4u * jl), "l"(&digits[lbeg + jl].x) : "memory");
+        }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
     // ---- K0 + K1: this warp (re)builds the slot v of line p from the line's digits -----------------------------------
     // staged: the tq words [0, min(len,cap)) were already copied by prefetch_line.
-    auto build_line = [&](int p, int v, bool staged) {
+    auto build_line = [&](int p, int v, bool staged, bool xstaged) {
         uint32_t* slot = rg.slot(v);
         {
             uint4* z = reinterpret_cast<uint4*>(slot);
@@ -197,14 +204,19 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             if (jl < rg.cap) slot[rg.wpl + jl] = y;
             return y;
         };
+        auto load_x = [&](uint32_t jl) -> uint32_t {
+            if (jl >= len) return 0u;
+            if (xstaged && jl < rg.cap) return xst[jl];
+            return __ldg(&digits[lbeg + jl].x);
+        };
         uint32_t carry = 0;                                 // tq word of the digit before this chunk
-        uint32_t xn = lane < len ? __ldg(&digits[lbeg + lane].x) : 0u;   // both words are loaded one chunk ahead
+        uint32_t xn = load_x(lane);                         // both words are loaded one chunk ahead
         uint32_t yn = load_y(lane);
         for (uint32_t c0 = 0; c0 < len; c0 += 32) {
             const uint32_t jl = c0 + lane;
             const bool act = jl < len;
             const uint32_t dx = xn, dy = yn;
-            xn = (jl + 32 < len) ? __ldg(&digits[lbeg + jl + 32].x) : 0u;
+            xn = load_x(jl + 32);
             yn = load_y(jl + 32);
             uint32_t prevy = __shfl_up_sync(0xffffffffu, dy, 1);
             uint32_t nexty = __shfl_down_sync(0xffffffffu, dy, 1);
@@ -340,8 +352,8 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
 
     // ---- main loop -------------------------------------------------------------------------------------------------
     // Ring index of line p is (p - (pa - 2)) mod kSlots.  Prologue: lines pa-2 .. pa+S+1.
-    for (int i = warp; i < kS + 4; i += kWarps) prefetch_line(pa - 2 + i, i);
-    for (int i = warp; i < kS + 4; i += kWarps) build_line(pa - 2 + i, i, true);
+    for (int i = warp; i < kS + 4; i += kWarps) prefetch_line(pa - 2 + i, i, i < kWarps);
+    for (int i = warp; i < kS + 4; i += kWarps) build_line(pa - 2 + i, i, true, i < kWarps);
     __syncthreads();
     // Step (ONE barrier): every warp prefetches the line it will build, runs stages A+B+C on its current line
     // (lines l0-2 .. l0+S+1 are complete), then rebuilds the slot of a line that left the ring (l0-S-2 .. l0-3).
@@ -349,9 +361,9 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     for (int l0 = pa; l0 < pb; l0 += kS) {
         const bool more = l0 + kS < pb;                         // lines l0+S+2 .. l0+2S+1 enter the ring in this step
         const int pnew = l0 + kS + 2 + warp, vnew = ring_at(vl0, kS + 2 + warp - kSlots);
-        if (more) prefetch_line(pnew, vnew);
+        if (more) prefetch_line(pnew, vnew, true);
         if (l0 + warp < pb) stage_ab(l0 + warp, ring_at(vl0, warp));
-        if (more) build_line(pnew, vnew, true);
+        if (more) build_line(pnew, vnew, true, true);
         __syncthreads();
         vl0 = ring_at(vl0, kS);
     }
@@ -379,13 +391,14 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t wpl = (((g.n_time + 31) / 32 + 3) + 3u) & ~3u;   // guard word below, >= 2 above; multiple of 4
     const uint32_t pre_words = ((wpl >> 1) + 3u) & ~3u;
     uint32_t cap = ((uint32_t)(mean_len * 1.5) + 64u + 127u) & ~127u;
-    const uint32_t max_smem = 104 * 1024;                    // 2 CTAs per SM (+ ~8 KB static + 1 KB reserved each)
+    const uint32_t max_smem = 106 * 1024;                    // 2 CTAs per SM (+ ~5 KB static + 1 KB reserved each)
     const uint32_t fixed = kSlots * (wpl + pre_words) * 4;
-    if (fixed + kSlots * 128 * 4 + kSlots * 16 > 200 * 1024) return TPC_CF_E_GEOMETRY;   // cannot happen for n_time <= 65535
-    const uint32_t limit = fixed + kSlots * 128 * 4 + kSlots * 16 <= max_smem ? max_smem : 200 * 1024;
-    const uint32_t per_cap = kSlots * 4 + kSlots / 8 + 1;   // bytes per unit of cap: tq word + stage-A bit
+    const uint32_t per_cap0 = kSlots * 4 + kSlots / 8 + 1 + kWarps * 4;
+    if (fixed + per_cap0 * 128 > 200 * 1024) return TPC_CF_E_GEOMETRY;   // cannot happen for n_time <= 65535
+    const uint32_t limit = fixed + per_cap0 * 128 <= max_smem ? max_smem : 200 * 1024;
+    const uint32_t per_cap = kSlots * 4 + kSlots / 8 + 1 + kWarps * 4;   // bytes per unit of cap: tq word + stage-A bit + key staging
     if (fixed + per_cap * cap > limit) cap = ((limit - fixed) / per_cap) & ~127u;
-    const uint32_t smem = fixed + kSlots * (cap * 4 + (cap >> 5) * 4);
+    const uint32_t smem = fixed + kSlots * (cap * 4 + (cap >> 5) * 4) + kWarps * cap * 4;
     const uint32_t pads_per_unit = 6 * kS;                   // 48 pads: 6 steps per CTA, 4 halo lines
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
     static bool attr_set = false;
