@@ -85,13 +85,24 @@ __device__ __forceinline__ void window(const Ring& rg, const uint32_t* __restric
     const uint32_t bits = __funnelshift_r(lo, hi, s) & ((1u << (2 * H + 1)) - 1u);
     const uint32_t p0 = pre[w], p1 = pre[w + 1];
     const uint32_t idx = (lo >> s) ? p0 + (uint32_t)__popc(lo & ((1u << s) - 1u)) : p1;
+    if (bits == 0u) {
 #pragma unroll
-    for (int k = 0; k < 2 * H + 1; ++k) {
-        const uint32_t ik = idx + (uint32_t)__popc(bits & ((1u << k) - 1u));
-        uint32_t v = tq[min(ik, rg.cap - 1u)];
-        const bool present = (bits >> k) & 1u;
-        if (present && ik >= rg.cap) v = __ldg(&digits[min(gl + ik, n - 1u)].y);
-        c[k] = present ? (int)(v >> 16) : 0;
+        for (int k = 0; k < 2 * H + 1; ++k) c[k] = 0;
+    } else if (idx + (uint32_t)__popc(bits) <= rg.cap) {          // all present cells are in the staged tq area
+#pragma unroll
+        for (int k = 0; k < 2 * H + 1; ++k) {
+            const uint32_t v = tq[idx + (uint32_t)__popc(bits & ((1u << k) - 1u))];
+            c[k] = ((bits >> k) & 1u) ? (int)(v >> 16) : 0;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 2 * H + 1; ++k) {
+            const uint32_t ik = idx + (uint32_t)__popc(bits & ((1u << k) - 1u));
+            uint32_t v = tq[min(ik, rg.cap - 1u)];
+            const bool present = (bits >> k) & 1u;
+            if (present && ik >= rg.cap) v = __ldg(&digits[min(gl + ik, n - 1u)].y);
+            c[k] = present ? (int)(v >> 16) : 0;
+        }
     }
 }
 
@@ -197,7 +208,9 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         const bool owner = p >= pa && p < pb;
         uint32_t* sbm = slot + rg.wpl + rg.cap + rg.pre_words;   // stage-A result: one bit per digit index < cap
         // (time|charge) word of digit jl: from the staged tq area, else from the digit array (and into tq)
+        const bool fast = staged && xstaged && len <= rg.cap;   // the common case: both words of every digit are staged
         auto load_y = [&](uint32_t jl) -> uint32_t {
+            if (fast) return jl < len ? slot[rg.wpl + jl] : 0u;
             if (jl >= len) return 0u;
             if (staged && jl < rg.cap) return slot[rg.wpl + jl];
             const uint32_t y = __ldg(&digits[lbeg + jl].y);
@@ -205,6 +218,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             return y;
         };
         auto load_x = [&](uint32_t jl) -> uint32_t {
+            if (fast) return jl < len ? xst[jl] : 0u;
             if (jl >= len) return 0u;
             if (xstaged && jl < rg.cap) return xst[jl];
             return __ldg(&digits[lbeg + jl].x);
@@ -229,10 +243,8 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             const bool ok = act && (dx & 0x00ffffffu) == w0_line;
             if (act && (!ok || (!first && pt >= t))) bad_order = true;   // wrong line, not ascending, or duplicate cell
             const bool badd = ok && owner && (t >= (uint32_t)T || q == 0u);
-            if (__any_sync(0xffffffffu, badd)) {
-                const unsigned mbad = __ballot_sync(0xffffffffu, badd);
-                if (lane == 0) atomicAdd(&cnt->n_bad, (unsigned long long)__popc(mbad));
-            }
+            const unsigned mbad = __ballot_sync(0xffffffffu, badd);
+            if (mbad != 0u && lane == 0) atomicAdd(&cnt->n_bad, (unsigned long long)__popc(mbad));
             const bool valid = ok && t < (uint32_t)T;
             if (valid) {
                 const uint32_t bw = (t + 32u) >> 5;
@@ -250,16 +262,15 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
 
     // ---- K4 (stage C): 5x5 window from the slots of lines p-2..p+2, gated sums, record -> stage[j] ----------------
     // vp = ring index of line p.  Slots of lines outside the plane are empty (R2).
-    auto moments = [&](int p, uint32_t jl, int vp) {
-        const uint32_t gl = s_ls[p];
-        const uint32_t self = fetch(rg.slot(vp), gl, jl);
+    // sl[a] / gls[a]: slot and first-digit index of line p+a-2 (warp-uniform: a warp's peaks are all on its line)
+    auto moments = [&](int p, uint32_t jl, const uint32_t* const (&sl)[5], const uint32_t (&gls)[5]) {
+        const uint32_t self = fetch(sl[2], gls[2], jl);
         const int t = (int)(self & 0xffffu);
         int c[5][5];
 #pragma unroll
-        for (int a = 0; a < 5; ++a)
-            window<2>(rg, rg.slot(ring_at(vp, a - 2)), digits, s_ls[min(max(p + a - 2, 0), P)], n, t, c[a]);
+        for (int a = 0; a < 5; ++a) window<2>(rg, sl[a], digits, gls[a], n, t, c[a]);
         const ClusterWords r = cluster_from_window(c, w0_base | ((uint32_t)p << 16), (uint32_t)t, q_gate);
-        const size_t j = (size_t)gl + jl;
+        const size_t j = (size_t)gls[2] + jl;
         stage[2 * j] = r.lo;
         stage[2 * j + 1] = r.hi;
     };
@@ -268,10 +279,17 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     auto stage_ab = [&](int p, int vp) {
         const uint32_t gl = s_ls[p], len = s_ls[p + 1] - gl;
         if (len == 0) return;
-        const uint32_t* sp = rg.slot(vp);
-        const uint32_t* sm1 = rg.slot(ring_at(vp, -1));
-        const uint32_t* sp1 = rg.slot(ring_at(vp, 1));
-        const uint32_t glm = s_ls[max(p - 1, 0)], glp = s_ls[min(p + 1, P)];
+        const uint32_t* sl[5];
+        uint32_t gls[5];
+#pragma unroll
+        for (int a = 0; a < 5; ++a) {
+            sl[a] = rg.slot(ring_at(vp, a - 2));
+            gls[a] = s_ls[min(max(p + a - 2, 0), P)];
+        }
+        const uint32_t* sp = sl[2];
+        const uint32_t* sm1 = sl[1];
+        const uint32_t* sp1 = sl[3];
+        const uint32_t glm = gls[1], glp = gls[3];
         uint32_t* wq = s_wq[warp];
         uint32_t* pq = s_pq[warp];
         uint32_t pcount = 0;                                    // warp-uniform
@@ -300,7 +318,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             pcount += (uint32_t)__popc(pm);
             __syncwarp();
             if (pcount >= 32u) {
-                moments(p, pq[lane], vp);
+                moments(p, pq[lane], sl, gls);
                 const uint32_t mv = (lane + 32u < pcount) ? pq[lane + 32u] : 0u;
                 __syncwarp();
                 if (lane + 32u < pcount) pq[lane] = mv;
@@ -310,9 +328,9 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         };
 
         uint32_t wcount = 0;                                    // warp-uniform
-        auto enqueue = [&](bool surv, uint32_t jl) {            // survivors -> warp queue; stage B on every full 32
-            const unsigned m = __ballot_sync(0xffffffffu, surv);
+        auto enqueue_m = [&](unsigned m, uint32_t jl) {         // m = ballot of survivors; stage B on every full 32
             if (m == 0) return;
+            const bool surv = (m >> lane) & 1u;
             if (surv) wq[wcount + (uint32_t)__popc(m & ((1u << lane) - 1u))] = jl;
             wcount += (uint32_t)__popc(m);
             __syncwarp();
@@ -328,7 +346,8 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         // stage A was done when the line was built: one bit per digit index below cap
         const uint32_t* sbm = sp + rg.wpl + rg.cap + rg.pre_words;
         const uint32_t nstaged = min(len, rg.cap);
-        for (uint32_t c0 = 0; c0 < nstaged; c0 += 32) enqueue((sbm[c0 >> 5] >> lane) & 1u, c0 + lane);
+        auto enqueue = [&](bool surv, uint32_t jl) { enqueue_m(__ballot_sync(0xffffffffu, surv), jl); };
+        for (uint32_t c0 = 0; c0 < nstaged; c0 += 32) enqueue_m(sbm[c0 >> 5], c0 + lane);
         // tail of a line longer than cap: the own-line test from the digit array
         uint32_t carry = nstaged < len ? fetch(sp, gl, nstaged - 1) : 0u;
         for (uint32_t c0 = nstaged; c0 < len; c0 += 32) {
@@ -347,7 +366,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             enqueue(act && q >= q_peak_min && t < T && q > qm && q >= qp, jl);   // R1: (0,-1) strict, (0,+1) >=
         }
         if (wcount) stage_b((uint32_t)lane < wcount, (uint32_t)lane < wcount ? wq[lane] : 0u);
-        if ((uint32_t)lane < pcount) moments(p, pq[lane], vp);
+        if ((uint32_t)lane < pcount) moments(p, pq[lane], sl, gls);
     };
 
     // ---- main loop -------------------------------------------------------------------------------------------------
