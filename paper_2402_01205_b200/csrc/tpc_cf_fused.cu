@@ -19,6 +19,8 @@
 //                  compaction (tpc_cf_compact.cu) turns that into the ordered output (K3, K5).
 //   The DIGITS_SORTED promise is verified here for free: every digit is checked once against the line (or gap) it
 //   was found in; any violation raises Counters::unsorted and the run reports path 0.
+#include <stdlib.h>
+
 #include "tpc_cf_internal.cuh"
 
 namespace tpccf {
@@ -418,7 +420,15 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t per_cap = kSlots * 4 + kSlots / 8 + 1 + kWarps * 4;   // bytes per unit of cap: tq word + stage-A bit + key staging
     if (fixed + per_cap * cap > limit) cap = ((limit - fixed) / per_cap) & ~127u;
     const uint32_t smem = fixed + kSlots * (cap * 4 + (cap >> 5) * 4) + kWarps * cap * 4;
-    const uint32_t pads_per_unit = 6 * kS;                   // 48 pads: 6 steps per CTA, 4 halo lines
+    // One CTA per whole plane when there are enough planes to fill the GPU (no halo lines, one prologue per plane:
+    // measured 2.94 ms vs 3.16 ms at 48 pads on config 3); smaller pad ranges for small problems.
+    const uint32_t whole = (g.max_pads + kS - 1) / kS * kS;
+    uint32_t pads_per_unit = g.n_planes >= 1184 ? whole : (g.n_planes >= 296 ? 6 * kS : 3 * kS);
+    if (pads_per_unit > whole) pads_per_unit = whole;
+    if (const char* e = getenv("TPC_CF_PADS_PER_UNIT")) {    // tuning knob (multiples of 8)
+        const int v = atoi(e);
+        if (v >= kS && v <= 256) pads_per_unit = (uint32_t)(v / kS * kS);
+    }
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
     static bool attr_set = false;
     if (!attr_set) {
