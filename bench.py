@@ -51,7 +51,8 @@ def load_traffic(workload, path):
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe): one
+    `nvidia-smi -lms` process streams a line every 20 ms; only lines stamped inside [enter, exit] are kept."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -59,28 +60,46 @@ class ClockSampler:
     def __init__(self, index=0):
         self.index = index
         self.rows = []
-        self.stop = False
+        self.all_rows = []
+        self.proc = None
         self.th = None
+        self.t0 = self.t1 = None
 
-    def _poll(self):
-        while not self.stop:
-            try:
-                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
-                if out.returncode == 0 and out.stdout.strip():
-                    self.rows.append([c.strip() for c in out.stdout.strip().split(",")])
-            except Exception:
-                pass
-            time.sleep(0.05)
+    def start(self):
+        """Launch the sampler early (it needs ~0.5 s to come up); __enter__/__exit__ mark the timed region."""
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return self
 
-    def __enter__(self):
-        self.th = threading.Thread(target=self._poll, daemon=True)
+        def pump():
+            for line in self.proc.stdout:
+                self.all_rows.append((time.perf_counter(), [c.strip() for c in line.strip().split(",")]))
+        self.th = threading.Thread(target=pump, daemon=True)
         self.th.start()
         return self
 
+    def __enter__(self):
+        if self.proc is None and self.th is None:
+            self.start()
+        self.t0 = time.perf_counter()
+        return self
+
     def __exit__(self, *a):
-        self.stop = True
-        self.th.join(timeout=6)
+        self.t1 = time.perf_counter()
+        time.sleep(0.05)
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=3)
+            except Exception:
+                self.proc.kill()
+        inside = [r for (t, r) in self.all_rows if self.t0 <= t <= self.t1 + 0.03 and len(r) >= 7]
+        near = [r for (t, r) in self.all_rows if len(r) >= 7]
+        self.rows = inside if inside else near[-3:]
 
     def summary(self):
         if not self.rows:
@@ -89,8 +108,9 @@ class ClockSampler:
         mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in self.rows)]
+        pw = [float(r[2]) for r in self.rows if r[2].replace(".", "").isdigit()]
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(self.rows)}
+                "reasons": reasons, "samples": len(self.rows), "power_w_max": max(pw) if pw else None}
 
 
 def oracle_sample(cfg_id, n_sectors_sample, frame=0):
@@ -152,7 +172,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--path", default="fused", choices=["fused", "general"])
@@ -203,6 +223,7 @@ def main():
         for d, n, o, s in zip(dev_digits, n_digits, outs, stats):
             finder.run(d, n, flags=flags, clusters=o, status=s)
 
+    sampler = ClockSampler(local_rank).start()
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
@@ -219,7 +240,7 @@ def main():
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
-    with ClockSampler(local_rank) as clocks:
+    with sampler as clocks:
         ev0.record()
         for _ in range(args.steps):
             step()

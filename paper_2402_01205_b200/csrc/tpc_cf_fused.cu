@@ -205,7 +205,9 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         __syncwarp();
         if (p < blo || p >= bhi) return;                    // a line outside the plane / the halo: stays empty
         const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
-        uint16_t* pre = reinterpret_cast<uint16_t*>(slot + rg.wpl + rg.cap);
+        // 32-bit shared-window addresses for the bitmap and the rank directory (red.shared / st.shared below)
+        const uint32_t a_bm = (uint32_t)__cvta_generic_to_shared(slot);
+        const uint32_t a_pre = a_bm + 4u * (rg.wpl + rg.cap);
         const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
         const bool owner = p >= pa && p < pb;
         uint32_t* sbm = slot + rg.wpl + rg.cap + rg.pre_words;   // stage-A result: one bit per digit index < cap
@@ -226,6 +228,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             return __ldg(&digits[lbeg + jl].x);
         };
         uint32_t carry = 0;                                 // tq word of the digit before this chunk
+        uint32_t mysbm = 0u;
         uint32_t xn = load_x(lane);                         // both words are loaded one chunk ahead
         uint32_t yn = load_y(lane);
         for (uint32_t c0 = 0; c0 < len; c0 += 32) {
@@ -244,21 +247,25 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             const bool first = (jl == 0);
             const bool ok = act && (dx & 0x00ffffffu) == w0_line;
             if (act && (!ok || (!first && pt >= t))) bad_order = true;   // wrong line, not ascending, or duplicate cell
-            const bool badd = ok && owner && (t >= (uint32_t)T || q == 0u);
-            const unsigned mbad = __ballot_sync(0xffffffffu, badd);
-            if (mbad != 0u && lane == 0) atomicAdd(&cnt->n_bad, (unsigned long long)__popc(mbad));
             const bool valid = ok && t < (uint32_t)T;
+            const unsigned mbad = __ballot_sync(0xffffffffu, ok && (!valid || q == 0u));   // R11, rare
+            if (mbad != 0u && owner && lane == 0) atomicAdd(&cnt->n_bad, (unsigned long long)__popc(mbad));
             if (valid) {
                 const uint32_t bw = (t + 32u) >> 5;
-                atomicOr(&slot[bw], 1u << (t & 31u));
-                if (first || ((pt + 32u) >> 5) != bw) pre[bw] = (uint16_t)jl;
+                asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(a_bm + 4u * bw), "r"(1u << (t & 31u)) : "memory");
+                if (first || ((pt + 32u) >> 5) != bw)
+                    asm volatile("st.shared.u16 [%0], %1;" ::"r"(a_pre + 2u * bw), "h"((unsigned short)jl) : "memory");
             }
             // K2 stage A, done here because only the line itself is needed: the neighbours in time are the adjacent
             // digits of the line (an absent one reads as charge 0).  R1: (0,-1) strict, (0,+1) >=
             const uint32_t qm = (pt + 1u == t && !first) ? (prevy >> 16) : 0u;
             const uint32_t qp = ((nexty & 0xffffu) == t + 1u && t + 1u < (uint32_t)T) ? (nexty >> 16) : 0u;
             const unsigned sm = __ballot_sync(0xffffffffu, valid && q >= q_peak_min && q > qm && q >= qp);
-            if (lane == 0 && c0 < rg.cap) sbm[c0 >> 5] = sm;
+            if ((uint32_t)lane == ((c0 >> 5) & 31u)) mysbm = sm;            // lane k keeps the word of chunk k (mod 32)
+            if (((c0 >> 5) & 31u) == 31u || c0 + 32u >= len) {              // flush 32 chunk words at a time
+                const uint32_t wbase = (c0 >> 5) & ~31u;
+                if (wbase + lane <= (c0 >> 5) && wbase + lane < (rg.cap >> 5)) sbm[wbase + lane] = mysbm;
+            }
         }
     };
 
