@@ -356,7 +356,30 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         const uint32_t* sbm = sp + rg.wpl + rg.cap + rg.pre_words;
         const uint32_t nstaged = min(len, rg.cap);
         auto enqueue = [&](bool surv, uint32_t jl) { enqueue_m(__ballot_sync(0xffffffffu, surv), jl); };
-        for (uint32_t c0 = 0; c0 < nstaged; c0 += 32) enqueue_m(sbm[c0 >> 5], c0 + lane);
+        {   // expand all stage-A words at once: lane k owns word k (cap <= 1024 => at most 32 words); prefix sums of
+            // the popcounts give every lane its place in the list, then stage B runs over dense groups of 32
+            const uint32_t nw = (nstaged + 31u) >> 5;
+            uint32_t word = (uint32_t)lane < nw ? sbm[lane] : 0u;
+            const uint32_t cw = (uint32_t)__popc(word);
+            uint32_t inc = cw;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += u;
+            }
+            const uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
+            uint16_t* lst = reinterpret_cast<uint16_t*>(rg.sm + kSlots * rg.slot_words + kWarps * rg.cap) +
+                            (size_t)warp * (rg.cap + 32);         // every staged digit may survive
+            uint32_t o = inc - cw;
+            while (word) {
+                const uint32_t b = (uint32_t)__ffs(word) - 1u;
+                word &= word - 1u;
+                lst[o++] = (uint16_t)(32u * lane + b);
+            }
+            __syncwarp();
+            for (uint32_t i = 0; i < total; i += 32)
+                stage_b(i + lane < total, i + lane < total ? (uint32_t)lst[i + lane] : 0u);
+        }
         // tail of a line longer than cap: the own-line test from the digit array
         uint32_t carry = nstaged < len ? fetch(sp, gl, nstaged - 1) : 0u;
         for (uint32_t c0 = nstaged; c0 < len; c0 += 32) {
@@ -420,13 +443,14 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t pre_words = ((wpl >> 1) + 3u) & ~3u;
     uint32_t cap = ((uint32_t)(mean_len * 1.5) + 64u + 127u) & ~127u;
     const uint32_t max_smem = 106 * 1024;                    // 2 CTAs per SM (+ ~5 KB static + 1 KB reserved each)
-    const uint32_t fixed = kSlots * (wpl + pre_words) * 4;
-    const uint32_t per_cap0 = kSlots * 4 + kSlots / 8 + 1 + kWarps * 4;
+    const uint32_t fixed = kSlots * (wpl + pre_words) * 4 + kWarps * 64;
+    const uint32_t per_cap0 = kSlots * 4 + kSlots / 8 + 1 + kWarps * 4 + kWarps * 2;   // tq, stage-A bit, key staging, survivor list
     if (fixed + per_cap0 * 128 > 200 * 1024) return TPC_CF_E_GEOMETRY;   // cannot happen for n_time <= 65535
     const uint32_t limit = fixed + per_cap0 * 128 <= max_smem ? max_smem : 200 * 1024;
-    const uint32_t per_cap = kSlots * 4 + kSlots / 8 + 1 + kWarps * 4;   // bytes per unit of cap: tq word + stage-A bit + key staging
+    const uint32_t per_cap = per_cap0;
+    if (cap > 1024u) cap = 1024u;                            // the stage-A words of a line must fit one warp (32 words)
     if (fixed + per_cap * cap > limit) cap = ((limit - fixed) / per_cap) & ~127u;
-    const uint32_t smem = fixed + kSlots * (cap * 4 + (cap >> 5) * 4) + kWarps * cap * 4;
+    const uint32_t smem = fixed + kSlots * (cap * 4 + (cap >> 5) * 4) + kWarps * cap * 4 + kWarps * (cap + 32) * 2;
     // One CTA per whole plane when there are enough planes to fill the GPU (no halo lines, one prologue per plane:
     // measured 2.94 ms vs 3.16 ms at 48 pads on config 3); smaller pad ranges for small problems.
     const uint32_t whole = (g.max_pads + kS - 1) / kS * kS;
