@@ -109,23 +109,30 @@ k_gather(const uint32_t* __restrict__ peakmask, uint64_t nwords, const uint32_t*
          const uint4* __restrict__ stage, uint4* out, uint64_t capacity, uint4* compact, uint64_t max_clusters,
          int sort_if_unsorted, const Counters* cnt)
 {
+    // A block owns 256 mask words = 8192 digits.  Its peaks are first listed in shared memory in output order
+    // (local digit index), then copied by all threads: independent 32-byte loads, fully coalesced stores.
+    __shared__ uint16_t s_list[kCompactThreads * 32];
+    __shared__ uint32_t s_count;
     const uint64_t w = (uint64_t)blockIdx.x * kCompactThreads + threadIdx.x;
     uint32_t m = w < nwords ? peakmask[w] : 0u;
-    const uint32_t ex = block_exclusive_scan((uint32_t)__popc(m), nullptr);
-    uint4* dst = out;
-    uint64_t cap = capacity;
-    if (sort_if_unsorted && cnt->unsorted) { dst = compact; cap = max_clusters; }
-    uint64_t pos = (uint64_t)blk_off[blockIdx.x] + ex;
+    uint32_t pos = block_exclusive_scan((uint32_t)__popc(m), &s_count);
     while (m) {
         const int b = __ffs(m) - 1;
         m &= m - 1;
-        const uint64_t j = w * 32 + b;
-        if (pos < cap) {
-            const uint4 lo = __ldcs(stage + 2 * j), hi = __ldcs(stage + 2 * j + 1);
-            __stcs(dst + 2 * pos, lo);
-            __stcs(dst + 2 * pos + 1, hi);
-        }
-        ++pos;
+        s_list[pos++] = (uint16_t)(threadIdx.x * 32 + b);
+    }
+    __syncthreads();
+    uint4* dst = out;
+    uint64_t cap = capacity;
+    if (sort_if_unsorted && cnt->unsorted) { dst = compact; cap = max_clusters; }
+    const uint64_t base = blk_off[blockIdx.x];
+    const uint64_t j0 = (uint64_t)blockIdx.x * kCompactThreads * 32;
+    const uint32_t total = s_count;
+    // two 16-byte halves per record: thread pairs (2i, 2i+1) move one record, so a warp writes 512 contiguous bytes
+    for (uint32_t i = threadIdx.x; i < 2 * total; i += kCompactThreads) {
+        const uint32_t r = i >> 1, h = i & 1u;
+        const uint64_t p = base + r;
+        if (p < cap) __stcs(dst + 2 * p + h, __ldcs(stage + 2 * (j0 + s_list[r]) + h));
     }
 }
 
