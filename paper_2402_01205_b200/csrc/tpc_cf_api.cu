@@ -77,7 +77,9 @@ static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, ch
     w.ghist = (uint32_t*)take((size_t)tiles * 256 * 4);
     w.ghist_part = (uint32_t*)take((ceil_div_u64(tiles * 256, 1024) + 1) * 4);
     w.line_start = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
-    w.ovf = (uint32_t*)take((size_t)max_digits * 4);
+    w.line_cnt = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
+    w.line_off = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
+    w.line_part = (uint32_t*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 1024) + 1) * 4);
     if (ws) *ws = w;
     if (n_sort_tiles) *n_sort_tiles = (uint32_t)tiles;
     if (map_bytes) *map_bytes = mapb;
@@ -170,7 +172,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
                                     prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
         if (r < 0) return r;
         k += r;
-        k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, 0, st);
+        k += launch_compact_lines(h->geo, h->ws, out->clusters, out->capacity, st);
         k += launch_finalize(h->ws, out->status, out->capacity, 3u, 1, n, st);
     } else {
         // T1: K1 scatter -> K2+K4 digit-centric peaks + moments on the HBM map -> K3 compaction -> (K5 key sort)

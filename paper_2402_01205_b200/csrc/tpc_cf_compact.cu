@@ -150,6 +150,35 @@ int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t c
     return k + 1;
 }
 
+// ---- K3 + K5 for the fused path: the peaks of a line are already packed, in time order, at the start of the
+// line's own digit range in `stage`; a scan over the per-line counts gives each line its place in the output.
+__global__ void __launch_bounds__(256)
+k_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __restrict__ line_off,
+               const uint32_t* __restrict__ line_start, uint32_t n_lines, const uint4* __restrict__ stage,
+               uint4* __restrict__ out, uint64_t capacity)
+{
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t line = blockIdx.x * 8 + (threadIdx.x >> 5);          // one warp per line
+    if (line >= n_lines) return;
+    const uint32_t c = line_cnt[line];
+    if (c == 0) return;
+    const uint64_t dst = line_off[line];
+    const uint64_t src = line_start[line];
+    for (uint32_t i = lane; i < 2 * c; i += 32) {                       // 16-byte halves: contiguous on both sides
+        const uint64_t r = i >> 1;
+        if (dst + r < capacity) __stcs(out + 2 * dst + i, __ldcs(stage + 2 * src + i));
+    }
+}
+
+int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, uint64_t capacity, cudaStream_t st)
+{
+    const uint32_t n_lines = g.n_planes * g.LS;
+    int k = launch_scan_u32(ws.line_cnt, ws.line_off, n_lines, ws.line_part, &ws.counters->n_clusters, st);
+    k_gather_lines<<<(n_lines + 7) / 8, 256, 0, st>>>(ws.line_cnt, ws.line_off, ws.line_start, n_lines,
+                                                      (const uint4*)ws.stage, (uint4*)out, capacity);
+    return k + 1;
+}
+
 // ---- K5 for unsorted input: LSD radix sort of (key40, index), 8 bits per pass, warp-private tiles -------------
 static constexpr int kSortTile = 2048;     // elements per warp
 static constexpr int kSortWarps = 8;

@@ -15,8 +15,8 @@
 //                               gated sums, record -> stage[j]
 //                  Step = 8 lines, one barrier: each warp prefetches (cp.async) the line it will build, runs A+B+C on
 //                  its current line, then rebuilds the slot of a line that left the ring.
-//                  Peaks are recorded as one bit per digit (peakmask) and their cluster at stage[j]; the shared
-//                  compaction (tpc_cf_compact.cu) turns that into the ordered output (K3, K5).
+//                  The k-th peak of a line (time order) goes to stage[line_start + k] and the line's peak count to
+//                  line_cnt[]; a scan over the line counts and a per-line copy give the ordered output (K3, K5).
 //   The DIGITS_SORTED promise is verified here for free: every digit is checked once against the line (or gap) it
 //   was found in; any violation raises Counters::unsorted and the run reports path 0.
 #include <stdlib.h>
@@ -111,7 +111,7 @@ __device__ __forceinline__ void window(const Ring& rg, const uint32_t* __restric
 __global__ void __launch_bounds__(kFThreads, 2)
 k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
               uint32_t pads_per_unit, uint32_t units_per_plane, uint32_t wpl, uint32_t cap,
-              uint32_t q_peak_min, uint32_t q_gate, Counters* cnt, uint32_t* __restrict__ peakmask,
+              uint32_t q_peak_min, uint32_t q_gate, Counters* cnt, uint32_t* __restrict__ line_cnt,
               uint4* __restrict__ stage)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -272,14 +272,14 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     // ---- K4 (stage C): 5x5 window from the slots of lines p-2..p+2, gated sums, record -> stage[j] ----------------
     // vp = ring index of line p.  Slots of lines outside the plane are empty (R2).
     // sl[a] / gls[a]: slot and first-digit index of line p+a-2 (warp-uniform: a warp's peaks are all on its line)
-    auto moments = [&](int p, uint32_t jl, const uint32_t* const (&sl)[5], const uint32_t (&gls)[5]) {
+    auto moments = [&](int p, uint32_t jl, uint32_t k, const uint32_t* const (&sl)[5], const uint32_t (&gls)[5]) {
         const uint32_t self = fetch(sl[2], gls[2], jl);
         const int t = (int)(self & 0xffffu);
         int c[5][5];
 #pragma unroll
         for (int a = 0; a < 5; ++a) window<2>(rg, sl[a], digits, gls[a], n, t, c[a]);
         const ClusterWords r = cluster_from_window(c, w0_base | ((uint32_t)p << 16), (uint32_t)t, q_gate);
-        const size_t j = (size_t)gls[2] + jl;
+        const size_t j = (size_t)gls[2] + k;     // k-th peak of the line: packed at the start of the line's range
         stage[2 * j] = r.lo;
         stage[2 * j + 1] = r.hi;
     };
@@ -287,7 +287,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     // ---- K2: stages A and B for line p (ring index vp), owned by this warp; lo = p - l0 ------------------------------
     auto stage_ab = [&](int p, int vp) {
         const uint32_t gl = s_ls[p], len = s_ls[p + 1] - gl;
-        if (len == 0) return;
+        if (len == 0) { if (lane == 0) line_cnt[plane * g.LS + p] = 0u; return; }
         const uint32_t* sl[5];
         uint32_t gls[5];
 #pragma unroll
@@ -301,7 +301,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         const uint32_t glm = gls[1], glp = gls[3];
         uint32_t* wq = s_wq[warp];
         uint32_t* pq = s_pq[warp];
-        uint32_t pcount = 0;                                    // warp-uniform
+        uint32_t pcount = 0, pdone = 0;                         // warp-uniform: queued / already written peaks
 
         auto stage_b = [&](bool act, uint32_t jl) {
             bool peak = false;
@@ -319,15 +319,12 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             // peaks -> this warp's peak queue; stage C runs on every full 32 (dense lanes) and once at the end
             const unsigned pm = __ballot_sync(0xffffffffu, peak);
             if (pm == 0) return;
-            if (peak) {
-                const uint32_t j = gl + jl;
-                atomicOr(&peakmask[j >> 5], 1u << (j & 31u));
-                pq[pcount + (uint32_t)__popc(pm & ((1u << lane) - 1u))] = jl;
-            }
+            if (peak) pq[pcount + (uint32_t)__popc(pm & ((1u << lane) - 1u))] = jl;
             pcount += (uint32_t)__popc(pm);
             __syncwarp();
             if (pcount >= 32u) {
-                moments(p, pq[lane], sl, gls);
+                moments(p, pq[lane], pdone + lane, sl, gls);
+                pdone += 32u;
                 const uint32_t mv = (lane + 32u < pcount) ? pq[lane + 32u] : 0u;
                 __syncwarp();
                 if (lane + 32u < pcount) pq[lane] = mv;
@@ -398,7 +395,8 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             enqueue(act && q >= q_peak_min && t < T && q > qm && q >= qp, jl);   // R1: (0,-1) strict, (0,+1) >=
         }
         if (wcount) stage_b((uint32_t)lane < wcount, (uint32_t)lane < wcount ? wq[lane] : 0u);
-        if ((uint32_t)lane < pcount) moments(p, pq[lane], sl, gls);
+        if ((uint32_t)lane < pcount) moments(p, pq[lane], pdone + lane, sl, gls);
+        if (lane == 0) line_cnt[plane * g.LS + p] = pdone + pcount;   // peaks of this line, in time order
     };
 
     // ---- main loop -------------------------------------------------------------------------------------------------
@@ -427,10 +425,10 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
+    cudaMemsetAsync(ws.line_cnt, 0, ((size_t)g.n_planes * g.LS + 1) * 4, st);   // pads beyond npads[row] stay 0
     if (n == 0) return 0;
     int k = 0;
     const uint32_t entries = g.n_planes * g.LS + 1;
-    cudaMemsetAsync(ws.peakmask, 0, (size_t)ceil_div_u64(n, 32) * 4, st);
     k_line_index<<<(entries + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start);
     ++k;
 
@@ -470,7 +468,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     if (ev_k0) cudaEventRecord(ev_k0, st);
     k_fused_lines<<<g.n_planes * upp, kFThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
                                                              pads_per_unit, upp, wpl, cap, q_peak_min, q_gate,
-                                                             ws.counters, ws.peakmask, (uint4*)ws.stage);
+                                                             ws.counters, ws.line_cnt, (uint4*)ws.stage);
     if (ev_k1) cudaEventRecord(ev_k1, st);
     return k + 1;
 }

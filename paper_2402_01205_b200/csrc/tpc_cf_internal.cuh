@@ -26,7 +26,7 @@ struct Counters {
     unsigned long long n_used;
     unsigned long long n_clusters;  // total peaks
     unsigned int unsorted;          // 1 if digits[i-1] > digits[i] for some i (key = sector,row,pad,time)
-    unsigned int n_ovf;             // fused path: peaks routed to the exact slow path (k_fused_overflow)
+    unsigned int rsv;
 };
 
 // Pointers into the caller-owned workspace.
@@ -44,7 +44,9 @@ struct Workspace {
     uint32_t* ghist;      // [256][n_sort_tiles]
     uint32_t* ghist_part;
     uint32_t* line_start; // [n_planes*LS + 1] first digit of each (plane,pad) line (fused path)
-    uint32_t* ovf;        // [max_digits] digit indices of peaks handled by k_fused_overflow
+    uint32_t* line_cnt;   // [n_planes*LS + 1] peaks per line (fused path)
+    uint32_t* line_off;   // exclusive scan of line_cnt
+    uint32_t* line_part;  // scan partials for the line counts
 };
 
 struct Handle;
@@ -130,6 +132,8 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
 // compaction of stage[j] by peakmask into dst (= out, or ws.compact when a key sort must follow)
 int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t capacity, uint64_t max_clusters,
                    int sort_if_unsorted, cudaStream_t st);
+// fused path: scan of ws.line_cnt, then one warp per line copies stage[line_start + k] -> out[line_off + k]
+int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, uint64_t capacity, cudaStream_t st);
 int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_tiles, tpc_cluster* out,
                     uint64_t capacity, cudaStream_t st);
 int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,
