@@ -157,16 +157,32 @@ k_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __restrict
                const uint32_t* __restrict__ line_start, uint32_t n_lines, const uint4* __restrict__ stage,
                uint4* __restrict__ out, uint64_t capacity)
 {
-    const uint32_t lane = threadIdx.x & 31;
-    const uint32_t line = blockIdx.x * 8 + (threadIdx.x >> 5);          // one warp per line
-    if (line >= n_lines) return;
-    const uint32_t c = line_cnt[line];
-    if (c == 0) return;
-    const uint64_t dst = line_off[line];
-    const uint64_t src = line_start[line];
-    for (uint32_t i = lane; i < 2 * c; i += 32) {                       // 16-byte halves: contiguous on both sides
-        const uint64_t r = i >> 1;
-        if (dst + r < capacity) __stcs(out + 2 * dst + i, __ldcs(stage + 2 * src + i));
+    // A block owns 256 consecutive lines; their records are consecutive in the output, so the block copies
+    // one contiguous output range: every thread moves 16-byte halves, finding the source line of a record by a
+    // binary search in the block's prefix sums (shared memory).
+    __shared__ uint32_t s_pref[257];
+    __shared__ uint32_t s_src[256];
+    const uint32_t line = blockIdx.x * 256 + threadIdx.x;
+    const uint32_t c = line < n_lines ? line_cnt[line] : 0u;
+    uint32_t total;
+    {
+        __shared__ uint32_t s_total;
+        const uint32_t ex = block_exclusive_scan(c, &s_total);
+        s_pref[threadIdx.x] = ex;
+        s_src[threadIdx.x] = line < n_lines ? line_start[line] : 0u;
+        __syncthreads();
+        total = s_total;
+        if (threadIdx.x == 0) s_pref[256] = total;
+    }
+    __syncthreads();
+    if (total == 0) return;
+    const uint64_t dst0 = line_off[blockIdx.x * 256];
+    for (uint32_t i = threadIdx.x; i < 2 * total; i += 256) {
+        const uint32_t r = i >> 1;
+        uint32_t lo = 0, hi = 256;                       // last line with s_pref[line] <= r
+        while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (s_pref[mid] <= r) lo = mid; else hi = mid; }
+        const uint64_t src = (uint64_t)s_src[lo] + (r - s_pref[lo]);
+        if (dst0 + r < capacity) __stcs(out + 2 * (dst0 + r) + (i & 1u), __ldcs(stage + 2 * src + (i & 1u)));
     }
 }
 
@@ -174,7 +190,7 @@ int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, ui
 {
     const uint32_t n_lines = g.n_planes * g.LS;
     int k = launch_scan_u32(ws.line_cnt, ws.line_off, n_lines, ws.line_part, &ws.counters->n_clusters, st);
-    k_gather_lines<<<(n_lines + 7) / 8, 256, 0, st>>>(ws.line_cnt, ws.line_off, ws.line_start, n_lines,
+    k_gather_lines<<<(n_lines + 255) / 256, 256, 0, st>>>(ws.line_cnt, ws.line_off, ws.line_start, n_lines,
                                                       (const uint4*)ws.stage, (uint4*)out, capacity);
     return k + 1;
 }

@@ -1,6 +1,6 @@
 // tpc_cf_fused.cu — fused path ("T3") for digits sorted by (sector,row,pad,time): the charge map never exists in HBM.
 //
-//   k_line_index   lower_bound of every (plane,pad) line in the digit array -> ws.line_start
+//   k_plane_index, k_line_index   two-level lower_bound of every (plane,pad) line in the digit array -> ws.line_start
 //   k_fused_lines  one CTA (8 warps) per (plane, pad range).  The pad lines of the range stream through a ring of line
 //                  slots in shared memory.  A line slot is one line of the charge map in compressed form:
 //                     bm[w]   presence bitmap over time bins (bit t+32; guard words = zero border in time, R2)
@@ -35,22 +35,41 @@ __device__ __forceinline__ uint32_t key24_of(uint32_t w0)
     return ((w0 & 0xffu) << 16) | (w0 & 0xff00u) | ((w0 >> 16) & 0xffu);
 }
 
-__global__ void __launch_bounds__(256)
-k_line_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start)
+// lower_bound of a 24-bit (sector,row,pad) key in digits[lo, hi)
+__device__ __forceinline__ uint32_t lower_bound_key(const uint2* __restrict__ digits, uint32_t lo, uint32_t hi,
+                                                    uint32_t target)
 {
-    const uint32_t total = g.n_planes * g.LS + 1;
-    const uint32_t e = blockIdx.x * 256 + threadIdx.x;
-    if (e >= total) return;
-    if (e == total - 1) { line_start[e] = n; return; }
-    const uint32_t plane = e / g.LS, p = e % g.LS;
-    const uint32_t s = plane / g.n_rows, r = plane % g.n_rows;
-    const uint32_t target = (s << 16) | (r << 8) | p;
-    uint32_t lo = 0, hi = n;
     while (lo < hi) {
         const uint32_t mid = lo + ((hi - lo) >> 1);
         if (key24_of(__ldg(&digits[mid].x)) < target) lo = mid + 1; else hi = mid;
     }
-    line_start[e] = lo;
+    return lo;
+}
+
+// level 1: first digit of every plane (entry p = 0 of each plane; the final entry is n)
+__global__ void __launch_bounds__(256)
+k_plane_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start)
+{
+    const uint32_t plane = blockIdx.x * 256 + threadIdx.x;
+    if (plane > g.n_planes) return;
+    if (plane == g.n_planes) { line_start[(size_t)g.n_planes * g.LS] = n; return; }
+    const uint32_t s = plane / g.n_rows, r = plane % g.n_rows;
+    line_start[(size_t)plane * g.LS] = lower_bound_key(digits, 0, n, (s << 16) | (r << 8));
+}
+
+// level 2: the lines of a plane, searched inside the plane's own range
+__global__ void __launch_bounds__(256)
+k_line_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start)
+{
+    const uint32_t total = g.n_planes * g.LS;
+    const uint32_t e = blockIdx.x * 256 + threadIdx.x;
+    if (e >= total) return;
+    const uint32_t plane = e / g.LS, p = e % g.LS;
+    if (p == 0) return;                                   // written by k_plane_index
+    const uint32_t s = plane / g.n_rows, r = plane % g.n_rows;
+    uint32_t lo = line_start[(size_t)plane * g.LS], hi = line_start[(size_t)(plane + 1) * g.LS];
+    if (hi < lo || hi > n) { lo = 0; hi = n; }            // unsorted input: stay in bounds, the fused kernel reports it
+    line_start[e] = lower_bound_key(digits, lo, hi, (s << 16) | (r << 8) | p);
 }
 
 // Slot layout (warp-uniform).
@@ -429,8 +448,9 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     if (n == 0) return 0;
     int k = 0;
     const uint32_t entries = g.n_planes * g.LS + 1;
+    k_plane_index<<<(g.n_planes + 1 + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start);
     k_line_index<<<(entries + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start);
-    ++k;
+    k += 2;
 
     // launch shape: pad range per unit, tq capacity per slot from the mean line length (host-known)
     uint64_t total_pads = 0;
