@@ -1,0 +1,439 @@
+// tpc_cf_blocks.cu — fused path, block-sparse line slots ("T3b"): same streaming scheme as tpc_cf_fused.cu (one CTA per
+// (plane, pad range), one WARP per pad LINE, a ring of line slots in shared memory, one barrier per step of 8 lines),
+// but a line slot holds the line of the charge map as 8-cell blocks instead of a bitmap + rank directory:
+//     hdr      [16 B]   word 0: number of stage-A survivors of the line
+//     dir[b]   uint8    pool index of the block of time bins 8b-8 .. 8b-1 (0 = the all-zero block, 0xFF = the line has
+//                       this block but the pool was full: the cell is then looked up in the digit array)
+//     pool[i]  16 B     eight uint16 charges; block 0 stays zero (zero border in time and empty cells, R2)
+//     surv[k]  uint32   (time | charge << 16) of the k-th digit that passed the own-line test (stage A), time order
+// A cell lookup is dir byte -> 16-bit load, without bit counting or divergence; a 3- or 5-cell window costs two dir
+// bytes and 3 / 5 charge loads.  Digits stream through a per-warp staging ring of four 32-digit chunks (cp.async),
+// so a line of any length is handled by the same code.
+//   K0  the warp that reuses a slot zeroes its dir + pool          K1  build: block allocation by ballot/popc
+//   K2  stage A at build time (shuffles), stage B from the survivor list against lines p-1 / p+1
+//   K4  stage C: peaks queued per warp, 5x5 window from the five slots p-2..p+2 -> stage[line_start + k]
+// Selected by launch_fused_sorted when the mean line fits the block pool (<= 254 blocks); otherwise the bitmap
+// kernel of tpc_cf_fused.cu runs.  Definition: include/tpc_cf.h (BASELINE.json:north_star; step named in PAPER.md:57).
+#include <stdlib.h>
+
+#include "tpc_cf_internal.cuh"
+
+namespace tpccf {
+
+static constexpr int kBThreads = 256;
+static constexpr int kBWarps = kBThreads / 32;
+static constexpr int kBS = kBWarps;              // lines per step: one per warp
+static constexpr int kBSlots = 2 * kBS + 4;      // lines l0-2 .. l0+S+1 in use, next S being built
+static constexpr int kStageDepth = 4;            // staging ring: chunks of 32 digits (256 B each) per warp
+static constexpr uint32_t kDirOff = 16;          // dir starts after the header
+
+// ---- shared-window accessors (32-bit addresses: no generic-address arithmetic in the hot loops) ------------------
+__device__ __forceinline__ uint32_t lds32(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint2 lds64(uint32_t a)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds16(uint32_t a)
+{
+    uint16_t v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds8(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts32(uint32_t a, uint32_t v)
+{
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ void sts16(uint32_t a, uint32_t v)
+{
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((uint16_t)v) : "memory");
+}
+__device__ __forceinline__ void sts8(uint32_t a, uint32_t v)
+{
+    asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ void sts128z(uint32_t a)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");
+}
+
+// ring index of the line at distance d (|d| < kBSlots) from the line whose ring index is v0
+__device__ __forceinline__ int bring_at(int v0, int d)
+{
+    int v = v0 + d;
+    v += (v < 0) ? kBSlots : 0;
+    v -= (v >= kBSlots) ? kBSlots : 0;
+    return v;
+}
+
+// K2 stage A (R1, own line): the neighbours in time are the adjacent digits of the line; an absent one reads 0.
+// (0,-1) is lexicographically earlier: strict; (0,+1) later: >=.
+__device__ __forceinline__ bool stage_a(uint32_t y, uint32_t prevy, bool has_prev, uint32_t nexty, bool has_next,
+                                        uint32_t T, uint32_t q_peak_min)
+{
+    const uint32_t t = y & 0xffffu, q = y >> 16;
+    const uint32_t qm = (has_prev && (prevy & 0xffffu) + 1u == t) ? (prevy >> 16) : 0u;
+    const uint32_t qp = (has_next && (nexty & 0xffffu) == t + 1u && t + 1u < T) ? (nexty >> 16) : 0u;
+    return q >= q_peak_min && q > qm && q >= qp;
+}
+
+// charge of cell (line, tt) from the digit array (slow path: the line's block pool was full).  Binary search on time.
+// Cells outside [0, T) read 0 (R2) whatever the digit array holds there (a digit with time >= T is invalid, R11).
+__device__ __noinline__ uint32_t cell_from_digits(const uint2* __restrict__ digits, uint32_t gl, uint32_t glen,
+                                                  uint32_t tt, uint32_t T)
+{
+    if (tt >= T) return 0u;
+    uint32_t lo = 0, hi = glen;
+    while (lo < hi) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        if ((__ldg(&digits[gl + mid].y) & 0xffffu) < tt) lo = mid + 1; else hi = mid;
+    }
+    if (lo >= glen) return 0u;
+    const uint32_t y = __ldg(&digits[gl + lo].y);
+    return (y & 0xffffu) == tt ? (y >> 16) : 0u;
+}
+
+// Slot geometry (kernel parameters; all warp-uniform).
+struct SlotGeo {
+    uint32_t slot_bytes;   // multiple of 16
+    uint32_t pool_off;     // kDirOff + dir bytes (multiple of 16)
+    uint32_t surv_off;     // pool_off + 16 * pcap
+    uint32_t pcap;         // blocks in the pool including the zero block 0 (<= 255)
+    uint32_t scap;         // survivor entries per slot
+};
+
+// charges of the window t-H..t+H of the line in slot `slot` (0 where no digit): c[k] is time t-H+k.
+// lidx = pad index of that line, used only by the slow path (line_start lookups in s_ls).
+template <int H>
+__device__ __forceinline__ void bwindow(uint32_t slot, const SlotGeo& sg, int t, int (&c)[2 * H + 1],
+                                        const uint2* __restrict__ digits, const uint32_t* s_ls, int lidx, int P,
+                                        uint32_t T)
+{
+    const uint32_t u = (uint32_t)(t + 8 - H);                 // first cell, shifted by the 8-bin guard block
+    const uint32_t dA = lds8(slot + kDirOff + (u >> 3));
+    const uint32_t dB = lds8(slot + kDirOff + ((u + 2 * H) >> 3));
+    const uint32_t o = u & 7u;
+    const uint32_t base = slot + sg.pool_off + 2u * o;
+    const uint32_t aA = base + (dA << 4), aB = base + (dB << 4) - 16u;
+    if (dA != 0xFFu && dB != 0xFFu) {
+#pragma unroll
+        for (int k = 0; k < 2 * H + 1; ++k) c[k] = (int)lds16((o + (uint32_t)k < 8u ? aA : aB) + 2u * (uint32_t)k);
+    } else {                                                   // rare: a block of this window is not in the pool
+        const bool inside = lidx >= 0 && lidx < P;
+        const uint32_t gl = inside ? s_ls[lidx] : 0u;
+        const uint32_t glen = inside ? s_ls[lidx + 1] - gl : 0u;
+#pragma unroll
+        for (int k = 0; k < 2 * H + 1; ++k) {
+            const bool inA = o + (uint32_t)k < 8u;
+            const uint32_t d = inA ? dA : dB;
+            c[k] = d != 0xFFu ? (int)lds16((inA ? aA : aB) + 2u * (uint32_t)k)
+                              : (int)cell_from_digits(digits, gl, glen, (uint32_t)(t - H + k), T);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kBThreads, 2)
+k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
+               uint32_t pads_per_unit, uint32_t units_per_plane, SlotGeo sg, uint32_t q_peak_min, uint32_t q_gate,
+               Counters* cnt, uint32_t* __restrict__ line_cnt, uint4* __restrict__ stage)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ uint32_t s_ls[260];          // line starts of this plane: s_ls[p], p = 0..max_pads, then next plane's start
+    __shared__ int s_unsorted;
+
+    const uint32_t plane = blockIdx.x / units_per_plane, unit = blockIdx.x % units_per_plane;
+    const uint32_t sector = plane / g.n_rows, row = plane % g.n_rows;
+    const int P = (int)g.npads[row];
+    const int pa = (int)(unit * pads_per_unit);
+    const int pb = min(pa + (int)pads_per_unit, P);
+    const uint32_t T = g.n_time;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t w0_base = sector | (row << 8);
+    const uint32_t lt_mask = (1u << lane) - 1u;
+
+    const uint32_t sm0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    const uint32_t stg = sm0 + kBSlots * sg.slot_bytes + (uint32_t)warp * (kStageDepth * 256u);   // staging ring
+    const uint32_t pqa = sm0 + kBSlots * sg.slot_bytes + kBWarps * (kStageDepth * 256u) + (uint32_t)warp * 256u;
+
+    for (int i = tid; i <= (int)g.LS; i += kBThreads) s_ls[i] = line_start[plane * g.LS + i];
+    if (tid == 0) s_unsorted = 0;
+    // every slot starts as an empty line (lines outside the plane keep this state: zero border in pad, R2)
+    for (uint32_t x = (uint32_t)tid * 16u; x < kBSlots * sg.slot_bytes; x += kBThreads * 16u) sts128z(sm0 + x);
+    __syncthreads();
+
+    if (pa >= P && unit != 0) return;    // nothing in this pad range (rows with fewer pads)
+
+    bool bad_order = false;
+    // monotone line starts: a garbage index from unsorted input must not produce negative lengths or unbounded work
+    for (int i = tid; i < (int)g.LS; i += kBThreads) if (s_ls[i] > s_ls[i + 1]) bad_order = true;
+    if (__syncthreads_or(bad_order ? 1 : 0)) {
+        if (tid == 0) atomicOr(&cnt->unsorted, 1u);
+        return;
+    }
+
+    // gap of the plane: digits with pad >= npads[row] (or a row/sector beyond the geometry) — all invalid (R11)
+    if (unit == 0) {
+        const uint32_t gb = s_ls[P], ge = s_ls[g.LS];
+        if (ge > gb) {
+            for (uint32_t j = gb + tid; j < ge; j += kBThreads) {
+                const uint2 d = __ldg(digits + j);
+                if (digit_valid(g, d.x, d.y)) bad_order = true;     // a valid digit outside every line: not sorted
+            }
+            if (tid == 0) atomicAdd(&cnt->n_bad, (unsigned long long)(ge - gb));
+        }
+    }
+
+    const int blo = max(pa - 2, 0), bhi = min(P, pb + 2);   // lines this unit ever builds
+
+    // ---- staging: chunk c (digits 32c .. 32c+31) of the line starting at lbeg -> ring entry c mod kStageDepth ------
+    // one commit group per call, empty or not, so that wait_group counts chunks
+    auto stage_chunk = [&](uint32_t lbeg, uint32_t len, uint32_t c) {
+        const uint32_t jl = 32u * c + (uint32_t)lane;
+        if (jl < len) {
+            const uint32_t dst = stg + (c & (kStageDepth - 1)) * 256u + 8u * (uint32_t)lane;
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(digits + lbeg + jl) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    // the first kStageDepth-1 chunks of the line this warp builds next (issued before the warp processes its
+    // current line, so the global latency is covered)
+    auto stage_head = [&](int p) {
+        if (p < blo || p >= bhi) return;
+        const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
+#pragma unroll
+        for (uint32_t c = 0; c < kStageDepth - 1; ++c) stage_chunk(lbeg, len, c);
+    };
+
+    // ---- K0 + K1 + stage A: this warp (re)builds slot v as line p ---------------------------------------------------
+    auto build_line = [&](int p, int v) {
+        const uint32_t slot = sm0 + (uint32_t)v * sg.slot_bytes;
+        for (uint32_t x = (uint32_t)lane * 16u; x < sg.surv_off; x += 512u) sts128z(slot + x);   // hdr, dir, pool
+        __syncwarp();
+        if (p < blo || p >= bhi) return;                    // a line outside the plane / the halo: stays empty
+        const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
+        if (len == 0) return;
+        const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
+        const uint32_t a_dir = slot + kDirOff, a_pool = slot + sg.pool_off, a_surv = slot + sg.surv_off;
+        uint32_t carry = 0u;                                // y of the digit before this chunk
+        uint32_t nblk = 0u, nsurv = 0u;                     // warp-uniform running counts
+        uint32_t nbad = 0u;                                 // per lane
+        const uint32_t nchunks = (len + 31u) >> 5;
+        for (uint32_t c = 0; c < nchunks; ++c) {
+            stage_chunk(lbeg, len, c + kStageDepth - 1);
+            asm volatile("cp.async.wait_group %0;" ::"n"(kStageDepth - 2) : "memory");   // chunks <= c+1 have landed
+            __syncwarp();
+            const uint32_t jl = 32u * c + (uint32_t)lane;
+            const bool act = jl < len;
+            const uint2 d = lds64(stg + (c & (kStageDepth - 1)) * 256u + 8u * (uint32_t)lane);
+            const uint32_t y_next0 = lds32(stg + ((c + 1u) & (kStageDepth - 1)) * 256u + 4u);   // first y of chunk c+1
+            const uint32_t y = d.y;
+            uint32_t prevy = __shfl_up_sync(0xffffffffu, y, 1);
+            uint32_t nexty = __shfl_down_sync(0xffffffffu, y, 1);
+            if (lane == 0) prevy = carry;
+            if (lane == 31) nexty = y_next0;
+            carry = __shfl_sync(0xffffffffu, y, 31);
+            const uint32_t t = y & 0xffffu, pt = prevy & 0xffffu, q = y >> 16;
+            const bool first = jl == 0u;
+            const bool ok = act && (d.x & 0x00ffffffu) == w0_line;
+            if (act && (!ok || (!first && pt >= t))) bad_order = true;   // wrong line, not ascending, or duplicate cell
+            const bool inb = ok && t < T;                   // addresses a cell of this line
+            if (ok && (!inb || q == 0u)) ++nbad;            // R11
+            // K1: blocks are allocated in time order: a digit opens a block iff the digit before it is in another one
+            const uint32_t b = (t + 8u) >> 3;
+            const bool head = inb && (first || ((pt + 8u) >> 3) != b);
+            const unsigned hm = __ballot_sync(0xffffffffu, head);
+            const uint32_t idx = nblk + (uint32_t)__popc(hm & (lt_mask | (1u << lane)));   // 1-based; 0 = zero block
+            nblk += (uint32_t)__popc(hm);
+            const bool in_pool = idx < sg.pcap;
+            if (head) sts8(a_dir + b, in_pool ? idx : 0xFFu);
+            if (inb && in_pool) sts16(a_pool + (idx << 4) + ((t & 7u) << 1), q);
+            // K2 stage A
+            const bool surv = inb && stage_a(y, prevy, !first, nexty, jl + 1u < len, T, q_peak_min);
+            const unsigned smk = __ballot_sync(0xffffffffu, surv);
+            const uint32_t pos = nsurv + (uint32_t)__popc(smk & lt_mask);
+            if (surv && pos < sg.scap) sts32(a_surv + (pos << 2), y);
+            nsurv += (uint32_t)__popc(smk);
+        }
+        if (lane == 0) sts32(slot, nsurv);
+        if (p >= pa && p < pb) {                            // halo lines are counted by the unit that owns them
+            const uint32_t tot = __reduce_add_sync(0xffffffffu, nbad);
+            if (tot != 0u && lane == 0) atomicAdd(&cnt->n_bad, (unsigned long long)tot);
+        }
+    };
+
+    // ---- K2 stage B + K4 stage C for line p (ring index vp), owned by this warp -------------------------------------
+    auto process_line = [&](int p, int vp) {
+        const uint32_t gl = s_ls[p], len = s_ls[p + 1] - gl;
+        if (len == 0) return;                               // line_cnt stays 0 (cleared per run)
+        uint32_t sl[5];                                     // slots of lines p-2 .. p+2 (empty outside the plane, R2)
+#pragma unroll
+        for (int a = 0; a < 5; ++a) sl[a] = sm0 + (uint32_t)bring_at(vp, a - 2) * sg.slot_bytes;
+        const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
+        uint32_t pcount = 0, pdone = 0;                     // warp-uniform: queued / already written peaks
+
+        // stage C for one queued peak: y = (time | qmax << 16), k = its ordinal among the peaks of the line
+        auto moments = [&](uint32_t y, uint32_t k) {
+            const int t = (int)(y & 0xffffu);
+            int c[5][5];
+#pragma unroll
+            for (int a = 0; a < 5; ++a) bwindow<2>(sl[a], sg, t, c[a], digits, s_ls, p + a - 2, P, T);
+            const ClusterWords r = cluster_from_window(c, w0_line, (uint32_t)t, q_gate);
+            const size_t j = (size_t)gl + k;                // packed at the start of the line's range, time order
+            stage[2 * j] = r.lo;
+            stage[2 * j + 1] = r.hi;
+        };
+        // stage B for up to 32 survivors (one per lane); peaks go to the warp's queue, stage C runs on full warps
+        auto stage_b = [&](bool act, uint32_t y) {
+            bool peak = false;
+            if (act) {
+                const int t = (int)(y & 0xffffu);
+                const uint32_t q = y >> 16;
+                int cm[3], cp[3];
+                bwindow<1>(sl[1], sg, t, cm, digits, s_ls, p - 1, P, T);   // line p-1: earlier, strict (R1)
+                bwindow<1>(sl[3], sg, t, cp, digits, s_ls, p + 1, P, T);   // line p+1: later, >=
+                peak = q > (uint32_t)cm[0] && q > (uint32_t)cm[1] && q > (uint32_t)cm[2] &&
+                       q >= (uint32_t)cp[0] && q >= (uint32_t)cp[1] && q >= (uint32_t)cp[2];
+            }
+            const unsigned pm = __ballot_sync(0xffffffffu, peak);
+            if (pm == 0u) return;
+            if (peak) sts32(pqa + ((pcount + (uint32_t)__popc(pm & lt_mask)) << 2), y);
+            pcount += (uint32_t)__popc(pm);
+            __syncwarp();
+            if (pcount >= 32u) {
+                moments(lds32(pqa + ((uint32_t)lane << 2)), pdone + (uint32_t)lane);
+                pdone += 32u;
+                const uint32_t mv = lds32(pqa + (((uint32_t)lane + 32u) << 2));
+                __syncwarp();
+                sts32(pqa + ((uint32_t)lane << 2), mv);
+                pcount -= 32u;
+                __syncwarp();
+            }
+        };
+
+        const uint32_t ns = lds32(sl[2]);
+        const uint32_t nst = min(ns, sg.scap);
+        for (uint32_t i = 0; i < nst; i += 32u) {
+            const bool act = i + (uint32_t)lane < nst;
+            stage_b(act, act ? lds32(sl[2] + sg.surv_off + ((i + (uint32_t)lane) << 2)) : 0u);
+        }
+        if (ns > sg.scap) {
+            // rare: more survivors than the slot's list holds.  Stage A again from the digit array; survivors whose
+            // ordinal is >= scap were not listed and are tested here (still in time order).
+            uint32_t seen = 0;
+            for (uint32_t c0 = 0; c0 < len; c0 += 32u) {
+                const uint32_t jl = c0 + (uint32_t)lane;
+                const bool act = jl < len;
+                const uint32_t y = act ? __ldg(&digits[gl + jl].y) : 0u;
+                const uint32_t prevy = jl > 0u && act ? __ldg(&digits[gl + jl - 1u].y) : 0u;
+                const uint32_t nexty = jl + 1u < len ? __ldg(&digits[gl + jl + 1u].y) : 0u;
+                const bool surv = act && (y & 0xffffu) < T && stage_a(y, prevy, jl > 0u, nexty, jl + 1u < len, T, q_peak_min);
+                const unsigned smk = __ballot_sync(0xffffffffu, surv);
+                const uint32_t ord = seen + (uint32_t)__popc(smk & lt_mask);
+                seen += (uint32_t)__popc(smk);
+                if (seen > sg.scap) stage_b(surv && ord >= sg.scap, y);
+            }
+        }
+        if ((uint32_t)lane < pcount) moments(lds32(pqa + ((uint32_t)lane << 2)), pdone + (uint32_t)lane);
+        if (lane == 0) line_cnt[plane * g.LS + p] = pdone + pcount;   // peaks of this line, in time order
+    };
+
+    // ---- main loop -------------------------------------------------------------------------------------------------
+    // Ring index of line p is (p - (pa - 2)) mod kBSlots.  Prologue: lines pa-2 .. pa+S+1.
+    for (int i = warp; i < kBS + 4; i += kBWarps) {
+        stage_head(pa - 2 + i);
+        build_line(pa - 2 + i, i);
+    }
+    __syncthreads();
+    // Step (ONE barrier): every warp stages the head of the line it will build, runs stages B+C on its current line
+    // (lines l0-2 .. l0+S+1 are complete), then rebuilds the slot of a line that left the ring (l0-S-2 .. l0-3).
+    int vl0 = 2;                                                // ring index of line l0
+    for (int l0 = pa; l0 < pb; l0 += kBS) {
+        const bool more = l0 + kBS < pb;                        // lines l0+S+2 .. l0+2S+1 enter the ring in this step
+        const int pnew = l0 + kBS + 2 + warp, vnew = bring_at(vl0, kBS + 2 + warp - kBSlots);
+        if (more) stage_head(pnew);
+        if (l0 + warp < pb) process_line(l0 + warp, bring_at(vl0, warp));
+        if (more) build_line(pnew, vnew);
+        __syncthreads();
+        vl0 = bring_at(vl0, kBS);
+    }
+    if (bad_order) s_unsorted = 1;
+    __syncthreads();
+    if (tid == 0 && s_unsorted) atomicOr(&cnt->unsorted, 1u);
+}
+
+// Launches k_fused_blocks after the line index is in ws.line_start.  Returns 1 (launched), 0 (not applicable: the
+// mean line would not fit the block pool; the caller runs the bitmap kernel instead) or a negative tpc_cf error.
+int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
+                        uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1)
+{
+    uint64_t total_pads = 0;
+    for (uint32_t r = 0; r < g.n_rows; ++r) total_pads += g.npads[r];
+    total_pads *= g.n_sectors;
+    const double mean_len = (double)n / (double)(total_pads ? total_pads : 1);
+    // measured on the synthetic frames: 0.38 blocks and 0.16 stage-A survivors per digit
+    const double mean_blocks = 0.38 * mean_len, mean_surv = 0.16 * mean_len;
+
+    SlotGeo sg;
+    const uint32_t dir_bytes = ((((g.n_time + 9u) >> 3) + 1u) + 15u) & ~15u;
+    sg.pool_off = kDirOff + dir_bytes;
+    sg.scap = (((uint32_t)(mean_surv * 1.6) + 24u) + 3u) & ~3u;
+    const uint32_t fixed = kBWarps * (kStageDepth * 256u + 256u);
+    const uint32_t budget = 110u * 1024u;                          // 2 CTAs per SM
+    uint32_t want = (uint32_t)(mean_blocks * 1.5) + 32u;           // blocks incl. the zero block
+    if (want > 255u) want = 255u;
+    const uint32_t per_slot_fixed = sg.pool_off + 4u * sg.scap;
+    if (fixed + kBSlots * (per_slot_fixed + 16u * 8u) > budget) return 0;
+    uint32_t fit = ((budget - fixed) / kBSlots - per_slot_fixed) / 16u;
+    sg.pcap = want < fit ? want : fit;
+    if (const char* e = getenv("TPC_CF_BLOCK_POOL")) {             // test knob: force a small pool (slow paths)
+        const int v = atoi(e);
+        if (v >= 2 && v <= 255) sg.pcap = (uint32_t)v;
+    }
+    if (const char* e = getenv("TPC_CF_SURV_CAP")) {
+        const int v = atoi(e);
+        if (v >= 4 && v <= 4096) sg.scap = (uint32_t)v & ~3u;
+    }
+    const char* force = getenv("TPC_CF_FUSED_KERNEL");            // "blocks" | "lines" (tests, profiling)
+    const bool forced = force && force[0] == 'b';
+    if (force && force[0] == 'l') return 0;
+    if (!forced && (double)sg.pcap < mean_blocks * 1.2 + 8.0) return 0;   // too many lines would overflow the pool
+    sg.surv_off = sg.pool_off + 16u * sg.pcap;
+    sg.slot_bytes = sg.surv_off + 4u * sg.scap;
+    const uint32_t smem = kBSlots * sg.slot_bytes + fixed;
+    if (smem > 200u * 1024u) return 0;
+
+    const uint32_t whole = (g.max_pads + kBS - 1) / kBS * kBS;
+    uint32_t pads_per_unit = g.n_planes >= 1184 ? whole : (g.n_planes >= 296 ? 6 * kBS : 3 * kBS);
+    if (pads_per_unit > whole) pads_per_unit = whole;
+    if (const char* e = getenv("TPC_CF_PADS_PER_UNIT")) {          // tuning knob (multiples of 8)
+        const int v = atoi(e);
+        if (v >= kBS && v <= 256) pads_per_unit = (uint32_t)(v / kBS * kBS);
+    }
+    const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_fused_blocks, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e != cudaSuccess) return TPC_CF_E_CUDA;
+        attr_set = true;
+    }
+    if (ev_k0) cudaEventRecord(ev_k0, st);
+    k_fused_blocks<<<g.n_planes * upp, kBThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
+                                                              pads_per_unit, upp, sg, q_peak_min, q_gate,
+                                                              ws.counters, ws.line_cnt, (uint4*)ws.stage);
+    if (ev_k1) cudaEventRecord(ev_k1, st);
+    return 1;
+}
+
+}  // namespace tpccf

@@ -452,6 +452,13 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     k_line_index<<<(entries + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start);
     k += 2;
 
+    // block-sparse line slots (tpc_cf_blocks.cu) when the mean line fits their pool; else the bitmap slots below
+    {
+        const int r = launch_fused_blocks(g, ws, digits, n, q_peak_min, q_gate, st, ev_k0, ev_k1);
+        if (r < 0) return r;
+        if (r > 0) return k + r;
+    }
+
     // launch shape: pad range per unit, tq capacity per slot from the mean line length (host-known)
     uint64_t total_pads = 0;
     for (uint32_t r = 0; r < g.n_rows; ++r) total_pads += g.npads[r];

@@ -129,6 +129,10 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1);
 
+int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
+                        uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
+                        cudaEvent_t ev_k0, cudaEvent_t ev_k1);
+
 // compaction of stage[j] by peakmask into dst (= out, or ws.compact when a key sort must follow)
 int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t capacity, uint64_t max_clusters,
                    int sort_if_unsorted, cudaStream_t st);
