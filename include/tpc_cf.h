@@ -131,6 +131,11 @@ int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint64_t n,
 /* Number of kernel launches the last run enqueued (for bench.py's gpu_launches). */
 int tpc_cf_last_launch_count(const tpc_cf* h);
 
+/* Name of the dominant kernel the last run enqueued: "k_fused_blocks" or "k_fused_lines" on the fused sorted path
+ * (block-sparse or bitmap line slots, chosen from the mean line length), "k_peaks_map" on the general path.
+ * Static string, never NULL for a valid handle ("" before the first run). */
+const char* tpc_cf_last_kernel(const tpc_cf* h);
+
 /* Profiling (bench.py's roofline leg).  After tpc_cf_set_profiling(h, 1) every run records CUDA events on its
  * stream around the whole run and around its dominant kernel (the fused kernel on the sorted path, the
  * peak+moment kernel on the general path); the last 64 runs are kept.  tpc_cf_profile_ms(h, run, which) returns

@@ -25,7 +25,7 @@ DIGITS_SORTED = 1
 FORCE_GENERAL = 2
 
 EXPORTS = ["tpc_cf_workspace_bytes", "tpc_cf_create", "tpc_cf_run", "tpc_cf_run_host",
-           "tpc_cf_debug_dense_plane", "tpc_cf_last_launch_count", "tpc_cf_set_profiling",
+           "tpc_cf_debug_dense_plane", "tpc_cf_last_launch_count", "tpc_cf_last_kernel", "tpc_cf_set_profiling",
            "tpc_cf_profile_ms", "tpc_cf_destroy", "tpc_cf_strerror"]
 
 
@@ -81,6 +81,8 @@ def load(build_if_missing=True):
                                              ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
     lib.tpc_cf_last_launch_count.restype = ctypes.c_int
     lib.tpc_cf_last_launch_count.argtypes = [ctypes.c_void_p]
+    lib.tpc_cf_last_kernel.restype = ctypes.c_char_p
+    lib.tpc_cf_last_kernel.argtypes = [ctypes.c_void_p]
     lib.tpc_cf_set_profiling.restype = ctypes.c_int
     lib.tpc_cf_set_profiling.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.tpc_cf_profile_ms.restype = ctypes.c_float
@@ -218,6 +220,9 @@ class ClusterFinder:
 
     def last_launch_count(self):
         return int(self.lib.tpc_cf_last_launch_count(self.h))
+
+    def last_kernel(self):
+        return self.lib.tpc_cf_last_kernel(self.h).decode()
 
     def close(self):
         if getattr(self, "h", None) is not None:

@@ -17,6 +17,7 @@ struct tpc_cf {
     uint32_t n_sort_tiles;
     size_t map_bytes;
     int last_launches;
+    const char* last_kernel;
     int profiling;
     uint32_t run_index;         // runs since profiling was switched on
     cudaEvent_t ev[kProfSlots][4];   // per slot: run begin, dominant kernel begin, dominant kernel end, run end
@@ -188,6 +189,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(h, e, "kernel launch");
     h->last_launches = k;
+    h->last_kernel = g_last_kernel;
     return TPC_CF_OK;
 }
 
@@ -240,6 +242,8 @@ extern "C" int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint
 }
 
 extern "C" int tpc_cf_last_launch_count(const tpc_cf* h) { return h ? h->last_launches : TPC_CF_E_NULL; }
+
+extern "C" const char* tpc_cf_last_kernel(const tpc_cf* h) { return h && h->last_kernel ? h->last_kernel : ""; }
 
 extern "C" int tpc_cf_set_profiling(tpc_cf* h, int on)
 {

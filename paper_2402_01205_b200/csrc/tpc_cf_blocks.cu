@@ -197,23 +197,23 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 
     const int blo = max(pa - 2, 0), bhi = min(P, pb + 2);   // lines this unit ever builds
 
-    // ---- staging: chunk c (digits 32c .. 32c+31) of the line starting at lbeg -> ring entry c mod kStageDepth ------
-    // one commit group per call, empty or not, so that wait_group counts chunks
-    auto stage_chunk = [&](uint32_t lbeg, uint32_t len, uint32_t c) {
-        const uint32_t jl = 32u * c + (uint32_t)lane;
-        if (jl < len) {
-            const uint32_t dst = stg + (c & (kStageDepth - 1)) * 256u + 8u * (uint32_t)lane;
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(digits + lbeg + jl) : "memory");
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
+    // ---- staging: chunk c (digits 32c .. 32c+31) of a line -> ring entry c mod kStageDepth (cp.async, 8 B per lane) --
+    // one commit group per chunk, empty or not, so that wait_group counts chunks.  Prefetch distance: kAhead chunks.
+    constexpr uint32_t kAhead = kStageDepth - 1;
+    const uint32_t stg_lane = stg + 8u * (uint32_t)lane;
+    auto cp_async8 = [&](uint32_t dst, const uint2* src) {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
     };
-    // the first kStageDepth-1 chunks of the line this warp builds next (issued before the warp processes its
-    // current line, so the global latency is covered)
+    // the first kAhead chunks of the line this warp builds next (issued before the warp processes its current line,
+    // so the global latency is covered)
     auto stage_head = [&](int p) {
         if (p < blo || p >= bhi) return;
         const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
 #pragma unroll
-        for (uint32_t c = 0; c < kStageDepth - 1; ++c) stage_chunk(lbeg, len, c);
+        for (uint32_t c = 0; c < kAhead; ++c) {
+            if (32u * c + (uint32_t)lane < len) cp_async8(stg_lane + 256u * c, digits + lbeg + 32u * c + lane);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        }
     };
 
     // ---- K0 + K1 + stage A: this warp (re)builds slot v as line p ---------------------------------------------------
@@ -225,42 +225,53 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
         const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
         if (len == 0) return;
         const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
-        const uint32_t a_dir = slot + kDirOff, a_pool = slot + sg.pool_off, a_surv = slot + sg.surv_off;
+        const uint32_t a_dir1 = slot + kDirOff + 1u;        // dir byte of the block of time t: a_dir1 + (t >> 3)
+        const uint32_t a_pool = slot + sg.pool_off, a_surv = slot + sg.surv_off;
+        const uint32_t qmin_y = q_peak_min << 16;           // y >= qmin_y  <=>  charge >= q_peak_min
+        const uint32_t le_mask = lt_mask | (1u << lane);
+        const uint2* gp = digits + lbeg + 32u * kAhead + lane;   // this lane's digit of chunk c + kAhead
+        uint32_t ro = 0u;                                   // ring offset of chunk c
         uint32_t carry = 0u;                                // y of the digit before this chunk
         uint32_t nblk = 0u, nsurv = 0u;                     // warp-uniform running counts
         uint32_t nbad = 0u;                                 // per lane
-        const uint32_t nchunks = (len + 31u) >> 5;
-        for (uint32_t c = 0; c < nchunks; ++c) {
-            stage_chunk(lbeg, len, c + kStageDepth - 1);
-            asm volatile("cp.async.wait_group %0;" ::"n"(kStageDepth - 2) : "memory");   // chunks <= c+1 have landed
+        for (uint32_t c0 = 0; c0 < len; c0 += 32u) {
+            const uint32_t jl = c0 + (uint32_t)lane;
+            if (jl + 32u * kAhead < len) cp_async8(stg_lane + ((ro + 256u * kAhead) & (256u * (kStageDepth - 1))), gp);
+            gp += 32;
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group %0;" ::"n"(kAhead - 1) : "memory");   // chunks <= c+1 have landed
             __syncwarp();
-            const uint32_t jl = 32u * c + (uint32_t)lane;
-            const bool act = jl < len;
-            const uint2 d = lds64(stg + (c & (kStageDepth - 1)) * 256u + 8u * (uint32_t)lane);
-            const uint32_t y_next0 = lds32(stg + ((c + 1u) & (kStageDepth - 1)) * 256u + 4u);   // first y of chunk c+1
+            const uint2 d = lds64(stg_lane + ro);
+            ro = (ro + 256u) & (256u * (kStageDepth - 1));
+            const uint32_t y_next0 = lds32(stg + ro + 4u);  // first y of chunk c+1
             const uint32_t y = d.y;
             uint32_t prevy = __shfl_up_sync(0xffffffffu, y, 1);
             uint32_t nexty = __shfl_down_sync(0xffffffffu, y, 1);
             if (lane == 0) prevy = carry;
             if (lane == 31) nexty = y_next0;
             carry = __shfl_sync(0xffffffffu, y, 31);
-            const uint32_t t = y & 0xffffu, pt = prevy & 0xffffu, q = y >> 16;
-            const bool first = jl == 0u;
-            const bool ok = act && (d.x & 0x00ffffffu) == w0_line;
-            if (act && (!ok || (!first && pt >= t))) bad_order = true;   // wrong line, not ascending, or duplicate cell
+            const bool act = jl < len, nf = jl != 0u;
+            const uint32_t t = y & 0xffffu;
+            const bool ok = act && ((d.x ^ w0_line) & 0x00ffffffu) == 0u;
+            // wrong line, not ascending, or duplicate cell: the DIGITS_SORTED promise is false
+            if (act && (!ok || (nf && (prevy & 0xffffu) >= t))) bad_order = true;
             const bool inb = ok && t < T;                   // addresses a cell of this line
-            if (ok && (!inb || q == 0u)) ++nbad;            // R11
+            if (ok && !(inb && y >= 0x10000u)) ++nbad;      // R11: time out of range or zero charge
             // K1: blocks are allocated in time order: a digit opens a block iff the digit before it is in another one
-            const uint32_t b = (t + 8u) >> 3;
-            const bool head = inb && (first || ((pt + 8u) >> 3) != b);
+            const bool head = inb && (!nf || ((y ^ prevy) & 0xfff8u) != 0u);
             const unsigned hm = __ballot_sync(0xffffffffu, head);
-            const uint32_t idx = nblk + (uint32_t)__popc(hm & (lt_mask | (1u << lane)));   // 1-based; 0 = zero block
+            const uint32_t idx = nblk + (uint32_t)__popc(hm & le_mask);   // 1-based; 0 = zero block
             nblk += (uint32_t)__popc(hm);
             const bool in_pool = idx < sg.pcap;
-            if (head) sts8(a_dir + b, in_pool ? idx : 0xFFu);
-            if (inb && in_pool) sts16(a_pool + (idx << 4) + ((t & 7u) << 1), q);
-            // K2 stage A
-            const bool surv = inb && stage_a(y, prevy, !first, nexty, jl + 1u < len, T, q_peak_min);
+            if (head) sts8(a_dir1 + (t >> 3), in_pool ? idx : 0xFFu);
+            if (inb && in_pool) sts16(a_pool + (idx << 4) + ((y & 7u) << 1), y >> 16);
+            // K2 stage A (R1, own line) on the packed words: with equal time fields, comparing the words compares
+            // the charges.  (0,-1) is earlier: the digit loses to an adjacent previous charge >= its own;
+            // (0,+1) is later: it loses to an adjacent next charge > its own (cells at time >= T read 0).
+            const uint32_t A = prevy + 1u, B = nexty - 1u;
+            const bool kill_prev = nf && ((A ^ y) & 0xffffu) == 0u && A >= y;
+            const bool kill_next = jl + 1u < len && ((B ^ y) & 0xffffu) == 0u && B > y && (nexty & 0xffffu) < T;
+            const bool surv = inb && y >= qmin_y && !kill_prev && !kill_next;
             const unsigned smk = __ballot_sync(0xffffffffu, surv);
             const uint32_t pos = nsurv + (uint32_t)__popc(smk & lt_mask);
             if (surv && pos < sg.scap) sts32(a_surv + (pos << 2), y);
@@ -429,6 +440,7 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
         attr_set = true;
     }
     if (ev_k0) cudaEventRecord(ev_k0, st);
+    g_last_kernel = "k_fused_blocks";
     k_fused_blocks<<<g.n_planes * upp, kBThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
                                                               pads_per_unit, upp, sg, q_peak_min, q_gate,
                                                               ws.counters, ws.line_cnt, (uint4*)ws.stage);

@@ -493,6 +493,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
         attr_set = true;
     }
     if (ev_k0) cudaEventRecord(ev_k0, st);
+    g_last_kernel = "k_fused_lines";
     k_fused_lines<<<g.n_planes * upp, kFThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
                                                              pads_per_unit, upp, wpl, cap, q_peak_min, q_gate,
                                                              ws.counters, ws.line_cnt, (uint4*)ws.stage);

@@ -10,6 +10,8 @@
 
 namespace tpccf {
 
+thread_local const char* g_last_kernel = "";
+
 static constexpr int kThreads = 256;
 
 __device__ __forceinline__ size_t cell_offset(const Geo& g, uint32_t w0, uint32_t w1)
@@ -122,6 +124,7 @@ int launch_general_peaks(const Geo& g, const Workspace& ws, const tpc_digit* dig
     if (n == 0) return 0;
     k_scatter<<<grid_for(n), kThreads, 0, st>>>((const uint2*)digits, n, g, ws.map, ws.counters);
     if (ev_k0) cudaEventRecord(ev_k0, st);
+    g_last_kernel = "k_peaks_map";
     k_peaks_map<<<grid_for(n), kThreads, 0, st>>>((const uint2*)digits, n, g, ws.map, q_peak_min, q_gate,
                                                   ws.peakmask, (uint4*)ws.stage);
     if (ev_k1) cudaEventRecord(ev_k1, st);

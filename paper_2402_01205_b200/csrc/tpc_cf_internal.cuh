@@ -115,6 +115,9 @@ __device__ __forceinline__ ClusterWords cluster_from_window(const int (&c)[5][5]
     return r;
 }
 
+// name of the dominant kernel enqueued last by this host thread (set by the launchers, copied into the handle)
+extern thread_local const char* g_last_kernel;
+
 // ---- launchers (each returns the number of kernels it enqueued, or a negative tpc_cf error) -----------------
 
 int launch_general_peaks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,

@@ -36,7 +36,23 @@ def parse_golden(path=GOLDEN):
     return ex
 
 
-PATHS = {"general": 0, "general_hint": 3, "fused": 1}   # flags: DIGITS_SORTED=1, FORCE_GENERAL=2
+# flags: DIGITS_SORTED=1, FORCE_GENERAL=2.  "fused" lets the library choose the fused kernel from the mean line length;
+# "fused_blocks" / "fused_lines" force the block-sparse / bitmap line-slot kernel (TPC_CF_FUSED_KERNEL), so that each
+# runs every case — including the ones far outside its range, which exercise its exact slow paths.
+PATHS = {"general": 0, "general_hint": 3, "fused": 1, "fused_blocks": 1, "fused_lines": 1}
+FUSED_KERNEL = {"fused_blocks": "k_fused_blocks", "fused_lines": "k_fused_lines"}
+
+
+@pytest.fixture(autouse=True)
+def _fused_kernel_env(request, monkeypatch):
+    """Sets the library's kernel-selection knob from the test's `path` parameter (read with getenv at every run)."""
+    params = getattr(getattr(request.node, "callspec", None), "params", {})
+    for k in ("TPC_CF_FUSED_KERNEL", "TPC_CF_BLOCK_POOL", "TPC_CF_SURV_CAP"):
+        monkeypatch.delenv(k, raising=False)
+    path = params.get("path")
+    if path in FUSED_KERNEL:
+        monkeypatch.setenv("TPC_CF_FUSED_KERNEL", "blocks" if path == "fused_blocks" else "lines")
+    yield
 
 
 def gpu_run(digits, geom, flags, max_clusters=None, capacity=None, q_peak_min=4, q_inner_gate=2, finder=None):
@@ -51,6 +67,10 @@ def gpu_run(digits, geom, flags, max_clusters=None, capacity=None, q_peak_min=4,
     d = cf.to_device(digits)
     finder.run(d, n, flags=flags, capacity=capacity)
     cl, st = finder.result()
+    st["kernel"] = finder.last_kernel()
+    forced = os.environ.get("TPC_CF_FUSED_KERNEL")
+    if forced and n and st["path"] == 3:
+        assert st["kernel"] == "k_fused_" + forced, (st["kernel"], forced)
     if capacity is not None:
         cl = cl[:capacity]
     if own:
@@ -75,7 +95,7 @@ def test_worked_examples(path):
     ora, ost = orc.run(digits, *geom[:4])
     cl, st = gpu_run(digits, geom, PATHS[path])
     assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == 0 and st["overflow"] == 0
-    assert st["path"] == (3 if path == "fused" else 1)
+    assert st["path"] == (3 if path.startswith("fused") else 1)
     assert_clusters_equal(cl, ora, "worked examples/" + path)
 
 
@@ -302,3 +322,26 @@ def test_dense_isolated_peaks_overflow_the_peak_queue(path):
     cl, st = gpu_run(digits, geom, PATHS[path])
     assert st["n_clusters"] == ost["n_clusters"]
     assert_clusters_equal(cl, ora, "dense isolated peaks/" + path)
+
+
+@pytest.mark.parametrize("pool,scap", [(2, 4), (9, 8), (40, 4), (255, 12)])
+def test_block_kernel_slow_paths(pool, scap, monkeypatch):
+    """k_fused_blocks with a block pool / survivor list far too small for the data (TPC_CF_BLOCK_POOL,
+    TPC_CF_SURV_CAP): window cells whose block is not in the pool are looked up in the digit array, survivors beyond
+    the list are re-derived from the digit array.  Results must not change (config 1, and a ~5 % single row)."""
+    monkeypatch.setenv("TPC_CF_FUSED_KERNEL", "blocks")
+    monkeypatch.setenv("TPC_CF_BLOCK_POOL", str(pool))
+    monkeypatch.setenv("TPC_CF_SURV_CAP", str(scap))
+    digits = gen.generate(1)
+    geom = gen.geometry(1)
+    ora, ost = orc.run(digits, *geom[:4], npads=geom[4])
+    cl, st = gpu_run(digits, geom, 1)
+    assert st["kernel"] == "k_fused_blocks" and st["n_clusters"] == ost["n_clusters"]
+    assert_clusters_equal(cl, ora, "config 1, pool %d scap %d" % (pool, scap))
+    c = dict(gen.CONFIGS[2]); c["n_rows"] = 2
+    geom = gen.geometry(c)
+    digits = gen.generate(c)
+    ora, ost = orc.run(digits, *geom[:4])
+    cl, st = gpu_run(digits, geom, 1)
+    assert st["kernel"] == "k_fused_blocks" and st["n_clusters"] == ost["n_clusters"]
+    assert_clusters_equal(cl, ora, "config 2 (2 rows), pool %d scap %d" % (pool, scap))
