@@ -175,10 +175,10 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 
     if (pa >= P && unit != 0) return;    // nothing in this pad range (rows with fewer pads)
 
-    bool bad_order = false;
+    uint32_t bad_order = 0u;
     // monotone line starts: a garbage index from unsorted input must not produce negative lengths or unbounded work
-    for (int i = tid; i < (int)g.LS; i += kBThreads) if (s_ls[i] > s_ls[i + 1]) bad_order = true;
-    if (__syncthreads_or(bad_order ? 1 : 0)) {
+    for (int i = tid; i < (int)g.LS; i += kBThreads) if (s_ls[i] > s_ls[i + 1]) bad_order = 1u;
+    if (__syncthreads_or((int)bad_order)) {
         if (tid == 0) atomicOr(&cnt->unsorted, 1u);
         return;
     }
@@ -189,7 +189,7 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
         if (ge > gb) {
             for (uint32_t j = gb + tid; j < ge; j += kBThreads) {
                 const uint2 d = __ldg(digits + j);
-                if (digit_valid(g, d.x, d.y)) bad_order = true;     // a valid digit outside every line: not sorted
+                if (digit_valid(g, d.x, d.y)) bad_order = 1u;     // a valid digit outside every line: not sorted
             }
             if (tid == 0) atomicAdd(&cnt->n_bad, (unsigned long long)(ge - gb));
         }
@@ -252,9 +252,10 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
             carry = __shfl_sync(0xffffffffu, y, 31);
             const bool act = jl < len, nf = jl != 0u;
             const uint32_t t = y & 0xffffu;
-            const bool ok = act && ((d.x ^ w0_line) & 0x00ffffffu) == 0u;
+            const uint32_t xkey = (d.x ^ w0_line) & 0x00ffffffu;
+            const bool ok = act && xkey == 0u;
             // wrong line, not ascending, or duplicate cell: the DIGITS_SORTED promise is false
-            if (act && (!ok || (nf && (prevy & 0xffffu) >= t))) bad_order = true;
+            bad_order |= (act && (xkey != 0u || (nf && (prevy & 0xffffu) >= t))) ? 1u : 0u;
             const bool inb = ok && t < T;                   // addresses a cell of this line
             if (ok && !(inb && y >= 0x10000u)) ++nbad;      // R11: time out of range or zero charge
             // K1: blocks are allocated in time order: a digit opens a block iff the digit before it is in another one
@@ -372,9 +373,34 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
     int vl0 = 2;                                                // ring index of line l0
     for (int l0 = pa; l0 < pb; l0 += kBS) {
         const bool more = l0 + kBS < pb;                        // lines l0+S+2 .. l0+2S+1 enter the ring in this step
-        const int pnew = l0 + kBS + 2 + warp, vnew = bring_at(vl0, kBS + 2 + warp - kBSlots);
+        // Load balance inside the step: a warp's work is one line to process plus one line to build, both
+        // proportional to the line lengths (known from the index).  The warp with the longest line to process gets
+        // the shortest line to build, and so on: the 8 sums come out nearly equal and the barrier waits less.
+        int ip = warp, ib = warp;                               // which of the 8 lines this warp processes / builds
+        {
+            uint32_t lp = 0u, lb = 0u;
+            if (lane < kBS) {
+                const int p = l0 + lane, q = l0 + kBS + 2 + lane;
+                if (p < pb) lp = min(s_ls[p + 1] - s_ls[p], 0xfffeu) + 1u;
+                if (more && q >= blo && q < bhi) lb = min(s_ls[q + 1] - s_ls[q], 0xfffeu) + 1u;
+            }
+            const uint32_t mine = lp | (lb << 16);
+            uint32_t rp = 0u, rb = 0u;                          // rank of lane's process line (descending) / build line (ascending)
+#pragma unroll
+            for (int j = 0; j < kBS; ++j) {
+                const uint32_t o = __shfl_sync(0xffffffffu, mine, j);
+                const uint32_t op = o & 0xffffu, ob = o >> 16;
+                rp += (op > lp || (op == lp && j < lane)) ? 1u : 0u;
+                rb += (ob < lb || (ob == lb && j < lane)) ? 1u : 0u;
+            }
+            const unsigned mp = __ballot_sync(0xffffffffu, lane < kBS && rp == (uint32_t)warp);
+            const unsigned mb = __ballot_sync(0xffffffffu, lane < kBS && rb == (uint32_t)warp);
+            ip = __ffs(mp) - 1;
+            ib = __ffs(mb) - 1;
+        }
+        const int pnew = l0 + kBS + 2 + ib, vnew = bring_at(vl0, kBS + 2 + ib - kBSlots);
         if (more) stage_head(pnew);
-        if (l0 + warp < pb) process_line(l0 + warp, bring_at(vl0, warp));
+        if (l0 + ip < pb) process_line(l0 + ip, bring_at(vl0, ip));
         if (more) build_line(pnew, vnew);
         __syncthreads();
         vl0 = bring_at(vl0, kBS);
