@@ -112,18 +112,21 @@ struct SlotGeo {
     uint32_t surv_off;     // pool_off + 16 * pcap
     uint32_t pcap;         // blocks in the pool including the zero block 0 (<= 255)
     uint32_t scap;         // survivor entries per slot
+    uint32_t n_pass;       // the time axis is covered in n_pass segments, one pass over the unit's lines each
+    uint32_t seg_len;      // time bins per segment (multiple of 8); n_pass * seg_len >= n_time
 };
 
 // charges of the window t-H..t+H of the line in slot `slot` (0 where no digit): c[k] is time t-H+k.
 // lidx = pad index of that line, used only by the slow path (line_start lookups in s_ls).
 template <int H>
-__device__ __forceinline__ void bwindow(uint32_t slot, const SlotGeo& sg, int t, int (&c)[2 * H + 1],
+__device__ __forceinline__ void bwindow(uint32_t slot, uint32_t dsub, const SlotGeo& sg, int t, int (&c)[2 * H + 1],
                                         const uint2* __restrict__ digits, const uint32_t* s_ls, int lidx, int P,
                                         uint32_t T)
 {
     const uint32_t u = (uint32_t)(t + 8 - H);                 // first cell, shifted by the 8-bin guard block
-    const uint32_t dA = lds8(slot + kDirOff + (u >> 3));
-    const uint32_t dB = lds8(slot + kDirOff + ((u + 2 * H) >> 3));
+    const uint32_t dir = slot + kDirOff - dsub;               // dsub = first time bin of the pass / 8
+    const uint32_t dA = lds8(dir + (u >> 3));
+    const uint32_t dB = lds8(dir + ((u + 2 * H) >> 3));
     const uint32_t o = u & 7u;
     const uint32_t base = slot + sg.pool_off + 2u * o;
     const uint32_t aA = base + (dA << 4), aB = base + (dB << 4) - 16u;
@@ -144,6 +147,7 @@ __device__ __forceinline__ void bwindow(uint32_t slot, const SlotGeo& sg, int t,
     }
 }
 
+template <bool MULTI>   // MULTI: the time axis is covered in sg.n_pass > 1 passes (long lines)
 __global__ void __launch_bounds__(kBThreads, 2)
 k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
                uint32_t pads_per_unit, uint32_t units_per_plane, SlotGeo sg, uint32_t q_peak_min, uint32_t q_gate,
@@ -151,6 +155,8 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_ls[260];          // line starts of this plane: s_ls[p], p = 0..max_pads, then next plane's start
+    __shared__ uint32_t s_pos[260];         // first digit of line p that the current pass needs (time >= pass start - 2)
+    __shared__ uint32_t s_cnt[260];         // peaks of line p found by the passes so far
     __shared__ int s_unsorted;
 
     const uint32_t plane = blockIdx.x / units_per_plane, unit = blockIdx.x % units_per_plane;
@@ -167,7 +173,10 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
     const uint32_t stg = sm0 + kBSlots * sg.slot_bytes + (uint32_t)warp * (kStageDepth * 256u);   // staging ring
     const uint32_t pqa = sm0 + kBSlots * sg.slot_bytes + kBWarps * (kStageDepth * 256u) + (uint32_t)warp * 256u;
 
-    for (int i = tid; i <= (int)g.LS; i += kBThreads) s_ls[i] = line_start[plane * g.LS + i];
+    for (int i = tid; i <= (int)g.LS; i += kBThreads) {
+        const uint32_t v = line_start[plane * g.LS + i];
+        s_ls[i] = v; s_pos[i] = v; s_cnt[i] = 0u;
+    }
     if (tid == 0) s_unsorted = 0;
     // every slot starts as an empty line (lines outside the plane keep this state: zero border in pad, R2)
     for (uint32_t x = (uint32_t)tid * 16u; x < kBSlots * sg.slot_bytes; x += kBThreads * 16u) sts128z(sm0 + x);
@@ -197,6 +206,12 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 
     const int blo = max(pa - 2, 0), bhi = min(P, pb + 2);   // lines this unit ever builds
 
+    // Time window of the current pass (set in the pass loop below).  Owned cells [tlo, thi): their peaks are found
+    // in this pass.  Stored cells [wlo, whi) = owned +- 2 bins: the 5x5 windows of owned peaks stay inside.
+    // With a single pass (MULTI = false) these are constants and the pass logic folds away.
+    uint32_t tlo = 0u, thi = T, wlo = 0u, whi = T, dsub = 0u;
+    bool last_pass = true;
+
     // ---- staging: chunk c (digits 32c .. 32c+31) of a line -> ring entry c mod kStageDepth (cp.async, 8 B per lane) --
     // one commit group per chunk, empty or not, so that wait_group counts chunks.  Prefetch distance: kAhead chunks.
     constexpr uint32_t kAhead = kStageDepth - 1;
@@ -208,7 +223,7 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
     // so the global latency is covered)
     auto stage_head = [&](int p) {
         if (p < blo || p >= bhi) return;
-        const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
+        const uint32_t lbeg = s_pos[p], len = s_ls[p + 1] - lbeg;
 #pragma unroll
         for (uint32_t c = 0; c < kAhead; ++c) {
             if (32u * c + (uint32_t)lane < len) cp_async8(stg_lane + 256u * c, digits + lbeg + 32u * c + lane);
@@ -222,18 +237,23 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
         for (uint32_t x = (uint32_t)lane * 16u; x < sg.surv_off; x += 512u) sts128z(slot + x);   // hdr, dir, pool
         __syncwarp();
         if (p < blo || p >= bhi) return;                    // a line outside the plane / the halo: stays empty
-        const uint32_t lbeg = s_ls[p], len = s_ls[p + 1] - lbeg;
+        const uint32_t lbeg = s_pos[p], lend = s_ls[p + 1], len = lend - lbeg;
+        if (lane == 0) sts32(slot + 4u, lbeg);              // hdr word 1: where this pass started in the line
         if (len == 0) return;
         const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
-        const uint32_t a_dir1 = slot + kDirOff + 1u;        // dir byte of the block of time t: a_dir1 + (t >> 3)
+        const uint32_t a_dir1 = slot + kDirOff + 1u - (MULTI ? dsub : 0u); // dir byte of the block of time t: a_dir1 + (t >> 3)
         const uint32_t a_pool = slot + sg.pool_off, a_surv = slot + sg.surv_off;
         const uint32_t qmin_y = q_peak_min << 16;           // y >= qmin_y  <=>  charge >= q_peak_min
         const uint32_t le_mask = lt_mask | (1u << lane);
+        const uint32_t own_span = thi - tlo, win_span = whi - wlo;
+        const uint32_t nlo = thi - 2u;                      // the next pass needs the line from this time on
         const uint2* gp = digits + lbeg + 32u * kAhead + lane;   // this lane's digit of chunk c + kAhead
         uint32_t ro = 0u;                                   // ring offset of chunk c
         uint32_t carry = 0u;                                // y of the digit before this chunk
         uint32_t nblk = 0u, nsurv = 0u;                     // warp-uniform running counts
         uint32_t nbad = 0u;                                 // per lane
+        uint32_t next_pos = lend;                           // first digit with time >= nlo (warp-uniform)
+        bool found = false;
         for (uint32_t c0 = 0; c0 < len; c0 += 32u) {
             const uint32_t jl = c0 + (uint32_t)lane;
             if (jl + 32u * kAhead < len) cp_async8(stg_lane + ((ro + 256u * kAhead) & (256u * (kStageDepth - 1))), gp);
@@ -256,8 +276,10 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
             const bool ok = act && xkey == 0u;
             // wrong line, not ascending, or duplicate cell: the DIGITS_SORTED promise is false
             bad_order |= (act && (xkey != 0u || (nf && (prevy & 0xffffu) >= t))) ? 1u : 0u;
-            const bool inb = ok && t < T;                   // addresses a cell of this line
-            if (ok && !(inb && y >= 0x10000u)) ++nbad;      // R11: time out of range or zero charge
+            const bool inb = MULTI ? (ok && (t - wlo) < win_span) : (ok && t < T);    // a cell this pass stores
+            const bool own = MULTI ? (ok && (t - tlo) < own_span) : inb;   // a cell this pass decides (ends at T at the latest)
+            // R11: time out of range or zero charge, counted by the pass that owns the digit's time
+            if ((!MULTI ? ok : (last_pass ? (ok && t >= tlo) : own)) && !(own && y >= 0x10000u)) ++nbad;
             // K1: blocks are allocated in time order: a digit opens a block iff the digit before it is in another one
             const bool head = inb && (!nf || ((y ^ prevy) & 0xfff8u) != 0u);
             const unsigned hm = __ballot_sync(0xffffffffu, head);
@@ -272,13 +294,29 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
             const uint32_t A = prevy + 1u, B = nexty - 1u;
             const bool kill_prev = nf && ((A ^ y) & 0xffffu) == 0u && A >= y;
             const bool kill_next = jl + 1u < len && ((B ^ y) & 0xffffu) == 0u && B > y && (nexty & 0xffffu) < T;
-            const bool surv = inb && y >= qmin_y && !kill_prev && !kill_next;
+            const bool surv = own && y >= qmin_y && !kill_prev && !kill_next;
             const unsigned smk = __ballot_sync(0xffffffffu, surv);
             const uint32_t pos = nsurv + (uint32_t)__popc(smk & lt_mask);
             if (surv && pos < sg.scap) sts32(a_surv + (pos << 2), y);
             nsurv += (uint32_t)__popc(smk);
+            if (MULTI && !last_pass) {
+                // where the next pass starts in this line, and whether this pass has seen all it stores
+                const bool tail = c0 + 32u >= len;
+                const uint32_t t31 = carry & 0xffffu;       // time of the chunk's last digit (full chunks)
+                if (!found && (tail || t31 >= nlo)) {
+                    const unsigned m = __ballot_sync(0xffffffffu, act && t >= nlo);
+                    if (m) { next_pos = lbeg + c0 + (uint32_t)__ffs(m) - 1u; found = true; }
+                }
+                if (!tail && t31 >= whi) {                  // every later digit is beyond the window
+                    asm volatile("cp.async.wait_group 0;" ::: "memory");   // the ring is reused by the next line
+                    break;
+                }
+            }
         }
-        if (lane == 0) sts32(slot, nsurv);
+        if (lane == 0) {
+            sts32(slot, nsurv);
+            if (MULTI && !last_pass) s_pos[p] = next_pos;
+        }
         if (p >= pa && p < pb) {                            // halo lines are counted by the unit that owns them
             const uint32_t tot = __reduce_add_sync(0xffffffffu, nbad);
             if (tot != 0u && lane == 0) atomicAdd(&cnt->n_bad, (unsigned long long)tot);
@@ -287,20 +325,20 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 
     // ---- K2 stage B + K4 stage C for line p (ring index vp), owned by this warp -------------------------------------
     auto process_line = [&](int p, int vp) {
-        const uint32_t gl = s_ls[p], len = s_ls[p + 1] - gl;
-        if (len == 0) return;                               // line_cnt stays 0 (cleared per run)
+        const uint32_t gl = s_ls[p], lend = s_ls[p + 1];
+        if (lend == gl) return;                             // line_cnt stays 0 (cleared per run)
         uint32_t sl[5];                                     // slots of lines p-2 .. p+2 (empty outside the plane, R2)
 #pragma unroll
         for (int a = 0; a < 5; ++a) sl[a] = sm0 + (uint32_t)bring_at(vp, a - 2) * sg.slot_bytes;
         const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
-        uint32_t pcount = 0, pdone = 0;                     // warp-uniform: queued / already written peaks
+        uint32_t pcount = 0, pdone = MULTI ? s_cnt[p] : 0u; // warp-uniform: queued / already written peaks of the line
 
         // stage C for one queued peak: y = (time | qmax << 16), k = its ordinal among the peaks of the line
         auto moments = [&](uint32_t y, uint32_t k) {
             const int t = (int)(y & 0xffffu);
             int c[5][5];
 #pragma unroll
-            for (int a = 0; a < 5; ++a) bwindow<2>(sl[a], sg, t, c[a], digits, s_ls, p + a - 2, P, T);
+            for (int a = 0; a < 5; ++a) bwindow<2>(sl[a], MULTI ? dsub : 0u, sg, t, c[a], digits, s_ls, p + a - 2, P, T);
             const ClusterWords r = cluster_from_window(c, w0_line, (uint32_t)t, q_gate);
             const size_t j = (size_t)gl + k;                // packed at the start of the line's range, time order
             stage[2 * j] = r.lo;
@@ -313,8 +351,8 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
                 const int t = (int)(y & 0xffffu);
                 const uint32_t q = y >> 16;
                 int cm[3], cp[3];
-                bwindow<1>(sl[1], sg, t, cm, digits, s_ls, p - 1, P, T);   // line p-1: earlier, strict (R1)
-                bwindow<1>(sl[3], sg, t, cp, digits, s_ls, p + 1, P, T);   // line p+1: later, >=
+                bwindow<1>(sl[1], MULTI ? dsub : 0u, sg, t, cm, digits, s_ls, p - 1, P, T);   // line p-1: earlier, strict (R1)
+                bwindow<1>(sl[3], MULTI ? dsub : 0u, sg, t, cp, digits, s_ls, p + 1, P, T);   // line p+1: later, >=
                 peak = q > (uint32_t)cm[0] && q > (uint32_t)cm[1] && q > (uint32_t)cm[2] &&
                        q >= (uint32_t)cp[0] && q >= (uint32_t)cp[1] && q >= (uint32_t)cp[2];
             }
@@ -341,27 +379,44 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
             stage_b(act, act ? lds32(sl[2] + sg.surv_off + ((i + (uint32_t)lane) << 2)) : 0u);
         }
         if (ns > sg.scap) {
-            // rare: more survivors than the slot's list holds.  Stage A again from the digit array; survivors whose
-            // ordinal is >= scap were not listed and are tested here (still in time order).
+            // rare: more survivors than the slot's list holds.  Stage A again from the digit array, from where this
+            // pass started in the line; survivors whose ordinal is >= scap were not listed and are tested here
+            // (still in time order).
+            const uint32_t lbeg = lds32(sl[2] + 4u), len = lend - lbeg;
             uint32_t seen = 0;
             for (uint32_t c0 = 0; c0 < len; c0 += 32u) {
                 const uint32_t jl = c0 + (uint32_t)lane;
                 const bool act = jl < len;
-                const uint32_t y = act ? __ldg(&digits[gl + jl].y) : 0u;
-                const uint32_t prevy = jl > 0u && act ? __ldg(&digits[gl + jl - 1u].y) : 0u;
-                const uint32_t nexty = jl + 1u < len ? __ldg(&digits[gl + jl + 1u].y) : 0u;
-                const bool surv = act && (y & 0xffffu) < T && stage_a(y, prevy, jl > 0u, nexty, jl + 1u < len, T, q_peak_min);
+                const uint32_t y = act ? __ldg(&digits[lbeg + jl].y) : 0u;
+                const uint32_t prevy = jl > 0u && act ? __ldg(&digits[lbeg + jl - 1u].y) : 0u;
+                const uint32_t nexty = jl + 1u < len ? __ldg(&digits[lbeg + jl + 1u].y) : 0u;
+                const bool surv = act && (MULTI ? ((y & 0xffffu) - tlo) < (thi - tlo) : (y & 0xffffu) < T) &&
+                                  stage_a(y, prevy, jl > 0u, nexty, jl + 1u < len, T, q_peak_min);
                 const unsigned smk = __ballot_sync(0xffffffffu, surv);
                 const uint32_t ord = seen + (uint32_t)__popc(smk & lt_mask);
                 seen += (uint32_t)__popc(smk);
                 if (seen > sg.scap) stage_b(surv && ord >= sg.scap, y);
+                if (seen >= ns) break;                      // all survivors of this pass have been seen
             }
         }
         if ((uint32_t)lane < pcount) moments(lds32(pqa + ((uint32_t)lane << 2)), pdone + (uint32_t)lane);
-        if (lane == 0) line_cnt[plane * g.LS + p] = pdone + pcount;   // peaks of this line, in time order
+        if (lane == 0) {
+            if (MULTI) s_cnt[p] = pdone + pcount;           // peaks of this line so far, in time order
+            if (!MULTI || last_pass) line_cnt[plane * g.LS + p] = pdone + pcount;
+        }
     };
 
     // ---- main loop -------------------------------------------------------------------------------------------------
+    // The time axis is covered in sg.n_pass passes over the unit's lines (smaller slots -> more CTAs per SM).
+    for (uint32_t pass = 0; pass < (MULTI ? sg.n_pass : 1u); ++pass) {
+    if (MULTI) {
+        last_pass = pass + 1u == sg.n_pass;
+        tlo = pass * sg.seg_len;
+        thi = last_pass ? T : min(tlo + sg.seg_len, T);
+        wlo = tlo >= 2u ? tlo - 2u : 0u;
+        whi = min(thi + 2u, T);
+        dsub = tlo >> 3;
+    }
     // Ring index of line p is (p - (pa - 2)) mod kBSlots.  Prologue: lines pa-2 .. pa+S+1.
     for (int i = warp; i < kBS + 4; i += kBWarps) {
         stage_head(pa - 2 + i);
@@ -405,6 +460,7 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
         __syncthreads();
         vl0 = bring_at(vl0, kBS);
     }
+    }   // passes
     if (bad_order) s_unsorted = 1;
     __syncthreads();
     if (tid == 0 && s_unsorted) atomicOr(&cnt->unsorted, 1u);
@@ -412,6 +468,10 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 
 // Launches k_fused_blocks after the line index is in ws.line_start.  Returns 1 (launched), 0 (not applicable: the
 // mean line would not fit the block pool; the caller runs the bitmap kernel instead) or a negative tpc_cf error.
+//
+// Launch shape: 2 CTAs of 8 warps per SM (the kernel is latency bound — 8 -> 16 warps per SM is 1.67x faster — but
+// 20 line slots of ~5 KB leave no room for a third CTA).  Lines too long for the 254-block pool are covered in several
+// passes over the time axis (dir, pool and survivor list all scale with the segment length).
 int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
@@ -422,34 +482,57 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
     // measured on the synthetic frames: 0.38 blocks and 0.16 stage-A survivors per digit
     const double mean_blocks = 0.38 * mean_len, mean_surv = 0.16 * mean_len;
 
-    SlotGeo sg;
-    const uint32_t dir_bytes = ((((g.n_time + 9u) >> 3) + 1u) + 15u) & ~15u;
-    sg.pool_off = kDirOff + dir_bytes;
-    sg.scap = (((uint32_t)(mean_surv * 1.6) + 24u) + 3u) & ~3u;
-    const uint32_t fixed = kBWarps * (kStageDepth * 256u + 256u);
-    const uint32_t budget = 110u * 1024u;                          // 2 CTAs per SM
-    uint32_t want = (uint32_t)(mean_blocks * 1.5) + 32u;           // blocks incl. the zero block
-    if (want > 255u) want = 255u;
-    const uint32_t per_slot_fixed = sg.pool_off + 4u * sg.scap;
-    if (fixed + kBSlots * (per_slot_fixed + 16u * 8u) > budget) return 0;
-    uint32_t fit = ((budget - fixed) / kBSlots - per_slot_fixed) / 16u;
-    sg.pcap = want < fit ? want : fit;
-    if (const char* e = getenv("TPC_CF_BLOCK_POOL")) {             // test knob: force a small pool (slow paths)
-        const int v = atoi(e);
-        if (v >= 2 && v <= 255) sg.pcap = (uint32_t)v;
-    }
-    if (const char* e = getenv("TPC_CF_SURV_CAP")) {
-        const int v = atoi(e);
-        if (v >= 4 && v <= 4096) sg.scap = (uint32_t)v & ~3u;
-    }
     const char* force = getenv("TPC_CF_FUSED_KERNEL");            // "blocks" | "lines" (tests, profiling)
     const bool forced = force && force[0] == 'b';
     if (force && force[0] == 'l') return 0;
-    if (!forced && (double)sg.pcap < mean_blocks * 1.2 + 8.0) return 0;   // too many lines would overflow the pool
+    int env_pass = 0;                                              // tuning / test knob
+    if (const char* e = getenv("TPC_CF_PASSES")) env_pass = atoi(e);
+
+    const uint32_t fixed = kBWarps * (kStageDepth * 256u + 256u);
+    const uint32_t budget = 227u * 1024u / 2u - 1024u - 3328u;     // 2 CTAs per SM: - 1 KB reserved - ~3.2 KB static
+    auto shape = [&](uint32_t n_pass, bool must, SlotGeo* out) -> bool {
+        SlotGeo sg;
+        sg.n_pass = n_pass;
+        sg.seg_len = (((g.n_time + n_pass - 1u) / n_pass) + 7u) & ~7u;
+        const uint32_t dir_bytes = ((sg.seg_len >> 3) + 2u + 15u) & ~15u;
+        sg.pool_off = kDirOff + dir_bytes;
+        const double mb = mean_blocks / n_pass + (n_pass > 1 ? 1.0 : 0.0), ms = mean_surv / n_pass;
+        sg.scap = (((uint32_t)(ms * 1.6) + 16u) + 3u) & ~3u;
+        uint32_t want = (uint32_t)(mb * 1.5) + 24u;                // blocks incl. the zero block
+        if (want > 255u) want = 255u;
+        const uint32_t per_slot_fixed = sg.pool_off + 4u * sg.scap;
+        if (fixed + kBSlots * (per_slot_fixed + 16u * 8u) > budget) return false;
+        const uint32_t fit = ((budget - fixed) / kBSlots - per_slot_fixed) / 16u;
+        sg.pcap = want < fit ? want : fit;
+        if (!must && (double)sg.pcap < mb * 1.25 + 8.0) return false;   // too many lines would overflow the pool
+        *out = sg;
+        return true;
+    };
+    // Passes: 1 when the mean line fits the pool, else the fewest that do (each pass costs a partly used chunk and a
+    // partly filled survivor / peak batch per line, so fewer is better: measured 1.90 -> 2.87 ms at 2 passes on config 3).
+    SlotGeo sg;
+    bool have = false;
+    for (uint32_t np = 1; np <= 6 && !have; ++np) {
+        if (env_pass && (int)np != env_pass) continue;
+        if (np > 1 && g.n_time < 64u * np) break;
+        have = shape(np, false, &sg);
+    }
+    if (!have) {
+        if (!forced) return 0;
+        const uint32_t np = env_pass >= 1 && env_pass <= 8 && g.n_time >= 64u * (uint32_t)env_pass ? (uint32_t)env_pass : 1u;
+        if (!shape(np, true, &sg)) return 0;
+    }
+    if (const char* e = getenv("TPC_CF_BLOCK_POOL")) {             // test knob: force a small pool (slow paths)
+        const int v = atoi(e);
+        if (v >= 2 && v <= 255 && (uint32_t)v <= sg.pcap) sg.pcap = (uint32_t)v;
+    }
+    if (const char* e = getenv("TPC_CF_SURV_CAP")) {
+        const int v = atoi(e);
+        if (v >= 4 && (uint32_t)v <= sg.scap) sg.scap = (uint32_t)v & ~3u;
+    }
     sg.surv_off = sg.pool_off + 16u * sg.pcap;
     sg.slot_bytes = sg.surv_off + 4u * sg.scap;
     const uint32_t smem = kBSlots * sg.slot_bytes + fixed;
-    if (smem > 200u * 1024u) return 0;
 
     const uint32_t whole = (g.max_pads + kBS - 1) / kBS * kBS;
     uint32_t pads_per_unit = g.n_planes >= 1184 ? whole : (g.n_planes >= 296 ? 6 * kBS : 3 * kBS);
@@ -461,15 +544,17 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_fused_blocks, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_fused_blocks<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_blocks<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
         if (e != cudaSuccess) return TPC_CF_E_CUDA;
         attr_set = true;
     }
     if (ev_k0) cudaEventRecord(ev_k0, st);
     g_last_kernel = "k_fused_blocks";
-    k_fused_blocks<<<g.n_planes * upp, kBThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
-                                                              pads_per_unit, upp, sg, q_peak_min, q_gate,
-                                                              ws.counters, ws.line_cnt, (uint4*)ws.stage);
+    auto kern = sg.n_pass > 1 ? k_fused_blocks<true> : k_fused_blocks<false>;
+    kern<<<g.n_planes * upp, kBThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
+                                                    pads_per_unit, upp, sg, q_peak_min, q_gate,
+                                                    ws.counters, ws.line_cnt, (uint4*)ws.stage);
     if (ev_k1) cudaEventRecord(ev_k1, st);
     return 1;
 }

@@ -39,19 +39,22 @@ def parse_golden(path=GOLDEN):
 # flags: DIGITS_SORTED=1, FORCE_GENERAL=2.  "fused" lets the library choose the fused kernel from the mean line length;
 # "fused_blocks" / "fused_lines" force the block-sparse / bitmap line-slot kernel (TPC_CF_FUSED_KERNEL), so that each
 # runs every case — including the ones far outside its range, which exercise its exact slow paths.
-PATHS = {"general": 0, "general_hint": 3, "fused": 1, "fused_blocks": 1, "fused_lines": 1}
-FUSED_KERNEL = {"fused_blocks": "k_fused_blocks", "fused_lines": "k_fused_lines"}
+# "fused_blocks_p3" additionally covers the time axis in 3 passes (TPC_CF_PASSES), the shape long lines get.
+PATHS = {"general": 0, "general_hint": 3, "fused": 1, "fused_blocks": 1, "fused_blocks_p3": 1, "fused_lines": 1}
+FUSED_KERNEL = {"fused_blocks": "k_fused_blocks", "fused_blocks_p3": "k_fused_blocks", "fused_lines": "k_fused_lines"}
 
 
 @pytest.fixture(autouse=True)
 def _fused_kernel_env(request, monkeypatch):
     """Sets the library's kernel-selection knob from the test's `path` parameter (read with getenv at every run)."""
     params = getattr(getattr(request.node, "callspec", None), "params", {})
-    for k in ("TPC_CF_FUSED_KERNEL", "TPC_CF_BLOCK_POOL", "TPC_CF_SURV_CAP"):
+    for k in ("TPC_CF_FUSED_KERNEL", "TPC_CF_BLOCK_POOL", "TPC_CF_SURV_CAP", "TPC_CF_PASSES"):
         monkeypatch.delenv(k, raising=False)
     path = params.get("path")
     if path in FUSED_KERNEL:
-        monkeypatch.setenv("TPC_CF_FUSED_KERNEL", "blocks" if path == "fused_blocks" else "lines")
+        monkeypatch.setenv("TPC_CF_FUSED_KERNEL", "lines" if path == "fused_lines" else "blocks")
+        if path == "fused_blocks_p3":
+            monkeypatch.setenv("TPC_CF_PASSES", "3")
     yield
 
 
@@ -324,14 +327,16 @@ def test_dense_isolated_peaks_overflow_the_peak_queue(path):
     assert_clusters_equal(cl, ora, "dense isolated peaks/" + path)
 
 
+@pytest.mark.parametrize("passes", [1, 2, 5])
 @pytest.mark.parametrize("pool,scap", [(2, 4), (9, 8), (40, 4), (255, 12)])
-def test_block_kernel_slow_paths(pool, scap, monkeypatch):
+def test_block_kernel_slow_paths(pool, scap, passes, monkeypatch):
     """k_fused_blocks with a block pool / survivor list far too small for the data (TPC_CF_BLOCK_POOL,
     TPC_CF_SURV_CAP): window cells whose block is not in the pool are looked up in the digit array, survivors beyond
     the list are re-derived from the digit array.  Results must not change (config 1, and a ~5 % single row)."""
     monkeypatch.setenv("TPC_CF_FUSED_KERNEL", "blocks")
     monkeypatch.setenv("TPC_CF_BLOCK_POOL", str(pool))
     monkeypatch.setenv("TPC_CF_SURV_CAP", str(scap))
+    monkeypatch.setenv("TPC_CF_PASSES", str(passes))
     digits = gen.generate(1)
     geom = gen.geometry(1)
     ora, ost = orc.run(digits, *geom[:4], npads=geom[4])
