@@ -38,14 +38,15 @@ def load_peaks():
         return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
 
 
-def load_traffic(workload, path):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture, or None."""
+def load_traffic(workload, path, kernel):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture, or None (also None
+    when the capture is of another kernel than the one that ran)."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     try:
         with open(p) as f:
             t = json.load(f)
         e = t.get("%s/%s" % (workload, path))
-        return float(e["dram_bytes_per_launch"]) if e else None
+        return float(e["dram_bytes_per_launch"]) if e and e.get("kernel") == kernel else None
     except Exception:
         return None
 
@@ -131,10 +132,12 @@ def time_oracle(digits, geom, n_sectors_sample):
     return dt, st
 
 
-def sample_sectors(cfg_id):
-    # ~8 ms per 138x14336 plane single-threaded => 8 sectors (1216 planes) ~ 10-15 s; config 1/2 have one sector
+def sample_sectors(cfg_id, per_step=False):
+    # measured ~2 ms per 138x14336 plane single-threaded (config 3): the whole frame is ~11 s (config 4 ~28 s), which
+    # is the cpu_baseline sample; the --impl reference arm times 8 sectors per step (~2.5 s) so that K + W steps
+    # end within minutes.  config 1/2 have one sector.
     from datagen import gen
-    return min(gen.CONFIGS[cfg_id]["n_sectors"], 8)
+    return min(gen.CONFIGS[cfg_id]["n_sectors"], 8 if per_step else 36)
 
 
 def run_reference(args):
@@ -145,7 +148,7 @@ def run_reference(args):
     from datagen import gen
     from oracle import oracle as orc
     orc.build()
-    ns = sample_sectors(args.config)
+    ns = sample_sectors(args.config, per_step=True)
     digits, geom = oracle_sample(args.config, ns)
     for _ in range(min(args.warmup, 1)):
         time_oracle(digits, geom, ns)
@@ -233,6 +236,7 @@ def main():
             raise RuntimeError("bench run invalid: status %r" % (st,))
     n_clusters = [st["n_clusters"] for st in sts]
     launches_per_step = finder.last_launch_count() * n_frames
+    dominant_kernel = finder.last_kernel()
 
     # ---- timed region: K steps, device-resident inputs (each frame > L2, so no L2 flush is needed) ----
     finder.set_profiling(True)
@@ -297,12 +301,11 @@ def main():
     # ---- roofline of the dominant kernel (HBM-bound: stencil/compaction work, no contraction) ----
     peak, peak_src = load_peaks()
     nd, nc = n_digits[-1], n_clusters[-1]     # per launch: one frame
+    kname = dominant_kernel
     if args.path == "fused":
-        kname = "k_fused_lines"
-        # algorithmic bytes per launch: 8 B/digit read, 32 B/cluster staged, 1 bit/digit peak mask
-        alg_bytes = 8.0 * nd + 32.0 * nc + nd / 8.0
+        # algorithmic bytes per launch: 8 B/digit read, 32 B/cluster staged, 4 B per pad line (peak count)
+        alg_bytes = 8.0 * nd + 32.0 * nc + 4.0 * geom[0] * geom[1] * geom[2]
     else:
-        kname = "k_peaks_map"
         # 8 B/digit read + 3x3 neighbourhood of every digit >= threshold is covered by the 2 B/digit map cells of
         # three lines (each map sector counted once) + 32 B/cluster staged + peak mask
         alg_bytes = 8.0 * nd + 2.0 * nd + 32.0 * nc + nd / 8.0
@@ -310,7 +313,7 @@ def main():
     roof = {"bound": "hbm", "kernel": kname, "achieved": (alg_bytes / (k_ms * 1e-3) / 1e9) if k_ms else None,
             "peak": peak, "unit": "GB/s", "peak_source": peak_src,
             "frac": (alg_bytes / (k_ms * 1e-3) / 1e9 / peak) if k_ms else None,
-            "traffic": load_traffic("config%d" % args.config, args.path),
+            "traffic": load_traffic("config%d" % args.config, args.path, kname),
             "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms,
             "kernel_share_of_step": (k_ms * n_frames / ms_per_step) if k_ms else None}
     io_bytes = 8.0 * digits_per_step + 32.0 * clusters_per_step
