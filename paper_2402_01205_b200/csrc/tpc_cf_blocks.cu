@@ -328,8 +328,16 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
         const uint32_t gl = s_ls[p], lend = s_ls[p + 1];
         if (lend == gl) return;                             // line_cnt stays 0 (cleared per run)
         uint32_t sl[5];                                     // slots of lines p-2 .. p+2 (empty outside the plane, R2)
+        {
+            const uint32_t ring_end = sm0 + kBSlots * sg.slot_bytes;
+            uint32_t a0 = sm0 + (uint32_t)bring_at(vp, -2) * sg.slot_bytes;
 #pragma unroll
-        for (int a = 0; a < 5; ++a) sl[a] = sm0 + (uint32_t)bring_at(vp, a - 2) * sg.slot_bytes;
+            for (int a = 0; a < 5; ++a) {
+                sl[a] = a0;
+                a0 += sg.slot_bytes;
+                if (a0 == ring_end) a0 = sm0;
+            }
+        }
         const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
         uint32_t pcount = 0, pdone = MULTI ? s_cnt[p] : 0u; // warp-uniform: queued / already written peaks of the line
 
@@ -399,7 +407,37 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
                 if (seen >= ns) break;                      // all survivors of this pass have been seen
             }
         }
-        if ((uint32_t)lane < pcount) moments(lds32(pqa + ((uint32_t)lane << 2)), pdone + (uint32_t)lane);
+        if (pcount > 16u) {
+            if ((uint32_t)lane < pcount) moments(lds32(pqa + ((uint32_t)lane << 2)), pdone + (uint32_t)lane);
+        } else if (pcount > 0u) {
+            // the usual case (a line has ~14 peaks): two lanes per peak, each gathers the rows on one side of the
+            // peak plus the peak's row (3 windows instead of 5); the halves of the integer sums are added by shuffle
+            const uint32_t i = (uint32_t)lane & 15u;
+            const bool neg = lane >= 16;                        // this lane takes dp < 0 (lines p-2, p-1)
+            const bool valid = i < pcount;
+            ClusterSums h = {0, 0, 0, 0, 0};
+            uint32_t y = 0u;
+            if (valid) {
+                y = lds32(pqa + (i << 2));
+                const int t = (int)(y & 0xffffu);
+                int o[5], m[5], z[5];
+                bwindow<2>(neg ? sl[0] : sl[4], MULTI ? dsub : 0u, sg, t, o, digits, s_ls, neg ? p - 2 : p + 2, P, T);
+                bwindow<2>(neg ? sl[1] : sl[3], MULTI ? dsub : 0u, sg, t, m, digits, s_ls, neg ? p - 1 : p + 1, P, T);
+                bwindow<2>(sl[2], MULTI ? dsub : 0u, sg, t, z, digits, s_ls, p, P, T);
+                h = cluster_half_sums(o, m, z, neg ? -1 : 1, !neg, q_gate);
+            }
+            h.S0 += __shfl_xor_sync(0xffffffffu, h.S0, 16);
+            h.S1p += __shfl_xor_sync(0xffffffffu, h.S1p, 16);
+            h.S1t += __shfl_xor_sync(0xffffffffu, h.S1t, 16);
+            h.S2p += __shfl_xor_sync(0xffffffffu, h.S2p, 16);
+            h.S2t += __shfl_xor_sync(0xffffffffu, h.S2t, 16);
+            if (valid && !neg) {
+                const ClusterWords r = cluster_finish(h, w0_line, y & 0xffffu, y >> 16);
+                const size_t j = (size_t)gl + pdone + i;
+                stage[2 * j] = r.lo;
+                stage[2 * j + 1] = r.hi;
+            }
+        }
         if (lane == 0) {
             if (MULTI) s_cnt[p] = pdone + pcount;           // peaks of this line so far, in time order
             if (!MULTI || last_pass) line_cnt[plane * g.LS + p] = pdone + pcount;

@@ -75,11 +75,36 @@ __device__ __forceinline__ uint64_t key40(uint32_t w0, uint32_t w1)
 // Sums are integers taken relative to the peak, |S| <= 25*65535*4 < 2^24 (R8), so any order is exact;
 // the variance numerator S0*S2 - S1^2 is formed in int64 and rounded once.
 struct ClusterWords { uint4 lo, hi; };
+struct ClusterSums { int S0, S1p, S1t, S2p, S2t; };   // integer sums relative to the peak cell (R8)
+
+// R7: record from the sums.  qmax = charge of the peak cell.
+__device__ __forceinline__ ClusterWords cluster_finish(const ClusterSums& m, uint32_t w0, uint32_t time, uint32_t qmax)
+{
+    const uint32_t pad = (w0 >> 16) & 0xffu;
+    const float f0 = (float)m.S0;
+    const float den = f0 * f0;
+    const long long np = (long long)m.S0 * m.S2p - (long long)m.S1p * m.S1p;
+    const long long nt = (long long)m.S0 * m.S2t - (long long)m.S1t * m.S1t;
+    const float pad_mean = (float)pad + (float)m.S1p / f0;      // R7
+    const float time_mean = (float)time + (float)m.S1t / f0;
+    const float sp = sqrtf(fmaxf((float)np, 0.f) / den);
+    const float st = sqrtf(fmaxf((float)nt, 0.f) / den);
+    ClusterWords r;
+    r.lo.x = w0 & 0x00ffffffu;                                // sector,row,pad,flags=0
+    r.lo.y = time | (qmax << 16);                             // time,qmax
+    r.lo.z = (uint32_t)m.S0;                                  // qtot
+    r.lo.w = __float_as_uint(pad_mean);
+    r.hi.x = __float_as_uint(time_mean);
+    r.hi.y = __float_as_uint(sp);
+    r.hi.z = __float_as_uint(st);
+    r.hi.w = 0u;
+    return r;
+}
 
 __device__ __forceinline__ ClusterWords cluster_from_window(const int (&c)[5][5], uint32_t w0, uint32_t time,
                                                             uint32_t gate)
 {
-    int S0 = 0, S1p = 0, S1t = 0, S2p = 0, S2t = 0;
+    ClusterSums m = {0, 0, 0, 0, 0};
 #pragma unroll
     for (int a = 0; a < 5; ++a) {
 #pragma unroll
@@ -91,27 +116,34 @@ __device__ __forceinline__ ClusterWords cluster_from_window(const int (&c)[5][5]
                 const int ga = a - (dp > 0) + (dp < 0), gb = b - (dt > 0) + (dt < 0);
                 v = ((uint32_t)c[ga][gb] >= gate) ? v : 0;
             }
-            S0 += v; S1p += v * dp; S1t += v * dt; S2p += v * dp * dp; S2t += v * dt * dt;
+            m.S0 += v; m.S1p += v * dp; m.S1t += v * dt; m.S2p += v * dp * dp; m.S2t += v * dt * dt;
         }
     }
-    const uint32_t pad = (w0 >> 16) & 0xffu;
-    const float f0 = (float)S0;
-    const float den = f0 * f0;
-    const long long np = (long long)S0 * S2p - (long long)S1p * S1p;
-    const long long nt = (long long)S0 * S2t - (long long)S1t * S1t;
-    const float pad_mean = (float)pad + (float)S1p / f0;      // R7
-    const float time_mean = (float)time + (float)S1t / f0;
-    const float sp = sqrtf(fmaxf((float)np, 0.f) / den);
-    const float st = sqrtf(fmaxf((float)nt, 0.f) / den);
-    ClusterWords r;
-    r.lo.x = w0 & 0x00ffffffu;                                // sector,row,pad,flags=0
-    r.lo.y = time | ((uint32_t)c[2][2] << 16);                // time,qmax
-    r.lo.z = (uint32_t)S0;                                    // qtot
-    r.lo.w = __float_as_uint(pad_mean);
-    r.hi.x = __float_as_uint(time_mean);
-    r.hi.y = __float_as_uint(sp);
-    r.hi.z = __float_as_uint(st);
-    r.hi.w = 0u;
+    return cluster_finish(m, w0, time, (uint32_t)c[2][2]);
+}
+
+// One half of the same sums, for two lanes sharing a peak: the rows on one side of the peak (o: |dp| = 2, m: |dp| = 1,
+// sgn = sign of dp) and, if with_center, the peak's own row z.  The gate of an outer cell lies one step towards the
+// peak (R3): row o is gated by row m, the dt = +-2 cells of rows m and z by z[1] / z[3] — so a half needs rows o, m, z
+// only, and the two halves add up to cluster_from_window's sums exactly (integers).
+__device__ __forceinline__ ClusterSums cluster_half_sums(const int (&o)[5], const int (&m)[5], const int (&z)[5],
+                                                         int sgn, bool with_center, uint32_t gate)
+{
+    ClusterSums r = {0, 0, 0, 0, 0};
+#pragma unroll
+    for (int b = 0; b < 5; ++b) {
+        const int dt = b - 2;
+        const int gb = b - (dt > 0) + (dt < 0);                       // dt one step towards the peak
+        const int vo = ((uint32_t)m[gb] >= gate) ? o[b] : 0;          // |dp| = 2: gate (|dp| = 1, dt -+ 1)
+        const bool edge = dt == 2 || dt == -2;
+        const int vm = (!edge || (uint32_t)z[gb] >= gate) ? m[b] : 0; // |dp| = 1: only dt = +-2 is gated, by (0, +-1)
+        const int vz = (with_center && (!edge || (uint32_t)z[gb] >= gate)) ? z[b] : 0;
+        r.S0 += vo + vm + vz;
+        r.S1p += sgn * (2 * vo + vm);
+        r.S1t += dt * (vo + vm + vz);
+        r.S2p += 4 * vo + vm;
+        r.S2t += dt * dt * (vo + vm + vz);
+    }
     return r;
 }
 
