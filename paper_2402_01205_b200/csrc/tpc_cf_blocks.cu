@@ -116,15 +116,34 @@ struct SlotGeo {
     uint32_t seg_len;      // time bins per segment (multiple of 8); n_pass * seg_len >= n_time
 };
 
+// Slow path of bwindow (rare: a block of the window is not in the pool): cells of missing blocks come from the digit
+// array.  Out of line, result in registers, to keep the hot code small.
+struct Win5 { int c[5]; };
+__device__ __noinline__ Win5 bwindow_slow(uint32_t aA, uint32_t aB, uint32_t dA, uint32_t dB, uint32_t o, int t0, int n,
+                                          const uint2* __restrict__ digits, uint32_t gl, uint32_t glen, uint32_t T)
+{
+    Win5 r;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const bool inA = o + (uint32_t)k < 8u;
+        const uint32_t d = inA ? dA : dB;
+        r.c[k] = k >= n ? 0
+               : (d != 0xFFu ? (int)lds16((inA ? aA : aB) + 2u * (uint32_t)k)
+                             : (int)cell_from_digits(digits, gl, glen, (uint32_t)(t0 + k), T));
+    }
+    return r;
+}
+
 // charges of the window t-H..t+H of the line in slot `slot` (0 where no digit): c[k] is time t-H+k.
-// lidx = pad index of that line, used only by the slow path (line_start lookups in s_ls).
+// dsub = first time bin of the pass / 8.  lidx = pad index of that line, used only by the slow path (line_start
+// lookups in s_ls).
 template <int H>
 __device__ __forceinline__ void bwindow(uint32_t slot, uint32_t dsub, const SlotGeo& sg, int t, int (&c)[2 * H + 1],
                                         const uint2* __restrict__ digits, const uint32_t* s_ls, int lidx, int P,
                                         uint32_t T)
 {
     const uint32_t u = (uint32_t)(t + 8 - H);                 // first cell, shifted by the 8-bin guard block
-    const uint32_t dir = slot + kDirOff - dsub;               // dsub = first time bin of the pass / 8
+    const uint32_t dir = slot + kDirOff - dsub;
     const uint32_t dA = lds8(dir + (u >> 3));
     const uint32_t dB = lds8(dir + ((u + 2 * H) >> 3));
     const uint32_t o = u & 7u;
@@ -133,17 +152,13 @@ __device__ __forceinline__ void bwindow(uint32_t slot, uint32_t dsub, const Slot
     if (dA != 0xFFu && dB != 0xFFu) {
 #pragma unroll
         for (int k = 0; k < 2 * H + 1; ++k) c[k] = (int)lds16((o + (uint32_t)k < 8u ? aA : aB) + 2u * (uint32_t)k);
-    } else {                                                   // rare: a block of this window is not in the pool
+    } else {
         const bool inside = lidx >= 0 && lidx < P;
         const uint32_t gl = inside ? s_ls[lidx] : 0u;
         const uint32_t glen = inside ? s_ls[lidx + 1] - gl : 0u;
+        const Win5 r = bwindow_slow(aA, aB, dA, dB, o, t - H, 2 * H + 1, digits, gl, glen, T);
 #pragma unroll
-        for (int k = 0; k < 2 * H + 1; ++k) {
-            const bool inA = o + (uint32_t)k < 8u;
-            const uint32_t d = inA ? dA : dB;
-            c[k] = d != 0xFFu ? (int)lds16((inA ? aA : aB) + 2u * (uint32_t)k)
-                              : (int)cell_from_digits(digits, gl, glen, (uint32_t)(t - H + k), T);
-        }
+        for (int k = 0; k < 2 * H + 1; ++k) c[k] = r.c[k];
     }
 }
 
