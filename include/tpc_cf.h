@@ -117,7 +117,12 @@ int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n,
 
 /* End-to-end convenience used by bench.py's `e2e` leg: HOST digits in (pinned or pageable), HOST clusters and
  * status out; copies host->device, runs, copies the status and the clusters back, synchronises the stream.
- * dev_digits / dev_clusters / dev_status are caller-owned DEVICE staging buffers (max_digits / capacity / 1). */
+ * dev_digits / dev_clusters / dev_status are caller-owned DEVICE staging buffers (max_digits / capacity / 1).
+ * A frame of >= 4 Mi digits in >= 2 sectors that carries TPC_CF_DIGITS_SORTED is pipelined over groups of whole
+ * sectors (sectors are independent, R2): the copy-in of the next group, the run of the current one and the copy-out of
+ * the previous one overlap on three streams (two of them internal to the handle); with pinned host buffers the call
+ * then costs about the host->device copy alone.  The result is the same array.  A false promise, or a group that
+ * needs more than its share of `capacity`, falls back to the single-shot route by itself. */
 int tpc_cf_run_host(tpc_cf* h, const tpc_digit* host_digits, uint64_t n,
                     const tpc_cf_geometry* geom, const tpc_cf_params* params,
                     tpc_digit* dev_digits, tpc_cluster* dev_clusters, tpc_cf_status* dev_status,

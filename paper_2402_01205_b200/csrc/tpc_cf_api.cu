@@ -9,6 +9,7 @@
 using namespace tpccf;
 
 static constexpr int kProfSlots = 64;
+static constexpr int kMaxGroups = 12;    // sector groups of the tpc_cf_run_host pipeline
 
 struct tpc_cf {
     Geo geo;
@@ -21,6 +22,11 @@ struct tpc_cf {
     int profiling;
     uint32_t run_index;         // runs since profiling was switched on
     cudaEvent_t ev[kProfSlots][4];   // per slot: run begin, dominant kernel begin, dominant kernel end, run end
+    // tpc_cf_run_host pipeline (created on first use): copy-in / copy-out streams, per-group events, pinned status
+    bool pipe_ready;
+    cudaStream_t s_in, s_out;
+    cudaEvent_t ev_fork, ev_join, ev_in[kMaxGroups], ev_run[kMaxGroups];
+    tpc_cf_status* pinned_status;    // [kMaxGroups], cudaHostAlloc
     char cuda_msg[256];
 };
 
@@ -81,6 +87,7 @@ static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, ch
     w.line_cnt = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
     w.line_off = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
     w.line_part = (uint32_t*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 1024) + 1) * 4);
+    w.group_status = (tpc_cf_status*)take(sizeof(tpc_cf_status) * 16);
     if (ws) *ws = w;
     if (n_sort_tiles) *n_sort_tiles = (uint32_t)tiles;
     if (map_bytes) *map_bytes = mapb;
@@ -193,6 +200,109 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     return TPC_CF_OK;
 }
 
+static bool ensure_pipe(tpc_cf* h)
+{
+    if (h->pipe_ready) return true;
+    bool ok = cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; ok && i < kMaxGroups; ++i)
+        ok = cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&h->ev_run[i], cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaHostAlloc((void**)&h->pinned_status, sizeof(tpc_cf_status) * kMaxGroups, cudaHostAllocDefault) == cudaSuccess;
+    if (!ok) { (void)cudaGetLastError(); return false; }    // leaks a few handles on a failing device; caller falls back
+    h->pipe_ready = true;
+    return true;
+}
+
+// first index in host digits [0, n) whose sector is >= s (digits promised sorted; terminates on any input)
+static uint64_t host_lower_bound_sector(const tpc_digit* d, uint64_t n, uint32_t s)
+{
+    uint64_t lo = 0, hi = n;
+    while (lo < hi) {
+        const uint64_t mid = lo + ((hi - lo) >> 1);
+        if (d[mid].sector < s) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+// Sorted frames are pipelined over groups of whole sectors: the copy-in of group g+1 (stream s_in) overlaps the run of
+// group g (caller's stream) and the copy-out of group g-1 (stream s_out).  Sectors are independent (R2), groups are in
+// sector order, so the concatenated outputs are the frame's output.  Returns 1 if the frame was delivered, 0 if the
+// caller must take the single-shot route (false promise, a group over its share of the capacity, CUDA hiccup in the
+// pipeline set-up), < 0 on error.
+static int run_host_pipelined(tpc_cf* h, const tpc_digit* host_digits, uint64_t n, const tpc_cf_geometry* geom,
+                              const tpc_cf_params* params, tpc_digit* dev_digits, tpc_cluster* dev_clusters,
+                              tpc_cluster* host_clusters, uint64_t capacity, tpc_cf_status* host_status,
+                              cudaStream_t st, bool* digits_on_device)
+{
+    if (!ensure_pipe(h)) return 0;
+    // group boundaries: sector-aligned, near equal digit counts
+    uint64_t b[kMaxGroups + 1];
+    int G = 0;
+    b[0] = 0;
+    const int want = (int)(geom->n_sectors < (uint32_t)kMaxGroups ? geom->n_sectors : (uint32_t)kMaxGroups);
+    for (int g = 1; g < want; ++g) {
+        const uint64_t probe = n * (uint64_t)g / (uint64_t)want;
+        const uint64_t cut = host_lower_bound_sector(host_digits, n, host_digits[probe].sector);
+        if (cut > b[G] && cut < n) b[++G] = cut;
+    }
+    b[++G] = n;
+    if (G < 2) return 0;
+
+    cudaError_t e = cudaEventRecord(h->ev_fork, st);                 // earlier work on the caller's stream comes first
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(h->s_in, h->ev_fork, 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(h->s_out, h->ev_fork, 0);
+    for (int g = 0; e == cudaSuccess && g < G; ++g) {
+        e = cudaMemcpyAsync(dev_digits + b[g], host_digits + b[g], (b[g + 1] - b[g]) * sizeof(tpc_digit),
+                            cudaMemcpyHostToDevice, h->s_in);
+        if (e == cudaSuccess) e = cudaEventRecord(h->ev_in[g], h->s_in);
+    }
+    if (e != cudaSuccess) return cuda_fail(h, e, "pipeline H2D");
+    *digits_on_device = true;                                        // (once s_in has drained)
+    uint64_t off[kMaxGroups + 1];
+    off[0] = 0;
+    for (int g = 0; g < G; ++g) {
+        const uint64_t ng = b[g + 1] - b[g];
+        const uint64_t cap = g + 1 < G ? (uint64_t)((double)capacity * ((double)ng / (double)n)) : capacity - off[g];
+        off[g + 1] = off[g] + cap;
+        e = cudaStreamWaitEvent(st, h->ev_in[g], 0);
+        if (e != cudaSuccess) return cuda_fail(h, e, "pipeline wait");
+        tpc_cf_out out = { dev_clusters + off[g], cap, h->ws.group_status + g, (void*)st };
+        const int rc = tpc_cf_run(h, dev_digits + b[g], ng, geom, params, &out);
+        if (rc != TPC_CF_OK) { cudaStreamSynchronize(h->s_in); cudaStreamSynchronize(st); return rc; }
+        e = cudaMemcpyAsync(h->pinned_status + g, h->ws.group_status + g, sizeof(tpc_cf_status), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaEventRecord(h->ev_run[g], st);
+        if (e != cudaSuccess) return cuda_fail(h, e, "pipeline status");
+    }
+    tpc_cf_status tot;
+    memset(&tot, 0, sizeof tot);
+    tot.path = 3;
+    bool redo = false;
+    for (int g = 0; g < G; ++g) {
+        e = cudaEventSynchronize(h->ev_run[g]);
+        if (e != cudaSuccess) return cuda_fail(h, e, "pipeline sync");
+        const tpc_cf_status s = h->pinned_status[g];
+        if (s.path != 3 || s.overflow) redo = true;                  // false promise / group over its share
+        if (redo) continue;
+        if (s.n_clusters) {
+            e = cudaMemcpyAsync(host_clusters + tot.n_clusters, dev_clusters + off[g], s.n_clusters * sizeof(tpc_cluster),
+                                cudaMemcpyDeviceToHost, h->s_out);
+            if (e != cudaSuccess) return cuda_fail(h, e, "pipeline D2H");
+        }
+        tot.n_clusters += s.n_clusters;
+        tot.n_digits_used += s.n_digits_used;
+        tot.n_bad_digits += s.n_bad_digits;
+    }
+    e = cudaStreamSynchronize(h->s_out);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->s_in);
+    if (e != cudaSuccess) return cuda_fail(h, e, "pipeline drain");
+    if (redo) return 0;
+    *host_status = tot;
+    return 1;
+}
+
 extern "C" int tpc_cf_run_host(tpc_cf* h, const tpc_digit* host_digits, uint64_t n, const tpc_cf_geometry* geom,
                                const tpc_cf_params* params, tpc_digit* dev_digits, tpc_cluster* dev_clusters,
                                tpc_cf_status* dev_status, tpc_cluster* host_clusters, uint64_t capacity,
@@ -202,7 +312,14 @@ extern "C" int tpc_cf_run_host(tpc_cf* h, const tpc_digit* host_digits, uint64_t
     if (capacity && (!dev_clusters || !host_clusters)) return TPC_CF_E_NULL;
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e = cudaSuccess;
-    if (n) e = cudaMemcpyAsync(dev_digits, host_digits, n * sizeof(tpc_digit), cudaMemcpyHostToDevice, st);
+    bool on_device = false;
+    const bool sorted_hint = (params->flags & TPC_CF_DIGITS_SORTED) && !(params->flags & TPC_CF_FORCE_GENERAL);
+    if (sorted_hint && geom && geom->n_sectors >= 2 && n >= (1u << 22) && n <= h->max_digits && capacity >= 1024) {
+        const int r = run_host_pipelined(h, host_digits, n, geom, params, dev_digits, dev_clusters, host_clusters,
+                                         capacity, host_status, st, &on_device);
+        if (r != 0) return r < 0 ? r : TPC_CF_OK;
+    }
+    if (n && !on_device) e = cudaMemcpyAsync(dev_digits, host_digits, n * sizeof(tpc_digit), cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemcpyAsync(H2D digits)");
     tpc_cf_params prm = *params;
     for (int attempt = 0; attempt < 2; ++attempt) {
@@ -269,6 +386,12 @@ extern "C" int tpc_cf_destroy(tpc_cf* h)
 {
     if (!h) return TPC_CF_E_NULL;
     for (int i = 0; i < kProfSlots * 4; ++i) cudaEventDestroy(h->ev[i / 4][i % 4]);
+    if (h->pipe_ready) {
+        cudaStreamDestroy(h->s_in); cudaStreamDestroy(h->s_out);
+        cudaEventDestroy(h->ev_fork); cudaEventDestroy(h->ev_join);
+        for (int i = 0; i < kMaxGroups; ++i) { cudaEventDestroy(h->ev_in[i]); cudaEventDestroy(h->ev_run[i]); }
+        cudaFreeHost(h->pinned_status);
+    }
     delete h;
     return TPC_CF_OK;
 }

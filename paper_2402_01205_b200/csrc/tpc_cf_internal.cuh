@@ -47,6 +47,7 @@ struct Workspace {
     uint32_t* line_cnt;   // [n_planes*LS + 1] peaks per line (fused path)
     uint32_t* line_off;   // exclusive scan of line_cnt
     uint32_t* line_part;  // scan partials for the line counts
+    tpc_cf_status* group_status;   // [16] per-group status blocks of the tpc_cf_run_host pipeline
 };
 
 struct Handle;

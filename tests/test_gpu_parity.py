@@ -350,3 +350,44 @@ def test_block_kernel_slow_paths(pool, scap, passes, monkeypatch):
     cl, st = gpu_run(digits, geom, 1)
     assert st["kernel"] == "k_fused_blocks" and st["n_clusters"] == ost["n_clusters"]
     assert_clusters_equal(cl, ora, "config 2 (2 rows), pool %d scap %d" % (pool, scap))
+
+
+def test_run_host_pipelined_over_sector_groups():
+    """tpc_cf_run_host on a frame large enough for its sector-group pipeline (config 3 cut to 4 sectors, ~24 M digits):
+    same array as one device-resident run and as the oracle on sampled planes; a false promise (two digits swapped
+    across sectors) and a capacity too small for a group's share fall back to the single-shot route."""
+    import torch
+    cf = _cf()
+    c = dict(gen.CONFIGS[3]); c["n_sectors"] = 4
+    geom = gen.geometry(c)
+    digits = gen.generate(c)
+    n = digits.shape[0]
+    assert n >= (1 << 22)
+    f = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=n // 12)
+    d = cf.to_device(digits)
+    f.run(d, n, flags=cf.DIGITS_SORTED)
+    ref, rst = f.result()
+    ref = ref.copy()
+    pinned = torch.from_numpy(digits.view(np.uint8)).pin_memory()
+    cl, st = f.run_host(pinned, flags=cf.DIGITS_SORTED)
+    assert st["path"] == 3 and st["n_clusters"] == rst["n_clusters"] and st["n_digits_used"] == n
+    assert np.array_equal(cl.view(np.uint8), ref.view(np.uint8)), "pipelined run_host differs from the device-resident run"
+    dplane = digits["sector"].astype(np.int64) * geom[1] + digits["row"]
+    lo, hi = np.searchsorted(dplane, [2 * geom[1], 2 * geom[1] + 3])
+    ora, _ = orc.run(digits[lo:hi], *geom[:4], planes=(2 * geom[1], 2 * geom[1] + 3))
+    a, b = np.searchsorted(key(cl), [np.uint64(2) << np.uint64(32), (np.uint64(2) << np.uint64(32)) + (np.uint64(3) << np.uint64(24))])
+    assert_clusters_equal(cl[a:b].copy(), ora, "pipelined run_host, sector 2 rows 0..2")
+    # false promise: swap one digit of sector 0 with one of sector 3
+    sw = digits.copy()
+    i, j = 12345, n - 54321
+    sw[[i, j]] = sw[[j, i]]
+    cl2, st2 = f.run_host(sw, flags=cf.DIGITS_SORTED)
+    assert st2["path"] == 1 and st2["n_clusters"] == rst["n_clusters"]
+    assert np.array_equal(cl2.view(np.uint8), ref.view(np.uint8))
+    f.close()
+    # capacity that holds the frame but not a proportional share per group is still honoured
+    f = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=int(rst["n_clusters"]) + 8)
+    cl3, st3 = f.run_host(pinned, flags=cf.DIGITS_SORTED)
+    assert st3["n_clusters"] == rst["n_clusters"] and st3["overflow"] == 0
+    assert np.array_equal(cl3.view(np.uint8), ref.view(np.uint8))
+    f.close()
