@@ -2,6 +2,7 @@
 // The library never allocates device memory; the handle owns host state and a few CUDA events only.
 #include <new>
 #include <stdio.h>
+#include <time.h>
 #include <string.h>
 
 #include "tpc_cf_internal.cuh"
@@ -9,7 +10,7 @@
 using namespace tpccf;
 
 static constexpr int kProfSlots = 64;
-static constexpr int kMaxGroups = 12;    // sector groups of the tpc_cf_run_host pipeline
+static constexpr int kMaxGroups = 18;    // sector groups of the tpc_cf_run_host pipeline
 
 struct tpc_cf {
     Geo geo;
@@ -18,6 +19,7 @@ struct tpc_cf {
     uint32_t n_sort_tiles;
     size_t map_bytes;
     int last_launches;
+    uint64_t shape_n;           // digits of the whole frame while tpc_cf_run_host runs it group by group, else 0
     const char* last_kernel;
     int profiling;
     uint32_t run_index;         // runs since profiling was switched on
@@ -87,7 +89,7 @@ static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, ch
     w.line_cnt = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
     w.line_off = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
     w.line_part = (uint32_t*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 1024) + 1) * 4);
-    w.group_status = (tpc_cf_status*)take(sizeof(tpc_cf_status) * 16);
+    w.group_status = (tpc_cf_status*)take(sizeof(tpc_cf_status) * 32);
     if (ws) *ws = w;
     if (n_sort_tiles) *n_sort_tiles = (uint32_t)tiles;
     if (map_bytes) *map_bytes = mapb;
@@ -176,7 +178,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
 
     if (fused) {
         // T3: line index -> fused smem kernel (scatter into smem lines, peak test, moments) -> compaction
-        int r = launch_fused_sorted(h->geo, h->ws, digits, n, params->q_peak_min, params->q_inner_gate, st,
+        int r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n, params->q_peak_min, params->q_inner_gate, st,
                                     prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
         if (r < 0) return r;
         k += r;
@@ -270,7 +272,9 @@ static int run_host_pipelined(tpc_cf* h, const tpc_digit* host_digits, uint64_t 
         e = cudaStreamWaitEvent(st, h->ev_in[g], 0);
         if (e != cudaSuccess) return cuda_fail(h, e, "pipeline wait");
         tpc_cf_out out = { dev_clusters + off[g], cap, h->ws.group_status + g, (void*)st };
+        h->shape_n = n;
         const int rc = tpc_cf_run(h, dev_digits + b[g], ng, geom, params, &out);
+        h->shape_n = 0;
         if (rc != TPC_CF_OK) { cudaStreamSynchronize(h->s_in); cudaStreamSynchronize(st); return rc; }
         e = cudaMemcpyAsync(h->pinned_status + g, h->ws.group_status + g, sizeof(tpc_cf_status), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaEventRecord(h->ev_run[g], st);
@@ -280,8 +284,12 @@ static int run_host_pipelined(tpc_cf* h, const tpc_digit* host_digits, uint64_t 
     memset(&tot, 0, sizeof tot);
     tot.path = 3;
     bool redo = false;
+    const bool trace = getenv("TPC_CF_TRACE") != nullptr;
+    struct timespec ts0; clock_gettime(CLOCK_MONOTONIC, &ts0);
+    auto now_ms = [&]() { struct timespec t; clock_gettime(CLOCK_MONOTONIC, &t); return (t.tv_sec - ts0.tv_sec) * 1e3 + (t.tv_nsec - ts0.tv_nsec) * 1e-6; };
     for (int g = 0; g < G; ++g) {
         e = cudaEventSynchronize(h->ev_run[g]);
+        if (trace) fprintf(stderr, "group %d done at %.2f ms (digits %llu)\n", g, now_ms(), (unsigned long long)(b[g + 1] - b[g]));
         if (e != cudaSuccess) return cuda_fail(h, e, "pipeline sync");
         const tpc_cf_status s = h->pinned_status[g];
         if (s.path != 3 || s.overflow) redo = true;                  // false promise / group over its share
@@ -296,6 +304,7 @@ static int run_host_pipelined(tpc_cf* h, const tpc_digit* host_digits, uint64_t 
         tot.n_bad_digits += s.n_bad_digits;
     }
     e = cudaStreamSynchronize(h->s_out);
+    if (trace) fprintf(stderr, "copy-out drained at %.2f ms\n", now_ms());
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->s_in);
     if (e != cudaSuccess) return cuda_fail(h, e, "pipeline drain");
     if (redo) return 0;

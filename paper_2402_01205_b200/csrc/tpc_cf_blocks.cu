@@ -525,13 +525,14 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 // Launch shape: 2 CTAs of 8 warps per SM (the kernel is latency bound — 8 -> 16 warps per SM is 1.67x faster — but
 // 20 line slots of ~5 KB leave no room for a third CTA).  Lines too long for the 254-block pool are covered in several
 // passes over the time axis (dir, pool and survivor list all scale with the segment length).
-int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
+int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
     uint64_t total_pads = 0;
     for (uint32_t r = 0; r < g.n_rows; ++r) total_pads += g.npads[r];
     total_pads *= g.n_sectors;
-    const double mean_len = (double)n / (double)(total_pads ? total_pads : 1);
+    // shape_n: digits of the whole frame when this run covers only some of its sectors (tpc_cf_run_host pipeline)
+    const double mean_len = (double)(shape_n ? shape_n : n) / (double)(total_pads ? total_pads : 1);
     // measured on the synthetic frames: 0.38 blocks and 0.16 stage-A survivors per digit
     const double mean_blocks = 0.38 * mean_len, mean_surv = 0.16 * mean_len;
 

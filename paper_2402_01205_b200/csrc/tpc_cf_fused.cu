@@ -440,7 +440,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     if (tid == 0 && s_unsorted) atomicOr(&cnt->unsorted, 1u);
 }
 
-int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
+int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
@@ -454,7 +454,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
 
     // block-sparse line slots (tpc_cf_blocks.cu) when the mean line fits their pool; else the bitmap slots below
     {
-        const int r = launch_fused_blocks(g, ws, digits, n, q_peak_min, q_gate, st, ev_k0, ev_k1);
+        const int r = launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, st, ev_k0, ev_k1);
         if (r < 0) return r;
         if (r > 0) return k + r;
     }
@@ -463,7 +463,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     uint64_t total_pads = 0;
     for (uint32_t r = 0; r < g.n_rows; ++r) total_pads += g.npads[r];
     total_pads *= g.n_sectors;
-    const double mean_len = (double)n / (double)(total_pads ? total_pads : 1);
+    const double mean_len = (double)(shape_n ? shape_n : n) / (double)(total_pads ? total_pads : 1);
     const uint32_t wpl = (((g.n_time + 31) / 32 + 3) + 3u) & ~3u;   // guard word below, >= 2 above; multiple of 4
     const uint32_t pre_words = ((wpl >> 1) + 3u) & ~3u;
     uint32_t cap = ((uint32_t)(mean_len * 1.5) + 64u + 127u) & ~127u;

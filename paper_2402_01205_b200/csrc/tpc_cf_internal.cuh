@@ -47,7 +47,7 @@ struct Workspace {
     uint32_t* line_cnt;   // [n_planes*LS + 1] peaks per line (fused path)
     uint32_t* line_off;   // exclusive scan of line_cnt
     uint32_t* line_part;  // scan partials for the line counts
-    tpc_cf_status* group_status;   // [16] per-group status blocks of the tpc_cf_run_host pipeline
+    tpc_cf_status* group_status;   // [32] per-group status blocks of the tpc_cf_run_host pipeline
 };
 
 struct Handle;
@@ -161,11 +161,11 @@ int launch_scatter_only(const Geo& g, const Workspace& ws, const tpc_digit* digi
 int launch_copy_plane(const Geo& g, const Workspace& ws, uint32_t plane, uint32_t P, uint16_t* dense,
                       cudaStream_t st);
 
-int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
+int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1);
 
-int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
+int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1);
 
