@@ -31,7 +31,13 @@ class _Geometry(ctypes.Structure):
 
 class _Params(ctypes.Structure):
     _fields_ = [("q_peak_min", ctypes.c_uint16), ("q_inner_gate", ctypes.c_uint16),
-                ("flags", ctypes.c_uint32)]
+                ("flags", ctypes.c_uint32), ("q_tot_min", ctypes.c_uint32),
+                ("q_saturation", ctypes.c_uint16), ("rsv", ctypes.c_uint16)]
+
+
+# variant bits of params.flags (restated from tpc_cf_oracle.h) and cluster flag bits (V1)
+CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME = 4, 8, 16
+F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED = 1, 2, 4, 8, 16
 
 
 class _Status(ctypes.Structure):
@@ -78,7 +84,7 @@ def _geom(n_sectors, n_rows, max_pads, n_time, npads):
 
 
 def run(digits, n_sectors, n_rows, max_pads, n_time, npads=None, q_peak_min=4, q_inner_gate=2,
-        capacity=None, planes=None):
+        capacity=None, planes=None, flags=0, q_tot_min=0, q_saturation=0):
     """Run the oracle.  digits: numpy array of DIGIT (any order).  Returns (clusters, status dict).
 
     planes=(begin, end) restricts the run to planes sector*n_rows+row in [begin, end).
@@ -90,7 +96,7 @@ def run(digits, n_sectors, n_rows, max_pads, n_time, npads=None, q_peak_min=4, q
         capacity = max(n, 1)
     out = np.zeros(int(capacity), dtype=CLUSTER)
     g, keep = _geom(n_sectors, n_rows, max_pads, n_time, npads)
-    prm = _Params(q_peak_min, q_inner_gate, 0)
+    prm = _Params(q_peak_min, q_inner_gate, flags, q_tot_min, q_saturation, 0)
     st = _Status()
     b, e = planes if planes is not None else (0, n_sectors * n_rows)
     rc = lib.tpc_cf_oracle_run_planes(ctypes.c_void_p(digits.ctypes.data), ctypes.c_uint64(n),

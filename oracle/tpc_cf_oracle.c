@@ -83,6 +83,17 @@ static int64_t scan_plane(const uint16_t* Q, uint32_t P, uint32_t T,
             if (S0 >= (1 << 24) || llabs(S1p) >= (1 << 24) || llabs(S1t) >= (1 << 24) ||
                 S2p >= (1 << 24) || S2t >= (1 << 24)) return -3;
 
+            /* V1 / V2: flags from the peak cell and the sums, then the cuts */
+            unsigned fl = 0;
+            if (p < 2 || p + 2 >= (int)P) fl |= ORC_F_EDGE_PAD;
+            if (t < 2 || t + 2 >= (int)T) fl |= ORC_F_EDGE_TIME;
+            if (S2p == 0) fl |= ORC_F_SINGLE_PAD;
+            if (S2t == 0) fl |= ORC_F_SINGLE_TIME;
+            if (prm->q_saturation != 0 && q >= prm->q_saturation) fl |= ORC_F_SATURATED;
+            if (S0 < (int64_t)prm->q_tot_min) continue;
+            if ((prm->flags & ORC_CUT_SINGLE_PAD) && (fl & ORC_F_SINGLE_PAD)) continue;
+            if ((prm->flags & ORC_CUT_SINGLE_TIME) && (fl & ORC_F_SINGLE_TIME)) continue;
+
             if ((uint64_t)n_found < room) {
                 const double mp = (double)S1p / (double)S0;
                 const double mt = (double)S1t / (double)S0;
@@ -92,7 +103,8 @@ static int64_t scan_plane(const uint16_t* Q, uint32_t P, uint32_t T,
                 if (vt < 0) vt = 0;
                 orc_cluster c;
                 memset(&c, 0, sizeof c);
-                c.sector = (uint8_t)s; c.row = (uint8_t)r; c.pad = (uint8_t)p; c.flags = 0;
+                c.sector = (uint8_t)s; c.row = (uint8_t)r; c.pad = (uint8_t)p;
+                c.flags = (prm->flags & ORC_CLUSTER_FLAGS) ? (uint8_t)fl : 0;
                 c.time = (uint16_t)t; c.qmax = q; c.qtot = (uint32_t)S0;
                 c.pad_mean = (float)((double)p + mp);         /* R7 */
                 c.time_mean = (float)((double)t + mt);

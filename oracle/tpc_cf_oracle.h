@@ -34,7 +34,7 @@ typedef struct {
 } orc_digit;
 
 /* 32-byte output record: one cluster (north_star: "qTot, qMax, pad and time centroids and sigmas").
- * (sector,row,pad,time) is the peak cell; flags and rsv are 0. */
+ * (sector,row,pad,time) is the peak cell; flags: V1 below (0 unless requested); rsv is 0. */
 typedef struct {
     uint8_t  sector, row, pad, flags;
     uint16_t time, qmax;
@@ -48,14 +48,31 @@ typedef struct {
     const uint16_t* npads;      /* host, n_rows entries; NULL => every row has max_pads pads */
 } orc_geometry;
 
+/* Cluster-finder variants ("different cuts" in PAPER.md:21 — the paper names none,
+ * the definitions are this repository's, DESIGN.md §3 V1..V3).  Peaks are found exactly as before; then
+ *   V1 flags (written iff ORC_CLUSTER_FLAGS, else 0), from the peak cell and the sums of the accepted cells:
+ *        1 EDGE_PAD     pad < 2 or pad + 2 >= npads[row]      (the 5x5 window is clipped by the plane in pad)
+ *        2 EDGE_TIME    time < 2 or time + 2 >= n_time
+ *        4 SINGLE_PAD   no charge outside the peak's pad line entered qTot   (sum c*dp*dp == 0)
+ *        8 SINGLE_TIME  no charge outside the peak's time bin entered qTot   (sum c*dt*dt == 0)
+ *       16 SATURATED    q_saturation != 0 and qMax >= q_saturation
+ *   V2 cuts: a peak whose cluster has qTot < q_tot_min, or is SINGLE_PAD / SINGLE_TIME while the matching
+ *        ORC_CUT_* bit is set, yields no cluster and is not counted in n_clusters.
+ *   V3 a cut never changes which cells are peaks. */
+enum { ORC_CLUSTER_FLAGS = 4u, ORC_CUT_SINGLE_PAD = 8u, ORC_CUT_SINGLE_TIME = 16u };
+enum { ORC_F_EDGE_PAD = 1, ORC_F_EDGE_TIME = 2, ORC_F_SINGLE_PAD = 4, ORC_F_SINGLE_TIME = 8, ORC_F_SATURATED = 16 };
+
 typedef struct {
     uint16_t q_peak_min;        /* R6: peak threshold, default 4 */
     uint16_t q_inner_gate;      /* R4: gate threshold on the inner cell, default 2 */
-    uint32_t flags;             /* ignored by the oracle */
+    uint32_t flags;             /* ORC_* bits above; every other bit is ignored by the oracle */
+    uint32_t q_tot_min;         /* V2: minimum qTot, 0 = no cut */
+    uint16_t q_saturation;      /* V1: saturation threshold for the SATURATED flag, 0 = never */
+    uint16_t rsv;
 } orc_params;
 
 typedef struct {
-    uint64_t n_clusters;        /* true number of peaks, even if > capacity */
+    uint64_t n_clusters;        /* true number of clusters (peaks that pass the cuts), even if > capacity */
     uint64_t n_digits_used;
     uint64_t n_bad_digits;      /* R11: out-of-range or zero-charge digits, skipped */
     uint32_t overflow;          /* 1 if n_clusters > capacity */

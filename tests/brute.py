@@ -104,3 +104,40 @@ def find_clusters(cells, P, T, q_peak_min=4, q_inner_gate=2):
         if is_peak(cells, P, T, p, t, q_peak_min):
             out.append((p, t, cells[(p, t)]) + cluster_at(cells, P, T, p, t, q_inner_gate))
     return out
+
+
+# ---- variants (DESIGN.md §3 V1..V3), formulated differently from the oracle ---------------
+F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED = 1, 2, 4, 8, 16
+
+
+def cluster_flags(cells, P, T, p, t, q_inner_gate=2, q_saturation=0):
+    """V1 by enumeration: EDGE_* iff some cell of the 5x5 window falls outside the plane in that coordinate;
+    SINGLE_* iff the set of pads / time bins that contributed charge is just the peak's own."""
+    fl = 0
+    window = [(p + dp, t + dt) for dp in range(-2, 3) for dt in range(-2, 3)]
+    if any(pp < 0 or pp >= P for pp, _ in window):
+        fl |= F_EDGE_PAD
+    if any(tt < 0 or tt >= T for _, tt in window):
+        fl |= F_EDGE_TIME
+    cc = [(dp, dt) for dp, dt, c in counted_cells(cells, P, T, p, t, q_inner_gate) if c > 0]
+    if {dp for dp, _ in cc} <= {0}:
+        fl |= F_SINGLE_PAD
+    if {dt for _, dt in cc} <= {0}:
+        fl |= F_SINGLE_TIME
+    if q_saturation and cells[(p, t)] >= q_saturation:
+        fl |= F_SATURATED
+    return fl
+
+
+def find_clusters_variants(cells, P, T, q_peak_min=4, q_inner_gate=2, q_tot_min=0, q_saturation=0,
+                           cut_single_pad=False, cut_single_time=False):
+    """V2/V3: the base list, each entry with its flags appended, minus the entries that fail a cut."""
+    out = []
+    for c in find_clusters(cells, P, T, q_peak_min, q_inner_gate):
+        fl = cluster_flags(cells, P, T, c[0], c[1], q_inner_gate, q_saturation)
+        if c[3] < q_tot_min:
+            continue
+        if (cut_single_pad and fl & F_SINGLE_PAD) or (cut_single_time and fl & F_SINGLE_TIME):
+            continue
+        out.append(c + (fl,))
+    return out
