@@ -34,7 +34,7 @@ typedef struct {
 } tpc_digit;
 
 /* 32-byte output record (north_star: "clusters (qTot, qMax, pad and time centroids and sigmas)").
- * (sector,row,pad,time) is the peak cell; flags and rsv are written as 0. */
+ * (sector,row,pad,time) is the peak cell; flags: TPC_CF_F_* bits if TPC_CF_CLUSTER_FLAGS was set, else 0; rsv = 0. */
 typedef struct {
     uint8_t  sector, row, pad, flags;
     uint16_t time, qmax;
@@ -57,18 +57,36 @@ enum {
                                    free; if it is false nothing is output and status.path = 0, n_clusters = 0
                                    (rerun without the flag; tpc_cf_run_host does that by itself).  A wrong result
                                    is never returned silently. */
-    TPC_CF_FORCE_GENERAL = 2u   /* always run the general (map in HBM, "T1") path, whatever the order */
+    TPC_CF_FORCE_GENERAL = 2u,  /* always run the general (map in HBM, "T1") path, whatever the order */
+    /* Cluster-finder variants.  The paper only says that "different cuts" are used in the
+     * synchronous phase and names none; these definitions are this library's (DESIGN.md §3 V1..V3).
+     * Peaks are always found by the same rule (R1): a cut never changes which cells are peaks (V3). */
+    TPC_CF_CLUSTER_FLAGS = 4u,    /* V1: fill tpc_cluster.flags with the TPC_CF_F_* bits below (else the byte is 0) */
+    TPC_CF_CUT_SINGLE_PAD = 8u,   /* V2: a SINGLE_PAD cluster is not output and not counted */
+    TPC_CF_CUT_SINGLE_TIME = 16u  /* V2: same for SINGLE_TIME */
+};
+
+/* V1: bits of tpc_cluster.flags, from the peak cell and the cells that entered qTot. */
+enum {
+    TPC_CF_F_EDGE_PAD = 1u,     /* pad < 2 or pad + 2 >= npads[row]: the 5x5 window is clipped by the plane in pad */
+    TPC_CF_F_EDGE_TIME = 2u,    /* time < 2 or time + 2 >= n_time */
+    TPC_CF_F_SINGLE_PAD = 4u,   /* no charge outside the peak's pad line entered qTot (sigma_pad == 0) */
+    TPC_CF_F_SINGLE_TIME = 8u,  /* no charge outside the peak's time bin entered qTot (sigma_time == 0) */
+    TPC_CF_F_SATURATED = 16u    /* q_saturation != 0 and qMax >= q_saturation */
 };
 
 typedef struct {
     uint16_t q_peak_min;    /* R6, default 4; 0 is rejected */
     uint16_t q_inner_gate;  /* R4, default 2 */
     uint32_t flags;         /* TPC_CF_* bits */
+    uint32_t q_tot_min;     /* V2: clusters with qTot < q_tot_min are not output and not counted; 0 = no cut */
+    uint16_t q_saturation;  /* V1: threshold of the SATURATED flag; 0 = never */
+    uint16_t rsv;           /* 0 */
 } tpc_cf_params;
 
 /* Written last on the stream, by the device. */
 typedef struct {
-    uint64_t n_clusters;     /* true number of peaks, even if > capacity */
+    uint64_t n_clusters;     /* true number of clusters (peaks that pass the cuts), even if > capacity */
     uint64_t n_digits_used;  /* valid digits */
     uint64_t n_bad_digits;   /* R11: out-of-range or zero-charge digits: skipped and counted */
     uint32_t overflow;       /* 1 if n_clusters > capacity: the first `capacity` clusters in output order are written */

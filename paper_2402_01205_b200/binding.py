@@ -23,6 +23,9 @@ assert DIGIT.itemsize == 8 and CLUSTER.itemsize == 32 and STATUS.itemsize == 32
 
 DIGITS_SORTED = 1
 FORCE_GENERAL = 2
+# cluster-finder variants (include/tpc_cf.h V1..V3): params.flags bits and tpc_cluster.flags bits
+CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME = 4, 8, 16
+F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED = 1, 2, 4, 8, 16
 
 EXPORTS = ["tpc_cf_workspace_bytes", "tpc_cf_create", "tpc_cf_run", "tpc_cf_run_host",
            "tpc_cf_debug_dense_plane", "tpc_cf_last_launch_count", "tpc_cf_last_kernel", "tpc_cf_set_profiling",
@@ -37,7 +40,8 @@ class Geometry(ctypes.Structure):
 
 class Params(ctypes.Structure):
     _fields_ = [("q_peak_min", ctypes.c_uint16), ("q_inner_gate", ctypes.c_uint16),
-                ("flags", ctypes.c_uint32)]
+                ("flags", ctypes.c_uint32), ("q_tot_min", ctypes.c_uint32),
+                ("q_saturation", ctypes.c_uint16), ("rsv", ctypes.c_uint16)]
 
 
 class Out(ctypes.Structure):
@@ -137,7 +141,7 @@ class ClusterFinder:
     run(digits_dev, n) only enqueues on the current torch stream; result() synchronises and reads back."""
 
     def __init__(self, n_sectors, n_rows, max_pads, n_time, npads=None, max_digits=1 << 20, max_clusters=None,
-                 q_peak_min=4, q_inner_gate=2, device="cuda:0"):
+                 q_peak_min=4, q_inner_gate=2, q_tot_min=0, q_saturation=0, device="cuda:0"):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("tpc_cf needs a CUDA device; there is no CPU fallback")
@@ -147,7 +151,7 @@ class ClusterFinder:
         self.geom, self._keep = make_geometry(n_sectors, n_rows, max_pads, n_time, npads)
         self.max_digits = int(max_digits)
         self.max_clusters = int(max_clusters if max_clusters is not None else max(1, self.max_digits // 4))
-        self.params = Params(q_peak_min, q_inner_gate, 0)
+        self.params = Params(q_peak_min, q_inner_gate, 0, q_tot_min, q_saturation, 0)
         nbytes = tpc_cf_workspace_bytes(self.geom, self.max_digits, self.max_clusters)
         if nbytes == 0:
             raise TpcCfError(-2, "invalid geometry or capacities")

@@ -152,7 +152,8 @@ static int check_run_args(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     if (!geometry_to_geo(geom, &g) || !same_geometry(g, h->geo)) return TPC_CF_E_GEOMETRY;
     if (n > h->max_digits) return TPC_CF_E_CAPACITY;
     if (params->q_peak_min == 0) return TPC_CF_E_PARAMS;
-    if (params->flags & ~(uint32_t)(TPC_CF_DIGITS_SORTED | TPC_CF_FORCE_GENERAL)) return TPC_CF_E_PARAMS;
+    if (params->flags & ~(uint32_t)(TPC_CF_DIGITS_SORTED | TPC_CF_FORCE_GENERAL | TPC_CF_CLUSTER_FLAGS |
+                                    TPC_CF_CUT_SINGLE_PAD | TPC_CF_CUT_SINGLE_TIME)) return TPC_CF_E_PARAMS;
     if (((uintptr_t)digits & 7u) != 0) return TPC_CF_E_NULL;
     return TPC_CF_OK;
 }
@@ -171,6 +172,12 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     cudaEvent_t* ev = h->ev[h->run_index % kProfSlots];
     int k = 0;
 
+    Variant var;
+    var.q_tot_min = params->q_tot_min;
+    var.q_saturation = params->q_saturation;
+    var.vflags = params->flags & (TPC_CF_CLUSTER_FLAGS | TPC_CF_CUT_SINGLE_PAD | TPC_CF_CUT_SINGLE_TIME);
+    var.active = (var.q_tot_min != 0u || var.vflags != 0u) ? 1u : 0u;
+
     (void)cudaGetLastError();
     if (prof) cudaEventRecord(ev[0], st);
     cudaError_t e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), st);
@@ -178,7 +185,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
 
     if (fused) {
         // T3: line index -> fused smem kernel (scatter into smem lines, peak test, moments) -> compaction
-        int r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n, params->q_peak_min, params->q_inner_gate, st,
+        int r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n, params->q_peak_min, params->q_inner_gate, var, st,
                                     prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
         if (r < 0) return r;
         k += r;
@@ -187,7 +194,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     } else {
         // T1: K1 scatter -> K2+K4 digit-centric peaks + moments on the HBM map -> K3 compaction -> (K5 key sort)
         //     -> K0 un-scatter
-        k += launch_general_peaks(h->geo, h->ws, digits, n, params->q_peak_min, params->q_inner_gate, st,
+        k += launch_general_peaks(h->geo, h->ws, digits, n, params->q_peak_min, params->q_inner_gate, var, st,
                                   prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
         k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, hint ? 0 : 1, st);
         if (!hint) k += launch_key_sort(h->ws, h->max_clusters, h->n_sort_tiles, out->clusters, out->capacity, st);

@@ -166,7 +166,7 @@ template <bool MULTI>   // MULTI: the time axis is covered in sg.n_pass > 1 pass
 __global__ void __launch_bounds__(kBThreads, 2)
 k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
                uint32_t pads_per_unit, uint32_t units_per_plane, SlotGeo sg, uint32_t q_peak_min, uint32_t q_gate,
-               Counters* cnt, uint32_t* __restrict__ line_cnt, uint4* __restrict__ stage)
+               Variant var, Counters* cnt, uint32_t* __restrict__ line_cnt, uint4* __restrict__ stage)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_ls[260];          // line starts of this plane: s_ls[p], p = 0..max_pads, then next plane's start
@@ -356,16 +356,28 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
         const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
         uint32_t pcount = 0, pdone = MULTI ? s_cnt[p] : 0u; // warp-uniform: queued / already written peaks of the line
 
-        // stage C for one queued peak: y = (time | qmax << 16), k = its ordinal among the peaks of the line
-        auto moments = [&](uint32_t y, uint32_t k) {
-            const int t = (int)(y & 0xffffu);
-            int c[5][5];
+        // stage C for up to 32 queued peaks (one per lane): y = (time | qmax << 16).  Clusters that pass the cuts (V2;
+        // all of them by default) are written in lane order from ordinal `pdone` on; returns how many.
+        auto moments = [&](bool valid, uint32_t y) -> uint32_t {
+            bool keep = false;
+            ClusterSums sums = {0, 0, 0, 0, 0};
+            uint32_t fl = 0u;
+            const uint32_t t = y & 0xffffu;
+            if (valid) {
+                int c[5][5];
 #pragma unroll
-            for (int a = 0; a < 5; ++a) bwindow<2>(sl[a], MULTI ? dsub : 0u, sg, t, c[a], digits, s_ls, p + a - 2, P, T);
-            const ClusterWords r = cluster_from_window(c, w0_line, (uint32_t)t, q_gate);
-            const size_t j = (size_t)gl + k;                // packed at the start of the line's range, time order
-            stage[2 * j] = r.lo;
-            stage[2 * j + 1] = r.hi;
+                for (int a = 0; a < 5; ++a) bwindow<2>(sl[a], MULTI ? dsub : 0u, sg, (int)t, c[a], digits, s_ls, p + a - 2, P, T);
+                sums = cluster_sums(c, q_gate);
+                keep = var.active ? cluster_variant(sums, (uint32_t)p, t, y >> 16, (uint32_t)P, T, var, &fl) : true;
+            }
+            const unsigned km = __ballot_sync(0xffffffffu, keep);
+            if (keep) {
+                const ClusterWords r = cluster_finish(sums, w0_line, t, y >> 16, fl);
+                const size_t j = (size_t)gl + pdone + (uint32_t)__popc(km & lt_mask);   // line's range, time order
+                stage[2 * j] = r.lo;
+                stage[2 * j + 1] = r.hi;
+            }
+            return (uint32_t)__popc(km);
         };
         // stage B for up to 32 survivors (one per lane); peaks go to the warp's queue, stage C runs on full warps
         auto stage_b = [&](bool act, uint32_t y) {
@@ -385,8 +397,7 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
             pcount += (uint32_t)__popc(pm);
             __syncwarp();
             if (pcount >= 32u) {
-                moments(lds32(pqa + ((uint32_t)lane << 2)), pdone + (uint32_t)lane);
-                pdone += 32u;
+                pdone += moments(true, lds32(pqa + ((uint32_t)lane << 2)));
                 const uint32_t mv = lds32(pqa + (((uint32_t)lane + 32u) << 2));
                 __syncwarp();
                 sts32(pqa + ((uint32_t)lane << 2), mv);
@@ -423,7 +434,7 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
             }
         }
         if (pcount > 16u) {
-            if ((uint32_t)lane < pcount) moments(lds32(pqa + ((uint32_t)lane << 2)), pdone + (uint32_t)lane);
+            pdone += moments((uint32_t)lane < pcount, lds32(pqa + (((uint32_t)lane & 31u) << 2)));
         } else if (pcount > 0u) {
             // the usual case (a line has ~14 peaks): two lanes per peak, each gathers the rows on one side of the
             // peak plus the peak's row (3 windows instead of 5); the halves of the integer sums are added by shuffle
@@ -446,16 +457,22 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
             h.S1t += __shfl_xor_sync(0xffffffffu, h.S1t, 16);
             h.S2p += __shfl_xor_sync(0xffffffffu, h.S2p, 16);
             h.S2t += __shfl_xor_sync(0xffffffffu, h.S2t, 16);
-            if (valid && !neg) {
-                const ClusterWords r = cluster_finish(h, w0_line, y & 0xffffu, y >> 16);
-                const size_t j = (size_t)gl + pdone + i;
+            bool keep = valid && !neg;
+            uint32_t fl = 0u;
+            if (keep && var.active)
+                keep = cluster_variant(h, (uint32_t)p, y & 0xffffu, y >> 16, (uint32_t)P, T, var, &fl);
+            const unsigned km = __ballot_sync(0xffffffffu, keep);
+            if (keep) {
+                const ClusterWords r = cluster_finish(h, w0_line, y & 0xffffu, y >> 16, fl);
+                const size_t j = (size_t)gl + pdone + (uint32_t)__popc(km & lt_mask);
                 stage[2 * j] = r.lo;
                 stage[2 * j + 1] = r.hi;
             }
+            pdone += (uint32_t)__popc(km);
         }
         if (lane == 0) {
-            if (MULTI) s_cnt[p] = pdone + pcount;           // peaks of this line so far, in time order
-            if (!MULTI || last_pass) line_cnt[plane * g.LS + p] = pdone + pcount;
+            if (MULTI) s_cnt[p] = pdone;                    // clusters of this line so far, in time order
+            if (!MULTI || last_pass) line_cnt[plane * g.LS + p] = pdone;
         }
     };
 
@@ -526,7 +543,8 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 // 20 line slots of ~5 KB leave no room for a third CTA).  Lines too long for the 254-block pool are covered in several
 // passes over the time axis (dir, pool and survivor list all scale with the segment length).
 int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1)
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
+                        cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
     uint64_t total_pads = 0;
     for (uint32_t r = 0; r < g.n_rows; ++r) total_pads += g.npads[r];
@@ -607,7 +625,7 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
     g_last_kernel = "k_fused_blocks";
     auto kern = sg.n_pass > 1 ? k_fused_blocks<true> : k_fused_blocks<false>;
     kern<<<g.n_planes * upp, kBThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
-                                                    pads_per_unit, upp, sg, q_peak_min, q_gate,
+                                                    pads_per_unit, upp, sg, q_peak_min, q_gate, var,
                                                     ws.counters, ws.line_cnt, (uint4*)ws.stage);
     if (ev_k1) cudaEventRecord(ev_k1, st);
     return 1;

@@ -130,7 +130,7 @@ __device__ __forceinline__ void window(const Ring& rg, const uint32_t* __restric
 __global__ void __launch_bounds__(kFThreads, 2)
 k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
               uint32_t pads_per_unit, uint32_t units_per_plane, uint32_t wpl, uint32_t cap,
-              uint32_t q_peak_min, uint32_t q_gate, Counters* cnt, uint32_t* __restrict__ line_cnt,
+              uint32_t q_peak_min, uint32_t q_gate, Variant var, Counters* cnt, uint32_t* __restrict__ line_cnt,
               uint4* __restrict__ stage)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -291,16 +291,31 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     // ---- K4 (stage C): 5x5 window from the slots of lines p-2..p+2, gated sums, record -> stage[j] ----------------
     // vp = ring index of line p.  Slots of lines outside the plane are empty (R2).
     // sl[a] / gls[a]: slot and first-digit index of line p+a-2 (warp-uniform: a warp's peaks are all on its line)
-    auto moments = [&](int p, uint32_t jl, uint32_t k, const uint32_t* const (&sl)[5], const uint32_t (&gls)[5]) {
-        const uint32_t self = fetch(sl[2], gls[2], jl);
-        const int t = (int)(self & 0xffffu);
-        int c[5][5];
+    // valid lanes hold one queued peak each (jl = its index in the line); clusters that pass the cuts (V2; all of them
+    // by default) are written in lane order from ordinal k0 on; returns how many.
+    auto moments = [&](bool valid, int p, uint32_t jl, uint32_t k0, const uint32_t* const (&sl)[5],
+                       const uint32_t (&gls)[5]) -> uint32_t {
+        bool keep = false;
+        ClusterSums sums = {0, 0, 0, 0, 0};
+        uint32_t fl = 0u, t = 0u, qmax = 0u;
+        if (valid) {
+            const uint32_t self = fetch(sl[2], gls[2], jl);
+            t = self & 0xffffu;
+            qmax = self >> 16;
+            int c[5][5];
 #pragma unroll
-        for (int a = 0; a < 5; ++a) window<2>(rg, sl[a], digits, gls[a], n, t, c[a]);
-        const ClusterWords r = cluster_from_window(c, w0_base | ((uint32_t)p << 16), (uint32_t)t, q_gate);
-        const size_t j = (size_t)gls[2] + k;     // k-th peak of the line: packed at the start of the line's range
-        stage[2 * j] = r.lo;
-        stage[2 * j + 1] = r.hi;
+            for (int a = 0; a < 5; ++a) window<2>(rg, sl[a], digits, gls[a], n, (int)t, c[a]);
+            sums = cluster_sums(c, q_gate);
+            keep = var.active ? cluster_variant(sums, (uint32_t)p, t, qmax, (uint32_t)P, (uint32_t)T, var, &fl) : true;
+        }
+        const unsigned km = __ballot_sync(0xffffffffu, keep);
+        if (keep) {
+            const ClusterWords r = cluster_finish(sums, w0_base | ((uint32_t)p << 16), t, qmax, fl);
+            const size_t j = (size_t)gls[2] + k0 + (uint32_t)__popc(km & ((1u << lane) - 1u));
+            stage[2 * j] = r.lo;
+            stage[2 * j + 1] = r.hi;
+        }
+        return (uint32_t)__popc(km);
     };
 
     // ---- K2: stages A and B for line p (ring index vp), owned by this warp; lo = p - l0 ------------------------------
@@ -342,8 +357,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             pcount += (uint32_t)__popc(pm);
             __syncwarp();
             if (pcount >= 32u) {
-                moments(p, pq[lane], pdone + lane, sl, gls);
-                pdone += 32u;
+                pdone += moments(true, p, pq[lane], pdone, sl, gls);
                 const uint32_t mv = (lane + 32u < pcount) ? pq[lane + 32u] : 0u;
                 __syncwarp();
                 if (lane + 32u < pcount) pq[lane] = mv;
@@ -414,8 +428,8 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             enqueue(act && q >= q_peak_min && t < T && q > qm && q >= qp, jl);   // R1: (0,-1) strict, (0,+1) >=
         }
         if (wcount) stage_b((uint32_t)lane < wcount, (uint32_t)lane < wcount ? wq[lane] : 0u);
-        if ((uint32_t)lane < pcount) moments(p, pq[lane], pdone + lane, sl, gls);
-        if (lane == 0) line_cnt[plane * g.LS + p] = pdone + pcount;   // peaks of this line, in time order
+        if (pcount) pdone += moments((uint32_t)lane < pcount, p, pq[lane], pdone, sl, gls);
+        if (lane == 0) line_cnt[plane * g.LS + p] = pdone;   // clusters of this line, in time order
     };
 
     // ---- main loop -------------------------------------------------------------------------------------------------
@@ -441,7 +455,7 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
 }
 
 int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
     cudaMemsetAsync(ws.line_cnt, 0, ((size_t)g.n_planes * g.LS + 1) * 4, st);   // pads beyond npads[row] stay 0
@@ -454,7 +468,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
 
     // block-sparse line slots (tpc_cf_blocks.cu) when the mean line fits their pool; else the bitmap slots below
     {
-        const int r = launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, st, ev_k0, ev_k1);
+        const int r = launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, st, ev_k0, ev_k1);
         if (r < 0) return r;
         if (r > 0) return k + r;
     }
@@ -495,7 +509,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     if (ev_k0) cudaEventRecord(ev_k0, st);
     g_last_kernel = "k_fused_lines";
     k_fused_lines<<<g.n_planes * upp, kFThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
-                                                             pads_per_unit, upp, wpl, cap, q_peak_min, q_gate,
+                                                             pads_per_unit, upp, wpl, cap, q_peak_min, q_gate, var,
                                                              ws.counters, ws.line_cnt, (uint4*)ws.stage);
     if (ev_k1) cudaEventRecord(ev_k1, st);
     return k + 1;

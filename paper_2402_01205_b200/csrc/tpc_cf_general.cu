@@ -59,7 +59,8 @@ k_unscatter(const uint2* __restrict__ digits, uint64_t n, Geo g, uint16_t* __res
 
 __global__ void __launch_bounds__(kThreads)
 k_peaks_map(const uint2* __restrict__ digits, uint64_t n, Geo g, const uint16_t* __restrict__ map,
-            uint32_t q_peak_min, uint32_t q_gate, uint32_t* __restrict__ peakmask, uint4* __restrict__ stage)
+            uint32_t q_peak_min, uint32_t q_gate, Variant var, uint32_t* __restrict__ peakmask,
+            uint4* __restrict__ stage)
 {
     const uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
     bool peak = false;
@@ -77,18 +78,26 @@ k_peaks_map(const uint2* __restrict__ digits, uint64_t n, Geo g, const uint16_t*
                    q >= (uint32_t)c0[TS - 1] && q >= (uint32_t)c0[TS] && q >= (uint32_t)c0[TS + 1];
         }
     }
-    const unsigned m = __ballot_sync(0xffffffffu, peak);
-    if ((threadIdx.x & 31) == 0 && i < n) peakmask[i >> 5] = m;
+    // K4 before the peak bit is recorded: a cluster that fails a cut (V2) is not a set bit
     if (peak) {
         int c[5][5];
 #pragma unroll
         for (int a = 0; a < 5; ++a)
 #pragma unroll
             for (int b = 0; b < 5; ++b) c[a][b] = (int)c0[(a - 2) * TS + (b - 2)];
-        const ClusterWords r = cluster_from_window(c, d.x, d.y & 0xffffu, q_gate);
-        stage[2 * i] = r.lo;
-        stage[2 * i + 1] = r.hi;
+        const ClusterSums sums = cluster_sums(c, q_gate);
+        uint32_t fl = 0u;
+        if (var.active)
+            peak = cluster_variant(sums, (d.x >> 16) & 0xffu, d.y & 0xffffu, d.y >> 16, g.npads[(d.x >> 8) & 0xffu],
+                                   g.n_time, var, &fl);
+        if (peak) {
+            const ClusterWords r = cluster_finish(sums, d.x, d.y & 0xffffu, d.y >> 16, fl);
+            stage[2 * i] = r.lo;
+            stage[2 * i + 1] = r.hi;
+        }
     }
+    const unsigned m = __ballot_sync(0xffffffffu, peak);
+    if ((threadIdx.x & 31) == 0 && i < n) peakmask[i >> 5] = m;
 }
 
 __global__ void k_copy_plane(Geo g, const uint16_t* __restrict__ map, uint32_t plane, uint32_t P,
@@ -118,14 +127,14 @@ int launch_unscatter(const Geo& g, const Workspace& ws, const tpc_digit* digits,
 }
 
 int launch_general_peaks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
-                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
+                         uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
                          cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
     if (n == 0) return 0;
     k_scatter<<<grid_for(n), kThreads, 0, st>>>((const uint2*)digits, n, g, ws.map, ws.counters);
     if (ev_k0) cudaEventRecord(ev_k0, st);
     g_last_kernel = "k_peaks_map";
-    k_peaks_map<<<grid_for(n), kThreads, 0, st>>>((const uint2*)digits, n, g, ws.map, q_peak_min, q_gate,
+    k_peaks_map<<<grid_for(n), kThreads, 0, st>>>((const uint2*)digits, n, g, ws.map, q_peak_min, q_gate, var,
                                                   ws.peakmask, (uint4*)ws.stage);
     if (ev_k1) cudaEventRecord(ev_k1, st);
     return 2;

@@ -78,8 +78,35 @@ __device__ __forceinline__ uint64_t key40(uint32_t w0, uint32_t w1)
 struct ClusterWords { uint4 lo, hi; };
 struct ClusterSums { int S0, S1p, S1t, S2p, S2t; };   // integer sums relative to the peak cell (R8)
 
-// R7: record from the sums.  qmax = charge of the peak cell.
-__device__ __forceinline__ ClusterWords cluster_finish(const ClusterSums& m, uint32_t w0, uint32_t time, uint32_t qmax)
+// Cluster-finder variants (include/tpc_cf.h V1..V3): knobs of one run, warp-uniform kernel parameter.
+struct Variant {
+    uint32_t q_tot_min;      // V2: minimum qTot (0 = no cut)
+    uint32_t q_saturation;   // V1: SATURATED threshold (0 = never)
+    uint32_t vflags;         // TPC_CF_CLUSTER_FLAGS | TPC_CF_CUT_SINGLE_PAD | TPC_CF_CUT_SINGLE_TIME
+    uint32_t active;         // any of the above set: the default run skips all of it
+};
+
+// V1 flags of a cluster from its peak cell and sums; returns false if a cut (V2) drops it.
+// P = pads of the peak's row, T = n_time.
+__device__ __forceinline__ bool cluster_variant(const ClusterSums& m, uint32_t pad, uint32_t time, uint32_t qmax,
+                                                uint32_t P, uint32_t T, const Variant& v, uint32_t* flags)
+{
+    uint32_t fl = 0u;
+    if (pad < 2u || pad + 2u >= P) fl |= TPC_CF_F_EDGE_PAD;
+    if (time < 2u || time + 2u >= T) fl |= TPC_CF_F_EDGE_TIME;
+    if (m.S2p == 0) fl |= TPC_CF_F_SINGLE_PAD;
+    if (m.S2t == 0) fl |= TPC_CF_F_SINGLE_TIME;
+    if (v.q_saturation != 0u && qmax >= v.q_saturation) fl |= TPC_CF_F_SATURATED;
+    *flags = (v.vflags & TPC_CF_CLUSTER_FLAGS) ? fl : 0u;
+    if ((uint32_t)m.S0 < v.q_tot_min) return false;
+    if ((v.vflags & TPC_CF_CUT_SINGLE_PAD) && (fl & TPC_CF_F_SINGLE_PAD)) return false;
+    if ((v.vflags & TPC_CF_CUT_SINGLE_TIME) && (fl & TPC_CF_F_SINGLE_TIME)) return false;
+    return true;
+}
+
+// R7: record from the sums.  qmax = charge of the peak cell, flags = V1 byte (0 by default).
+__device__ __forceinline__ ClusterWords cluster_finish(const ClusterSums& m, uint32_t w0, uint32_t time, uint32_t qmax,
+                                                       uint32_t flags = 0u)
 {
     const uint32_t pad = (w0 >> 16) & 0xffu;
     const float f0 = (float)m.S0;
@@ -91,7 +118,7 @@ __device__ __forceinline__ ClusterWords cluster_finish(const ClusterSums& m, uin
     const float sp = sqrtf(fmaxf((float)np, 0.f) / den);
     const float st = sqrtf(fmaxf((float)nt, 0.f) / den);
     ClusterWords r;
-    r.lo.x = w0 & 0x00ffffffu;                                // sector,row,pad,flags=0
+    r.lo.x = (w0 & 0x00ffffffu) | (flags << 24);              // sector,row,pad,flags
     r.lo.y = time | (qmax << 16);                             // time,qmax
     r.lo.z = (uint32_t)m.S0;                                  // qtot
     r.lo.w = __float_as_uint(pad_mean);
@@ -102,8 +129,7 @@ __device__ __forceinline__ ClusterWords cluster_finish(const ClusterSums& m, uin
     return r;
 }
 
-__device__ __forceinline__ ClusterWords cluster_from_window(const int (&c)[5][5], uint32_t w0, uint32_t time,
-                                                            uint32_t gate)
+__device__ __forceinline__ ClusterSums cluster_sums(const int (&c)[5][5], uint32_t gate)
 {
     ClusterSums m = {0, 0, 0, 0, 0};
 #pragma unroll
@@ -120,7 +146,13 @@ __device__ __forceinline__ ClusterWords cluster_from_window(const int (&c)[5][5]
             m.S0 += v; m.S1p += v * dp; m.S1t += v * dt; m.S2p += v * dp * dp; m.S2t += v * dt * dt;
         }
     }
-    return cluster_finish(m, w0, time, (uint32_t)c[2][2]);
+    return m;
+}
+
+__device__ __forceinline__ ClusterWords cluster_from_window(const int (&c)[5][5], uint32_t w0, uint32_t time,
+                                                            uint32_t gate)
+{
+    return cluster_finish(cluster_sums(c, gate), w0, time, (uint32_t)c[2][2]);
 }
 
 // One half of the same sums, for two lanes sharing a peak: the rows on one side of the peak (o: |dp| = 2, m: |dp| = 1,
@@ -154,7 +186,7 @@ extern thread_local const char* g_last_kernel;
 // ---- launchers (each returns the number of kernels it enqueued, or a negative tpc_cf error) -----------------
 
 int launch_general_peaks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n,
-                         uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
+                         uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
                          cudaEvent_t ev_k0, cudaEvent_t ev_k1);
 int launch_unscatter(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, cudaStream_t st);
 int launch_scatter_only(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, cudaStream_t st);
@@ -162,11 +194,11 @@ int launch_copy_plane(const Geo& g, const Workspace& ws, uint32_t plane, uint32_
                       cudaStream_t st);
 
 int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1);
 
 int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, cudaStream_t st,
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1);
 
 // compaction of stage[j] by peakmask into dst (= out, or ws.compact when a key sort must follow)

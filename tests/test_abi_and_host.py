@@ -46,7 +46,7 @@ def test_struct_layouts_match_header():
     import paper_2402_01205_b200 as cf
     assert cf.DIGIT.itemsize == 8 and cf.CLUSTER.itemsize == 32 and cf.STATUS.itemsize == 32
     assert cf.CLUSTER.fields["qtot"][1] == 8 and cf.CLUSTER.fields["pad_mean"][1] == 12
-    assert ctypes.sizeof(cf.Geometry) == 24 and ctypes.sizeof(cf.Params) == 8 and ctypes.sizeof(cf.Out) == 32
+    assert ctypes.sizeof(cf.Geometry) == 24 and ctypes.sizeof(cf.Params) == 16 and ctypes.sizeof(cf.Out) == 32
 
 
 def test_workspace_bytes_and_geometry_limits():

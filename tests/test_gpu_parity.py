@@ -58,7 +58,8 @@ def _fused_kernel_env(request, monkeypatch):
     yield
 
 
-def gpu_run(digits, geom, flags, max_clusters=None, capacity=None, q_peak_min=4, q_inner_gate=2, finder=None):
+def gpu_run(digits, geom, flags, max_clusters=None, capacity=None, q_peak_min=4, q_inner_gate=2, finder=None,
+            q_tot_min=0, q_saturation=0):
     cf = _cf()
     n_sectors, n_rows, max_pads, n_time, npads = geom
     n = int(digits.shape[0])
@@ -66,7 +67,8 @@ def gpu_run(digits, geom, flags, max_clusters=None, capacity=None, q_peak_min=4,
     if own:
         finder = cf.ClusterFinder(n_sectors, n_rows, max_pads, n_time, npads=npads, max_digits=max(n, 1),
                                   max_clusters=max_clusters if max_clusters is not None else max(n, 1),
-                                  q_peak_min=q_peak_min, q_inner_gate=q_inner_gate)
+                                  q_peak_min=q_peak_min, q_inner_gate=q_inner_gate, q_tot_min=q_tot_min,
+                                  q_saturation=q_saturation)
     d = cf.to_device(digits)
     finder.run(d, n, flags=flags, capacity=capacity)
     cl, st = finder.result()
@@ -391,3 +393,47 @@ def test_run_host_pipelined_over_sector_groups():
     assert st3["n_clusters"] == rst["n_clusters"] and st3["overflow"] == 0
     assert np.array_equal(cl3.view(np.uint8), ref.view(np.uint8))
     f.close()
+
+
+# ---- variants (flags V1, cuts V2/V3) ------------------------------------------------------
+VARIANTS = [dict(vflags=4, q_tot_min=0, q_saturation=150), dict(vflags=0, q_tot_min=60, q_saturation=0),
+            dict(vflags=4 | 8, q_tot_min=0, q_saturation=0), dict(vflags=4 | 8 | 16, q_tot_min=25, q_saturation=90)]
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_variant_worked_examples(path):
+    """tests/golden/variant_examples.txt through every CUDA path, against the oracle with the same knobs."""
+    import test_oracle_variants as tv
+    for ex in tv.EXAMPLES:
+        kw = tv.variant_kwargs(ex["v"])
+        digits = sort_digits(orc.make_digits(ex["digits"]))
+        geom = (1, 1, 12, 12, None)
+        ora, ost = orc.run(digits, *geom[:4], **kw)
+        cl, st = gpu_run(digits, geom, PATHS[path] | kw["flags"], q_tot_min=kw["q_tot_min"],
+                         q_saturation=kw["q_saturation"])
+        assert st["n_clusters"] == ost["n_clusters"] == len(ex["clusters"]), ex["name"]
+        assert_clusters_equal(cl, ora, "variant %s/%s" % (ex["name"], path))
+        assert [int(f) for f in cl["flags"]] == [c[8] for c in ex["clusters"]], ex["name"]
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("v", VARIANTS, ids=["flags", "qtot60", "flags+cut_pad", "all"])
+def test_variants_full_parity(v, path):
+    """Flags and cuts on config 1, on a 10 % frame slice (config 4, 3 rows) and on a variable-pads slice of config 5:
+    bit-exact flags, counts and order against the oracle; the cut changes counts and ordinals in every kernel."""
+    cases = [(gen.generate(1), gen.geometry(1))]
+    c = dict(gen.CONFIGS[4]); c["n_sectors"] = 1; c["n_rows"] = 3
+    cases.append((gen.generate(c), gen.geometry(c)))
+    c = dict(gen.CONFIGS[5]); c["n_sectors"] = 1; c["n_rows"] = 6
+    c["npads"] = gen.npads_linear(152, 66, 138)[::30][:6]
+    cases.append((gen.generate(c), gen.geometry(c)))
+    for digits, geom in cases:
+        ora, ost = orc.run(digits, *geom[:4], npads=geom[4], flags=v["vflags"], q_tot_min=v["q_tot_min"],
+                           q_saturation=v["q_saturation"])
+        cl, st = gpu_run(digits, geom, PATHS[path] | v["vflags"], q_tot_min=v["q_tot_min"],
+                         q_saturation=v["q_saturation"], max_clusters=ost["n_clusters"] + 16)
+        assert st["n_clusters"] == ost["n_clusters"]
+        assert_clusters_equal(cl, ora, "variants %r/%s" % (v, path))
+        assert np.array_equal(cl["flags"], ora["flags"])
+        if v["vflags"] & 4:
+            assert np.count_nonzero(cl["flags"]) > 0
