@@ -162,7 +162,9 @@ __device__ __forceinline__ void bwindow(uint32_t slot, uint32_t dsub, const Slot
     }
 }
 
-template <bool MULTI>   // MULTI: the time axis is covered in sg.n_pass > 1 passes (long lines)
+// MULTI: the time axis is covered in sg.n_pass > 1 passes (long lines).  VAR: flags / cuts requested (V1..V3); the
+// default instantiation carries none of that code.
+template <bool MULTI, bool VAR>
 __global__ void __launch_bounds__(kBThreads, 2)
 k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
                uint32_t pads_per_unit, uint32_t units_per_plane, SlotGeo sg, uint32_t q_peak_min, uint32_t q_gate,
@@ -368,7 +370,7 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 #pragma unroll
                 for (int a = 0; a < 5; ++a) bwindow<2>(sl[a], MULTI ? dsub : 0u, sg, (int)t, c[a], digits, s_ls, p + a - 2, P, T);
                 sums = cluster_sums(c, q_gate);
-                keep = var.active ? cluster_variant(sums, (uint32_t)p, t, y >> 16, (uint32_t)P, T, var, &fl) : true;
+                keep = VAR ? cluster_variant(sums, (uint32_t)p, t, y >> 16, (uint32_t)P, T, var, &fl) : true;
             }
             const unsigned km = __ballot_sync(0xffffffffu, keep);
             if (keep) {
@@ -459,7 +461,7 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
             h.S2t += __shfl_xor_sync(0xffffffffu, h.S2t, 16);
             bool keep = valid && !neg;
             uint32_t fl = 0u;
-            if (keep && var.active)
+            if (VAR && keep)
                 keep = cluster_variant(h, (uint32_t)p, y & 0xffffu, y >> 16, (uint32_t)P, T, var, &fl);
             const unsigned km = __ballot_sync(0xffffffffu, keep);
             if (keep) {
@@ -616,14 +618,17 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_fused_blocks<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_blocks<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_fused_blocks<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_blocks<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_blocks<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_blocks<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
         if (e != cudaSuccess) return TPC_CF_E_CUDA;
         attr_set = true;
     }
     if (ev_k0) cudaEventRecord(ev_k0, st);
     g_last_kernel = "k_fused_blocks";
-    auto kern = sg.n_pass > 1 ? k_fused_blocks<true> : k_fused_blocks<false>;
+    auto kern = sg.n_pass > 1 ? (var.active ? k_fused_blocks<true, true> : k_fused_blocks<true, false>)
+                              : (var.active ? k_fused_blocks<false, true> : k_fused_blocks<false, false>);
     kern<<<g.n_planes * upp, kBThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
                                                     pads_per_unit, upp, sg, q_peak_min, q_gate, var,
                                                     ws.counters, ws.line_cnt, (uint4*)ws.stage);
