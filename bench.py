@@ -182,6 +182,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--variant", default="none", choices=["none", "flags", "cuts"],
+                    help="cluster-finder variants (SURVEY.md §8(f) NEXT #1): 'flags' = per-cluster flags, 'cuts' = "
+                         "flags + q_tot_min 40 + single-pad cut; the default run has none")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
@@ -213,8 +216,11 @@ def main():
     n_digits = [int(f.shape[0]) for f in frames]
     nmax = max(n_digits)
     max_clusters = nmax // 10 + 1024
-    finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=nmax, max_clusters=max_clusters, device=dev)
-    flags = cf.DIGITS_SORTED if args.path == "fused" else (cf.DIGITS_SORTED | cf.FORCE_GENERAL)
+    vflags = {"none": 0, "flags": cf.CLUSTER_FLAGS, "cuts": cf.CLUSTER_FLAGS | cf.CUT_SINGLE_PAD}[args.variant]
+    finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=nmax, max_clusters=max_clusters, device=dev,
+                              q_tot_min=40 if args.variant == "cuts" else 0,
+                              q_saturation=1000 if args.variant != "none" else 0)
+    flags = (cf.DIGITS_SORTED if args.path == "fused" else (cf.DIGITS_SORTED | cf.FORCE_GENERAL)) | vflags
 
     pinned = [torch.from_numpy(f.view(np.uint8)).pin_memory() for f in frames]
     dev_digits = [p.to(dev, non_blocking=True) for p in pinned]
@@ -336,6 +342,7 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u16/i32/f32", "data": "synthetic",
             "config": {"workload": "config%d: %s" % (args.config, cfg["label"]), "path": args.path,
+                       "variant": args.variant,
                        "frames_per_step": n_frames, "digits_per_frame": nd, "clusters_per_frame": nc,
                        "occupancy": gen.occupancy(frames[0], args.config), "parallelism": "replicas x%d" % world,
                        "l2": "inputs (%.2f GB digits per frame) larger than the 126 MB L2; no flush" % (nd * 8 / 1e9),

@@ -303,6 +303,21 @@ def test_full_frame_sampled_planes():
     cl2, st2 = f.result()
     assert st2["path"] == 1 and st2["n_clusters"] == st["n_clusters"]
     assert np.array_equal(cl2.view(np.uint8), cl.view(np.uint8)), "general and fused path differ on config 3"
+    # variants at full size (flags + q_tot_min cut + single-pad cut): count by filtering the uncut output, sampled
+    # planes one by one against the oracle with the same knobs
+    f.params.q_tot_min, f.params.q_saturation = 40, 200
+    vflags = cf.CLUSTER_FLAGS | cf.CUT_SINGLE_PAD
+    f.run(d, n, flags=cf.DIGITS_SORTED | vflags)
+    cv, sv = f.result()
+    keep = (cl["qtot"] >= 40) & (cl["sigma_pad"] != 0)
+    assert sv["n_clusters"] == int(keep.sum()) and np.array_equal(key(cv), key(cl[keep]))
+    vplane = cv["sector"].astype(np.int64) * geom[1] + cv["row"]
+    for pl in (0, 1234, geom[0] * geom[1] - 1):
+        lo, hi = np.searchsorted(dplane, [pl, pl + 1])
+        ora, ost = orc.run(digits[lo:hi], *geom[:4], planes=(int(pl), int(pl) + 1), flags=vflags, q_tot_min=40,
+                           q_saturation=200)
+        a, b = np.searchsorted(vplane, [pl, pl + 1])
+        assert_clusters_equal(cv[a:b], ora, "config 3 variants plane %d" % pl)
     f.close()
 
 
