@@ -545,7 +545,7 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 // 20 line slots of ~5 KB leave no room for a third CTA).  Lines too long for the 254-block pool are covered in several
 // passes over the time axis (dir, pool and survivor list all scale with the segment length).
 int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, bool must, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
     uint64_t total_pads = 0;
@@ -557,8 +557,8 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const double mean_blocks = 0.38 * mean_len, mean_surv = 0.16 * mean_len;
 
     const char* force = getenv("TPC_CF_FUSED_KERNEL");            // "blocks" | "lines" (tests, profiling)
-    const bool forced = force && force[0] == 'b';
-    if (force && force[0] == 'l') return 0;
+    const bool forced = must || (force && force[0] == 'b');   // must: the bitmap kernel cannot take this geometry
+    if (!must && force && force[0] == 'l') return 0;
     int env_pass = 0;                                              // tuning / test knob
     if (const char* e = getenv("TPC_CF_PASSES")) env_pass = atoi(e);
 
@@ -593,8 +593,9 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
     }
     if (!have) {
         if (!forced) return 0;
-        const uint32_t np = env_pass >= 1 && env_pass <= 8 && g.n_time >= 64u * (uint32_t)env_pass ? (uint32_t)env_pass : 1u;
-        if (!shape(np, true, &sg)) return 0;
+        if (env_pass >= 1 && env_pass <= 8 && g.n_time >= 64u * (uint32_t)env_pass) have = shape((uint32_t)env_pass, true, &sg);
+        for (uint32_t np = 1; np <= 8 && !have; ++np) have = (np == 1 || g.n_time >= 64u * np) && shape(np, true, &sg);
+        if (!have) return 0;
     }
     if (const char* e = getenv("TPC_CF_BLOCK_POOL")) {             // test knob: force a small pool (slow paths)
         const int v = atoi(e);

@@ -468,7 +468,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
 
     // block-sparse line slots (tpc_cf_blocks.cu) when the mean line fits their pool; else the bitmap slots below
     {
-        const int r = launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, st, ev_k0, ev_k1);
+        const int r = launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, false, st, ev_k0, ev_k1);
         if (r < 0) return r;
         if (r > 0) return k + r;
     }
@@ -484,7 +484,12 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t max_smem = 106 * 1024;                    // 2 CTAs per SM (+ ~5 KB static + 1 KB reserved each)
     const uint32_t fixed = kSlots * (wpl + pre_words) * 4 + kWarps * 64;
     const uint32_t per_cap0 = kSlots * 4 + kSlots / 8 + 1 + kWarps * 4 + kWarps * 2;   // tq, stage-A bit, key staging, survivor list
-    if (fixed + per_cap0 * 128 > 200 * 1024) return TPC_CF_E_GEOMETRY;   // cannot happen for n_time <= 65535
+    if (fixed + per_cap0 * 128 > 200 * 1024) {
+        // the bitmap slots of 20 lines do not fit (n_time above ~50 k): the block kernel covers the time axis in passes
+        const int r = launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, true, st, ev_k0, ev_k1);
+        if (r < 0) return r;
+        return r > 0 ? k + r : TPC_CF_E_GEOMETRY;
+    }
     const uint32_t limit = fixed + per_cap0 * 128 <= max_smem ? max_smem : 200 * 1024;
     const uint32_t per_cap = per_cap0;
     if (cap > 1024u) cap = 1024u;                            // the stage-A words of a line must fit one warp (32 words)

@@ -198,7 +198,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1);
 
 int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, bool must, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1);
 
 // compaction of stage[j] by peakmask into dst (= out, or ws.compact when a key sort must follow)

@@ -452,3 +452,33 @@ def test_variants_full_parity(v, path):
         assert np.array_equal(cl["flags"], ora["flags"])
         if v["vflags"] & 4:
             assert np.count_nonzero(cl["flags"]) > 0
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_maximum_geometry(path, monkeypatch):
+    """The largest plane the 8/16-bit record fields allow (255 pads x 65535 time bins), sparse clusters plus digits in
+    the last pads and time bins, and odd sizes that are no multiple of the kernels' tile sizes (7 pads x 61 bins)."""
+    rng = np.random.default_rng(21)
+    for (P, T, ncl) in ((255, 65535, 4000), (7, 61, 12), (9, 257, 40)):
+        cells = {}
+        for _ in range(ncl):
+            p0, t0 = int(rng.integers(0, P)), int(rng.integers(0, T))
+            for dp in range(-1, 2):
+                for dt in range(-2, 3):
+                    p, t = p0 + dp, t0 + dt
+                    if 0 <= p < P and 0 <= t < T and rng.random() < 0.8:
+                        cells[(p, t)] = int(rng.integers(1, 400))
+        for p, t in ((P - 1, T - 1), (P - 1, T - 2), (P - 2, T - 1), (0, 0), (0, T - 1), (P - 1, 0)):
+            cells[(p, t)] = int(rng.integers(4, 999))
+        digits = sort_digits(orc.make_digits([(p, t, q) for (p, t), q in cells.items()]))
+        geom = (1, 1, P, T, None)
+        ora, ost = orc.run(digits, *geom[:4])
+        if path == "fused_lines" and T > 40000:
+            # 20 bitmap slots of 65535 bins do not fit in shared memory: the library runs the block kernel instead
+            monkeypatch.delenv("TPC_CF_FUSED_KERNEL")
+        cl, st = gpu_run(digits, geom, PATHS[path], max_clusters=ost["n_clusters"] + 8)
+        if path == "fused_lines" and T > 40000:
+            assert st["kernel"] == "k_fused_blocks"
+            monkeypatch.setenv("TPC_CF_FUSED_KERNEL", "lines")
+        assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == 0
+        assert_clusters_equal(cl, ora, "max geometry %dx%d/%s" % (P, T, path))
