@@ -164,8 +164,9 @@ __device__ __forceinline__ void bwindow(uint32_t slot, uint32_t dsub, const Slot
 
 // MULTI: the time axis is covered in sg.n_pass > 1 passes (long lines).  VAR: flags / cuts requested (V1..V3); the
 // default instantiation carries none of that code.
-template <bool MULTI, bool VAR>
-__global__ void __launch_bounds__(kBThreads, 2)
+// MINB: CTAs per SM the registers are limited for (3 when the slots are small enough for a third CTA).
+template <bool MULTI, bool VAR, int MINB>
+__global__ void __launch_bounds__(kBThreads, MINB)
 k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
                uint32_t pads_per_unit, uint32_t units_per_plane, SlotGeo sg, uint32_t q_peak_min, uint32_t q_gate,
                Variant var, Counters* cnt, uint32_t* __restrict__ line_cnt, uint4* __restrict__ stage)
@@ -619,17 +620,28 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_fused_blocks<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_blocks<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_blocks<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_blocks<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+        cudaError_t e = cudaSuccess;
+        auto set = [&](const void* f, int bytes) {
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        };
+        set((const void*)k_fused_blocks<false, false, 2>, 112 * 1024); set((const void*)k_fused_blocks<true, false, 2>, 112 * 1024);
+        set((const void*)k_fused_blocks<false, true, 2>, 112 * 1024);  set((const void*)k_fused_blocks<true, true, 2>, 112 * 1024);
+        set((const void*)k_fused_blocks<false, false, 3>, 72 * 1024);  set((const void*)k_fused_blocks<true, false, 3>, 72 * 1024);
+        set((const void*)k_fused_blocks<false, true, 3>, 72 * 1024);   set((const void*)k_fused_blocks<true, true, 3>, 72 * 1024);
         if (e != cudaSuccess) return TPC_CF_E_CUDA;
         attr_set = true;
     }
     if (ev_k0) cudaEventRecord(ev_k0, st);
     g_last_kernel = "k_fused_blocks";
-    auto kern = sg.n_pass > 1 ? (var.active ? k_fused_blocks<true, true> : k_fused_blocks<true, false>)
-                              : (var.active ? k_fused_blocks<false, true> : k_fused_blocks<false, false>);
+    // a third CTA per SM when the slots are small (short lines): the kernel is latency bound
+    const uint32_t budget3 = 227u * 1024u / 3u - 1024u - 3328u;
+    bool three = smem <= budget3;
+    if (const char* e3 = getenv("TPC_CF_CTAS_PER_SM")) three = three && atoi(e3) != 2;
+    const bool m = sg.n_pass > 1, v = var.active != 0u;
+    auto kern = three ? (m ? (v ? k_fused_blocks<true, true, 3> : k_fused_blocks<true, false, 3>)
+                           : (v ? k_fused_blocks<false, true, 3> : k_fused_blocks<false, false, 3>))
+                      : (m ? (v ? k_fused_blocks<true, true, 2> : k_fused_blocks<true, false, 2>)
+                           : (v ? k_fused_blocks<false, true, 2> : k_fused_blocks<false, false, 2>));
     kern<<<g.n_planes * upp, kBThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
                                                     pads_per_unit, upp, sg, q_peak_min, q_gate, var,
                                                     ws.counters, ws.line_cnt, (uint4*)ws.stage);
