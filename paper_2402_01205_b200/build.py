@@ -11,7 +11,8 @@ SO = os.path.join(_HERE, "libtpc_cf.so")
 SOURCES = ["tpc_cf_api.cu", "tpc_cf_general.cu", "tpc_cf_fused.cu", "tpc_cf_blocks.cu", "tpc_cf_compact.cu"]
 HEADERS = [os.path.join(CSRC, "tpc_cf_internal.cuh"),
            os.path.join(os.path.dirname(_HERE), "include", "tpc_cf.h")]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+EXTRA = os.environ.get("TPC_CF_NVCC_EXTRA", "").split()
+NVCC_FLAGS = EXTRA + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall"]
 
 

@@ -26,6 +26,10 @@ static constexpr int kBS = kBWarps;              // lines per step: one per warp
 static constexpr int kBSlots = 2 * kBS + 4;      // lines l0-2 .. l0+S+1 in use, next S being built
 static constexpr int kStageDepth = 4;            // staging ring: chunks of 32 digits (256 B each) per warp
 static constexpr uint32_t kDirOff = 16;          // dir starts after the header
+#ifndef TPC_CF_BALANCE
+#define TPC_CF_BALANCE 1
+#endif
+static constexpr bool kBalance = TPC_CF_BALANCE != 0;   // in-step load balancing by line length
 
 // ---- shared-window accessors (32-bit addresses: no generic-address arithmetic in the hot loops) ------------------
 __device__ __forceinline__ uint32_t lds32(uint32_t a)
@@ -505,7 +509,7 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
         // proportional to the line lengths (known from the index).  The warp with the longest line to process gets
         // the shortest line to build, and so on: the 8 sums come out nearly equal and the barrier waits less.
         int ip = warp, ib = warp;                               // which of the 8 lines this warp processes / builds
-        {
+        if (kBalance) {
             uint32_t lp = 0u, lb = 0u;
             if (lane < kBS) {
                 const int p = l0 + lane, q = l0 + kBS + 2 + lane;
@@ -513,14 +517,21 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
                 if (more && q >= blo && q < bhi) lb = min(s_ls[q + 1] - s_ls[q], 0xfffeu) + 1u;
             }
             const uint32_t mine = lp | (lb << 16);
-            uint32_t rp = 0u, rb = 0u;                          // rank of lane's process line (descending) / build line (ascending)
-#pragma unroll
-            for (int j = 0; j < kBS; ++j) {
-                const uint32_t o = __shfl_sync(0xffffffffu, mine, j);
-                const uint32_t op = o & 0xffffu, ob = o >> 16;
-                rp += (op > lp || (op == lp && j < lane)) ? 1u : 0u;
-                rb += (ob < lb || (ob == lb && j < lane)) ? 1u : 0u;
-            }
+            // ranks of the 8 lines by all-pairs comparison, two pairs per lane: lane L compares line i = L & 7 with
+            // lines j = L >> 3 and j + 4; the four partial counts of a line are added across lanes i, i+8, i+16, i+24.
+            // rp: rank of line i among the lines to process, longest first; rb: among the lines to build, shortest first.
+            const int i = lane & 7, j0 = lane >> 3;
+            const uint32_t vi = __shfl_sync(0xffffffffu, mine, i);
+            const uint32_t va = __shfl_sync(0xffffffffu, mine, j0), vb = __shfl_sync(0xffffffffu, mine, j0 + 4);
+            const uint32_t pi = vi & 0xffffu, bi = vi >> 16;
+            uint32_t cnt = 0u;                                  // process count | build count << 8
+            cnt += ((va & 0xffffu) > pi || ((va & 0xffffu) == pi && j0 < i)) ? 1u : 0u;
+            cnt += ((vb & 0xffffu) > pi || ((vb & 0xffffu) == pi && j0 + 4 < i)) ? 1u : 0u;
+            cnt += ((va >> 16) < bi || ((va >> 16) == bi && j0 < i)) ? 256u : 0u;
+            cnt += ((vb >> 16) < bi || ((vb >> 16) == bi && j0 + 4 < i)) ? 256u : 0u;
+            cnt += __shfl_xor_sync(0xffffffffu, cnt, 8);
+            cnt += __shfl_xor_sync(0xffffffffu, cnt, 16);
+            const uint32_t rp = cnt & 0xffu, rb = cnt >> 8;
             const unsigned mp = __ballot_sync(0xffffffffu, lane < kBS && rp == (uint32_t)warp);
             const unsigned mb = __ballot_sync(0xffffffffu, lane < kBS && rb == (uint32_t)warp);
             ip = __ffs(mp) - 1;

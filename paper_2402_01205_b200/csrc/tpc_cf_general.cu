@@ -57,6 +57,7 @@ k_unscatter(const uint2* __restrict__ digits, uint64_t n, Geo g, uint16_t* __res
     if (digit_valid(g, d.x, d.y)) map[cell_offset(g, d.x, d.y)] = 0;
 }
 
+template <bool VAR>   // VAR: flags / cuts requested (V1..V3)
 __global__ void __launch_bounds__(kThreads)
 k_peaks_map(const uint2* __restrict__ digits, uint64_t n, Geo g, const uint16_t* __restrict__ map,
             uint32_t q_peak_min, uint32_t q_gate, Variant var, uint32_t* __restrict__ peakmask,
@@ -87,7 +88,7 @@ k_peaks_map(const uint2* __restrict__ digits, uint64_t n, Geo g, const uint16_t*
             for (int b = 0; b < 5; ++b) c[a][b] = (int)c0[(a - 2) * TS + (b - 2)];
         const ClusterSums sums = cluster_sums(c, q_gate);
         uint32_t fl = 0u;
-        if (var.active)
+        if (VAR)
             peak = cluster_variant(sums, (d.x >> 16) & 0xffu, d.y & 0xffffu, d.y >> 16, g.npads[(d.x >> 8) & 0xffu],
                                    g.n_time, var, &fl);
         if (peak) {
@@ -134,8 +135,12 @@ int launch_general_peaks(const Geo& g, const Workspace& ws, const tpc_digit* dig
     k_scatter<<<grid_for(n), kThreads, 0, st>>>((const uint2*)digits, n, g, ws.map, ws.counters);
     if (ev_k0) cudaEventRecord(ev_k0, st);
     g_last_kernel = "k_peaks_map";
-    k_peaks_map<<<grid_for(n), kThreads, 0, st>>>((const uint2*)digits, n, g, ws.map, q_peak_min, q_gate, var,
-                                                  ws.peakmask, (uint4*)ws.stage);
+    if (var.active)
+        k_peaks_map<true><<<grid_for(n), kThreads, 0, st>>>((const uint2*)digits, n, g, ws.map, q_peak_min, q_gate, var,
+                                                            ws.peakmask, (uint4*)ws.stage);
+    else
+        k_peaks_map<false><<<grid_for(n), kThreads, 0, st>>>((const uint2*)digits, n, g, ws.map, q_peak_min, q_gate, var,
+                                                             ws.peakmask, (uint4*)ws.stage);
     if (ev_k1) cudaEventRecord(ev_k1, st);
     return 2;
 }
