@@ -271,27 +271,32 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
         const uint32_t nlo = thi - 2u;                      // the next pass needs the line from this time on
         const uint2* gp = digits + lbeg + 32u * kAhead + lane;   // this lane's digit of chunk c + kAhead
         uint32_t ro = 0u;                                   // ring offset of chunk c
-        uint32_t carry = 0u;                                // y of the digit before this chunk
+        const uint32_t off_own = (8u * (uint32_t)lane + kStageDepth * 256u - 8u) & (kStageDepth * 256u - 1u);
+        const uint32_t off_prev = (8u * (uint32_t)lane + kStageDepth * 256u - 16u) & (kStageDepth * 256u - 1u);
         uint32_t nblk = 0u, nsurv = 0u;                     // warp-uniform running counts
         uint32_t nbad = 0u;                                 // per lane
         uint32_t next_pos = lend;                           // first digit with time >= nlo (warp-uniform)
         bool found = false;
-        for (uint32_t c0 = 0; c0 < len; c0 += 32u) {
-            const uint32_t jl = c0 + (uint32_t)lane;
-            if (jl + 32u * kAhead < len) cp_async8(stg_lane + ((ro + 256u * kAhead) & (256u * (kStageDepth - 1))), gp);
+        // Iteration c works on the digits 32c-1 .. 32c+30 (lane i: digit 32c+i-1): with this one-digit shift the
+        // successor of the last digit of the iteration is still in chunk c, so only chunk c has to have landed and
+        // the copies of chunks c+1, c+2 stay in flight (one more chunk of slack than with a look-ahead into chunk c+1).
+        for (uint32_t c0 = 0; c0 <= len; c0 += 32u) {
+            const uint32_t jl = c0 + (uint32_t)lane - 1u;   // 0xffffffff for the digit before the line: inactive
+            // chunks 0 .. c+2 are committed at this point; all but the two newest have landed: chunks <= c
+            asm volatile("cp.async.wait_group %0;" ::"n"(kAhead - 1) : "memory");
+            __syncwarp();
+            // this digit and its neighbours in the line, straight from the staging ring (one contiguous 1 KB window per
+            // warp, so "previous / next digit" is -8 / +8 bytes modulo 1 KB): three independent loads.  Chunk c-1 is
+            // still there: its entry is recycled by the cp.async below, after these loads.
+            const uint2 d = lds64(stg + ((off_own + ro) & (kStageDepth * 256u - 1u)));
+            const uint32_t prevy = lds32(stg + ((off_prev + ro) & (kStageDepth * 256u - 1u)) + 4u);
+            const uint32_t nexty = lds32(stg_lane + ro + 4u);
+            const uint32_t y = d.y;
+            if (32u * kAhead + c0 + (uint32_t)lane < len)
+                cp_async8(stg_lane + ((ro + 256u * kAhead) & (256u * (kStageDepth - 1))), gp);
             gp += 32;
             asm volatile("cp.async.commit_group;" ::: "memory");
-            asm volatile("cp.async.wait_group %0;" ::"n"(kAhead - 1) : "memory");   // chunks <= c+1 have landed
-            __syncwarp();
-            const uint2 d = lds64(stg_lane + ro);
             ro = (ro + 256u) & (256u * (kStageDepth - 1));
-            const uint32_t y_next0 = lds32(stg + ro + 4u);  // first y of chunk c+1
-            const uint32_t y = d.y;
-            uint32_t prevy = __shfl_up_sync(0xffffffffu, y, 1);
-            uint32_t nexty = __shfl_down_sync(0xffffffffu, y, 1);
-            if (lane == 0) prevy = carry;
-            if (lane == 31) nexty = y_next0;
-            carry = __shfl_sync(0xffffffffu, y, 31);
             const bool act = jl < len, nf = jl != 0u;
             const uint32_t t = y & 0xffffu;
             const uint32_t xkey = (d.x ^ w0_line) & 0x00ffffffu;
@@ -323,11 +328,11 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
             nsurv += (uint32_t)__popc(smk);
             if (MULTI && !last_pass) {
                 // where the next pass starts in this line, and whether this pass has seen all it stores
-                const bool tail = c0 + 32u >= len;
-                const uint32_t t31 = carry & 0xffffu;       // time of the chunk's last digit (full chunks)
+                const bool tail = c0 + 31u >= len;           // this iteration reaches the last digit of the line
+                const uint32_t t31 = __shfl_sync(0xffffffffu, y, 31) & 0xffffu;   // time of the iteration's last digit (if not tail)
                 if (!found && (tail || t31 >= nlo)) {
                     const unsigned m = __ballot_sync(0xffffffffu, act && t >= nlo);
-                    if (m) { next_pos = lbeg + c0 + (uint32_t)__ffs(m) - 1u; found = true; }
+                    if (m) { next_pos = lbeg + c0 + (uint32_t)__ffs(m) - 2u; found = true; }   // digit of lane i: c0+i-1
                 }
                 if (!tail && t31 >= whi) {                  // every later digit is beyond the window
                     asm volatile("cp.async.wait_group 0;" ::: "memory");   // the ring is reused by the next line
