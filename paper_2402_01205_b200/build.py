@@ -1,4 +1,4 @@
-"""Builds libtpc_cf.so (the C-ABI library of include/tpc_cf.h) in-tree with nvcc for sm_100a.
+"""Builds libtpc_cf.so (the C-ABI library of include/tpc_cf.h and include/tpc_ec.h) in-tree with nvcc for sm_100a.
 
 nvcc cross-compiles without a GPU.  The built .so is git-ignored but travels with the snapshot to the GPU box.
 """
@@ -8,9 +8,11 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libtpc_cf.so")
-SOURCES = ["tpc_cf_api.cu", "tpc_cf_general.cu", "tpc_cf_fused.cu", "tpc_cf_blocks.cu", "tpc_cf_compact.cu"]
+SOURCES = ["tpc_cf_api.cu", "tpc_cf_general.cu", "tpc_cf_fused.cu", "tpc_cf_blocks.cu", "tpc_cf_compact.cu",
+           "tpc_ec.cu"]
 HEADERS = [os.path.join(CSRC, "tpc_cf_internal.cuh"),
-           os.path.join(os.path.dirname(_HERE), "include", "tpc_cf.h")]
+           os.path.join(os.path.dirname(_HERE), "include", "tpc_cf.h"),
+           os.path.join(os.path.dirname(_HERE), "include", "tpc_ec.h")]
 EXTRA = os.environ.get("TPC_CF_NVCC_EXTRA", "").split()
 NVCC_FLAGS = EXTRA + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall"]

@@ -1,0 +1,624 @@
+// tpc_ec.cu — entropy coder for the TPC cluster stream ("TPC-EC v1", include/tpc_ec.h; step named in PAPER.md:55, 57).
+// Product code, sm_100a.  Shares nothing with oracle/tpc_ec_oracle.c: the format text in the header is the only link.
+//
+// Encoder, on the caller's stream:
+//   k_ec_symbolize   (Q) one thread per cluster: 13 symbol bytes (SoA streams in the workspace), order / range checks,
+//                    histograms (warp-aggregated shared-memory atomics, one flush per CTA)
+//   k_ec_plane_count plane_count[] of the container: two lower_bounds per plane on the sorted cluster keys
+//   k_ec_normalize   (N) one warp per stream: 12-bit frequencies -> container table and (f | cum << 16) coding table
+//   k_ec_code<0>     (C) sizes: one warp per (stream, block), one rANS state per lane; byte counts per lane
+//   k_ec_layout      exclusive scan of the record sizes -> directory, header, status; capacity check
+//   k_ec_code<1>     (C) again, this time storing every byte at its final place (no worst-case staging buffer: the
+//                    coder is cheap — ~50 instructions per symbol — and the payload is written exactly once)
+// Decoder:
+//   k_ec_dec_tables  header check, table sums, slot -> symbol table (4096 bytes per stream), plane starts
+//   k_ec_decode      one warp per (stream, block): 32 lanes decode forwards into the symbol streams
+//   k_ec_rebuild     inverse of (Q): one warp per plane, pads by a warp scan, times by a segmented warp scan
+#include <new>
+#include <string.h>
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tpc_ec.h"
+
+namespace tpcec {
+
+static constexpr uint32_t kStreams = 13;
+static constexpr uint32_t kBlock = 16384;          // symbols per block
+static constexpr uint32_t kLanes = 32;
+static constexpr uint32_t kPerLane = kBlock / kLanes;
+static constexpr uint32_t kProbBits = 12, kProbScale = 1u << kProbBits;
+static constexpr uint32_t kL = 1u << 23;
+static constexpr uint32_t kRecFixed = kLanes * 4 + kLanes * 2;   // states + byte counts
+static constexpr uint32_t kMagic = 0x45435054u;
+
+struct Layout {                // byte offsets inside the container (all host-computable from n and the geometry)
+    uint64_t off_counts, off_freq, off_dir, off_records;
+    uint32_t n_blocks, n_planes;
+};
+
+static inline Layout layout_of(uint32_t n_sectors, uint32_t n_rows, uint64_t n)
+{
+    Layout l;
+    l.n_planes = n_sectors * n_rows;
+    l.n_blocks = (uint32_t)((n + kBlock - 1) / kBlock);
+    l.off_counts = 64;
+    l.off_freq = l.off_counts + 4ull * l.n_planes;
+    l.off_dir = (l.off_freq + 2ull * 256 * kStreams + 7) & ~7ull;
+    l.off_records = l.off_dir + 8ull * ((uint64_t)kStreams * l.n_blocks + 1);
+    return l;
+}
+
+struct Ws {
+    uint8_t* sym;          // [13][stride]
+    uint64_t stride;
+    uint32_t* hist;        // [13][256]
+    uint32_t* ftab;        // [13][256]  f | cum << 16
+    uint16_t* lane_nb;     // [13 * max_blocks * 32]
+    uint32_t* rec_size;    // [13 * max_blocks]
+    uint8_t* lut;          // [13][4096] slot -> symbol
+    uint32_t* plane_start; // [planes + 1]
+    uint32_t* flags;       // [4]: error bits, payload-fits flag
+};
+
+// ---- (Q) ----------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t quant(float v)
+{
+    return (uint32_t)fminf(fmaxf(rintf(v), 0.0f), 255.0f);      // NaN -> 0
+}
+
+__global__ void __launch_bounds__(256)
+k_ec_symbolize(const uint4* __restrict__ cl, uint32_t n, uint32_t n_sectors, uint32_t n_rows, Ws ws)
+{
+    __shared__ uint32_t s_hist[kStreams * 256];
+    for (uint32_t i = threadIdx.x; i < kStreams * 256; i += blockDim.x) s_hist[i] = 0u;
+    __syncthreads();
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool act = i < n;
+    uint32_t sym[kStreams];
+    uint32_t err = 0u;
+    if (act) {
+        const uint4 lo = __ldg(cl + 2 * (size_t)i), hi = __ldg(cl + 2 * (size_t)i + 1);
+        const uint32_t sector = lo.x & 0xffu, row = (lo.x >> 8) & 0xffu, pad = (lo.x >> 16) & 0xffu, fl = lo.x >> 24;
+        const uint32_t time = lo.y & 0xffffu, qmax = lo.y >> 16, qtot = lo.z;
+        bool same = false;
+        uint32_t ppad = 0u, ptime = 0u;
+        if (sector >= n_sectors || row >= n_rows) err |= TPC_EC_ERR_UNSORTED;
+        if (i > 0u) {
+            const uint2 p = __ldg((const uint2*)(cl + 2 * (size_t)(i - 1)));
+            const uint32_t ps = p.x & 0xffu, pr = (p.x >> 8) & 0xffu;
+            ppad = (p.x >> 16) & 0xffu; ptime = p.y & 0xffffu;
+            const uint64_t kp = ((uint64_t)ps << 32) | ((uint64_t)pr << 24) | ((uint64_t)ppad << 16) | ptime;
+            const uint64_t kc = ((uint64_t)sector << 32) | ((uint64_t)row << 24) | ((uint64_t)pad << 16) | time;
+            if (kp >= kc) err |= TPC_EC_ERR_UNSORTED;
+            same = ps == sector && pr == row;
+        }
+        const uint32_t dpad = same ? ((pad - ppad) & 0xffu) : pad;
+        const uint32_t v = (same && pad == ppad) ? ((time - ptime) & 0xffffu) : time;
+        const uint32_t dq = (qtot - qmax) & 0xffffffu;
+        if (qtot < qmax || qtot - qmax >= (1u << 24)) err |= TPC_EC_ERR_QTOT;
+        sym[0] = dpad; sym[1] = v & 255u; sym[2] = v >> 8; sym[3] = qmax & 255u; sym[4] = qmax >> 8;
+        sym[5] = dq & 255u; sym[6] = (dq >> 8) & 255u; sym[7] = dq >> 16; sym[8] = fl;
+        // fp32, one rounding per operation (explicit intrinsics: no contraction)
+        sym[9] = quant(__fmul_rn(__fadd_rn(__fsub_rn(__uint_as_float(lo.w), (float)pad), 2.0f), 64.0f));
+        sym[10] = quant(__fmul_rn(__fadd_rn(__fsub_rn(__uint_as_float(hi.x), (float)time), 2.0f), 64.0f));
+        sym[11] = quant(__fmul_rn(__uint_as_float(hi.y), 128.0f));
+        sym[12] = quant(__fmul_rn(__uint_as_float(hi.z), 128.0f));
+#pragma unroll
+        for (uint32_t s = 0; s < kStreams; ++s) ws.sym[s * ws.stride + i] = (uint8_t)sym[s];
+    }
+    // histograms: lanes with the same symbol elect a leader (the streams are skewed: plain atomics would serialise)
+    const unsigned amask = __ballot_sync(0xffffffffu, act);
+    if (act) {
+        const uint32_t lane = threadIdx.x & 31u;
+#pragma unroll
+        for (uint32_t s = 0; s < kStreams; ++s) {
+            const unsigned peers = __match_any_sync(amask, sym[s]);
+            if ((uint32_t)(__ffs(peers) - 1) == lane) atomicAdd(&s_hist[s * 256 + sym[s]], (uint32_t)__popc(peers));
+        }
+    }
+    if (err) atomicOr(&ws.flags[0], err);
+    __syncthreads();
+    for (uint32_t k = threadIdx.x; k < kStreams * 256; k += blockDim.x)
+        if (s_hist[k]) atomicAdd(&ws.hist[k], s_hist[k]);
+}
+
+// plane_count[p] = lower_bound(p + 1) - lower_bound(p) on the plane number of the sorted clusters
+__global__ void k_ec_plane_count(const uint4* __restrict__ cl, uint32_t n, uint32_t n_rows, uint32_t n_planes,
+                                 uint32_t* __restrict__ counts)
+{
+    const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_planes) return;
+    auto lb = [&](uint32_t plane) {
+        uint32_t lo = 0, hi = n;
+        while (lo < hi) {
+            const uint32_t mid = lo + ((hi - lo) >> 1);
+            const uint32_t w = __ldg((const uint32_t*)(cl + 2 * (size_t)mid));
+            if ((w & 0xffu) * n_rows + ((w >> 8) & 0xffu) < plane) lo = mid + 1; else hi = mid;
+        }
+        return lo;
+    };
+    counts[p] = lb(p + 1) - lb(p);
+}
+
+// ---- (N) one warp per stream; lane 0 walks the 256 counts (a few microseconds; exactness over speed) -----------------
+__global__ void k_ec_normalize(uint32_t n, Ws ws, uint16_t* __restrict__ freq_out)
+{
+    __shared__ uint32_t f[256];
+    const uint32_t s = blockIdx.x;
+    const uint32_t* hist = ws.hist + s * 256;
+    for (uint32_t a = threadIdx.x; a < 256; a += blockDim.x) {
+        const uint32_t c = hist[a];
+        uint32_t q = 0u;
+        if (n != 0u && c != 0u) {
+            q = (uint32_t)(((uint64_t)c * kProbScale) / n);
+            if (q < 1u) q = 1u;
+        }
+        f[a] = q;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && n != 0u) {
+        long long D = kProbScale;
+        for (int a = 0; a < 256; ++a) D -= f[a];
+        if (D > 0) {
+            int b = 0;
+            for (int a = 1; a < 256; ++a) if (hist[a] > hist[b]) b = a;
+            f[b] += (uint32_t)D;
+        }
+        while (D < 0) {
+            int b = 0;
+            for (int a = 1; a < 256; ++a) if (f[a] > f[b]) b = a;
+            const long long d = -D < (long long)f[b] - 1 ? -D : (long long)f[b] - 1;
+            f[b] -= (uint32_t)d;
+            D += d;
+        }
+        uint32_t cum = 0u;
+        for (int a = 0; a < 256; ++a) {
+            ws.ftab[s * 256 + a] = f[a] | (cum << 16);
+            cum += f[a];
+        }
+    }
+    __syncthreads();
+    for (uint32_t a = threadIdx.x; a < 256; a += blockDim.x) {
+        freq_out[s * 256 + a] = (uint16_t)f[a];
+        if (n == 0u) ws.ftab[s * 256 + a] = 0u;
+    }
+}
+
+// ---- (C) encoder -------------------------------------------------------------------------------------------------
+// WRITE = false: byte counts only.  WRITE = true: the same walk, bytes stored at their final place.
+template <bool WRITE>
+__global__ void __launch_bounds__(256)
+k_ec_code(uint32_t n, uint32_t n_blocks, Ws ws, uint8_t* __restrict__ out, const uint64_t* __restrict__ rec_off)
+{
+    __shared__ uint32_t s_tab[256];
+    const uint32_t s = blockIdx.y;
+    s_tab[threadIdx.x] = ws.ftab[s * 256 + threadIdx.x];
+    __syncthreads();
+    if (WRITE && ws.flags[1] == 0u) return;                    // the payload does not fit: nothing beyond the directory
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t b = blockIdx.x * (blockDim.x >> 5) + warp;
+    if (b >= n_blocks) return;
+    const uint32_t e = s * n_blocks + b;
+    const uint32_t first = b * kBlock + lane;
+    uint32_t m = 0u;
+    if (first < n) {
+        m = (n - first + kLanes - 1) / kLanes;
+        if (m > kPerLane) m = kPerLane;
+    }
+    uint8_t* dst = nullptr;
+    if (WRITE) {
+        const uint32_t nb = ws.lane_nb[(size_t)e * kLanes + lane];
+        uint32_t incl = nb;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+            if ((int)lane >= d) incl += t;
+        }
+        uint8_t* rec = out + rec_off[e];
+        dst = rec + kRecFixed + (incl - nb);
+        ((uint16_t*)(rec + kLanes * 4))[lane] = (uint16_t)nb;
+        const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
+        if (lane < ((4u - (total & 3u)) & 3u)) rec[kRecFixed + total + lane] = 0;      // zero padding to 4
+    }
+    const uint8_t* src = ws.sym + s * ws.stride + first;
+    uint32_t x = kL, nbytes = 0u;
+    for (uint32_t k = m; k-- > 0u;) {
+        const uint32_t tab = s_tab[src[(size_t)k * kLanes]];
+        const uint32_t f = tab & 0xffffu, c = tab >> 16;
+        const uint32_t x_max = f << 19;                        // (L >> 12 << 8) * f <= 2^31
+        while (x >= x_max) {
+            if (WRITE) dst[nbytes] = (uint8_t)x;
+            ++nbytes;
+            x >>= 8;
+        }
+        const uint32_t q = x / f;
+        x = (q << kProbBits) + (x - q * f) + c;
+    }
+    if (WRITE) {
+        ((uint32_t*)(out + rec_off[e]))[lane] = x;
+    } else {
+        ws.lane_nb[(size_t)e * kLanes + lane] = (uint16_t)nbytes;
+        const uint32_t total = __reduce_add_sync(0xffffffffu, nbytes);
+        if (lane == 0) ws.rec_size[e] = (kRecFixed + total + 3u) & ~3u;
+    }
+}
+
+// exclusive scan of the record sizes (one CTA; at most a few 10^4 entries) -> directory, header, status
+__global__ void __launch_bounds__(1024)
+k_ec_layout(uint32_t n, uint32_t n_sectors, uint32_t n_rows, Layout lay, Ws ws, uint8_t* __restrict__ out,
+            uint64_t capacity, tpc_ec_status* __restrict__ status)
+{
+    __shared__ unsigned long long s_warp[32];
+    __shared__ unsigned long long s_base;
+    const uint32_t entries = kStreams * lay.n_blocks;
+    uint64_t* dir = (uint64_t*)(out + lay.off_dir);
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_base = lay.off_records;
+    __syncthreads();
+    for (uint32_t c0 = 0; c0 < entries; c0 += 1024u) {
+        const uint32_t i = c0 + threadIdx.x;
+        const unsigned long long v = i < entries ? ws.rec_size[i] : 0ull;
+        unsigned long long incl = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned long long t = __shfl_up_sync(0xffffffffu, incl, d);
+            if ((int)lane >= d) incl += t;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            unsigned long long w = s_warp[lane], wi = w;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned long long t = __shfl_up_sync(0xffffffffu, wi, d);
+                if ((int)lane >= d) wi += t;
+            }
+            s_warp[lane] = wi - w;                              // exclusive over warps
+        }
+        __syncthreads();
+        const unsigned long long base = s_base;
+        if (i < entries) dir[i] = base + s_warp[warp] + (incl - v);
+        __syncthreads();
+        if (threadIdx.x == 1023) s_base = base + s_warp[31] + incl;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const unsigned long long total = s_base;
+        dir[entries] = total;
+        uint32_t* h = (uint32_t*)out;
+        h[0] = kMagic; h[1] = 1u; h[2] = n; h[3] = 0u; h[4] = n_sectors; h[5] = n_rows; h[6] = kStreams; h[7] = kBlock;
+        h[8] = lay.n_blocks; h[9] = 0u; h[10] = (uint32_t)total; h[11] = (uint32_t)(total >> 32);
+        h[12] = h[13] = h[14] = h[15] = 0u;
+        const bool fits = total <= capacity;
+        ws.flags[1] = fits ? 1u : 0u;
+        status->n_clusters = n;
+        status->bytes = total;
+        status->error = ws.flags[0] | (fits ? 0u : TPC_EC_ERR_CAPACITY);
+        status->rsv = 0u;
+    }
+    // zero padding between the tables and the directory
+    for (uint64_t a = lay.off_freq + 2ull * 256 * kStreams + threadIdx.x; a < lay.off_dir; a += 1024u) out[a] = 0;
+}
+
+// ---- decoder -----------------------------------------------------------------------------------------------------
+// grid = 13 + 1: CTA s < 13 checks table s and builds its slot -> symbol table; the last CTA checks the header and
+// scans the plane counts.
+__global__ void __launch_bounds__(256)
+k_ec_dec_tables(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, uint32_t n_sectors, uint32_t n_rows,
+                Layout lay, Ws ws)
+{
+    __shared__ uint32_t s_f[256], s_c[257];
+    __shared__ unsigned long long s_sum;
+    if (blockIdx.x < kStreams) {
+        const uint32_t s = blockIdx.x;
+        const uint16_t* freq = (const uint16_t*)(in + lay.off_freq) + s * 256;
+        s_f[threadIdx.x] = freq[threadIdx.x];
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            uint32_t cum = 0u;
+            for (int a = 0; a < 256; ++a) { s_c[a] = cum; cum += s_f[a]; }
+            s_c[256] = cum;
+            if (n != 0u && cum != kProbScale) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER);
+        }
+        __syncthreads();
+        const bool ok = s_c[256] == kProbScale;
+        const uint32_t a = threadIdx.x;
+        ws.ftab[s * 256 + a] = ok ? (s_f[a] | (s_c[a] << 16)) : 0u;
+        if (ok) for (uint32_t k = 0; k < s_f[a]; ++k) ws.lut[s * kProbScale + s_c[a] + k] = (uint8_t)a;
+        return;
+    }
+    // header
+    if (threadIdx.x == 0) {
+        const uint32_t* h = (const uint32_t*)in;
+        const unsigned long long total = (unsigned long long)h[10] | ((unsigned long long)h[11] << 32);
+        const bool ok = h[0] == kMagic && h[1] == 1u && h[2] == n && h[3] == 0u && h[4] == n_sectors && h[5] == n_rows &&
+                        h[6] == kStreams && h[7] == kBlock && h[8] == lay.n_blocks && total == in_bytes;
+        if (!ok) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER);
+        s_sum = 0ull;
+    }
+    __syncthreads();
+    // plane starts: exclusive scan of the plane counts, clamped to n so that no later write can leave the output
+    const uint32_t* counts = (const uint32_t*)(in + lay.off_counts);
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    __shared__ unsigned long long s_w[8];
+    for (uint32_t c0 = 0; c0 < lay.n_planes; c0 += 256u) {
+        const uint32_t p = c0 + threadIdx.x;
+        const unsigned long long v = p < lay.n_planes ? counts[p] : 0ull;
+        unsigned long long incl = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned long long t = __shfl_up_sync(0xffffffffu, incl, d);
+            if ((int)lane >= d) incl += t;
+        }
+        if (lane == 31) s_w[warp] = incl;
+        __syncthreads();
+        unsigned long long wbase = 0ull;
+        for (uint32_t w = 0; w < warp; ++w) wbase += s_w[w];
+        const unsigned long long base = s_sum;
+        const unsigned long long excl = base + wbase + incl - v;
+        if (p < lay.n_planes) ws.plane_start[p] = (uint32_t)(excl < n ? excl : n);
+        __syncthreads();
+        if (threadIdx.x == 255) s_sum = base + wbase + incl;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        ws.plane_start[lay.n_planes] = (uint32_t)(s_sum < n ? s_sum : n);
+        if (s_sum != n) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_ec_decode(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, Layout lay, Ws ws)
+{
+    __shared__ uint32_t s_tab[256];
+    __shared__ __align__(16) uint8_t s_lut[kProbScale];
+    const uint32_t s = blockIdx.y;
+    s_tab[threadIdx.x] = ws.ftab[s * 256 + threadIdx.x];
+    for (uint32_t k = threadIdx.x; k < kProbScale / 16; k += blockDim.x)
+        ((uint4*)s_lut)[k] = ((const uint4*)(ws.lut + s * kProbScale))[k];
+    __syncthreads();
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t b = blockIdx.x * (blockDim.x >> 5) + warp;
+    if (b >= lay.n_blocks) return;
+    const uint32_t e = s * lay.n_blocks + b;
+    const uint64_t* dir = (const uint64_t*)(in + lay.off_dir);
+    const uint64_t r0 = dir[e], r1 = dir[e + 1];
+    bool bad = r0 < lay.off_records || r0 > r1 || r1 > in_bytes || r1 - r0 < kRecFixed || (r0 & 3u) != 0u;
+    bad = __any_sync(0xffffffffu, bad);
+    if (bad) { if (lane == 0) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER); return; }
+    const uint8_t* rec = in + r0;
+    uint32_t x = ((const uint32_t*)rec)[lane];
+    const uint32_t nb = ((const uint16_t*)(rec + kLanes * 4))[lane];
+    uint32_t incl = nb;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+        if ((int)lane >= d) incl += t;
+    }
+    const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
+    if ((uint64_t)kRecFixed + total > r1 - r0) { if (lane == 0) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER); return; }
+    const uint8_t* bytes = rec + kRecFixed + (incl - nb);
+    uint32_t ptr = nb;
+    const uint32_t first = b * kBlock + lane;
+    uint32_t m = 0u;
+    if (first < n) {
+        m = (n - first + kLanes - 1) / kLanes;
+        if (m > kPerLane) m = kPerLane;
+    }
+    uint8_t* dst = ws.sym + s * ws.stride + first;
+    bool fail = false;
+    for (uint32_t k = 0; k < m; ++k) {
+        const uint32_t slot = x & (kProbScale - 1u);
+        const uint32_t a = s_lut[slot];
+        const uint32_t tab = s_tab[a];
+        dst[(size_t)k * kLanes] = (uint8_t)a;
+        x = (tab & 0xffffu) * (x >> kProbBits) + slot - (tab >> 16);
+        while (x < kL) {
+            if (ptr == 0u) { fail = true; x = kL; break; }
+            x = (x << 8) | bytes[--ptr];
+        }
+    }
+    if (x != kL || ptr != 0u) fail = true;
+    if (fail) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER);
+}
+
+// inverse of (Q): one warp per plane
+__global__ void __launch_bounds__(256)
+k_ec_rebuild(uint32_t n, uint32_t n_rows, uint32_t n_planes, uint64_t capacity, Ws ws, uint4* __restrict__ out)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t plane = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (plane >= n_planes) return;
+    const uint32_t beg = ws.plane_start[plane], end = ws.plane_start[plane + 1];
+    const uint32_t w0 = (plane / n_rows) | ((plane % n_rows) << 8);
+    uint32_t carry_pad = 0u, carry_time = 0u;
+    for (uint32_t c0 = beg; c0 < end; c0 += 32u) {
+        const uint32_t i = c0 + lane;
+        const bool act = i < end;
+        uint32_t sy[kStreams];
+#pragma unroll
+        for (uint32_t s = 0; s < kStreams; ++s) sy[s] = act ? ws.sym[s * ws.stride + i] : 0u;
+        uint32_t pad = sy[0];
+        uint32_t tv = sy[1] | (sy[2] << 8);
+        bool head = act && (sy[0] != 0u || i == beg);          // starts a pad line: its time is absolute
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t pu = __shfl_up_sync(0xffffffffu, pad, d);
+            const uint32_t tu = __shfl_up_sync(0xffffffffu, tv, d);
+            const bool hu = __shfl_up_sync(0xffffffffu, head, d);
+            if ((int)lane >= d) {
+                pad += pu;
+                if (!head) { tv += tu; head = hu; }
+            }
+        }
+        pad += carry_pad;
+        if (!head) tv += carry_time;                            // no line start at or before this lane in the chunk
+        carry_pad = __shfl_sync(0xffffffffu, pad, 31);
+        carry_time = __shfl_sync(0xffffffffu, tv, 31);          // inactive tail lanes add 0 and start nothing
+        if (act && i < capacity) {
+            const uint32_t qmax = sy[3] | (sy[4] << 8);
+            const uint32_t dq = sy[5] | (sy[6] << 8) | (sy[7] << 16);
+            pad &= 0xffu; tv &= 0xffffu;
+            uint4 lo, hi;
+            lo.x = w0 | (pad << 16) | (sy[8] << 24);
+            lo.y = tv | (qmax << 16);
+            lo.z = qmax + dq;
+            lo.w = __float_as_uint(__fadd_rn((float)pad, __fmul_rn((float)sy[9] - 128.0f, 0.015625f)));
+            hi.x = __float_as_uint(__fadd_rn((float)tv, __fmul_rn((float)sy[10] - 128.0f, 0.015625f)));
+            hi.y = __float_as_uint(__fmul_rn((float)sy[11], 0.0078125f));
+            hi.z = __float_as_uint(__fmul_rn((float)sy[12], 0.0078125f));
+            hi.w = 0u;
+            out[2 * (size_t)i] = lo;
+            out[2 * (size_t)i + 1] = hi;
+        }
+    }
+}
+
+__global__ void k_ec_dec_status(uint32_t n, uint64_t in_bytes, uint64_t capacity, Ws ws, tpc_ec_status* status)
+{
+    status->n_clusters = n;
+    status->bytes = in_bytes;
+    status->error = ws.flags[0] | (n > capacity ? TPC_EC_ERR_CAPACITY : 0u);
+    status->rsv = 0u;
+}
+
+}  // namespace tpcec
+
+using namespace tpcec;
+
+struct tpc_ec {
+    uint32_t n_sectors, n_rows;
+    uint64_t max_clusters;
+    Ws ws;
+    int last_launches;
+};
+
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static size_t carve(uint32_t n_sectors, uint32_t n_rows, uint64_t max_clusters, char* base, Ws* ws)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) { char* p = base ? base + off : nullptr; off += align256(bytes ? bytes : 1); return p; };
+    const uint64_t max_blocks = (max_clusters + kBlock - 1) / kBlock + 1;
+    Ws w;
+    w.stride = align256(max_clusters ? max_clusters : 1);
+    w.sym = (uint8_t*)take((size_t)kStreams * w.stride);
+    w.hist = (uint32_t*)take(kStreams * 256 * 4);
+    w.ftab = (uint32_t*)take(kStreams * 256 * 4);
+    w.lane_nb = (uint16_t*)take((size_t)kStreams * max_blocks * kLanes * 2);
+    w.rec_size = (uint32_t*)take((size_t)kStreams * max_blocks * 4);
+    w.lut = (uint8_t*)take((size_t)kStreams * kProbScale);
+    w.plane_start = (uint32_t*)take(((size_t)n_sectors * n_rows + 1) * 4);
+    w.flags = (uint32_t*)take(16);
+    if (ws) *ws = w;
+    return off;
+}
+
+static bool geometry_ok(uint32_t n_sectors, uint32_t n_rows, uint64_t max_clusters)
+{
+    return n_sectors >= 1 && n_sectors <= 256 && n_rows >= 1 && n_rows <= 256 && max_clusters < (1ull << 32);
+}
+
+extern "C" size_t tpc_ec_workspace_bytes(uint32_t n_sectors, uint32_t n_rows, uint64_t max_clusters)
+{
+    if (!geometry_ok(n_sectors, n_rows, max_clusters)) return 0;
+    return carve(n_sectors, n_rows, max_clusters, nullptr, nullptr);
+}
+
+extern "C" uint64_t tpc_ec_max_encoded_bytes(uint32_t n_sectors, uint32_t n_rows, uint64_t n)
+{
+    if (!geometry_ok(n_sectors, n_rows, n)) return 0;
+    const Layout l = layout_of(n_sectors, n_rows, n);
+    // per record: fixed part, < 4 bytes of padding, and per lane at most 12 bits per symbol plus 2 bytes of slack
+    return l.off_records + (uint64_t)kStreams * l.n_blocks * (kRecFixed + 4 + 2 * kLanes) + kStreams * ((3 * n + 1) / 2);
+}
+
+extern "C" int tpc_ec_create(tpc_ec** h, uint32_t n_sectors, uint32_t n_rows, uint64_t max_clusters,
+                             void* workspace, size_t workspace_bytes)
+{
+    if (!h || !workspace) return TPC_CF_E_NULL;
+    if (n_sectors == 0 || n_sectors > 256 || n_rows == 0 || n_rows > 256) return TPC_CF_E_GEOMETRY;
+    if (max_clusters >= (1ull << 32)) return TPC_CF_E_CAPACITY;
+    if (((uintptr_t)workspace & 255u) != 0 || workspace_bytes < carve(n_sectors, n_rows, max_clusters, nullptr, nullptr))
+        return TPC_CF_E_WORKSPACE;
+    tpc_ec* e = new (std::nothrow) tpc_ec;
+    if (!e) return TPC_CF_E_NOMEM;
+    e->n_sectors = n_sectors; e->n_rows = n_rows; e->max_clusters = max_clusters; e->last_launches = 0;
+    carve(n_sectors, n_rows, max_clusters, (char*)workspace, &e->ws);
+    *h = e;
+    return TPC_CF_OK;
+}
+
+extern "C" int tpc_ec_encode(tpc_ec* h, const tpc_cluster* clusters, uint64_t n, uint8_t* out, uint64_t out_capacity,
+                             tpc_ec_status* status, void* stream)
+{
+    if (!h || !out || !status || (n && !clusters)) return TPC_CF_E_NULL;
+    if (n > h->max_clusters) return TPC_CF_E_CAPACITY;
+    if (((uintptr_t)out & 15u) != 0 || ((uintptr_t)clusters & 15u) != 0) return TPC_CF_E_WORKSPACE;
+    const Layout lay = layout_of(h->n_sectors, h->n_rows, n);
+    if (out_capacity < lay.off_records) return TPC_CF_E_CAPACITY;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Ws& ws = h->ws;
+    const uint32_t n32 = (uint32_t)n;
+    int launches = 0;
+    cudaMemsetAsync(ws.hist, 0, kStreams * 256 * 4, st);
+    cudaMemsetAsync(ws.flags, 0, 16, st);
+    if (n32) {
+        k_ec_symbolize<<<(n32 + 255) / 256, 256, 0, st>>>((const uint4*)clusters, n32, h->n_sectors, h->n_rows, ws);
+        ++launches;
+    }
+    k_ec_plane_count<<<(lay.n_planes + 127) / 128, 128, 0, st>>>((const uint4*)clusters, n32, h->n_rows, lay.n_planes,
+                                                                  (uint32_t*)(out + lay.off_counts));
+    k_ec_normalize<<<kStreams, 256, 0, st>>>(n32, ws, (uint16_t*)(out + lay.off_freq));
+    launches += 2;
+    const dim3 grid((lay.n_blocks + 7) / 8, kStreams);
+    if (lay.n_blocks) {
+        k_ec_code<false><<<grid, 256, 0, st>>>(n32, lay.n_blocks, ws, nullptr, nullptr);
+        ++launches;
+    }
+    k_ec_layout<<<1, 1024, 0, st>>>(n32, h->n_sectors, h->n_rows, lay, ws, out, out_capacity, status);
+    ++launches;
+    if (lay.n_blocks) {
+        k_ec_code<true><<<grid, 256, 0, st>>>(n32, lay.n_blocks, ws, out, (const uint64_t*)(out + lay.off_dir));
+        ++launches;
+    }
+    h->last_launches = launches;
+    return cudaGetLastError() == cudaSuccess ? TPC_CF_OK : TPC_CF_E_CUDA;
+}
+
+extern "C" int tpc_ec_decode(tpc_ec* h, const uint8_t* in, uint64_t in_bytes, uint64_t n, tpc_cluster* clusters,
+                             uint64_t capacity, tpc_ec_status* status, void* stream)
+{
+    if (!h || !in || !status || (n && !clusters)) return TPC_CF_E_NULL;
+    if (n > h->max_clusters) return TPC_CF_E_CAPACITY;
+    if (((uintptr_t)in & 15u) != 0 || ((uintptr_t)clusters & 15u) != 0) return TPC_CF_E_WORKSPACE;
+    const Layout lay = layout_of(h->n_sectors, h->n_rows, n);
+    if (in_bytes < lay.off_records) return TPC_CF_E_CAPACITY;     // not even the fixed part
+    cudaStream_t st = (cudaStream_t)stream;
+    const Ws& ws = h->ws;
+    const uint32_t n32 = (uint32_t)n;
+    int launches = 0;
+    cudaMemsetAsync(ws.flags, 0, 16, st);
+    k_ec_dec_tables<<<kStreams + 1, 256, 0, st>>>(in, in_bytes, n32, h->n_sectors, h->n_rows, lay, ws);
+    ++launches;
+    if (lay.n_blocks) {
+        k_ec_decode<<<dim3((lay.n_blocks + 7) / 8, kStreams), 256, 0, st>>>(in, in_bytes, n32, lay, ws);
+        k_ec_rebuild<<<(lay.n_planes + 7) / 8, 256, 0, st>>>(n32, h->n_rows, lay.n_planes, capacity, ws, (uint4*)clusters);
+        launches += 2;
+    }
+    k_ec_dec_status<<<1, 1, 0, st>>>(n32, in_bytes, capacity, ws, status);
+    ++launches;
+    h->last_launches = launches;
+    return cudaGetLastError() == cudaSuccess ? TPC_CF_OK : TPC_CF_E_CUDA;
+}
+
+extern "C" int tpc_ec_last_launch_count(const tpc_ec* h) { return h ? h->last_launches : TPC_CF_E_NULL; }
+
+extern "C" int tpc_ec_destroy(tpc_ec* h)
+{
+    if (!h) return TPC_CF_E_NULL;
+    delete h;
+    return TPC_CF_OK;
+}

@@ -15,10 +15,10 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "tpc_cf.h")).read()
+def declared_symbols(header="tpc_cf.h", prefix="tpc_cf_"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(tpc_cf_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(%s[a-z_]+)\s*\(" % prefix, text)))
 
 
 def test_library_exports_every_declared_symbol():
@@ -29,6 +29,57 @@ def test_library_exports_every_declared_symbol():
     for s in syms:
         assert hasattr(lib, s), "libtpc_cf.so does not export %s" % s
     assert sorted(cf.EXPORTS) == syms, "binding.EXPORTS and include/tpc_cf.h disagree"
+
+
+def test_every_header_under_include_is_covered():
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["tpc_cf.h", "tpc_ec.h"]
+
+
+def test_library_exports_every_entropy_coder_symbol():
+    import paper_2402_01205_b200 as cf
+    lib = cf.load()
+    syms = declared_symbols("tpc_ec.h", "tpc_ec_")
+    assert "tpc_ec_encode" in syms and "tpc_ec_decode" in syms
+    for s in syms:
+        assert hasattr(lib, s), "libtpc_cf.so does not export %s" % s
+    assert sorted(cf.EC_EXPORTS) == syms, "ec_binding.EC_EXPORTS and include/tpc_ec.h disagree"
+    src = open(os.path.join(ROOT, "paper_2402_01205_b200", "ec_binding.py")).read()
+    assert "oracle" not in src, "the product binding must not reference the oracle"
+
+
+def test_entropy_coder_host_logic_without_a_device():
+    """sizes and synchronous argument errors of include/tpc_ec.h (no kernel is launched: create / destroy keep host
+    state only, and every check below fails before the first enqueue)"""
+    import paper_2402_01205_b200 as cf
+    from paper_2402_01205_b200 import ec_binding as eb
+    assert cf.EC_STATUS.itemsize == 24
+    assert cf.tpc_ec_workspace_bytes(0, 152, 100) == 0 and cf.tpc_ec_workspace_bytes(36, 257, 100) == 0
+    assert cf.tpc_ec_workspace_bytes(36, 152, 1 << 32) == 0
+    w = cf.tpc_ec_workspace_bytes(36, 152, 12_000_000)
+    assert 13 * 12_000_000 < w < 16 * 12_000_000 + (1 << 20)          # 13 symbol bytes per cluster dominate
+    # fixed part of the container: header, plane counts, 13 tables, directory; then <= 12 bits per symbol + slack
+    n = 100_000
+    nb = (n + 16383) // 16384
+    fixed = ((64 + 4 * 36 * 152 + 2 * 256 * 13 + 7) & ~7) + 8 * (13 * nb + 1)
+    m = cf.tpc_ec_max_encoded_bytes(36, 152, n)
+    assert fixed + 13 * n * 3 // 2 <= m <= fixed + 13 * n * 3 // 2 + 13 * nb * 300
+    assert cf.tpc_ec_max_encoded_bytes(36, 152, 0) == fixed - 8 * 13 * nb
+    lib = eb._lib()
+    h = ctypes.c_void_p()
+    fake = ctypes.c_void_p(1 << 20)                                   # never dereferenced by the calls below
+    assert lib.tpc_ec_create(ctypes.byref(h), 36, 152, 1000, None, w) == -1
+    assert lib.tpc_ec_create(ctypes.byref(h), 0, 152, 1000, fake, w) == -2
+    assert lib.tpc_ec_create(ctypes.byref(h), 36, 152, 1000, ctypes.c_void_p((1 << 20) + 8), w) != 0   # misaligned
+    assert lib.tpc_ec_create(ctypes.byref(h), 36, 152, 1000, fake, 1000) != 0                         # too small
+    assert lib.tpc_ec_create(ctypes.byref(h), 36, 152, 1000, fake, w) == 0
+    assert lib.tpc_ec_encode(h, fake, 1001, fake, 1 << 30, fake, None) != 0       # n > max_clusters
+    assert lib.tpc_ec_encode(h, fake, 10, None, 1 << 30, fake, None) == -1        # NULL out
+    assert lib.tpc_ec_encode(h, fake, 10, fake, 100, fake, None) != 0             # below the fixed part
+    assert lib.tpc_ec_encode(h, fake, 10, ctypes.c_void_p((1 << 20) + 4), 1 << 30, fake, None) != 0   # misaligned
+    assert lib.tpc_ec_decode(h, fake, 40, 10, fake, 10, fake, None) != 0          # shorter than the fixed part
+    assert lib.tpc_ec_decode(h, None, 1 << 20, 10, fake, 10, fake, None) == -1
+    assert lib.tpc_ec_destroy(h) == 0
+    assert lib.tpc_ec_destroy(None) == -1
 
 
 def test_library_is_sm100a_and_uses_no_fallback():

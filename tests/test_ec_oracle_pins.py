@@ -13,6 +13,7 @@ import numpy as np
 import pytest
 
 import ec_brute
+from datagen.ec_gen import synthetic_clusters
 from oracle import ec_oracle as eco
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "ec_examples.txt")
@@ -161,25 +162,6 @@ def test_symbol_streams_hand_evaluated():
     for s in range(13):
         assert list(st[s]) == GSTREAMS[s], s
     assert np.array_equal(ec_brute.symbol_bytes(cl, 4), st)
-
-
-def synthetic_clusters(rng, n_sectors, n_rows, n, max_pads=138, n_time=2000):
-    """sorted, unique keys; fields drawn like cluster-finder output (qtot >= qmax, offsets inside the 5x5 window)"""
-    key = np.unique(rng.integers(0, n_sectors * n_rows * max_pads * n_time, size=n))
-    cl = np.zeros(key.shape[0], dtype=eco.CLUSTER)
-    cl["time"] = key % n_time
-    cl["pad"] = (key // n_time) % max_pads
-    cl["row"] = (key // (n_time * max_pads)) % n_rows
-    cl["sector"] = key // (n_time * max_pads * n_rows)
-    m = key.shape[0]
-    cl["qmax"] = np.minimum(65535, 4 + rng.geometric(0.05, size=m))
-    cl["qtot"] = cl["qmax"].astype(np.uint32) + rng.geometric(0.01, size=m).astype(np.uint32) - 1
-    cl["flags"] = rng.choice([0, 0, 0, 1, 4, 12], size=m)
-    cl["pad_mean"] = (cl["pad"] + rng.normal(0, 0.3, size=m).clip(-1.9, 1.9)).astype(np.float32)
-    cl["time_mean"] = (cl["time"] + rng.normal(0, 0.4, size=m).clip(-1.9, 1.9)).astype(np.float32)
-    cl["sigma_pad"] = np.abs(rng.normal(0.6, 0.2, size=m)).clip(0, 1.9).astype(np.float32)
-    cl["sigma_time"] = np.abs(rng.normal(0.9, 0.3, size=m)).clip(0, 1.9).astype(np.float32)
-    return cl
 
 
 def test_symbol_streams_against_independent_symboliser():
