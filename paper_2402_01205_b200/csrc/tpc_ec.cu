@@ -2,16 +2,18 @@
 // Product code, sm_100a.  Shares nothing with oracle/tpc_ec_oracle.c: the format text in the header is the only link.
 //
 // Encoder, on the caller's stream:
-//   k_ec_symbolize   (Q) one thread per cluster: 13 symbol bytes (SoA streams in the workspace), order / range checks,
-//                    histograms (warp-aggregated shared-memory atomics, one flush per CTA)
+//   k_ec_symbolize   (Q) one thread per cluster: 13 symbol bytes (SoA streams in the workspace), order / range checks
+//   k_ec_hist        (N) counts: per-thread private byte counters in shared memory (no atomics: the streams are skewed,
+//                    and a shared-memory atomic costs 2 cycles per lane), folded every 240 symbols per thread
 //   k_ec_plane_count plane_count[] of the container: two lower_bounds per plane on the sorted cluster keys
-//   k_ec_normalize   (N) one warp per stream: 12-bit frequencies -> container table and (f | cum << 16) coding table
-//   k_ec_code<0>     (C) sizes: one warp per (stream, block), one rANS state per lane; byte counts per lane
+//   k_ec_normalize   (N) one CTA per stream: 12-bit frequencies -> container table and the coding table
+//                    (reciprocal | f, shift, bias: the coder divides by multiplying)
+//   k_ec_code        (C) one warp per (stream, block), one rANS state per lane; bytes collected in a 64-bit register and
+//                    stored 8 at a time into the lane's worst-case slot of a scratch area (L2-resident)
 //   k_ec_layout      exclusive scan of the record sizes -> directory, header, status; capacity check
-//   k_ec_code<1>     (C) again, this time storing every byte at its final place (no worst-case staging buffer: the
-//                    coder is cheap — ~50 instructions per symbol — and the payload is written exactly once)
+//   k_ec_pack        one CTA per record: lane slots -> record image in shared memory -> coalesced word stores
 // Decoder:
-//   k_ec_dec_tables  header check, table sums, slot -> symbol table (4096 bytes per stream), plane starts
+//   k_ec_dec_tables  header check, table sums, slot -> (symbol, f, slot - cum) table (16 KB per stream), plane starts
 //   k_ec_decode      one warp per (stream, block): 32 lanes decode forwards into the symbol streams
 //   k_ec_rebuild     inverse of (Q): one warp per plane, pads by a warp scan, times by a segmented warp scan
 #include <new>
@@ -32,6 +34,10 @@ static constexpr uint32_t kProbBits = 12, kProbScale = 1u << kProbBits;
 static constexpr uint32_t kL = 1u << 23;
 static constexpr uint32_t kRecFixed = kLanes * 4 + kLanes * 2;   // states + byte counts
 static constexpr uint32_t kMagic = 0x45435054u;
+// a lane codes at most 512 symbols at <= 12 bits (+ 2^-11 relative) each: <= 768 bytes; stores are whole 8-byte words
+static constexpr uint32_t kSlot = 776;
+static constexpr uint32_t kHistPerThread = 240;    // symbols per thread between two folds of the byte counters (< 256)
+static constexpr uint32_t kHistRound = 256 * kHistPerThread;
 
 struct Layout {                // byte offsets inside the container (all host-computable from n and the geometry)
     uint64_t off_counts, off_freq, off_dir, off_records;
@@ -54,10 +60,12 @@ struct Ws {
     uint8_t* sym;          // [13][stride]
     uint64_t stride;
     uint32_t* hist;        // [13][256]
-    uint32_t* ftab;        // [13][256]  f | cum << 16
+    uint2* ctab;           // [13][256]  coding table: reciprocal, f | shift << 13 | bias << 18
+    uint32_t* dtab;        // [13][4096] decoding table: symbol | (f - 1) << 8 | (slot - cum) << 20
     uint16_t* lane_nb;     // [13 * max_blocks * 32]
+    uint32_t* lane_x;      // [13 * max_blocks * 32] final states
+    uint8_t* slots;        // [13 * max_blocks * 32][kSlot] lane bytes before packing
     uint32_t* rec_size;    // [13 * max_blocks]
-    uint8_t* lut;          // [13][4096] slot -> symbol
     uint32_t* plane_start; // [planes + 1]
     uint32_t* flags;       // [4]: error bits, payload-fits flag
 };
@@ -71,57 +79,84 @@ __device__ __forceinline__ uint32_t quant(float v)
 __global__ void __launch_bounds__(256)
 k_ec_symbolize(const uint4* __restrict__ cl, uint32_t n, uint32_t n_sectors, uint32_t n_rows, Ws ws)
 {
-    __shared__ uint32_t s_hist[kStreams * 256];
-    for (uint32_t i = threadIdx.x; i < kStreams * 256; i += blockDim.x) s_hist[i] = 0u;
-    __syncthreads();
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool act = i < n;
-    uint32_t sym[kStreams];
+    if (i >= n) return;
     uint32_t err = 0u;
-    if (act) {
-        const uint4 lo = __ldg(cl + 2 * (size_t)i), hi = __ldg(cl + 2 * (size_t)i + 1);
-        const uint32_t sector = lo.x & 0xffu, row = (lo.x >> 8) & 0xffu, pad = (lo.x >> 16) & 0xffu, fl = lo.x >> 24;
-        const uint32_t time = lo.y & 0xffffu, qmax = lo.y >> 16, qtot = lo.z;
-        bool same = false;
-        uint32_t ppad = 0u, ptime = 0u;
-        if (sector >= n_sectors || row >= n_rows) err |= TPC_EC_ERR_UNSORTED;
-        if (i > 0u) {
-            const uint2 p = __ldg((const uint2*)(cl + 2 * (size_t)(i - 1)));
-            const uint32_t ps = p.x & 0xffu, pr = (p.x >> 8) & 0xffu;
-            ppad = (p.x >> 16) & 0xffu; ptime = p.y & 0xffffu;
-            const uint64_t kp = ((uint64_t)ps << 32) | ((uint64_t)pr << 24) | ((uint64_t)ppad << 16) | ptime;
-            const uint64_t kc = ((uint64_t)sector << 32) | ((uint64_t)row << 24) | ((uint64_t)pad << 16) | time;
-            if (kp >= kc) err |= TPC_EC_ERR_UNSORTED;
-            same = ps == sector && pr == row;
-        }
-        const uint32_t dpad = same ? ((pad - ppad) & 0xffu) : pad;
-        const uint32_t v = (same && pad == ppad) ? ((time - ptime) & 0xffffu) : time;
-        const uint32_t dq = (qtot - qmax) & 0xffffffu;
-        if (qtot < qmax || qtot - qmax >= (1u << 24)) err |= TPC_EC_ERR_QTOT;
-        sym[0] = dpad; sym[1] = v & 255u; sym[2] = v >> 8; sym[3] = qmax & 255u; sym[4] = qmax >> 8;
-        sym[5] = dq & 255u; sym[6] = (dq >> 8) & 255u; sym[7] = dq >> 16; sym[8] = fl;
-        // fp32, one rounding per operation (explicit intrinsics: no contraction)
-        sym[9] = quant(__fmul_rn(__fadd_rn(__fsub_rn(__uint_as_float(lo.w), (float)pad), 2.0f), 64.0f));
-        sym[10] = quant(__fmul_rn(__fadd_rn(__fsub_rn(__uint_as_float(hi.x), (float)time), 2.0f), 64.0f));
-        sym[11] = quant(__fmul_rn(__uint_as_float(hi.y), 128.0f));
-        sym[12] = quant(__fmul_rn(__uint_as_float(hi.z), 128.0f));
-#pragma unroll
-        for (uint32_t s = 0; s < kStreams; ++s) ws.sym[s * ws.stride + i] = (uint8_t)sym[s];
+    const uint4 lo = __ldg(cl + 2 * (size_t)i), hi = __ldg(cl + 2 * (size_t)i + 1);
+    const uint32_t sector = lo.x & 0xffu, row = (lo.x >> 8) & 0xffu, pad = (lo.x >> 16) & 0xffu, fl = lo.x >> 24;
+    const uint32_t time = lo.y & 0xffffu, qmax = lo.y >> 16, qtot = lo.z;
+    bool same = false;
+    uint32_t ppad = 0u, ptime = 0u;
+    if (sector >= n_sectors || row >= n_rows) err |= TPC_EC_ERR_UNSORTED;
+    if (i > 0u) {
+        const uint2 p = __ldg((const uint2*)(cl + 2 * (size_t)(i - 1)));
+        const uint32_t ps = p.x & 0xffu, pr = (p.x >> 8) & 0xffu;
+        ppad = (p.x >> 16) & 0xffu; ptime = p.y & 0xffffu;
+        const uint64_t kp = ((uint64_t)ps << 32) | ((uint64_t)pr << 24) | ((uint64_t)ppad << 16) | ptime;
+        const uint64_t kc = ((uint64_t)sector << 32) | ((uint64_t)row << 24) | ((uint64_t)pad << 16) | time;
+        if (kp >= kc) err |= TPC_EC_ERR_UNSORTED;
+        same = ps == sector && pr == row;
     }
-    // histograms: lanes with the same symbol elect a leader (the streams are skewed: plain atomics would serialise)
-    const unsigned amask = __ballot_sync(0xffffffffu, act);
-    if (act) {
-        const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t dpad = same ? ((pad - ppad) & 0xffu) : pad;
+    const uint32_t v = (same && pad == ppad) ? ((time - ptime) & 0xffffu) : time;
+    const uint32_t dq = (qtot - qmax) & 0xffffffu;
+    if (qtot < qmax || qtot - qmax >= (1u << 24)) err |= TPC_EC_ERR_QTOT;
+    uint32_t sym[kStreams];
+    sym[0] = dpad; sym[1] = v & 255u; sym[2] = v >> 8; sym[3] = qmax & 255u; sym[4] = qmax >> 8;
+    sym[5] = dq & 255u; sym[6] = (dq >> 8) & 255u; sym[7] = dq >> 16; sym[8] = fl;
+    // fp32, one rounding per operation (explicit intrinsics: no contraction)
+    sym[9] = quant(__fmul_rn(__fadd_rn(__fsub_rn(__uint_as_float(lo.w), (float)pad), 2.0f), 64.0f));
+    sym[10] = quant(__fmul_rn(__fadd_rn(__fsub_rn(__uint_as_float(hi.x), (float)time), 2.0f), 64.0f));
+    sym[11] = quant(__fmul_rn(__uint_as_float(hi.y), 128.0f));
+    sym[12] = quant(__fmul_rn(__uint_as_float(hi.z), 128.0f));
 #pragma unroll
-        for (uint32_t s = 0; s < kStreams; ++s) {
-            const unsigned peers = __match_any_sync(amask, sym[s]);
-            if ((uint32_t)(__ffs(peers) - 1) == lane) atomicAdd(&s_hist[s * 256 + sym[s]], (uint32_t)__popc(peers));
-        }
-    }
+    for (uint32_t s = 0; s < kStreams; ++s) ws.sym[s * ws.stride + i] = (uint8_t)sym[s];     // 32 bytes per warp and stream
     if (err) atomicOr(&ws.flags[0], err);
+}
+
+// (N) counts.  grid = (chunks, 13); a CTA walks `rounds` rounds of kHistRound symbols of one stream.  Thread t keeps a
+// private byte counter per symbol value: word = value * 64 + (warp >> 2) * 32 + lane, byte = warp & 3, so the 32 lanes
+// of an access hit 32 banks.  After at most 240 symbols per thread the counters are folded into the CTA's histogram.
+__global__ void __launch_bounds__(256)
+k_ec_hist(uint32_t n, uint32_t rounds, Ws ws)
+{
+    extern __shared__ __align__(16) uint8_t s_cnt[];           // 256 values x 256 threads
+    __shared__ uint32_t s_hist[256];
+    const uint32_t t = threadIdx.x, lane = t & 31u, warp = t >> 5;
+    const uint32_t s = blockIdx.y;
+    for (uint32_t k = t; k < 256u * 256u / 16u; k += 256u) ((uint4*)s_cnt)[k] = make_uint4(0u, 0u, 0u, 0u);
+    s_hist[t] = 0u;
     __syncthreads();
-    for (uint32_t k = threadIdx.x; k < kStreams * 256; k += blockDim.x)
-        if (s_hist[k]) atomicAdd(&ws.hist[k], s_hist[k]);
+    const uint8_t* src = ws.sym + s * ws.stride;               // 256-byte aligned
+    uint8_t* mine = s_cnt + 4u * ((warp >> 2) * 32u + lane) + (warp & 3u);
+    uint32_t* words = (uint32_t*)s_cnt;
+    for (uint32_t r = 0; r < rounds; ++r) {
+        const uint64_t base = ((uint64_t)blockIdx.x * rounds + r) * kHistRound;
+        if (base >= n) break;
+#pragma unroll 3
+        for (uint32_t j = 0; j < kHistPerThread / 16u; ++j) {
+            const uint64_t at = base + ((uint64_t)j * 256u + t) * 16u;
+            if (at >= n) break;
+            const uint4 v = *(const uint4*)(src + at);
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+            const uint32_t left = n - at >= 16u ? 16u : (uint32_t)(n - at);
+#pragma unroll
+            for (uint32_t k = 0; k < 16u; ++k)
+                if (k < left) ++mine[256u * ((w[k >> 2] >> (8u * (k & 3u))) & 255u)];
+        }
+        __syncthreads();
+        // fold: thread t sums the 64 words of value t (rotated start: conflict-free) and clears them
+        uint32_t sum = 0u;
+#pragma unroll 8
+        for (uint32_t j = 0; j < 64u; ++j) {
+            const uint32_t w = t * 64u + ((j + lane) & 63u);
+            sum = __dp4a(words[w], 0x01010101u, sum);
+            words[w] = 0u;
+        }
+        s_hist[t] += sum;
+        __syncthreads();
+    }
+    if (s_hist[t]) atomicAdd(&ws.hist[s * 256 + t], s_hist[t]);
 }
 
 // plane_count[p] = lower_bound(p + 1) - lower_bound(p) on the plane number of the sorted clusters
@@ -145,9 +180,10 @@ __global__ void k_ec_plane_count(const uint4* __restrict__ cl, uint32_t n, uint3
 // ---- (N) one warp per stream; lane 0 walks the 256 counts (a few microseconds; exactness over speed) -----------------
 __global__ void k_ec_normalize(uint32_t n, Ws ws, uint16_t* __restrict__ freq_out)
 {
-    __shared__ uint32_t f[256];
+    __shared__ uint32_t f[256], c[256];
     const uint32_t s = blockIdx.x;
     const uint32_t* hist = ws.hist + s * 256;
+    for (uint32_t a = threadIdx.x; a < 256; a += blockDim.x) c[a] = 0u;
     for (uint32_t a = threadIdx.x; a < 256; a += blockDim.x) {
         const uint32_t c = hist[a];
         uint32_t q = 0u;
@@ -174,29 +210,54 @@ __global__ void k_ec_normalize(uint32_t n, Ws ws, uint16_t* __restrict__ freq_ou
             D += d;
         }
         uint32_t cum = 0u;
-        for (int a = 0; a < 256; ++a) {
-            ws.ftab[s * 256 + a] = f[a] | (cum << 16);
-            cum += f[a];
-        }
+        for (int a = 0; a < 256; ++a) { c[a] = cum; cum += f[a]; }
     }
     __syncthreads();
     for (uint32_t a = threadIdx.x; a < 256; a += blockDim.x) {
         freq_out[s * 256 + a] = (uint16_t)f[a];
-        if (n == 0u) ws.ftab[s * 256 + a] = 0u;
+        // x / f for x < 2^31 as umulhi(x, rcp) >> sh with rcp = ceil(2^(31 + ceil(log2 f)) / f), sh = ceil(log2 f) - 1
+        // (exact for every x < 2^31); f == 1: rcp = 2^32 - 1 gives x - 1, made up for by a bias of M - 1
+        const uint32_t fa = f[a];
+        uint32_t rcp = 0u, sh = 0u, bias = 0u;
+        if (fa == 1u) { rcp = 0xffffffffu; sh = 0u; bias = c[a] + kProbScale - 1u; }
+        else if (fa > 1u) {
+            const uint32_t lg = 32u - (uint32_t)__clz(fa - 1u);
+            rcp = (uint32_t)((((uint64_t)1 << (31u + lg)) + fa - 1u) / fa);
+            sh = lg - 1u;
+            bias = c[a];
+        }
+        ws.ctab[s * 256 + a] = make_uint2(rcp, fa | (sh << 13) | (bias << 18));
     }
 }
 
 // ---- (C) encoder -------------------------------------------------------------------------------------------------
-// WRITE = false: byte counts only.  WRITE = true: the same walk, bytes stored at their final place.
-template <bool WRITE>
-__global__ void __launch_bounds__(256)
-k_ec_code(uint32_t n, uint32_t n_blocks, Ws ws, uint8_t* __restrict__ out, const uint64_t* __restrict__ rec_off)
+// One coding step.  tab.x = reciprocal, tab.y = f | shift << 13 | bias << 18.  At most two bytes leave the state per
+// symbol (x < 2^31, x_max >= 2^19); they enter a 64-bit shift register from the top, so that after eight pushes the
+// register holds them in emission order, lowest address first.
+__device__ __forceinline__ void code_step(uint32_t& x, uint32_t& lo, uint32_t& hi, uint32_t& cnt, uint2*& dst, const uint2 tab)
 {
-    __shared__ uint32_t s_tab[256];
+    const uint32_t f = tab.y & 0x1fffu;
+    const uint32_t x_max = f << 19;                            // (L >> 12 << 8) * f <= 2^31
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        if (x >= x_max) {
+            lo = __funnelshift_r(lo, hi, 8);
+            hi = __funnelshift_r(hi, x, 8);
+            x >>= 8;
+            if (++cnt == 8u) { *dst++ = make_uint2(lo, hi); cnt = 0u; }
+        }
+    }
+    const uint32_t q = __umulhi(x, tab.x) >> ((tab.y >> 13) & 31u);
+    x = x + (tab.y >> 18) + q * (kProbScale - f);              // = (x / f) * M + x % f + cum
+}
+
+__global__ void __launch_bounds__(256)
+k_ec_code(uint32_t n, uint32_t n_blocks, Ws ws)
+{
+    __shared__ uint2 s_tab[256];
     const uint32_t s = blockIdx.y;
-    s_tab[threadIdx.x] = ws.ftab[s * 256 + threadIdx.x];
+    s_tab[threadIdx.x] = ws.ctab[s * 256 + threadIdx.x];
     __syncthreads();
-    if (WRITE && ws.flags[1] == 0u) return;                    // the payload does not fit: nothing beyond the directory
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t b = blockIdx.x * (blockDim.x >> 5) + warp;
     if (b >= n_blocks) return;
@@ -207,42 +268,81 @@ k_ec_code(uint32_t n, uint32_t n_blocks, Ws ws, uint8_t* __restrict__ out, const
         m = (n - first + kLanes - 1) / kLanes;
         if (m > kPerLane) m = kPerLane;
     }
-    uint8_t* dst = nullptr;
-    if (WRITE) {
+    const uint8_t* src = ws.sym + s * ws.stride + first;
+    uint2* const slot = (uint2*)(ws.slots + ((size_t)e * kLanes + lane) * kSlot);
+    uint2* dst = slot;
+    uint32_t x = kL, lo = 0u, hi = 0u, cnt = 0u;
+    uint32_t k = m;
+    while (k & 7u) { --k; code_step(x, lo, hi, cnt, dst, s_tab[src[(size_t)k * kLanes]]); }
+    // groups of eight symbols; the next group's bytes are fetched before the current group's dependent chain
+    uint32_t nxt[8];
+    if (k) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) nxt[j] = src[(size_t)(k - 8u + j) * kLanes];
+    }
+    while (k) {
+        uint2 tab[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) tab[j] = s_tab[nxt[j]];
+        k -= 8u;
+        if (k) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) nxt[j] = src[(size_t)(k - 8u + j) * kLanes];
+        }
+#pragma unroll
+        for (int j = 7; j >= 0; --j) code_step(x, lo, hi, cnt, dst, tab[j]);
+    }
+    const uint32_t nbytes = (uint32_t)(dst - slot) * 8u + cnt;
+    if (cnt) {                                                 // the last cnt bytes sit at the top of the register
+        const uint64_t v = (((uint64_t)hi << 32) | lo) >> (8u * (8u - cnt));
+        *dst = make_uint2((uint32_t)v, (uint32_t)(v >> 32));
+    }
+    ws.lane_x[(size_t)e * kLanes + lane] = x;
+    ws.lane_nb[(size_t)e * kLanes + lane] = (uint16_t)nbytes;
+    const uint32_t total = __reduce_add_sync(0xffffffffu, nbytes);
+    if (lane == 0) ws.rec_size[e] = (kRecFixed + total + 3u) & ~3u;
+}
+
+// Record e: states, byte counts, the lanes' bytes back to back, zero padding to 4 — assembled in shared memory, stored
+// as whole words.
+__global__ void __launch_bounds__(256)
+k_ec_pack(Ws ws, uint8_t* __restrict__ out, const uint64_t* __restrict__ rec_off)
+{
+    __shared__ __align__(16) uint8_t s_rec[kRecFixed + kLanes * 768 + 8];
+    __shared__ uint32_t s_off[kLanes + 1];
+    if (ws.flags[1] == 0u) return;                             // the payload does not fit: nothing beyond the directory
+    const uint32_t e = blockIdx.x;
+    const uint32_t t = threadIdx.x, lane = t & 31u, warp = t >> 5;
+    if (warp == 0) {
         const uint32_t nb = ws.lane_nb[(size_t)e * kLanes + lane];
         uint32_t incl = nb;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
-            if ((int)lane >= d) incl += t;
+            const uint32_t u = __shfl_up_sync(0xffffffffu, incl, d);
+            if ((int)lane >= d) incl += u;
         }
-        uint8_t* rec = out + rec_off[e];
-        dst = rec + kRecFixed + (incl - nb);
-        ((uint16_t*)(rec + kLanes * 4))[lane] = (uint16_t)nb;
-        const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
-        if (lane < ((4u - (total & 3u)) & 3u)) rec[kRecFixed + total + lane] = 0;      // zero padding to 4
+        s_off[lane] = incl - nb;
+        if (lane == 31) s_off[32] = incl;
+        ((uint32_t*)s_rec)[lane] = ws.lane_x[(size_t)e * kLanes + lane];
+        ((uint16_t*)(s_rec + kLanes * 4))[lane] = (uint16_t)nb;
     }
-    const uint8_t* src = ws.sym + s * ws.stride + first;
-    uint32_t x = kL, nbytes = 0u;
-    for (uint32_t k = m; k-- > 0u;) {
-        const uint32_t tab = s_tab[src[(size_t)k * kLanes]];
-        const uint32_t f = tab & 0xffffu, c = tab >> 16;
-        const uint32_t x_max = f << 19;                        // (L >> 12 << 8) * f <= 2^31
-        while (x >= x_max) {
-            if (WRITE) dst[nbytes] = (uint8_t)x;
-            ++nbytes;
-            x >>= 8;
+    __syncthreads();
+    const uint32_t total = s_off[32];
+    if (t < 4u) s_rec[kRecFixed + total + t] = 0;               // padding (the bytes beyond it are not stored)
+    for (uint32_t l = warp; l < kLanes; l += 8u) {
+        const uint32_t off = kRecFixed + s_off[l], nb = s_off[l + 1] - s_off[l];
+        const uint32_t* from = (const uint32_t*)(ws.slots + ((size_t)e * kLanes + l) * kSlot);
+        for (uint32_t j = lane; 4u * j < nb; j += 32u) {
+            const uint32_t v = from[j];
+#pragma unroll
+            for (uint32_t k = 0; k < 4u; ++k)
+                if (4u * j + k < nb) s_rec[off + 4u * j + k] = (uint8_t)(v >> (8u * k));
         }
-        const uint32_t q = x / f;
-        x = (q << kProbBits) + (x - q * f) + c;
     }
-    if (WRITE) {
-        ((uint32_t*)(out + rec_off[e]))[lane] = x;
-    } else {
-        ws.lane_nb[(size_t)e * kLanes + lane] = (uint16_t)nbytes;
-        const uint32_t total = __reduce_add_sync(0xffffffffu, nbytes);
-        if (lane == 0) ws.rec_size[e] = (kRecFixed + total + 3u) & ~3u;
-    }
+    __syncthreads();
+    const uint32_t words = (kRecFixed + total + 3u) >> 2;
+    uint32_t* to = (uint32_t*)(out + rec_off[e]);
+    for (uint32_t j = t; j < words; j += 256u) to[j] = ((const uint32_t*)s_rec)[j];
 }
 
 // exclusive scan of the record sizes (one CTA; at most a few 10^4 entries) -> directory, header, status
@@ -325,8 +425,10 @@ k_ec_dec_tables(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, u
         __syncthreads();
         const bool ok = s_c[256] == kProbScale;
         const uint32_t a = threadIdx.x;
-        ws.ftab[s * 256 + a] = ok ? (s_f[a] | (s_c[a] << 16)) : 0u;
-        if (ok) for (uint32_t k = 0; k < s_f[a]; ++k) ws.lut[s * kProbScale + s_c[a] + k] = (uint8_t)a;
+        // slot -> symbol | (f - 1) << 8 | (slot - cum) << 20; a table that does not sum to 4096 decodes as "symbol 0,
+        // f = 1" everywhere (harmless: the error bit is already set)
+        if (ok) for (uint32_t k = 0; k < s_f[a]; ++k) ws.dtab[s * kProbScale + s_c[a] + k] = a | ((s_f[a] - 1u) << 8) | (k << 20);
+        else for (uint32_t k = a; k < kProbScale; k += 256u) ws.dtab[s * kProbScale + k] = 0u;
         return;
     }
     // header
@@ -372,12 +474,10 @@ k_ec_dec_tables(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, u
 __global__ void __launch_bounds__(256)
 k_ec_decode(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, Layout lay, Ws ws)
 {
-    __shared__ uint32_t s_tab[256];
-    __shared__ __align__(16) uint8_t s_lut[kProbScale];
+    __shared__ __align__(16) uint32_t s_tab[kProbScale];
     const uint32_t s = blockIdx.y;
-    s_tab[threadIdx.x] = ws.ftab[s * 256 + threadIdx.x];
-    for (uint32_t k = threadIdx.x; k < kProbScale / 16; k += blockDim.x)
-        ((uint4*)s_lut)[k] = ((const uint4*)(ws.lut + s * kProbScale))[k];
+    for (uint32_t k = threadIdx.x; k < kProbScale / 4; k += blockDim.x)
+        ((uint4*)s_tab)[k] = ((const uint4*)(ws.dtab + s * kProbScale))[k];
     __syncthreads();
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t b = blockIdx.x * (blockDim.x >> 5) + warp;
@@ -399,8 +499,12 @@ k_ec_decode(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, Layou
     }
     const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
     if ((uint64_t)kRecFixed + total > r1 - r0) { if (lane == 0) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER); return; }
-    const uint8_t* bytes = rec + kRecFixed + (incl - nb);
-    uint32_t ptr = nb;
+    // The lane's bytes are consumed from the last one down.  They are fetched as aligned 32-bit words (in is 16-byte
+    // aligned and in_bytes a multiple of 4, so a word never leaves the buffer); `have` counts the bytes of `buf` (kept
+    // at its top) that belong to the lane and have not been consumed.
+    const uint64_t start = r0 + kRecFixed + (incl - nb);        // offset of the lane's first byte
+    uint64_t end = start + nb;                                  // offset one past the next byte to consume
+    uint32_t ptr = nb, buf = 0u, have = 0u;
     const uint32_t first = b * kBlock + lane;
     uint32_t m = 0u;
     if (first < n) {
@@ -411,13 +515,21 @@ k_ec_decode(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, Layou
     bool fail = false;
     for (uint32_t k = 0; k < m; ++k) {
         const uint32_t slot = x & (kProbScale - 1u);
-        const uint32_t a = s_lut[slot];
-        const uint32_t tab = s_tab[a];
-        dst[(size_t)k * kLanes] = (uint8_t)a;
-        x = (tab & 0xffffu) * (x >> kProbBits) + slot - (tab >> 16);
+        const uint32_t tab = s_tab[slot];
+        dst[(size_t)k * kLanes] = (uint8_t)tab;
+        x = (((tab >> 8) & 0xfffu) + 1u) * (x >> kProbBits) + (tab >> 20);
         while (x < kL) {
             if (ptr == 0u) { fail = true; x = kL; break; }
-            x = (x << 8) | bytes[--ptr];
+            if (have == 0u) {
+                const uint64_t w = (end - 1u) & ~(uint64_t)3;
+                const uint32_t valid = (uint32_t)(end - w);     // bytes of the word below `end`: 1..4
+                buf = __ldg((const uint32_t*)(in + w)) << (8u * (4u - valid));
+                have = valid < ptr ? valid : ptr;
+                end -= have;
+            }
+            x = (x << 8) | (buf >> 24);
+            buf <<= 8;
+            --have; --ptr;
         }
     }
     if (x != kL || ptr != 0u) fail = true;
@@ -492,6 +604,7 @@ struct tpc_ec {
     uint32_t n_sectors, n_rows;
     uint64_t max_clusters;
     Ws ws;
+    uint32_t hist_ctas;    // CTAs of k_ec_hist that are resident at once
     int last_launches;
 };
 
@@ -501,15 +614,17 @@ static size_t carve(uint32_t n_sectors, uint32_t n_rows, uint64_t max_clusters, 
 {
     size_t off = 0;
     auto take = [&](size_t bytes) { char* p = base ? base + off : nullptr; off += align256(bytes ? bytes : 1); return p; };
-    const uint64_t max_blocks = (max_clusters + kBlock - 1) / kBlock + 1;
+    const uint64_t max_blocks = (max_clusters + kBlock - 1) / kBlock;
     Ws w;
     w.stride = align256(max_clusters ? max_clusters : 1);
     w.sym = (uint8_t*)take((size_t)kStreams * w.stride);
     w.hist = (uint32_t*)take(kStreams * 256 * 4);
-    w.ftab = (uint32_t*)take(kStreams * 256 * 4);
+    w.ctab = (uint2*)take(kStreams * 256 * 8);
+    w.dtab = (uint32_t*)take((size_t)kStreams * kProbScale * 4);
     w.lane_nb = (uint16_t*)take((size_t)kStreams * max_blocks * kLanes * 2);
+    w.lane_x = (uint32_t*)take((size_t)kStreams * max_blocks * kLanes * 4);
+    w.slots = (uint8_t*)take((size_t)kStreams * max_blocks * kLanes * kSlot);
     w.rec_size = (uint32_t*)take((size_t)kStreams * max_blocks * 4);
-    w.lut = (uint8_t*)take((size_t)kStreams * kProbScale);
     w.plane_start = (uint32_t*)take(((size_t)n_sectors * n_rows + 1) * 4);
     w.flags = (uint32_t*)take(16);
     if (ws) *ws = w;
@@ -547,6 +662,16 @@ extern "C" int tpc_ec_create(tpc_ec** h, uint32_t n_sectors, uint32_t n_rows, ui
     if (!e) return TPC_CF_E_NOMEM;
     e->n_sectors = n_sectors; e->n_rows = n_rows; e->max_clusters = max_clusters; e->last_launches = 0;
     carve(n_sectors, n_rows, max_clusters, (char*)workspace, &e->ws);
+    // k_ec_hist needs 64 KB of dynamic shared memory; without a device (host-only tests) the call fails harmlessly
+    e->hist_ctas = 3 * 148;
+    if (cudaFuncSetAttribute(k_ec_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536) == cudaSuccess) {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+            e->hist_ctas = 3u * (uint32_t)sms;
+    } else {
+        cudaGetLastError();
+    }
     *h = e;
     return TPC_CF_OK;
 }
@@ -567,21 +692,25 @@ extern "C" int tpc_ec_encode(tpc_ec* h, const tpc_cluster* clusters, uint64_t n,
     cudaMemsetAsync(ws.flags, 0, 16, st);
     if (n32) {
         k_ec_symbolize<<<(n32 + 255) / 256, 256, 0, st>>>((const uint4*)clusters, n32, h->n_sectors, h->n_rows, ws);
-        ++launches;
+        // rounds of kHistRound symbols, shared out so that the grid is about one wave of 3 CTAs per SM
+        const uint32_t total_rounds = (n32 + kHistRound - 1) / kHistRound;
+        const uint32_t per = (kStreams * total_rounds + h->hist_ctas - 1) / h->hist_ctas;
+        const dim3 hgrid((total_rounds + per - 1) / per, kStreams);
+        k_ec_hist<<<hgrid, 256, 65536, st>>>(n32, per, ws);
+        launches += 2;
     }
     k_ec_plane_count<<<(lay.n_planes + 127) / 128, 128, 0, st>>>((const uint4*)clusters, n32, h->n_rows, lay.n_planes,
                                                                   (uint32_t*)(out + lay.off_counts));
     k_ec_normalize<<<kStreams, 256, 0, st>>>(n32, ws, (uint16_t*)(out + lay.off_freq));
     launches += 2;
-    const dim3 grid((lay.n_blocks + 7) / 8, kStreams);
     if (lay.n_blocks) {
-        k_ec_code<false><<<grid, 256, 0, st>>>(n32, lay.n_blocks, ws, nullptr, nullptr);
+        k_ec_code<<<dim3((lay.n_blocks + 7) / 8, kStreams), 256, 0, st>>>(n32, lay.n_blocks, ws);
         ++launches;
     }
     k_ec_layout<<<1, 1024, 0, st>>>(n32, h->n_sectors, h->n_rows, lay, ws, out, out_capacity, status);
     ++launches;
     if (lay.n_blocks) {
-        k_ec_code<true><<<grid, 256, 0, st>>>(n32, lay.n_blocks, ws, out, (const uint64_t*)(out + lay.off_dir));
+        k_ec_pack<<<kStreams * lay.n_blocks, 256, 0, st>>>(ws, out, (const uint64_t*)(out + lay.off_dir));
         ++launches;
     }
     h->last_launches = launches;
@@ -595,7 +724,7 @@ extern "C" int tpc_ec_decode(tpc_ec* h, const uint8_t* in, uint64_t in_bytes, ui
     if (n > h->max_clusters) return TPC_CF_E_CAPACITY;
     if (((uintptr_t)in & 15u) != 0 || ((uintptr_t)clusters & 15u) != 0) return TPC_CF_E_WORKSPACE;
     const Layout lay = layout_of(h->n_sectors, h->n_rows, n);
-    if (in_bytes < lay.off_records) return TPC_CF_E_CAPACITY;     // not even the fixed part
+    if (in_bytes < lay.off_records || (in_bytes & 3u) != 0) return TPC_CF_E_CAPACITY;   // not even the fixed part / not whole words
     cudaStream_t st = (cudaStream_t)stream;
     const Ws& ws = h->ws;
     const uint32_t n32 = (uint32_t)n;
