@@ -2,15 +2,15 @@
 // Product code, sm_100a.  Shares nothing with oracle/tpc_ec_oracle.c: the format text in the header is the only link.
 //
 // Encoder, on the caller's stream:
-//   k_ec_symbolize   (Q) one thread per cluster: 13 symbol bytes (SoA streams in the workspace), order / range checks
+//   k_ec_symbolize   (Q) one thread per cluster: 13 symbol bytes (SoA streams in the workspace), order / range checks;
+//                    the cluster that opens a plane records where the plane starts
 //   k_ec_hist        (N) counts: per-thread private byte counters in shared memory (no atomics: the streams are skewed,
 //                    and a shared-memory atomic costs 2 cycles per lane), folded every 240 symbols per thread
-//   k_ec_plane_count plane_count[] of the container: two lower_bounds per plane on the sorted cluster keys
 //   k_ec_normalize   (N) one CTA per stream: 12-bit frequencies -> container table and the coding table
 //                    (reciprocal | f, shift, bias: the coder divides by multiplying)
 //   k_ec_code        (C) one warp per (stream, block), one rANS state per lane; bytes collected in a 64-bit register and
 //                    stored 8 at a time into the lane's worst-case slot of a scratch area (L2-resident)
-//   k_ec_layout      exclusive scan of the record sizes -> directory, header, status; capacity check
+//   k_ec_layout      exclusive scan of the record sizes -> directory; plane counts, header, status; capacity check
 //   k_ec_pack        one CTA per record: lane slots -> record image in shared memory -> coalesced word stores
 // Decoder:
 //   k_ec_dec_tables  header check, table sums, slot -> (symbol, f, slot - cum) table (16 KB per stream), plane starts
@@ -88,6 +88,11 @@ k_ec_symbolize(const uint4* __restrict__ cl, uint32_t n, uint32_t n_sectors, uin
     bool same = false;
     uint32_t ppad = 0u, ptime = 0u;
     if (sector >= n_sectors || row >= n_rows) err |= TPC_EC_ERR_UNSORTED;
+    // plane_start[q] = index of the first cluster of a plane >= q: written by the cluster that opens plane p for every
+    // q in (plane of its predecessor, p]; the last cluster closes the planes behind its own
+    const uint32_t n_planes = n_sectors * n_rows;
+    const uint32_t plane = sector * n_rows + row;
+    uint32_t q_lo = 0u, q_hi = plane;                          // planes [q_lo, q_hi] start at i
     if (i > 0u) {
         const uint2 p = __ldg((const uint2*)(cl + 2 * (size_t)(i - 1)));
         const uint32_t ps = p.x & 0xffu, pr = (p.x >> 8) & 0xffu;
@@ -96,6 +101,11 @@ k_ec_symbolize(const uint4* __restrict__ cl, uint32_t n, uint32_t n_sectors, uin
         const uint64_t kc = ((uint64_t)sector << 32) | ((uint64_t)row << 24) | ((uint64_t)pad << 16) | time;
         if (kp >= kc) err |= TPC_EC_ERR_UNSORTED;
         same = ps == sector && pr == row;
+        q_lo = ps * n_rows + pr + 1u;
+    }
+    if (err == 0u) {                                           // (an unsorted or out-of-range stream: content unspecified)
+        for (uint32_t q = q_lo; q <= q_hi; ++q) ws.plane_start[q] = i;
+        if (i == n - 1u) for (uint32_t q = plane + 1u; q <= n_planes; ++q) ws.plane_start[q] = n;
     }
     const uint32_t dpad = same ? ((pad - ppad) & 0xffu) : pad;
     const uint32_t v = (same && pad == ppad) ? ((time - ptime) & 0xffffu) : time;
@@ -139,10 +149,22 @@ k_ec_hist(uint32_t n, uint32_t rounds, Ws ws)
             if (at >= n) break;
             const uint4 v = *(const uint4*)(src + at);
             const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-            const uint32_t left = n - at >= 16u ? 16u : (uint32_t)(n - at);
+            if (n - at >= 16u) {
+                // two symbols at a time: both counters are read before either is written (two loads in flight); equal
+                // symbols both write "old + 2"
 #pragma unroll
-            for (uint32_t k = 0; k < 16u; ++k)
-                if (k < left) ++mine[256u * ((w[k >> 2] >> (8u * (k & 3u))) & 255u)];
+                for (uint32_t k = 0; k < 16u; k += 2u) {
+                    uint8_t* pa = mine + 256u * ((w[k >> 2] >> (8u * (k & 3u))) & 255u);
+                    uint8_t* pb = mine + 256u * ((w[k >> 2] >> (8u * (k & 3u) + 8u)) & 255u);
+                    const uint32_t ca = *pa, cb = *pb;
+                    const uint32_t both = pa == pb ? 1u : 0u;
+                    *pa = (uint8_t)(ca + 1u + both);
+                    *pb = (uint8_t)(cb + 1u + both);
+                }
+            } else {
+                const uint32_t left = (uint32_t)(n - at);
+                for (uint32_t k = 0; k < left; ++k) ++mine[256u * src[at + k]];
+            }
         }
         __syncthreads();
         // fold: thread t sums the 64 words of value t (rotated start: conflict-free) and clears them
@@ -159,93 +181,104 @@ k_ec_hist(uint32_t n, uint32_t rounds, Ws ws)
     if (s_hist[t]) atomicAdd(&ws.hist[s * 256 + t], s_hist[t]);
 }
 
-// plane_count[p] = lower_bound(p + 1) - lower_bound(p) on the plane number of the sorted clusters
-__global__ void k_ec_plane_count(const uint4* __restrict__ cl, uint32_t n, uint32_t n_rows, uint32_t n_planes,
-                                 uint32_t* __restrict__ counts)
+// ---- (N) one warp per stream; lane l owns the symbols 8l .. 8l + 7 ---------------------------------------------------
+// first lane-symbol (lowest symbol) at which `v` is largest over the warp's 256 values
+__device__ __forceinline__ uint32_t warp_argmax(const uint32_t (&v)[8], uint32_t lane)
 {
-    const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n_planes) return;
-    auto lb = [&](uint32_t plane) {
-        uint32_t lo = 0, hi = n;
-        while (lo < hi) {
-            const uint32_t mid = lo + ((hi - lo) >> 1);
-            const uint32_t w = __ldg((const uint32_t*)(cl + 2 * (size_t)mid));
-            if ((w & 0xffu) * n_rows + ((w >> 8) & 0xffu) < plane) lo = mid + 1; else hi = mid;
-        }
-        return lo;
-    };
-    counts[p] = lb(p + 1) - lb(p);
+    uint32_t best = v[0], at = lane * 8u;
+#pragma unroll
+    for (uint32_t j = 1; j < 8u; ++j) if (v[j] > best) { best = v[j]; at = lane * 8u + j; }
+    const uint32_t top = __reduce_max_sync(0xffffffffu, best);
+    return __reduce_min_sync(0xffffffffu, best == top ? at : 0xffffffffu);
 }
 
-// ---- (N) one warp per stream; lane 0 walks the 256 counts (a few microseconds; exactness over speed) -----------------
-__global__ void k_ec_normalize(uint32_t n, Ws ws, uint16_t* __restrict__ freq_out)
+__global__ void __launch_bounds__(32)
+k_ec_normalize(uint32_t n, Ws ws, uint16_t* __restrict__ freq_out)
 {
-    __shared__ uint32_t f[256], c[256];
-    const uint32_t s = blockIdx.x;
-    const uint32_t* hist = ws.hist + s * 256;
-    for (uint32_t a = threadIdx.x; a < 256; a += blockDim.x) c[a] = 0u;
-    for (uint32_t a = threadIdx.x; a < 256; a += blockDim.x) {
-        const uint32_t c = hist[a];
+    const uint32_t s = blockIdx.x, lane = threadIdx.x;
+    uint32_t c[8], f[8];
+    uint32_t sum = 0u;
+#pragma unroll
+    for (uint32_t j = 0; j < 8u; ++j) {
+        c[j] = ws.hist[s * 256 + lane * 8u + j];
         uint32_t q = 0u;
-        if (n != 0u && c != 0u) {
-            q = (uint32_t)(((uint64_t)c * kProbScale) / n);
+        if (n != 0u && c[j] != 0u) {
+            q = (uint32_t)(((uint64_t)c[j] * kProbScale) / n);
             if (q < 1u) q = 1u;
         }
-        f[a] = q;
+        f[j] = q;
+        sum += q;
     }
-    __syncthreads();
-    if (threadIdx.x == 0 && n != 0u) {
-        long long D = kProbScale;
-        for (int a = 0; a < 256; ++a) D -= f[a];
-        if (D > 0) {
-            int b = 0;
-            for (int a = 1; a < 256; ++a) if (hist[a] > hist[b]) b = a;
-            f[b] += (uint32_t)D;
+    sum = __reduce_add_sync(0xffffffffu, sum);
+    if (n != 0u) {
+        int D = (int)kProbScale - (int)sum;                    // |D| <= 256 + 4096
+        if (D > 0) {                                           // surplus to the symbol with the largest count
+            const uint32_t a = warp_argmax(c, lane);
+#pragma unroll
+            for (uint32_t j = 0; j < 8u; ++j) if (lane * 8u + j == a) f[j] += (uint32_t)D;
         }
-        while (D < 0) {
-            int b = 0;
-            for (int a = 1; a < 256; ++a) if (f[a] > f[b]) b = a;
-            const long long d = -D < (long long)f[b] - 1 ? -D : (long long)f[b] - 1;
-            f[b] -= (uint32_t)d;
+        while (D < 0) {                                        // deficit from the symbol with the largest f, down to 1
+            const uint32_t a = warp_argmax(f, lane);
+            uint32_t fa = 0u;
+#pragma unroll
+            for (uint32_t j = 0; j < 8u; ++j) if (lane * 8u + j == a) fa = f[j];
+            fa = __shfl_sync(0xffffffffu, fa, a >> 3);
+            const int d = -D < (int)fa - 1 ? -D : (int)fa - 1;
+#pragma unroll
+            for (uint32_t j = 0; j < 8u; ++j) if (lane * 8u + j == a) f[j] -= (uint32_t)d;
             D += d;
         }
-        uint32_t cum = 0u;
-        for (int a = 0; a < 256; ++a) { c[a] = cum; cum += f[a]; }
     }
-    __syncthreads();
-    for (uint32_t a = threadIdx.x; a < 256; a += blockDim.x) {
-        freq_out[s * 256 + a] = (uint16_t)f[a];
+    uint32_t mine = 0u;
+#pragma unroll
+    for (uint32_t j = 0; j < 8u; ++j) mine += f[j];
+    uint32_t incl = mine;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, incl, d);
+        if ((int)lane >= d) incl += u;
+    }
+    uint32_t cum = incl - mine;
+#pragma unroll
+    for (uint32_t j = 0; j < 8u; ++j) {
+        const uint32_t a = lane * 8u + j;
+        freq_out[s * 256 + a] = (uint16_t)f[j];
         // x / f for x < 2^31 as umulhi(x, rcp) >> sh with rcp = ceil(2^(31 + ceil(log2 f)) / f), sh = ceil(log2 f) - 1
         // (exact for every x < 2^31); f == 1: rcp = 2^32 - 1 gives x - 1, made up for by a bias of M - 1
-        const uint32_t fa = f[a];
+        const uint32_t fa = f[j];
         uint32_t rcp = 0u, sh = 0u, bias = 0u;
-        if (fa == 1u) { rcp = 0xffffffffu; sh = 0u; bias = c[a] + kProbScale - 1u; }
+        if (fa == 1u) { rcp = 0xffffffffu; sh = 0u; bias = cum + kProbScale - 1u; }
         else if (fa > 1u) {
             const uint32_t lg = 32u - (uint32_t)__clz(fa - 1u);
             rcp = (uint32_t)((((uint64_t)1 << (31u + lg)) + fa - 1u) / fa);
             sh = lg - 1u;
-            bias = c[a];
+            bias = cum;
         }
         ws.ctab[s * 256 + a] = make_uint2(rcp, fa | (sh << 13) | (bias << 18));
+        cum += fa;
     }
 }
 
 // ---- (C) encoder -------------------------------------------------------------------------------------------------
-// One coding step.  tab.x = reciprocal, tab.y = f | shift << 13 | bias << 18.  At most two bytes leave the state per
-// symbol (x < 2^31, x_max >= 2^19); they enter a 64-bit shift register from the top, so that after eight pushes the
-// register holds them in emission order, lowest address first.
-__device__ __forceinline__ void code_step(uint32_t& x, uint32_t& lo, uint32_t& hi, uint32_t& cnt, uint2*& dst, const uint2 tab)
+// One coding step.  tab.x = reciprocal, tab.y = f | shift << 13 | bias << 18.  Zero, one or two bytes leave the state
+// per symbol (x < 2^31, x_max >= 2^19), without a branch: they enter a 96-bit shift register (r0 lowest) from the top;
+// `bits` of it are valid.  As soon as 64 bits are there, the oldest eight bytes are stored as one word.
+struct Emit { uint32_t r0, r1, r2, bits, words; };
+
+__device__ __forceinline__ void code_step(uint32_t& x, Emit& em, uint2* slot, const uint2 tab)
 {
     const uint32_t f = tab.y & 0x1fffu;
     const uint32_t x_max = f << 19;                            // (L >> 12 << 8) * f <= 2^31
-#pragma unroll
-    for (int r = 0; r < 2; ++r) {
-        if (x >= x_max) {
-            lo = __funnelshift_r(lo, hi, 8);
-            hi = __funnelshift_r(hi, x, 8);
-            x >>= 8;
-            if (++cnt == 8u) { *dst++ = make_uint2(lo, hi); cnt = 0u; }
-        }
+    const uint32_t sh = (x >> 8) >= x_max ? 16u : (x >= x_max ? 8u : 0u);
+    em.r0 = __funnelshift_r(em.r0, em.r1, sh);
+    em.r1 = __funnelshift_r(em.r1, em.r2, sh);
+    em.r2 = __funnelshift_r(em.r2, x, sh);
+    x >>= sh;
+    em.bits += sh;
+    if (em.bits >= 64u) {                                      // 64 or 72 valid bits: the oldest 64 start at bit 96 - bits
+        const uint32_t off = 96u - em.bits;
+        slot[em.words++] = make_uint2(__funnelshift_rc(em.r0, em.r1, off), __funnelshift_rc(em.r1, em.r2, off));
+        em.bits -= 64u;
     }
     const uint32_t q = __umulhi(x, tab.x) >> ((tab.y >> 13) & 31u);
     x = x + (tab.y >> 18) + q * (kProbScale - f);              // = (x / f) * M + x % f + cum
@@ -270,10 +303,10 @@ k_ec_code(uint32_t n, uint32_t n_blocks, Ws ws)
     }
     const uint8_t* src = ws.sym + s * ws.stride + first;
     uint2* const slot = (uint2*)(ws.slots + ((size_t)e * kLanes + lane) * kSlot);
-    uint2* dst = slot;
-    uint32_t x = kL, lo = 0u, hi = 0u, cnt = 0u;
+    Emit em = {0u, 0u, 0u, 0u, 0u};
+    uint32_t x = kL;
     uint32_t k = m;
-    while (k & 7u) { --k; code_step(x, lo, hi, cnt, dst, s_tab[src[(size_t)k * kLanes]]); }
+    while (k & 7u) { --k; code_step(x, em, slot, s_tab[src[(size_t)k * kLanes]]); }
     // groups of eight symbols; the next group's bytes are fetched before the current group's dependent chain
     uint32_t nxt[8];
     if (k) {
@@ -290,12 +323,12 @@ k_ec_code(uint32_t n, uint32_t n_blocks, Ws ws)
             for (int j = 0; j < 8; ++j) nxt[j] = src[(size_t)(k - 8u + j) * kLanes];
         }
 #pragma unroll
-        for (int j = 7; j >= 0; --j) code_step(x, lo, hi, cnt, dst, tab[j]);
+        for (int j = 7; j >= 0; --j) code_step(x, em, slot, tab[j]);
     }
-    const uint32_t nbytes = (uint32_t)(dst - slot) * 8u + cnt;
-    if (cnt) {                                                 // the last cnt bytes sit at the top of the register
-        const uint64_t v = (((uint64_t)hi << 32) | lo) >> (8u * (8u - cnt));
-        *dst = make_uint2((uint32_t)v, (uint32_t)(v >> 32));
+    const uint32_t nbytes = em.words * 8u + (em.bits >> 3);
+    if (em.bits) {                                             // the last bits / 8 < 8 bytes sit at the top of r2:r1
+        const uint64_t v = (((uint64_t)em.r2 << 32) | em.r1) >> (64u - em.bits);
+        slot[em.words] = make_uint2((uint32_t)v, (uint32_t)(v >> 32));
     }
     ws.lane_x[(size_t)e * kLanes + lane] = x;
     ws.lane_nb[(size_t)e * kLanes + lane] = (uint16_t)nbytes;
@@ -398,6 +431,9 @@ k_ec_layout(uint32_t n, uint32_t n_sectors, uint32_t n_rows, Layout lay, Ws ws, 
         status->error = ws.flags[0] | (fits ? 0u : TPC_EC_ERR_CAPACITY);
         status->rsv = 0u;
     }
+    uint32_t* counts = (uint32_t*)(out + lay.off_counts);
+    for (uint32_t p = threadIdx.x; p < lay.n_planes; p += 1024u)
+        counts[p] = n ? ws.plane_start[p + 1] - ws.plane_start[p] : 0u;
     // zero padding between the tables and the directory
     for (uint64_t a = lay.off_freq + 2ull * 256 * kStreams + threadIdx.x; a < lay.off_dir; a += 1024u) out[a] = 0;
 }
@@ -416,19 +452,39 @@ k_ec_dec_tables(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, u
         const uint16_t* freq = (const uint16_t*)(in + lay.off_freq) + s * 256;
         s_f[threadIdx.x] = freq[threadIdx.x];
         __syncthreads();
-        if (threadIdx.x == 0) {
-            uint32_t cum = 0u;
-            for (int a = 0; a < 256; ++a) { s_c[a] = cum; cum += s_f[a]; }
-            s_c[256] = cum;
-            if (n != 0u && cum != kProbScale) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER);
+        if (threadIdx.x < 32u) {                               // exclusive prefix sums: lane l owns 8 symbols
+            const uint32_t lane = threadIdx.x;
+            uint32_t mine = 0u;
+#pragma unroll
+            for (uint32_t j = 0; j < 8u; ++j) mine += s_f[lane * 8u + j];
+            uint32_t incl = mine;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, incl, d);
+                if ((int)lane >= d) incl += u;
+            }
+            uint32_t cum = incl - mine;
+#pragma unroll
+            for (uint32_t j = 0; j < 8u; ++j) { s_c[lane * 8u + j] = cum; cum += s_f[lane * 8u + j]; }
+            if (lane == 31u) {
+                s_c[256] = cum;
+                if (n != 0u && cum != kProbScale) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER);
+            }
         }
         __syncthreads();
         const bool ok = s_c[256] == kProbScale;
-        const uint32_t a = threadIdx.x;
-        // slot -> symbol | (f - 1) << 8 | (slot - cum) << 20; a table that does not sum to 4096 decodes as "symbol 0,
-        // f = 1" everywhere (harmless: the error bit is already set)
-        if (ok) for (uint32_t k = 0; k < s_f[a]; ++k) ws.dtab[s * kProbScale + s_c[a] + k] = a | ((s_f[a] - 1u) << 8) | (k << 20);
-        else for (uint32_t k = a; k < kProbScale; k += 256u) ws.dtab[s * kProbScale + k] = 0u;
+        // slot -> symbol | (f - 1) << 8 | (slot - cum) << 20, the symbol found by bisection on the prefix sums; a table
+        // that does not sum to 4096 decodes as "symbol 0, f = 1" everywhere (harmless: the error bit is already set)
+        for (uint32_t slot = threadIdx.x; slot < kProbScale; slot += 256u) {
+            uint32_t v = 0u;
+            if (ok) {
+                uint32_t a = 0u;                               // largest a with s_c[a] <= slot and f[a] > 0: the last one
+#pragma unroll
+                for (uint32_t step = 128u; step > 0u; step >>= 1) if (s_c[a + step] <= slot) a += step;
+                v = a | ((s_f[a] - 1u) << 8) | ((slot - s_c[a]) << 20);
+            }
+            ws.dtab[s * kProbScale + slot] = v;
+        }
         return;
     }
     // header
@@ -499,12 +555,18 @@ k_ec_decode(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, Layou
     }
     const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
     if ((uint64_t)kRecFixed + total > r1 - r0) { if (lane == 0) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER); return; }
-    // The lane's bytes are consumed from the last one down.  They are fetched as aligned 32-bit words (in is 16-byte
-    // aligned and in_bytes a multiple of 4, so a word never leaves the buffer); `have` counts the bytes of `buf` (kept
-    // at its top) that belong to the lane and have not been consumed.
-    const uint64_t start = r0 + kRecFixed + (incl - nb);        // offset of the lane's first byte
-    uint64_t end = start + nb;                                  // offset one past the next byte to consume
-    uint32_t ptr = nb, buf = 0u, have = 0u;
+    // The lane's bytes are consumed from the last one down, through a 64-bit register that keeps the next bytes at its
+    // top (`have` of them).  They are fetched as aligned 32-bit words, one word ahead of their use (in is 16-byte
+    // aligned and in_bytes a multiple of 4, so a word never leaves the buffer; at most 2 bytes per symbol are consumed,
+    // so even a malformed lane stays within 1 KB below its end, inside the fixed part).  A well-formed lane consumes
+    // exactly its nb bytes — whatever lies below them in the register is never used — and ends at x == L.
+    const uint64_t end = r0 + kRecFixed + incl;                 // offset one past the lane's last byte
+    const uint32_t* wp = (const uint32_t*)(in + ((end - 1u) & ~(uint64_t)3));      // word holding that byte
+    const uint32_t valid = (uint32_t)(end - ((end - 1u) & ~(uint64_t)3));           // its bytes below `end`: 1..4
+    uint32_t b_hi = __ldg(wp) << (8u * (4u - valid));
+    uint32_t b_lo = 0u;
+    uint32_t have = valid;
+    uint32_t ahead = __ldg(--wp);
     const uint32_t first = b * kBlock + lane;
     uint32_t m = 0u;
     if (first < n) {
@@ -512,28 +574,27 @@ k_ec_decode(const uint8_t* __restrict__ in, uint64_t in_bytes, uint32_t n, Layou
         if (m > kPerLane) m = kPerLane;
     }
     uint8_t* dst = ws.sym + s * ws.stride + first;
-    bool fail = false;
+    uint32_t used = 0u;
     for (uint32_t k = 0; k < m; ++k) {
+        if (have <= 4u) {                                       // room for a word: it goes right below the valid bytes
+            const uint64_t w = (uint64_t)ahead << (32u - 8u * have);
+            b_hi |= (uint32_t)(w >> 32);
+            b_lo = (uint32_t)w;
+            have += 4u;
+            ahead = __ldg(--wp);
+        }
         const uint32_t slot = x & (kProbScale - 1u);
         const uint32_t tab = s_tab[slot];
         dst[(size_t)k * kLanes] = (uint8_t)tab;
         x = (((tab >> 8) & 0xfffu) + 1u) * (x >> kProbBits) + (tab >> 20);
-        while (x < kL) {
-            if (ptr == 0u) { fail = true; x = kL; break; }
-            if (have == 0u) {
-                const uint64_t w = (end - 1u) & ~(uint64_t)3;
-                const uint32_t valid = (uint32_t)(end - w);     // bytes of the word below `end`: 1..4
-                buf = __ldg((const uint32_t*)(in + w)) << (8u * (4u - valid));
-                have = valid < ptr ? valid : ptr;
-                end -= have;
-            }
-            x = (x << 8) | (buf >> 24);
-            buf <<= 8;
-            --have; --ptr;
-        }
+        const uint32_t sh = x < (kL >> 8) ? 16u : (x < kL ? 8u : 0u);          // bytes needed to reach x >= L
+        x = __funnelshift_l(b_hi, x, sh);                       // (x << sh) | top sh bits of the register
+        b_hi = __funnelshift_l(b_lo, b_hi, sh);
+        b_lo <<= sh;
+        have -= sh >> 3;
+        used += sh >> 3;
     }
-    if (x != kL || ptr != 0u) fail = true;
-    if (fail) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER);
+    if (x != kL || used != nb) atomicOr(&ws.flags[0], TPC_EC_ERR_CONTAINER);
 }
 
 // inverse of (Q): one warp per plane
@@ -699,10 +760,8 @@ extern "C" int tpc_ec_encode(tpc_ec* h, const tpc_cluster* clusters, uint64_t n,
         k_ec_hist<<<hgrid, 256, 65536, st>>>(n32, per, ws);
         launches += 2;
     }
-    k_ec_plane_count<<<(lay.n_planes + 127) / 128, 128, 0, st>>>((const uint4*)clusters, n32, h->n_rows, lay.n_planes,
-                                                                  (uint32_t*)(out + lay.off_counts));
-    k_ec_normalize<<<kStreams, 256, 0, st>>>(n32, ws, (uint16_t*)(out + lay.off_freq));
-    launches += 2;
+    k_ec_normalize<<<kStreams, 32, 0, st>>>(n32, ws, (uint16_t*)(out + lay.off_freq));
+    ++launches;
     if (lay.n_blocks) {
         k_ec_code<<<dim3((lay.n_blocks + 7) / 8, kStreams), 256, 0, st>>>(n32, lay.n_blocks, ws);
         ++launches;
