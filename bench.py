@@ -172,6 +172,126 @@ def run_reference(args):
     return 0
 
 
+def run_ec(args):
+    """--stage ec: the entropy coder (include/tpc_ec.h) on the cluster stream of one frame of the chosen config, as
+    the chain of PAPER.md:57 has it: the cluster finder's output is coded on the device without leaving it.  One GPU.
+    A step = one tpc_ec_encode (all its kernels); the decoder is timed the same way and reported beside it."""
+    import torch
+    from datagen import gen
+    import paper_2402_01205_b200 as cf
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    cfg = gen.CONFIGS[args.config]
+    geom = gen.geometry(args.config)
+    digits = gen.generate(args.config)
+    nd = int(digits.shape[0])
+    finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=nd, max_clusters=nd // 10 + 1024, device=dev)
+    d = cf.to_device(digits)
+    finder.run(d, nd, flags=cf.DIGITS_SORTED)
+    cl_host, st = finder.result()
+    n = st["n_clusters"]
+    clusters = finder.clusters[:n * 32].clone()
+    del d
+    finder.close()
+    del finder
+    torch.cuda.empty_cache()
+    coder = cf.ClusterCoder(geom[0], geom[1], n, device=dev)
+    out = torch.empty(coder.max_encoded_bytes(n), dtype=torch.uint8, device=dev)
+    back = torch.empty(n * 32, dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2, written between timed calls
+
+    def timed(fn, steps):
+        ms = []
+        for _ in range(steps):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        return ms
+
+    enc = lambda: coder.encode(clusters, n, out)
+    sampler = ClockSampler(0).start()
+    timed(enc, args.warmup)
+    est = coder.read_status()
+    if est["error"]:
+        raise RuntimeError("encode failed: %r" % (est,))
+    total = est["bytes"]
+    enc_launches = coder.last_launch_count()
+    dec = lambda: coder.decode(out, total, n, back)
+    timed(dec, args.warmup)
+    dst = coder.read_status()
+    if dst["error"]:
+        raise RuntimeError("decode failed: %r" % (dst,))
+    dec_launches = coder.last_launch_count()
+    with sampler as clocks:
+        enc_ms = timed(enc, args.steps)
+        dec_ms = timed(dec, args.steps)
+    e_ms, d_ms = float(np.mean(enc_ms)), float(np.mean(dec_ms))
+    # integer fields must survive the round trip bit-exactly (the floats are quantised by the format)
+    b = back.cpu().numpy().view(cf.CLUSTER)
+    for fld in ("sector", "row", "pad", "time", "qmax", "qtot", "flags"):
+        if not np.array_equal(b[fld], cl_host[fld]):
+            raise RuntimeError("round trip changed field %s" % fld)
+    peak, peak_src = load_peaks()
+    # algorithmic bytes of one encode: 32 B/cluster read + 13 B/cluster symbol streams written and read twice
+    # (histogram, coder) + the container written; DESIGN.md §10
+    alg = 32.0 * n + 13.0 * n * 3 + float(total)
+    host_out = torch.empty(out.numel(), dtype=torch.uint8, pin_memory=True)
+    host_in = torch.from_numpy(cl_host.view(np.uint8)).pin_memory()
+    dev_in = torch.empty(n * 32, dtype=torch.uint8, device=dev)
+
+    def e2e_step():
+        dev_in.copy_(host_in, non_blocking=True)
+        coder.encode(dev_in, n, out)
+        s = coder.read_status()
+        host_out[:s["bytes"]].copy_(out[:s["bytes"]], non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_step()
+    t0 = time.perf_counter()
+    for _ in range(3):
+        e2e_step()
+    x_ms = (time.perf_counter() - t0) * 1e3 / 3
+    line = {"metric": "tpc_clusters_encoded_per_second", "value": n / (e_ms * 1e-3), "unit": "clusters/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": e_ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u8/u32", "data": "synthetic",
+            "config": {"workload": "entropy coder (TPC-EC v1) on the cluster stream of config%d: %s" % (
+                           args.config, cfg["label"]), "stage": "ec", "clusters": n, "container_bytes": total,
+                       "bits_per_cluster": 8.0 * total / n, "ratio_vs_32B_records": 32.0 * n / total,
+                       "l2": "256 MB written between timed calls (L2 flush)"},
+            "decode": {"ms": d_ms, "clusters_per_s": n / (d_ms * 1e-3), "gpu_launches": dec_launches},
+            "roofline": {"bound": "hbm", "kernel": "tpc_ec_encode (all %d kernels)" % enc_launches,
+                         "achieved": alg / (e_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s", "peak_source": peak_src,
+                         "frac": alg / (e_ms * 1e-3) / 1e9 / peak, "traffic": None,
+                         "algorithmic_bytes_per_launch": alg,
+                         "note": "the coder is bound by the serial rANS recurrence per lane (ALU latency), not by HBM"},
+            "cpu_baseline": None,
+            "e2e": {"value": n / (x_ms * 1e-3), "unit": "clusters/s", "ms_per_step": x_ms,
+                    "h2d_bytes_per_step": int(n * 32), "d2h_bytes_per_step": int(total + 24)},
+            "gpu_launches": enc_launches * args.steps, "clocks": clocks.summary()}
+    if not args.no_cpu_baseline:
+        from oracle import ec_oracle as eco
+        eco.build()
+        m = min(n, 2_000_000)
+        # whole planes only: cut at the first cluster of a plane
+        key = cl_host["sector"][:m].astype(np.int64) * 256 + cl_host["row"][:m]
+        m = int(np.searchsorted(key, key[-1])) if m < n else m
+        t0 = time.perf_counter()
+        buf, err, tot = eco.encode(cl_host[:m], geom[0], geom[1])
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": m / dt, "unit": "clusters/s", "cores": 1, "kind": "oracle",
+                                "sample": "first %d clusters (whole planes) of the stream, %.1f s, single thread" % (m, dt)}
+    print(json.dumps(line))
+    coder.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -185,11 +305,16 @@ def main():
     ap.add_argument("--variant", default="none", choices=["none", "flags", "cuts"],
                     help="cluster-finder variants (SURVEY.md §8(f) NEXT #1): 'flags' = per-cluster flags, 'cuts' = "
                          "flags + q_tot_min 40 + single-pad cut; the default run has none")
+    ap.add_argument("--stage", default="cf", choices=["cf", "ec"],
+                    help="'cf' = the cluster finder (the headline path); 'ec' = the entropy coder of the cluster stream "
+                         "(SURVEY.md §8(f) NEXT #2): encode and decode of the frame's clusters, one JSON line")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.stage == "ec":
+        return run_ec(args)
 
     import torch
     import torch.distributed as dist
