@@ -129,10 +129,10 @@ def test_impulse_tail_decays_geometrically():
     ped4 = np.full((1, W), 400, dtype=np.uint16)
     raw = np.full((1, T, W), 100, dtype=np.uint16)
     raw[0, 2, :P] = 100 + 1024
-    A2 = 300
+    A2 = 600
     for p in range(P):
         raw[0, 2 + p + 1, p] = 100 + A2
-    prm = dict(zs_threshold=290, cm_quiet4=12, cm_min_pads=60000, it_decay_shift=2)
+    prm = dict(zs_threshold=500, cm_quiet4=12, cm_min_pads=60000, it_decay_shift=2)
     out, _ = feo.run(raw, ped4, 1, 1, P, T, it_kappa_shift=2, **prm)
     want = []
     for p in range(P):
