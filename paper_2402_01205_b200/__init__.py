@@ -1,6 +1,6 @@
 """B200-native TPC cluster finder (arXiv:2402.01205, step named in PAPER.md:57): C-ABI library + thin binding.
 
-    from paper_2402_01205_b200 import ClusterFinder, ClusterCoder
+    from paper_2402_01205_b200 import ClusterFinder, ClusterCoder, FrontEndFilter
 The CUDA library (libtpc_cf.so) is loaded on first use; there is no CPU fallback.
 """
 from .binding import (CLUSTER, CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME, DIGIT, DIGITS_SORTED, EXPORTS,
@@ -12,7 +12,12 @@ from .ec_binding import (EC_ERR_CAPACITY, EC_ERR_CONTAINER, EC_ERR_QTOT, EC_ERR_
                          ClusterCoder, clusters_to_device, tpc_ec_create, tpc_ec_decode, tpc_ec_destroy,
                          tpc_ec_encode, tpc_ec_max_encoded_bytes, tpc_ec_workspace_bytes)
 
-__all__ = ["EC_ERR_CAPACITY", "EC_ERR_CONTAINER", "EC_ERR_QTOT", "EC_ERR_UNSORTED", "EC_EXPORTS", "EC_STATUS",
+from .fe_binding import (FE_DEFAULTS, FE_EXPORTS, FE_OVF_OUTPUT, FE_OVF_PLANE, FE_STATUS, FeParams, FrontEndFilter,
+                         tpc_fe_create, tpc_fe_destroy, tpc_fe_pad_stride, tpc_fe_run, tpc_fe_workspace_bytes)
+
+__all__ = ["FE_DEFAULTS", "FE_EXPORTS", "FE_OVF_OUTPUT", "FE_OVF_PLANE", "FE_STATUS", "FeParams", "FrontEndFilter",
+           "tpc_fe_create", "tpc_fe_destroy", "tpc_fe_pad_stride", "tpc_fe_run", "tpc_fe_workspace_bytes",
+           "EC_ERR_CAPACITY", "EC_ERR_CONTAINER", "EC_ERR_QTOT", "EC_ERR_UNSORTED", "EC_EXPORTS", "EC_STATUS",
            "ClusterCoder", "clusters_to_device", "tpc_ec_create", "tpc_ec_decode", "tpc_ec_destroy", "tpc_ec_encode",
            "tpc_ec_max_encoded_bytes", "tpc_ec_workspace_bytes",
            "CLUSTER", "DIGIT", "STATUS", "DIGITS_SORTED", "FORCE_GENERAL", "CLUSTER_FLAGS", "CUT_SINGLE_PAD",

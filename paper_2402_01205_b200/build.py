@@ -1,4 +1,4 @@
-"""Builds libtpc_cf.so (the C-ABI library of include/tpc_cf.h and include/tpc_ec.h) in-tree with nvcc for sm_100a.
+"""Builds libtpc_cf.so (the C-ABI library of include/tpc_cf.h, include/tpc_ec.h and include/tpc_fe.h) in-tree with nvcc for sm_100a.
 
 nvcc cross-compiles without a GPU.  The built .so is git-ignored but travels with the snapshot to the GPU box.
 """
@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libtpc_cf.so")
 SOURCES = ["tpc_cf_api.cu", "tpc_cf_general.cu", "tpc_cf_fused.cu", "tpc_cf_blocks.cu", "tpc_cf_compact.cu",
-           "tpc_ec.cu"]
+           "tpc_ec.cu", "tpc_fe.cu"]
 HEADERS = [os.path.join(CSRC, "tpc_cf_internal.cuh"),
            os.path.join(os.path.dirname(_HERE), "include", "tpc_cf.h"),
            os.path.join(os.path.dirname(_HERE), "include", "tpc_ec.h")]

@@ -1,0 +1,465 @@
+// tpc_fe.cu — TPC front-end filter "TPC-FE v1" (include/tpc_fe.h; step named in PAPER.md:57): common-mode correction,
+// ion-tail cancellation and zero suppression of the raw, time-major ADC samples -> sorted tpc_digit records.
+// Product code, sm_100a.  Shares nothing with oracle/tpc_fe_oracle.c: the definition text in the header is the only link.
+//
+// On the caller's stream:
+//   k_fe_filter   the dense pass (HBM-bound by design: every raw sample is read exactly once).  Persistent CTAs, one
+//                 (sector,row) plane at a time, one thread per pad.  The plane streams through a ring of kStages
+//                 tiles of kTT time bins in shared memory; a tile is one contiguous piece of the time-major input and
+//                 is fetched with one bulk copy (cp.async.bulk + mbarrier transaction count), kStages - 1 tiles ahead.
+//                 Per tile: (1) a warp per time bin forms the quiet-pad sum and count in one packed accumulator and one
+//                 warp reduction -> cm[t]; (2) every thread walks its pad through the tile's time bins with the tail
+//                 state in a register, marks the kept bins in a 64-bit mask and overwrites their cells with q;
+//                 (3) a block scan of the kept counts places the tile's records (pad, rank in the pad line, time, q)
+//                 in the plane's staging area.  Per-line and per-plane counts at the end of the plane.
+//   k_fe_scan     exclusive scan of the plane counts; status
+//   k_fe_order    one CTA per plane: line offsets from the line counts, then every staged record goes to
+//                 out[plane offset + line offset + rank]: ascending (sector,row,pad,time) without a sort
+#include <new>
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tpc_fe.h"
+
+namespace tpcfe {
+
+static constexpr int kTT = 64;          // time bins per tile (the kept-bin mask is 64 bits)
+static constexpr int kStages = 4;       // tiles in the ring: kStages - 1 in flight ahead of the one in work
+static constexpr int kAccShift = 22;    // packed quiet-pad accumulator: count << 22 | sum (|sum| < 2^20)
+
+struct Args {
+    const uint16_t* raw;
+    const uint16_t* ped4;
+    const uint32_t* npads;      // [n_rows]
+    uint32_t n_planes, n_rows, n_time, W;
+    uint32_t zs, c, m, k, mul;  // zs_threshold, cm_quiet4, cm_min_pads, it_decay_shift, 1 << (14 - kappa) or 0
+    uint32_t cap;               // staged records per plane
+    uint2* temp;                // [n_planes][cap]
+    uint32_t* line_cnt;         // [n_planes][W]
+    uint32_t* plane_cnt;        // [n_planes]
+    uint32_t* flags;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+// one contiguous piece of global memory -> shared memory, completion counted in bytes on the mbarrier
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, unsigned long long* bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int NW>
+__global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint16_t* tiles = (uint16_t*)smem;                    // [kStages][kTT * W]
+    __shared__ __align__(8) unsigned long long s_bar[kStages];
+    __shared__ __align__(16) int s_cm[2][kTT];
+    __shared__ uint32_t s_wtot[8];
+
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t W = a.W, T = a.n_time;
+    const uint32_t tile_elems = kTT * W;
+    const uint32_t tpp = (T + kTT - 1) / kTT;                                   // tiles per plane
+    const uint32_t my_planes = blockIdx.x < a.n_planes ? (a.n_planes - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const uint32_t total_tiles = my_planes * tpp;
+
+    if (tid == 0) {
+        for (int s = 0; s < kStages; s++) mbar_init(&s_bar[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    auto issue = [&](uint32_t m) {                                              // thread 0 only
+        const uint32_t lp = m / tpp, tl = m - lp * tpp;
+        const uint32_t plane = blockIdx.x + lp * gridDim.x;
+        const uint32_t t0 = tl * kTT;
+        const uint32_t nt = min((uint32_t)kTT, T - t0);
+        const uint16_t* src = a.raw + ((size_t)plane * T + t0) * W;
+        bulk_load(tiles + (size_t)(m % kStages) * tile_elems, src, nt * W * 2u, &s_bar[m % kStages]);
+    };
+    if (tid == 0)
+        for (uint32_t m = 0; m < (uint32_t)(kStages - 1) && m < total_tiles; m++) issue(m);
+
+    const uint32_t c2 = 2u * a.c;
+    const uint32_t bias = (1u << kAccShift) - a.c;
+    uint32_t n = 0;                                                             // tile sequence number of this CTA
+    for (uint32_t lp = 0; lp < my_planes; lp++) {
+        const uint32_t plane = blockIdx.x + lp * gridDim.x;
+        const uint32_t P = a.npads[plane % a.n_rows];
+        const bool active = tid < P;
+        const uint16_t* ped = a.ped4 + (size_t)plane * W;
+        const int pedneg2 = active ? 2 - (int)ped[tid] : 0;                     // z + 2 = 4 raw + (2 - ped) - cm + tail
+        // phase-1 view: lane handles pads lane + 32 g
+        uint32_t pedq[NW], offs[NW];
+#pragma unroll
+        for (int g = 0; g < NW; g++) {
+            const uint32_t pad = lane + 32u * g;
+            offs[g] = min(pad, W - 1);
+            pedq[g] = pad < P ? a.c - (uint32_t)ped[pad] : 0x40000000u;         // beyond the row: never quiet
+        }
+        int S = 0;
+        uint32_t cnt = 0;       // kept samples of this pad line so far (rank of the next one)
+        uint32_t pos = 0;       // kept samples of the plane so far (same value in every thread)
+        uint2* temp = a.temp + (size_t)plane * a.cap;
+
+        for (uint32_t tl = 0; tl < tpp; tl++, n++) {
+            const uint32_t t0 = tl * kTT;
+            const uint32_t nt = min((uint32_t)kTT, T - t0);
+            uint16_t* tile = tiles + (size_t)(n % kStages) * tile_elems;
+            int* cmv = s_cm[n & 1];
+            mbar_wait(&s_bar[n % kStages], (n / kStages) & 1u);
+
+            // ---- (1) common mode of every time bin of the tile: warp `warp` takes bins warp, warp + NW, ...
+            for (uint32_t b0 = 0; b0 * NW + warp < nt; b0 += 32) {
+                int mine = 0;
+                for (uint32_t b = b0; b < b0 + 32; b++) {
+                    const uint32_t i = b * NW + warp;
+                    if (i >= nt) break;
+                    const uint16_t* row = tile + i * W;
+                    int acc = 0;
+#pragma unroll
+                    for (int g = 0; g < NW; g++) {
+                        const uint32_t xb = (uint32_t)row[offs[g]] * 4u + pedq[g];   // x + c
+                        if (xb <= c2) acc += (int)(xb + bias);                       // x + 2^22
+                    }
+                    acc = __reduce_add_sync(0xffffffffu, acc);
+                    if (lane == b - b0) mine = acc;
+                }
+                const uint32_t i = (b0 + lane) * NW + warp;
+                if (i < nt) {
+                    const int nq = (mine + (1 << (kAccShift - 1))) >> kAccShift;
+                    const int s = mine - (nq << kAccShift);
+                    int cm = 0;
+                    if (nq >= (int)a.m && nq > 0) {
+                        const int num = 2 * s + nq, den = 2 * nq;
+                        cm = num / den;
+                        if (num - cm * den < 0) cm -= 1;                             // floor
+                    }
+                    cmv[i] = cm;
+                }
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // this thread's q stores into tile n - 1
+            __syncthreads();
+            // every thread is past tile n - 1: its stage is free for tile n + kStages - 1
+            if (tid == 0 && n + kStages - 1 < total_tiles) issue(n + kStages - 1);
+
+            // ---- (2) the pad's walk through the tile
+            uint32_t mlo = 0, mhi = 0;
+            if (active) {
+                uint16_t* cell = tile + tid;
+                if (nt == (uint32_t)kTT) {
+#pragma unroll
+                    for (int i4 = 0; i4 < kTT; i4 += 4) {
+                        const int4 cm4 = *(const int4*)(cmv + i4);
+                        const int cma[4] = {cm4.x, cm4.y, cm4.z, cm4.w};
+#pragma unroll
+                        for (int u = 0; u < 4; u++) {
+                            const int i = i4 + u;
+                            const int z2 = (int)cell[i * W] * 4 + pedneg2 - cma[u] + (S >> 12);
+                            const int q = min(z2 >> 2, 65535);
+                            S -= S >> a.k;
+                            if (q >= (int)a.zs) {
+                                S += q * (int)a.mul;
+                                cell[i * W] = (uint16_t)q;
+                                if (i < 32) mlo |= 1u << i; else mhi |= 1u << (i - 32);
+                            }
+                        }
+                    }
+                } else {
+                    for (uint32_t i = 0; i < nt; i++) {
+                        const int z2 = (int)cell[i * W] * 4 + pedneg2 - cmv[i] + (S >> 12);
+                        const int q = min(z2 >> 2, 65535);
+                        S -= S >> a.k;
+                        if (q >= (int)a.zs) {
+                            S += q * (int)a.mul;
+                            cell[i * W] = (uint16_t)q;
+                            if (i < 32) mlo |= 1u << i; else mhi |= 1u << (i - 32);
+                        }
+                    }
+                }
+            }
+
+            // ---- (3) place the tile's records: block scan of the kept counts
+            const uint32_t c = __popc(mlo) + __popc(mhi);
+            uint32_t incl = c;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= (uint32_t)d) incl += v;
+            }
+            if (lane == 31) s_wtot[warp] = incl;
+            __syncthreads();
+            uint32_t before = 0, tile_total = 0;
+#pragma unroll
+            for (int w = 0; w < NW; w++) {
+                const uint32_t v = s_wtot[w];
+                if ((uint32_t)w < warp) before += v;
+                tile_total += v;
+            }
+            uint32_t idx = pos + before + incl - c;
+            uint32_t rank = cnt;
+            const uint16_t* cell = tile + tid;
+            while (mlo) {
+                const uint32_t i = __ffs(mlo) - 1;
+                mlo &= mlo - 1;
+                if (idx < a.cap) temp[idx] = make_uint2(tid | (rank << 8), (t0 + i) | ((uint32_t)cell[i * W] << 16));
+                idx++; rank++;
+            }
+            while (mhi) {
+                const uint32_t i = __ffs(mhi) + 31;
+                mhi &= mhi - 1;
+                if (idx < a.cap) temp[idx] = make_uint2(tid | (rank << 8), (t0 + i) | ((uint32_t)cell[i * W] << 16));
+                idx++; rank++;
+            }
+            cnt = rank;
+            pos += tile_total;
+        }
+        if (tid < W) a.line_cnt[(size_t)plane * W + tid] = cnt;
+        if (tid == 0) {
+            a.plane_cnt[plane] = pos;
+            if (pos > a.cap) atomicOr(a.flags, (uint32_t)TPC_FE_OVF_PLANE);
+        }
+    }
+}
+
+// exclusive scan of the plane counts (one CTA), status
+__global__ void __launch_bounds__(1024) k_fe_scan(const uint32_t* plane_cnt, uint32_t n_planes, uint64_t* plane_off,
+                                                  uint32_t* flags)
+{
+    __shared__ uint64_t s_w[32];
+    __shared__ uint64_t s_carry;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    for (uint32_t b = 0; b < n_planes; b += 1024) {
+        const uint32_t i = b + tid;
+        const uint64_t v = i < n_planes ? plane_cnt[i] : 0;
+        uint64_t incl = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint64_t u = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= (uint32_t)d) incl += u;
+        }
+        if (lane == 31) s_w[warp] = incl;
+        __syncthreads();
+        uint64_t before = s_carry;
+        for (uint32_t w = 0; w < warp; w++) before += s_w[w];
+        if (i < n_planes) plane_off[i] = before + incl - v;
+        __syncthreads();
+        if (tid == 1023) s_carry = before + incl;
+        __syncthreads();
+    }
+    if (tid == 0) *(uint64_t*)(flags + 2) = s_carry;       // total; the status is written by the last CTA of k_fe_order
+}
+
+// one CTA per plane: staged records -> their place in the sorted output
+__global__ void __launch_bounds__(256) k_fe_order(const uint2* temp_all, uint32_t cap, const uint32_t* line_cnt,
+                                                  const uint32_t* plane_cnt, const uint64_t* plane_off, uint32_t W,
+                                                  uint32_t n_rows, uint2* out, uint64_t capacity, uint32_t* flags,
+                                                  tpc_fe_status* status)
+{
+    __shared__ uint32_t s_off[256];
+    __shared__ uint32_t s_w[8];
+    const uint32_t plane = blockIdx.x, tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t v = tid < W ? line_cnt[(size_t)plane * W + tid] : 0;
+    uint32_t incl = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= (uint32_t)d) incl += u;
+    }
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    uint32_t before = 0;
+    for (uint32_t w = 0; w < warp; w++) before += s_w[w];
+    s_off[tid] = before + incl - v;
+    __syncthreads();
+    const uint32_t n = min(plane_cnt[plane], cap);
+    const uint64_t base = plane_off[plane];
+    const uint2* temp = temp_all + (size_t)plane * cap;
+    const uint32_t head = (plane / n_rows) | ((plane % n_rows) << 8);
+    for (uint32_t i = tid; i < n; i += 256) {
+        const uint2 r = temp[i];
+        const uint32_t pad = r.x & 255u;
+        const uint64_t dst = base + s_off[pad] + (r.x >> 8);
+        if (dst < capacity) out[dst] = make_uint2(head | (pad << 16), r.y);
+    }
+    // the status is written last: by the CTA that finishes last
+    __threadfence();
+    __syncthreads();
+    if (tid == 0 && atomicAdd(flags + 1, 1u) == gridDim.x - 1) {
+        const uint64_t total = *(const volatile uint64_t*)(flags + 2);
+        status->n_digits = total;
+        status->overflow = *(const volatile uint32_t*)flags | (total > capacity ? (uint32_t)TPC_FE_OVF_OUTPUT : 0u);
+        status->rsv = 0;
+    }
+}
+
+}  // namespace tpcfe
+
+using namespace tpcfe;
+
+struct tpc_fe {
+    uint32_t n_sectors, n_rows, max_pads, n_time, W, n_planes;
+    uint64_t cap;
+    uint2* temp;
+    uint32_t* line_cnt;
+    uint32_t* plane_cnt;
+    uint64_t* plane_off;
+    uint32_t* npads;
+    uint32_t* flags;
+    uint32_t grid, smem;
+    int last_launches;
+};
+
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static size_t carve(uint32_t n_planes, uint32_t n_rows, uint32_t W, uint64_t cap, char* base, tpc_fe* e)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align256(bytes); return base ? base + o : (char*)nullptr; };
+    char* p;
+    p = take(256);                                   if (e) e->flags = (uint32_t*)p;
+    p = take(4ull * n_rows);                         if (e) e->npads = (uint32_t*)p;
+    p = take(4ull * n_planes);                       if (e) e->plane_cnt = (uint32_t*)p;
+    p = take(8ull * n_planes);                       if (e) e->plane_off = (uint64_t*)p;
+    p = take(4ull * n_planes * W);                   if (e) e->line_cnt = (uint32_t*)p;
+    p = take(8ull * n_planes * cap);                 if (e) e->temp = (uint2*)p;
+    return off;
+}
+
+static bool geometry_ok(const tpc_cf_geometry* g)
+{
+    if (g->n_sectors == 0 || g->n_sectors > 256 || g->n_rows == 0 || g->n_rows > 256 || g->max_pads == 0 ||
+        g->max_pads > 255 || g->n_time == 0 || g->n_time > 65535) return false;
+    if (g->npads)
+        for (uint32_t r = 0; r < g->n_rows; r++)
+            if (g->npads[r] == 0 || g->npads[r] > g->max_pads) return false;
+    return true;
+}
+
+extern "C" uint32_t tpc_fe_pad_stride(uint32_t max_pads) { return (max_pads + 7u) / 8u * 8u; }
+
+extern "C" size_t tpc_fe_workspace_bytes(const tpc_cf_geometry* g, uint64_t max_digits_per_plane)
+{
+    if (!g || !geometry_ok(g) || max_digits_per_plane == 0 || max_digits_per_plane >= (1ull << 32)) return 0;
+    return carve(g->n_sectors * g->n_rows, g->n_rows, tpc_fe_pad_stride(g->max_pads), max_digits_per_plane, nullptr,
+                 nullptr);
+}
+
+template <int NW>
+static void setup_kernel(tpc_fe* e)
+{
+    int dev = 0, sms = 148, per_sm = 1;
+    if (cudaFuncSetAttribute(k_fe_filter<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e->smem) != cudaSuccess ||
+        cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fe_filter<NW>, NW * 32, e->smem) != cudaSuccess) {
+        cudaGetLastError();      // no device (host-only tests): the launch will report it
+        sms = 148; per_sm = 1;
+    }
+    if (per_sm < 1) per_sm = 1;
+    e->grid = (uint32_t)(sms * per_sm);
+}
+
+extern "C" int tpc_fe_create(tpc_fe** h, const tpc_cf_geometry* g, uint64_t max_digits_per_plane, void* workspace,
+                             size_t workspace_bytes)
+{
+    if (!h || !g || !workspace) return TPC_CF_E_NULL;
+    if (!geometry_ok(g)) return TPC_CF_E_GEOMETRY;
+    if (max_digits_per_plane == 0 || max_digits_per_plane >= (1ull << 32)) return TPC_CF_E_CAPACITY;
+    const uint32_t W = tpc_fe_pad_stride(g->max_pads), n_planes = g->n_sectors * g->n_rows;
+    if (((uintptr_t)workspace & 255u) != 0 ||
+        workspace_bytes < carve(n_planes, g->n_rows, W, max_digits_per_plane, nullptr, nullptr))
+        return TPC_CF_E_WORKSPACE;
+    tpc_fe* e = new (std::nothrow) tpc_fe;
+    if (!e) return TPC_CF_E_NOMEM;
+    e->n_sectors = g->n_sectors; e->n_rows = g->n_rows; e->max_pads = g->max_pads; e->n_time = g->n_time;
+    e->W = W; e->n_planes = n_planes; e->cap = max_digits_per_plane; e->last_launches = 0;
+    carve(n_planes, g->n_rows, W, max_digits_per_plane, (char*)workspace, e);
+    uint32_t np[256];
+    for (uint32_t r = 0; r < g->n_rows; r++) np[r] = g->npads ? g->npads[r] : g->max_pads;
+    if (cudaMemcpy(e->npads, np, 4ull * g->n_rows, cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        delete e;
+        return TPC_CF_E_CUDA;
+    }
+    e->smem = (uint32_t)(kStages * kTT * W * 2u);
+    switch ((W + 31) / 32) {
+        case 1: setup_kernel<1>(e); break;
+        case 2: setup_kernel<2>(e); break;
+        case 3: setup_kernel<3>(e); break;
+        case 4: setup_kernel<4>(e); break;
+        case 5: setup_kernel<5>(e); break;
+        case 6: setup_kernel<6>(e); break;
+        case 7: setup_kernel<7>(e); break;
+        default: setup_kernel<8>(e); break;
+    }
+    *h = e;
+    return TPC_CF_OK;
+}
+
+extern "C" int tpc_fe_run(tpc_fe* h, const uint16_t* raw, const uint16_t* ped4, const tpc_fe_params* p, tpc_digit* out,
+                          uint64_t capacity, tpc_fe_status* status, void* stream)
+{
+    if (!h || !raw || !ped4 || !p || !status || (!out && capacity)) return TPC_CF_E_NULL;
+    const int k = p->it_decay_shift, j = p->it_kappa_shift;
+    if (p->zs_threshold < 1 || p->cm_quiet4 > 4095 || p->cm_min_pads < 1 || k < 1 || k > 15 ||
+        (j != 0 && (j < k || j > 14))) return TPC_CF_E_PARAMS;
+    if (((uintptr_t)raw & 15u) != 0 || ((uintptr_t)out & 7u) != 0) return TPC_CF_E_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    Args a;
+    a.raw = raw; a.ped4 = ped4; a.npads = h->npads;
+    a.n_planes = h->n_planes; a.n_rows = h->n_rows; a.n_time = h->n_time; a.W = h->W;
+    a.zs = p->zs_threshold; a.c = p->cm_quiet4; a.m = p->cm_min_pads; a.k = (uint32_t)k;
+    a.mul = j ? 1u << (14 - j) : 0u;
+    a.cap = (uint32_t)h->cap; a.temp = h->temp; a.line_cnt = h->line_cnt; a.plane_cnt = h->plane_cnt; a.flags = h->flags;
+    cudaMemsetAsync(h->flags, 0, 16, st);
+    const uint32_t grid = h->grid < h->n_planes ? h->grid : h->n_planes;
+    switch ((h->W + 31) / 32) {
+        case 1: k_fe_filter<1><<<grid, 32, h->smem, st>>>(a); break;
+        case 2: k_fe_filter<2><<<grid, 64, h->smem, st>>>(a); break;
+        case 3: k_fe_filter<3><<<grid, 96, h->smem, st>>>(a); break;
+        case 4: k_fe_filter<4><<<grid, 128, h->smem, st>>>(a); break;
+        case 5: k_fe_filter<5><<<grid, 160, h->smem, st>>>(a); break;
+        case 6: k_fe_filter<6><<<grid, 192, h->smem, st>>>(a); break;
+        case 7: k_fe_filter<7><<<grid, 224, h->smem, st>>>(a); break;
+        default: k_fe_filter<8><<<grid, 256, h->smem, st>>>(a); break;
+    }
+    k_fe_scan<<<1, 1024, 0, st>>>(h->plane_cnt, h->n_planes, h->plane_off, h->flags);
+    k_fe_order<<<h->n_planes, 256, 0, st>>>(h->temp, (uint32_t)h->cap, h->line_cnt, h->plane_cnt, h->plane_off, h->W,
+                                            h->n_rows, (uint2*)out, capacity, h->flags, status);
+    h->last_launches = 3;
+    return cudaGetLastError() == cudaSuccess ? TPC_CF_OK : TPC_CF_E_CUDA;
+}
+
+extern "C" int tpc_fe_last_launch_count(const tpc_fe* h) { return h ? h->last_launches : 0; }
+
+extern "C" int tpc_fe_destroy(tpc_fe* h)
+{
+    if (!h) return TPC_CF_E_NULL;
+    delete h;
+    return TPC_CF_OK;
+}

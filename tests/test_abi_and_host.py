@@ -32,7 +32,7 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_every_header_under_include_is_covered():
-    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["tpc_cf.h", "tpc_ec.h"]
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["tpc_cf.h", "tpc_ec.h", "tpc_fe.h"]
 
 
 def test_library_exports_every_entropy_coder_symbol():
@@ -45,6 +45,49 @@ def test_library_exports_every_entropy_coder_symbol():
     assert sorted(cf.EC_EXPORTS) == syms, "ec_binding.EC_EXPORTS and include/tpc_ec.h disagree"
     src = open(os.path.join(ROOT, "paper_2402_01205_b200", "ec_binding.py")).read()
     assert "oracle" not in src, "the product binding must not reference the oracle"
+
+
+def test_library_exports_every_front_end_filter_symbol():
+    import paper_2402_01205_b200 as cf
+    lib = cf.load()
+    syms = declared_symbols("tpc_fe.h", "tpc_fe_")
+    assert "tpc_fe_create" in syms and "tpc_fe_run" in syms and "tpc_fe_destroy" in syms
+    for s in syms:
+        assert hasattr(lib, s), "libtpc_cf.so does not export %s" % s
+    assert sorted(cf.FE_EXPORTS) == syms, "fe_binding.FE_EXPORTS and include/tpc_fe.h disagree"
+    src = open(os.path.join(ROOT, "paper_2402_01205_b200", "fe_binding.py")).read()
+    assert "oracle" not in src, "the product binding must not reference the oracle"
+    src = open(os.path.join(ROOT, "paper_2402_01205_b200", "csrc", "tpc_fe.cu")).read()
+    assert "#include \"../../oracle" not in src and "tpc_fe_oracle.h" not in src
+
+
+def test_front_end_filter_host_logic_without_a_device():
+    """sizes and the synchronous argument errors of include/tpc_fe.h that are decided before any device call"""
+    import paper_2402_01205_b200 as cf
+    from paper_2402_01205_b200 import fe_binding as fb
+    assert cf.FE_STATUS.itemsize == 16 and ctypes.sizeof(cf.FeParams) == 8
+    assert [cf.tpc_fe_pad_stride(p) for p in (1, 8, 9, 138, 255)] == [8, 8, 16, 144, 256]
+    g, keep = cf.make_geometry(36, 152, 138, 14336)
+    w = cf.tpc_fe_workspace_bytes(g, 65536)
+    planes = 36 * 152
+    assert 8 * planes * 65536 + 4 * planes * 144 < w < 8 * planes * 65536 + 4 * planes * 144 + 16 * planes + 4096
+    assert cf.tpc_fe_workspace_bytes(g, 0) == 0 and cf.tpc_fe_workspace_bytes(g, 1 << 32) == 0
+    bad, _ = cf.make_geometry(36, 152, 256, 14336)
+    assert cf.tpc_fe_workspace_bytes(bad, 100) == 0
+    lib = fb._lib()
+    h = ctypes.c_void_p()
+    fake = ctypes.c_void_p(1 << 20)
+    assert lib.tpc_fe_create(ctypes.byref(h), ctypes.byref(g), 65536, None, w) == -1
+    assert lib.tpc_fe_create(ctypes.byref(h), ctypes.byref(bad), 65536, fake, w) == -2
+    assert lib.tpc_fe_create(ctypes.byref(h), ctypes.byref(g), 0, fake, w) == -3
+    assert lib.tpc_fe_create(ctypes.byref(h), ctypes.byref(g), 65536, ctypes.c_void_p((1 << 20) + 8), w) == -4
+    assert lib.tpc_fe_create(ctypes.byref(h), ctypes.byref(g), 65536, fake, 1000) == -4
+    assert lib.tpc_fe_destroy(None) == -1
+    with pytest.raises(RuntimeError):
+        import torch
+        if torch.cuda.is_available():
+            raise RuntimeError("device present: the no-fallback check is for CPU boxes")
+        cf.FrontEndFilter(1, 1, 8, 64)
 
 
 def test_entropy_coder_host_logic_without_a_device():
