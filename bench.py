@@ -292,6 +292,126 @@ def run_ec(args):
     return 0
 
 
+def run_fe(args):
+    """--stage fe: the front-end filter (include/tpc_fe.h) on the raw samples of one frame of the chosen config
+    (datagen/fe_gen.py's forward model over the config's digits).  One GPU.  A step = one tpc_fe_run (all its kernels)
+    over the whole frame, resident in HBM; value = raw samples per second."""
+    import torch
+    from datagen import gen, fe_gen
+    import paper_2402_01205_b200 as cf
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    cfg = dict(gen.CONFIGS[args.config])
+    if args.fe_sectors:
+        cfg["n_sectors"] = min(cfg["n_sectors"], args.fe_sectors)
+    ns, nr, mp, nt, npads = gen.geometry(cfg)
+    W = cf.tpc_fe_pad_stride(mp)
+    n_planes = ns * nr
+    zs = 3
+    t0 = time.perf_counter()
+    host_raw = torch.empty((n_planes, nt, W), dtype=torch.int16, pin_memory=True)
+    host_ped = torch.empty((n_planes, W), dtype=torch.int16, pin_memory=True)
+    raw_np, ped_np = host_raw.numpy().view(np.uint16), host_ped.numpy().view(np.uint16)
+    n_truth = 0
+    for s in range(ns):
+        d = gen.generate(cfg, sectors=(s, s + 1))
+        n_truth += int(d.shape[0])
+        fe_gen.raw_from_digits(d, ns, nr, mp, nt, npads=npads, seed=cfg["seed"], planes=(s * nr, (s + 1) * nr),
+                               out=(raw_np[s * nr:(s + 1) * nr], ped_np[s * nr:(s + 1) * nr]))
+    gen_s = time.perf_counter() - t0
+    raw = host_raw.to(dev)
+    ped = host_ped.to(dev)
+    pads = int(np.sum(npads)) if npads is not None else nr * mp
+    cells = ns * pads * nt                                     # valid samples
+    cap_plane = int(min(nt * mp, max(4096, 2.0 * n_truth / n_planes)))
+    flt = cf.FrontEndFilter(ns, nr, mp, nt, npads=npads, max_digits_per_plane=cap_plane, device=dev)
+    cap = int(1.3 * n_truth) + 4096
+    out = torch.empty(cap * 8, dtype=torch.uint8, device=dev)
+    step = lambda: flt.run(raw, ped, out, capacity=cap, zs_threshold=zs)
+    sampler = ClockSampler(0).start()
+    for _ in range(args.warmup):
+        step()
+    st = flt.read_status()
+    if st["overflow"]:
+        raise RuntimeError("bench run invalid: status %r" % (st,))
+    n_dig = st["n_digits"]
+    flt.set_profiling(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kern = []
+    torch.cuda.synchronize()
+    with sampler as clocks:
+        ev0.record()
+        for _ in range(args.steps):
+            step()
+        ev1.record()
+        torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    for _ in range(min(args.steps, 5)):                       # the dominant kernel alone, by its own event pair
+        step()
+        kern.append(flt.profile_ms())
+    flt.set_profiling(False)
+    k_ms = float(np.mean(kern))
+    peak, peak_src = load_peaks()
+    # algorithmic bytes of k_fe_filter per launch: 2 B per valid sample read once, 8 B per kept sample staged,
+    # pedestals and line counts (DESIGN.md §11)
+    alg = 2.0 * cells + 8.0 * n_dig + 2.0 * n_planes * W + 4.0 * n_planes * W
+    # e2e: host raw (pinned) -> device, filter, digits and status back
+    host_out = torch.empty(cap * 8, dtype=torch.uint8, pin_memory=True)
+    e2e = None
+    if not args.no_e2e:
+        def e2e_step():
+            raw.copy_(host_raw, non_blocking=True)
+            ped.copy_(host_ped, non_blocking=True)
+            step()
+            s2 = flt.read_status()
+            host_out[:s2["n_digits"] * 8].copy_(out[:s2["n_digits"] * 8], non_blocking=True)
+            torch.cuda.synchronize()
+        e2e_step()
+        t0 = time.perf_counter()
+        for _ in range(2):
+            e2e_step()
+        x_ms = (time.perf_counter() - t0) * 1e3 / 2
+        e2e = {"value": cells / (x_ms * 1e-3), "unit": "samples/s", "ms_per_step": x_ms,
+               "h2d_bytes_per_step": int(raw.numel() * 2 + ped.numel() * 2), "d2h_bytes_per_step": int(n_dig * 8 + 16)}
+    line = {"metric": "tpc_raw_samples_filtered_per_second", "value": cells / (ms * 1e-3), "unit": "samples/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u16/i32", "data": "synthetic",
+            "config": {"workload": "front-end filter (TPC-FE v1) on the raw samples of config%d: %s" % (
+                           args.config, cfg["label"]), "stage": "fe", "sectors": ns, "planes": n_planes,
+                       "valid_samples": cells, "raw_bytes": int(raw.numel() * 2), "digits_out": n_dig,
+                       "digits_of_the_generator": n_truth, "zs_threshold": zs, "gen_seconds": gen_s,
+                       "l2": "input (%.2f GB) larger than the 126 MB L2; no flush" % (raw.numel() * 2 / 1e9)},
+            "digits_per_s": n_dig / (ms * 1e-3),
+            "roofline": {"bound": "hbm", "kernel": "k_fe_filter", "achieved": alg / (k_ms * 1e-3) / 1e9, "peak": peak,
+                         "unit": "GB/s", "peak_source": peak_src, "frac": alg / (k_ms * 1e-3) / 1e9 / peak,
+                         "traffic": load_traffic("config%d" % args.config, "fe", "k_fe_filter"),
+                         "algorithmic_bytes_per_launch": alg, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms},
+            "cpu_baseline": None, "e2e": e2e, "gpu_launches": flt.last_launch_count() * args.steps,
+            "clocks": clocks.summary()}
+    if not args.no_cpu_baseline:
+        from oracle import fe_oracle as feo
+        feo.build()
+        sp = min(n_planes, 3 * nr)
+        t0 = time.perf_counter()
+        od, ost = feo.run(raw_np[:sp], ped_np[:sp], max(1, sp // nr), nr, mp, nt, npads=npads, planes=(0, sp),
+                          zs_threshold=zs)
+        dt = time.perf_counter() - t0
+        got = out[:ost["n_digits"] * 8].cpu().numpy()
+        if got.tobytes() != od.tobytes():
+            raise RuntimeError("bench: the filter's digits differ from the oracle's on the sample")
+        sc = cells * sp / n_planes if npads is None else int(np.sum(npads)) * nt * (sp // nr)
+        line["cpu_baseline"] = {"value": sc / dt, "unit": "samples/s", "cores": 1, "kind": "oracle",
+                                "sample": "first %d planes (%d samples, %d digits, equal to the GPU's), %.1f s, "
+                                          "single thread" % (sp, sc, ost["n_digits"], dt)}
+    print(json.dumps(line))
+    flt.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -305,9 +425,12 @@ def main():
     ap.add_argument("--variant", default="none", choices=["none", "flags", "cuts"],
                     help="cluster-finder variants (SURVEY.md §8(f) NEXT #1): 'flags' = per-cluster flags, 'cuts' = "
                          "flags + q_tot_min 40 + single-pad cut; the default run has none")
-    ap.add_argument("--stage", default="cf", choices=["cf", "ec"],
+    ap.add_argument("--stage", default="cf", choices=["cf", "ec", "fe"],
                     help="'cf' = the cluster finder (the headline path); 'ec' = the entropy coder of the cluster stream "
-                         "(SURVEY.md §8(f) NEXT #2): encode and decode of the frame's clusters, one JSON line")
+                         "(SURVEY.md §8(f) NEXT #2): encode and decode of the frame's clusters, one JSON line; 'fe' = the "
+                         "front-end filter (NEXT #3) on the frame's raw samples")
+    ap.add_argument("--fe-sectors", type=int, default=0,
+                    help="--stage fe: sectors of the frame to filter (0 = all of the config's)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
@@ -315,6 +438,8 @@ def main():
         return run_reference(args)
     if args.stage == "ec":
         return run_ec(args)
+    if args.stage == "fe":
+        return run_fe(args)
 
     import torch
     import torch.distributed as dist

@@ -82,6 +82,12 @@ int tpc_fe_run(tpc_fe* h, const uint16_t* raw, const uint16_t* ped4, const tpc_f
 /* Kernel launches enqueued by the last run (bench.py's gpu_launches). */
 int tpc_fe_last_launch_count(const tpc_fe* h);
 
+/* Profiling for bench.py's roofline: with on != 0 every run records two events around its dominant kernel
+ * (k_fe_filter) on the run's stream.  tpc_fe_profile_ms waits for the last run's pair and returns the elapsed
+ * milliseconds (a negative value if there is none). */
+int tpc_fe_set_profiling(tpc_fe* h, int on);
+float tpc_fe_profile_ms(tpc_fe* h);
+
 int tpc_fe_destroy(tpc_fe* h);
 
 #ifdef __cplusplus

@@ -25,7 +25,8 @@
 namespace tpcfe {
 
 static constexpr int kTT = 64;          // time bins per tile (the kept-bin mask is 64 bits)
-static constexpr int kStages = 4;       // tiles in the ring: kStages - 1 in flight ahead of the one in work
+static constexpr int kStages = 2;       // tiles in the ring: kStages - 1 in flight ahead of the one in work
+static constexpr int kSlack = 128;      // bytes after the ring: phase 1 may read up to 31 samples past a row's pitch
 static constexpr int kAccShift = 22;    // packed quiet-pad accumulator: count << 22 | sum (|sum| < 2^20)
 
 struct Args {
@@ -69,7 +70,8 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-template <int NW>
+// NW = warps per CTA = ceil(W / 32); WC = W when it is known at compile time (immediate offsets), else 0
+template <int NW, int WC>
 __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -79,7 +81,7 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
     __shared__ uint32_t s_wtot[8];
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    const uint32_t W = a.W, T = a.n_time;
+    const uint32_t W = WC ? (uint32_t)WC : a.W, T = a.n_time;
     const uint32_t tile_elems = kTT * W;
     const uint32_t tpp = (T + kTT - 1) / kTT;                                   // tiles per plane
     const uint32_t my_planes = blockIdx.x < a.n_planes ? (a.n_planes - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
@@ -103,6 +105,9 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
         for (uint32_t m = 0; m < (uint32_t)(kStages - 1) && m < total_tiles; m++) issue(m);
 
     const uint32_t c2 = 2u * a.c;
+    const int kk = (int)a.k, zs = (int)a.zs;
+    int mul = (int)a.mul;
+    asm volatile("" : "+r"(mul));       // keep it in a register (else a predicated constant load per sample)
     const uint32_t bias = (1u << kAccShift) - a.c;
     uint32_t n = 0;                                                             // tile sequence number of this CTA
     for (uint32_t lp = 0; lp < my_planes; lp++) {
@@ -112,12 +117,11 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
         const uint16_t* ped = a.ped4 + (size_t)plane * W;
         const int pedneg2 = active ? 2 - (int)ped[tid] : 0;                     // z + 2 = 4 raw + (2 - ped) - cm + tail
         // phase-1 view: lane handles pads lane + 32 g
-        uint32_t pedq[NW], offs[NW];
+        uint32_t pedq[NW];
 #pragma unroll
         for (int g = 0; g < NW; g++) {
             const uint32_t pad = lane + 32u * g;
-            offs[g] = min(pad, W - 1);
-            pedq[g] = pad < P ? a.c - (uint32_t)ped[pad] : 0x40000000u;         // beyond the row: never quiet
+            pedq[g] = pad < P ? a.c - (uint32_t)ped[min(pad, W - 1)] : 0x40000000u;         // beyond the row: never quiet
         }
         int S = 0;
         uint32_t cnt = 0;       // kept samples of this pad line so far (rank of the next one)
@@ -131,34 +135,38 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
             int* cmv = s_cm[n & 1];
             mbar_wait(&s_bar[n % kStages], (n / kStages) & 1u);
 
-            // ---- (1) common mode of every time bin of the tile: warp `warp` takes bins warp, warp + NW, ...
-            for (uint32_t b0 = 0; b0 * NW + warp < nt; b0 += 32) {
+            // ---- (1) common mode of every time bin of the tile: warp `warp` takes bins warp, warp + NW, ...; lane l
+            // keeps the packed sum of the warp's l-th bin and turns it into cm when 32 bins (or the tile) are done
+            {
+                auto flush = [&](uint32_t b_first, uint32_t n_bins, int mine) {
+                    if (lane < n_bins) {
+                        const uint32_t i = warp + (b_first + lane) * NW;
+                        const int nq = (mine + (1 << (kAccShift - 1))) >> kAccShift;
+                        const int s = mine - (nq << kAccShift);
+                        int cm = 0;
+                        if (nq >= (int)a.m && nq > 0) {
+                            const int num = 2 * s + nq, den = 2 * nq;
+                            cm = num / den;
+                            if (num - cm * den < 0) cm -= 1;                             // floor
+                        }
+                        cmv[i] = cm;
+                    }
+                };
+                uint32_t b = 0;
                 int mine = 0;
-                for (uint32_t b = b0; b < b0 + 32; b++) {
-                    const uint32_t i = b * NW + warp;
-                    if (i >= nt) break;
-                    const uint16_t* row = tile + i * W;
+                for (uint32_t i = warp; i < nt; i += NW, b++) {
+                    const uint16_t* row = tile + i * W + lane;
                     int acc = 0;
 #pragma unroll
                     for (int g = 0; g < NW; g++) {
-                        const uint32_t xb = (uint32_t)row[offs[g]] * 4u + pedq[g];   // x + c
-                        if (xb <= c2) acc += (int)(xb + bias);                       // x + 2^22
+                        const uint32_t xb = (uint32_t)row[32 * g] * 4u + pedq[g];        // x + c
+                        acc += xb <= c2 ? (int)(xb + bias) : 0;                          // x + 2^22
                     }
                     acc = __reduce_add_sync(0xffffffffu, acc);
-                    if (lane == b - b0) mine = acc;
+                    if (lane == (b & 31u)) mine = acc;
+                    if ((b & 31u) == 31u) { flush(b - 31u, 32u, mine); mine = 0; }
                 }
-                const uint32_t i = (b0 + lane) * NW + warp;
-                if (i < nt) {
-                    const int nq = (mine + (1 << (kAccShift - 1))) >> kAccShift;
-                    const int s = mine - (nq << kAccShift);
-                    int cm = 0;
-                    if (nq >= (int)a.m && nq > 0) {
-                        const int num = 2 * s + nq, den = 2 * nq;
-                        cm = num / den;
-                        if (num - cm * den < 0) cm -= 1;                             // floor
-                    }
-                    cmv[i] = cm;
-                }
+                if (b & 31u) flush(b & ~31u, b & 31u, mine);
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // this thread's q stores into tile n - 1
             __syncthreads();
@@ -177,11 +185,11 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
 #pragma unroll
                         for (int u = 0; u < 4; u++) {
                             const int i = i4 + u;
-                            const int z2 = (int)cell[i * W] * 4 + pedneg2 - cma[u] + (S >> 12);
-                            const int q = min(z2 >> 2, 65535);
-                            S -= S >> a.k;
-                            if (q >= (int)a.zs) {
-                                S += q * (int)a.mul;
+                            const int base = (int)cell[i * W] * 4 + (pedneg2 - cma[u]);     // independent of S
+                            const int q = min((base + (S >> 12)) >> 2, 65535);
+                            S -= S >> kk;
+                            if (q >= zs) {
+                                S += q * mul;
                                 cell[i * W] = (uint16_t)q;
                                 if (i < 32) mlo |= 1u << i; else mhi |= 1u << (i - 32);
                             }
@@ -189,11 +197,11 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
                     }
                 } else {
                     for (uint32_t i = 0; i < nt; i++) {
-                        const int z2 = (int)cell[i * W] * 4 + pedneg2 - cmv[i] + (S >> 12);
-                        const int q = min(z2 >> 2, 65535);
-                        S -= S >> a.k;
-                        if (q >= (int)a.zs) {
-                            S += q * (int)a.mul;
+                        const int base = (int)cell[i * W] * 4 + (pedneg2 - cmv[i]);
+                        const int q = min((base + (S >> 12)) >> 2, 65535);
+                        S -= S >> kk;
+                        if (q >= zs) {
+                            S += q * mul;
                             cell[i * W] = (uint16_t)q;
                             if (i < 32) mlo |= 1u << i; else mhi |= 1u << (i - 32);
                         }
@@ -332,6 +340,8 @@ struct tpc_fe {
     uint32_t* flags;
     uint32_t grid, smem;
     int last_launches;
+    int profiling, have_pair;
+    cudaEvent_t ev0, ev1;
 };
 
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -369,14 +379,14 @@ extern "C" size_t tpc_fe_workspace_bytes(const tpc_cf_geometry* g, uint64_t max_
                  nullptr);
 }
 
-template <int NW>
+template <int NW, int WC>
 static void setup_kernel(tpc_fe* e)
 {
     int dev = 0, sms = 148, per_sm = 1;
-    if (cudaFuncSetAttribute(k_fe_filter<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e->smem) != cudaSuccess ||
+    if (cudaFuncSetAttribute(k_fe_filter<NW, WC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e->smem) != cudaSuccess ||
         cudaGetDevice(&dev) != cudaSuccess ||
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fe_filter<NW>, NW * 32, e->smem) != cudaSuccess) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fe_filter<NW, WC>, NW * 32, e->smem) != cudaSuccess) {
         cudaGetLastError();      // no device (host-only tests): the launch will report it
         sms = 148; per_sm = 1;
     }
@@ -398,6 +408,7 @@ extern "C" int tpc_fe_create(tpc_fe** h, const tpc_cf_geometry* g, uint64_t max_
     if (!e) return TPC_CF_E_NOMEM;
     e->n_sectors = g->n_sectors; e->n_rows = g->n_rows; e->max_pads = g->max_pads; e->n_time = g->n_time;
     e->W = W; e->n_planes = n_planes; e->cap = max_digits_per_plane; e->last_launches = 0;
+    e->profiling = 0; e->have_pair = 0; e->ev0 = nullptr; e->ev1 = nullptr;
     carve(n_planes, g->n_rows, W, max_digits_per_plane, (char*)workspace, e);
     uint32_t np[256];
     for (uint32_t r = 0; r < g->n_rows; r++) np[r] = g->npads ? g->npads[r] : g->max_pads;
@@ -406,16 +417,16 @@ extern "C" int tpc_fe_create(tpc_fe** h, const tpc_cf_geometry* g, uint64_t max_
         delete e;
         return TPC_CF_E_CUDA;
     }
-    e->smem = (uint32_t)(kStages * kTT * W * 2u);
+    e->smem = (uint32_t)(kStages * kTT * W * 2u) + kSlack;
     switch ((W + 31) / 32) {
-        case 1: setup_kernel<1>(e); break;
-        case 2: setup_kernel<2>(e); break;
-        case 3: setup_kernel<3>(e); break;
-        case 4: setup_kernel<4>(e); break;
-        case 5: setup_kernel<5>(e); break;
-        case 6: setup_kernel<6>(e); break;
-        case 7: setup_kernel<7>(e); break;
-        default: setup_kernel<8>(e); break;
+        case 1: setup_kernel<1, 0>(e); break;
+        case 2: setup_kernel<2, 0>(e); break;
+        case 3: setup_kernel<3, 0>(e); break;
+        case 4: setup_kernel<4, 0>(e); break;
+        case 5: if (W == 144) setup_kernel<5, 144>(e); else setup_kernel<5, 0>(e); break;
+        case 6: setup_kernel<6, 0>(e); break;
+        case 7: setup_kernel<7, 0>(e); break;
+        default: setup_kernel<8, 0>(e); break;
     }
     *h = e;
     return TPC_CF_OK;
@@ -438,16 +449,21 @@ extern "C" int tpc_fe_run(tpc_fe* h, const uint16_t* raw, const uint16_t* ped4, 
     a.cap = (uint32_t)h->cap; a.temp = h->temp; a.line_cnt = h->line_cnt; a.plane_cnt = h->plane_cnt; a.flags = h->flags;
     cudaMemsetAsync(h->flags, 0, 16, st);
     const uint32_t grid = h->grid < h->n_planes ? h->grid : h->n_planes;
+    if (h->profiling) cudaEventRecord(h->ev0, st);
     switch ((h->W + 31) / 32) {
-        case 1: k_fe_filter<1><<<grid, 32, h->smem, st>>>(a); break;
-        case 2: k_fe_filter<2><<<grid, 64, h->smem, st>>>(a); break;
-        case 3: k_fe_filter<3><<<grid, 96, h->smem, st>>>(a); break;
-        case 4: k_fe_filter<4><<<grid, 128, h->smem, st>>>(a); break;
-        case 5: k_fe_filter<5><<<grid, 160, h->smem, st>>>(a); break;
-        case 6: k_fe_filter<6><<<grid, 192, h->smem, st>>>(a); break;
-        case 7: k_fe_filter<7><<<grid, 224, h->smem, st>>>(a); break;
-        default: k_fe_filter<8><<<grid, 256, h->smem, st>>>(a); break;
+        case 1: k_fe_filter<1, 0><<<grid, 32, h->smem, st>>>(a); break;
+        case 2: k_fe_filter<2, 0><<<grid, 64, h->smem, st>>>(a); break;
+        case 3: k_fe_filter<3, 0><<<grid, 96, h->smem, st>>>(a); break;
+        case 4: k_fe_filter<4, 0><<<grid, 128, h->smem, st>>>(a); break;
+        case 5:
+            if (h->W == 144) k_fe_filter<5, 144><<<grid, 160, h->smem, st>>>(a);
+            else k_fe_filter<5, 0><<<grid, 160, h->smem, st>>>(a);
+            break;
+        case 6: k_fe_filter<6, 0><<<grid, 192, h->smem, st>>>(a); break;
+        case 7: k_fe_filter<7, 0><<<grid, 224, h->smem, st>>>(a); break;
+        default: k_fe_filter<8, 0><<<grid, 256, h->smem, st>>>(a); break;
     }
+    if (h->profiling) { cudaEventRecord(h->ev1, st); h->have_pair = 1; }
     k_fe_scan<<<1, 1024, 0, st>>>(h->plane_cnt, h->n_planes, h->plane_off, h->flags);
     k_fe_order<<<h->n_planes, 256, 0, st>>>(h->temp, (uint32_t)h->cap, h->line_cnt, h->plane_cnt, h->plane_off, h->W,
                                             h->n_rows, (uint2*)out, capacity, h->flags, status);
@@ -457,9 +473,36 @@ extern "C" int tpc_fe_run(tpc_fe* h, const uint16_t* raw, const uint16_t* ped4, 
 
 extern "C" int tpc_fe_last_launch_count(const tpc_fe* h) { return h ? h->last_launches : 0; }
 
+extern "C" int tpc_fe_set_profiling(tpc_fe* h, int on)
+{
+    if (!h) return TPC_CF_E_NULL;
+    if (on && !h->ev0) {
+        if (cudaEventCreate(&h->ev0) != cudaSuccess || cudaEventCreate(&h->ev1) != cudaSuccess) {
+            cudaGetLastError();
+            return TPC_CF_E_CUDA;
+        }
+    }
+    h->profiling = on ? 1 : 0;
+    if (!on) h->have_pair = 0;
+    return TPC_CF_OK;
+}
+
+extern "C" float tpc_fe_profile_ms(tpc_fe* h)
+{
+    if (!h || !h->have_pair) return -1.0f;
+    float ms = -1.0f;
+    if (cudaEventSynchronize(h->ev1) != cudaSuccess || cudaEventElapsedTime(&ms, h->ev0, h->ev1) != cudaSuccess) {
+        cudaGetLastError();
+        return -1.0f;
+    }
+    return ms;
+}
+
 extern "C" int tpc_fe_destroy(tpc_fe* h)
 {
     if (!h) return TPC_CF_E_NULL;
+    if (h->ev0) cudaEventDestroy(h->ev0);
+    if (h->ev1) cudaEventDestroy(h->ev1);
     delete h;
     return TPC_CF_OK;
 }

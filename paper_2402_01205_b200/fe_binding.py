@@ -16,7 +16,7 @@ FE_OVF_PLANE, FE_OVF_OUTPUT = 1, 2
 FE_DEFAULTS = dict(zs_threshold=2, cm_quiet4=12, cm_min_pads=8, it_decay_shift=6, it_kappa_shift=8)
 
 FE_EXPORTS = ["tpc_fe_pad_stride", "tpc_fe_workspace_bytes", "tpc_fe_create", "tpc_fe_run", "tpc_fe_last_launch_count",
-              "tpc_fe_destroy"]
+              "tpc_fe_set_profiling", "tpc_fe_profile_ms", "tpc_fe_destroy"]
 
 
 class FeParams(ctypes.Structure):
@@ -42,6 +42,10 @@ def _lib():
         lib.tpc_fe_run.argtypes = [vp, vp, vp, ctypes.POINTER(FeParams), vp, u64, vp, vp]
         lib.tpc_fe_last_launch_count.restype = ctypes.c_int
         lib.tpc_fe_last_launch_count.argtypes = [vp]
+        lib.tpc_fe_set_profiling.restype = ctypes.c_int
+        lib.tpc_fe_set_profiling.argtypes = [vp, ctypes.c_int]
+        lib.tpc_fe_profile_ms.restype = ctypes.c_float
+        lib.tpc_fe_profile_ms.argtypes = [vp]
         lib.tpc_fe_destroy.restype = ctypes.c_int
         lib.tpc_fe_destroy.argtypes = [vp]
         _typed = True
@@ -118,6 +122,13 @@ class FrontEndFilter:
 
     def last_launch_count(self):
         return int(_lib().tpc_fe_last_launch_count(self.h))
+
+    def set_profiling(self, on):
+        _check(_lib().tpc_fe_set_profiling(self.h, 1 if on else 0))
+
+    def profile_ms(self):
+        """milliseconds of the dominant kernel (k_fe_filter) in the last run; waits for it"""
+        return float(_lib().tpc_fe_profile_ms(self.h))
 
     def close(self):
         if getattr(self, "h", None) is not None:
