@@ -48,7 +48,9 @@ typedef struct {
 } tpc_fe_params;
 
 enum {
-    TPC_FE_OVF_PLANE = 1u,    /* a plane kept more samples than max_digits_per_plane: output incomplete */
+    TPC_FE_OVF_PLANE = 1u,    /* a plane's staging area overflowed: output incomplete.  The area of max_digits_per_plane
+                                 records is shared evenly by the plane's groups of 32 pads (ceil(W / 32) of them), so
+                                 size it for the densest group: 2x the expected digits per plane is plenty */
     TPC_FE_OVF_OUTPUT = 2u    /* more digits than `capacity`: only records below `capacity` are written */
 };
 
@@ -65,7 +67,7 @@ typedef struct tpc_fe tpc_fe;   /* opaque handle: host state only */
 uint32_t tpc_fe_pad_stride(uint32_t max_pads);
 
 /* Bytes of DEVICE workspace: per plane a staging area of max_digits_per_plane 8-byte records, per pad line a count,
- * per plane a count and an offset.  0 on invalid arguments. */
+ * per plane eight group counts and an offset.  0 on invalid arguments. */
 size_t tpc_fe_workspace_bytes(const tpc_cf_geometry* g, uint64_t max_digits_per_plane);
 
 /* workspace: DEVICE, 256-byte aligned, >= tpc_fe_workspace_bytes.  Geometry limits as in tpc_cf.h.

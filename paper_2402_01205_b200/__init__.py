@@ -15,7 +15,9 @@ from .ec_binding import (EC_ERR_CAPACITY, EC_ERR_CONTAINER, EC_ERR_QTOT, EC_ERR_
 from .fe_binding import (FE_DEFAULTS, FE_EXPORTS, FE_OVF_OUTPUT, FE_OVF_PLANE, FE_STATUS, FeParams, FrontEndFilter,
                          tpc_fe_create, tpc_fe_destroy, tpc_fe_pad_stride, tpc_fe_run, tpc_fe_workspace_bytes)
 
-__all__ = ["FE_DEFAULTS", "FE_EXPORTS", "FE_OVF_OUTPUT", "FE_OVF_PLANE", "FE_STATUS", "FeParams", "FrontEndFilter",
+from .shard import ShardedClusterFinder, gather_records, plane_counts, plane_partition
+
+__all__ = ["ShardedClusterFinder", "gather_records", "plane_counts", "plane_partition", "FE_DEFAULTS", "FE_EXPORTS", "FE_OVF_OUTPUT", "FE_OVF_PLANE", "FE_STATUS", "FeParams", "FrontEndFilter",
            "tpc_fe_create", "tpc_fe_destroy", "tpc_fe_pad_stride", "tpc_fe_run", "tpc_fe_workspace_bytes",
            "EC_ERR_CAPACITY", "EC_ERR_CONTAINER", "EC_ERR_QTOT", "EC_ERR_UNSORTED", "EC_EXPORTS", "EC_STATUS",
            "ClusterCoder", "clusters_to_device", "tpc_ec_create", "tpc_ec_decode", "tpc_ec_destroy", "tpc_ec_encode",

@@ -38,7 +38,7 @@ struct Args {
     uint32_t cap;               // staged records per plane
     uint2* temp;                // [n_planes][cap]
     uint32_t* line_cnt;         // [n_planes][W]
-    uint32_t* plane_cnt;        // [n_planes]
+    uint32_t* warp_cnt;         // [n_planes][8]: kept samples of the pads of warp w (pads 32 w .. 32 w + 31)
     uint32_t* flags;
 };
 
@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
     uint16_t* tiles = (uint16_t*)smem;                    // [kStages][kTT * W]
     __shared__ __align__(8) unsigned long long s_bar[kStages];
     __shared__ __align__(16) int s_cm[2][kTT];
-    __shared__ uint32_t s_wtot[8];
+    __shared__ int s_mul;
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t W = WC ? (uint32_t)WC : a.W, T = a.n_time;
@@ -88,6 +88,7 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
     const uint32_t total_tiles = my_planes * tpp;
 
     if (tid == 0) {
+        s_mul = (int)a.mul;
         for (int s = 0; s < kStages; s++) mbar_init(&s_bar[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -105,9 +106,11 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
         for (uint32_t m = 0; m < (uint32_t)(kStages - 1) && m < total_tiles; m++) issue(m);
 
     const uint32_t c2 = 2u * a.c;
+    const uint32_t capw = a.cap / NW;                                           // staged records per warp and plane
     const int kk = (int)a.k, zs = (int)a.zs;
-    int mul = (int)a.mul;
-    asm volatile("" : "+r"(mul));       // keep it in a register (else a predicated constant load per sample)
+    // read back from shared memory so that it lives in a register (else the compiler reloads it from the constant bank,
+    // predicated, once per sample)
+    const int mul = *(volatile int*)&s_mul;
     const uint32_t bias = (1u << kAccShift) - a.c;
     uint32_t n = 0;                                                             // tile sequence number of this CTA
     for (uint32_t lp = 0; lp < my_planes; lp++) {
@@ -125,8 +128,8 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
         }
         int S = 0;
         uint32_t cnt = 0;       // kept samples of this pad line so far (rank of the next one)
-        uint32_t pos = 0;       // kept samples of the plane so far (same value in every thread)
-        uint2* temp = a.temp + (size_t)plane * a.cap;
+        uint32_t wpos = 0;      // kept samples of this warp's pads so far (same value in every lane)
+        uint2* wtemp = a.temp + (size_t)plane * a.cap + (size_t)warp * capw;
 
         for (uint32_t tl = 0; tl < tpp; tl++, n++) {
             const uint32_t t0 = tl * kTT;
@@ -209,51 +212,47 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
                 }
             }
 
-            // ---- (3) place the tile's records: block scan of the kept counts
-            const uint32_t c = __popc(mlo) + __popc(mhi);
-            uint32_t incl = c;
+            // ---- (3) place the tile's records in the warp's part of the plane's staging area: a warp scan of the
+            // kept counts, no block barrier (k_fe_order finds every record by its pad and rank, not by its place)
+            {
+                const uint32_t c = __popc(mlo) + __popc(mhi);
+                uint32_t incl = c;
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
-                if (lane >= (uint32_t)d) incl += v;
+                for (int d = 1; d < 32; d <<= 1) {
+                    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
+                    if (lane >= (uint32_t)d) incl += v;
+                }
+                const uint32_t wtotal = __shfl_sync(0xffffffffu, incl, 31);
+                const uint32_t idx = wpos + incl - c;
+                wpos += wtotal;
+                if (c) {
+                    const uint32_t n_ok = idx >= capw ? 0u : min(c, capw - idx);     // records that still fit
+                    uint2* dst = wtemp + idx;
+                    const uint32_t cell_addr = smem_u32(tile + tid);
+                    uint32_t w0 = tid | (cnt << 8), j = 0;
+                    auto put = [&](uint32_t i) {
+                        uint32_t q;
+                        asm volatile("ld.shared.u16 %0, [%1];" : "=r"(q) : "r"(cell_addr + i * (W * 2u)));
+                        if (j < n_ok) dst[j] = make_uint2(w0, (t0 + i) | (q << 16));
+                        j++; w0 += 256u;
+                    };
+                    while (mlo) { put(__ffs(mlo) - 1); mlo &= mlo - 1; }
+                    while (mhi) { put(__ffs(mhi) + 31); mhi &= mhi - 1; }
+                    cnt += c;
+                }
             }
-            if (lane == 31) s_wtot[warp] = incl;
-            __syncthreads();
-            uint32_t before = 0, tile_total = 0;
-#pragma unroll
-            for (int w = 0; w < NW; w++) {
-                const uint32_t v = s_wtot[w];
-                if ((uint32_t)w < warp) before += v;
-                tile_total += v;
-            }
-            uint32_t idx = pos + before + incl - c;
-            uint32_t rank = cnt;
-            const uint16_t* cell = tile + tid;
-            while (mlo) {
-                const uint32_t i = __ffs(mlo) - 1;
-                mlo &= mlo - 1;
-                if (idx < a.cap) temp[idx] = make_uint2(tid | (rank << 8), (t0 + i) | ((uint32_t)cell[i * W] << 16));
-                idx++; rank++;
-            }
-            while (mhi) {
-                const uint32_t i = __ffs(mhi) + 31;
-                mhi &= mhi - 1;
-                if (idx < a.cap) temp[idx] = make_uint2(tid | (rank << 8), (t0 + i) | ((uint32_t)cell[i * W] << 16));
-                idx++; rank++;
-            }
-            cnt = rank;
-            pos += tile_total;
         }
         if (tid < W) a.line_cnt[(size_t)plane * W + tid] = cnt;
-        if (tid == 0) {
-            a.plane_cnt[plane] = pos;
-            if (pos > a.cap) atomicOr(a.flags, (uint32_t)TPC_FE_OVF_PLANE);
+        if (lane == 0) {
+            a.warp_cnt[(size_t)plane * 8 + warp] = wpos;
+            if (wpos > capw) atomicOr(a.flags, (uint32_t)TPC_FE_OVF_PLANE);
         }
+        if (tid >= NW && tid < 8) a.warp_cnt[(size_t)plane * 8 + tid] = 0;
     }
 }
 
 // exclusive scan of the plane counts (one CTA), status
-__global__ void __launch_bounds__(1024) k_fe_scan(const uint32_t* plane_cnt, uint32_t n_planes, uint64_t* plane_off,
+__global__ void __launch_bounds__(1024) k_fe_scan(const uint32_t* warp_cnt, uint32_t n_planes, uint64_t* plane_off,
                                                   uint32_t* flags)
 {
     __shared__ uint64_t s_w[32];
@@ -263,7 +262,11 @@ __global__ void __launch_bounds__(1024) k_fe_scan(const uint32_t* plane_cnt, uin
     __syncthreads();
     for (uint32_t b = 0; b < n_planes; b += 1024) {
         const uint32_t i = b + tid;
-        const uint64_t v = i < n_planes ? plane_cnt[i] : 0;
+        uint64_t v = 0;
+        if (i < n_planes) {
+            const uint4 a4 = ((const uint4*)warp_cnt)[2 * (size_t)i], b4 = ((const uint4*)warp_cnt)[2 * (size_t)i + 1];
+            v = (uint64_t)a4.x + a4.y + a4.z + a4.w + b4.x + b4.y + b4.z + b4.w;
+        }
         uint64_t incl = v;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -284,7 +287,7 @@ __global__ void __launch_bounds__(1024) k_fe_scan(const uint32_t* plane_cnt, uin
 
 // one CTA per plane: staged records -> their place in the sorted output
 __global__ void __launch_bounds__(256) k_fe_order(const uint2* temp_all, uint32_t cap, const uint32_t* line_cnt,
-                                                  const uint32_t* plane_cnt, const uint64_t* plane_off, uint32_t W,
+                                                  const uint32_t* warp_cnt, const uint64_t* plane_off, uint32_t W,
                                                   uint32_t n_rows, uint2* out, uint64_t capacity, uint32_t* flags,
                                                   tpc_fe_status* status)
 {
@@ -304,15 +307,18 @@ __global__ void __launch_bounds__(256) k_fe_order(const uint2* temp_all, uint32_
     for (uint32_t w = 0; w < warp; w++) before += s_w[w];
     s_off[tid] = before + incl - v;
     __syncthreads();
-    const uint32_t n = min(plane_cnt[plane], cap);
     const uint64_t base = plane_off[plane];
-    const uint2* temp = temp_all + (size_t)plane * cap;
     const uint32_t head = (plane / n_rows) | ((plane % n_rows) << 8);
-    for (uint32_t i = tid; i < n; i += 256) {
-        const uint2 r = temp[i];
-        const uint32_t pad = r.x & 255u;
-        const uint64_t dst = base + s_off[pad] + (r.x >> 8);
-        if (dst < capacity) out[dst] = make_uint2(head | (pad << 16), r.y);
+    const uint32_t nw = (W + 31) / 32, capw = cap / nw;
+    for (uint32_t w = 0; w < nw; w++) {
+        const uint32_t n = min(warp_cnt[(size_t)plane * 8 + w], capw);
+        const uint2* temp = temp_all + (size_t)plane * cap + (size_t)w * capw;
+        for (uint32_t i = tid; i < n; i += 256) {
+            const uint2 r = temp[i];
+            const uint32_t pad = r.x & 255u;
+            const uint64_t dst = base + s_off[pad] + (r.x >> 8);
+            if (dst < capacity) out[dst] = make_uint2(head | (pad << 16), r.y);
+        }
     }
     // the status is written last: by the CTA that finishes last
     __threadfence();
@@ -334,7 +340,7 @@ struct tpc_fe {
     uint64_t cap;
     uint2* temp;
     uint32_t* line_cnt;
-    uint32_t* plane_cnt;
+    uint32_t* warp_cnt;
     uint64_t* plane_off;
     uint32_t* npads;
     uint32_t* flags;
@@ -353,7 +359,7 @@ static size_t carve(uint32_t n_planes, uint32_t n_rows, uint32_t W, uint64_t cap
     char* p;
     p = take(256);                                   if (e) e->flags = (uint32_t*)p;
     p = take(4ull * n_rows);                         if (e) e->npads = (uint32_t*)p;
-    p = take(4ull * n_planes);                       if (e) e->plane_cnt = (uint32_t*)p;
+    p = take(32ull * n_planes);                      if (e) e->warp_cnt = (uint32_t*)p;
     p = take(8ull * n_planes);                       if (e) e->plane_off = (uint64_t*)p;
     p = take(4ull * n_planes * W);                   if (e) e->line_cnt = (uint32_t*)p;
     p = take(8ull * n_planes * cap);                 if (e) e->temp = (uint2*)p;
@@ -446,7 +452,7 @@ extern "C" int tpc_fe_run(tpc_fe* h, const uint16_t* raw, const uint16_t* ped4, 
     a.n_planes = h->n_planes; a.n_rows = h->n_rows; a.n_time = h->n_time; a.W = h->W;
     a.zs = p->zs_threshold; a.c = p->cm_quiet4; a.m = p->cm_min_pads; a.k = (uint32_t)k;
     a.mul = j ? 1u << (14 - j) : 0u;
-    a.cap = (uint32_t)h->cap; a.temp = h->temp; a.line_cnt = h->line_cnt; a.plane_cnt = h->plane_cnt; a.flags = h->flags;
+    a.cap = (uint32_t)h->cap; a.temp = h->temp; a.line_cnt = h->line_cnt; a.warp_cnt = h->warp_cnt; a.flags = h->flags;
     cudaMemsetAsync(h->flags, 0, 16, st);
     const uint32_t grid = h->grid < h->n_planes ? h->grid : h->n_planes;
     if (h->profiling) cudaEventRecord(h->ev0, st);
@@ -464,8 +470,8 @@ extern "C" int tpc_fe_run(tpc_fe* h, const uint16_t* raw, const uint16_t* ped4, 
         default: k_fe_filter<8, 0><<<grid, 256, h->smem, st>>>(a); break;
     }
     if (h->profiling) { cudaEventRecord(h->ev1, st); h->have_pair = 1; }
-    k_fe_scan<<<1, 1024, 0, st>>>(h->plane_cnt, h->n_planes, h->plane_off, h->flags);
-    k_fe_order<<<h->n_planes, 256, 0, st>>>(h->temp, (uint32_t)h->cap, h->line_cnt, h->plane_cnt, h->plane_off, h->W,
+    k_fe_scan<<<1, 1024, 0, st>>>(h->warp_cnt, h->n_planes, h->plane_off, h->flags);
+    k_fe_order<<<h->n_planes, 256, 0, st>>>(h->temp, (uint32_t)h->cap, h->line_cnt, h->warp_cnt, h->plane_off, h->W,
                                             h->n_rows, (uint2*)out, capacity, h->flags, status);
     h->last_launches = 3;
     return cudaGetLastError() == cudaSuccess ? TPC_CF_OK : TPC_CF_E_CUDA;

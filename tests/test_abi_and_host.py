@@ -70,7 +70,7 @@ def test_front_end_filter_host_logic_without_a_device():
     g, keep = cf.make_geometry(36, 152, 138, 14336)
     w = cf.tpc_fe_workspace_bytes(g, 65536)
     planes = 36 * 152
-    assert 8 * planes * 65536 + 4 * planes * 144 < w < 8 * planes * 65536 + 4 * planes * 144 + 16 * planes + 4096
+    assert 8 * planes * 65536 + 4 * planes * 144 < w < 8 * planes * 65536 + 4 * planes * 144 + 48 * planes + 4096
     assert cf.tpc_fe_workspace_bytes(g, 0) == 0 and cf.tpc_fe_workspace_bytes(g, 1 << 32) == 0
     bad, _ = cf.make_geometry(36, 152, 256, 14336)
     assert cf.tpc_fe_workspace_bytes(bad, 100) == 0
@@ -289,3 +289,79 @@ def test_replica_sharding_world_size_2_gloo(tmp_path):
     n0 = gen.generate(1, frame=0).shape[0]
     n1 = gen.generate(1, frame=1).shape[0]
     assert res["tmax"] == 11.0 and res["digits"] == n0 + n1 and res["own"] == n0 and n0 != n1
+
+
+# ---- N > 1, latency mode: one frame cut into plane ranges -------------------------------
+
+def test_plane_partition_is_contiguous_complete_and_balanced():
+    import paper_2402_01205_b200 as cf
+    from datagen import gen
+    c = dict(gen.CONFIGS[1])
+    d = gen.generate(c)
+    ns, nr = c["n_sectors"], c["n_rows"]
+    ps = cf.plane_counts(d, ns, nr)
+    assert ps.shape == (ns * nr + 1,) and ps[0] == 0 and ps[-1] == d.shape[0] and np.all(np.diff(ps) >= 0)
+    key = d["sector"].astype(np.int64) * nr + d["row"]
+    assert np.array_equal(np.diff(ps), np.bincount(key, minlength=ns * nr))
+    biggest = int(np.diff(ps).max())
+    for world in (1, 2, 3, 8, 200):
+        part = cf.plane_partition(ps, world)
+        assert len(part) == world and part[0][0] == 0 and part[-1][1] == ns * nr
+        for a, b in zip(part, part[1:]):
+            assert a[1] == b[0] and a[3] == b[2]                          # contiguous in planes and in digits
+        for (pb, pe, db, de) in part:
+            assert pb <= pe and db == ps[pb] and de == ps[pe]
+            assert de - db <= d.shape[0] // world + biggest + 1            # balanced up to one plane
+    # degenerate inputs: no digits at all, everything in one plane
+    assert cf.plane_partition(np.zeros(11, dtype=np.int64), 3)[-1][1] == 10
+    one = np.zeros(11, dtype=np.int64)
+    one[4:] = 1000
+    part = cf.plane_partition(one, 4)
+    assert sum(p[3] - p[2] for p in part) == 1000 and max(p[3] - p[2] for p in part) == 1000
+
+
+_SHARD_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %(root)r)
+import numpy as np
+import torch, torch.distributed as dist
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%(port)d", rank=int(sys.argv[1]), world_size=2)
+rank = dist.get_rank()
+from datagen import gen
+from oracle import oracle as orc
+from paper_2402_01205_b200.shard import plane_counts, plane_partition, gather_records
+cfg = dict(gen.CONFIGS[1])
+g = gen.geometry(cfg)
+d = gen.generate(cfg)
+part = plane_partition(plane_counts(d, g[0], g[1]), 2)[rank]
+# the rank's compute step: here the CPU oracle stands in for the CUDA cluster finder (no GPU in this test)
+mine = d[part[2]:part[3]]
+cl, st = orc.run(mine, *g[:4], planes=(part[0], part[1]))
+local = torch.from_numpy(cl.view(np.uint8).copy())
+out, counts = gather_records(local, cl.shape[0], 32, 0)
+if rank == 0:
+    whole, wst = orc.run(d, *g[:4])
+    same = out.numpy().tobytes() == whole.tobytes()
+    print(json.dumps({"same": bool(same), "counts": counts, "total": int(wst["n_clusters"]), "part": list(part)}))
+else:
+    assert out is None
+dist.barrier()
+dist.destroy_process_group()
+"""
+
+
+def test_sector_sharded_frame_world_size_2_gloo(tmp_path):
+    """Latency mode: the frame's planes are cut into two contiguous ranges balanced by digit count, every rank
+    processes its slice alone, and the variable-size gather in rank order gives exactly the single-rank result
+    (planes are independent, R2).  gloo backend on CPU; the oracle stands in for the per-rank CUDA step."""
+    port = 31500 + (os.getpid() % 2000)
+    script = tmp_path / "shard_worker.py"
+    script.write_text(_SHARD_WORKER % {"root": ROOT, "port": port})
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE, stderr=subprocess.PIPE,
+                              text=True) for r in range(2)]
+    outs = [p.communicate(timeout=300) for p in procs]
+    for p, (o, e) in zip(procs, outs):
+        assert p.returncode == 0, e[-2000:]
+    import json
+    res = json.loads(outs[0][0].strip().splitlines()[-1])
+    assert res["same"] and sum(res["counts"]) == res["total"] and min(res["counts"]) > 0.4 * res["total"]

@@ -20,7 +20,7 @@ def gpu_run(raw, ped4, ns, nr, mp, nt, npads=None, cap_plane=None, capacity=None
     own = flt is None
     if own:
         flt = cf.FrontEndFilter(ns, nr, mp, nt, npads=npads,
-                                max_digits_per_plane=cap_plane if cap_plane else max(1, nt * mp))
+                                max_digits_per_plane=cap_plane if cap_plane else nt * ((mp + 31) // 32 * 32))   # every group of 32 pads may keep all
     r = torch.from_numpy(np.ascontiguousarray(raw).view(np.int16)).cuda()
     p = torch.from_numpy(np.ascontiguousarray(ped4).view(np.int16)).cuda()
     cap = capacity if capacity is not None else ns * nr * nt * mp
