@@ -292,6 +292,80 @@ def run_ec(args):
     return 0
 
 
+def run_shard(args):
+    """--shard: one frame over the N ranks (paper_2402_01205_b200/shard.py).  A step = every rank's tpc_cf_run on its
+    plane range + the variable-size gather of the clusters into rank 0; time = max over ranks; value = the frame's
+    digits / that time (strong scaling: the total work is fixed)."""
+    import torch
+    import torch.distributed as dist
+    from datagen import gen
+    import paper_2402_01205_b200 as cf
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = "cuda:%d" % local_rank
+    if not dist.is_initialized():
+        if world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", str(29400 + os.getpid() % 500))
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device(dev))
+    cfg = gen.CONFIGS[args.config]
+    geom = gen.geometry(args.config)
+    digits = gen.generate(args.config)                                  # every rank generates the same frame
+    part = cf.plane_partition(cf.plane_counts(digits, geom[0], geom[1]), world)[rank]
+    mine = digits[part[2]:part[3]]
+    n = int(mine.shape[0])
+    finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=max(n, 1), max_clusters=n // 10 + 1024, device=dev)
+    d = cf.to_device(mine, device=dev)
+    n_cl = [0]
+
+    def step():
+        finder.run(d, n, flags=cf.DIGITS_SORTED)
+        st = finder.status.cpu().numpy().view(cf.STATUS)[0]              # the count decides the transfer size
+        n_cl[0] = int(st["n_clusters"])
+        return cf.gather_records(finder.clusters, n_cl[0], 32, 0)
+
+    sampler = ClockSampler(local_rank).start()
+    for _ in range(args.warmup):
+        out, counts = step()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist.barrier()
+    torch.cuda.synchronize()
+    with sampler as clocks:
+        ev0.record()
+        for _ in range(args.steps):
+            out, counts = step()
+        ev1.record()
+        torch.cuda.synchronize()
+    dist.barrier()
+    t = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item()) / args.steps
+    if rank == 0:
+        nd = int(digits.shape[0])
+        peak, peak_src = load_peaks()
+        line = {"metric": METRIC, "value": nd / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": "u16/i32/f32", "data": "synthetic",
+                "config": {"workload": "config%d: %s" % (args.config, cfg["label"]), "mode": "shard (one frame over the "
+                           "ranks, contiguous plane ranges balanced by digits, clusters gathered into rank 0)",
+                           "digits_per_frame": nd, "clusters_per_frame": int(sum(counts)),
+                           "clusters_per_rank": counts, "rank0_planes": list(part[:2]),
+                           "l2": "inputs larger than the 126 MB L2; no flush", "parallelism": "shard x%d" % world},
+                "clusters_per_s": sum(counts) / (ms * 1e-3),
+                "f_io": {"value": (8.0 * nd + 32.0 * sum(counts)) / (ms * 1e-3) / 1e9 / (peak * world),
+                         "note": "compulsory I/O / time / (peak x ranks)"},
+                "roofline": None, "cpu_baseline": None, "e2e": None,
+                "gpu_launches": finder.last_launch_count() * args.steps, "clocks": clocks.summary()}
+        print(json.dumps(line))
+    finder.close()
+    dist.destroy_process_group()
+    return 0
+
+
 def run_fe(args):
     """--stage fe: the front-end filter (include/tpc_fe.h) on the raw samples of one frame of the chosen config
     (datagen/fe_gen.py's forward model over the config's digits).  One GPU.  A step = one tpc_fe_run (all its kernels)
@@ -429,6 +503,10 @@ def main():
                     help="'cf' = the cluster finder (the headline path); 'ec' = the entropy coder of the cluster stream "
                          "(SURVEY.md §8(f) NEXT #2): encode and decode of the frame's clusters, one JSON line; 'fe' = the "
                          "front-end filter (NEXT #3) on the frame's raw samples")
+    ap.add_argument("--shard", action="store_true",
+                    help="latency mode (SURVEY.md §8(e), NEXT #4): ONE frame is cut into contiguous plane ranges over the "
+                         "N ranks, every rank runs the single-GPU path on its slice, rank 0 gathers the clusters "
+                         "(scaling: strong)")
     ap.add_argument("--fe-sectors", type=int, default=0,
                     help="--stage fe: sectors of the frame to filter (0 = all of the config's)")
     args = ap.parse_args()
@@ -440,6 +518,8 @@ def main():
         return run_ec(args)
     if args.stage == "fe":
         return run_fe(args)
+    if args.shard:
+        return run_shard(args)
 
     import torch
     import torch.distributed as dist
