@@ -366,6 +366,89 @@ def run_shard(args):
     return 0
 
 
+def run_chain(args):
+    """--stage chain: the paper's synchronous TPC chain around the cluster finder on one GPU, without a
+    host round trip: raw samples -> tpc_fe_run -> digits -> tpc_cf_run -> clusters -> tpc_ec_encode -> container.  A step
+    = one frame through all three calls; the digit and cluster counts that size the next call's arguments are read from
+    the device status blocks (one small synchronising read each, inside the timed region)."""
+    import torch
+    from datagen import gen, fe_gen
+    import paper_2402_01205_b200 as cf
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    cfg = dict(gen.CONFIGS[args.config])
+    if args.fe_sectors:
+        cfg["n_sectors"] = min(cfg["n_sectors"], args.fe_sectors)
+    ns, nr, mp, nt, npads = gen.geometry(cfg)
+    W = cf.tpc_fe_pad_stride(mp)
+    n_planes = ns * nr
+    host_raw = np.empty((n_planes, nt, W), dtype=np.uint16)
+    host_ped = np.empty((n_planes, W), dtype=np.uint16)
+    n_truth = 0
+    for s_ in range(ns):
+        d = gen.generate(cfg, sectors=(s_, s_ + 1))
+        n_truth += int(d.shape[0])
+        fe_gen.raw_from_digits(d, ns, nr, mp, nt, npads=npads, seed=cfg["seed"], planes=(s_ * nr, (s_ + 1) * nr),
+                               out=(host_raw[s_ * nr:(s_ + 1) * nr], host_ped[s_ * nr:(s_ + 1) * nr]))
+    raw = torch.from_numpy(host_raw.view(np.int16)).to(dev)
+    ped = torch.from_numpy(host_ped.view(np.int16)).to(dev)
+    del host_raw
+    pads = int(np.sum(npads)) if npads is not None else nr * mp
+    cells = ns * pads * nt
+    max_d = int(1.3 * n_truth) + 4096
+    max_c = max_d // 8 + 1024
+    flt = cf.FrontEndFilter(ns, nr, mp, nt, npads=npads, device=dev,
+                            max_digits_per_plane=int(min(nt * mp, max(4096, 2.0 * n_truth / n_planes))))
+    finder = cf.ClusterFinder(ns, nr, mp, nt, npads=npads, max_digits=max_d, max_clusters=max_c, device=dev)
+    coder = cf.ClusterCoder(ns, nr, max_c, device=dev)
+    digits = torch.empty(max_d * 8, dtype=torch.uint8, device=dev)
+    box = torch.empty(coder.max_encoded_bytes(max_c), dtype=torch.uint8, device=dev)
+    res = {}
+
+    def step():
+        flt.run(raw, ped, digits, capacity=max_d, zs_threshold=3)
+        fs = flt.read_status()
+        finder.run(digits, fs["n_digits"], flags=cf.DIGITS_SORTED)
+        st = finder.status.cpu().numpy().view(cf.STATUS)[0]
+        coder.encode(finder.clusters, int(st["n_clusters"]), box)
+        res.update(fe=fs, path=int(st["path"]), n_clusters=int(st["n_clusters"]), cf_overflow=int(st["overflow"]))
+
+    sampler = ClockSampler(0).start()
+    for _ in range(args.warmup):
+        step()
+    es = coder.read_status()
+    if res["fe"]["overflow"] or res["path"] != 3 or res["cf_overflow"] or es["error"]:
+        raise RuntimeError("chain run invalid: %r %r" % (res, es))
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    with sampler as clocks:
+        ev0.record()
+        for _ in range(args.steps):
+            step()
+        ev1.record()
+        torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    es = coder.read_status()
+    launches = flt.last_launch_count() + finder.last_launch_count() + coder.last_launch_count()
+    line = {"metric": "tpc_raw_samples_per_second_through_filter_finder_coder", "value": cells / (ms * 1e-3),
+            "unit": "samples/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u16/i32/f32", "data": "synthetic",
+            "config": {"workload": "filter -> cluster finder -> entropy coder on config%d: %s" % (args.config, cfg["label"]),
+                       "stage": "chain", "sectors": ns, "valid_samples": cells, "raw_bytes": int(raw.numel() * 2),
+                       "digits": res["fe"]["n_digits"], "clusters": res["n_clusters"], "container_bytes": es["bytes"],
+                       "raw_to_container_ratio": raw.numel() * 2.0 / max(1, es["bytes"]),
+                       "l2": "input (%.2f GB) larger than the 126 MB L2; no flush" % (raw.numel() * 2 / 1e9)},
+            "frames_per_s": 1e3 / ms, "roofline": None, "cpu_baseline": None, "e2e": None,
+            "gpu_launches": launches * args.steps, "clocks": clocks.summary()}
+    print(json.dumps(line))
+    flt.close(); finder.close(); coder.close()
+    return 0
+
+
 def run_fe(args):
     """--stage fe: the front-end filter (include/tpc_fe.h) on the raw samples of one frame of the chosen config
     (datagen/fe_gen.py's forward model over the config's digits).  One GPU.  A step = one tpc_fe_run (all its kernels)
@@ -499,10 +582,11 @@ def main():
     ap.add_argument("--variant", default="none", choices=["none", "flags", "cuts"],
                     help="cluster-finder variants (SURVEY.md §8(f) NEXT #1): 'flags' = per-cluster flags, 'cuts' = "
                          "flags + q_tot_min 40 + single-pad cut; the default run has none")
-    ap.add_argument("--stage", default="cf", choices=["cf", "ec", "fe"],
+    ap.add_argument("--stage", default="cf", choices=["cf", "ec", "fe", "chain"],
                     help="'cf' = the cluster finder (the headline path); 'ec' = the entropy coder of the cluster stream "
                          "(SURVEY.md §8(f) NEXT #2): encode and decode of the frame's clusters, one JSON line; 'fe' = the "
-                         "front-end filter (NEXT #3) on the frame's raw samples")
+                         "front-end filter (NEXT #3) on the frame's raw samples; 'chain' = filter -> cluster finder -> coder on "
+                         "the device, one frame per step")
     ap.add_argument("--shard", action="store_true",
                     help="latency mode (SURVEY.md §8(e), NEXT #4): ONE frame is cut into contiguous plane ranges over the "
                          "N ranks, every rank runs the single-GPU path on its slice, rank 0 gathers the clusters "
@@ -518,6 +602,8 @@ def main():
         return run_ec(args)
     if args.stage == "fe":
         return run_fe(args)
+    if args.stage == "chain":
+        return run_chain(args)
     if args.shard:
         return run_shard(args)
 
