@@ -145,6 +145,8 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
+    if args.stage in ("fe", "ec"):
+        return run_reference_stage(args)
     from datagen import gen
     from oracle import oracle as orc
     orc.build()
@@ -168,6 +170,53 @@ def run_reference(args):
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "clusters_per_s": st["n_clusters"] / (ms * 1e-3)}
+    print(json.dumps(line))
+    return 0
+
+
+def run_reference_stage(args):
+    """--impl reference --stage fe|ec: that stage's oracle, as it stands, single thread, on a bounded sample of the
+    same workload per step (fe: the raw samples of the first sector; ec: the first ~2 M clusters of the oracle cluster
+    finder's output on the first 8 sectors)."""
+    from datagen import gen
+    cfg = dict(gen.CONFIGS[args.config])
+    if args.stage == "fe":
+        from datagen import fe_gen
+        from oracle import fe_oracle as feo
+        feo.build()
+        ns, nr, mp, nt, npads = gen.geometry(cfg)
+        d = gen.generate(cfg, sectors=(0, 1))
+        raw, ped4 = fe_gen.raw_from_digits(d, ns, nr, mp, nt, npads=npads, seed=cfg["seed"], planes=(0, nr))
+        units = (int(np.sum(npads)) if npads is not None else nr * mp) * nt
+        fn = lambda: feo.run(raw, ped4, 1, nr, mp, nt, npads=npads, zs_threshold=3)
+        metric, unit = "tpc_raw_samples_filtered_per_second", "samples/s"
+        sample = "raw samples of the first sector (%d valid samples) per step" % units
+    else:
+        from oracle import oracle as orc, ec_oracle as eco
+        orc.build(); eco.build()
+        ns = min(cfg["n_sectors"], 8)
+        geom = gen.geometry(cfg)
+        d = gen.generate(cfg, sectors=(0, ns))
+        cl, _ = orc.run(d, geom[0], geom[1], geom[2], geom[3], npads=geom[4], planes=(0, ns * geom[1]))
+        units = int(cl.shape[0])
+        fn = lambda: eco.encode(cl, geom[0], geom[1])
+        metric, unit = "tpc_clusters_encoded_per_second", "clusters/s"
+        sample = "the %d clusters of the first %d sectors per step" % (units, ns)
+    for _ in range(min(args.warmup, 1)):
+        fn()
+    times = []
+    for _ in range(args.steps):
+        t0 = time.perf_counter()
+        fn()
+        times.append(time.perf_counter() - t0)
+    ms = 1e3 * float(np.mean(times))
+    value = units / (ms * 1e-3)
+    line = {"metric": metric, "value": value, "unit": unit, "impl": "reference", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "i64", "data": "synthetic",
+            "config": {"workload": "%s stage on config%d: %s" % (args.stage, args.config, cfg["label"]), "sample": sample},
+            "cpu_baseline": {"value": value, "unit": unit, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
     return 0
 

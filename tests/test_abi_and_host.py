@@ -365,3 +365,31 @@ def test_sector_sharded_frame_world_size_2_gloo(tmp_path):
     import json
     res = json.loads(outs[0][0].strip().splitlines()[-1])
     assert res["same"] and sum(res["counts"]) == res["total"] and min(res["counts"]) > 0.4 * res["total"]
+
+
+# ---- bench.py's reference arm (the oracle timed on the host cores) runs without a GPU ------------------------------
+
+@pytest.mark.parametrize("stage,metric,unit", [("cf", "tpc_digits_per_second", "digits/s"),
+                                               ("fe", "tpc_raw_samples_filtered_per_second", "samples/s"),
+                                               ("ec", "tpc_clusters_encoded_per_second", "clusters/s")])
+def test_bench_reference_arm_prints_one_json_line(stage, metric, unit):
+    import json
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--stage", stage,
+                          "--config", "1", "--steps", "1", "--warmup", "1"], capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    j = json.loads(lines[0])
+    assert j["impl"] == "reference" and j["metric"] == metric and j["unit"] == unit and j["value"] > 0
+    assert j["cpu_baseline"]["kind"] == "oracle" and j["cpu_baseline"]["cores"] == 1
+    assert j["e2e"]["h2d_bytes_per_step"] == 0 and j["e2e"]["d2h_bytes_per_step"] == 0
+
+
+def test_bench_product_arm_refuses_to_run_without_a_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("device present")
+    for extra in ([], ["--stage", "fe"], ["--stage", "ec"], ["--stage", "chain"]):
+        out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--config", "1", "--steps", "1"] + extra,
+                             capture_output=True, text=True, timeout=300)
+        assert out.returncode != 0 and "no CPU fallback" in out.stderr
