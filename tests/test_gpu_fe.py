@@ -131,20 +131,22 @@ def test_generated_frame_config1_defaults_and_chain_into_the_cluster_finder():
     flt.close()
 
 
-def test_full_length_planes_in_the_bench_configuration():
-    """the launch configuration bench.py --stage fe times (n_time 14336, 138 pads, ~2 % occupancy: config 3's first
-    rows), a handle reused for two runs, against the oracle on every record"""
+@pytest.mark.parametrize("cfg_id", [3, 4, 5])
+def test_full_length_planes_in_the_bench_configuration(cfg_id):
+    """the launch configuration bench.py --stage fe times (n_time 14336, 138 pads; config 3's ~2 %, config 4's ~10 % with
+    close pairs and plateaus, config 5's pads 66 -> 138), a handle reused for two runs, against the oracle on every
+    record"""
     import torch
     cf = _cf()
-    c = dict(gen.CONFIGS[3])
+    c = dict(gen.CONFIGS[cfg_id])
     c["n_sectors"], c["n_rows"] = 1, 6
     ns, nr, mp, nt, npads = gen.geometry(c)
     d = gen.generate(c)
-    raw, ped4 = fe_gen.raw_from_digits(d, ns, nr, mp, nt, seed=3)
-    want, wst = feo.run(raw, ped4, ns, nr, mp, nt, zs_threshold=3)
-    flt = cf.FrontEndFilter(ns, nr, mp, nt, max_digits_per_plane=1 << 17)
+    raw, ped4 = fe_gen.raw_from_digits(d, ns, nr, mp, nt, npads=npads, seed=3)
+    want, wst = feo.run(raw, ped4, ns, nr, mp, nt, npads=npads, zs_threshold=3)
+    flt = cf.FrontEndFilter(ns, nr, mp, nt, npads=npads, max_digits_per_plane=1 << 19)
     for _ in range(2):
-        got, st = gpu_run(raw, ped4, ns, nr, mp, nt, flt=flt, zs_threshold=3)
+        got, st = gpu_run(raw, ped4, ns, nr, mp, nt, npads=npads, flt=flt, zs_threshold=3)
         assert st == {"n_digits": wst["n_digits"], "overflow": 0} and got.tobytes() == want.tobytes()
     flt.close()
     assert 0.6 * d.shape[0] < want.shape[0] < 1.1 * d.shape[0]
