@@ -451,7 +451,7 @@ def run_chain(args):
     max_d = int(1.3 * n_truth) + 4096
     max_c = max_d // 8 + 1024
     flt = cf.FrontEndFilter(ns, nr, mp, nt, npads=npads, device=dev,
-                            max_digits_per_plane=int(min(nt * mp, max(4096, 2.0 * n_truth / n_planes))))
+                            max_digits_per_plane=int(min((nt + 32) * W, max(8192, 2.0 * n_truth / n_planes + 64 * W))))
     finder = cf.ClusterFinder(ns, nr, mp, nt, npads=npads, max_digits=max_d, max_clusters=max_c, device=dev)
     coder = cf.ClusterCoder(ns, nr, max_c, device=dev)
     digits = torch.empty(max_d * 8, dtype=torch.uint8, device=dev)
@@ -533,7 +533,7 @@ def run_fe(args):
     ped = host_ped.to(dev)
     pads = int(np.sum(npads)) if npads is not None else nr * mp
     cells = ns * pads * nt                                     # valid samples
-    cap_plane = int(min(nt * mp, max(4096, 2.0 * n_truth / n_planes)))
+    cap_plane = int(min((nt + 32) * W, max(8192, 2.0 * n_truth / n_planes + 64 * W)))
     flt = cf.FrontEndFilter(ns, nr, mp, nt, npads=npads, max_digits_per_plane=cap_plane, device=dev)
     cap = int(1.3 * n_truth) + 4096
     out = torch.empty(cap * 8, dtype=torch.uint8, device=dev)

@@ -49,8 +49,10 @@ typedef struct {
 
 enum {
     TPC_FE_OVF_PLANE = 1u,    /* a plane's staging area overflowed: output incomplete.  The area of max_digits_per_plane
-                                 records is shared evenly by the plane's groups of 32 pads (ceil(W / 32) of them), so
-                                 size it for the densest group: 2x the expected digits per plane is plenty */
+                                 records is cut into chunks of 32 records, shared evenly by the plane's groups of 32 pads
+                                 (ceil(W / 32) of them); a pad line occupies whole chunks.  Size it for the densest
+                                 group: 2x the expected digits per plane + 64 per pad is plenty; n_time + 32 per pad
+                                 (pads rounded up to 32) can never overflow */
     TPC_FE_OVF_OUTPUT = 2u    /* more digits than `capacity`: only records below `capacity` are written */
 };
 
@@ -66,8 +68,9 @@ typedef struct tpc_fe tpc_fe;   /* opaque handle: host state only */
 /* Row pitch of raw and ped4 in samples: max_pads rounded up to a multiple of 8 (16-byte rows). */
 uint32_t tpc_fe_pad_stride(uint32_t max_pads);
 
-/* Bytes of DEVICE workspace: per plane a staging area of max_digits_per_plane 8-byte records, per pad line a count,
- * per plane eight group counts and an offset.  0 on invalid arguments. */
+/* Bytes of DEVICE workspace: per plane a staging area of max_digits_per_plane 4-byte records in chunks of 32 with a
+ * 4-byte directory entry per chunk, per pad line a count, per plane 2 x 8 group counts and an offset.  0 on invalid
+ * arguments. */
 size_t tpc_fe_workspace_bytes(const tpc_cf_geometry* g, uint64_t max_digits_per_plane);
 
 /* workspace: DEVICE, 256-byte aligned, >= tpc_fe_workspace_bytes.  Geometry limits as in tpc_cf.h.

@@ -10,11 +10,13 @@
 //                 Per tile: (1) a warp per time bin forms the quiet-pad sum and count in one packed accumulator and one
 //                 warp reduction -> cm[t]; (2) every thread walks its pad through the tile's time bins with the tail
 //                 state in a register, marks the kept bins in a 64-bit mask and overwrites their cells with q;
-//                 (3) a block scan of the kept counts places the tile's records (pad, rank in the pad line, time, q)
-//                 in the plane's staging area.  Per-line and per-plane counts at the end of the plane.
-//   k_fe_scan     exclusive scan of the plane counts; status
-//   k_fe_order    one CTA per plane: line offsets from the line counts, then every staged record goes to
-//                 out[plane offset + line offset + rank]: ascending (sector,row,pad,time) without a sort
+//                 (3) every pad line appends its kept (time, q) words to 32-record chunks of the plane's staging area; a
+//                 warp scan hands out the chunks, a directory entry names a chunk's pad and first rank.  Per-line and
+//                 per-warp counts at the end of the plane.
+//   k_fe_scan     exclusive scan of the plane counts
+//   k_fe_order    one CTA per plane: line offsets from the line counts, then a warp per chunk copies it (128 bytes in,
+//                 256 bytes out) to out[plane offset + line offset + first rank ..]: ascending (sector,row,pad,time)
+//                 without a sort; the status is written by the CTA that finishes last
 #include <new>
 
 #include <cuda_runtime.h>
@@ -27,6 +29,7 @@ namespace tpcfe {
 static constexpr int kTT = 64;          // time bins per tile (the kept-bin mask is 64 bits)
 static constexpr int kStages = 2;       // tiles in the ring: kStages - 1 in flight ahead of the one in work
 static constexpr int kSlack = 128;      // bytes after the ring: phase 1 may read up to 31 samples past a row's pitch
+static constexpr int kChunk = 32;       // records per staging chunk (one 128-byte line)
 static constexpr int kAccShift = 22;    // packed quiet-pad accumulator: count << 22 | sum (|sum| < 2^20)
 
 struct Args {
@@ -35,10 +38,12 @@ struct Args {
     const uint32_t* npads;      // [n_rows]
     uint32_t n_planes, n_rows, n_time, W;
     uint32_t zs, c, m, k, mul;  // zs_threshold, cm_quiet4, cm_min_pads, it_decay_shift, 1 << (14 - kappa) or 0
-    uint32_t cap;               // staged records per plane
-    uint2* temp;                // [n_planes][cap]
+    uint32_t cpp;               // staging chunks per plane (a chunk = kChunk records of one pad line, consecutive ranks)
+    uint32_t* temp;             // [n_planes][cpp][kChunk]: (time | q << 16)
+    uint32_t* dir;              // [n_planes][cpp]: pad | (rank / kChunk) << 8 of the chunk
     uint32_t* line_cnt;         // [n_planes][W]
     uint32_t* warp_cnt;         // [n_planes][8]: kept samples of the pads of warp w (pads 32 w .. 32 w + 31)
+    uint32_t* warp_chunks;      // [n_planes][8]: chunks opened by warp w
     uint32_t* flags;
 };
 
@@ -106,7 +111,7 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
         for (uint32_t m = 0; m < (uint32_t)(kStages - 1) && m < total_tiles; m++) issue(m);
 
     const uint32_t c2 = 2u * a.c;
-    const uint32_t capw = a.cap / NW;                                           // staged records per warp and plane
+    const uint32_t capw = a.cpp / NW;                                           // staging chunks per warp and plane
     const int kk = (int)a.k, zs = (int)a.zs;
     // read back from shared memory so that it lives in a register (else the compiler reloads it from the constant bank,
     // predicated, once per sample)
@@ -129,7 +134,10 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
         int S = 0;
         uint32_t cnt = 0;       // kept samples of this pad line so far (rank of the next one)
         uint32_t wpos = 0;      // kept samples of this warp's pads so far (same value in every lane)
-        uint2* wtemp = a.temp + (size_t)plane * a.cap + (size_t)warp * capw;
+        uint32_t wchunks = 0;   // chunks opened by this warp so far (same value in every lane)
+        uint32_t cur = 0;       // the chunk this pad line is filling
+        uint32_t* wtemp = a.temp + ((size_t)plane * a.cpp + (size_t)warp * capw) * kChunk;
+        uint32_t* wdir = a.dir + (size_t)plane * a.cpp + (size_t)warp * capw;
 
         for (uint32_t tl = 0; tl < tpp; tl++, n++) {
             const uint32_t t0 = tl * kTT;
@@ -212,42 +220,50 @@ __global__ void __launch_bounds__(NW * 32) k_fe_filter(const Args a)
                 }
             }
 
-            // ---- (3) place the tile's records in the warp's part of the plane's staging area: a warp scan of the
-            // kept counts, no block barrier (k_fe_order finds every record by its pad and rank, not by its place)
+            // ---- (3) stage the tile's records: a pad line fills chunks of kChunk records (consecutive ranks) taken from
+            // the warp's part of the plane's staging area; a warp scan hands out the chunks the lanes open in this tile
+            // (no block barrier; k_fe_order copies chunk by chunk, coalesced, to where the line's ranks belong)
             {
                 const uint32_t c = __popc(mlo) + __popc(mhi);
-                uint32_t incl = c;
+                const uint32_t opened = ((cnt + c + kChunk - 1) / kChunk) - ((cnt + kChunk - 1) / kChunk);
+                uint32_t incl = opened;
 #pragma unroll
                 for (int d = 1; d < 32; d <<= 1) {
                     const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
                     if (lane >= (uint32_t)d) incl += v;
                 }
-                const uint32_t wtotal = __shfl_sync(0xffffffffu, incl, 31);
-                const uint32_t idx = wpos + incl - c;
-                wpos += wtotal;
+                uint32_t next_new = wchunks + incl - opened;
+                wchunks += __shfl_sync(0xffffffffu, incl, 31);
+                wpos += (uint32_t)__reduce_add_sync(0xffffffffu, c);
                 if (c) {
-                    const uint32_t n_ok = idx >= capw ? 0u : min(c, capw - idx);     // records that still fit
-                    uint2* dst = wtemp + idx;
                     const uint32_t cell_addr = smem_u32(tile + tid);
-                    uint32_t w0 = tid | (cnt << 8), j = 0;
+                    uint32_t rank = cnt;
                     auto put = [&](uint32_t i) {
                         uint32_t q;
                         asm volatile("ld.shared.u16 %0, [%1];" : "=r"(q) : "r"(cell_addr + i * (W * 2u)));
-                        if (j < n_ok) dst[j] = make_uint2(w0, (t0 + i) | (q << 16));
-                        j++; w0 += 256u;
+                        if ((rank & (kChunk - 1)) == 0u) {
+                            cur = next_new++;
+                            if (cur < capw) wdir[cur] = tid | ((rank / kChunk) << 8);
+                        }
+                        if (cur < capw) wtemp[cur * kChunk + (rank & (kChunk - 1))] = (t0 + i) | (q << 16);
+                        rank++;
                     };
                     while (mlo) { put(__ffs(mlo) - 1); mlo &= mlo - 1; }
                     while (mhi) { put(__ffs(mhi) + 31); mhi &= mhi - 1; }
-                    cnt += c;
+                    cnt = rank;
                 }
             }
         }
         if (tid < W) a.line_cnt[(size_t)plane * W + tid] = cnt;
         if (lane == 0) {
             a.warp_cnt[(size_t)plane * 8 + warp] = wpos;
-            if (wpos > capw) atomicOr(a.flags, (uint32_t)TPC_FE_OVF_PLANE);
+            a.warp_chunks[(size_t)plane * 8 + warp] = wchunks;
+            if (wchunks > capw) atomicOr(a.flags, (uint32_t)TPC_FE_OVF_PLANE);
         }
-        if (tid >= NW && tid < 8) a.warp_cnt[(size_t)plane * 8 + tid] = 0;
+        if (tid >= NW && tid < 8) {
+            a.warp_cnt[(size_t)plane * 8 + tid] = 0;
+            a.warp_chunks[(size_t)plane * 8 + tid] = 0;
+        }
     }
 }
 
@@ -285,13 +301,14 @@ __global__ void __launch_bounds__(1024) k_fe_scan(const uint32_t* warp_cnt, uint
     if (tid == 0) *(uint64_t*)(flags + 2) = s_carry;       // total; the status is written by the last CTA of k_fe_order
 }
 
-// one CTA per plane: staged records -> their place in the sorted output
-__global__ void __launch_bounds__(256) k_fe_order(const uint2* temp_all, uint32_t cap, const uint32_t* line_cnt,
-                                                  const uint32_t* warp_cnt, const uint64_t* plane_off, uint32_t W,
-                                                  uint32_t n_rows, uint2* out, uint64_t capacity, uint32_t* flags,
-                                                  tpc_fe_status* status)
+// one CTA per plane: staged chunks -> their place in the sorted output (a warp per chunk: 128 bytes in, 256 bytes out)
+__global__ void __launch_bounds__(256) k_fe_order(const uint32_t* temp_all, const uint32_t* dir_all, uint32_t cpp,
+                                                  const uint32_t* line_cnt, const uint32_t* warp_chunks,
+                                                  const uint64_t* plane_off, uint32_t W, uint32_t n_rows, uint2* out,
+                                                  uint64_t capacity, uint32_t* flags, tpc_fe_status* status)
 {
     __shared__ uint32_t s_off[256];
+    __shared__ uint32_t s_cnt[256];
     __shared__ uint32_t s_w[8];
     const uint32_t plane = blockIdx.x, tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t v = tid < W ? line_cnt[(size_t)plane * W + tid] : 0;
@@ -306,18 +323,23 @@ __global__ void __launch_bounds__(256) k_fe_order(const uint2* temp_all, uint32_
     uint32_t before = 0;
     for (uint32_t w = 0; w < warp; w++) before += s_w[w];
     s_off[tid] = before + incl - v;
+    s_cnt[tid] = v;
     __syncthreads();
     const uint64_t base = plane_off[plane];
     const uint32_t head = (plane / n_rows) | ((plane % n_rows) << 8);
-    const uint32_t nw = (W + 31) / 32, capw = cap / nw;
+    const uint32_t nw = (W + 31) / 32, capw = cpp / nw;
     for (uint32_t w = 0; w < nw; w++) {
-        const uint32_t n = min(warp_cnt[(size_t)plane * 8 + w], capw);
-        const uint2* temp = temp_all + (size_t)plane * cap + (size_t)w * capw;
-        for (uint32_t i = tid; i < n; i += 256) {
-            const uint2 r = temp[i];
-            const uint32_t pad = r.x & 255u;
-            const uint64_t dst = base + s_off[pad] + (r.x >> 8);
-            if (dst < capacity) out[dst] = make_uint2(head | (pad << 16), r.y);
+        const uint32_t n = min(warp_chunks[(size_t)plane * 8 + w], capw);
+        const uint32_t* temp = temp_all + ((size_t)plane * cpp + (size_t)w * capw) * kChunk;
+        const uint32_t* dir = dir_all + (size_t)plane * cpp + (size_t)w * capw;
+        for (uint32_t ch = warp; ch < n; ch += 8) {
+            const uint32_t e = dir[ch];
+            const uint32_t pad = e & 255u, first = (e >> 8) * kChunk;          // rank of the chunk's first record
+            const uint32_t cnt = s_cnt[pad];
+            if (first + lane < cnt) {
+                const uint64_t dst = base + s_off[pad] + first + lane;
+                if (dst < capacity) out[dst] = make_uint2(head | (pad << 16), temp[ch * kChunk + lane]);
+            }
         }
     }
     // the status is written last: by the CTA that finishes last
@@ -338,9 +360,11 @@ using namespace tpcfe;
 struct tpc_fe {
     uint32_t n_sectors, n_rows, max_pads, n_time, W, n_planes;
     uint64_t cap;
-    uint2* temp;
+    uint32_t* temp;
+    uint32_t* dir;
     uint32_t* line_cnt;
     uint32_t* warp_cnt;
+    uint32_t* warp_chunks;
     uint64_t* plane_off;
     uint32_t* npads;
     uint32_t* flags;
@@ -360,9 +384,11 @@ static size_t carve(uint32_t n_planes, uint32_t n_rows, uint32_t W, uint64_t cap
     p = take(256);                                   if (e) e->flags = (uint32_t*)p;
     p = take(4ull * n_rows);                         if (e) e->npads = (uint32_t*)p;
     p = take(32ull * n_planes);                      if (e) e->warp_cnt = (uint32_t*)p;
+    p = take(32ull * n_planes);                      if (e) e->warp_chunks = (uint32_t*)p;
+    p = take(4ull * n_planes * (cap / kChunk));      if (e) e->dir = (uint32_t*)p;
     p = take(8ull * n_planes);                       if (e) e->plane_off = (uint64_t*)p;
     p = take(4ull * n_planes * W);                   if (e) e->line_cnt = (uint32_t*)p;
-    p = take(8ull * n_planes * cap);                 if (e) e->temp = (uint2*)p;
+    p = take(4ull * n_planes * (cap / kChunk) * kChunk); if (e) e->temp = (uint32_t*)p;
     return off;
 }
 
@@ -452,7 +478,8 @@ extern "C" int tpc_fe_run(tpc_fe* h, const uint16_t* raw, const uint16_t* ped4, 
     a.n_planes = h->n_planes; a.n_rows = h->n_rows; a.n_time = h->n_time; a.W = h->W;
     a.zs = p->zs_threshold; a.c = p->cm_quiet4; a.m = p->cm_min_pads; a.k = (uint32_t)k;
     a.mul = j ? 1u << (14 - j) : 0u;
-    a.cap = (uint32_t)h->cap; a.temp = h->temp; a.line_cnt = h->line_cnt; a.warp_cnt = h->warp_cnt; a.flags = h->flags;
+    a.cpp = (uint32_t)(h->cap / kChunk); a.temp = h->temp; a.dir = h->dir; a.line_cnt = h->line_cnt;
+    a.warp_cnt = h->warp_cnt; a.warp_chunks = h->warp_chunks; a.flags = h->flags;
     cudaMemsetAsync(h->flags, 0, 16, st);
     const uint32_t grid = h->grid < h->n_planes ? h->grid : h->n_planes;
     if (h->profiling) cudaEventRecord(h->ev0, st);
@@ -471,7 +498,7 @@ extern "C" int tpc_fe_run(tpc_fe* h, const uint16_t* raw, const uint16_t* ped4, 
     }
     if (h->profiling) { cudaEventRecord(h->ev1, st); h->have_pair = 1; }
     k_fe_scan<<<1, 1024, 0, st>>>(h->warp_cnt, h->n_planes, h->plane_off, h->flags);
-    k_fe_order<<<h->n_planes, 256, 0, st>>>(h->temp, (uint32_t)h->cap, h->line_cnt, h->warp_cnt, h->plane_off, h->W,
+    k_fe_order<<<h->n_planes, 256, 0, st>>>(h->temp, h->dir, (uint32_t)(h->cap / kChunk), h->line_cnt, h->warp_chunks, h->plane_off, h->W,
                                             h->n_rows, (uint2*)out, capacity, h->flags, status);
     h->last_launches = 3;
     return cudaGetLastError() == cudaSuccess ? TPC_CF_OK : TPC_CF_E_CUDA;

@@ -70,7 +70,8 @@ def test_front_end_filter_host_logic_without_a_device():
     g, keep = cf.make_geometry(36, 152, 138, 14336)
     w = cf.tpc_fe_workspace_bytes(g, 65536)
     planes = 36 * 152
-    assert 8 * planes * 65536 + 4 * planes * 144 < w < 8 * planes * 65536 + 4 * planes * 144 + 48 * planes + 4096
+    fixed = 4 * planes * 65536 + 4 * planes * 2048 + 4 * planes * 144      # records, chunk directory, line counts
+    assert fixed < w < fixed + 80 * planes + 4096
     assert cf.tpc_fe_workspace_bytes(g, 0) == 0 and cf.tpc_fe_workspace_bytes(g, 1 << 32) == 0
     bad, _ = cf.make_geometry(36, 152, 256, 14336)
     assert cf.tpc_fe_workspace_bytes(bad, 100) == 0

@@ -20,7 +20,7 @@ def gpu_run(raw, ped4, ns, nr, mp, nt, npads=None, cap_plane=None, capacity=None
     own = flt is None
     if own:
         flt = cf.FrontEndFilter(ns, nr, mp, nt, npads=npads,
-                                max_digits_per_plane=cap_plane if cap_plane else nt * ((mp + 31) // 32 * 32))   # every group of 32 pads may keep all
+                                max_digits_per_plane=cap_plane if cap_plane else (nt + 32) * ((mp + 31) // 32 * 32))   # can never overflow
     r = torch.from_numpy(np.ascontiguousarray(raw).view(np.int16)).cuda()
     p = torch.from_numpy(np.ascontiguousarray(ped4).view(np.int16)).cuda()
     cap = capacity if capacity is not None else ns * nr * nt * mp
@@ -107,7 +107,7 @@ def test_generated_frame_config1_defaults_and_chain_into_the_cluster_finder():
     d = gen.generate(1)
     raw, ped4 = fe_gen.raw_from_digits(d, *g[:4], npads=g[4], seed=11)
     want, wst = feo.run(raw, ped4, *g[:4], npads=g[4], zs_threshold=3)
-    flt = cf.FrontEndFilter(*g[:4], npads=g[4], max_digits_per_plane=4096)
+    flt = cf.FrontEndFilter(*g[:4], npads=g[4], max_digits_per_plane=8192)
     r = torch.from_numpy(raw.view(np.int16)).cuda()
     p = torch.from_numpy(ped4.view(np.int16)).cuda()
     out = torch.zeros(want.shape[0] * 8 + 800, dtype=torch.uint8, device="cuda:0")
