@@ -151,11 +151,24 @@ int tpc_cf_run_host(tpc_cf* h, const tpc_digit* host_digits, uint64_t n,
 int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint64_t n,
                              uint32_t sector, uint32_t row, uint16_t* dense, void* stream);
 
+/* Test / tuning overrides of one handle (the tests force every kernel and every slow path with them; profiling uses
+ * them to compare launch shapes).  They select among exact implementations and never change the result.  value 0
+ * restores the library's own choice.  Returns TPC_CF_OK, TPC_CF_E_NULL or TPC_CF_E_PARAMS (unknown key, value < 0). */
+enum {
+    TPC_CF_DEBUG_FUSED_KERNEL = 1,  /* 1 k_fused_pairs, 2 k_fused_blocks (first generation), 3 k_fused_lines (bitmap slots) */
+    TPC_CF_DEBUG_PASSES = 2,        /* passes over the time axis of the block-sparse kernels */
+    TPC_CF_DEBUG_BLOCK_POOL = 3,    /* pool blocks per line slot (a small pool forces the cell-from-digit-array path) */
+    TPC_CF_DEBUG_SURV_CAP = 4,      /* stage-A survivor entries per line slot (a small list forces its overflow path) */
+    TPC_CF_DEBUG_PADS_PER_UNIT = 5, /* pads per CTA (multiple of 8) */
+    TPC_CF_DEBUG_CTAS_PER_SM = 6    /* 2: never use the 3-CTAs-per-SM instantiation */
+};
+int tpc_cf_debug_set(tpc_cf* h, int key, int value);
+
 /* Number of kernel launches the last run enqueued (for bench.py's gpu_launches). */
 int tpc_cf_last_launch_count(const tpc_cf* h);
 
-/* Name of the dominant kernel the last run enqueued: "k_fused_blocks" or "k_fused_lines" on the fused sorted path
- * (block-sparse or bitmap line slots, chosen from the mean line length), "k_peaks_map" on the general path.
+/* Name of the dominant kernel the last run enqueued: "k_fused_pairs" ("k_fused_blocks" / "k_fused_lines" where the
+ * mean line length or tpc_cf_debug_set asks for them) on the fused sorted path, "k_peaks_map" on the general path.
  * Static string, never NULL for a valid handle ("" before the first run). */
 const char* tpc_cf_last_kernel(const tpc_cf* h);
 

@@ -136,3 +136,52 @@ def make_digits(cells, sector=0, row=0):
     for i, (p, t, q) in enumerate(cells):
         d[i] = (sector, row, p, 0, t, q)
     return d
+
+
+def run_parallel(digits, n_sectors, n_rows, max_pads, n_time, npads=None, n_threads=None, **kw):
+    """The same single-threaded routine called on contiguous blocks of (sector,row) planes from n_threads host
+    threads; outputs concatenated in plane order.  Planes are independent (R2), so the result
+    is the single-threaded result; the caller may check that.  Needs digits whose planes are non-decreasing (sorted
+    input), so that a plane block is one contiguous slice; otherwise falls back to one thread.
+    Returns (clusters, status dict, threads used)."""
+    import concurrent.futures
+    import os
+    digits = np.ascontiguousarray(digits, dtype=DIGIT)
+    n = int(digits.shape[0])
+    n_planes = n_sectors * n_rows
+    if n_threads is None:
+        n_threads = os.cpu_count() or 1
+    plane = digits["sector"].astype(np.int32) * np.int32(n_rows) + digits["row"]
+    ok = n > 0 and bool(np.all(plane[1:] >= plane[:-1])) and int(plane[-1]) < n_planes and n_threads > 1
+    if not ok:
+        cl, st = run(digits, n_sectors, n_rows, max_pads, n_time, npads=npads, **kw)
+        return cl, st, 1
+    # blocks: ~8 per thread, cut at plane boundaries by digit count
+    n_blocks = min(n_planes, 8 * n_threads)
+    starts = np.searchsorted(plane, np.arange(n_planes + 1))
+    cuts = [0]
+    for b in range(1, n_blocks):
+        p = int(np.searchsorted(starts, n * b // n_blocks))
+        p = min(max(p, cuts[-1]), n_planes)
+        if p > cuts[-1]:
+            cuts.append(p)
+    if cuts[-1] != n_planes:
+        cuts.append(n_planes)
+    del plane
+
+    def work(i):
+        b, e = cuts[i], cuts[i + 1]
+        lo, hi = int(starts[b]), int(starts[e])
+        cap = kw.get("capacity")
+        return run(digits[lo:hi], n_sectors, n_rows, max_pads, n_time, npads=npads, planes=(b, e),
+                   **{k: v for k, v in kw.items() if k != "capacity"},
+                   capacity=max(1, (hi - lo) // 4 + 64) if cap is None else cap)
+
+    with concurrent.futures.ThreadPoolExecutor(max_workers=n_threads) as ex:
+        parts = list(ex.map(work, range(len(cuts) - 1)))
+    for cl, st in parts:
+        if st["overflow"]:
+            raise RuntimeError("oracle block overflowed its output estimate")
+    status = {k: sum(st[k] for _, st in parts) for k in ("n_clusters", "n_digits_used", "n_bad_digits")}
+    status["overflow"] = 0
+    return np.concatenate([cl for cl, _ in parts]), status, n_threads

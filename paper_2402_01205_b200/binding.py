@@ -27,8 +27,12 @@ FORCE_GENERAL = 2
 CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME = 4, 8, 16
 F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED = 1, 2, 4, 8, 16
 
+# tpc_cf_debug_set keys and the values of "fused_kernel" (include/tpc_cf.h)
+DEBUG_KEYS = {"fused_kernel": 1, "passes": 2, "block_pool": 3, "surv_cap": 4, "pads_per_unit": 5, "ctas_per_sm": 6}
+FUSED_KERNELS = {"auto": 0, "pairs": 1, "blocks": 2, "lines": 3}
+
 EXPORTS = ["tpc_cf_workspace_bytes", "tpc_cf_create", "tpc_cf_run", "tpc_cf_run_host",
-           "tpc_cf_debug_dense_plane", "tpc_cf_last_launch_count", "tpc_cf_last_kernel", "tpc_cf_set_profiling",
+           "tpc_cf_debug_dense_plane", "tpc_cf_debug_set", "tpc_cf_last_launch_count", "tpc_cf_last_kernel", "tpc_cf_set_profiling",
            "tpc_cf_profile_ms", "tpc_cf_destroy", "tpc_cf_strerror"]
 
 
@@ -83,6 +87,8 @@ def load(build_if_missing=True):
     lib.tpc_cf_debug_dense_plane.restype = ctypes.c_int
     lib.tpc_cf_debug_dense_plane.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32,
                                              ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
+    lib.tpc_cf_debug_set.restype = ctypes.c_int
+    lib.tpc_cf_debug_set.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]
     lib.tpc_cf_last_launch_count.restype = ctypes.c_int
     lib.tpc_cf_last_launch_count.argtypes = [ctypes.c_void_p]
     lib.tpc_cf_last_kernel.restype = ctypes.c_char_p
@@ -215,6 +221,14 @@ class ClusterFinder:
         _check(self.lib.tpc_cf_debug_dense_plane(self.h, digits_dev.data_ptr() if n else None, n, sector, row,
                                                  dense.data_ptr(), stream))
         return dense.cpu().numpy().view(np.uint16).reshape(npads_row, self.geom.n_time)
+
+    def debug_set(self, **kw):
+        """Test / tuning overrides of this handle (include/tpc_cf.h TPC_CF_DEBUG_*): fused_kernel ("pairs", "blocks",
+        "lines" or 0), passes, block_pool, surv_cap, pads_per_unit, ctas_per_sm.  0 restores the library's choice."""
+        for name, value in kw.items():
+            if name == "fused_kernel" and isinstance(value, str):
+                value = FUSED_KERNELS[value]
+            _check(self.lib.tpc_cf_debug_set(self.h, DEBUG_KEYS[name], int(value)))
 
     def set_profiling(self, on):
         _check(self.lib.tpc_cf_set_profiling(self.h, 1 if on else 0))

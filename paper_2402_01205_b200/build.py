@@ -8,11 +8,12 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libtpc_cf.so")
-SOURCES = ["tpc_cf_api.cu", "tpc_cf_general.cu", "tpc_cf_fused.cu", "tpc_cf_blocks.cu", "tpc_cf_compact.cu",
-           "tpc_ec.cu", "tpc_fe.cu"]
-HEADERS = [os.path.join(CSRC, "tpc_cf_internal.cuh"),
-           os.path.join(os.path.dirname(_HERE), "include", "tpc_cf.h"),
-           os.path.join(os.path.dirname(_HERE), "include", "tpc_ec.h")]
+import glob
+
+SOURCES = ["tpc_cf_api.cu", "tpc_cf_general.cu", "tpc_cf_fused.cu", "tpc_cf_blocks.cu", "tpc_cf_pairs.cu",
+           "tpc_cf_compact.cu", "tpc_ec.cu", "tpc_fe.cu"]
+HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh")) +
+                 glob.glob(os.path.join(os.path.dirname(_HERE), "include", "*.h")))
 EXTRA = os.environ.get("TPC_CF_NVCC_EXTRA", "").split()
 NVCC_FLAGS = EXTRA + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall"]

@@ -2,7 +2,6 @@
 // The library never allocates device memory; the handle owns host state and a few CUDA events only.
 #include <new>
 #include <stdio.h>
-#include <time.h>
 #include <string.h>
 
 #include "tpc_cf_internal.cuh"
@@ -20,6 +19,7 @@ struct tpc_cf {
     size_t map_bytes;
     int last_launches;
     uint64_t shape_n;           // digits of the whole frame while tpc_cf_run_host runs it group by group, else 0
+    Tuning tun;                 // tpc_cf_debug_set overrides (all 0 by default)
     const char* last_kernel;
     int profiling;
     uint32_t run_index;         // runs since profiling was switched on
@@ -132,13 +132,17 @@ extern "C" int tpc_cf_create(tpc_cf** hp, const tpc_cf_geometry* geom, uint64_t 
         cudaError_t e = cudaEventCreate(&h->ev[i / 4][i % 4]);
         if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaEventCreate"); }
     }
+    // the fused kernels use more than 48 KB of dynamic shared memory: a per-device attribute, set for this handle's device
+    cudaError_t e = fused_pairs_set_attributes();
+    if (e == cudaSuccess) e = fused_blocks_set_attributes();
+    if (e == cudaSuccess) e = fused_lines_set_attributes();
     // K0, once: the charge map starts zero; every run restores it (un-scatter).
-    cudaError_t e = cudaMemsetAsync(h->ws.map, 0, h->map_bytes, (cudaStream_t)stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->ws.map, 0, h->map_bytes, (cudaStream_t)stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), (cudaStream_t)stream);
     if (e != cudaSuccess) {
         for (int i = 0; i < kProfSlots * 4; ++i) cudaEventDestroy(h->ev[i / 4][i % 4]);
         delete h;
-        return cuda_fail(nullptr, e, "cudaMemsetAsync(map)");
+        return cuda_fail(nullptr, e, "tpc_cf_create (kernel attributes / map zeroing)");
     }
     *hp = h;
     return TPC_CF_OK;
@@ -185,7 +189,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
 
     if (fused) {
         // T3: line index -> fused smem kernel (scatter into smem lines, peak test, moments) -> compaction
-        int r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n, params->q_peak_min, params->q_inner_gate, var, st,
+        int r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n, params->q_peak_min, params->q_inner_gate, var, h->tun, st,
                                     prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
         if (r < 0) return r;
         k += r;
@@ -291,12 +295,8 @@ static int run_host_pipelined(tpc_cf* h, const tpc_digit* host_digits, uint64_t 
     memset(&tot, 0, sizeof tot);
     tot.path = 3;
     bool redo = false;
-    const bool trace = getenv("TPC_CF_TRACE") != nullptr;
-    struct timespec ts0; clock_gettime(CLOCK_MONOTONIC, &ts0);
-    auto now_ms = [&]() { struct timespec t; clock_gettime(CLOCK_MONOTONIC, &t); return (t.tv_sec - ts0.tv_sec) * 1e3 + (t.tv_nsec - ts0.tv_nsec) * 1e-6; };
     for (int g = 0; g < G; ++g) {
         e = cudaEventSynchronize(h->ev_run[g]);
-        if (trace) fprintf(stderr, "group %d done at %.2f ms (digits %llu)\n", g, now_ms(), (unsigned long long)(b[g + 1] - b[g]));
         if (e != cudaSuccess) return cuda_fail(h, e, "pipeline sync");
         const tpc_cf_status s = h->pinned_status[g];
         if (s.path != 3 || s.overflow) redo = true;                  // false promise / group over its share
@@ -311,7 +311,6 @@ static int run_host_pipelined(tpc_cf* h, const tpc_digit* host_digits, uint64_t 
         tot.n_bad_digits += s.n_bad_digits;
     }
     e = cudaStreamSynchronize(h->s_out);
-    if (trace) fprintf(stderr, "copy-out drained at %.2f ms\n", now_ms());
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->s_in);
     if (e != cudaSuccess) return cuda_fail(h, e, "pipeline drain");
     if (redo) return 0;
@@ -371,6 +370,22 @@ extern "C" int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint
     launch_unscatter(h->geo, h->ws, digits, n, st);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(h, e, "debug_dense_plane");
+    return TPC_CF_OK;
+}
+
+extern "C" int tpc_cf_debug_set(tpc_cf* h, int key, int value)
+{
+    if (!h) return TPC_CF_E_NULL;
+    if (value < 0) return TPC_CF_E_PARAMS;
+    switch (key) {
+    case TPC_CF_DEBUG_FUSED_KERNEL: if (value > 3) return TPC_CF_E_PARAMS; h->tun.fused_kernel = value; break;
+    case TPC_CF_DEBUG_PASSES: h->tun.passes = value; break;
+    case TPC_CF_DEBUG_BLOCK_POOL: h->tun.block_pool = value; break;
+    case TPC_CF_DEBUG_SURV_CAP: h->tun.surv_cap = value; break;
+    case TPC_CF_DEBUG_PADS_PER_UNIT: h->tun.pads_per_unit = value; break;
+    case TPC_CF_DEBUG_CTAS_PER_SM: h->tun.ctas_per_sm = value; break;
+    default: return TPC_CF_E_PARAMS;
+    }
     return TPC_CF_OK;
 }
 

@@ -14,8 +14,6 @@
 //   K4  stage C: peaks queued per warp, 5x5 window from the five slots p-2..p+2 -> stage[line_start + k]
 // Selected by launch_fused_sorted when the mean line fits the block pool (<= 254 blocks); otherwise the bitmap
 // kernel of tpc_cf_fused.cu runs.  Definition: include/tpc_cf.h (BASELINE.json:north_star; step named in PAPER.md:57).
-#include <stdlib.h>
-
 #include "tpc_cf_internal.cuh"
 
 namespace tpccf {
@@ -108,17 +106,6 @@ __device__ __noinline__ uint32_t cell_from_digits(const uint2* __restrict__ digi
     const uint32_t y = __ldg(&digits[gl + lo].y);
     return (y & 0xffffu) == tt ? (y >> 16) : 0u;
 }
-
-// Slot geometry (kernel parameters; all warp-uniform).
-struct SlotGeo {
-    uint32_t slot_bytes;   // multiple of 16
-    uint32_t pool_off;     // kDirOff + dir bytes (multiple of 16)
-    uint32_t surv_off;     // pool_off + 16 * pcap
-    uint32_t pcap;         // blocks in the pool including the zero block 0 (<= 255)
-    uint32_t scap;         // survivor entries per slot
-    uint32_t n_pass;       // the time axis is covered in n_pass segments, one pass over the unit's lines each
-    uint32_t seg_len;      // time bins per segment (multiple of 8); n_pass * seg_len >= n_time
-};
 
 // Slow path of bwindow (rare: a block of the window is not in the pool): cells of missing blocks come from the digit
 // array.  Out of line, result in registers, to keep the hot code small.
@@ -555,6 +542,20 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
     if (tid == 0 && s_unsorted) atomicOr(&cnt->unsorted, 1u);
 }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: tpc_cf_create sets it for its device.
+cudaError_t fused_blocks_set_attributes()
+{
+    cudaError_t e = cudaSuccess;
+    auto set = [&](const void* f, int bytes) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    };
+    set((const void*)k_fused_blocks<false, false, 2>, 112 * 1024); set((const void*)k_fused_blocks<true, false, 2>, 112 * 1024);
+    set((const void*)k_fused_blocks<false, true, 2>, 112 * 1024);  set((const void*)k_fused_blocks<true, true, 2>, 112 * 1024);
+    set((const void*)k_fused_blocks<false, false, 3>, 72 * 1024);  set((const void*)k_fused_blocks<true, false, 3>, 72 * 1024);
+    set((const void*)k_fused_blocks<false, true, 3>, 72 * 1024);   set((const void*)k_fused_blocks<true, true, 3>, 72 * 1024);
+    return e;
+}
+
 // Launches k_fused_blocks after the line index is in ws.line_start.  Returns 1 (launched), 0 (not applicable: the
 // mean line would not fit the block pool; the caller runs the bitmap kernel instead) or a negative tpc_cf error.
 //
@@ -562,8 +563,8 @@ k_fused_blocks(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32
 // 20 line slots of ~5 KB leave no room for a third CTA).  Lines too long for the 254-block pool are covered in several
 // passes over the time axis (dir, pool and survivor list all scale with the segment length).
 int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, bool must, cudaStream_t st,
-                        cudaEvent_t ev_k0, cudaEvent_t ev_k1)
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, bool must,
+                        cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
     uint64_t total_pads = 0;
     for (uint32_t r = 0; r < g.n_rows; ++r) total_pads += g.npads[r];
@@ -573,11 +574,8 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
     // measured on the synthetic frames: 0.38 blocks and 0.16 stage-A survivors per digit
     const double mean_blocks = 0.38 * mean_len, mean_surv = 0.16 * mean_len;
 
-    const char* force = getenv("TPC_CF_FUSED_KERNEL");            // "blocks" | "lines" (tests, profiling)
-    const bool forced = must || (force && force[0] == 'b');   // must: the bitmap kernel cannot take this geometry
-    if (!must && force && force[0] == 'l') return 0;
-    int env_pass = 0;                                              // tuning / test knob
-    if (const char* e = getenv("TPC_CF_PASSES")) env_pass = atoi(e);
+    const bool forced = must || tun.fused_kernel == 2;        // must: the bitmap kernel cannot take this geometry
+    const int env_pass = tun.passes;
 
     const uint32_t fixed = kBWarps * (kStageDepth * 256u + 256u);
     const uint32_t budget = 227u * 1024u / 2u - 1024u - 3328u;     // 2 CTAs per SM: - 1 KB reserved - ~3.2 KB static
@@ -614,14 +612,8 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
         for (uint32_t np = 1; np <= 8 && !have; ++np) have = (np == 1 || g.n_time >= 64u * np) && shape(np, true, &sg);
         if (!have) return 0;
     }
-    if (const char* e = getenv("TPC_CF_BLOCK_POOL")) {             // test knob: force a small pool (slow paths)
-        const int v = atoi(e);
-        if (v >= 2 && v <= 255 && (uint32_t)v <= sg.pcap) sg.pcap = (uint32_t)v;
-    }
-    if (const char* e = getenv("TPC_CF_SURV_CAP")) {
-        const int v = atoi(e);
-        if (v >= 4 && (uint32_t)v <= sg.scap) sg.scap = (uint32_t)v & ~3u;
-    }
+    if (tun.block_pool >= 2 && tun.block_pool <= 255 && (uint32_t)tun.block_pool <= sg.pcap) sg.pcap = (uint32_t)tun.block_pool;
+    if (tun.surv_cap >= 4 && (uint32_t)tun.surv_cap <= sg.scap) sg.scap = (uint32_t)tun.surv_cap & ~3u;
     sg.surv_off = sg.pool_off + 16u * sg.pcap;
     sg.slot_bytes = sg.surv_off + 4u * sg.scap;
     const uint32_t smem = kBSlots * sg.slot_bytes + fixed;
@@ -629,30 +621,13 @@ int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t whole = (g.max_pads + kBS - 1) / kBS * kBS;
     uint32_t pads_per_unit = g.n_planes >= 1184 ? whole : (g.n_planes >= 296 ? 6 * kBS : 3 * kBS);
     if (pads_per_unit > whole) pads_per_unit = whole;
-    if (const char* e = getenv("TPC_CF_PADS_PER_UNIT")) {          // tuning knob (multiples of 8)
-        const int v = atoi(e);
-        if (v >= kBS && v <= 256) pads_per_unit = (uint32_t)(v / kBS * kBS);
-    }
+    if (tun.pads_per_unit >= kBS && tun.pads_per_unit <= 256) pads_per_unit = (uint32_t)(tun.pads_per_unit / kBS * kBS);
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaSuccess;
-        auto set = [&](const void* f, int bytes) {
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-        };
-        set((const void*)k_fused_blocks<false, false, 2>, 112 * 1024); set((const void*)k_fused_blocks<true, false, 2>, 112 * 1024);
-        set((const void*)k_fused_blocks<false, true, 2>, 112 * 1024);  set((const void*)k_fused_blocks<true, true, 2>, 112 * 1024);
-        set((const void*)k_fused_blocks<false, false, 3>, 72 * 1024);  set((const void*)k_fused_blocks<true, false, 3>, 72 * 1024);
-        set((const void*)k_fused_blocks<false, true, 3>, 72 * 1024);   set((const void*)k_fused_blocks<true, true, 3>, 72 * 1024);
-        if (e != cudaSuccess) return TPC_CF_E_CUDA;
-        attr_set = true;
-    }
     if (ev_k0) cudaEventRecord(ev_k0, st);
     g_last_kernel = "k_fused_blocks";
     // a third CTA per SM when the slots are small (short lines): the kernel is latency bound
     const uint32_t budget3 = 227u * 1024u / 3u - 1024u - 3328u;
-    bool three = smem <= budget3;
-    if (const char* e3 = getenv("TPC_CF_CTAS_PER_SM")) three = three && atoi(e3) != 2;
+    const bool three = smem <= budget3 && tun.ctas_per_sm != 2;
     const bool m = sg.n_pass > 1, v = var.active != 0u;
     auto kern = three ? (m ? (v ? k_fused_blocks<true, true, 3> : k_fused_blocks<true, false, 3>)
                            : (v ? k_fused_blocks<false, true, 3> : k_fused_blocks<false, false, 3>))

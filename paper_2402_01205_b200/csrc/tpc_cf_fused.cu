@@ -19,8 +19,6 @@
 //                  line_cnt[]; a scan over the line counts and a per-line copy give the ordered output (K3, K5).
 //   The DIGITS_SORTED promise is verified here for free: every digit is checked once against the line (or gap) it
 //   was found in; any violation raises Counters::unsorted and the run reports path 0.
-#include <stdlib.h>
-
 #include "tpc_cf_internal.cuh"
 
 namespace tpccf {
@@ -454,8 +452,13 @@ k_fused_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     if (tid == 0 && s_unsorted) atomicOr(&cnt->unsorted, 1u);
 }
 
+cudaError_t fused_lines_set_attributes()
+{
+    return cudaFuncSetAttribute(k_fused_lines, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+}
+
 int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
     cudaMemsetAsync(ws.line_cnt, 0, ((size_t)g.n_planes * g.LS + 1) * 4, st);   // pads beyond npads[row] stay 0
@@ -466,9 +469,13 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     k_line_index<<<(entries + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start);
     k += 2;
 
-    // block-sparse line slots (tpc_cf_blocks.cu) when the mean line fits their pool; else the bitmap slots below
-    {
-        const int r = launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, false, st, ev_k0, ev_k1);
+    // Kernel choice.  Block-sparse line slots when the mean line fits their pool (k_fused_pairs, tpc_cf_pairs.cu; its
+    // first generation k_fused_blocks, tpc_cf_blocks.cu, only on request), else the bitmap slots below.
+    // tun.fused_kernel (tests, profiling): 1 pairs, 2 blocks, 3 lines.
+    if (tun.fused_kernel != 3) {
+        const int r = tun.fused_kernel == 2
+            ? launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, tun, false, st, ev_k0, ev_k1)
+            : launch_fused_pairs(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, tun, tun.fused_kernel == 1, st, ev_k0, ev_k1);
         if (r < 0) return r;
         if (r > 0) return k + r;
     }
@@ -486,7 +493,9 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t per_cap0 = kSlots * 4 + kSlots / 8 + 1 + kWarps * 4 + kWarps * 2;   // tq, stage-A bit, key staging, survivor list
     if (fixed + per_cap0 * 128 > 200 * 1024) {
         // the bitmap slots of 20 lines do not fit (n_time above ~50 k): the block kernel covers the time axis in passes
-        const int r = launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, true, st, ev_k0, ev_k1);
+        int r = launch_fused_pairs(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, tun, true, st, ev_k0, ev_k1);
+        if (r == 0)     // (k_fused_pairs declines n_time above its sentinel times; its first generation takes any geometry)
+            r = launch_fused_blocks(g, ws, digits, n, shape_n, q_peak_min, q_gate, var, tun, true, st, ev_k0, ev_k1);
         if (r < 0) return r;
         return r > 0 ? k + r : TPC_CF_E_GEOMETRY;
     }
@@ -500,17 +509,8 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t whole = (g.max_pads + kS - 1) / kS * kS;
     uint32_t pads_per_unit = g.n_planes >= 1184 ? whole : (g.n_planes >= 296 ? 6 * kS : 3 * kS);
     if (pads_per_unit > whole) pads_per_unit = whole;
-    if (const char* e = getenv("TPC_CF_PADS_PER_UNIT")) {    // tuning knob (multiples of 8)
-        const int v = atoi(e);
-        if (v >= kS && v <= 256) pads_per_unit = (uint32_t)(v / kS * kS);
-    }
+    if (tun.pads_per_unit >= kS && tun.pads_per_unit <= 256) pads_per_unit = (uint32_t)(tun.pads_per_unit / kS * kS);
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_fused_lines, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e != cudaSuccess) return TPC_CF_E_CUDA;
-        attr_set = true;
-    }
     if (ev_k0) cudaEventRecord(ev_k0, st);
     g_last_kernel = "k_fused_lines";
     k_fused_lines<<<g.n_planes * upp, kFThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,

@@ -50,7 +50,26 @@ struct Workspace {
     tpc_cf_status* group_status;   // [32] per-group status blocks of the tpc_cf_run_host pipeline
 };
 
-struct Handle;
+// Slot geometry of the block-sparse fused kernels (kernel parameter; all warp-uniform).
+struct SlotGeo {
+    uint32_t slot_bytes;   // multiple of 16
+    uint32_t pool_off;     // header + dir bytes (multiple of 16)
+    uint32_t surv_off;     // pool_off + 16 * pcap
+    uint32_t pcap;         // blocks in the pool including the zero block 0 (<= 255)
+    uint32_t scap;         // survivor entries per slot
+    uint32_t n_pass;       // the time axis is covered in n_pass segments, one pass over the unit's lines each
+    uint32_t seg_len;      // time bins per segment (multiple of 8); n_pass * seg_len >= n_time
+};
+
+// Test / tuning overrides of a handle (tpc_cf_debug_set; all 0 = the library decides).  They never change the result.
+struct Tuning {
+    int fused_kernel;      // TPC_CF_DEBUG_FUSED_KERNEL: 0 auto, 1 k_fused_pairs, 2 k_fused_blocks, 3 k_fused_lines
+    int passes;            // TPC_CF_DEBUG_PASSES: time passes of the block-sparse kernels
+    int block_pool;        // TPC_CF_DEBUG_BLOCK_POOL: pool blocks per slot (forces the pool-overflow slow path)
+    int surv_cap;          // TPC_CF_DEBUG_SURV_CAP: survivor entries per slot (forces the list-overflow slow path)
+    int pads_per_unit;     // TPC_CF_DEBUG_PADS_PER_UNIT: pads per CTA (multiple of 8)
+    int ctas_per_sm;       // TPC_CF_DEBUG_CTAS_PER_SM: 2 = never use the 3-CTA instantiation
+};
 
 // ---- shared device arithmetic -------------------------------------------------------------------------------
 
@@ -198,12 +217,22 @@ int launch_copy_plane(const Geo& g, const Workspace& ws, uint32_t plane, uint32_
                       cudaStream_t st);
 
 int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, cudaStream_t st,
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1);
 
+// Block-sparse fused kernels after the line index is in ws.line_start.  Return 1 (launched), 0 (not applicable: the
+// caller runs another kernel) or a negative tpc_cf error.  must: no other kernel can take this geometry.
 int launch_fused_blocks(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, bool must, cudaStream_t st,
-                        cudaEvent_t ev_k0, cudaEvent_t ev_k1);
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, bool must,
+                        cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1);
+int launch_fused_pairs(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
+                       uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, bool must,
+                       cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1);
+// cudaFuncAttributeMaxDynamicSharedMemorySize of the fused kernels, for the CURRENT device (called by tpc_cf_create:
+// the attribute is per device)
+cudaError_t fused_lines_set_attributes();
+cudaError_t fused_blocks_set_attributes();
+cudaError_t fused_pairs_set_attributes();
 
 // compaction of stage[j] by peakmask into dst (= out, or ws.compact when a key sort must follow)
 int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t capacity, uint64_t max_clusters,

@@ -1,0 +1,837 @@
+// tpc_cf_pairs.cu — fused path, second generation ("T3c"): block-sparse line slots in shared memory as in
+// tpc_cf_blocks.cu (one CTA per (plane, pad range), one WARP per pad LINE, a ring of line slots, one barrier per step
+// of 8 lines), rebuilt around the instruction count (profiles/r2a_*: the build loop was 54 % of all issued
+// instructions, 95 SASS instructions per 32 digits, 60 % of them on the ALU pipe):
+//   * the digit stream reaches shared memory by 1-D bulk copies (cp.async.bulk + mbarrier transaction counts; SASS
+//     UBLKCP), 128 digits = 1 KB per copy, issued by one lane into a two-piece ring, two iterations ahead;
+//   * every lane works on TWO consecutive digits per iteration (64 digits per warp iteration): one of the two neighbour
+//     relations of a digit is in-register, ballots / rank arithmetic / loop control are paid once per 64 digits;
+//   * neighbours in the line are read from the staging ring at immediate offsets of one address (no shuffles, no
+//     carried state between iterations): lane i holds digits 2i-1 and 2i of the chunk, so that the successor of the
+//     last digit is still in the same chunk and the predecessor of the first one is the tail of the chunk before
+//     (a 16-byte guard in front of the ring carries it across the wrap);
+//   * the in-step load balance (which warp builds / processes which line) is computed once per CTA, not per step;
+//   * a slot is cleaned by what its last line used (directory + allocated blocks), not by its capacity;
+//   * windows skip the "block not in the pool" test when none of the five lines overflowed its pool.
+// Slot of one pad line (all offsets multiples of 16):
+//     hdr   [16 B]  word 0: stage-A survivors of the line; 1: first digit this pass streamed; 2: blocks the line opened;
+//                   3: 1 if a block did not fit the pool (its dir byte is 0xFF: cells come from the digit array)
+//     dir[b] uint8  pool index of the block of time bins 8b-8 .. 8b-1 (0 = the all-zero block)
+//     pool[i] 16 B  eight uint16 charges; block 0 stays zero (zero border in time and empty cells, R2)
+//     surv[k] u32   (time | charge << 16) of the k-th digit that passed the own-line test (stage A), time order
+//   K0 the warp that reuses a slot zeroes it      K1 build: block allocation by ballot / popc, in time order
+//   K2 stage A at build time, stage B from the survivor list against lines p-1 / p+1
+//   K4 stage C: peaks queued per warp, 5x5 window from the five slots p-2..p+2 -> stage[line_start + k]
+// Definition: include/tpc_cf.h (BASELINE.json:north_star; step named in PAPER.md:57).  Readings R1..R19: DESIGN.md §3.
+#include "tpc_cf_internal.cuh"
+
+namespace tpccf {
+
+static constexpr int kPThreads = 256;
+static constexpr int kPWarps = kPThreads / 32;
+static constexpr int kPS = kPWarps;               // lines per step: one per warp
+static constexpr int kPSlots = 2 * kPS + 4;       // lines l0-2 .. l0+S+1 in use, next S being built
+static constexpr uint32_t kChunkBytes = 512;      // one build iteration: 64 digits
+static constexpr uint32_t kPieceBytes = 1024;     // one bulk copy: 128 digits = two iterations
+static constexpr uint32_t kNH = 2;                // staging ring per warp: two pieces, one mbarrier each
+static constexpr uint32_t kGuard = 16;            // in front of the ring: copy of the ring's last 16 bytes
+static constexpr uint32_t kStgBytes = kGuard + kNH * kPieceBytes;
+static constexpr uint32_t kPqBytes = 256;         // per-warp peak queue (64 entries)
+static constexpr uint32_t kHdrBytes = 16;
+static constexpr int kMaxSteps = 32;              // 256 pads / 8
+static constexpr uint32_t kSentT0 = 65470u;       // time of the first trailing sentinel digit (+ up to 63); n_time <= this
+
+// ---- shared-memory accessors on 32-bit addresses -------------------------------------------------------------------
+__device__ __forceinline__ uint32_t p_lds32(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint2 p_lds64(uint32_t a)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint4 p_lds128(uint32_t a)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t p_lds16(uint32_t a)
+{
+    uint16_t v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t p_lds8(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void p_sts32(uint32_t a, uint32_t v)
+{
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ void p_sts16(uint32_t a, uint32_t v)
+{
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((uint16_t)v) : "memory");
+}
+__device__ __forceinline__ void p_sts8(uint32_t a, uint32_t v)
+{
+    asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ void p_sts128(uint32_t a, uint4 v)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void p_sts128z(uint32_t a)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");
+}
+
+// ---- mbarrier + 1-D bulk copy (global -> shared, completion counted in bytes) ----------------------------------------
+__device__ __forceinline__ void p_mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ bool p_mbar_try(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0u;
+}
+__device__ __forceinline__ void p_mbar_wait(uint32_t bar, uint32_t parity)
+{
+    while (!p_mbar_try(bar, parity)) { }
+}
+__device__ __forceinline__ void p_mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void p_bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// ring index of the line at distance d (|d| < kPSlots) from the line whose ring index is v0
+__device__ __forceinline__ int pring_at(int v0, int d)
+{
+    int v = v0 + d;
+    v += (v < 0) ? kPSlots : 0;
+    v -= (v >= kPSlots) ? kPSlots : 0;
+    return v;
+}
+
+// K2 stage A (R1, own line) from the digit array (slow path only): the neighbours in time are the adjacent digits of the
+// line; an absent one reads 0.  (0,-1) is lexicographically earlier: strict; (0,+1) later: >=.
+__device__ __forceinline__ bool p_stage_a(uint32_t y, uint32_t prevy, bool has_prev, uint32_t nexty, bool has_next,
+                                          uint32_t T, uint32_t q_peak_min)
+{
+    const uint32_t t = y & 0xffffu, q = y >> 16;
+    const uint32_t qm = (has_prev && (prevy & 0xffffu) + 1u == t) ? (prevy >> 16) : 0u;
+    const uint32_t qp = (has_next && (nexty & 0xffffu) == t + 1u && t + 1u < T) ? (nexty >> 16) : 0u;
+    return q >= q_peak_min && q > qm && q >= qp;
+}
+
+// charge of cell (line, tt) from the digit array (slow path: the line's block pool was full).  Binary search on time.
+// Cells outside [0, T) read 0 (R2) whatever the digit array holds there (a digit with time >= T is invalid, R11).
+__device__ __noinline__ uint32_t p_cell_from_digits(const uint2* __restrict__ digits, uint32_t gl, uint32_t glen,
+                                                    uint32_t tt, uint32_t T)
+{
+    if (tt >= T) return 0u;
+    uint32_t lo = 0, hi = glen;
+    while (lo < hi) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        if ((__ldg(&digits[gl + mid].y) & 0xffffu) < tt) lo = mid + 1; else hi = mid;
+    }
+    if (lo >= glen) return 0u;
+    const uint32_t y = __ldg(&digits[gl + lo].y);
+    return (y & 0xffffu) == tt ? (y >> 16) : 0u;
+}
+
+// Slow path of pwindow (rare: a block of the window is not in the pool): cells of missing blocks come from the digit
+// array.  Out of line, result in registers, to keep the hot code small.
+struct PWin5 { int c[5]; };
+__device__ __noinline__ PWin5 pwindow_slow(uint32_t aA, uint32_t aB, uint32_t dA, uint32_t dB, uint32_t o, int t0, int n,
+                                           const uint2* __restrict__ digits, uint32_t gl, uint32_t glen, uint32_t T)
+{
+    PWin5 r;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const bool inA = o + (uint32_t)k < 8u;
+        const uint32_t d = inA ? dA : dB;
+        r.c[k] = k >= n ? 0
+               : (d != 0xFFu ? (int)p_lds16((inA ? aA : aB) + 2u * (uint32_t)k)
+                             : (int)p_cell_from_digits(digits, gl, glen, (uint32_t)(t0 + k), T));
+    }
+    return r;
+}
+
+// charges of the window t-H..t+H of the line in slot `slot` (0 where no digit): c[k] is time t-H+k.
+// dsub = first time bin of the pass / 8.  OVF (warp-uniform): some line of the neighbourhood has blocks outside its
+// pool (their dir byte is 0xFF): only then are the directory bytes tested.  lidx = pad index of the line, slow path only.
+template <int H>
+__device__ __forceinline__ void pwindow(uint32_t slot, uint32_t dsub, const SlotGeo& sg, int t, int (&c)[2 * H + 1],
+                                        const uint2* __restrict__ digits, const uint32_t* s_ls, int lidx, int P,
+                                        uint32_t T, bool OVF)
+{
+    const uint32_t u = (uint32_t)(t + 8 - H);                 // first cell, shifted by the 8-bin guard block
+    const uint32_t dir = slot + kHdrBytes - dsub;
+    const uint32_t dA = p_lds8(dir + (u >> 3));
+    const uint32_t dB = p_lds8(dir + ((u + 2 * H) >> 3));
+    const uint32_t o = u & 7u;
+    const uint32_t base = slot + sg.pool_off + 2u * o;
+    const uint32_t aA = base + (dA << 4), aB = base + (dB << 4) - 16u;
+    if (!OVF || (dA != 0xFFu && dB != 0xFFu)) {
+        c[0] = (int)p_lds16(aA);
+#pragma unroll
+        for (int k = 1; k < 2 * H + 1; ++k) c[k] = (int)p_lds16((o < (uint32_t)(8 - k) ? aA : aB) + 2u * (uint32_t)k);
+    } else {
+        const bool inside = lidx >= 0 && lidx < P;
+        const uint32_t gl = inside ? s_ls[lidx] : 0u;
+        const uint32_t glen = inside ? s_ls[lidx + 1] - gl : 0u;
+        const PWin5 r = pwindow_slow(aA, aB, dA, dB, o, t - H, 2 * H + 1, digits, gl, glen, T);
+#pragma unroll
+        for (int k = 0; k < 2 * H + 1; ++k) c[k] = r.c[k];
+    }
+}
+
+// MULTI: the time axis is covered in sg.n_pass > 1 passes (long lines).  VAR: flags / cuts requested (V1..V3); the
+// default instantiation carries none of that code.  MINB: CTAs per SM the registers are limited for.
+template <bool MULTI, bool VAR, int MINB>
+__global__ void __launch_bounds__(kPThreads, MINB)
+k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
+              uint32_t pads_per_unit, uint32_t units_per_plane, SlotGeo sg, uint32_t q_peak_min, uint32_t q_gate,
+              Variant var, Counters* cnt, uint32_t* __restrict__ line_cnt, uint4* __restrict__ stage)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ uint32_t s_ls[260];          // line starts of this plane: s_ls[p], p = 0..max_pads, then next plane's start
+    __shared__ uint32_t s_pos[260];         // first digit of line p that the current pass needs (time >= pass start - 2)
+    __shared__ uint32_t s_cnt[260];         // peaks of line p found by the passes so far
+    __shared__ __align__(8) unsigned long long s_bar[kPWarps * kNH];
+    __shared__ __align__(4) uint8_t s_asg[kMaxSteps][kPWarps];   // per step and warp: line to process (low nibble) / to build (high)
+    __shared__ int s_unsorted;
+
+    const uint32_t plane = blockIdx.x / units_per_plane, unit = blockIdx.x % units_per_plane;
+    const uint32_t sector = plane / g.n_rows, row = plane % g.n_rows;
+    const int P = (int)g.npads[row];
+    const int pa = (int)(unit * pads_per_unit);
+    const int pb = min(pa + (int)pads_per_unit, P);
+    const uint32_t T = g.n_time;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);    // (the shuffle tells the compiler it is warp-uniform)
+    const uint32_t w0_base = sector | (row << 8);
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const uint32_t le_mask = lt_mask | (1u << lane);
+
+    const uint32_t sm0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    const uint32_t ring = sm0 + kPSlots * sg.slot_bytes + (uint32_t)warp * kStgBytes + kGuard;   // this warp's chunk 0
+    const uint32_t pqa = sm0 + kPSlots * sg.slot_bytes + kPWarps * kStgBytes + (uint32_t)warp * kPqBytes;
+    const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(&s_bar[warp * kNH]);
+    // 16-byte alignment of digit j in global memory: (j + gpar) even
+    const uint32_t gpar = (uint32_t)((reinterpret_cast<uintptr_t>(digits) >> 3) & 1u);
+    const uint32_t al_lo = gpar;                                  // first and one-past-last digit a bulk copy may touch
+    const uint32_t al_hi = n - ((n + gpar) & 1u);
+
+    for (int i = tid; i <= (int)g.LS; i += kPThreads) {
+        const uint32_t v = line_start[plane * g.LS + i];
+        s_ls[i] = v; s_pos[i] = v; s_cnt[i] = 0u;
+    }
+    if (tid == 0) s_unsorted = 0;
+    if (tid < kMaxSteps * kPWarps / 4) ((uint32_t*)&s_asg[0][0])[tid] = 0u;
+    if (tid < kPWarps * (int)kNH) p_mbar_init((uint32_t)__cvta_generic_to_shared(&s_bar[tid]), 1u);
+    // every slot starts as an empty line (lines outside the plane keep this state: zero border in pad, R2)
+    for (uint32_t x = (uint32_t)tid * 16u; x < kPSlots * sg.slot_bytes; x += kPThreads * 16u) p_sts128z(sm0 + x);
+    __syncthreads();
+
+    if (pa >= P && unit != 0) return;    // nothing in this pad range (rows with fewer pads)
+
+    uint32_t bad_order = 0u;
+    // monotone line starts: a garbage index from unsorted input must not produce negative lengths or unbounded work
+    for (int i = tid; i < (int)g.LS; i += kPThreads) if (s_ls[i] > s_ls[i + 1]) bad_order = 1u;
+    if (s_ls[g.LS] > n) bad_order = 1u;
+    if (__syncthreads_or((int)bad_order)) {
+        if (tid == 0) atomicOr(&cnt->unsorted, 1u);
+        return;
+    }
+
+    // gap of the plane: digits with pad >= npads[row] (or a row/sector beyond the geometry) — all invalid (R11)
+    if (unit == 0) {
+        const uint32_t gb = s_ls[P], ge = s_ls[g.LS];
+        if (ge > gb) {
+            for (uint32_t j = gb + tid; j < ge; j += kPThreads) {
+                const uint2 d = __ldg(digits + j);
+                if (digit_valid(g, d.x, d.y)) bad_order = 1u;     // a valid digit outside every line: not sorted
+            }
+            if (tid == 0) atomicAdd(&cnt->n_bad, (unsigned long long)(ge - gb));
+        }
+    }
+
+    const int blo = max(pa - 2, 0), bhi = min(P, pb + 2);   // lines this unit ever builds
+
+    // ---- in-step load balance, once per CTA ---------------------------------------------------------------------------
+    // A warp's work in a step is one line to process plus one line to build, both proportional to the line lengths
+    // (known from the index).  The warp with the longest line to process gets the shortest line to build, and so on:
+    // the 8 sums come out nearly equal and the barrier waits less.  Warp w ranks steps w, w + 8, ...
+    {
+        int k = warp;
+        for (int l0 = pa + warp * kPS; l0 < pb; l0 += kPS * kPWarps, k += kPWarps) {
+            const bool more = l0 + kPS < pb;
+            uint32_t lp = 0u, lb = 0u;
+            if (lane < kPS) {
+                const int p = l0 + lane, q = l0 + kPS + 2 + lane;
+                if (p < pb) lp = min(s_ls[p + 1] - s_ls[p], 0xfffeu) + 1u;
+                if (more && q >= blo && q < bhi) lb = min(s_ls[q + 1] - s_ls[q], 0xfffeu) + 1u;
+            }
+            const uint32_t mine = lp | (lb << 16);
+            // ranks of the 8 lines by all-pairs comparison, two pairs per lane: lane L compares line i = L & 7 with
+            // lines j = L >> 3 and j + 4; the four partial counts of a line are added across lanes i, i+8, i+16, i+24.
+            // rp: rank among the lines to process, longest first; rb: among the lines to build, shortest first.
+            const int i = lane & 7, j0 = lane >> 3;
+            const uint32_t vi = __shfl_sync(0xffffffffu, mine, i);
+            const uint32_t va = __shfl_sync(0xffffffffu, mine, j0), vb = __shfl_sync(0xffffffffu, mine, j0 + 4);
+            const uint32_t pi = vi & 0xffffu, bi = vi >> 16;
+            uint32_t c2 = 0u;                                   // process count | build count << 8
+            c2 += ((va & 0xffffu) > pi || ((va & 0xffffu) == pi && j0 < i)) ? 1u : 0u;
+            c2 += ((vb & 0xffffu) > pi || ((vb & 0xffffu) == pi && j0 + 4 < i)) ? 1u : 0u;
+            c2 += ((va >> 16) < bi || ((va >> 16) == bi && j0 < i)) ? 256u : 0u;
+            c2 += ((vb >> 16) < bi || ((vb >> 16) == bi && j0 + 4 < i)) ? 256u : 0u;
+            c2 += __shfl_xor_sync(0xffffffffu, c2, 8);
+            c2 += __shfl_xor_sync(0xffffffffu, c2, 16);
+            const uint32_t rp = c2 & 0xffu, rb = c2 >> 8;       // line i is processed by warp rp, built by warp rb
+            if (lane < kPS && k < kMaxSteps) {
+                // s_asg[k][w]: low nibble = line processed by warp w, high nibble = line built by warp w
+                atomicOr((unsigned int*)&s_asg[k][0] + (rp >> 2), (uint32_t)i << (8 * (rp & 3)));
+                atomicOr((unsigned int*)&s_asg[k][0] + (rb >> 2), (uint32_t)i << (8 * (rb & 3) + 4));
+            }
+        }
+    }
+
+    // Time window of the current pass (set in the pass loop below).  Owned cells [tlo, thi): their peaks are found
+    // in this pass.  Stored cells [wlo, whi) = owned +- 2 bins: the 5x5 windows of owned peaks stay inside.
+    // With a single pass (MULTI = false) these are constants and the pass logic folds away.
+    uint32_t tlo = 0u, thi = T, wlo = 0u, whi = T, dsub = 0u;
+    bool last_pass = true;
+    uint32_t phase = 0u;                    // bit h: parity the next wait on staging piece h expects
+
+    // ---- staging: piece k of a line = digit slots [base + 128k, base + 128k + 128), base = first digit of the pass in
+    // the line, rounded down to a 16-byte boundary of global memory; ring half k mod 2.  Only lane 0 issues.
+    // Bulk copies move the 16-byte aligned part [bs, be) of the piece, cut at the line's end rounded out to 16 bytes; the
+    // first / last digit of the whole array, where it is ragged (at most one each), is copied by hand before the barrier
+    // is armed (the arrive releases those stores to the lanes that wait on the barrier).
+    auto issue_piece = [&](uint32_t base, uint32_t lend, uint32_t k) {
+        const int s = (int)base + 128 * (int)k;             // -1: the piece in front of digit 0 of a buffer 8 bytes off
+        const uint32_t e = min((uint32_t)(s + 128), lend);
+        const uint32_t dst = ring + (k & 1u) * kPieceBytes;
+        const uint32_t bar = bar0 + 8u * (k & 1u);
+        uint32_t bs = (uint32_t)s, be = e + ((e + gpar) & 1u);
+        if (s < (int)al_lo) {
+            bs = al_lo;
+            if (e > 0u && bs > 0u) {
+                const uint2 d = __ldg(digits);
+                asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dst + 8u), "r"(d.x), "r"(d.y) : "memory");
+            }
+        }
+        if (be > al_hi) {
+            be = al_hi;
+            if (e > be && (int)be >= s) {
+                const uint2 d = __ldg(digits + be);
+                asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dst + 8u * (uint32_t)((int)be - s)), "r"(d.x), "r"(d.y) : "memory");
+            }
+        }
+        if (be > bs) p_bulk_load(dst + 8u * (uint32_t)((int)bs - s), digits + bs, 8u * (be - bs), bar);
+        else p_mbar_arrive(bar);
+    };
+    // the first two pieces of the line this warp builds next (issued before the warp processes its current line, so the
+    // global latency is covered)
+    auto stage_head = [&](int p) {
+        if (p < blo || p >= bhi) return;
+        const uint32_t lbeg = s_pos[p], lend = s_ls[p + 1];
+        if (lend == lbeg) return;
+        if (lane == 0) {
+            const uint32_t base = lbeg - ((lbeg + gpar) & 1u);
+            const uint32_t np = (lend - base + 127u) >> 7;
+            issue_piece(base, lend, 0u);
+            if (np > 1u) issue_piece(base, lend, 1u);
+        }
+    };
+
+    // ---- K0 + K1 + stage A: this warp (re)builds slot v as line p ---------------------------------------------------
+    // The loop body carries no "does this digit exist" logic: the digit slots in front of the line's first digit and
+    // behind its last one are overwritten in the staging ring with SENTINEL digits (right key word, charge 1, a time
+    // >= n_time + 1: 0xffff in front, kSentT0 + k behind, ascending) once their chunk has landed.  A sentinel stores no
+    // cell, opens no block, survives no test, is adjacent to no real digit and keeps the order check quiet.
+    // (n_time < kSentT0 is a condition of this kernel's launcher.)
+    auto build_line = [&](int p, int v) {
+        const uint32_t slot = sm0 + (uint32_t)v * sg.slot_bytes;
+        {
+            // K0: header + directory, and the pool blocks the slot's last line opened
+            const uint32_t oldn = __shfl_sync(0xffffffffu, p_lds32(slot + 8u), 0);
+            const uint32_t pend = sg.pool_off + 16u * (min(oldn, sg.pcap - 1u) + 1u);
+            for (uint32_t x = (uint32_t)lane * 16u; x < pend; x += 512u) p_sts128z(slot + x);
+            __syncwarp();
+        }
+        if (p < blo || p >= bhi) return;                    // a line outside the plane / the halo: stays empty
+        const uint32_t lbeg = s_pos[p], lend = s_ls[p + 1], len = lend - lbeg;
+        if (lane == 0) p_sts32(slot + 4u, lbeg);            // hdr word 1: where this pass started in the line
+        if (len == 0) return;
+        const uint32_t lk = w0_base | ((uint32_t)p << 16);  // key word of the line's digits
+        const uint32_t a_dir1 = slot + kHdrBytes + 1u - (MULTI ? dsub : 0u); // dir byte of the block of time t: a_dir1 + (t >> 3)
+        const uint32_t a_pool = slot + sg.pool_off, a_surv = slot + sg.surv_off;
+        const uint32_t own_span = thi - tlo, win_span = whi - wlo;
+        const uint32_t nlo = thi - 2u;                      // the next pass needs the line from this time on
+        const uint32_t odd = (lbeg + gpar) & 1u;
+        const uint32_t base = lbeg - odd;
+        const uint32_t L = len + odd;                       // digit slots from base to the end of the line
+        const uint32_t np = (L + 127u) >> 7;                // pieces (bulk copies) of the line
+        const uint32_t c_last = L >> 6;                     // iteration c works on slots 64c-1 .. 64c+62
+        const uint32_t pcap = sg.pcap, scap = sg.scap;
+        uint32_t nblk = 0u, nsurv = 0u;                     // warp-uniform running counts
+        uint32_t ymin = 0xffffffffu;                        // per lane: smallest (time | charge << 16) seen: < 0x10000 = a zero charge
+        const uint32_t ylast = __ldg(&digits[lend - 1u].y);  // the line's last digit: is its time in range? (R11)
+        uint32_t next_pos = lend;                           // first digit with time >= nlo (warp-uniform)
+        bool found = false;
+        uint32_t iters = 0u;                                // iterations run
+        // order check of the pairs (prev, a) and (a, b): off in iteration 0 where the earlier one is a leading sentinel
+        uint32_t m_pa = (lane == 0 || (lane == 1 && odd)) ? 0u : 0x80000000u, m_ab = lane == 0 ? 0u : 0x80000000u;
+        uint32_t bad = 0u;
+        for (uint32_t c = 0; c <= c_last; ++c) {
+            const uint32_t e = c & 3u;                      // chunk of the ring this iteration reads
+            const uint32_t ent = ring + e * kChunkBytes;
+            ++iters;
+            if ((c & 1u) == 0u && (c >> 1) < np) {          // a new piece: has it landed?
+                const uint32_t h = (c >> 1) & 1u;
+                p_mbar_wait(bar0 + 8u * h, (phase >> h) & 1u);
+                phase ^= 1u << h;
+            }
+            if (c == 0u) {
+                // leading sentinels: slots -2, -1 (the guard) and, if the line starts 8 bytes off a boundary, slot 0
+                if (lane == 0) {
+                    p_sts128(ring - kGuard, make_uint4(lk, 0x1ffffu, lk, 0x1ffffu));
+                    if (odd) asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(ring), "r"(lk), "r"(0x1ffffu) : "memory");
+                }
+            }
+            if (c == c_last) {
+                // trailing sentinels: slots L .. 64 c + 63 of this (the last) chunk
+                const uint32_t k0 = L - 64u * c;            // first sentinel slot within the chunk (0 .. 63)
+#pragma unroll
+                for (uint32_t r = 0; r < 2u; ++r) {
+                    const uint32_t k = k0 + (uint32_t)lane + 32u * r;
+                    if (k < 64u)
+                        asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(ent + 8u * k), "r"(lk), "r"(0x10000u + kSentT0 + k - k0) : "memory");
+                }
+            }
+            if (c == 0u || c == c_last) __syncwarp();
+            const uint32_t addr = ent + 16u * (uint32_t)lane;      // digit b; a at -8; e = 0: lane 0 reads the guard
+            const uint2 A = p_lds64(addr - 8u), B = p_lds64(addr);
+            const uint32_t prevy = p_lds32(addr - 12u), nexty = p_lds32(addr + 12u);
+            // the ring's last 16 bytes are kept in the guard for lane 0 of the next iteration (entry 0)
+            if (e == 3u && lane == 31) p_sts128(ring - kGuard, p_lds128(addr));
+            __syncwarp();
+            // the piece in front of this iteration's is dead now: its half receives the piece after the next one
+            if (lane == 0 && (c & 1u) == 0u && c >= 2u && (c >> 1) + 1u < np) issue_piece(base, lend, (c >> 1) + 1u);
+            const uint32_t ya = A.y, yb = B.y;
+            const uint32_t ta = ya & 0xffffu, tb = yb & 0xffffu, tp = prevy & 0xffffu, tn = nexty & 0xffffu;
+            const uint32_t qa = ya >> 16, qb = yb >> 16, qp = prevy >> 16, qn = nexty >> 16;
+            // DIGITS_SORTED promise: right line, strictly ascending times (a duplicate cell breaks it too)
+            const uint32_t d_pa = ta - tp - 1u, d_ab = tb - ta - 1u, d_bn = tn - tb - 1u;   // 0: adjacent cells; < 0: not ascending
+            bad |= ((A.x ^ lk) | (B.x ^ lk)) & 0x00ffffffu;
+            bad |= (d_pa & m_pa) | (d_ab & m_ab);
+            m_pa = 0x80000000u; m_ab = 0x80000000u;
+            const bool inb_a = MULTI ? (ta - wlo) < win_span : ta < T;    // a cell this pass stores
+            const bool inb_b = MULTI ? (tb - wlo) < win_span : tb < T;
+            const bool own_a = MULTI ? (ta - tlo) < own_span : inb_a;     // a cell this pass decides
+            const bool own_b = MULTI ? (tb - tlo) < own_span : inb_b;
+            ymin = min(ymin, min(ya, yb));                  // R11: zero charges are looked for here, counted below
+            // K1: blocks are allocated in time order: a digit opens a block iff the digit before it is in another one
+            const bool head_a = inb_a && (ta ^ tp) > 7u;
+            const bool head_b = inb_b && (tb ^ ta) > 7u;
+            const unsigned hma = __ballot_sync(0xffffffffu, head_a), hmb = __ballot_sync(0xffffffffu, head_b);
+            const uint32_t idx_a = nblk + (uint32_t)__popc(hma & le_mask) + (uint32_t)__popc(hmb & lt_mask);   // 1-based
+            const uint32_t idx_b = idx_a + (head_b ? 1u : 0u);
+            nblk = __shfl_sync(0xffffffffu, idx_b, 31);     // blocks opened so far
+            if (nblk < pcap) {                              // (warp-uniform) every block so far is in the pool
+                if (head_a) p_sts8(a_dir1 + (ta >> 3), idx_a);
+                if (head_b) p_sts8(a_dir1 + (tb >> 3), idx_b);
+                if (inb_a) p_sts16(a_pool + (idx_a << 4) + ((ta & 7u) << 1), qa);
+                if (inb_b) p_sts16(a_pool + (idx_b << 4) + ((tb & 7u) << 1), qb);
+            } else {
+                if (head_a) p_sts8(a_dir1 + (ta >> 3), idx_a < pcap ? idx_a : 0xFFu);
+                if (head_b) p_sts8(a_dir1 + (tb >> 3), idx_b < pcap ? idx_b : 0xFFu);
+                if (inb_a && idx_a < pcap) p_sts16(a_pool + (idx_a << 4) + ((ta & 7u) << 1), qa);
+                if (inb_b && idx_b < pcap) p_sts16(a_pool + (idx_b << 4) + ((tb & 7u) << 1), qb);
+            }
+            // K2 stage A (R1, own line).  (0,-1) is earlier: the digit loses to an adjacent previous charge >= its
+            // own; (0,+1) is later: it loses to an adjacent next charge > its own (cells at time >= T read 0).
+            // With qe = charge of the adjacent cell (0 if there is no digit there): survive iff q >= max(q_peak_min,
+            // qe(previous) + 1, qe(next)).
+            const bool adj_ab = d_ab == 0u && tb < T;
+            const uint32_t qpe_a = d_pa == 0u ? qp + 1u : 0u, qne_a = adj_ab ? qb : 0u;
+            const uint32_t qpe_b = adj_ab ? qa + 1u : 0u, qne_b = (d_bn == 0u && tn < T) ? qn : 0u;
+            const bool surv_a = own_a && qa >= max(max(qpe_a, qne_a), q_peak_min);
+            const bool surv_b = own_b && qb >= max(max(qpe_b, qne_b), q_peak_min);
+            const unsigned sma = __ballot_sync(0xffffffffu, surv_a), smb = __ballot_sync(0xffffffffu, surv_b);
+            const uint32_t pos_a = nsurv + (uint32_t)__popc(sma & lt_mask) + (uint32_t)__popc(smb & lt_mask);
+            const uint32_t pos_b = pos_a + (surv_a ? 1u : 0u);
+            nsurv = __shfl_sync(0xffffffffu, pos_b + (surv_b ? 1u : 0u), 31);   // survivors so far
+            if (nsurv <= scap) {                            // (warp-uniform) the list holds every survivor so far
+                if (surv_a) p_sts32(a_surv + (pos_a << 2), ya);
+                if (surv_b) p_sts32(a_surv + (pos_b << 2), yb);
+            } else {
+                if (surv_a && pos_a < scap) p_sts32(a_surv + (pos_a << 2), ya);
+                if (surv_b && pos_b < scap) p_sts32(a_surv + (pos_b << 2), yb);
+            }
+            if (MULTI && !last_pass) {
+                // where the next pass starts in this line, and whether this pass has seen all it stores
+                const bool tail = c == c_last;              // this iteration reaches the last digit of the line
+                const uint32_t t31 = __shfl_sync(0xffffffffu, tb, 31);   // time of the iteration's last slot
+                if (!found && (tail || t31 >= nlo)) {
+                    unsigned ma = __ballot_sync(0xffffffffu, ta >= nlo);
+                    unsigned mb = __ballot_sync(0xffffffffu, tb >= nlo);
+                    if (c == 0u) { ma &= ~1u; mb &= ~odd; }     // leading sentinels
+                    if (ma | mb) {
+                        // first slot in order a0 b0 a1 b1 ...; line index of lane i's a is 64c + 2i - 1 - odd
+                        const int fa = ma ? __ffs(ma) - 1 : 64, fb = mb ? __ffs(mb) - 1 : 64;
+                        const uint32_t first = fa <= fb ? 2u * (uint32_t)fa : 2u * (uint32_t)fb + 1u;
+                        next_pos = min(lbeg + 64u * c + first - 1u - odd, lend);    // (a trailing sentinel: lend)
+                        found = true;
+                    }
+                }
+                if (!tail && t31 >= whi) break;             // every later digit is beyond the window
+            }
+        }
+        bad_order |= bad;
+        // chunks that were issued for iterations this pass did not run (early exit): consume their barrier phases
+        if (MULTI) {
+            const uint32_t last = iters - 1u;               // last iteration run
+            const uint32_t issued = min(np, 2u + (last >> 1)), waited = min(np, (last >> 1) + 1u);
+            for (uint32_t k = waited; k < issued; ++k) {
+                const uint32_t h = k & 1u;
+                p_mbar_wait(bar0 + 8u * h, (phase >> h) & 1u);
+                phase ^= 1u << h;
+            }
+        }
+        if (lane == 0) {
+            p_sts32(slot, nsurv);
+            p_sts32(slot + 8u, nblk);
+            p_sts32(slot + 12u, nblk >= pcap ? 1u : 0u);
+            if (MULTI && !last_pass) s_pos[p] = next_pos;
+        }
+        // R11: digits that are no cell with charge (time out of range, zero charge) are skipped and counted, by the pass
+        // that owns their time (the last one for times >= n_time).  They are rare: found by the minimum above and by
+        // the line's last digit, then counted from the digit array.
+        if (p >= pa && p < pb) {                            // halo lines are counted by the unit that owns them
+            const bool zero_q = __reduce_min_sync(0xffffffffu, ymin) < 0x10000u;
+            const bool late_t = (!MULTI || last_pass) && (ylast & 0xffffu) >= T;
+            if (zero_q || late_t) {
+                uint32_t nbad = 0u;
+                for (uint32_t j = lbeg + (uint32_t)lane; j < lend; j += 32u) {
+                    const uint32_t y = __ldg(&digits[j].y), t = y & 0xffffu;
+                    const bool own = MULTI ? (t - tlo) < own_span : t < T;
+                    const bool considered = !MULTI ? true : (last_pass ? t >= tlo : own);
+                    if (considered && !(own && y >= 0x10000u)) ++nbad;
+                }
+                nbad = __reduce_add_sync(0xffffffffu, nbad);
+                if (nbad != 0u && lane == 0) atomicAdd(&cnt->n_bad, (unsigned long long)nbad);
+            }
+        }
+    };
+
+    // ---- K2 stage B + K4 stage C for line p (ring index vp), owned by this warp -------------------------------------
+    auto process_line = [&](int p, int vp, const bool OVF) {
+        const uint32_t gl = s_ls[p], lend = s_ls[p + 1];
+        uint32_t sl[5];                                     // slots of lines p-2 .. p+2 (empty outside the plane, R2)
+        {
+            const uint32_t ring_end = sm0 + kPSlots * sg.slot_bytes;
+            uint32_t a0 = sm0 + (uint32_t)pring_at(vp, -2) * sg.slot_bytes;
+#pragma unroll
+            for (int a = 0; a < 5; ++a) {
+                sl[a] = a0;
+                a0 += sg.slot_bytes;
+                if (a0 == ring_end) a0 = sm0;
+            }
+        }
+        const uint32_t w0_line = w0_base | ((uint32_t)p << 16);
+        uint32_t pcount = 0, pdone = MULTI ? s_cnt[p] : 0u; // warp-uniform: queued / already written peaks of the line
+
+        // stage C for up to 32 queued peaks (one per lane): y = (time | qmax << 16).  Clusters that pass the cuts (V2;
+        // all of them by default) are written in lane order from ordinal `pdone` on; returns how many.
+        auto moments = [&](bool valid, uint32_t y) -> uint32_t {
+            bool keep = false;
+            ClusterSums sums = {0, 0, 0, 0, 0};
+            uint32_t fl = 0u;
+            const uint32_t t = y & 0xffffu;
+            if (valid) {
+                int c[5][5];
+#pragma unroll
+                for (int a = 0; a < 5; ++a) pwindow<2>(sl[a], MULTI ? dsub : 0u, sg, (int)t, c[a], digits, s_ls, p + a - 2, P, T, OVF);
+                sums = cluster_sums(c, q_gate);
+                keep = VAR ? cluster_variant(sums, (uint32_t)p, t, y >> 16, (uint32_t)P, T, var, &fl) : true;
+            }
+            const unsigned km = __ballot_sync(0xffffffffu, keep);
+            if (keep) {
+                const ClusterWords r = cluster_finish(sums, w0_line, t, y >> 16, fl);
+                const size_t j = (size_t)gl + pdone + (uint32_t)__popc(km & lt_mask);   // line's range, time order
+                stage[2 * j] = r.lo;
+                stage[2 * j + 1] = r.hi;
+            }
+            return (uint32_t)__popc(km);
+        };
+        // stage B for up to 32 survivors (one per lane); peaks go to the warp's queue, stage C runs on full warps
+        auto stage_b = [&](bool act, uint32_t y) {
+            bool peak = false;
+            if (act) {
+                const int t = (int)(y & 0xffffu);
+                const uint32_t q = y >> 16;
+                int cm[3], cp[3];
+                pwindow<1>(sl[1], MULTI ? dsub : 0u, sg, t, cm, digits, s_ls, p - 1, P, T, OVF);   // line p-1: earlier, strict (R1)
+                pwindow<1>(sl[3], MULTI ? dsub : 0u, sg, t, cp, digits, s_ls, p + 1, P, T, OVF);   // line p+1: later, >=
+                peak = q > (uint32_t)max(cm[0], max(cm[1], cm[2])) && q >= (uint32_t)max(cp[0], max(cp[1], cp[2]));
+            }
+            const unsigned pm = __ballot_sync(0xffffffffu, peak);
+            if (pm == 0u) return;
+            if (peak) p_sts32(pqa + ((pcount + (uint32_t)__popc(pm & lt_mask)) << 2), y);
+            pcount += (uint32_t)__popc(pm);
+            __syncwarp();
+            if (pcount >= 32u) {
+                pdone += moments(true, p_lds32(pqa + ((uint32_t)lane << 2)));
+                const uint32_t mv = p_lds32(pqa + (((uint32_t)lane + 32u) << 2));
+                __syncwarp();
+                p_sts32(pqa + ((uint32_t)lane << 2), mv);
+                pcount -= 32u;
+                __syncwarp();
+            }
+        };
+
+        const uint32_t ns = p_lds32(sl[2]);
+        const uint32_t nst = min(ns, sg.scap);
+        for (uint32_t i = 0; i < nst; i += 32u) {
+            const bool act = i + (uint32_t)lane < nst;
+            stage_b(act, act ? p_lds32(sl[2] + sg.surv_off + ((i + (uint32_t)lane) << 2)) : 0u);
+        }
+        if (ns > sg.scap) {
+            // rare: more survivors than the slot's list holds.  Stage A again from the digit array, from where this
+            // pass started in the line; survivors whose ordinal is >= scap were not listed and are tested here
+            // (still in time order).
+            const uint32_t lbeg = p_lds32(sl[2] + 4u), len = lend - lbeg;
+            uint32_t seen = 0;
+            for (uint32_t c0 = 0; c0 < len; c0 += 32u) {
+                const uint32_t jl = c0 + (uint32_t)lane;
+                const bool act = jl < len;
+                const uint32_t y = act ? __ldg(&digits[lbeg + jl].y) : 0u;
+                const uint32_t prevy = jl > 0u && act ? __ldg(&digits[lbeg + jl - 1u].y) : 0u;
+                const uint32_t nexty = jl + 1u < len ? __ldg(&digits[lbeg + jl + 1u].y) : 0u;
+                const bool surv = act && (MULTI ? ((y & 0xffffu) - tlo) < (thi - tlo) : (y & 0xffffu) < T) &&
+                                  p_stage_a(y, prevy, jl > 0u, nexty, jl + 1u < len, T, q_peak_min);
+                const unsigned smk = __ballot_sync(0xffffffffu, surv);
+                const uint32_t ord = seen + (uint32_t)__popc(smk & lt_mask);
+                seen += (uint32_t)__popc(smk);
+                if (seen > sg.scap) stage_b(surv && ord >= sg.scap, y);
+                if (seen >= ns) break;                      // all survivors of this pass have been seen
+            }
+        }
+        if (pcount > 16u) {
+            pdone += moments((uint32_t)lane < pcount, p_lds32(pqa + (((uint32_t)lane & 31u) << 2)));
+        } else if (pcount > 0u) {
+            // the usual case (a line has ~14 peaks): two lanes per peak, each gathers the rows on one side of the
+            // peak plus the peak's row (3 windows instead of 5); the halves of the integer sums are added by shuffle
+            const uint32_t i = (uint32_t)lane & 15u;
+            const bool neg = lane >= 16;                        // this lane takes dp < 0 (lines p-2, p-1)
+            const bool valid = i < pcount;
+            ClusterSums h = {0, 0, 0, 0, 0};
+            uint32_t y = 0u;
+            if (valid) {
+                y = p_lds32(pqa + (i << 2));
+                const int t = (int)(y & 0xffffu);
+                int o[5], m[5], z[5];
+                pwindow<2>(neg ? sl[0] : sl[4], MULTI ? dsub : 0u, sg, t, o, digits, s_ls, neg ? p - 2 : p + 2, P, T, OVF);
+                pwindow<2>(neg ? sl[1] : sl[3], MULTI ? dsub : 0u, sg, t, m, digits, s_ls, neg ? p - 1 : p + 1, P, T, OVF);
+                pwindow<2>(sl[2], MULTI ? dsub : 0u, sg, t, z, digits, s_ls, p, P, T, OVF);
+                h = cluster_half_sums(o, m, z, neg ? -1 : 1, !neg, q_gate);
+            }
+            h.S0 += __shfl_xor_sync(0xffffffffu, h.S0, 16);
+            h.S1p += __shfl_xor_sync(0xffffffffu, h.S1p, 16);
+            h.S1t += __shfl_xor_sync(0xffffffffu, h.S1t, 16);
+            h.S2p += __shfl_xor_sync(0xffffffffu, h.S2p, 16);
+            h.S2t += __shfl_xor_sync(0xffffffffu, h.S2t, 16);
+            bool keep = valid && !neg;
+            uint32_t fl = 0u;
+            if (VAR && keep)
+                keep = cluster_variant(h, (uint32_t)p, y & 0xffffu, y >> 16, (uint32_t)P, T, var, &fl);
+            const unsigned km = __ballot_sync(0xffffffffu, keep);
+            if (keep) {
+                const ClusterWords r = cluster_finish(h, w0_line, y & 0xffffu, y >> 16, fl);
+                const size_t j = (size_t)gl + pdone + (uint32_t)__popc(km & lt_mask);
+                stage[2 * j] = r.lo;
+                stage[2 * j + 1] = r.hi;
+            }
+            pdone += (uint32_t)__popc(km);
+        }
+        if (lane == 0) {
+            if (MULTI) s_cnt[p] = pdone;                    // clusters of this line so far, in time order
+            if (!MULTI || last_pass) line_cnt[plane * g.LS + p] = pdone;
+        }
+    };
+    auto process = [&](int p, int vp) {
+        if (s_ls[p + 1] == s_ls[p]) return;                 // line_cnt stays 0 (cleared per run)
+        // does any of the five lines keep blocks outside its pool?  (hdr word 3; warp-uniform)
+        uint32_t ovf = 0u;
+#pragma unroll
+        for (int a = -2; a <= 2; ++a) ovf |= p_lds32(sm0 + (uint32_t)pring_at(vp, a) * sg.slot_bytes + 12u);
+        process_line(p, vp, ovf != 0u);
+    };
+
+    // ---- main loop -------------------------------------------------------------------------------------------------
+    // The time axis is covered in sg.n_pass passes over the unit's lines (smaller slots -> more CTAs per SM).
+    __syncthreads();                                            // s_asg complete
+    for (uint32_t pass = 0; pass < (MULTI ? sg.n_pass : 1u); ++pass) {
+    if (MULTI) {
+        last_pass = pass + 1u == sg.n_pass;
+        tlo = pass * sg.seg_len;
+        thi = last_pass ? T : min(tlo + sg.seg_len, T);
+        wlo = tlo >= 2u ? tlo - 2u : 0u;
+        whi = min(thi + 2u, T);
+        dsub = tlo >> 3;
+    }
+    // Ring index of line p is (p - (pa - 2)) mod kPSlots.  Rounds -2 and -1 build lines pa-2 .. pa+S+1 (S + 4 = 12 lines:
+    // warp w builds line pa-2+w, then warps 0..3 lines pa+S-2 .. pa+S+1).  Step l0 >= pa (ONE barrier): every warp stages
+    // the head of the line it will build, runs stages B+C on its current line (lines l0-2 .. l0+S+1 are complete), then
+    // rebuilds the slot of a line that left the ring (l0-S-2 .. l0-3).  One copy of the code serves both.
+    int vl0 = 2;                                                // ring index of line l0
+    int step = -2;
+    for (int l0 = pa - 2 * kPS; l0 < pb; l0 += kPS, ++step) {
+        int pnew, vnew;
+        bool doit;
+        int ip = 0;
+        if (step < 0) {
+            const int i = (step + 2) * kPS + warp;              // ring index = line - (pa - 2)
+            pnew = pa - 2 + i; vnew = i;
+            doit = i < kPS + 4;
+        } else {
+            const uint32_t asg = __shfl_sync(0xffffffffu, (uint32_t)s_asg[step & (kMaxSteps - 1)][warp], 0);
+            ip = (int)(asg & 15u);                              // which of the 8 lines this warp processes / builds
+            const int ib = (int)(asg >> 4);
+            pnew = l0 + kPS + 2 + ib; vnew = pring_at(vl0, kPS + 2 + ib - kPSlots);
+            doit = l0 + kPS < pb;                               // lines l0+S+2 .. l0+2S+1 enter the ring in this step
+        }
+        if (doit) stage_head(pnew);
+        if (step >= 0 && l0 + ip < pb) process(l0 + ip, pring_at(vl0, ip));
+        if (doit) build_line(pnew, vnew);
+        if (step != -2) {
+            __syncthreads();
+            if (step >= 0) vl0 = pring_at(vl0, kPS);
+        }
+    }
+    }   // passes
+    if (bad_order) s_unsorted = 1;
+    __syncthreads();
+    if (tid == 0 && s_unsorted) atomicOr(&cnt->unsorted, 1u);
+}
+
+cudaError_t fused_pairs_set_attributes()
+{
+    cudaError_t e = cudaSuccess;
+    auto set = [&](const void* f, int bytes) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    };
+    set((const void*)k_fused_pairs<false, false, 2>, 112 * 1024); set((const void*)k_fused_pairs<true, false, 2>, 112 * 1024);
+    set((const void*)k_fused_pairs<false, true, 2>, 112 * 1024);  set((const void*)k_fused_pairs<true, true, 2>, 112 * 1024);
+    set((const void*)k_fused_pairs<false, false, 3>, 72 * 1024);  set((const void*)k_fused_pairs<true, false, 3>, 72 * 1024);
+    set((const void*)k_fused_pairs<false, true, 3>, 72 * 1024);   set((const void*)k_fused_pairs<true, true, 3>, 72 * 1024);
+    return e;
+}
+
+// Launches k_fused_pairs after the line index is in ws.line_start.  Returns 1 (launched), 0 (not applicable: the
+// mean line would not fit the block pool in <= 6 passes; the caller runs the bitmap kernel instead) or a negative
+// tpc_cf error.  Launch shape: 2 CTAs of 8 warps per SM (3 when the slots are small: short lines).  Lines too long
+// for the 254-block pool are covered in several passes over the time axis (dir, pool and survivor list all scale with
+// the segment length).
+int launch_fused_pairs(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
+                       uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, bool must,
+                       cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1)
+{
+    if (g.n_time >= kSentT0) return 0;        // the sentinel digits of the build loop need times above every real one
+    uint64_t total_pads = 0;
+    for (uint32_t r = 0; r < g.n_rows; ++r) total_pads += g.npads[r];
+    total_pads *= g.n_sectors;
+    // shape_n: digits of the whole frame when this run covers only some of its sectors (tpc_cf_run_host pipeline)
+    const double mean_len = (double)(shape_n ? shape_n : n) / (double)(total_pads ? total_pads : 1);
+    // measured on the synthetic frames: 0.38 blocks and 0.16 stage-A survivors per digit
+    const double mean_blocks = 0.38 * mean_len, mean_surv = 0.16 * mean_len;
+
+    const uint32_t fixed = kPWarps * (kStgBytes + kPqBytes);
+    const uint32_t stat = 4608u;                                    // static shared memory of the kernel, rounded up
+    const uint32_t budget = 227u * 1024u / 2u - 1024u - stat;      // 2 CTAs per SM: - 1 KB reserved each
+    auto shape = [&](uint32_t n_pass, bool force, SlotGeo* out) -> bool {
+        SlotGeo sg;
+        sg.n_pass = n_pass;
+        sg.seg_len = (((g.n_time + n_pass - 1u) / n_pass) + 7u) & ~7u;
+        const uint32_t dir_bytes = ((sg.seg_len >> 3) + 2u + 15u) & ~15u;
+        sg.pool_off = kHdrBytes + dir_bytes;
+        const double mb = mean_blocks / n_pass + (n_pass > 1 ? 1.0 : 0.0), ms = mean_surv / n_pass;
+        sg.scap = (((uint32_t)(ms * 1.5) + 12u) + 3u) & ~3u;
+        uint32_t want = (uint32_t)(mb * 1.5) + 24u;                // blocks incl. the zero block
+        if (want > 255u) want = 255u;
+        const uint32_t per_slot_fixed = sg.pool_off + 4u * sg.scap;
+        if (fixed + kPSlots * (per_slot_fixed + 16u * 8u) > budget) return false;
+        const uint32_t fit = ((budget - fixed) / kPSlots - per_slot_fixed) / 16u;
+        sg.pcap = want < fit ? want : fit;
+        if (!force && (double)sg.pcap < mb * 1.2 + 8.0) return false;   // too many lines would overflow the pool
+        *out = sg;
+        return true;
+    };
+    // Passes: 1 when the mean line fits the pool, else the fewest that do (each pass costs a partly used chunk and a
+    // partly filled survivor / peak batch per line, so fewer is better).
+    SlotGeo sg;
+    bool have = false;
+    for (uint32_t np = 1; np <= 6 && !have; ++np) {
+        if (tun.passes && (int)np != tun.passes) continue;
+        if (np > 1 && g.n_time < 64u * np) break;
+        have = shape(np, false, &sg);
+    }
+    if (!have) {
+        if (!must) return 0;
+        if (tun.passes >= 1 && tun.passes <= 8 && g.n_time >= 64u * (uint32_t)tun.passes) have = shape((uint32_t)tun.passes, true, &sg);
+        for (uint32_t np = 1; np <= 8 && !have; ++np) have = (np == 1 || g.n_time >= 64u * np) && shape(np, true, &sg);
+        if (!have) return 0;
+    }
+    if (tun.block_pool >= 2 && tun.block_pool <= 255 && (uint32_t)tun.block_pool <= sg.pcap) sg.pcap = (uint32_t)tun.block_pool;
+    if (tun.surv_cap >= 4 && (uint32_t)tun.surv_cap <= sg.scap) sg.scap = (uint32_t)tun.surv_cap & ~3u;
+    sg.surv_off = sg.pool_off + 16u * sg.pcap;
+    sg.slot_bytes = sg.surv_off + 4u * sg.scap;
+    const uint32_t smem = kPSlots * sg.slot_bytes + fixed;
+
+    const uint32_t whole = (g.max_pads + kPS - 1) / kPS * kPS;
+    uint32_t pads_per_unit = g.n_planes >= 1184 ? whole : (g.n_planes >= 296 ? 6 * kPS : 3 * kPS);
+    if (pads_per_unit > whole) pads_per_unit = whole;
+    if (tun.pads_per_unit >= kPS && tun.pads_per_unit <= 256) pads_per_unit = (uint32_t)(tun.pads_per_unit / kPS * kPS);
+    const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
+    if (ev_k0) cudaEventRecord(ev_k0, st);
+    g_last_kernel = "k_fused_pairs";
+    // a third CTA per SM when the slots are small (short lines): the kernel is latency bound
+    const uint32_t budget3 = 227u * 1024u / 3u - 1024u - stat;
+    const bool three = smem <= budget3 && tun.ctas_per_sm != 2;
+    const bool m = sg.n_pass > 1, v = var.active != 0u;
+    auto kern = three ? (m ? (v ? k_fused_pairs<true, true, 3> : k_fused_pairs<true, false, 3>)
+                           : (v ? k_fused_pairs<false, true, 3> : k_fused_pairs<false, false, 3>))
+                      : (m ? (v ? k_fused_pairs<true, true, 2> : k_fused_pairs<true, false, 2>)
+                           : (v ? k_fused_pairs<false, true, 2> : k_fused_pairs<false, false, 2>));
+    kern<<<g.n_planes * upp, kPThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
+                                                    pads_per_unit, upp, sg, q_peak_min, q_gate, var,
+                                                    ws.counters, ws.line_cnt, (uint4*)ws.stage);
+    if (ev_k1) cudaEventRecord(ev_k1, st);
+    return 1;
+}
+
+}  // namespace tpccf

@@ -37,29 +37,29 @@ def parse_golden(path=GOLDEN):
 
 
 # flags: DIGITS_SORTED=1, FORCE_GENERAL=2.  "fused" lets the library choose the fused kernel from the mean line length;
-# "fused_blocks" / "fused_lines" force the block-sparse / bitmap line-slot kernel (TPC_CF_FUSED_KERNEL), so that each
+# "fused_pairs" / "fused_blocks" / "fused_lines" force one of the three fused kernels (tpc_cf_debug_set), so that each
 # runs every case — including the ones far outside its range, which exercise its exact slow paths.
-# "fused_blocks_p3" additionally covers the time axis in 3 passes (TPC_CF_PASSES), the shape long lines get.
-PATHS = {"general": 0, "general_hint": 3, "fused": 1, "fused_blocks": 1, "fused_blocks_p3": 1, "fused_lines": 1}
-FUSED_KERNEL = {"fused_blocks": "k_fused_blocks", "fused_blocks_p3": "k_fused_blocks", "fused_lines": "k_fused_lines"}
+# "*_p3" additionally covers the time axis in 3 passes, the shape long lines get.
+PATHS = {"general": 0, "general_hint": 3, "fused": 1, "fused_pairs": 1, "fused_pairs_p3": 1, "fused_blocks": 1,
+         "fused_blocks_p3": 1, "fused_lines": 1}
+TUNING = {"fused_pairs": dict(fused_kernel="pairs"), "fused_pairs_p3": dict(fused_kernel="pairs", passes=3),
+          "fused_blocks": dict(fused_kernel="blocks"), "fused_blocks_p3": dict(fused_kernel="blocks", passes=3),
+          "fused_lines": dict(fused_kernel="lines")}
+_tuning = {}
 
 
 @pytest.fixture(autouse=True)
-def _fused_kernel_env(request, monkeypatch):
-    """Sets the library's kernel-selection knob from the test's `path` parameter (read with getenv at every run)."""
+def _fused_kernel_tuning(request):
+    """The handle overrides (tpc_cf_debug_set) the test's `path` parameter asks for; gpu_run applies them."""
     params = getattr(getattr(request.node, "callspec", None), "params", {})
-    for k in ("TPC_CF_FUSED_KERNEL", "TPC_CF_BLOCK_POOL", "TPC_CF_SURV_CAP", "TPC_CF_PASSES"):
-        monkeypatch.delenv(k, raising=False)
-    path = params.get("path")
-    if path in FUSED_KERNEL:
-        monkeypatch.setenv("TPC_CF_FUSED_KERNEL", "lines" if path == "fused_lines" else "blocks")
-        if path == "fused_blocks_p3":
-            monkeypatch.setenv("TPC_CF_PASSES", "3")
+    _tuning.clear()
+    _tuning.update(TUNING.get(params.get("path"), {}))
     yield
+    _tuning.clear()
 
 
 def gpu_run(digits, geom, flags, max_clusters=None, capacity=None, q_peak_min=4, q_inner_gate=2, finder=None,
-            q_tot_min=0, q_saturation=0):
+            q_tot_min=0, q_saturation=0, tuning=None, expect_kernel=None):
     cf = _cf()
     n_sectors, n_rows, max_pads, n_time, npads = geom
     n = int(digits.shape[0])
@@ -69,11 +69,13 @@ def gpu_run(digits, geom, flags, max_clusters=None, capacity=None, q_peak_min=4,
                                   max_clusters=max_clusters if max_clusters is not None else max(n, 1),
                                   q_peak_min=q_peak_min, q_inner_gate=q_inner_gate, q_tot_min=q_tot_min,
                                   q_saturation=q_saturation)
+    tun = dict(_tuning) if tuning is None else dict(tuning)
+    finder.debug_set(**tun)
     d = cf.to_device(digits)
     finder.run(d, n, flags=flags, capacity=capacity)
     cl, st = finder.result()
     st["kernel"] = finder.last_kernel()
-    forced = os.environ.get("TPC_CF_FUSED_KERNEL")
+    forced = tun.get("fused_kernel") if expect_kernel is None else expect_kernel
     if forced and n and st["path"] == 3:
         assert st["kernel"] == "k_fused_" + forced, (st["kernel"], forced)
     if capacity is not None:
@@ -344,28 +346,26 @@ def test_dense_isolated_peaks_overflow_the_peak_queue(path):
     assert_clusters_equal(cl, ora, "dense isolated peaks/" + path)
 
 
+@pytest.mark.parametrize("kernel", ["pairs", "blocks"])
 @pytest.mark.parametrize("passes", [1, 2, 5])
 @pytest.mark.parametrize("pool,scap", [(2, 4), (9, 8), (40, 4), (255, 12)])
-def test_block_kernel_slow_paths(pool, scap, passes, monkeypatch):
-    """k_fused_blocks with a block pool / survivor list far too small for the data (TPC_CF_BLOCK_POOL,
-    TPC_CF_SURV_CAP): window cells whose block is not in the pool are looked up in the digit array, survivors beyond
-    the list are re-derived from the digit array.  Results must not change (config 1, and a ~5 % single row)."""
-    monkeypatch.setenv("TPC_CF_FUSED_KERNEL", "blocks")
-    monkeypatch.setenv("TPC_CF_BLOCK_POOL", str(pool))
-    monkeypatch.setenv("TPC_CF_SURV_CAP", str(scap))
-    monkeypatch.setenv("TPC_CF_PASSES", str(passes))
+def test_block_kernel_slow_paths(pool, scap, passes, kernel):
+    """The block-sparse kernels with a block pool / survivor list far too small for the data (tpc_cf_debug_set
+    block_pool, surv_cap): window cells whose block is not in the pool are looked up in the digit array, survivors
+    beyond the list are re-derived from the digit array.  Results must not change (config 1, and a ~5 % single row)."""
+    tun = dict(fused_kernel=kernel, block_pool=pool, surv_cap=scap, passes=passes)
     digits = gen.generate(1)
     geom = gen.geometry(1)
     ora, ost = orc.run(digits, *geom[:4], npads=geom[4])
-    cl, st = gpu_run(digits, geom, 1)
-    assert st["kernel"] == "k_fused_blocks" and st["n_clusters"] == ost["n_clusters"]
+    cl, st = gpu_run(digits, geom, 1, tuning=tun)
+    assert st["kernel"] == "k_fused_" + kernel and st["n_clusters"] == ost["n_clusters"]
     assert_clusters_equal(cl, ora, "config 1, pool %d scap %d" % (pool, scap))
     c = dict(gen.CONFIGS[2]); c["n_rows"] = 2
     geom = gen.geometry(c)
     digits = gen.generate(c)
     ora, ost = orc.run(digits, *geom[:4])
-    cl, st = gpu_run(digits, geom, 1)
-    assert st["kernel"] == "k_fused_blocks" and st["n_clusters"] == ost["n_clusters"]
+    cl, st = gpu_run(digits, geom, 1, tuning=tun)
+    assert st["kernel"] == "k_fused_" + kernel and st["n_clusters"] == ost["n_clusters"]
     assert_clusters_equal(cl, ora, "config 2 (2 rows), pool %d scap %d" % (pool, scap))
 
 
@@ -455,11 +455,13 @@ def test_variants_full_parity(v, path):
 
 
 @pytest.mark.parametrize("path", list(PATHS))
-def test_maximum_geometry(path, monkeypatch):
+def test_maximum_geometry(path):
     """The largest plane the 8/16-bit record fields allow (255 pads x 65535 time bins), sparse clusters plus digits in
-    the last pads and time bins, and odd sizes that are no multiple of the kernels' tile sizes (7 pads x 61 bins)."""
+    the last pads and time bins, and odd sizes that are no multiple of the kernels' tile sizes (7 pads x 61 bins).
+    The bitmap slots of k_fused_lines do not fit shared memory above ~50 k time bins and k_fused_pairs needs
+    n_time < 65470 (its sentinel times): the library then runs k_fused_blocks, which takes any geometry."""
     rng = np.random.default_rng(21)
-    for (P, T, ncl) in ((255, 65535, 4000), (7, 61, 12), (9, 257, 40)):
+    for (P, T, ncl) in ((255, 65535, 4000), (255, 65469, 2000), (7, 61, 12), (9, 257, 40)):
         cells = {}
         for _ in range(ncl):
             p0, t0 = int(rng.integers(0, P)), int(rng.integers(0, T))
@@ -473,12 +475,11 @@ def test_maximum_geometry(path, monkeypatch):
         digits = sort_digits(orc.make_digits([(p, t, q) for (p, t), q in cells.items()]))
         geom = (1, 1, P, T, None)
         ora, ost = orc.run(digits, *geom[:4])
-        if path == "fused_lines" and T > 40000:
-            # 20 bitmap slots of 65535 bins do not fit in shared memory: the library runs the block kernel instead
-            monkeypatch.delenv("TPC_CF_FUSED_KERNEL")
-        cl, st = gpu_run(digits, geom, PATHS[path], max_clusters=ost["n_clusters"] + 8)
-        if path == "fused_lines" and T > 40000:
-            assert st["kernel"] == "k_fused_blocks"
-            monkeypatch.setenv("TPC_CF_FUSED_KERNEL", "lines")
+        expect = None
+        if T > 65469 and path in ("fused_lines", "fused_pairs", "fused_pairs_p3"):
+            expect = "blocks"
+        elif T > 40000 and path == "fused_lines":
+            expect = "pairs"
+        cl, st = gpu_run(digits, geom, PATHS[path], max_clusters=ost["n_clusters"] + 8, expect_kernel=expect)
         assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == 0
         assert_clusters_equal(cl, ora, "max geometry %dx%d/%s" % (P, T, path))
