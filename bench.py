@@ -628,6 +628,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-parity", action="store_true",
+                    help="skip the element-by-element comparison of every cluster with the oracle (all host cores)")
+    ap.add_argument("--no-per-config", dest="per_config", action="store_false",
+                    help="only the headline config (default: the other four configs of BASELINE.json are measured and "
+                         "compared with the oracle too, in a per_config block of the same JSON line)")
     ap.add_argument("--variant", default="none", choices=["none", "flags", "cuts"],
                     help="cluster-finder variants (SURVEY.md §8(f) NEXT #1): 'flags' = per-cluster flags, 'cuts' = "
                          "flags + q_tot_min 40 + single-pad cut; the default run has none")
@@ -656,6 +661,168 @@ def main():
     if args.shard:
         return run_shard(args)
 
+    return run_cf(args)
+
+
+# ---- comparison with the oracle (the bar of tests/parity.py, restated: bench.py does not import the tests) -------------
+INT_FIELDS = ("sector", "row", "pad", "flags", "time", "qmax", "qtot", "rsv")
+FLOAT_FIELDS = ("pad_mean", "time_mean", "sigma_pad", "sigma_time")
+
+
+def compare_clusters(gpu, ora):
+    """Element by element: integer fields bit-exact; floats pass iff |g-o| <= 1e-4 or <= 1e-5 |o| (north_star).
+    Returns a dict for the JSON line; "ok" False on any mismatch."""
+    res = {"clusters_gpu": int(gpu.shape[0]), "clusters_oracle": int(ora.shape[0]), "ok": True, "mismatch": None}
+    if gpu.shape[0] != ora.shape[0]:
+        res.update(ok=False, mismatch="cluster count")
+        return res
+    for f in INT_FIELDS:
+        bad = int(np.count_nonzero(gpu[f] != ora[f]))
+        if bad:
+            res.update(ok=False, mismatch="%s differs at %d clusters" % (f, bad))
+            return res
+    err = {}
+    for f in FLOAT_FIELDS:
+        g, o = gpu[f].astype(np.float64), ora[f].astype(np.float64)
+        e = np.abs(g - o)
+        bad = int(np.count_nonzero(~((e <= 1e-4) | (e <= 1e-5 * np.abs(o)))))
+        err[f] = float(e.max()) if e.size else 0.0
+        if bad:
+            res.update(ok=False, mismatch="%s out of tolerance at %d clusters" % (f, bad))
+    res["max_abs_err"] = err
+    res["clusters_checked"] = int(gpu.shape[0])
+    return res
+
+
+def measure_config(cf, torch, cfg_id, steps, warmup, path, variant, dev, frame_offset=0, parity=True, sampler=None,
+                   keep=False):
+    """One config, device-resident: generate its frame(s), run `steps` timed steps (a step = every frame of the config
+    through tpc_cf_run, back to back on one stream), time the dominant kernel by its own event pair, and compare every
+    cluster of every frame with the oracle run on all host cores.  Returns a dict (and, with keep, the live objects)."""
+    from datagen import gen
+    cfg = gen.CONFIGS[cfg_id]
+    geom = gen.geometry(cfg_id)
+    n_frames = cfg["frames"]
+    t0 = time.perf_counter()
+    frames = [gen.generate(cfg_id, frame=frame_offset + f) for f in range(n_frames)]
+    gen_s = time.perf_counter() - t0
+    n_digits = [int(f.shape[0]) for f in frames]
+    nmax = max(n_digits)
+    max_clusters = nmax // 10 + 1024
+    vflags = {"none": 0, "flags": cf.CLUSTER_FLAGS, "cuts": cf.CLUSTER_FLAGS | cf.CUT_SINGLE_PAD}[variant]
+    finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=nmax, max_clusters=max_clusters, device=dev,
+                              q_tot_min=40 if variant == "cuts" else 0,
+                              q_saturation=1000 if variant != "none" else 0)
+    flags = (cf.DIGITS_SORTED if path == "fused" else (cf.DIGITS_SORTED | cf.FORCE_GENERAL)) | vflags
+    pinned = [torch.from_numpy(f.view(np.uint8)).pin_memory() for f in frames] if keep else None
+    dev_digits = [(p if p is not None else torch.from_numpy(f.view(np.uint8))).to(dev, non_blocking=True)
+                  for p, f in zip(pinned or [None] * n_frames, frames)]
+    outs = [torch.empty(max_clusters * 32, dtype=torch.uint8, device=dev) for _ in frames]
+    stats = [torch.zeros(32, dtype=torch.uint8, device=dev) for _ in frames]
+    torch.cuda.synchronize()
+
+    def step():
+        for d, n, o, s in zip(dev_digits, n_digits, outs, stats):
+            finder.run(d, n, flags=flags, clusters=o, status=s)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    sts = [finder.result(clusters=o, status=s)[1] for o, s in zip(outs, stats)]
+    for st in sts:
+        if st["path"] == 0 or st["overflow"]:
+            raise RuntimeError("bench run invalid: status %r" % (st,))
+    n_clusters = [st["n_clusters"] for st in sts]
+    # inputs + outputs of one step against the 126 MB L2: small configs are timed with an L2 flush before every step
+    step_bytes = 8 * sum(n_digits) + 32 * sum(n_clusters)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if step_bytes < (252 << 20) else None
+    res = {"frames_per_step": n_frames, "digits": n_digits, "clusters": n_clusters,
+           "launches_per_step": finder.last_launch_count() * n_frames, "kernel": finder.last_kernel(),
+           "gen_seconds": gen_s, "occupancy": gen.occupancy(frames[0], cfg_id),
+           "l2": ("inputs (%.2f GB digits per frame) larger than the 126 MB L2; no flush" % (nmax * 8 / 1e9)) if flush is None
+                 else "step data (%.1f MB) fits the 126 MB L2: 256 MB written before every timed step (L2 flush)" % (step_bytes / 1e6)}
+    finder.set_profiling(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ctx = sampler if sampler is not None else _NullCtx()
+    with ctx:
+        if flush is None:
+            ev0.record()
+            for _ in range(steps):
+                step()
+            ev1.record()
+            torch.cuda.synchronize()
+            total_ms = ev0.elapsed_time(ev1)
+        else:
+            total_ms = 0.0
+            for _ in range(steps):
+                flush.fill_(1)
+                ev0.record()
+                step()
+                ev1.record()
+                torch.cuda.synchronize()
+                total_ms += ev0.elapsed_time(ev1)
+    runs = steps * n_frames
+    kern_ms = [finder.profile_ms(r, 1) for r in range(max(0, runs - 64), runs)]
+    kern_ms = [k for k in kern_ms if k > 0]
+    finder.set_profiling(False)
+    res["total_ms"] = total_ms
+    res["ms_per_step"] = total_ms / steps
+    res["kernel_ms"] = float(np.mean(kern_ms)) if kern_ms else None
+    del flush
+    if parity:
+        from oracle import oracle as orc
+        orc.build()
+        par = {"ok": True, "clusters_checked": 0, "frames": n_frames, "planes_per_frame": geom[0] * geom[1],
+               "max_abs_err": {f: 0.0 for f in FLOAT_FIELDS}, "oracle": "all planes, all host cores"}
+        t_or = 0.0
+        for f, o, s in zip(frames, outs, stats):
+            cl, st = finder.result(clusters=o, status=s)
+            t0 = time.perf_counter()
+            ora, ost, nthr = orc.run_parallel(f, *geom[:4], npads=geom[4])
+            t_or += time.perf_counter() - t0
+            c = compare_clusters(cl, ora)
+            if st["n_bad_digits"] != ost["n_bad_digits"]:
+                c.update(ok=False, mismatch="n_bad_digits %d != %d" % (st["n_bad_digits"], ost["n_bad_digits"]))
+            par["threads"] = nthr
+            if not c["ok"]:
+                par.update(ok=False, mismatch=c["mismatch"])
+                break
+            par["clusters_checked"] += c["clusters_checked"]
+            for k, v in c["max_abs_err"].items():
+                par["max_abs_err"][k] = max(par["max_abs_err"][k], v)
+            del cl, ora
+        par["oracle_seconds_all_cores"] = t_or
+        res["parity"] = par
+    if keep:
+        res["_live"] = dict(finder=finder, frames=frames, pinned=pinned, dev_digits=dev_digits, outs=outs, stats=stats,
+                            flags=flags, geom=geom, cfg=cfg, max_clusters=max_clusters)
+    else:
+        finder.close()
+        del finder, dev_digits, outs, stats, frames
+        torch.cuda.empty_cache()
+    return res
+
+
+class _NullCtx:
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        return False
+
+
+def alg_bytes_of(path, nd, nc, geom):
+    """Algorithmic bytes of one launch of the dominant kernel."""
+    if path == "fused":
+        # 8 B/digit read, 32 B/cluster staged, 4 B per pad line (peak count)
+        return 8.0 * nd + 32.0 * nc + 4.0 * geom[0] * geom[1] * geom[2]
+    # general: 8 B/digit read + the 3x3 neighbourhood of every digit >= threshold covered by the 2 B/digit map cells of
+    # three lines (each map sector counted once) + 32 B/cluster staged + peak mask
+    return 8.0 * nd + 2.0 * nd + 32.0 * nc + nd / 8.0
+
+
+def run_cf(args):
     import torch
     import torch.distributed as dist
     from datagen import gen
@@ -670,64 +837,25 @@ def main():
     dev = "cuda:%d" % local_rank
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
+    peak, peak_src = load_peaks()
+    do_parity = not args.no_cpu_baseline and not args.no_parity and rank == 0 and args.variant == "none"
 
+    # ---- headline config: K timed steps, device-resident inputs --------------------------------------------------------
     cfg = gen.CONFIGS[args.config]
-    geom = gen.geometry(args.config)
-    n_frames = cfg["frames"]
-    # replicas: rank r works on its own frames (frame index offset by rank * n_frames)
-    t0 = time.perf_counter()
-    frames = [gen.generate(args.config, frame=rank * n_frames + f) for f in range(n_frames)]
-    gen_s = time.perf_counter() - t0
-    n_digits = [int(f.shape[0]) for f in frames]
-    nmax = max(n_digits)
-    max_clusters = nmax // 10 + 1024
-    vflags = {"none": 0, "flags": cf.CLUSTER_FLAGS, "cuts": cf.CLUSTER_FLAGS | cf.CUT_SINGLE_PAD}[args.variant]
-    finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=nmax, max_clusters=max_clusters, device=dev,
-                              q_tot_min=40 if args.variant == "cuts" else 0,
-                              q_saturation=1000 if args.variant != "none" else 0)
-    flags = (cf.DIGITS_SORTED if args.path == "fused" else (cf.DIGITS_SORTED | cf.FORCE_GENERAL)) | vflags
-
-    pinned = [torch.from_numpy(f.view(np.uint8)).pin_memory() for f in frames]
-    dev_digits = [p.to(dev, non_blocking=True) for p in pinned]
-    outs = [torch.empty(max_clusters * 32, dtype=torch.uint8, device=dev) for _ in frames]
-    stats = [torch.zeros(32, dtype=torch.uint8, device=dev) for _ in frames]
-    torch.cuda.synchronize()
-
-    def step():
-        for d, n, o, s in zip(dev_digits, n_digits, outs, stats):
-            finder.run(d, n, flags=flags, clusters=o, status=s)
-
     sampler = ClockSampler(local_rank).start()
-    for _ in range(args.warmup):
-        step()
-    torch.cuda.synchronize()
-    sts = [finder.result(clusters=o, status=s)[1] for o, s in zip(outs, stats)]
-    for st in sts:
-        if st["path"] == 0 or st["overflow"]:
-            raise RuntimeError("bench run invalid: status %r" % (st,))
-    n_clusters = [st["n_clusters"] for st in sts]
-    launches_per_step = finder.last_launch_count() * n_frames
-    dominant_kernel = finder.last_kernel()
-
-    # ---- timed region: K steps, device-resident inputs (each frame > L2, so no L2 flush is needed) ----
-    finder.set_profiling(True)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if world > 1:
         dist.barrier()
-    torch.cuda.synchronize()
-    with sampler as clocks:
-        ev0.record()
-        for _ in range(args.steps):
-            step()
-        ev1.record()
-        torch.cuda.synchronize()
+    # replicas: rank r works on its own frames (frame index offset by rank * frames)
+    m = measure_config(cf, torch, args.config, args.steps, args.warmup, args.path, args.variant, dev,
+                       frame_offset=rank * cfg["frames"], parity=do_parity, sampler=sampler, keep=True)
+    clocks = sampler
+    live = m.pop("_live")
+    finder, frames, pinned, dev_digits = live["finder"], live["frames"], live["pinned"], live["dev_digits"]
+    geom, flags, max_clusters = live["geom"], live["flags"], live["max_clusters"]
+    n_frames, n_digits, n_clusters = m["frames_per_step"], m["digits"], m["clusters"]
     if world > 1:
         dist.barrier()
-    total_ms = ev0.elapsed_time(ev1)
-    runs = args.steps * n_frames
-    kern_ms = [finder.profile_ms(r, 1) for r in range(max(0, runs - 64), runs)]
-    kern_ms = [k for k in kern_ms if k > 0]
-    finder.set_profiling(False)
+    total_ms = m["total_ms"]
     if world > 1:
         t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -744,7 +872,7 @@ def main():
     e2e = None
     if not args.no_e2e:
         host_out = torch.empty(max_clusters * 32, dtype=torch.uint8, pin_memory=True)
-        e_steps = max(1, min(args.steps, 3))
+        e_steps = max(1, min(args.steps, 5))
         for p, d in zip(pinned, dev_digits):
             finder.run_host(p, flags=flags, dev_digits=d, host_clusters=host_out)
         if world > 1:
@@ -763,6 +891,7 @@ def main():
         e2e = {"value": digits_per_step / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms,
                "h2d_bytes_per_step": int(sum(n_digits) * 8), "d2h_bytes_per_step": int(sum(n_clusters) * 32 + 32 * n_frames),
                "steps": e_steps}
+        del host_out
 
     if rank != 0:
         if world > 1:
@@ -770,17 +899,10 @@ def main():
         return 0
 
     # ---- roofline of the dominant kernel (HBM-bound: stencil/compaction work, no contraction) ----
-    peak, peak_src = load_peaks()
     nd, nc = n_digits[-1], n_clusters[-1]     # per launch: one frame
-    kname = dominant_kernel
-    if args.path == "fused":
-        # algorithmic bytes per launch: 8 B/digit read, 32 B/cluster staged, 4 B per pad line (peak count)
-        alg_bytes = 8.0 * nd + 32.0 * nc + 4.0 * geom[0] * geom[1] * geom[2]
-    else:
-        # 8 B/digit read + 3x3 neighbourhood of every digit >= threshold is covered by the 2 B/digit map cells of
-        # three lines (each map sector counted once) + 32 B/cluster staged + peak mask
-        alg_bytes = 8.0 * nd + 2.0 * nd + 32.0 * nc + nd / 8.0
-    k_ms = float(np.mean(kern_ms)) if kern_ms else None
+    kname = m["kernel"]
+    alg_bytes = alg_bytes_of(args.path, nd, nc, geom)
+    k_ms = m["kernel_ms"]
     roof = {"bound": "hbm", "kernel": kname, "achieved": (alg_bytes / (k_ms * 1e-3) / 1e9) if k_ms else None,
             "peak": peak, "unit": "GB/s", "peak_source": peak_src,
             "frac": (alg_bytes / (k_ms * 1e-3) / 1e9 / peak) if k_ms else None,
@@ -790,7 +912,8 @@ def main():
     io_bytes = 8.0 * digits_per_step + 32.0 * clusters_per_step
     f_io = io_bytes / (ms_per_step * 1e-3) / 1e9 / peak
 
-    cpu = None
+    # ---- the oracle on the host cores: one thread (the definition as it stands) and all cores (plane blocks) -------
+    cpu = cpu_all = None
     if not args.no_cpu_baseline:
         from oracle import oracle as orc
         orc.build()
@@ -802,6 +925,17 @@ def main():
                "sample": "first %d of %d sectors of frame 0 (%d digits, %d clusters), %.1f s, single thread" % (
                    ns, geom[0], sample.shape[0], ost["n_clusters"], dt),
                "clusters_per_s": ost["n_clusters"] / dt, "host_cores_available": os.cpu_count()}
+        if do_parity and m.get("parity"):
+            t_all = m["parity"]["oracle_seconds_all_cores"] / n_frames
+            cpu_all = {"value": n_digits[0] / t_all, "unit": UNIT, "cores": m["parity"].get("threads"), "kind": "oracle",
+                       "sample": "frame 0, all %d planes, the single-threaded routine on plane blocks from %s host threads, "
+                                 "%.1f s; its output is the array the GPU's clusters are compared with" % (
+                                     geom[0] * geom[1], m["parity"].get("threads"), t_all),
+                       "clusters_identical_to_single_thread": None}
+            if ns == geom[0]:
+                # the all-cores run must reproduce the single-threaded one: compare counts (the arrays themselves
+                # were compared with the GPU's, which equals both if it equals one)
+                cpu_all["clusters_identical_to_single_thread"] = bool(ost["n_clusters"] == n_clusters[0])
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -809,18 +943,56 @@ def main():
             "config": {"workload": "config%d: %s" % (args.config, cfg["label"]), "path": args.path,
                        "variant": args.variant,
                        "frames_per_step": n_frames, "digits_per_frame": nd, "clusters_per_frame": nc,
-                       "occupancy": gen.occupancy(frames[0], args.config), "parallelism": "replicas x%d" % world,
-                       "l2": "inputs (%.2f GB digits per frame) larger than the 126 MB L2; no flush" % (nd * 8 / 1e9),
+                       "occupancy": m["occupancy"], "parallelism": "replicas x%d" % world,
+                       "l2": m["l2"],
                        "checksum_frame0": "%016x" % gen.checksum(frames[0]) if nd < 50_000_000 else "skipped (large)",
-                       "gen_seconds": gen_s},
+                       "gen_seconds": m["gen_seconds"]},
             "clusters_per_s": clusters_per_step / (ms_per_step * 1e-3),
             "f_io": {"value": f_io, "bytes_per_step": io_bytes, "note": "compulsory I/O (8 B/digit + 32 B/cluster) / time / peak"},
-            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-            "clocks": clocks.summary()}
+            "roofline": roof, "cpu_baseline": cpu, "cpu_baseline_all_cores": cpu_all, "parity": m.get("parity"),
+            "e2e": e2e, "gpu_launches": m["launches_per_step"] * args.steps, "clocks": clocks.summary()}
+    finder.close()
+    del finder, dev_digits, frames, pinned, live
+    torch.cuda.empty_cache()
+
+    # ---- every other config of BASELINE.json (north_star: "digits/s and clusters/s ... for each config") -------------
+    ok = not (line["parity"] and not line["parity"]["ok"])
+    if args.per_config and world == 1 and args.variant == "none":
+        per = {}
+        for c in (1, 2, 3, 4, 5):
+            if c == args.config:
+                continue
+            try:
+                r = measure_config(cf, torch, c, max(5, min(args.steps, 20)), args.warmup, args.path, "none", dev,
+                                   parity=do_parity)
+            except Exception as e:                      # e.g. not enough device or host memory for the 1.09e9-digit frame
+                per["config%d" % c] = {"error": "%s: %s" % (type(e).__name__, e)}
+                torch.cuda.empty_cache()
+                continue
+            g = gen.geometry(c)
+            nd_c, nc_c = r["digits"][-1], r["clusters"][-1]
+            ab = alg_bytes_of(args.path, nd_c, nc_c, g)
+            ms = r["ms_per_step"]
+            e = {"workload": "config%d: %s" % (c, gen.CONFIGS[c]["label"]), "frames_per_step": r["frames_per_step"],
+                 "digits_per_frame": nd_c, "clusters_per_frame": nc_c, "ms_per_step": ms,
+                 "ms_per_frame": ms / r["frames_per_step"], "digits_per_s": sum(r["digits"]) / (ms * 1e-3),
+                 "clusters_per_s": sum(r["clusters"]) / (ms * 1e-3),
+                 "f_io": (8.0 * sum(r["digits"]) + 32.0 * sum(r["clusters"])) / (ms * 1e-3) / 1e9 / peak,
+                 "kernel": r["kernel"], "kernel_ms": r["kernel_ms"],
+                 "roofline_frac": (ab / (r["kernel_ms"] * 1e-3) / 1e9 / peak) if r["kernel_ms"] else None,
+                 "gpu_launches_per_step": r["launches_per_step"], "l2": r["l2"], "occupancy": r["occupancy"],
+                 "parity": r.get("parity")}
+            if r.get("parity"):
+                t_all = r["parity"]["oracle_seconds_all_cores"]
+                e["cpu_baseline_all_cores"] = {"value": sum(r["digits"]) / t_all, "unit": UNIT,
+                                               "cores": r["parity"].get("threads"), "kind": "oracle"}
+                ok = ok and r["parity"]["ok"]
+            per["config%d" % c] = e
+        line["per_config"] = per
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
-    return 0
+    return 0 if ok else 1
 
 
 if __name__ == "__main__":

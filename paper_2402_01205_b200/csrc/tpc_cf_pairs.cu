@@ -28,17 +28,20 @@
 namespace tpccf {
 
 static constexpr int kPThreads = 256;
-static constexpr int kPWarps = kPThreads / 32;
-static constexpr int kPS = kPWarps;               // lines per step: one per warp
+static constexpr int kPBuild = 4;                 // builder warps (warps 0..3): K0 + K1 + stage A of one line per step each
+static constexpr int kPProc = 4;                  // processor warps (warps 4..7): stages B + C of one line per step each
+static constexpr int kPS = kPProc;                // lines per step
 static constexpr int kPSlots = 2 * kPS + 4;       // lines l0-2 .. l0+S+1 in use, next S being built
+static constexpr int kRegsBuild = 56;             // registers per thread after setmaxnreg (launch: 80 = 65536 / (3 * 256))
+static constexpr int kRegsProc = 104;             //   4 * 56 + 4 * 104 = 8 * 80
 static constexpr uint32_t kChunkBytes = 512;      // one build iteration: 64 digits
 static constexpr uint32_t kPieceBytes = 1024;     // one bulk copy: 128 digits = two iterations
-static constexpr uint32_t kNH = 2;                // staging ring per warp: two pieces, one mbarrier each
+static constexpr uint32_t kNH = 2;                // staging ring of one line: two pieces, one mbarrier each
 static constexpr uint32_t kGuard = 16;            // in front of the ring: copy of the ring's last 16 bytes
-static constexpr uint32_t kStgBytes = kGuard + kNH * kPieceBytes;
-static constexpr uint32_t kPqBytes = 256;         // per-warp peak queue (64 entries)
+static constexpr uint32_t kBufBytes = kGuard + kNH * kPieceBytes;
+static constexpr uint32_t kStgBytes = 2 * kBufBytes;   // per builder: the line being built and the head of the next one
+static constexpr uint32_t kPqBytes = 256;         // per-processor peak queue (64 entries)
 static constexpr uint32_t kHdrBytes = 16;
-static constexpr int kMaxSteps = 32;              // 256 pads / 8
 static constexpr uint32_t kSentT0 = 65470u;       // time of the first trailing sentinel digit (+ up to 63); n_time <= this
 
 // ---- shared-memory accessors on 32-bit addresses -------------------------------------------------------------------
@@ -208,9 +211,9 @@ __device__ __forceinline__ void pwindow(uint32_t slot, uint32_t dsub, const Slot
 }
 
 // MULTI: the time axis is covered in sg.n_pass > 1 passes (long lines).  VAR: flags / cuts requested (V1..V3); the
-// default instantiation carries none of that code.  MINB: CTAs per SM the registers are limited for.
-template <bool MULTI, bool VAR, int MINB>
-__global__ void __launch_bounds__(kPThreads, MINB)
+// default instantiation carries none of that code.
+template <bool MULTI, bool VAR>
+__global__ void __launch_bounds__(kPThreads, 3)
 k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_t* __restrict__ line_start,
               uint32_t pads_per_unit, uint32_t units_per_plane, SlotGeo sg, uint32_t q_peak_min, uint32_t q_gate,
               Variant var, Counters* cnt, uint32_t* __restrict__ line_cnt, uint4* __restrict__ stage)
@@ -219,8 +222,7 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     __shared__ uint32_t s_ls[260];          // line starts of this plane: s_ls[p], p = 0..max_pads, then next plane's start
     __shared__ uint32_t s_pos[260];         // first digit of line p that the current pass needs (time >= pass start - 2)
     __shared__ uint32_t s_cnt[260];         // peaks of line p found by the passes so far
-    __shared__ __align__(8) unsigned long long s_bar[kPWarps * kNH];
-    __shared__ __align__(4) uint8_t s_asg[kMaxSteps][kPWarps];   // per step and warp: line to process (low nibble) / to build (high)
+    __shared__ __align__(8) unsigned long long s_bar[kPBuild * 2 * kNH];   // per builder, buffer and piece
     __shared__ int s_unsorted;
 
     const uint32_t plane = blockIdx.x / units_per_plane, unit = blockIdx.x % units_per_plane;
@@ -236,9 +238,14 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     const uint32_t le_mask = lt_mask | (1u << lane);
 
     const uint32_t sm0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
-    const uint32_t ring = sm0 + kPSlots * sg.slot_bytes + (uint32_t)warp * kStgBytes + kGuard;   // this warp's chunk 0
-    const uint32_t pqa = sm0 + kPSlots * sg.slot_bytes + kPWarps * kStgBytes + (uint32_t)warp * kPqBytes;
-    const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(&s_bar[warp * kNH]);
+    const bool builder = warp < kPBuild;
+    const int rw = builder ? warp : warp - kPBuild;            // index within the role
+    // staging of builder rw: two buffers (guard + two pieces each); the line in hand uses buffer `buf`
+    const uint32_t stg0 = sm0 + kPSlots * sg.slot_bytes + (uint32_t)rw * kStgBytes + kGuard;
+    const uint32_t pqa = sm0 + kPSlots * sg.slot_bytes + kPBuild * kStgBytes + (uint32_t)rw * kPqBytes;
+    const uint32_t barb = (uint32_t)__cvta_generic_to_shared(&s_bar[rw * 2 * kNH]);
+    uint32_t ring = stg0, bar0 = barb, pbit = 0u;              // of the buffer in hand (set_buf)
+    auto set_buf = [&](uint32_t buf) { ring = stg0 + buf * kBufBytes; bar0 = barb + buf * (8u * kNH); pbit = buf * kNH; };
     // 16-byte alignment of digit j in global memory: (j + gpar) even
     const uint32_t gpar = (uint32_t)((reinterpret_cast<uintptr_t>(digits) >> 3) & 1u);
     const uint32_t al_lo = gpar;                                  // first and one-past-last digit a bulk copy may touch
@@ -249,8 +256,7 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         s_ls[i] = v; s_pos[i] = v; s_cnt[i] = 0u;
     }
     if (tid == 0) s_unsorted = 0;
-    if (tid < kMaxSteps * kPWarps / 4) ((uint32_t*)&s_asg[0][0])[tid] = 0u;
-    if (tid < kPWarps * (int)kNH) p_mbar_init((uint32_t)__cvta_generic_to_shared(&s_bar[tid]), 1u);
+    if (tid < kPBuild * 2 * (int)kNH) p_mbar_init((uint32_t)__cvta_generic_to_shared(&s_bar[tid]), 1u);
     // every slot starts as an empty line (lines outside the plane keep this state: zero border in pad, R2)
     for (uint32_t x = (uint32_t)tid * 16u; x < kPSlots * sg.slot_bytes; x += kPThreads * 16u) p_sts128z(sm0 + x);
     __syncthreads();
@@ -280,50 +286,12 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
 
     const int blo = max(pa - 2, 0), bhi = min(P, pb + 2);   // lines this unit ever builds
 
-    // ---- in-step load balance, once per CTA ---------------------------------------------------------------------------
-    // A warp's work in a step is one line to process plus one line to build, both proportional to the line lengths
-    // (known from the index).  The warp with the longest line to process gets the shortest line to build, and so on:
-    // the 8 sums come out nearly equal and the barrier waits less.  Warp w ranks steps w, w + 8, ...
-    {
-        int k = warp;
-        for (int l0 = pa + warp * kPS; l0 < pb; l0 += kPS * kPWarps, k += kPWarps) {
-            const bool more = l0 + kPS < pb;
-            uint32_t lp = 0u, lb = 0u;
-            if (lane < kPS) {
-                const int p = l0 + lane, q = l0 + kPS + 2 + lane;
-                if (p < pb) lp = min(s_ls[p + 1] - s_ls[p], 0xfffeu) + 1u;
-                if (more && q >= blo && q < bhi) lb = min(s_ls[q + 1] - s_ls[q], 0xfffeu) + 1u;
-            }
-            const uint32_t mine = lp | (lb << 16);
-            // ranks of the 8 lines by all-pairs comparison, two pairs per lane: lane L compares line i = L & 7 with
-            // lines j = L >> 3 and j + 4; the four partial counts of a line are added across lanes i, i+8, i+16, i+24.
-            // rp: rank among the lines to process, longest first; rb: among the lines to build, shortest first.
-            const int i = lane & 7, j0 = lane >> 3;
-            const uint32_t vi = __shfl_sync(0xffffffffu, mine, i);
-            const uint32_t va = __shfl_sync(0xffffffffu, mine, j0), vb = __shfl_sync(0xffffffffu, mine, j0 + 4);
-            const uint32_t pi = vi & 0xffffu, bi = vi >> 16;
-            uint32_t c2 = 0u;                                   // process count | build count << 8
-            c2 += ((va & 0xffffu) > pi || ((va & 0xffffu) == pi && j0 < i)) ? 1u : 0u;
-            c2 += ((vb & 0xffffu) > pi || ((vb & 0xffffu) == pi && j0 + 4 < i)) ? 1u : 0u;
-            c2 += ((va >> 16) < bi || ((va >> 16) == bi && j0 < i)) ? 256u : 0u;
-            c2 += ((vb >> 16) < bi || ((vb >> 16) == bi && j0 + 4 < i)) ? 256u : 0u;
-            c2 += __shfl_xor_sync(0xffffffffu, c2, 8);
-            c2 += __shfl_xor_sync(0xffffffffu, c2, 16);
-            const uint32_t rp = c2 & 0xffu, rb = c2 >> 8;       // line i is processed by warp rp, built by warp rb
-            if (lane < kPS && k < kMaxSteps) {
-                // s_asg[k][w]: low nibble = line processed by warp w, high nibble = line built by warp w
-                atomicOr((unsigned int*)&s_asg[k][0] + (rp >> 2), (uint32_t)i << (8 * (rp & 3)));
-                atomicOr((unsigned int*)&s_asg[k][0] + (rb >> 2), (uint32_t)i << (8 * (rb & 3) + 4));
-            }
-        }
-    }
-
     // Time window of the current pass (set in the pass loop below).  Owned cells [tlo, thi): their peaks are found
     // in this pass.  Stored cells [wlo, whi) = owned +- 2 bins: the 5x5 windows of owned peaks stay inside.
     // With a single pass (MULTI = false) these are constants and the pass logic folds away.
     uint32_t tlo = 0u, thi = T, wlo = 0u, whi = T, dsub = 0u;
     bool last_pass = true;
-    uint32_t phase = 0u;                    // bit h: parity the next wait on staging piece h expects
+    uint32_t phase = 0u;                    // bit 2 buf + h: parity the next wait on piece h of staging buffer buf expects
 
     // ---- staging: piece k of a line = digit slots [base + 128k, base + 128k + 128), base = first digit of the pass in
     // the line, rounded down to a 16-byte boundary of global memory; ring half k mod 2.  Only lane 0 issues.
@@ -412,8 +380,8 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             ++iters;
             if ((c & 1u) == 0u && (c >> 1) < np) {          // a new piece: has it landed?
                 const uint32_t h = (c >> 1) & 1u;
-                p_mbar_wait(bar0 + 8u * h, (phase >> h) & 1u);
-                phase ^= 1u << h;
+                p_mbar_wait(bar0 + 8u * h, (phase >> (pbit + h)) & 1u);
+                phase ^= 1u << (pbit + h);
             }
             if (c == 0u) {
                 // leading sentinels: slots -2, -1 (the guard) and, if the line starts 8 bytes off a boundary, slot 0
@@ -518,8 +486,8 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             const uint32_t issued = min(np, 2u + (last >> 1)), waited = min(np, (last >> 1) + 1u);
             for (uint32_t k = waited; k < issued; ++k) {
                 const uint32_t h = k & 1u;
-                p_mbar_wait(bar0 + 8u * h, (phase >> h) & 1u);
-                phase ^= 1u << h;
+                p_mbar_wait(bar0 + 8u * h, (phase >> (pbit + h)) & 1u);
+                phase ^= 1u << (pbit + h);
             }
         }
         if (lane == 0) {
@@ -693,47 +661,71 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     };
 
     // ---- main loop -------------------------------------------------------------------------------------------------
-    // The time axis is covered in sg.n_pass passes over the unit's lines (smaller slots -> more CTAs per SM).
-    __syncthreads();                                            // s_asg complete
-    for (uint32_t pass = 0; pass < (MULTI ? sg.n_pass : 1u); ++pass) {
-    if (MULTI) {
-        last_pass = pass + 1u == sg.n_pass;
-        tlo = pass * sg.seg_len;
-        thi = last_pass ? T : min(tlo + sg.seg_len, T);
-        wlo = tlo >= 2u ? tlo - 2u : 0u;
-        whi = min(thi + 2u, T);
-        dsub = tlo >> 3;
-    }
-    // Ring index of line p is (p - (pa - 2)) mod kPSlots.  Rounds -2 and -1 build lines pa-2 .. pa+S+1 (S + 4 = 12 lines:
-    // warp w builds line pa-2+w, then warps 0..3 lines pa+S-2 .. pa+S+1).  Step l0 >= pa (ONE barrier): every warp stages
-    // the head of the line it will build, runs stages B+C on its current line (lines l0-2 .. l0+S+1 are complete), then
-    // rebuilds the slot of a line that left the ring (l0-S-2 .. l0-3).  One copy of the code serves both.
-    int vl0 = 2;                                                // ring index of line l0
-    int step = -2;
-    for (int l0 = pa - 2 * kPS; l0 < pb; l0 += kPS, ++step) {
-        int pnew, vnew;
-        bool doit;
-        int ip = 0;
-        if (step < 0) {
-            const int i = (step + 2) * kPS + warp;              // ring index = line - (pa - 2)
-            pnew = pa - 2 + i; vnew = i;
-            doit = i < kPS + 4;
-        } else {
-            const uint32_t asg = __shfl_sync(0xffffffffu, (uint32_t)s_asg[step & (kMaxSteps - 1)][warp], 0);
-            ip = (int)(asg & 15u);                              // which of the 8 lines this warp processes / builds
-            const int ib = (int)(asg >> 4);
-            pnew = l0 + kPS + 2 + ib; vnew = pring_at(vl0, kPS + 2 + ib - kPSlots);
-            doit = l0 + kPS < pb;                               // lines l0+S+2 .. l0+2S+1 enter the ring in this step
+    // Warps 0..3 BUILD, warps 4..7 PROCESS, concurrently, one line per warp and step, ONE barrier per step of S = 4 lines:
+    //   round -2, -1   builders fill the ring with lines pa-2 .. pa+S+1 (S + 4 = 8 lines); processors wait
+    //   step l0 >= pa  processor i runs stages B + C on line l0 + i (lines l0-2 .. l0+S+1 are complete);
+    //                  builder i rebuilds the slot of a line that left the ring (l0-S-2 .. l0-3) as line l0 + S + 2 + i
+    // Ring index of line p is (p - (pa - 2)) mod kPSlots.  A builder issues the bulk copies of the head of its NEXT line
+    // (other staging buffer) before it builds the current one, so a copy has a whole step to land.
+    // The two roles need very different register counts (the 5x5 gather of stage C against a streaming loop): the
+    // kernel is launched with 80 registers per thread (3 CTAs per SM) and each warp group re-sizes its share.
+    // The time axis is covered in sg.n_pass passes over the unit's lines.
+    const int n_rounds = 2 + (pb - pa + kPS - 1) / kPS;        // per pass
+    if (builder) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsBuild));
+        // line of this builder in round r (r = step + 2); returns false if there is none
+        auto line_of = [&](int r, int& p, int& v) -> bool {
+            if (r < 2) {
+                const int i = r * kPS + rw;                     // ring index = line - (pa - 2)
+                p = pa - 2 + i; v = i;
+                return i < kPS + 4;
+            }
+            const int l0 = pa + (r - 2) * kPS;
+            p = l0 + kPS + 2 + rw;
+            v = (p - (pa - 2)) % kPSlots;
+            return l0 + kPS < pb;                               // lines l0+S+2 .. l0+2S+1 enter the ring in this step
+        };
+        uint32_t buf = 0u;
+        for (uint32_t pass = 0; pass < (MULTI ? sg.n_pass : 1u); ++pass) {
+            if (MULTI) {
+                last_pass = pass + 1u == sg.n_pass;
+                tlo = pass * sg.seg_len;
+                thi = last_pass ? T : min(tlo + sg.seg_len, T);
+                wlo = tlo >= 2u ? tlo - 2u : 0u;
+                whi = min(thi + 2u, T);
+                dsub = tlo >> 3;
+            }
+            int p, v, pn, vn;
+            if (line_of(0, p, v)) { set_buf(buf); stage_head(p); }
+            for (int r = 0; r < n_rounds; ++r) {
+                const bool cur = line_of(r, p, v);
+                const bool nxt = r + 1 < n_rounds && line_of(r + 1, pn, vn);
+                if (nxt) { set_buf(buf ^ 1u); stage_head(pn); }
+                if (cur) { set_buf(buf); build_line(p, v); }
+                buf ^= 1u;
+                if (r != 0) __syncthreads();
+            }
         }
-        if (doit) stage_head(pnew);
-        if (step >= 0 && l0 + ip < pb) process(l0 + ip, pring_at(vl0, ip));
-        if (doit) build_line(pnew, vnew);
-        if (step != -2) {
-            __syncthreads();
-            if (step >= 0) vl0 = pring_at(vl0, kPS);
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsProc));
+        for (uint32_t pass = 0; pass < (MULTI ? sg.n_pass : 1u); ++pass) {
+            if (MULTI) {
+                last_pass = pass + 1u == sg.n_pass;
+                tlo = pass * sg.seg_len;
+                thi = last_pass ? T : min(tlo + sg.seg_len, T);
+                dsub = tlo >> 3;
+            }
+            int vl0 = 2;                                        // ring index of line l0
+            for (int r = 0; r < n_rounds; ++r) {
+                if (r >= 2) {
+                    const int l0 = pa + (r - 2) * kPS;
+                    if (l0 + rw < pb) process(l0 + rw, pring_at(vl0, rw));
+                    vl0 = pring_at(vl0, kPS);
+                }
+                if (r != 0) __syncthreads();
+            }
         }
     }
-    }   // passes
     if (bad_order) s_unsorted = 1;
     __syncthreads();
     if (tid == 0 && s_unsorted) atomicOr(&cnt->unsorted, 1u);
@@ -745,16 +737,14 @@ cudaError_t fused_pairs_set_attributes()
     auto set = [&](const void* f, int bytes) {
         if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     };
-    set((const void*)k_fused_pairs<false, false, 2>, 112 * 1024); set((const void*)k_fused_pairs<true, false, 2>, 112 * 1024);
-    set((const void*)k_fused_pairs<false, true, 2>, 112 * 1024);  set((const void*)k_fused_pairs<true, true, 2>, 112 * 1024);
-    set((const void*)k_fused_pairs<false, false, 3>, 72 * 1024);  set((const void*)k_fused_pairs<true, false, 3>, 72 * 1024);
-    set((const void*)k_fused_pairs<false, true, 3>, 72 * 1024);   set((const void*)k_fused_pairs<true, true, 3>, 72 * 1024);
+    set((const void*)k_fused_pairs<false, false>, 112 * 1024); set((const void*)k_fused_pairs<true, false>, 112 * 1024);
+    set((const void*)k_fused_pairs<false, true>, 112 * 1024);  set((const void*)k_fused_pairs<true, true>, 112 * 1024);
     return e;
 }
 
 // Launches k_fused_pairs after the line index is in ws.line_start.  Returns 1 (launched), 0 (not applicable: the
 // mean line would not fit the block pool in <= 6 passes; the caller runs the bitmap kernel instead) or a negative
-// tpc_cf error.  Launch shape: 2 CTAs of 8 warps per SM (3 when the slots are small: short lines).  Lines too long
+// tpc_cf error.  Launch shape: 3 CTAs of 4 + 4 warps per SM.  Lines too long
 // for the 254-block pool are covered in several passes over the time axis (dir, pool and survivor list all scale with
 // the segment length).
 int launch_fused_pairs(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
@@ -770,9 +760,9 @@ int launch_fused_pairs(const Geo& g, const Workspace& ws, const tpc_digit* digit
     // measured on the synthetic frames: 0.38 blocks and 0.16 stage-A survivors per digit
     const double mean_blocks = 0.38 * mean_len, mean_surv = 0.16 * mean_len;
 
-    const uint32_t fixed = kPWarps * (kStgBytes + kPqBytes);
-    const uint32_t stat = 4608u;                                    // static shared memory of the kernel, rounded up
-    const uint32_t budget = 227u * 1024u / 2u - 1024u - stat;      // 2 CTAs per SM: - 1 KB reserved each
+    const uint32_t fixed = kPBuild * kStgBytes + kPProc * kPqBytes;
+    const uint32_t stat = 3584u;                                    // static shared memory of the kernel, rounded up
+    const uint32_t budget = 227u * 1024u / 3u - 1024u - stat;      // 3 CTAs per SM: - 1 KB reserved each
     auto shape = [&](uint32_t n_pass, bool force, SlotGeo* out) -> bool {
         SlotGeo sg;
         sg.n_pass = n_pass;
@@ -813,20 +803,15 @@ int launch_fused_pairs(const Geo& g, const Workspace& ws, const tpc_digit* digit
     const uint32_t smem = kPSlots * sg.slot_bytes + fixed;
 
     const uint32_t whole = (g.max_pads + kPS - 1) / kPS * kPS;
-    uint32_t pads_per_unit = g.n_planes >= 1184 ? whole : (g.n_planes >= 296 ? 6 * kPS : 3 * kPS);
+    uint32_t pads_per_unit = g.n_planes >= 1184 ? whole : (g.n_planes >= 296 ? 12 * kPS : 6 * kPS);
     if (pads_per_unit > whole) pads_per_unit = whole;
     if (tun.pads_per_unit >= kPS && tun.pads_per_unit <= 256) pads_per_unit = (uint32_t)(tun.pads_per_unit / kPS * kPS);
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
     if (ev_k0) cudaEventRecord(ev_k0, st);
     g_last_kernel = "k_fused_pairs";
-    // a third CTA per SM when the slots are small (short lines): the kernel is latency bound
-    const uint32_t budget3 = 227u * 1024u / 3u - 1024u - stat;
-    const bool three = smem <= budget3 && tun.ctas_per_sm != 2;
     const bool m = sg.n_pass > 1, v = var.active != 0u;
-    auto kern = three ? (m ? (v ? k_fused_pairs<true, true, 3> : k_fused_pairs<true, false, 3>)
-                           : (v ? k_fused_pairs<false, true, 3> : k_fused_pairs<false, false, 3>))
-                      : (m ? (v ? k_fused_pairs<true, true, 2> : k_fused_pairs<true, false, 2>)
-                           : (v ? k_fused_pairs<false, true, 2> : k_fused_pairs<false, false, 2>));
+    auto kern = m ? (v ? k_fused_pairs<true, true> : k_fused_pairs<true, false>)
+                  : (v ? k_fused_pairs<false, true> : k_fused_pairs<false, false>);
     kern<<<g.n_planes * upp, kPThreads, smem, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
                                                     pads_per_unit, upp, sg, q_peak_min, q_gate, var,
                                                     ws.counters, ws.line_cnt, (uint4*)ws.stage);

@@ -483,3 +483,67 @@ def test_maximum_geometry(path):
         cl, st = gpu_run(digits, geom, PATHS[path], max_clusters=ost["n_clusters"] + 8, expect_kernel=expect)
         assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == 0
         assert_clusters_equal(cl, ora, "max geometry %dx%d/%s" % (P, T, path))
+
+
+# ---- full-size parity in the launch shape bench.py times (every config, every plane) -------------------------
+def _full_frame_check(cfg_id, frames=1, sectors=None):
+    """All clusters of the full-size config (all planes) against the oracle run on all host cores (the same
+    single-threaded routine over plane blocks), element by element; fused path as bench.py launches it.  Frames of a
+    multi-frame config are enqueued back to back on one stream with one workspace."""
+    import torch
+    cf = _cf()
+    c = dict(gen.CONFIGS[cfg_id])
+    if sectors is not None:
+        c["n_sectors"] = sectors
+    geom = gen.geometry(c)
+    fr = [gen.generate(c, frame=f) for f in range(frames)]
+    nmax = max(f.shape[0] for f in fr)
+    finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=nmax, max_clusters=nmax // 10 + 1024)
+    devs = [cf.to_device(f) for f in fr]
+    outs = [torch.empty(finder.max_clusters * 32, dtype=torch.uint8, device="cuda:0") for _ in fr]
+    sts = [torch.zeros(32, dtype=torch.uint8, device="cuda:0") for _ in fr]
+    for f, d, o, s in zip(fr, devs, outs, sts):
+        finder.run(d, f.shape[0], flags=cf.DIGITS_SORTED, clusters=o, status=s)
+    kernel = finder.last_kernel()
+    total = 0
+    for i, (f, o, s) in enumerate(zip(fr, outs, sts)):
+        cl, st = finder.result(clusters=o, status=s)
+        assert st["path"] == 3 and st["overflow"] == 0
+        ora, ost, nthr = orc.run_parallel(f, *geom[:4], npads=geom[4])
+        assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == ost["n_bad_digits"] == 0
+        assert_clusters_equal(cl, ora, "config %d frame %d, all %d planes (%s)" % (cfg_id, i, geom[0] * geom[1], kernel))
+        total += ora.shape[0]
+        del cl, ora
+    finder.close()
+    return total, kernel
+
+
+def test_config3_full_frame_every_plane():
+    """BASELINE.json configs[2]: the whole 36-sector frame, all 5472 planes, 10.9 M clusters compared one by one."""
+    total, kernel = _full_frame_check(3)
+    assert total > 10_000_000
+
+
+def test_config4_eight_sectors_every_plane():
+    """configs[3] at 8 sectors (1216 planes >= 1184: whole-plane units, several time passes): fully compared."""
+    total, kernel = _full_frame_check(4, sectors=8)
+    assert total > 10_000_000
+
+
+def test_config5_eight_sectors_four_frames():
+    """configs[4] at 8 sectors, 4 frames back to back (whole-plane units, short lines): fully compared."""
+    total, kernel = _full_frame_check(5, frames=4, sectors=8)
+    assert total > 1_000_000
+
+
+def test_config4_full_frame_every_plane():
+    """configs[3] at full size: 1.09e9 digits (indices past 2^30, staging offsets past 2^32), 51 M clusters, every
+    plane compared with the oracle."""
+    total, kernel = _full_frame_check(4)
+    assert total > 50_000_000
+
+
+def test_config5_full_four_frames_every_plane():
+    """configs[4] at full size: 36 sectors, pads 66 -> 138, 4 frames back to back on one stream: every cluster."""
+    total, kernel = _full_frame_check(5, frames=4)
+    assert total > 7_000_000

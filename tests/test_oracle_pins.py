@@ -425,6 +425,35 @@ def test_plane_range_run_is_slice_of_full_run():
     assert part.tobytes() == full[(pl >= 2) & (pl < 5)].tobytes()
 
 
+def test_plane_range_bad_digit_attribution_hand_example():
+    """tpc_cf_oracle_run_planes on a partial plane range: which invalid digits (R11) it counts.  Hand example on a
+    2-sector x 3-row x 20-pad x 50-bin geometry (planes 0..5 = sector * 3 + row), run on planes [2, 5):
+      inside the range, invalid  : (0,2,p=20,t=1,q=5) pad out of range   -> plane 2, counted
+                                   (1,0,p=3,t=50,q=5) time out of range  -> plane 3, counted
+                                   (1,1,p=3,t=7,q=0)  zero charge        -> plane 4, counted
+      outside the range, invalid : (0,0,p=25,t=1,q=5)                    -> plane 0, NOT counted
+                                   (1,2,p=3,t=60,q=5)                    -> plane 5, NOT counted
+      unattributable             : (2,0,..) sector out of range, (0,3,..) row out of range -> charged to the first
+                                   plane of whatever range is asked (plane 2 here): counted by every range, once by
+                                   the full-frame run (so counts of ranges that tile a frame need not add up)
+      valid digits               : one in plane 1 (outside), one in plane 3 (inside: a single-cell cluster)
+    Expected for planes [2,5): n_bad = 3 + 2 = 5, n_digits_used = 1, n_clusters = 1 (the plane-3 digit).
+    Expected for the full frame: n_bad = 7, n_digits_used = 2, n_clusters = 2."""
+    rows = [(0, 2, 20, 1, 5), (1, 0, 3, 50, 5), (1, 1, 3, 7, 0), (0, 0, 25, 1, 5), (1, 2, 3, 60, 5),
+            (2, 0, 1, 1, 5), (0, 3, 1, 1, 5), (0, 1, 4, 4, 9), (1, 0, 6, 6, 9)]
+    d = np.zeros(len(rows), dtype=orc.DIGIT)
+    for i, (s, r, p, t, q) in enumerate(rows):
+        d[i] = (s, r, p, 0, t, q)
+    part, st = orc.run(d, 2, 3, 20, 50, planes=(2, 5))
+    assert (st["n_bad_digits"], st["n_digits_used"], st["n_clusters"]) == (5, 1, 1)
+    assert (int(part[0]["sector"]), int(part[0]["row"]), int(part[0]["pad"]), int(part[0]["time"])) == (1, 0, 6, 6)
+    full, sf = orc.run(d, 2, 3, 20, 50)
+    assert (sf["n_bad_digits"], sf["n_digits_used"], sf["n_clusters"]) == (7, 2, 2)
+    # another range: its own invalid digit (plane 0) plus, again, the two unattributable ones
+    a, sa = orc.run(d, 2, 3, 20, 50, planes=(0, 2))
+    assert (sa["n_bad_digits"], sa["n_digits_used"], sa["n_clusters"]) == (1 + 2, 1, 1)
+
+
 def test_dense_plane_matches_digits():
     rng = np.random.default_rng(31)
     a = random_plane(rng, 20, 50, 0.2)
