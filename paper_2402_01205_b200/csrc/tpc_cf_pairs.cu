@@ -23,6 +23,8 @@
 //   K2 stage A at build time, stage B from the survivor list against lines p-1 / p+1
 //   K4 stage C: peaks queued per warp, 5x5 window from the five slots p-2..p+2 -> stage[line_start + k]
 // Definition: include/tpc_cf.h (BASELINE.json:north_star; step named in PAPER.md:57).  Readings R1..R19: DESIGN.md §3.
+#include <algorithm>
+
 #include "tpc_cf_internal.cuh"
 
 namespace tpccf {
@@ -32,8 +34,9 @@ static constexpr int kPBuild = 4;                 // builder warps (warps 0..3):
 static constexpr int kPProc = 4;                  // processor warps (warps 4..7): stages B + C of one line per step each
 static constexpr int kPS = kPProc;                // lines per step
 static constexpr int kPSlots = 2 * kPS + 4;       // lines l0-2 .. l0+S+1 in use, next S being built
-static constexpr int kRegsBuild = 56;             // registers per thread after setmaxnreg (launch: 80 = 65536 / (3 * 256))
-static constexpr int kRegsProc = 104;             //   4 * 56 + 4 * 104 = 8 * 80
+static constexpr int kRegsBuild = 72;             // registers per thread after setmaxnreg (launch: 80 = 65536 / (3 * 256));
+static constexpr int kRegsProc = 88;              //   4 * 72 + 4 * 88 = 8 * 80.  (ptxas allocates per region: without the
+                                                  //   split it spills at 80; at 56 the builder re-computes its lane masks)
 static constexpr uint32_t kChunkBytes = 512;      // one build iteration: 64 digits
 static constexpr uint32_t kPieceBytes = 1024;     // one bulk copy: 128 digits = two iterations
 static constexpr uint32_t kNH = 2;                // staging ring of one line: two pieces, one mbarrier each
@@ -210,6 +213,36 @@ __device__ __forceinline__ void pwindow(uint32_t slot, uint32_t dsub, const Slot
     }
 }
 
+// Piece k of a line that touches a ragged end of the digit array (called by one lane; rare: at most two lines of a
+// run).  Bulk copies move the 16-byte aligned part [bs, be) of the piece, cut at the line's end rounded out to 16 bytes;
+// the first / last digit of the whole array, where it is ragged, is copied by hand before the barrier is armed (the
+// arrive releases those stores to the lanes that wait on the barrier).
+__device__ __noinline__ void p_issue_piece_slow(const uint2* __restrict__ digits, uint32_t base, uint32_t lend, uint32_t k,
+                                            uint32_t ring, uint32_t bar0, uint32_t gpar, uint32_t al_lo, uint32_t al_hi)
+{
+    const int s = (int)base + 128 * (int)k;             // -1: the piece in front of digit 0 of a buffer 8 bytes off
+    const uint32_t e = min((uint32_t)(s + 128), lend);
+    const uint32_t dst = ring + (k & 1u) * kPieceBytes;
+    const uint32_t bar = bar0 + 8u * (k & 1u);
+    uint32_t bs = (uint32_t)s, be = e + ((e + gpar) & 1u);
+    if (s < (int)al_lo) {
+        bs = al_lo;
+        if (e > 0u && bs > 0u) {
+            const uint2 d = __ldg(digits);
+            asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dst + 8u), "r"(d.x), "r"(d.y) : "memory");
+        }
+    }
+    if (be > al_hi) {
+        be = al_hi;
+        if (e > be && (int)be >= s) {
+            const uint2 d = __ldg(digits + be);
+            asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dst + 8u * (uint32_t)((int)be - s)), "r"(d.x), "r"(d.y) : "memory");
+        }
+    }
+    if (be > bs) p_bulk_load(dst + 8u * (uint32_t)((int)bs - s), digits + bs, 8u * (be - bs), bar);
+    else p_mbar_arrive(bar);
+}
+
 // MULTI: the time axis is covered in sg.n_pass > 1 passes (long lines).  VAR: flags / cuts requested (V1..V3); the
 // default instantiation carries none of that code.
 template <bool MULTI, bool VAR>
@@ -298,40 +331,32 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     // Bulk copies move the 16-byte aligned part [bs, be) of the piece, cut at the line's end rounded out to 16 bytes; the
     // first / last digit of the whole array, where it is ragged (at most one each), is copied by hand before the barrier
     // is armed (the arrive releases those stores to the lanes that wait on the barrier).
+    // The usual case (warp-uniform test): the line touches neither ragged end of the array, so piece k is one copy of
+    // [base + 128k, min(base + 128k + 128, lend rounded out to 16 bytes)).  Called by all lanes; lane 0 issues.
     auto issue_piece = [&](uint32_t base, uint32_t lend, uint32_t k) {
-        const int s = (int)base + 128 * (int)k;             // -1: the piece in front of digit 0 of a buffer 8 bytes off
-        const uint32_t e = min((uint32_t)(s + 128), lend);
-        const uint32_t dst = ring + (k & 1u) * kPieceBytes;
-        const uint32_t bar = bar0 + 8u * (k & 1u);
-        uint32_t bs = (uint32_t)s, be = e + ((e + gpar) & 1u);
-        if (s < (int)al_lo) {
-            bs = al_lo;
-            if (e > 0u && bs > 0u) {
-                const uint2 d = __ldg(digits);
-                asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dst + 8u), "r"(d.x), "r"(d.y) : "memory");
-            }
+        const uint32_t lend_al = lend + ((lend + gpar) & 1u);
+        if ((int)base >= (int)al_lo && lend_al <= al_hi) {
+            const uint32_t s = base + 128u * k;
+            const uint32_t bytes = 8u * (min(s + 128u, lend_al) - s);
+            if (lane == 0) p_bulk_load(ring + (k & 1u) * kPieceBytes, digits + s, bytes, bar0 + 8u * (k & 1u));
+        } else if (lane == 0) {
+            p_issue_piece_slow(digits, base, lend, k, ring, bar0, gpar, al_lo, al_hi);
         }
-        if (be > al_hi) {
-            be = al_hi;
-            if (e > be && (int)be >= s) {
-                const uint2 d = __ldg(digits + be);
-                asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dst + 8u * (uint32_t)((int)be - s)), "r"(d.x), "r"(d.y) : "memory");
-            }
-        }
-        if (be > bs) p_bulk_load(dst + 8u * (uint32_t)((int)bs - s), digits + bs, 8u * (be - bs), bar);
-        else p_mbar_arrive(bar);
     };
-    // the first two pieces of the line this warp builds next (issued before the warp processes its current line, so the
-    // global latency is covered)
+    // The head of the line this warp builds next: its first two pieces, issued a step ahead (so the global latency is
+    // covered) as ONE copy of up to 256 digits that completes on the barrier of piece 0; a line at a ragged end of the
+    // array gets two separate pieces instead (head_split below).
     auto stage_head = [&](int p) {
         if (p < blo || p >= bhi) return;
         const uint32_t lbeg = s_pos[p], lend = s_ls[p + 1];
         if (lend == lbeg) return;
-        if (lane == 0) {
-            const uint32_t base = lbeg - ((lbeg + gpar) & 1u);
-            const uint32_t np = (lend - base + 127u) >> 7;
-            issue_piece(base, lend, 0u);
-            if (np > 1u) issue_piece(base, lend, 1u);
+        const uint32_t base = lbeg - ((lbeg + gpar) & 1u);
+        const uint32_t lend_al = lend + ((lend + gpar) & 1u);
+        if ((int)base >= (int)al_lo && lend_al <= al_hi) {
+            if (lane == 0) p_bulk_load(ring, digits + base, 8u * (min(base + 256u, lend_al) - base), bar0);
+        } else if (lane == 0) {
+            p_issue_piece_slow(digits, base, lend, 0u, ring, bar0, gpar, al_lo, al_hi);
+            if (lend - base > 128u) p_issue_piece_slow(digits, base, lend, 1u, ring, bar0, gpar, al_lo, al_hi);
         }
     };
 
@@ -362,7 +387,9 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         const uint32_t odd = (lbeg + gpar) & 1u;
         const uint32_t base = lbeg - odd;
         const uint32_t L = len + odd;                       // digit slots from base to the end of the line
-        const uint32_t np = (L + 127u) >> 7;                // pieces (bulk copies) of the line
+        const uint32_t np = (L + 127u) >> 7;                // pieces of the line
+        // was the head issued as two pieces (stage_head's rule)?  Else piece 1 came with piece 0: no wait of its own
+        const bool head_split = !((int)base >= (int)al_lo && lend + ((lend + gpar) & 1u) <= al_hi);
         const uint32_t c_last = L >> 6;                     // iteration c works on slots 64c-1 .. 64c+62
         const uint32_t pcap = sg.pcap, scap = sg.scap;
         uint32_t nblk = 0u, nsurv = 0u;                     // warp-uniform running counts
@@ -374,15 +401,20 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
         // order check of the pairs (prev, a) and (a, b): off in iteration 0 where the earlier one is a leading sentinel
         uint32_t m_pa = (lane == 0 || (lane == 1 && odd)) ? 0u : 0x80000000u, m_ab = lane == 0 ? 0u : 0x80000000u;
         uint32_t bad = 0u;
-        for (uint32_t c = 0; c <= c_last; ++c) {
-            const uint32_t e = c & 3u;                      // chunk of the ring this iteration reads
-            const uint32_t ent = ring + e * kChunkBytes;
-            ++iters;
-            if ((c & 1u) == 0u && (c >> 1) < np) {          // a new piece: has it landed?
-                const uint32_t h = (c >> 1) & 1u;
+        // piece k = chunks 2k, 2k+1 (ring half k & 1); iteration c reads chunk c and the tail of chunk c - 1
+        uint32_t c = 0u;
+        bool done = false;
+        for (uint32_t k = 0; !done; ++k) {
+            const uint32_t h = k & 1u;
+            if (k < np && (k != 1u || head_split)) {        // has the piece landed?
                 p_mbar_wait(bar0 + 8u * h, (phase >> (pbit + h)) & 1u);
                 phase ^= 1u << (pbit + h);
             }
+#pragma unroll
+            for (uint32_t j = 0; j < 2u; ++j) {
+            if (done) break;
+            const uint32_t ent = ring + h * kPieceBytes + j * kChunkBytes;
+            ++iters;
             if (c == 0u) {
                 // leading sentinels: slots -2, -1 (the guard) and, if the line starts 8 bytes off a boundary, slot 0
                 if (lane == 0) {
@@ -395,20 +427,20 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
                 const uint32_t k0 = L - 64u * c;            // first sentinel slot within the chunk (0 .. 63)
 #pragma unroll
                 for (uint32_t r = 0; r < 2u; ++r) {
-                    const uint32_t k = k0 + (uint32_t)lane + 32u * r;
-                    if (k < 64u)
-                        asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(ent + 8u * k), "r"(lk), "r"(0x10000u + kSentT0 + k - k0) : "memory");
+                    const uint32_t kk = k0 + (uint32_t)lane + 32u * r;
+                    if (kk < 64u)
+                        asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(ent + 8u * kk), "r"(lk), "r"(0x10000u + kSentT0 + kk - k0) : "memory");
                 }
             }
             if (c == 0u || c == c_last) __syncwarp();
-            const uint32_t addr = ent + 16u * (uint32_t)lane;      // digit b; a at -8; e = 0: lane 0 reads the guard
+            const uint32_t addr = ent + 16u * (uint32_t)lane;      // digit b; a at -8; chunk 0 of the ring: lane 0 reads the guard
             const uint2 A = p_lds64(addr - 8u), B = p_lds64(addr);
             const uint32_t prevy = p_lds32(addr - 12u), nexty = p_lds32(addr + 12u);
-            // the ring's last 16 bytes are kept in the guard for lane 0 of the next iteration (entry 0)
-            if (e == 3u && lane == 31) p_sts128(ring - kGuard, p_lds128(addr));
+            // the ring's last 16 bytes are kept in the guard for lane 0 of the next iteration (chunk 0 of the ring)
+            if (h == 1u && j == 1u && lane == 31) p_sts128(ring - kGuard, p_lds128(addr));
             __syncwarp();
-            // the piece in front of this iteration's is dead now: its half receives the piece after the next one
-            if (lane == 0 && (c & 1u) == 0u && c >= 2u && (c >> 1) + 1u < np) issue_piece(base, lend, (c >> 1) + 1u);
+            // the piece in front of this one is dead now: its half receives the piece after this one
+            if (j == 0u && k >= 1u && k + 1u < np) issue_piece(base, lend, k + 1u);
             const uint32_t ya = A.y, yb = B.y;
             const uint32_t ta = ya & 0xffffu, tb = yb & 0xffffu, tp = prevy & 0xffffu, tn = nexty & 0xffffu;
             const uint32_t qa = ya >> 16, qb = yb >> 16, qp = prevy >> 16, qn = nexty >> 16;
@@ -476,16 +508,21 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
                         found = true;
                     }
                 }
-                if (!tail && t31 >= whi) break;             // every later digit is beyond the window
+                if (!tail && t31 >= whi) done = true;       // every later digit is beyond the window
             }
+            if (c == c_last) done = true;
+            ++c;
+            }   // chunks of the piece
         }
         bad_order |= bad;
         // chunks that were issued for iterations this pass did not run (early exit): consume their barrier phases
         if (MULTI) {
-            const uint32_t last = iters - 1u;               // last iteration run
+            const uint32_t last = iters - 1u;               // last iteration run: chunk `last`, piece last >> 1
+            // issued: pieces 0, 1 ahead of the loop, piece k + 1 in the first chunk of every piece k >= 1
             const uint32_t issued = min(np, 2u + (last >> 1)), waited = min(np, (last >> 1) + 1u);
             for (uint32_t k = waited; k < issued; ++k) {
                 const uint32_t h = k & 1u;
+                if (k == 1u && !head_split) continue;
                 p_mbar_wait(bar0 + 8u * h, (phase >> (pbit + h)) & 1u);
                 phase ^= 1u << (pbit + h);
             }
@@ -667,8 +704,7 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
     //                  builder i rebuilds the slot of a line that left the ring (l0-S-2 .. l0-3) as line l0 + S + 2 + i
     // Ring index of line p is (p - (pa - 2)) mod kPSlots.  A builder issues the bulk copies of the head of its NEXT line
     // (other staging buffer) before it builds the current one, so a copy has a whole step to land.
-    // The two roles need very different register counts (the 5x5 gather of stage C against a streaming loop): the
-    // kernel is launched with 80 registers per thread (3 CTAs per SM) and each warp group re-sizes its share.
+    // The kernel is launched with 80 registers per thread (3 CTAs per SM) and each warp group re-sizes its share.
     // The time axis is covered in sg.n_pass passes over the unit's lines.
     const int n_rounds = 2 + (pb - pa + kPS - 1) / kPS;        // per pass
     if (builder) {
@@ -695,15 +731,17 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
                 whi = min(thi + 2u, T);
                 dsub = tlo >> 3;
             }
-            int p, v, pn, vn;
-            if (line_of(0, p, v)) { set_buf(buf); stage_head(p); }
-            for (int r = 0; r < n_rounds; ++r) {
-                const bool cur = line_of(r, p, v);
+            // round r builds the line whose head round r - 1 issued (one call site each: the code is large)
+            int p = 0, v = 0;
+            bool cur = false;
+            for (int r = -1; r < n_rounds; ++r) {
+                int pn = 0, vn = 0;
                 const bool nxt = r + 1 < n_rounds && line_of(r + 1, pn, vn);
                 if (nxt) { set_buf(buf ^ 1u); stage_head(pn); }
                 if (cur) { set_buf(buf); build_line(p, v); }
                 buf ^= 1u;
-                if (r != 0) __syncthreads();
+                cur = nxt; p = pn; v = vn;
+                if (r >= 1) __syncthreads();
             }
         }
     } else {
@@ -802,9 +840,20 @@ int launch_fused_pairs(const Geo& g, const Workspace& ws, const tpc_digit* digit
     sg.slot_bytes = sg.surv_off + 4u * sg.scap;
     const uint32_t smem = kPSlots * sg.slot_bytes + fixed;
 
+    // Pads per CTA: a CTA builds its pad range plus a halo of 4 lines and pays a fixed prologue (~2 lines' worth), and
+    // the grid runs in waves of 148 x (CTAs per SM) CTAs: take the range that minimises waves x (range + 6).  A full
+    // frame gets whole planes; a single sector is cut so that the last wave is not nearly empty.
     const uint32_t whole = (g.max_pads + kPS - 1) / kPS * kPS;
-    uint32_t pads_per_unit = g.n_planes >= 1184 ? whole : (g.n_planes >= 296 ? 12 * kPS : 6 * kPS);
-    if (pads_per_unit > whole) pads_per_unit = whole;
+    const uint32_t resident = 148u * (uint32_t)std::max(1, std::min(4, (int)(227u * 1024u / (smem + 1024u + stat))));
+    uint32_t pads_per_unit = whole;
+    {
+        uint64_t best = ~0ull;
+        for (uint32_t u = 3 * kPS; u <= whole; u += kPS) {
+            const uint64_t units = (uint64_t)g.n_planes * ((g.max_pads + u - 1) / u);
+            const uint64_t cost = ((units + resident - 1) / resident) * (u + 6);
+            if (cost <= best) { best = cost; pads_per_unit = u; }     // ties: the larger range (less halo)
+        }
+    }
     if (tun.pads_per_unit >= kPS && tun.pads_per_unit <= 256) pads_per_unit = (uint32_t)(tun.pads_per_unit / kPS * kPS);
     const uint32_t upp = (g.max_pads + pads_per_unit - 1) / pads_per_unit;
     if (ev_k0) cudaEventRecord(ev_k0, st);

@@ -547,3 +547,29 @@ def test_config5_full_four_frames_every_plane():
     """configs[4] at full size: 36 sectors, pads 66 -> 138, 4 frames back to back on one stream: every cluster."""
     total, kernel = _full_frame_check(5, frames=4)
     assert total > 7_000_000
+
+
+@pytest.mark.parametrize("path", ["fused_pairs", "fused_blocks", "fused_lines", "general"])
+@pytest.mark.parametrize("odd_n", [0, 1])
+def test_digit_buffer_eight_bytes_off_a_16_byte_boundary(path, odd_n):
+    """The ABI asks for 8-byte aligned digits only: a buffer that starts 8 bytes off a 16-byte boundary (and one whose
+    last digit ends 8 bytes off) must give the same clusters — the bulk copies of k_fused_pairs move 16-byte aligned
+    pieces and copy the ragged first / last digit of the array by hand."""
+    import torch
+    cf = _cf()
+    digits = gen.generate(1)
+    if (digits.shape[0] & 1) != odd_n:
+        digits = digits[:-1]
+    geom = gen.geometry(1)
+    ora, ost = orc.run(digits, *geom[:4])
+    n = digits.shape[0]
+    finder = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=ost["n_clusters"] + 16)
+    finder.debug_set(**TUNING.get(path, {}))
+    buf = torch.zeros((n + 2) * 8, dtype=torch.uint8, device="cuda:0")
+    assert buf.data_ptr() % 16 == 0
+    buf[8:8 + n * 8] = torch.from_numpy(digits.view(np.uint8)).cuda()
+    finder.run(buf[8:], n, flags=PATHS[path])
+    cl, st = finder.result()
+    assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == 0
+    assert_clusters_equal(cl, ora, "misaligned buffer/" + path)
+    finder.close()
