@@ -16,7 +16,7 @@ HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh")) +
                  glob.glob(os.path.join(os.path.dirname(_HERE), "include", "*.h")))
 EXTRA = os.environ.get("TPC_CF_NVCC_EXTRA", "").split()
 NVCC_FLAGS = EXTRA + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall"]
+              "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-ldl"]
 
 
 def _nvcc():

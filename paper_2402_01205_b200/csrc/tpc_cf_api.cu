@@ -4,9 +4,18 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "tpc_cf_internal.cuh"
 
 using namespace tpccf;
+
+// NVTX range over a group of launches (host side: marks the enqueue; a profiler correlates the kernels under it).
+// A no-op unless a tool is attached.
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 static constexpr int kProfSlots = 64;
 static constexpr int kMaxGroups = 18;    // sector groups of the tpc_cf_run_host pipeline
@@ -87,8 +96,7 @@ static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, ch
     w.ghist_part = (uint32_t*)take((ceil_div_u64(tiles * 256, 1024) + 1) * 4);
     w.line_start = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
     w.line_cnt = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
-    w.line_off = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
-    w.line_part = (uint32_t*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 1024) + 1) * 4);
+    w.line_desc = (unsigned long long*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 256) + 1) * 8);
     w.group_status = (tpc_cf_status*)take(sizeof(tpc_cf_status) * 32);
     if (ws) *ws = w;
     if (n_sort_tiles) *n_sort_tiles = (uint32_t)tiles;
@@ -184,25 +192,35 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
 
     (void)cudaGetLastError();
     if (prof) cudaEventRecord(ev[0], st);
-    cudaError_t e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), st);
-    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(counters)");
+    cudaError_t e = cudaSuccess;
+    if (!fused || n == 0) {       // (the fused path's index kernel zeroes the counters)
+        e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), st);
+        if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(counters)");
+    }
 
+    NvtxRange nv_run(fused ? "tpc_cf_run (fused path)" : "tpc_cf_run (general path)");
     if (fused) {
         // T3: line index -> fused smem kernel (scatter into smem lines, peak test, moments) -> compaction
-        int r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n, params->q_peak_min, params->q_inner_gate, var, h->tun, st,
+        int r;
+        {
+            NvtxRange nv("K0 K1 K2 K4: line index + fused kernel (clean, scatter, peaks, moments)");
+            r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n, params->q_peak_min, params->q_inner_gate, var, h->tun, st,
                                     prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
+        }
         if (r < 0) return r;
         k += r;
-        k += launch_compact_lines(h->geo, h->ws, out->clusters, out->capacity, st);
-        k += launch_finalize(h->ws, out->status, out->capacity, 3u, 1, n, st);
+        NvtxRange nv("K3 K5: scan + ordered copy + status");
+        k += launch_compact_lines(h->geo, h->ws, out->clusters, out->capacity, out->status, n, st);
     } else {
         // T1: K1 scatter -> K2+K4 digit-centric peaks + moments on the HBM map -> K3 compaction -> (K5 key sort)
         //     -> K0 un-scatter
-        k += launch_general_peaks(h->geo, h->ws, digits, n, params->q_peak_min, params->q_inner_gate, var, st,
-                                  prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
-        k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, hint ? 0 : 1, st);
-        if (!hint) k += launch_key_sort(h->ws, h->max_clusters, h->n_sort_tiles, out->clusters, out->capacity, st);
-        k += launch_unscatter(h->geo, h->ws, digits, n, st);
+        { NvtxRange nv("K1 K2 K4: scatter, peaks + moments on the map");
+          k += launch_general_peaks(h->geo, h->ws, digits, n, params->q_peak_min, params->q_inner_gate, var, st,
+                                    prof ? ev[1] : nullptr, prof ? ev[2] : nullptr); }
+        { NvtxRange nv("K3: compaction");
+          k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, hint ? 0 : 1, st); }
+        if (!hint) { NvtxRange nv("K5: key sort"); k += launch_key_sort(h->ws, h->max_clusters, h->n_sort_tiles, out->clusters, out->capacity, st); }
+        { NvtxRange nv("K0: un-scatter"); k += launch_unscatter(h->geo, h->ws, digits, n, st); }
         k += launch_finalize(h->ws, out->status, out->capacity, 1u, hint ? 1 : 0, n, st);
     }
     if (prof) { cudaEventRecord(ev[3], st); ++h->run_index; }

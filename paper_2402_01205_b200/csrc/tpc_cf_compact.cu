@@ -152,16 +152,22 @@ int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t c
 
 // ---- K3 + K5 for the fused path: the peaks of a line are already packed, in time order, at the start of the
 // line's own digit range in `stage`; a scan over the per-line counts gives each line its place in the output.
+// ONE kernel: a block owns 256 consecutive lines; it scans their counts, publishes its total in line_desc[block] and
+// finds the clusters in front of it by a decoupled look-back (a warp reads the 32 descriptors before it at a time:
+// flag 1 = this block's total, flag 2 = total of everything up to and including this block), then copies its records:
+// they are consecutive in the output, so the block copies one contiguous output range, every thread moving 16-byte
+// halves and finding the source line of a record by a binary search in the block's prefix sums (shared memory).
+// The last block knows the frame's cluster count and writes the status block.
+static constexpr unsigned long long kDescMask = (1ull << 62) - 1ull;
+
 __global__ void __launch_bounds__(256)
-k_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __restrict__ line_off,
-               const uint32_t* __restrict__ line_start, uint32_t n_lines, const uint4* __restrict__ stage,
-               uint4* __restrict__ out, uint64_t capacity)
+k_scan_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __restrict__ line_start, uint32_t n_lines,
+                    const uint4* __restrict__ stage, uint4* __restrict__ out, uint64_t capacity,
+                    unsigned long long* line_desc, Counters* cnt, tpc_cf_status* status, uint64_t n)
 {
-    // A block owns 256 consecutive lines; their records are consecutive in the output, so the block copies
-    // one contiguous output range: every thread moves 16-byte halves, finding the source line of a record by a
-    // binary search in the block's prefix sums (shared memory).
     __shared__ uint32_t s_pref[257];
     __shared__ uint32_t s_src[256];
+    __shared__ unsigned long long s_excl;
     const uint32_t line = blockIdx.x * 256 + threadIdx.x;
     const uint32_t c = line < n_lines ? line_cnt[line] : 0u;
     uint32_t total;
@@ -174,9 +180,52 @@ k_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __restrict
         total = s_total;
         if (threadIdx.x == 0) s_pref[256] = total;
     }
+    if (threadIdx.x < 32) {
+        volatile unsigned long long* desc = line_desc;
+        const unsigned lane = threadIdx.x;
+        unsigned long long excl = 0ull;
+        if (blockIdx.x == 0) {
+            if (lane == 0) desc[0] = (2ull << 62) | (unsigned long long)total;
+        } else {
+            if (lane == 0) desc[blockIdx.x] = (1ull << 62) | (unsigned long long)total;
+            int j = (int)blockIdx.x - 1;                      // descriptor lane 0 looks at
+            while (true) {
+                const int idx = j - (int)lane;
+                unsigned long long v = idx >= 0 ? desc[idx] : (2ull << 62);      // in front of block 0: prefix 0
+                while (__any_sync(0xffffffffu, (v >> 62) == 0ull)) v = idx >= 0 ? desc[idx] : (2ull << 62);
+                const unsigned full = __ballot_sync(0xffffffffu, (v >> 62) == 2ull);
+                const unsigned upto = full ? (unsigned)__ffs(full) : 32u;       // lanes < upto contribute
+                unsigned long long part = lane < upto ? (v & kDescMask) : 0ull;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+                excl += part;
+                if (full) break;
+                j -= 32;
+            }
+            if (lane == 0) desc[blockIdx.x] = (2ull << 62) | (excl + (unsigned long long)total);
+        }
+        if (lane == 0) {
+            s_excl = excl;
+            if (blockIdx.x == gridDim.x - 1) {               // the frame's count is known here: status, written last
+                tpc_cf_status s;
+                s.n_clusters = excl + total;
+                s.n_digits_used = n - cnt->n_bad;
+                s.n_bad_digits = cnt->n_bad;
+                s.overflow = s.n_clusters > capacity ? 1u : 0u;
+                s.path = 3u;
+                if (cnt->unsorted) {      // false DIGITS_SORTED promise: detected, no output (include/tpc_cf.h)
+                    s.n_clusters = 0;
+                    s.overflow = 0;
+                    s.path = 0;
+                }
+                cnt->n_clusters = excl + total;
+                *status = s;
+            }
+        }
+    }
     __syncthreads();
     if (total == 0) return;
-    const uint64_t dst0 = line_off[blockIdx.x * 256];
+    const uint64_t dst0 = s_excl;
     for (uint32_t i = threadIdx.x; i < 2 * total; i += 256) {
         const uint32_t r = i >> 1;
         uint32_t lo = 0, hi = 256;                       // last line with s_pref[line] <= r
@@ -186,13 +235,14 @@ k_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __restrict
     }
 }
 
-int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, uint64_t capacity, cudaStream_t st)
+int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, uint64_t capacity,
+                         tpc_cf_status* status, uint64_t n, cudaStream_t st)
 {
     const uint32_t n_lines = g.n_planes * g.LS;
-    int k = launch_scan_u32(ws.line_cnt, ws.line_off, n_lines, ws.line_part, &ws.counters->n_clusters, st);
-    k_gather_lines<<<(n_lines + 255) / 256, 256, 0, st>>>(ws.line_cnt, ws.line_off, ws.line_start, n_lines,
-                                                      (const uint4*)ws.stage, (uint4*)out, capacity);
-    return k + 1;
+    k_scan_gather_lines<<<(n_lines + 255) / 256, 256, 0, st>>>(ws.line_cnt, ws.line_start, n_lines,
+                                                               (const uint4*)ws.stage, (uint4*)out, capacity,
+                                                               ws.line_desc, ws.counters, status, n);
+    return 1;
 }
 
 // ---- K5 for unsorted input: LSD radix sort of (key40, index), 8 bits per pass, warp-private tiles -------------

@@ -46,9 +46,10 @@ __device__ __forceinline__ uint32_t lower_bound_key(const uint2* __restrict__ di
 
 // level 1: first digit of every plane (entry p = 0 of each plane; the final entry is n)
 __global__ void __launch_bounds__(256)
-k_plane_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start)
+k_plane_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start, Counters* cnt)
 {
     const uint32_t plane = blockIdx.x * 256 + threadIdx.x;
+    if (plane == 0) { cnt->n_bad = 0ull; cnt->n_used = 0ull; cnt->n_clusters = 0ull; cnt->unsorted = 0u; cnt->rsv = 0u; }
     if (plane > g.n_planes) return;
     if (plane == g.n_planes) { line_start[(size_t)g.n_planes * g.LS] = n; return; }
     const uint32_t s = plane / g.n_rows, r = plane % g.n_rows;
@@ -57,10 +58,14 @@ k_plane_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __r
 
 // level 2: the lines of a plane, searched inside the plane's own range
 __global__ void __launch_bounds__(256)
-k_line_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start)
+k_line_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start,
+             uint32_t* __restrict__ line_cnt, unsigned long long* __restrict__ line_desc)
 {
     const uint32_t total = g.n_planes * g.LS;
     const uint32_t e = blockIdx.x * 256 + threadIdx.x;
+    // per-run state of the compaction: peak counts (pads beyond npads[row] stay 0) and scan descriptors
+    if (e <= total) line_cnt[e] = 0u;
+    if (e <= (total + 255u) / 256u) line_desc[e] = 0ull;
     if (e >= total) return;
     const uint32_t plane = e / g.LS, p = e % g.LS;
     if (p == 0) return;                                   // written by k_plane_index
@@ -461,12 +466,17 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
                         uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, cudaStream_t st,
                         cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
-    cudaMemsetAsync(ws.line_cnt, 0, ((size_t)g.n_planes * g.LS + 1) * 4, st);   // pads beyond npads[row] stay 0
-    if (n == 0) return 0;
-    int k = 0;
     const uint32_t entries = g.n_planes * g.LS + 1;
-    k_plane_index<<<(g.n_planes + 1 + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start);
-    k_line_index<<<(entries + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start);
+    if (n == 0) {     // nothing to index: only the per-run state of the compaction (the caller zeroed the counters)
+        cudaMemsetAsync(ws.line_cnt, 0, (size_t)entries * 4, st);
+        cudaMemsetAsync(ws.line_desc, 0, ((size_t)(entries + 255) / 256 + 1) * 8, st);
+        return 0;
+    }
+    int k = 0;
+    k_plane_index<<<(g.n_planes + 1 + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
+                                                                 ws.counters);
+    k_line_index<<<(entries + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
+                                                        ws.line_cnt, ws.line_desc);
     k += 2;
 
     // Kernel choice.  Block-sparse line slots when the mean line fits their pool (k_fused_pairs, tpc_cf_pairs.cu; its

@@ -45,8 +45,8 @@ struct Workspace {
     uint32_t* ghist_part;
     uint32_t* line_start; // [n_planes*LS + 1] first digit of each (plane,pad) line (fused path)
     uint32_t* line_cnt;   // [n_planes*LS + 1] peaks per line (fused path)
-    uint32_t* line_off;   // exclusive scan of line_cnt
-    uint32_t* line_part;  // scan partials for the line counts
+    unsigned long long* line_desc;   // [n_lines / 256 + 1] per 256-line block: (flag << 62) | clusters, for the
+                                     // single-pass scan of k_scan_gather_lines (fused path); zeroed by k_line_index
     tpc_cf_status* group_status;   // [32] per-group status blocks of the tpc_cf_run_host pipeline
 };
 
@@ -237,8 +237,10 @@ cudaError_t fused_pairs_set_attributes();
 // compaction of stage[j] by peakmask into dst (= out, or ws.compact when a key sort must follow)
 int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t capacity, uint64_t max_clusters,
                    int sort_if_unsorted, cudaStream_t st);
-// fused path: scan of ws.line_cnt, then one warp per line copies stage[line_start + k] -> out[line_off + k]
-int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, uint64_t capacity, cudaStream_t st);
+// fused path, ONE kernel: single-pass scan of ws.line_cnt (decoupled look-back over blocks of 256 lines), copy
+// stage[line_start + k] -> out[offset + k], and the status block (written by the last block).
+int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, uint64_t capacity,
+                         tpc_cf_status* status, uint64_t n, cudaStream_t st);
 int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_tiles, tpc_cluster* out,
                     uint64_t capacity, cudaStream_t st);
 int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,
