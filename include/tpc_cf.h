@@ -89,7 +89,10 @@ typedef struct {
     uint64_t n_clusters;     /* true number of clusters (peaks that pass the cuts), even if > capacity */
     uint64_t n_digits_used;  /* valid digits */
     uint64_t n_bad_digits;   /* R11: out-of-range or zero-charge digits: skipped and counted */
-    uint32_t overflow;       /* 1 if n_clusters > capacity: the first `capacity` clusters in output order are written */
+    uint32_t overflow;       /* 1 if n_clusters > capacity: the first `capacity` clusters in output order are written.
+                                Unsorted input is ordered by a key sort that holds at most the max_clusters given to
+                                create: with more peaks than that, overflow = 1 too, and what is written are the first
+                                max_clusters peaks in DIGIT order, sorted (A2) */
     uint32_t path;           /* 1 = general path (T1) produced the output, 3 = fused sorted path (T3),
                                 0 = no output: DIGITS_SORTED was promised but the digits are not sorted */
 } tpc_cf_status;
@@ -115,9 +118,20 @@ enum {
 };
 
 /* Bytes of DEVICE workspace `create` needs for this geometry and these capacities (0 on invalid geometry).
- * Layout: dense uint16 charge map with a 2-cell zero border per plane, line index, unit tables,
- * cluster staging (32 B per max_clusters), sort scratch for the general path. */
+ * Layout: dense uint16 charge map with a 2-cell zero border per plane (general path: 22.3 GB for the
+ * full 36-sector geometry), peak mask, line index and counts, cluster staging (32 B per max_DIGITS: the cluster of a
+ * peak is staged at its line's digit range, only peak slots are ever touched), and 56 B per max_clusters of
+ * compaction + sort scratch for unsorted input. */
 size_t tpc_cf_workspace_bytes(const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters);
+
+/* Workspace variants.  TPC_CF_WS_SORTED_ONLY: the caller will only ever run with TPC_CF_DIGITS_SORTED (and without
+ * TPC_CF_FORCE_GENERAL): the workspace then holds no charge map, no peak mask and no sort scratch — line index,
+ * counts and staging only.  A run that would need the general path returns TPC_CF_E_PARAMS on such a handle, and
+ * tpc_cf_run_host does not fall back on a false promise (the status then says path 0). */
+enum { TPC_CF_WS_SORTED_ONLY = 1u };
+size_t tpc_cf_workspace_bytes_ex(const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters, uint32_t ws_flags);
+int tpc_cf_create_ex(tpc_cf** h, const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters,
+                     uint32_t ws_flags, void* workspace, size_t workspace_bytes, void* stream);
 
 /* Creates a handle bound to a caller-owned DEVICE workspace (256-byte aligned, >= tpc_cf_workspace_bytes).
  * Enqueues on `stream` the one-time zeroing of the charge map; every run leaves the map zero again (K0 is an
@@ -150,6 +164,13 @@ int tpc_cf_run_host(tpc_cf* h, const tpc_digit* host_digits, uint64_t n,
  * (sector,row) into `dense` (DEVICE, npads(row) x n_time uint16, pad-major), and un-scatters again. */
 int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint64_t n,
                              uint32_t sector, uint32_t row, uint16_t* dense, void* stream);
+
+/* Launch-shape hint for runs that cover only part of a frame (one frame cut over several GPUs, paper_2402_01205_b200/
+ * shard.py; PAPER.md:100 has whole frames per GPU instead).  The fused path sizes its shared-memory line slots from
+ * the mean digits per pad line = n / (pads of the WHOLE geometry); a run on a slice of the planes would take them N
+ * times too small and fall back to its (exact, slower) overflow paths.  frame_digits = digits of the whole frame the
+ * following runs are slices of; 0 = every run is a whole frame (default).  Never changes the result. */
+int tpc_cf_set_frame_digits(tpc_cf* h, uint64_t frame_digits);
 
 /* Test / tuning overrides of one handle (the tests force every kernel and every slow path with them; profiling uses
  * them to compare launch shapes).  They select among exact implementations and never change the result.  value 0

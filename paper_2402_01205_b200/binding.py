@@ -23,6 +23,7 @@ assert DIGIT.itemsize == 8 and CLUSTER.itemsize == 32 and STATUS.itemsize == 32
 
 DIGITS_SORTED = 1
 FORCE_GENERAL = 2
+WS_SORTED_ONLY = 1      # tpc_cf_create_ex / tpc_cf_workspace_bytes_ex
 # cluster-finder variants (include/tpc_cf.h V1..V3): params.flags bits and tpc_cluster.flags bits
 CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME = 4, 8, 16
 F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED = 1, 2, 4, 8, 16
@@ -31,8 +32,8 @@ F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED = 1, 2, 4, 8, 
 DEBUG_KEYS = {"fused_kernel": 1, "passes": 2, "block_pool": 3, "surv_cap": 4, "pads_per_unit": 5, "ctas_per_sm": 6}
 FUSED_KERNELS = {"auto": 0, "pairs": 1, "blocks": 2, "lines": 3}
 
-EXPORTS = ["tpc_cf_workspace_bytes", "tpc_cf_create", "tpc_cf_run", "tpc_cf_run_host",
-           "tpc_cf_debug_dense_plane", "tpc_cf_debug_set", "tpc_cf_last_launch_count", "tpc_cf_last_kernel", "tpc_cf_set_profiling",
+EXPORTS = ["tpc_cf_workspace_bytes", "tpc_cf_workspace_bytes_ex", "tpc_cf_create", "tpc_cf_create_ex", "tpc_cf_run", "tpc_cf_run_host",
+           "tpc_cf_debug_dense_plane", "tpc_cf_debug_set", "tpc_cf_set_frame_digits", "tpc_cf_last_launch_count", "tpc_cf_last_kernel", "tpc_cf_set_profiling",
            "tpc_cf_profile_ms", "tpc_cf_destroy", "tpc_cf_strerror"]
 
 
@@ -77,6 +78,11 @@ def load(build_if_missing=True):
     lib.tpc_cf_create.restype = ctypes.c_int
     lib.tpc_cf_create.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.POINTER(Geometry), ctypes.c_uint64,
                                   ctypes.c_uint64, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
+    lib.tpc_cf_workspace_bytes_ex.restype = ctypes.c_size_t
+    lib.tpc_cf_workspace_bytes_ex.argtypes = [ctypes.POINTER(Geometry), ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32]
+    lib.tpc_cf_create_ex.restype = ctypes.c_int
+    lib.tpc_cf_create_ex.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.POINTER(Geometry), ctypes.c_uint64,
+                                     ctypes.c_uint64, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
     lib.tpc_cf_run.restype = ctypes.c_int
     lib.tpc_cf_run.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.POINTER(Geometry),
                                ctypes.POINTER(Params), ctypes.POINTER(Out)]
@@ -87,6 +93,8 @@ def load(build_if_missing=True):
     lib.tpc_cf_debug_dense_plane.restype = ctypes.c_int
     lib.tpc_cf_debug_dense_plane.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32,
                                              ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
+    lib.tpc_cf_set_frame_digits.restype = ctypes.c_int
+    lib.tpc_cf_set_frame_digits.argtypes = [ctypes.c_void_p, ctypes.c_uint64]
     lib.tpc_cf_debug_set.restype = ctypes.c_int
     lib.tpc_cf_debug_set.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]
     lib.tpc_cf_last_launch_count.restype = ctypes.c_int
@@ -147,7 +155,9 @@ class ClusterFinder:
     run(digits_dev, n) only enqueues on the current torch stream; result() synchronises and reads back."""
 
     def __init__(self, n_sectors, n_rows, max_pads, n_time, npads=None, max_digits=1 << 20, max_clusters=None,
-                 q_peak_min=4, q_inner_gate=2, q_tot_min=0, q_saturation=0, device="cuda:0"):
+                 q_peak_min=4, q_inner_gate=2, q_tot_min=0, q_saturation=0, device="cuda:0", sorted_only=False):
+        """sorted_only: a workspace without the dense charge map and the sort scratch (TPC_CF_WS_SORTED_ONLY): every
+        run must then carry DIGITS_SORTED (22 GB less for the full 36-sector geometry)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("tpc_cf needs a CUDA device; there is no CPU fallback")
@@ -158,7 +168,9 @@ class ClusterFinder:
         self.max_digits = int(max_digits)
         self.max_clusters = int(max_clusters if max_clusters is not None else max(1, self.max_digits // 4))
         self.params = Params(q_peak_min, q_inner_gate, 0, q_tot_min, q_saturation, 0)
-        nbytes = tpc_cf_workspace_bytes(self.geom, self.max_digits, self.max_clusters)
+        ws_flags = WS_SORTED_ONLY if sorted_only else 0
+        nbytes = int(self.lib.tpc_cf_workspace_bytes_ex(ctypes.byref(self.geom), self.max_digits, self.max_clusters,
+                                                        ws_flags))
         if nbytes == 0:
             raise TpcCfError(-2, "invalid geometry or capacities")
         self.workspace_bytes = nbytes
@@ -168,7 +180,9 @@ class ClusterFinder:
             self.clusters = torch.empty(self.max_clusters * 32, dtype=torch.uint8, device=self.device)
             self.status = torch.zeros(32, dtype=torch.uint8, device=self.device)
             stream = torch.cuda.current_stream(self.device).cuda_stream
-            self.h = tpc_cf_create(self.geom, self.max_digits, self.max_clusters, self._ws_ptr, nbytes, stream)
+            self.h = ctypes.c_void_p()
+            _check(self.lib.tpc_cf_create_ex(ctypes.byref(self.h), ctypes.byref(self.geom), self.max_digits,
+                                             self.max_clusters, ws_flags, self._ws_ptr, nbytes, stream))
 
     def run(self, digits_dev, n=None, flags=0, clusters=None, capacity=None, status=None):
         """digits_dev: torch uint8 tensor on the device holding n 8-byte records."""
@@ -221,6 +235,10 @@ class ClusterFinder:
         _check(self.lib.tpc_cf_debug_dense_plane(self.h, digits_dev.data_ptr() if n else None, n, sector, row,
                                                  dense.data_ptr(), stream))
         return dense.cpu().numpy().view(np.uint16).reshape(npads_row, self.geom.n_time)
+
+    def set_frame_digits(self, frame_digits):
+        """Launch-shape hint: the following runs are slices of a frame of `frame_digits` digits (0 = whole frames)."""
+        _check(self.lib.tpc_cf_set_frame_digits(self.h, int(frame_digits)))
 
     def debug_set(self, **kw):
         """Test / tuning overrides of this handle (include/tpc_cf.h TPC_CF_DEBUG_*): fused_kernel ("pairs", "blocks",

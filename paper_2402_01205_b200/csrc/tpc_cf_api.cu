@@ -29,6 +29,8 @@ struct tpc_cf {
     int last_launches;
     uint64_t shape_n;           // digits of the whole frame while tpc_cf_run_host runs it group by group, else 0
     Tuning tun;                 // tpc_cf_debug_set overrides (all 0 by default)
+    uint32_t ws_flags;          // TPC_CF_WS_* the workspace was carved with
+    uint64_t shape_hint;        // tpc_cf_set_frame_digits: digits of the whole frame when runs cover a part of it, else 0
     const char* last_kernel;
     int profiling;
     uint32_t run_index;         // runs since profiling was switched on
@@ -70,22 +72,24 @@ static bool same_geometry(const Geo& a, const Geo& b)
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // Carves the workspace; base may be NULL to compute the size only.
-static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, char* base, Workspace* ws,
-                    uint32_t* n_sort_tiles, size_t* map_bytes)
+static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, uint32_t ws_flags, char* base,
+                    Workspace* ws, uint32_t* n_sort_tiles, size_t* map_bytes)
 {
+    const bool sorted_only = (ws_flags & TPC_CF_WS_SORTED_ONLY) != 0;   // no map, no mask, no sort scratch
     size_t off = 0;
     auto take = [&](size_t bytes) { char* p = base ? base + off : nullptr; off += align256(bytes ? bytes : 1); return p; };
     const uint64_t nwords = ceil_div_u64(max_digits, 32) + 1;
     const uint64_t nblk = ceil_div_u64(nwords, 256) + 1;
     const uint64_t tiles = ceil_div_u64(max_clusters ? max_clusters : 1, 2048);
-    const size_t mapb = (size_t)g.n_planes * g.PS * g.TS * sizeof(uint16_t);
+    const size_t mapb = sorted_only ? 0 : (size_t)g.n_planes * g.PS * g.TS * sizeof(uint16_t);
+    if (sorted_only) max_clusters = 0;
     Workspace w;
     w.counters = (Counters*)take(sizeof(Counters));
     w.map = (uint16_t*)take(mapb);
-    w.peakmask = (uint32_t*)take(nwords * 4);
-    w.blk_cnt = (uint32_t*)take(nblk * 4);
-    w.blk_off = (uint32_t*)take(nblk * 4);
-    w.scan_part = (uint32_t*)take((ceil_div_u64(nblk, 1024) + 1) * 4);
+    w.peakmask = (uint32_t*)take(sorted_only ? 0 : nwords * 4);
+    w.blk_cnt = (uint32_t*)take(sorted_only ? 0 : nblk * 4);
+    w.blk_off = (uint32_t*)take(sorted_only ? 0 : nblk * 4);
+    w.scan_part = (uint32_t*)take(sorted_only ? 0 : (ceil_div_u64(nblk, 1024) + 1) * 4);
     w.stage = (tpc_cluster*)take((size_t)max_digits * sizeof(tpc_cluster));
     w.compact = (tpc_cluster*)take((size_t)max_clusters * sizeof(tpc_cluster));
     w.keyA = (uint64_t*)take((size_t)max_clusters * 8);
@@ -111,23 +115,37 @@ static int cuda_fail(tpc_cf* h, cudaError_t e, const char* where)
     return TPC_CF_E_CUDA;
 }
 
-extern "C" size_t tpc_cf_workspace_bytes(const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters)
+extern "C" size_t tpc_cf_workspace_bytes_ex(const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters,
+                                            uint32_t ws_flags)
 {
     Geo g;
     if (!geom || !geometry_to_geo(geom, &g)) return 0;
     if (max_digits >= (1ull << 32) || max_clusters >= (1ull << 32)) return 0;
-    return carve(g, max_digits, max_clusters, nullptr, nullptr, nullptr, nullptr);
+    if (ws_flags & ~(uint32_t)TPC_CF_WS_SORTED_ONLY) return 0;
+    return carve(g, max_digits, max_clusters, ws_flags, nullptr, nullptr, nullptr, nullptr);
+}
+
+extern "C" size_t tpc_cf_workspace_bytes(const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters)
+{
+    return tpc_cf_workspace_bytes_ex(geom, max_digits, max_clusters, 0u);
 }
 
 extern "C" int tpc_cf_create(tpc_cf** hp, const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters,
                              void* workspace, size_t workspace_bytes, void* stream)
 {
+    return tpc_cf_create_ex(hp, geom, max_digits, max_clusters, 0u, workspace, workspace_bytes, stream);
+}
+
+extern "C" int tpc_cf_create_ex(tpc_cf** hp, const tpc_cf_geometry* geom, uint64_t max_digits, uint64_t max_clusters,
+                                uint32_t ws_flags, void* workspace, size_t workspace_bytes, void* stream)
+{
+    if (ws_flags & ~(uint32_t)TPC_CF_WS_SORTED_ONLY) return TPC_CF_E_PARAMS;
     if (!hp || !geom || !workspace) return TPC_CF_E_NULL;
     Geo g;
     if (!geometry_to_geo(geom, &g)) return TPC_CF_E_GEOMETRY;
     if (max_digits >= (1ull << 32) || max_clusters >= (1ull << 32)) return TPC_CF_E_CAPACITY;
     if (((uintptr_t)workspace & 255u) != 0) return TPC_CF_E_WORKSPACE;
-    if (carve(g, max_digits, max_clusters, nullptr, nullptr, nullptr, nullptr) > workspace_bytes)
+    if (carve(g, max_digits, max_clusters, ws_flags, nullptr, nullptr, nullptr, nullptr) > workspace_bytes)
         return TPC_CF_E_WORKSPACE;
     tpc_cf* h = new (std::nothrow) tpc_cf;
     if (!h) return TPC_CF_E_NOMEM;
@@ -135,7 +153,8 @@ extern "C" int tpc_cf_create(tpc_cf** hp, const tpc_cf_geometry* geom, uint64_t 
     h->geo = g;
     h->max_digits = max_digits;
     h->max_clusters = max_clusters;
-    carve(g, max_digits, max_clusters, (char*)workspace, &h->ws, &h->n_sort_tiles, &h->map_bytes);
+    h->ws_flags = ws_flags;
+    carve(g, max_digits, max_clusters, ws_flags, (char*)workspace, &h->ws, &h->n_sort_tiles, &h->map_bytes);
     for (int i = 0; i < kProfSlots * 4; ++i) {
         cudaError_t e = cudaEventCreate(&h->ev[i / 4][i % 4]);
         if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaEventCreate"); }
@@ -145,7 +164,7 @@ extern "C" int tpc_cf_create(tpc_cf** hp, const tpc_cf_geometry* geom, uint64_t 
     if (e == cudaSuccess) e = fused_blocks_set_attributes();
     if (e == cudaSuccess) e = fused_lines_set_attributes();
     // K0, once: the charge map starts zero; every run restores it (un-scatter).
-    if (e == cudaSuccess) e = cudaMemsetAsync(h->ws.map, 0, h->map_bytes, (cudaStream_t)stream);
+    if (e == cudaSuccess && h->map_bytes) e = cudaMemsetAsync(h->ws.map, 0, h->map_bytes, (cudaStream_t)stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), (cudaStream_t)stream);
     if (e != cudaSuccess) {
         for (int i = 0; i < kProfSlots * 4; ++i) cudaEventDestroy(h->ev[i / 4][i % 4]);
@@ -180,6 +199,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     cudaStream_t st = (cudaStream_t)out->stream;
     const bool hint = (params->flags & TPC_CF_DIGITS_SORTED) != 0;
     const bool fused = hint && !(params->flags & TPC_CF_FORCE_GENERAL);
+    if (!fused && (h->ws_flags & TPC_CF_WS_SORTED_ONLY)) return TPC_CF_E_PARAMS;   // no map in this workspace
     const bool prof = h->profiling != 0;
     cudaEvent_t* ev = h->ev[h->run_index % kProfSlots];
     int k = 0;
@@ -204,7 +224,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
         int r;
         {
             NvtxRange nv("K0 K1 K2 K4: line index + fused kernel (clean, scatter, peaks, moments)");
-            r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n, params->q_peak_min, params->q_inner_gate, var, h->tun, st,
+            r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n ? h->shape_n : h->shape_hint, params->q_peak_min, params->q_inner_gate, var, h->tun, st,
                                     prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
         }
         if (r < 0) return r;
@@ -221,7 +241,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
           k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, hint ? 0 : 1, st); }
         if (!hint) { NvtxRange nv("K5: key sort"); k += launch_key_sort(h->ws, h->max_clusters, h->n_sort_tiles, out->clusters, out->capacity, st); }
         { NvtxRange nv("K0: un-scatter"); k += launch_unscatter(h->geo, h->ws, digits, n, st); }
-        k += launch_finalize(h->ws, out->status, out->capacity, 1u, hint ? 1 : 0, n, st);
+        k += launch_finalize(h->ws, out->status, out->capacity, 1u, hint ? 1 : 0, n, h->max_clusters, st);
     }
     if (prof) { cudaEventRecord(ev[3], st); ++h->run_index; }
     e = cudaGetLastError();
@@ -362,7 +382,7 @@ extern "C" int tpc_cf_run_host(tpc_cf* h, const tpc_digit* host_digits, uint64_t
         e = cudaMemcpyAsync(host_status, dev_status, sizeof(tpc_cf_status), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) return cuda_fail(h, e, "status readback");
-        if (host_status->path != 0) break;
+        if (host_status->path != 0 || (h->ws_flags & TPC_CF_WS_SORTED_ONLY)) break;   // (no general path to fall back on)
         prm.flags &= ~(uint32_t)TPC_CF_DIGITS_SORTED;   // the promise was false: rerun on the general path
     }
     uint64_t m = host_status->n_clusters < capacity ? host_status->n_clusters : capacity;
@@ -380,6 +400,7 @@ extern "C" int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint
     if (!h || !dense || (n && !digits)) return TPC_CF_E_NULL;
     if (n > h->max_digits) return TPC_CF_E_CAPACITY;
     if (sector >= h->geo.n_sectors || row >= h->geo.n_rows) return TPC_CF_E_GEOMETRY;
+    if (h->ws_flags & TPC_CF_WS_SORTED_ONLY) return TPC_CF_E_PARAMS;
     cudaStream_t st = (cudaStream_t)stream;
     (void)cudaGetLastError();
     cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), st);
@@ -388,6 +409,13 @@ extern "C" int tpc_cf_debug_dense_plane(tpc_cf* h, const tpc_digit* digits, uint
     launch_unscatter(h->geo, h->ws, digits, n, st);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(h, e, "debug_dense_plane");
+    return TPC_CF_OK;
+}
+
+extern "C" int tpc_cf_set_frame_digits(tpc_cf* h, uint64_t frame_digits)
+{
+    if (!h) return TPC_CF_E_NULL;
+    h->shape_hint = frame_digits;
     return TPC_CF_OK;
 }
 
@@ -453,7 +481,7 @@ extern "C" const char* tpc_cf_strerror(int code)
     case TPC_CF_E_GEOMETRY: return "invalid geometry, or geometry differs from create";
     case TPC_CF_E_CAPACITY: return "n exceeds max_digits, or a capacity is >= 2^32";
     case TPC_CF_E_WORKSPACE: return "workspace too small or not 256-byte aligned";
-    case TPC_CF_E_PARAMS: return "invalid params (q_peak_min == 0 or unknown flag bits)";
+    case TPC_CF_E_PARAMS: return "invalid params (q_peak_min == 0, unknown flag bits, or a general-path run on a sorted-only workspace)";
     case TPC_CF_E_CUDA: return g_last_cuda_msg[0] ? g_last_cuda_msg : "CUDA error";
     case TPC_CF_E_NOMEM: return "host allocation failed";
     default: return "unknown error";

@@ -364,7 +364,7 @@ int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_
 
 // ---- status ---------------------------------------------------------------------------------------------------
 __global__ void k_finalize(const Counters* cnt, tpc_cf_status* status, uint64_t capacity, uint32_t path,
-                           int hint_sorted, uint64_t n)
+                           int hint_sorted, uint64_t n, uint64_t max_clusters)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     tpc_cf_status s;
@@ -372,6 +372,9 @@ __global__ void k_finalize(const Counters* cnt, tpc_cf_status* status, uint64_t 
     s.n_digits_used = n - cnt->n_bad;
     s.n_bad_digits = cnt->n_bad;
     s.overflow = s.n_clusters > capacity ? 1u : 0u;
+    // unsorted input goes through the key sort, which holds at most the workspace's max_clusters records (A2): beyond
+    // that only the first max_clusters peaks in digit order were kept (sorted), whatever the caller's capacity
+    if (!hint_sorted && cnt->unsorted && s.n_clusters > max_clusters) s.overflow = 1u;
     s.path = path;
     if (hint_sorted && cnt->unsorted) {   // false DIGITS_SORTED promise: detected, no output (include/tpc_cf.h)
         s.n_clusters = 0;
@@ -382,9 +385,9 @@ __global__ void k_finalize(const Counters* cnt, tpc_cf_status* status, uint64_t 
 }
 
 int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,
-                    int hint_sorted, uint64_t n, cudaStream_t st)
+                    int hint_sorted, uint64_t n, uint64_t max_clusters, cudaStream_t st)
 {
-    k_finalize<<<1, 32, 0, st>>>(ws.counters, status, capacity, path, hint_sorted, n);
+    k_finalize<<<1, 32, 0, st>>>(ws.counters, status, capacity, path, hint_sorted, n, max_clusters);
     return 1;
 }
 

@@ -44,6 +44,28 @@ __device__ __forceinline__ uint32_t lower_bound_key(const uint2* __restrict__ di
     return lo;
 }
 
+// the same result by an 8-ary search: 7 independent probes per step instead of one (the search is bound by the latency
+// of dependent loads: 6 steps instead of 16 for a plane of 40 k digits)
+__device__ __forceinline__ uint32_t lower_bound_key8(const uint2* __restrict__ digits, uint32_t lo, uint32_t hi,
+                                                     uint32_t target)
+{
+    while (hi - lo > 8u) {
+        const uint32_t step = (hi - lo) >> 3;
+        uint32_t k[7];
+#pragma unroll
+        for (int i = 0; i < 7; ++i) k[i] = key24_of(__ldg(&digits[lo + (uint32_t)(i + 1) * step].x));
+        // first pivot whose key is >= target bounds the answer from above; the one before it from below
+        uint32_t nlo = lo, nhi = hi;
+#pragma unroll
+        for (int i = 6; i >= 0; --i) if (k[i] >= target) nhi = lo + (uint32_t)(i + 1) * step;
+#pragma unroll
+        for (int i = 0; i < 7; ++i) if (k[i] < target) nlo = lo + (uint32_t)(i + 1) * step + 1u;
+        if (nlo > nhi) nlo = nhi;        // keys not ascending (false DIGITS_SORTED promise): stay in bounds, terminate
+        lo = nlo; hi = nhi;
+    }
+    return lower_bound_key(digits, lo, hi, target);
+}
+
 // level 1: first digit of every plane (entry p = 0 of each plane; the final entry is n)
 __global__ void __launch_bounds__(256)
 k_plane_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start, Counters* cnt)
@@ -53,7 +75,7 @@ k_plane_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __r
     if (plane > g.n_planes) return;
     if (plane == g.n_planes) { line_start[(size_t)g.n_planes * g.LS] = n; return; }
     const uint32_t s = plane / g.n_rows, r = plane % g.n_rows;
-    line_start[(size_t)plane * g.LS] = lower_bound_key(digits, 0, n, (s << 16) | (r << 8));
+    line_start[(size_t)plane * g.LS] = lower_bound_key8(digits, 0, n, (s << 16) | (r << 8));
 }
 
 // level 2: the lines of a plane, searched inside the plane's own range
@@ -72,7 +94,7 @@ k_line_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __re
     const uint32_t s = plane / g.n_rows, r = plane % g.n_rows;
     uint32_t lo = line_start[(size_t)plane * g.LS], hi = line_start[(size_t)(plane + 1) * g.LS];
     if (hi < lo || hi > n) { lo = 0; hi = n; }            // unsorted input: stay in bounds, the fused kernel reports it
-    line_start[e] = lower_bound_key(digits, lo, hi, (s << 16) | (r << 8) | p);
+    line_start[e] = lower_bound_key(digits, lo, hi, (s << 16) | (r << 8) | p);   // (8-ary measured slower here: 122 vs 100 us — request-bound, not latency-bound)
 }
 
 // Slot layout (warp-uniform).

@@ -244,7 +244,7 @@ int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, ui
 int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_tiles, tpc_cluster* out,
                     uint64_t capacity, cudaStream_t st);
 int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,
-                    int hint_sorted, uint64_t n, cudaStream_t st);
+                    int hint_sorted, uint64_t n, uint64_t max_clusters, cudaStream_t st);
 
 // exclusive scan of n uint32 (in -> out, may alias); total (optional) receives the sum as 64-bit.
 int launch_scan_u32(const uint32_t* in, uint32_t* out, uint64_t n, uint32_t* partials,

@@ -40,7 +40,9 @@ def plane_partition(plane_start, world):
 def gather_records(local, n_local, record_bytes=32, dst=0, group=None):
     """local: torch uint8 tensor holding n_local records of this rank (device or CPU, matching the backend).
     Returns (records, counts) on rank dst — records = the ranks' records concatenated in rank order — and
-    (None, counts) elsewhere.  counts: python list of per-rank record counts (all ranks)."""
+    (None, counts) elsewhere.  counts: python list of per-rank record counts (all ranks).
+    A rank whose compute failed passes n_local < 0: the all-gather of the counts tells every rank, and ALL of them
+    raise before any record moves (nobody is left waiting in a send or receive)."""
     import torch
     import torch.distributed as dist
     world, rank = dist.get_world_size(group), dist.get_rank(group)
@@ -48,6 +50,9 @@ def gather_records(local, n_local, record_bytes=32, dst=0, group=None):
     allc = [torch.zeros(1, dtype=torch.int64, device=local.device) for _ in range(world)]
     dist.all_gather(allc, mine, group=group)
     counts = [int(c.item()) for c in allc]
+    failed = [r for r, c in enumerate(counts) if c < 0]
+    if failed:
+        raise RuntimeError("sharded run failed on rank(s) %r (this is rank %d)" % (failed, rank))
     if rank != dst:
         if n_local:
             dist.send(local[:n_local * record_bytes].contiguous(), dst=dst, group=group)
@@ -88,18 +93,27 @@ class ShardedClusterFinder:
         world, rank = dist.get_world_size(self.group), dist.get_rank(self.group)
         part = plane_partition(plane_counts(digits_host, self.geom[0], self.geom[1]), world)[rank]
         mine = digits_host[part[2]:part[3]]
-        d = to_device(mine, device=self.finder.device) if mine.shape[0] else None
         n = int(mine.shape[0])
-        if n:
-            self.finder.run(d, n, flags=DIGITS_SORTED if flags is None else flags)
-            raw = self.finder.status.cpu().numpy().view(STATUS)[0]      # synchronises this rank's stream
-            st = {k: int(raw[k]) for k in STATUS.names}
-            if st["path"] == 0 or st["overflow"]:
-                raise RuntimeError("shard %d: cluster finder status %r" % (rank, st))
-            n_cl = st["n_clusters"]
-        else:
-            n_cl = 0
-        out, counts = gather_records(self.finder.clusters, n_cl, 32, 0, self.group)
+        n_cl, err = 0, None
+        try:
+            if n:
+                d = to_device(mine, device=self.finder.device)
+                # the launch shape comes from the WHOLE frame's line length, not from this rank's slice
+                self.finder.set_frame_digits(int(digits_host.shape[0]))
+                self.finder.run(d, n, flags=DIGITS_SORTED if flags is None else flags)
+                raw = self.finder.status.cpu().numpy().view(STATUS)[0]      # synchronises this rank's stream
+                st = {k: int(raw[k]) for k in STATUS.names}
+                if st["path"] == 0 or st["overflow"]:
+                    raise RuntimeError("shard %d: cluster finder status %r" % (rank, st))
+                n_cl = st["n_clusters"]
+        except Exception as e:                                   # tell the peers (count -1) before raising
+            n_cl, err = -1, e
+        try:
+            out, counts = gather_records(self.finder.clusters, n_cl, 32, 0, self.group)
+        except RuntimeError:
+            if err is not None:
+                raise err
+            raise
         return out, counts, part
 
     def close(self):

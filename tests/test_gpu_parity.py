@@ -573,3 +573,82 @@ def test_digit_buffer_eight_bytes_off_a_16_byte_boundary(path, odd_n):
     assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == 0
     assert_clusters_equal(cl, ora, "misaligned buffer/" + path)
     finder.close()
+
+
+def test_sharded_cluster_finder_world_size_1_nccl():
+    """NEXT #4 on the one GPU there is: ShardedClusterFinder under a world-size-1 NCCL group drives plane_partition ->
+    tpc_cf_run (with the frame-wide launch-shape hint) -> gather_records on device tensors; result against the oracle."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    cf = _cf()
+    c = dict(gen.CONFIGS[3]); c["n_sectors"] = 2
+    geom = gen.geometry(c)
+    digits = gen.generate(c)
+    ora, ost = orc.run_parallel(digits, *geom[:4])[:2]
+    created = not dist.is_initialized()
+    if created:
+        s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % port, rank=0, world_size=1,
+                                device_id=torch.device("cuda:0"))
+    try:
+        sf = cf.ShardedClusterFinder(*geom[:4], max_digits=digits.shape[0], max_clusters=ost["n_clusters"] + 16)
+        out, counts, part = sf.run(digits)
+        assert counts == [ost["n_clusters"]] and part[:2] == (0, geom[0] * geom[1])
+        cl = out.cpu().numpy().view(cf.CLUSTER)
+        assert_clusters_equal(cl, ora, "sharded, world size 1")
+        sf.close()
+    finally:
+        if created:
+            dist.destroy_process_group()
+
+
+def test_unsorted_input_more_peaks_than_the_workspace_holds():
+    """unsorted input, workspace max_clusters < n_clusters <= capacity: the key sort keeps max_clusters
+    records only, so the run must say overflow = 1 (and the true count) instead of handing back uninitialised tail
+    records.  What is written: the first max_clusters peaks in digit order, sorted by key (A2)."""
+    import torch
+    cf = _cf()
+    digits = gen.generate(1)
+    geom = gen.geometry(1)
+    ora, ost = orc.run(digits, *geom[:4])
+    n = digits.shape[0]
+    sh = digits[np.random.default_rng(5).permutation(n)]
+    mc = 1000
+    f = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=mc)
+    big = torch.zeros(ost["n_clusters"] * 32 + 64, dtype=torch.uint8, device="cuda:0")
+    f.run(cf.to_device(sh), n, flags=0, clusters=big, capacity=ost["n_clusters"] + 2)
+    cl, st = f.result(clusters=big)
+    assert st["path"] == 1 and st["n_clusters"] == ost["n_clusters"] and st["overflow"] == 1
+    # the kept subset: peaks of the first digits (in the shuffled order) that are peaks, mc of them, sorted
+    k_all = key(ora)
+    dk = ((sh["sector"].astype(np.uint64) << 32) | (sh["row"].astype(np.uint64) << 24) |
+          (sh["pad"].astype(np.uint64) << 16) | sh["time"].astype(np.uint64))
+    is_peak = np.isin(dk, k_all)
+    first = np.sort(dk[is_peak][:mc])
+    assert np.array_equal(key(cl[:mc]), first)
+    f.close()
+
+
+def test_sorted_only_workspace():
+    """TPC_CF_WS_SORTED_ONLY: no charge map, no sort scratch in the workspace (22 GB less at the full geometry); sorted
+    runs give the same clusters; a run that needs the general path is refused synchronously."""
+    cf = _cf()
+    digits = gen.generate(2)
+    geom = gen.geometry(2)
+    ora, ost = orc.run_parallel(digits, *geom[:4])[:2]
+    n = digits.shape[0]
+    full = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=ost["n_clusters"] + 16)
+    lean = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=ost["n_clusters"] + 16, sorted_only=True)
+    assert lean.workspace_bytes < full.workspace_bytes - 2 * 152 * 138 * 14336
+    full.close()
+    d = cf.to_device(digits)
+    lean.run(d, n, flags=cf.DIGITS_SORTED)
+    cl, st = lean.result()
+    assert st["path"] == 3 and st["n_clusters"] == ost["n_clusters"]
+    assert_clusters_equal(cl, ora, "sorted-only workspace")
+    for flags in (0, cf.DIGITS_SORTED | cf.FORCE_GENERAL):
+        with pytest.raises(cf.TpcCfError) as e:
+            lean.run(d, n, flags=flags)
+        assert e.value.code == -5
+    lean.close()
