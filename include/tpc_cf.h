@@ -201,6 +201,25 @@ const char* tpc_cf_last_kernel(const tpc_cf* h);
 int   tpc_cf_set_profiling(tpc_cf* h, int on);
 float tpc_cf_profile_ms(tpc_cf* h, uint32_t run, int which);
 
+/* Exclusive prefix sum of n uint32 (in -> out, DEVICE pointers, may alias; *total, optional DEVICE pointer, receives
+ * the sum as 64-bit) WITHOUT any allocation and without a handle: the scan of K3 (compaction) for callers that cannot
+ * allocate — code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc.  The kernels are the ones
+ * tpc_cf_run uses; their scratch (one partial sum per 1024 elements) lives in a file-scope device array of the
+ * library: 257 KB that every GPU which loads the library holds until exit.  Limit: n <= tpc_cf_scan_static_max_n() =
+ * 2^26 elements per call; beyond it the call enqueues nothing and returns TPC_CF_E_CAPACITY.  Calls no cudaMalloc /
+ * cudaFree / allocating routine; enqueues on `stream` and returns.  All calls on a device share the scratch: each
+ * overwrites what it reads, so back-to-back calls on one stream are independent, but calls that OVERLAP on the GPU
+ * (several streams, concurrent graph replays) race.  The array's device address is resolved once per device by
+ * tpc_cf_scan_static_setup() (cudaGetSymbolAddress with that device current); the scan calls it on first use — call it
+ * yourself before capturing a graph. */
+uint64_t tpc_cf_scan_static_max_n(void);
+int tpc_cf_scan_static_setup(void);
+int tpc_cf_scan_u32_static(const uint32_t* in, uint32_t* out, uint64_t n, unsigned long long* total, void* stream);
+
+/* Test hook: the same scan with its scratch taken from the handle's caller-owned workspace (the path tpc_cf_run
+ * takes); n is limited by the workspace.  tests/test_zz_no_alloc.py compares the two. */
+int tpc_cf_debug_scan_u32(tpc_cf* h, const uint32_t* in, uint32_t* out, uint64_t n, unsigned long long* total, void* stream);
+
 int tpc_cf_destroy(tpc_cf* h);
 
 const char* tpc_cf_strerror(int code);

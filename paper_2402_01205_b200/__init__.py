@@ -5,8 +5,8 @@ The CUDA library (libtpc_cf.so) is loaded on first use; there is no CPU fallback
 """
 from .binding import (CLUSTER, CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME, DIGIT, DIGITS_SORTED, EXPORTS,
                       F_EDGE_PAD, F_EDGE_TIME, F_SATURATED, F_SINGLE_PAD, F_SINGLE_TIME, FORCE_GENERAL, STATUS, ClusterFinder, Geometry, Out,
-                      Params, TpcCfError, load, make_geometry, to_device, tpc_cf_create, tpc_cf_destroy,
-                      tpc_cf_run, tpc_cf_workspace_bytes)
+                      Params, TpcCfError, load, make_geometry, scan_u32_static, to_device, tpc_cf_create,
+                      tpc_cf_destroy, tpc_cf_run, tpc_cf_workspace_bytes)
 
 from .ec_binding import (EC_ERR_CAPACITY, EC_ERR_CONTAINER, EC_ERR_QTOT, EC_ERR_UNSORTED, EC_EXPORTS, EC_STATUS,
                          ClusterCoder, clusters_to_device, tpc_ec_create, tpc_ec_decode, tpc_ec_destroy,
@@ -24,5 +24,5 @@ __all__ = ["ShardedClusterFinder", "gather_records", "plane_counts", "plane_part
            "tpc_ec_max_encoded_bytes", "tpc_ec_workspace_bytes",
            "CLUSTER", "DIGIT", "STATUS", "DIGITS_SORTED", "FORCE_GENERAL", "CLUSTER_FLAGS", "CUT_SINGLE_PAD",
            "CUT_SINGLE_TIME", "F_EDGE_PAD", "F_EDGE_TIME", "F_SINGLE_PAD", "F_SINGLE_TIME", "F_SATURATED", "EXPORTS", "ClusterFinder", "Geometry",
-           "Out", "Params", "TpcCfError", "load", "make_geometry", "to_device", "tpc_cf_create", "tpc_cf_destroy",
+           "Out", "Params", "TpcCfError", "load", "make_geometry", "scan_u32_static", "to_device", "tpc_cf_create", "tpc_cf_destroy",
            "tpc_cf_run", "tpc_cf_workspace_bytes"]

@@ -33,7 +33,8 @@ DEBUG_KEYS = {"fused_kernel": 1, "passes": 2, "block_pool": 3, "surv_cap": 4, "p
 FUSED_KERNELS = {"auto": 0, "pairs": 1, "blocks": 2, "lines": 3}
 
 EXPORTS = ["tpc_cf_workspace_bytes", "tpc_cf_workspace_bytes_ex", "tpc_cf_create", "tpc_cf_create_ex", "tpc_cf_run", "tpc_cf_run_host",
-           "tpc_cf_debug_dense_plane", "tpc_cf_debug_set", "tpc_cf_set_frame_digits", "tpc_cf_last_launch_count", "tpc_cf_last_kernel", "tpc_cf_set_profiling",
+           "tpc_cf_debug_dense_plane", "tpc_cf_debug_set", "tpc_cf_set_frame_digits", "tpc_cf_scan_static_max_n",
+           "tpc_cf_scan_static_setup", "tpc_cf_scan_u32_static", "tpc_cf_debug_scan_u32", "tpc_cf_last_launch_count", "tpc_cf_last_kernel", "tpc_cf_set_profiling",
            "tpc_cf_profile_ms", "tpc_cf_destroy", "tpc_cf_strerror"]
 
 
@@ -95,6 +96,15 @@ def load(build_if_missing=True):
                                              ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
     lib.tpc_cf_set_frame_digits.restype = ctypes.c_int
     lib.tpc_cf_set_frame_digits.argtypes = [ctypes.c_void_p, ctypes.c_uint64]
+    lib.tpc_cf_scan_static_max_n.restype = ctypes.c_uint64
+    lib.tpc_cf_scan_static_max_n.argtypes = []
+    lib.tpc_cf_scan_static_setup.restype = ctypes.c_int
+    lib.tpc_cf_scan_static_setup.argtypes = []
+    lib.tpc_cf_scan_u32_static.restype = ctypes.c_int
+    lib.tpc_cf_scan_u32_static.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_void_p, ctypes.c_void_p]
+    lib.tpc_cf_debug_scan_u32.restype = ctypes.c_int
+    lib.tpc_cf_debug_scan_u32.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64,
+                                          ctypes.c_void_p, ctypes.c_void_p]
     lib.tpc_cf_debug_set.restype = ctypes.c_int
     lib.tpc_cf_debug_set.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]
     lib.tpc_cf_last_launch_count.restype = ctypes.c_int
@@ -143,6 +153,16 @@ def tpc_cf_create(geom, max_digits, max_clusters, workspace_ptr, workspace_bytes
 
 def tpc_cf_run(h, digits_ptr, n, geom, params, out):
     _check(load().tpc_cf_run(h, digits_ptr, n, ctypes.byref(geom), ctypes.byref(params), ctypes.byref(out)))
+
+
+def scan_u32_static(inp, out, n, total=None):
+    """tpc_cf_scan_u32_static on torch device tensors (uint32 viewed as int32 or uint8 storage): no allocation, scratch
+    in the library's static device array; enqueues on the current torch stream.  Raises TpcCfError beyond the limit."""
+    import torch
+    stream = torch.cuda.current_stream(inp.device).cuda_stream
+    with torch.cuda.device(inp.device):
+        _check(load().tpc_cf_scan_u32_static(inp.data_ptr() if n else None, out.data_ptr() if n else None, int(n),
+                                             total.data_ptr() if total is not None else None, stream))
 
 
 def tpc_cf_destroy(h):
@@ -247,6 +267,12 @@ class ClusterFinder:
             if name == "fused_kernel" and isinstance(value, str):
                 value = FUSED_KERNELS[value]
             _check(self.lib.tpc_cf_debug_set(self.h, DEBUG_KEYS[name], int(value)))
+
+    def debug_scan_u32(self, inp, out, n, total=None):
+        """The existing scan path: scratch in this handle's workspace (tpc_cf_debug_scan_u32)."""
+        stream = self.torch.cuda.current_stream(self.device).cuda_stream
+        _check(self.lib.tpc_cf_debug_scan_u32(self.h, inp.data_ptr() if n else None, out.data_ptr() if n else None, int(n),
+                                              total.data_ptr() if total is not None else None, stream))
 
     def set_profiling(self, on):
         _check(self.lib.tpc_cf_set_profiling(self.h, 1 if on else 0))

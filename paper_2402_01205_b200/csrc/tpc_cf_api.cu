@@ -435,6 +435,19 @@ extern "C" int tpc_cf_debug_set(tpc_cf* h, int key, int value)
     return TPC_CF_OK;
 }
 
+extern "C" int tpc_cf_debug_scan_u32(tpc_cf* h, const uint32_t* in, uint32_t* out, uint64_t n, unsigned long long* total,
+                                     void* stream)
+{
+    if (!h || (n && (!in || !out))) return TPC_CF_E_NULL;
+    // partial sums in the handle's workspace (the cluster staging area is idle between runs)
+    if ((ceil_div_u64(n, 1024) + 1) * 4 > h->max_digits * sizeof(tpc_cluster)) return TPC_CF_E_CAPACITY;
+    (void)cudaGetLastError();
+    launch_scan_u32(in, out, n, (uint32_t*)h->ws.stage, total, (cudaStream_t)stream);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(h, e, "debug_scan_u32");
+    return TPC_CF_OK;
+}
+
 extern "C" int tpc_cf_last_launch_count(const tpc_cf* h) { return h ? h->last_launches : TPC_CF_E_NULL; }
 
 extern "C" const char* tpc_cf_last_kernel(const tpc_cf* h) { return h && h->last_kernel ? h->last_kernel : ""; }

@@ -391,4 +391,59 @@ int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacit
     return 1;
 }
 
+// ---- exclusive scan without any allocation: scratch in a file-scope device array ----------------------------------
+// For callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+// the same three scan kernels as launch_scan_u32, with the per-block partial sums in a static device array instead of
+// a caller-owned workspace.  Every GPU that loads the library holds the array (257 KB) until exit.
+// In HOST code the array's name is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, resolved once per device with that device current (tpc_cf_scan_static_setup).
+// All calls on a device share the array: it keeps the last call's partials, every call overwrites the entries it will
+// read (partials [0, ceil(n / 1024)) by k_scan_reduce) before it reads them, so nothing has to start at zero — but two
+// calls that overlap on the GPU (different streams, or graphs replayed concurrently) race on it.
+static constexpr uint64_t kScanStaticMaxN = 1ull << 26;                       // elements per call
+static constexpr uint32_t kScanStaticPartials = (uint32_t)(kScanStaticMaxN / kScanThreads) + 256u;
+static __device__ __align__(256) uint32_t g_scan_static_partials[kScanStaticPartials];
+
+static constexpr int kMaxDevices = 64;
+static uint32_t* g_scan_static_ptr[kMaxDevices];     // device address of the array, per device (0 = not resolved)
+
 }  // namespace tpccf
+
+using namespace tpccf;
+
+extern "C" uint64_t tpc_cf_scan_static_max_n(void) { return kScanStaticMaxN; }
+
+extern "C" int tpc_cf_scan_static_setup(void)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return TPC_CF_E_CUDA;
+    if (g_scan_static_ptr[dev]) return TPC_CF_OK;
+    uint32_t* p = nullptr;
+    if (cudaGetSymbolAddress((void**)&p, g_scan_static_partials) != cudaSuccess || !p) {
+        (void)cudaGetLastError();
+        return TPC_CF_E_CUDA;
+    }
+    g_scan_static_ptr[dev] = p;
+    return TPC_CF_OK;
+}
+
+extern "C" int tpc_cf_scan_u32_static(const uint32_t* in, uint32_t* out, uint64_t n, unsigned long long* total,
+                                      void* stream)
+{
+    if (n && (!in || !out)) return TPC_CF_E_NULL;
+    if (n > kScanStaticMaxN) return TPC_CF_E_CAPACITY;        // beyond the static scratch: use a handle's workspace
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return TPC_CF_E_CUDA;
+    if (!g_scan_static_ptr[dev]) {
+        const int rc = tpc_cf_scan_static_setup();            // (callers that capture graphs call the set-up beforehand)
+        if (rc != TPC_CF_OK) return rc;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n == 0) {
+        if (total && cudaMemsetAsync(total, 0, sizeof *total, st) != cudaSuccess) return TPC_CF_E_CUDA;
+        return TPC_CF_OK;
+    }
+    (void)cudaGetLastError();
+    launch_scan_u32(in, out, n, g_scan_static_ptr[dev], total, st);
+    return cudaGetLastError() == cudaSuccess ? TPC_CF_OK : TPC_CF_E_CUDA;
+}
