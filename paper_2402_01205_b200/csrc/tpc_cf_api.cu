@@ -100,7 +100,7 @@ static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, ui
     w.ghist_part = (uint32_t*)take((ceil_div_u64(tiles * 256, 1024) + 1) * 4);
     w.line_start = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
     w.line_cnt = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
-    w.line_desc = (unsigned long long*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 256) + 1) * 8);
+    w.line_desc = (unsigned long long*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 64) + 1) * 8);
     w.group_status = (tpc_cf_status*)take(sizeof(tpc_cf_status) * 32);
     if (ws) *ws = w;
     if (n_sort_tiles) *n_sort_tiles = (uint32_t)tiles;

@@ -160,25 +160,29 @@ int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t c
 // The last block knows the frame's cluster count and writes the status block.
 static constexpr unsigned long long kDescMask = (1ull << 62) - 1ull;
 
+template <int LINES>      // lines per block: 256, or 64 for small geometries (a single sector has only 21 k lines)
 __global__ void __launch_bounds__(256)
 k_scan_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __restrict__ line_start, uint32_t n_lines,
                     const uint4* __restrict__ stage, uint4* __restrict__ out, uint64_t capacity,
                     unsigned long long* line_desc, Counters* cnt, tpc_cf_status* status, uint64_t n)
 {
-    __shared__ uint32_t s_pref[257];
-    __shared__ uint32_t s_src[256];
+    __shared__ uint32_t s_pref[LINES + 1];
+    __shared__ uint32_t s_src[LINES];
     __shared__ unsigned long long s_excl;
-    const uint32_t line = blockIdx.x * 256 + threadIdx.x;
-    const uint32_t c = line < n_lines ? line_cnt[line] : 0u;
+    const uint32_t line = blockIdx.x * LINES + threadIdx.x;
+    const bool mine = threadIdx.x < LINES && line < n_lines;
+    const uint32_t c = mine ? line_cnt[line] : 0u;
     uint32_t total;
     {
         __shared__ uint32_t s_total;
         const uint32_t ex = block_exclusive_scan(c, &s_total);
-        s_pref[threadIdx.x] = ex;
-        s_src[threadIdx.x] = line < n_lines ? line_start[line] : 0u;
+        if (threadIdx.x < LINES) {
+            s_pref[threadIdx.x] = ex;
+            s_src[threadIdx.x] = mine ? line_start[line] : 0u;
+        }
         __syncthreads();
         total = s_total;
-        if (threadIdx.x == 0) s_pref[256] = total;
+        if (threadIdx.x == 0) s_pref[LINES] = total;
     }
     if (threadIdx.x < 32) {
         volatile unsigned long long* desc = line_desc;
@@ -228,7 +232,7 @@ k_scan_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __res
     const uint64_t dst0 = s_excl;
     for (uint32_t i = threadIdx.x; i < 2 * total; i += 256) {
         const uint32_t r = i >> 1;
-        uint32_t lo = 0, hi = 256;                       // last line with s_pref[line] <= r
+        uint32_t lo = 0, hi = LINES;                     // last line with s_pref[line] <= r
         while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (s_pref[mid] <= r) lo = mid; else hi = mid; }
         const uint64_t src = (uint64_t)s_src[lo] + (r - s_pref[lo]);
         if (dst0 + r < capacity) __stcs(out + 2 * (dst0 + r) + (i & 1u), __ldcs(stage + 2 * src + (i & 1u)));
@@ -239,9 +243,15 @@ int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, ui
                          tpc_cf_status* status, uint64_t n, cudaStream_t st)
 {
     const uint32_t n_lines = g.n_planes * g.LS;
-    k_scan_gather_lines<<<(n_lines + 255) / 256, 256, 0, st>>>(ws.line_cnt, ws.line_start, n_lines,
-                                                               (const uint4*)ws.stage, (uint4*)out, capacity,
-                                                               ws.line_desc, ws.counters, status, n);
+    // (line_desc holds one descriptor per 64 lines: tpc_cf_api.cu carve, k_line_index)
+    if (n_lines >= 64u * 148u * 16u)
+        k_scan_gather_lines<256><<<(n_lines + 255) / 256, 256, 0, st>>>(ws.line_cnt, ws.line_start, n_lines,
+                                                                        (const uint4*)ws.stage, (uint4*)out, capacity,
+                                                                        ws.line_desc, ws.counters, status, n);
+    else
+        k_scan_gather_lines<64><<<(n_lines + 63) / 64, 256, 0, st>>>(ws.line_cnt, ws.line_start, n_lines,
+                                                                     (const uint4*)ws.stage, (uint4*)out, capacity,
+                                                                     ws.line_desc, ws.counters, status, n);
     return 1;
 }
 

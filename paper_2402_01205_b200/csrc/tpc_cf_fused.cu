@@ -87,7 +87,7 @@ k_line_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __re
     const uint32_t e = blockIdx.x * 256 + threadIdx.x;
     // per-run state of the compaction: peak counts (pads beyond npads[row] stay 0) and scan descriptors
     if (e <= total) line_cnt[e] = 0u;
-    if (e <= (total + 255u) / 256u) line_desc[e] = 0ull;
+    if (e <= (total + 63u) / 64u) line_desc[e] = 0ull;
     if (e >= total) return;
     const uint32_t plane = e / g.LS, p = e % g.LS;
     if (p == 0) return;                                   // written by k_plane_index
@@ -491,7 +491,7 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     const uint32_t entries = g.n_planes * g.LS + 1;
     if (n == 0) {     // nothing to index: only the per-run state of the compaction (the caller zeroed the counters)
         cudaMemsetAsync(ws.line_cnt, 0, (size_t)entries * 4, st);
-        cudaMemsetAsync(ws.line_desc, 0, ((size_t)(entries + 255) / 256 + 1) * 8, st);
+        cudaMemsetAsync(ws.line_desc, 0, ((size_t)(entries + 63) / 64 + 1) * 8, st);
         return 0;
     }
     int k = 0;
