@@ -628,6 +628,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--shuffle", action="store_true",
+                    help="a seeded random permutation of the frame's digits, without the DIGITS_SORTED promise (the any-order "
+                         "contract): digit sort on the device + fused path by default, the general path with --path "
+                         "general; implies --no-e2e --no-per-config")
     ap.add_argument("--no-parity", action="store_true",
                     help="skip the element-by-element comparison of every cluster with the oracle (all host cores)")
     ap.add_argument("--no-per-config", dest="per_config", action="store_false",
@@ -650,6 +654,8 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
+    if args.shuffle:
+        args.no_e2e, args.per_config = True, False
     if args.impl == "reference":
         return run_reference(args)
     if args.stage == "ec":
@@ -695,7 +701,7 @@ def compare_clusters(gpu, ora):
 
 
 def measure_config(cf, torch, cfg_id, steps, warmup, path, variant, dev, frame_offset=0, parity=True, sampler=None,
-                   keep=False):
+                   keep=False, shuffle=False):
     """One config, device-resident: generate its frame(s), run `steps` timed steps (a step = every frame of the config
     through tpc_cf_run, back to back on one stream), time the dominant kernel by its own event pair, and compare every
     cluster of every frame with the oracle run on all host cores.  Returns a dict (and, with keep, the live objects)."""
@@ -717,6 +723,14 @@ def measure_config(cf, torch, cfg_id, steps, warmup, path, variant, dev, frame_o
     pinned = [torch.from_numpy(f.view(np.uint8)).pin_memory() for f in frames] if keep else None
     dev_digits = [(p if p is not None else torch.from_numpy(f.view(np.uint8))).to(dev, non_blocking=True)
                   for p, f in zip(pinned or [None] * n_frames, frames)]
+    if shuffle:
+        # any-order contract: a seeded random permutation of the device-resident digits, no
+        # DIGITS_SORTED promise; the result must be the same array (R12), so the oracle still runs on the sorted frame
+        gsh = torch.Generator(device=dev)
+        gsh.manual_seed(2402)
+        dev_digits = [d.view(torch.int64)[torch.randperm(n, device=dev, generator=gsh)].contiguous().view(torch.uint8)
+                      for d, n in zip(dev_digits, n_digits)]
+        flags = vflags | (cf.FORCE_GENERAL if path == "general" else 0)
     outs = [torch.empty(max_clusters * 32, dtype=torch.uint8, device=dev) for _ in frames]
     stats = [torch.zeros(32, dtype=torch.uint8, device=dev) for _ in frames]
     torch.cuda.synchronize()
@@ -847,7 +861,8 @@ def run_cf(args):
         dist.barrier()
     # replicas: rank r works on its own frames (frame index offset by rank * frames)
     m = measure_config(cf, torch, args.config, args.steps, args.warmup, args.path, args.variant, dev,
-                       frame_offset=rank * cfg["frames"], parity=do_parity, sampler=sampler, keep=True)
+                       frame_offset=rank * cfg["frames"], parity=do_parity, sampler=sampler, keep=True,
+                       shuffle=args.shuffle)
     clocks = sampler
     live = m.pop("_live")
     finder, frames, pinned, dev_digits = live["finder"], live["frames"], live["pinned"], live["dev_digits"]
@@ -941,7 +956,7 @@ def run_cf(args):
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u16/i32/f32", "data": "synthetic",
             "config": {"workload": "config%d: %s" % (args.config, cfg["label"]), "path": args.path,
-                       "variant": args.variant,
+                       "variant": args.variant, "digit_order": "shuffled (seeded permutation)" if args.shuffle else "sorted",
                        "frames_per_step": n_frames, "digits_per_frame": nd, "clusters_per_frame": nc,
                        "occupancy": m["occupancy"], "parallelism": "replicas x%d" % world,
                        "l2": m["l2"],

@@ -93,8 +93,10 @@ typedef struct {
                                 Unsorted input is ordered by a key sort that holds at most the max_clusters given to
                                 create: with more peaks than that, overflow = 1 too, and what is written are the first
                                 max_clusters peaks in DIGIT order, sorted (A2) */
-    uint32_t path;           /* 1 = general path (T1) produced the output, 3 = fused sorted path (T3),
-                                0 = no output: DIGITS_SORTED was promised but the digits are not sorted */
+    uint32_t path;           /* 1 = general path (T1) produced the output, 3 = fused sorted path (T3), 2 = the digits were
+                                sorted on the device and the fused path ran on the sorted copy (input without the
+                                DIGITS_SORTED promise), 0 = no output: DIGITS_SORTED was promised but the digits are not
+                                sorted, or (path 2) two digits address the same cell */
 } tpc_cf_status;
 
 typedef struct {

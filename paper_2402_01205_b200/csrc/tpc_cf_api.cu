@@ -102,6 +102,9 @@ static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, ui
     w.line_cnt = (uint32_t*)take(((size_t)g.n_planes * g.LS + 2) * 4);
     w.line_desc = (unsigned long long*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 64) + 1) * 8);
     w.group_status = (tpc_cf_status*)take(sizeof(tpc_cf_status) * 32);
+    w.sort_tmp = (tpc_digit*)take(sorted_only ? 0 : (size_t)max_digits * sizeof(tpc_digit));
+    w.sort_top = (uint32_t*)take(1032 * 4);
+    w.sort_part = (uint32_t*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 1024) + 4) * 4);
     if (ws) *ws = w;
     if (n_sort_tiles) *n_sort_tiles = (uint32_t)tiles;
     if (map_bytes) *map_bytes = mapb;
@@ -163,6 +166,7 @@ extern "C" int tpc_cf_create_ex(tpc_cf** hp, const tpc_cf_geometry* geom, uint64
     cudaError_t e = fused_pairs_set_attributes();
     if (e == cudaSuccess) e = fused_blocks_set_attributes();
     if (e == cudaSuccess) e = fused_lines_set_attributes();
+    if (e == cudaSuccess) e = sort_set_attributes();
     // K0, once: the charge map starts zero; every run restores it (un-scatter).
     if (e == cudaSuccess && h->map_bytes) e = cudaMemsetAsync(h->ws.map, 0, h->map_bytes, (cudaStream_t)stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->ws.counters, 0, sizeof(Counters), (cudaStream_t)stream);
@@ -199,7 +203,9 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     cudaStream_t st = (cudaStream_t)out->stream;
     const bool hint = (params->flags & TPC_CF_DIGITS_SORTED) != 0;
     const bool fused = hint && !(params->flags & TPC_CF_FORCE_GENERAL);
-    if (!fused && (h->ws_flags & TPC_CF_WS_SORTED_ONLY)) return TPC_CF_E_PARAMS;   // no map in this workspace
+    if (!fused && (h->ws_flags & TPC_CF_WS_SORTED_ONLY)) return TPC_CF_E_PARAMS;   // no map, no sort buffer in this workspace
+    // no promise about the order: sort the digits on the device, then the fused path (tpc_cf_sort.cu)
+    const bool sortfuse = !hint && !(params->flags & TPC_CF_FORCE_GENERAL) && n > 0;
     const bool prof = h->profiling != 0;
     cudaEvent_t* ev = h->ev[h->run_index % kProfSlots];
     int k = 0;
@@ -218,19 +224,25 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
         if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(counters)");
     }
 
-    NvtxRange nv_run(fused ? "tpc_cf_run (fused path)" : "tpc_cf_run (general path)");
-    if (fused) {
-        // T3: line index -> fused smem kernel (scatter into smem lines, peak test, moments) -> compaction
+    NvtxRange nv_run(fused ? "tpc_cf_run (fused path)" : sortfuse ? "tpc_cf_run (digit sort + fused path)" : "tpc_cf_run (general path)");
+    if (fused || sortfuse) {
+        // T3: (digit sort ->) line index -> fused smem kernel (scatter into smem lines, peak test, moments) -> compaction
+        const tpc_digit* src = digits;
+        if (sortfuse) {
+            NvtxRange nv("K5 first: digit sort (partition by pad line, rank by time)");
+            k += launch_sort_digits(h->geo, h->ws, digits, n, st);
+            src = h->ws.sort_tmp;
+        }
         int r;
         {
             NvtxRange nv("K0 K1 K2 K4: line index + fused kernel (clean, scatter, peaks, moments)");
-            r = launch_fused_sorted(h->geo, h->ws, digits, n, h->shape_n ? h->shape_n : h->shape_hint, params->q_peak_min, params->q_inner_gate, var, h->tun, st,
-                                    prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
+            r = launch_fused_sorted(h->geo, h->ws, src, n, h->shape_n ? h->shape_n : h->shape_hint, params->q_peak_min,
+                                    params->q_inner_gate, var, h->tun, sortfuse, st, prof ? ev[1] : nullptr, prof ? ev[2] : nullptr);
         }
         if (r < 0) return r;
         k += r;
         NvtxRange nv("K3 K5: scan + ordered copy + status");
-        k += launch_compact_lines(h->geo, h->ws, out->clusters, out->capacity, out->status, n, st);
+        k += launch_compact_lines(h->geo, h->ws, out->clusters, out->capacity, out->status, n, sortfuse ? 2u : 3u, st);
     } else {
         // T1: K1 scatter -> K2+K4 digit-centric peaks + moments on the HBM map -> K3 compaction -> (K5 key sort)
         //     -> K0 un-scatter

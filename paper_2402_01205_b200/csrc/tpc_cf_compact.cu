@@ -164,7 +164,7 @@ template <int LINES>      // lines per block: 256, or 64 for small geometries (a
 __global__ void __launch_bounds__(256)
 k_scan_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __restrict__ line_start, uint32_t n_lines,
                     const uint4* __restrict__ stage, uint4* __restrict__ out, uint64_t capacity,
-                    unsigned long long* line_desc, Counters* cnt, tpc_cf_status* status, uint64_t n)
+                    unsigned long long* line_desc, Counters* cnt, tpc_cf_status* status, uint64_t n, uint32_t path)
 {
     __shared__ uint32_t s_pref[LINES + 1];
     __shared__ uint32_t s_src[LINES];
@@ -216,7 +216,7 @@ k_scan_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __res
                 s.n_digits_used = n - cnt->n_bad;
                 s.n_bad_digits = cnt->n_bad;
                 s.overflow = s.n_clusters > capacity ? 1u : 0u;
-                s.path = 3u;
+                s.path = path;
                 if (cnt->unsorted) {      // false DIGITS_SORTED promise: detected, no output (include/tpc_cf.h)
                     s.n_clusters = 0;
                     s.overflow = 0;
@@ -240,18 +240,18 @@ k_scan_gather_lines(const uint32_t* __restrict__ line_cnt, const uint32_t* __res
 }
 
 int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, uint64_t capacity,
-                         tpc_cf_status* status, uint64_t n, cudaStream_t st)
+                         tpc_cf_status* status, uint64_t n, uint32_t path, cudaStream_t st)
 {
     const uint32_t n_lines = g.n_planes * g.LS;
     // (line_desc holds one descriptor per 64 lines: tpc_cf_api.cu carve, k_line_index)
     if (n_lines >= 64u * 148u * 16u)
         k_scan_gather_lines<256><<<(n_lines + 255) / 256, 256, 0, st>>>(ws.line_cnt, ws.line_start, n_lines,
                                                                         (const uint4*)ws.stage, (uint4*)out, capacity,
-                                                                        ws.line_desc, ws.counters, status, n);
+                                                                        ws.line_desc, ws.counters, status, n, path);
     else
         k_scan_gather_lines<64><<<(n_lines + 63) / 64, 256, 0, st>>>(ws.line_cnt, ws.line_start, n_lines,
                                                                      (const uint4*)ws.stage, (uint4*)out, capacity,
-                                                                     ws.line_desc, ws.counters, status, n);
+                                                                     ws.line_desc, ws.counters, status, n, path);
     return 1;
 }
 

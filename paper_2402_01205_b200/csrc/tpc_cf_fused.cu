@@ -485,8 +485,8 @@ cudaError_t fused_lines_set_attributes()
 }
 
 int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, cudaStream_t st,
-                        cudaEvent_t ev_k0, cudaEvent_t ev_k1)
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, bool have_index,
+                        cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1)
 {
     const uint32_t entries = g.n_planes * g.LS + 1;
     if (n == 0) {     // nothing to index: only the per-run state of the compaction (the caller zeroed the counters)
@@ -495,11 +495,13 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
         return 0;
     }
     int k = 0;
-    k_plane_index<<<(g.n_planes + 1 + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
-                                                                 ws.counters);
-    k_line_index<<<(entries + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
-                                                        ws.line_cnt, ws.line_desc);
-    k += 2;
+    if (!have_index) {
+        k_plane_index<<<(g.n_planes + 1 + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
+                                                                     ws.counters);
+        k_line_index<<<(entries + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
+                                                            ws.line_cnt, ws.line_desc);
+        k += 2;
+    }
 
     // Kernel choice.  Block-sparse line slots when the mean line fits their pool (k_fused_pairs, tpc_cf_pairs.cu; its
     // first generation k_fused_blocks, tpc_cf_blocks.cu, only on request), else the bitmap slots below.

@@ -48,6 +48,9 @@ struct Workspace {
     unsigned long long* line_desc;   // [n_lines / 256 + 1] per 256-line block: (flag << 62) | clusters, for the
                                      // single-pass scan of k_scan_gather_lines (fused path); zeroed by k_line_index
     tpc_cf_status* group_status;   // [32] per-group status blocks of the tpc_cf_run_host pipeline
+    tpc_digit* sort_tmp;  // [max_digits] digits sorted on the device (any-order input, tpc_cf_sort.cu); absent in sorted-only workspaces
+    uint32_t* sort_top;   // [1025] top-level bucket histogram / cursors of the digit sort
+    uint32_t* sort_part;  // scan partials of the digit sort
 };
 
 // Slot geometry of the block-sparse fused kernels (kernel parameter; all warp-uniform).
@@ -216,9 +219,13 @@ int launch_scatter_only(const Geo& g, const Workspace& ws, const tpc_digit* digi
 int launch_copy_plane(const Geo& g, const Workspace& ws, uint32_t plane, uint32_t P, uint16_t* dense,
                       cudaStream_t st);
 
+// have_index: ws.line_start already holds the line index and line_cnt / line_desc are zero (the digit sort left them so)
 int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, uint64_t shape_n,
-                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, cudaStream_t st,
-                        cudaEvent_t ev_k0, cudaEvent_t ev_k1);
+                        uint32_t q_peak_min, uint32_t q_gate, const Variant& var, const Tuning& tun, bool have_index,
+                        cudaStream_t st, cudaEvent_t ev_k0, cudaEvent_t ev_k1);
+// any-order input: digits -> ws.sort_tmp in (sector,row,pad,time) order + the line index (tpc_cf_sort.cu)
+int launch_sort_digits(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, cudaStream_t st);
+cudaError_t sort_set_attributes();
 
 // Block-sparse fused kernels after the line index is in ws.line_start.  Return 1 (launched), 0 (not applicable: the
 // caller runs another kernel) or a negative tpc_cf error.  must: no other kernel can take this geometry.
@@ -240,7 +247,7 @@ int launch_compact(const Workspace& ws, uint64_t n, tpc_cluster* out, uint64_t c
 // fused path, ONE kernel: single-pass scan of ws.line_cnt (decoupled look-back over blocks of 256 lines), copy
 // stage[line_start + k] -> out[offset + k], and the status block (written by the last block).
 int launch_compact_lines(const Geo& g, const Workspace& ws, tpc_cluster* out, uint64_t capacity,
-                         tpc_cf_status* status, uint64_t n, cudaStream_t st);
+                         tpc_cf_status* status, uint64_t n, uint32_t path, cudaStream_t st);
 int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_tiles, tpc_cluster* out,
                     uint64_t capacity, cudaStream_t st);
 int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,

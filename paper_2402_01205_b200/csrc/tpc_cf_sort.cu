@@ -1,0 +1,220 @@
+// tpc_cf_sort.cu — any digit order at the speed of the fused path: the digits are SORTED ON THE DEVICE into
+// (sector,row,pad,time) order, then the fused sorted path runs on the sorted copy (K5's "deterministic output ordering"
+// moved in front of the pipeline).  Measured before this file existed: a randomly ordered config-3 frame took 29.3 ms on
+// the general path (random 2-byte map writes: k_scatter / k_unscatter 9.8 ms each, k_peaks_map 6.7 ms, key sort of the
+// clusters 2.9 ms) against 1.85 ms for the sorted frame.
+//
+// The sort uses what the key is: a digit's key is (pad line, time); lines are few (755 k for the full geometry), times are
+// unique inside a line (R11: one digit per cell).  So: an UNSTABLE two-level partition of the digits by pad line (order
+// inside a line does not matter yet), then one warp per line ranks its digits by time with a bitmap (rank = set bits
+// below).  No comparison sort, no stable radix pass:
+//   k_sort_hist        digits -> 1024-bin histogram of the line index's top bits (+ invalid digits counted, R11)
+//   scan (1024)        -> cursors of the top-level buckets
+//   k_sort_scatter_top tile of 2048 digits: ranks inside the tile by shared-memory atomics, one global atomic per
+//                      (tile, bucket) reserves the range -> digits grouped by bucket in ws.sort_tmp
+//   k_sort_count_lines digits per pad line (no-return atomics; a bucket's 1024 counters are L2-resident)
+//   scan (n_lines + 1) -> line_start: THE LINE INDEX OF THE FUSED PATH (k_plane_index / k_line_index are not needed)
+//   k_sort_scatter_line digit -> its line's range (atomic cursor per line), into the cluster staging area (idle here)
+//   k_sort_rank_lines  one warp per line: time bitmap + rank directory in shared memory -> sorted digits in ws.sort_tmp
+// Invalid digits (R11: out-of-range sector / row / pad / time, zero charge) go to an overflow bin behind the last line:
+// counted, never seen by the fused kernel.  A duplicate cell shows up as a bit already set in a line's bitmap: reported
+// like a false DIGITS_SORTED promise (status.path = 0, no output) — on the general path it was "unspecified".
+// Definition: include/tpc_cf.h (R10, R12: exactly one correct output array, independent of the input order).
+#include "tpc_cf_internal.cuh"
+
+namespace tpccf {
+
+static constexpr int kSortThreads = 256;
+static constexpr int kSortPerThread = 8;
+static constexpr int kSortTileN = kSortThreads * kSortPerThread;     // digits per tile
+static constexpr uint32_t kSortTopBins = 1024;
+
+// line index of a digit in the fused path's table (plane * LS + pad), or n_lines for an invalid digit (R11)
+__device__ __forceinline__ uint32_t sort_line_of(const Geo& g, uint32_t w0, uint32_t w1, uint32_t n_lines)
+{
+    const uint32_t s = w0 & 0xffu, r = (w0 >> 8) & 0xffu, p = (w0 >> 16) & 0xffu;
+    return digit_valid(g, w0, w1) ? (s * g.n_rows + r) * g.LS + p : n_lines;
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+k_sort_hist(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t n_lines, uint32_t shift,
+            uint32_t* __restrict__ top_hist, Counters* cnt)
+{
+    __shared__ uint32_t s_h[kSortTopBins];
+    for (int i = threadIdx.x; i < (int)kSortTopBins; i += kSortThreads) s_h[i] = 0u;
+    __syncthreads();
+    uint32_t bad = 0u;
+    for (uint64_t i = (uint64_t)blockIdx.x * kSortThreads + threadIdx.x; i < n; i += (uint64_t)gridDim.x * kSortThreads) {
+        const uint2 d = __ldg(digits + i);
+        const uint32_t l = sort_line_of(g, d.x, d.y, n_lines);
+        bad += l == n_lines ? 1u : 0u;
+        atomicAdd(&s_h[l >> shift], 1u);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < (int)kSortTopBins; i += kSortThreads)
+        if (s_h[i]) atomicAdd(&top_hist[i], s_h[i]);
+    bad = __reduce_add_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&cnt->n_bad, (unsigned long long)bad);
+}
+
+// in -> out grouped by top-level bucket.  cursor[b] starts at the bucket's first position (exclusive scan of the
+// histogram) and is advanced by one atomic per (tile, bucket).
+__global__ void __launch_bounds__(kSortThreads)
+k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32_t n, Geo g, uint32_t n_lines,
+                   uint32_t shift, uint32_t* __restrict__ cursor)
+{
+    __shared__ uint32_t s_cnt[kSortTopBins];
+    __shared__ uint32_t s_base[kSortTopBins];
+    const uint32_t n_tiles = (n + kSortTileN - 1) / kSortTileN;
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        for (int i = threadIdx.x; i < (int)kSortTopBins; i += kSortThreads) s_cnt[i] = 0u;
+        __syncthreads();
+        uint2 d[kSortPerThread];
+        uint32_t bin[kSortPerThread], rk[kSortPerThread];
+        const uint64_t base = (uint64_t)tile * kSortTileN + threadIdx.x;
+#pragma unroll
+        for (int j = 0; j < kSortPerThread; ++j) {
+            const uint64_t i = base + (uint64_t)j * kSortThreads;
+            bin[j] = 0xffffffffu;
+            if (i < n) {
+                d[j] = __ldg(in + i);
+                bin[j] = sort_line_of(g, d[j].x, d[j].y, n_lines) >> shift;
+                rk[j] = atomicAdd(&s_cnt[bin[j]], 1u);
+            }
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < (int)kSortTopBins; i += kSortThreads)
+            if (s_cnt[i]) s_base[i] = atomicAdd(&cursor[i], s_cnt[i]);
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < kSortPerThread; ++j)
+            if (bin[j] != 0xffffffffu) out[s_base[bin[j]] + rk[j]] = d[j];
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+k_sort_count_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t n_lines, uint32_t* __restrict__ line_cnt)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * kSortThreads + threadIdx.x; i < n; i += (uint64_t)gridDim.x * kSortThreads) {
+        const uint2 d = __ldg(digits + i);
+        atomicAdd(&line_cnt[sort_line_of(g, d.x, d.y, n_lines)], 1u);
+    }
+}
+
+// cursor[l] starts at line_start[l]
+__global__ void __launch_bounds__(kSortThreads)
+k_sort_scatter_line(const uint2* __restrict__ in, uint2* __restrict__ out, uint32_t n, Geo g, uint32_t n_lines,
+                    uint32_t* __restrict__ cursor)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * kSortThreads + threadIdx.x; i < n; i += (uint64_t)gridDim.x * kSortThreads) {
+        const uint2 d = __ldg(in + i);
+        const uint32_t pos = atomicAdd(&cursor[sort_line_of(g, d.x, d.y, n_lines)], 1u);
+        out[pos] = d;
+    }
+}
+
+// One warp per pad line: the line's digits (any order) -> time order.  Shared memory per warp: a bitmap over the time
+// axis (bm, kept all-zero between lines: a line clears the words it set) and the number of set bits in front of every
+// bitmap word (pre).  rank(t) = pre[t / 32] + popc(bm[t / 32] below bit t): the digit's place in the sorted line.
+// A bit found already set is a duplicate cell (R11 contract violation): raised as Counters::unsorted.
+// The zeroing of line_cnt / line_desc for the fused kernels that follow rides along (line_cnt was the scatter cursor).
+__global__ void __launch_bounds__(kSortThreads)
+k_sort_rank_lines(const uint2* __restrict__ in, uint2* __restrict__ out, const uint32_t* __restrict__ line_start,
+                  uint32_t n_lines, uint32_t n_time, uint32_t words, uint32_t* __restrict__ line_cnt,
+                  unsigned long long* __restrict__ line_desc, Counters* cnt)
+{
+    extern __shared__ __align__(16) uint32_t s_sort[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = kSortThreads / 32;
+    uint32_t* bm = s_sort + (size_t)warp * (words + (words + 1) / 2);
+    uint16_t* pre = (uint16_t*)(bm + words);
+    for (uint32_t w = lane; w < words; w += 32) bm[w] = 0u;
+    __syncwarp();
+    const uint32_t total_warps = gridDim.x * nwarp;
+    uint32_t dup = 0u;
+    for (uint32_t l = blockIdx.x * nwarp + warp; l < n_lines; l += total_warps) {
+        const uint32_t ls = line_start[l], len = line_start[l + 1] - ls;
+        if (lane == 0) line_cnt[l] = 0u;
+        if (lane == 1 && (l & 63u) == 0u) line_desc[l >> 6] = 0ull;
+        if (len == 0u) continue;
+        if (len == 1u) { if (lane == 0) out[ls] = in[ls]; continue; }
+        uint32_t wlo = 0xffffffffu, whi = 0u;               // words this line touches
+        for (uint32_t i = lane; i < len; i += 32) {
+            const uint32_t t = __ldg(&in[ls + i].y) & 0xffffu;   // (valid digits only: t < n_time)
+            const uint32_t old = atomicOr(&bm[t >> 5], 1u << (t & 31u));
+            dup |= (old >> (t & 31u)) & 1u;
+            wlo = min(wlo, t >> 5); whi = max(whi, t >> 5);
+        }
+        wlo = __reduce_min_sync(0xffffffffu, wlo);
+        whi = __reduce_max_sync(0xffffffffu, whi);
+        __syncwarp();
+        // set bits in front of every word of [wlo, whi]: every lane takes a contiguous run of words
+        const uint32_t span = whi - wlo + 1u, per = (span + 31u) / 32u;
+        const uint32_t w0 = wlo + (uint32_t)lane * per, w1 = min(w0 + per, whi + 1u);
+        uint32_t mine = 0u;
+        for (uint32_t w = w0; w < w1; ++w) mine += (uint32_t)__popc(bm[w]);
+        uint32_t inc = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t up = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += up;
+        }
+        uint32_t run = inc - mine;
+        for (uint32_t w = w0; w < w1; ++w) { pre[w] = (uint16_t)run; run += (uint32_t)__popc(bm[w]); }
+        __syncwarp();
+        for (uint32_t i = lane; i < len; i += 32) {
+            const uint2 d = __ldg(in + ls + i);
+            const uint32_t t = d.y & 0xffffu;
+            const uint32_t rank = (uint32_t)pre[t >> 5] + (uint32_t)__popc(bm[t >> 5] & ((1u << (t & 31u)) - 1u));
+            out[ls + min(rank, len - 1u)] = d;              // (min: stays inside the line if a duplicate broke the ranks)
+        }
+        __syncwarp();
+        for (uint32_t w = w0; w < w1; ++w) bm[w] = 0u;
+        __syncwarp();
+    }
+    if (lane == 0 && blockIdx.x == 0 && warp == 0) { line_cnt[n_lines] = 0u; line_desc[(n_lines >> 6) + 1u] = 0ull; }
+    if (__any_sync(0xffffffffu, dup != 0u) && lane == 0) atomicOr(&cnt->unsorted, 1u);
+}
+
+static uint32_t sort_rank_smem(const Geo& g, uint32_t* words_out)
+{
+    const uint32_t words = ((g.n_time + 31u) / 32u + 3u) & ~3u;
+    *words_out = words;
+    return (kSortThreads / 32) * (words + (words + 1) / 2) * 4u;
+}
+
+cudaError_t sort_set_attributes()
+{
+    return cudaFuncSetAttribute(k_sort_rank_lines, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+}
+
+// Sorts `n` digits into ws.sort_tmp and leaves the fused path's line index in ws.line_start (and line_cnt / line_desc
+// zeroed).  The counters must have been zeroed on the stream before.  Returns the number of launches.
+int launch_sort_digits(const Geo& g, const Workspace& ws, const tpc_digit* digits, uint64_t n, cudaStream_t st)
+{
+    const uint32_t n_lines = g.n_planes * g.LS;
+    uint32_t shift = 0;
+    while (((n_lines + 1u) >> shift) >= kSortTopBins) ++shift;      // top-level bucket = line >> shift, < 1024 buckets
+    const uint2* in = (const uint2*)digits;
+    uint2* tmp = (uint2*)ws.sort_tmp;
+    uint2* tmp2 = (uint2*)ws.stage;                                 // the cluster staging area is idle until the fused kernel
+    const int grid = 148 * 8;
+    int k = 0;
+    cudaMemsetAsync(ws.sort_top, 0, (kSortTopBins + 1) * 4, st);
+    cudaMemsetAsync(ws.line_cnt, 0, ((size_t)n_lines + 2) * 4, st);
+    k_sort_hist<<<grid, kSortThreads, 0, st>>>(in, (uint32_t)n, g, n_lines, shift, ws.sort_top, ws.counters);
+    k += 1 + launch_scan_u32(ws.sort_top, ws.sort_top, kSortTopBins + 1, ws.sort_part, nullptr, st);
+    k_sort_scatter_top<<<grid, kSortThreads, 0, st>>>(in, tmp, (uint32_t)n, g, n_lines, shift, ws.sort_top);
+    k_sort_count_lines<<<grid, kSortThreads, 0, st>>>(tmp, (uint32_t)n, g, n_lines, ws.line_cnt);
+    k += 2 + launch_scan_u32(ws.line_cnt, ws.line_start, (uint64_t)n_lines + 1, ws.sort_part, nullptr, st);
+    // the fused kernels read line_start[n_lines] as the end of the last plane: the overflow bin (invalid digits) starts there
+    cudaMemcpyAsync(ws.line_cnt, ws.line_start, ((size_t)n_lines + 1) * 4, cudaMemcpyDeviceToDevice, st);
+    k_sort_scatter_line<<<grid, kSortThreads, 0, st>>>(tmp, tmp2, (uint32_t)n, g, n_lines, ws.line_cnt);
+    uint32_t words;
+    const uint32_t smem = sort_rank_smem(g, &words);
+    k_sort_rank_lines<<<grid, kSortThreads, smem, st>>>(tmp2, tmp, ws.line_start, n_lines, g.n_time, words, ws.line_cnt,
+                                                        ws.line_desc, ws.counters);
+    return k + 2;
+}
+
+}  // namespace tpccf

@@ -40,8 +40,11 @@ def parse_golden(path=GOLDEN):
 # "fused_pairs" / "fused_blocks" / "fused_lines" force one of the three fused kernels (tpc_cf_debug_set), so that each
 # runs every case — including the ones far outside its range, which exercise its exact slow paths.
 # "*_p3" additionally covers the time axis in 3 passes, the shape long lines get.
-PATHS = {"general": 0, "general_hint": 3, "fused": 1, "fused_pairs": 1, "fused_pairs_p3": 1, "fused_blocks": 1,
-         "fused_blocks_p3": 1, "fused_lines": 1}
+# "sorted_on_device": no promise, no FORCE_GENERAL: the library sorts the digits on the device and runs the fused path
+# (status.path 2); "general": FORCE_GENERAL without the hint (map in HBM + key sort of the clusters).
+PATHS = {"general": 2, "general_hint": 3, "sorted_on_device": 0, "fused": 1, "fused_pairs": 1, "fused_pairs_p3": 1,
+         "fused_blocks": 1, "fused_blocks_p3": 1, "fused_lines": 1}
+EXPECT_PATH = {"general": 1, "general_hint": 1, "sorted_on_device": 2}
 TUNING = {"fused_pairs": dict(fused_kernel="pairs"), "fused_pairs_p3": dict(fused_kernel="pairs", passes=3),
           "fused_blocks": dict(fused_kernel="blocks"), "fused_blocks_p3": dict(fused_kernel="blocks", passes=3),
           "fused_lines": dict(fused_kernel="lines")}
@@ -102,7 +105,7 @@ def test_worked_examples(path):
     ora, ost = orc.run(digits, *geom[:4])
     cl, st = gpu_run(digits, geom, PATHS[path])
     assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == 0 and st["overflow"] == 0
-    assert st["path"] == (3 if path.startswith("fused") else 1)
+    assert st["path"] == EXPECT_PATH.get(path, 3)
     assert_clusters_equal(cl, ora, "worked examples/" + path)
 
 
@@ -133,17 +136,19 @@ def test_config_full_parity(cfg, path):
     assert_clusters_equal(cl, ora, "config %d/%s" % (cfg, path))
 
 
+@pytest.mark.parametrize("route", ["sorted_on_device", "general"])
 @pytest.mark.parametrize("cfg", [1, 2])
-def test_shuffled_input_general(cfg):
-    """Any-order contract (R12, I1): a random permutation of the digits gives the identical output array."""
+def test_shuffled_input_general(cfg, route):
+    """Any-order contract (R12, I1): a random permutation of the digits gives the identical output array — by the
+    digit sort + fused path (the default for input without the promise) and by the general path (FORCE_GENERAL)."""
     digits = gen.generate(cfg)
     geom = gen.geometry(cfg)
     ora, ost = orc.run(digits, *geom[:4])
     rng = np.random.default_rng(100 + cfg)
     sh = digits[rng.permutation(digits.shape[0])]
-    cl, st = gpu_run(sh, geom, 0, max_clusters=ost["n_clusters"] + 16)
-    assert st["path"] == 1 and st["n_clusters"] == ost["n_clusters"]
-    assert_clusters_equal(cl, ora, "config %d shuffled" % cfg)
+    cl, st = gpu_run(sh, geom, PATHS[route], max_clusters=ost["n_clusters"] + 16)
+    assert st["path"] == EXPECT_PATH[route] and st["n_clusters"] == ost["n_clusters"]
+    assert_clusters_equal(cl, ora, "config %d shuffled/%s" % (cfg, route))
 
 
 @pytest.mark.parametrize("flags", [1, 3])
@@ -164,7 +169,7 @@ def test_run_host_retries_on_false_promise():
     sh = digits[np.random.default_rng(8).permutation(digits.shape[0])]
     f = cf.ClusterFinder(*geom[:4], max_digits=digits.shape[0], max_clusters=ora.shape[0] + 8)
     cl, st = f.run_host(sh, flags=cf.DIGITS_SORTED)
-    assert st["path"] == 1
+    assert st["path"] == 2                                   # rerun without the promise: digit sort + fused path
     assert_clusters_equal(cl.copy(), ora, "run_host retry")
     cl, st = f.run_host(digits, flags=cf.DIGITS_SORTED)
     assert st["path"] == 3
@@ -399,7 +404,7 @@ def test_run_host_pipelined_over_sector_groups():
     i, j = 12345, n - 54321
     sw[[i, j]] = sw[[j, i]]
     cl2, st2 = f.run_host(sw, flags=cf.DIGITS_SORTED)
-    assert st2["path"] == 1 and st2["n_clusters"] == rst["n_clusters"]
+    assert st2["path"] == 2 and st2["n_clusters"] == rst["n_clusters"]
     assert np.array_equal(cl2.view(np.uint8), ref.view(np.uint8))
     f.close()
     # capacity that holds the frame but not a proportional share per group is still honoured
@@ -549,7 +554,7 @@ def test_config5_full_four_frames_every_plane():
     assert total > 7_000_000
 
 
-@pytest.mark.parametrize("path", ["fused_pairs", "fused_blocks", "fused_lines", "general"])
+@pytest.mark.parametrize("path", ["fused_pairs", "fused_blocks", "fused_lines", "general", "sorted_on_device"])
 @pytest.mark.parametrize("odd_n", [0, 1])
 def test_digit_buffer_eight_bytes_off_a_16_byte_boundary(path, odd_n):
     """The ABI asks for 8-byte aligned digits only: a buffer that starts 8 bytes off a 16-byte boundary (and one whose
@@ -617,7 +622,7 @@ def test_unsorted_input_more_peaks_than_the_workspace_holds():
     mc = 1000
     f = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=mc)
     big = torch.zeros(ost["n_clusters"] * 32 + 64, dtype=torch.uint8, device="cuda:0")
-    f.run(cf.to_device(sh), n, flags=0, clusters=big, capacity=ost["n_clusters"] + 2)
+    f.run(cf.to_device(sh), n, flags=cf.FORCE_GENERAL, clusters=big, capacity=ost["n_clusters"] + 2)
     cl, st = f.result(clusters=big)
     assert st["path"] == 1 and st["n_clusters"] == ost["n_clusters"] and st["overflow"] == 1
     # the kept subset: peaks of the first digits (in the shuffled order) that are peaks, mc of them, sorted
@@ -652,3 +657,42 @@ def test_sorted_only_workspace():
             lean.run(d, n, flags=flags)
         assert e.value.code == -5
     lean.close()
+
+
+@pytest.mark.parametrize("route", ["sorted_on_device", "general"])
+def test_shuffled_full_frame_config3(route):
+    """Any-order contract at full size: the whole 36-sector config-3 frame in a random order, no
+    DIGITS_SORTED promise: the identical array (R12), every cluster against the oracle — digit sort + fused path, and
+    the general path + key sort of the clusters."""
+    import torch
+    cf = _cf()
+    geom = gen.geometry(3)
+    digits = gen.generate(3)
+    n = digits.shape[0]
+    ora, ost, _ = orc.run_parallel(digits, *geom[:4])
+    f = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=ost["n_clusters"] + 1024)
+    d = cf.to_device(digits)
+    g = torch.Generator(device="cuda:0")
+    g.manual_seed(3)
+    sh = d.view(torch.int64)[torch.randperm(n, device="cuda:0", generator=g)].contiguous().view(torch.uint8)
+    del d
+    f.run(sh, n, flags=PATHS[route])
+    cl, st = f.result()
+    assert st["path"] == EXPECT_PATH[route] and st["overflow"] == 0 and st["n_clusters"] == ost["n_clusters"]
+    assert st["n_bad_digits"] == 0 and st["n_digits_used"] == n
+    assert_clusters_equal(cl, ora, "config 3 shuffled/" + route)
+    f.close()
+
+
+def test_duplicate_cell_in_unsorted_input_is_reported():
+    """Two digits on the same cell are a contract violation (R11).  On input without the DIGITS_SORTED promise the digit
+    sort sees the cell's bit already set in the line's time bitmap: the run reports path 0 and no output, exactly like a
+    false promise (on the general path the result for that cell stays unspecified, but nothing crashes)."""
+    digits = gen.generate(1)
+    geom = gen.geometry(1)
+    dup = np.concatenate([digits, digits[1234:1235]])
+    dup = dup[np.random.default_rng(9).permutation(dup.shape[0])]
+    cl, st = gpu_run(dup, geom, PATHS["sorted_on_device"])
+    assert st["path"] == 0 and st["n_clusters"] == 0
+    cl, st = gpu_run(dup, geom, PATHS["general"])
+    assert st["path"] == 1 and st["n_clusters"] > 3000
