@@ -8,13 +8,15 @@
 // unique inside a line (R11: one digit per cell).  So: an UNSTABLE two-level partition of the digits by pad line (order
 // inside a line does not matter yet), then one warp per line ranks its digits by time with a bitmap (rank = set bits
 // below).  No comparison sort, no stable radix pass:
-//   k_sort_hist        digits -> 1024-bin histogram of the line index's top bits (+ invalid digits counted, R11)
-//   scan (1024)        -> cursors of the top-level buckets
-//   k_sort_scatter_top tile of 2048 digits: ranks inside the tile by shared-memory atomics, one global atomic per
-//                      (tile, bucket) reserves the range -> digits grouped by bucket in ws.sort_tmp
+//   k_sort_hist        per block (a contiguous digit range): 1024-bin histogram of the line index's top bits -> table
+//                      (+ invalid digits counted, R11)
+//   scan (table)       -> where each block's digits of each top-level bucket go: no atomics, deterministic
+//   k_sort_scatter_top tile of 2048 digits: ranks inside the tile by shared-memory atomics, block-private cursors ->
+//                      digits grouped by bucket in ws.sort_tmp
 //   k_sort_count_lines digits per pad line (no-return atomics; a bucket's 1024 counters are L2-resident)
 //   scan (n_lines + 1) -> line_start: THE LINE INDEX OF THE FUSED PATH (k_plane_index / k_line_index are not needed)
-//   k_sort_scatter_line digit -> its line's range (atomic cursor per line), into the cluster staging area (idle here)
+//   k_sort_scatter_line tile of 8192 digits (few buckets): ranks per line in shared memory, one global atomic per
+//                      (tile, line) -> digits grouped by line in the cluster staging area (idle here)
 //   k_sort_rank_lines  one warp per line: time bitmap + rank directory in shared memory -> sorted digits in ws.sort_tmp
 // Invalid digits (R11: out-of-range sector / row / pad / time, zero charge) go to an overflow bin behind the last line:
 // counted, never seen by the fused kernel.  A duplicate cell shows up as a bit already set in a line's bitmap: reported
@@ -26,7 +28,6 @@ namespace tpccf {
 
 static constexpr int kSortThreads = 256;
 static constexpr int kSortPerThread = 8;
-static constexpr int kSortTileN = kSortThreads * kSortPerThread;     // digits per tile
 static constexpr uint32_t kSortTopBins = 1024;
 
 // line index of a digit in the fused path's table (plane * LS + pad), or n_lines for an invalid digit (R11)
@@ -36,59 +37,111 @@ __device__ __forceinline__ uint32_t sort_line_of(const Geo& g, uint32_t w0, uint
     return digit_valid(g, w0, w1) ? (s * g.n_rows + r) * g.LS + p : n_lines;
 }
 
-__global__ void __launch_bounds__(kSortThreads)
-k_sort_hist(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t n_lines, uint32_t shift,
-            uint32_t* __restrict__ top_hist, Counters* cnt)
+static constexpr int kTopThreads = 1024;                             // top-level pass: tiles of 8192 digits, so that a
+static constexpr int kTopTileN = kTopThreads * kSortPerThread;       //   (tile, bucket) run is ~11 digits, not ~3
+static constexpr int kSortBlocks = 148 * 2;                          // persistent blocks of the top-level pass
+static constexpr int kLineThreads = 1024;                            // line-level scatter: tiles of 8192 digits
+static constexpr int kLineTileN = kLineThreads * kSortPerThread;
+static constexpr uint32_t kLineBins = 4096;                          // lines a tile may span for the aggregated path
+
+// Top level, deterministic and without global atomics: block b owns the contiguous digit range [b * chunk, (b + 1) *
+// chunk); k_sort_hist writes its bucket counts to table[bucket * kSortBlocks + b]; an exclusive scan of the table (bucket
+// major) turns the entry into the position where block b's digits of that bucket start; k_sort_scatter_top keeps the 1024
+// cursors of its block in shared memory and advances them tile by tile.
+__global__ void __launch_bounds__(kTopThreads)
+k_sort_hist(const uint2* __restrict__ digits, uint32_t n, uint32_t chunk, Geo g, uint32_t n_lines, uint32_t shift,
+            uint32_t* __restrict__ table, Counters* cnt)
 {
     __shared__ uint32_t s_h[kSortTopBins];
-    for (int i = threadIdx.x; i < (int)kSortTopBins; i += kSortThreads) s_h[i] = 0u;
+    for (int i = threadIdx.x; i < (int)kSortTopBins; i += kTopThreads) s_h[i] = 0u;
     __syncthreads();
     uint32_t bad = 0u;
-    for (uint64_t i = (uint64_t)blockIdx.x * kSortThreads + threadIdx.x; i < n; i += (uint64_t)gridDim.x * kSortThreads) {
+    const uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
+    for (uint64_t i = lo + threadIdx.x; i < hi; i += kTopThreads) {
         const uint2 d = __ldg(digits + i);
         const uint32_t l = sort_line_of(g, d.x, d.y, n_lines);
         bad += l == n_lines ? 1u : 0u;
         atomicAdd(&s_h[l >> shift], 1u);
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < (int)kSortTopBins; i += kSortThreads)
-        if (s_h[i]) atomicAdd(&top_hist[i], s_h[i]);
+    for (int i = threadIdx.x; i < (int)kSortTopBins; i += kTopThreads) table[(size_t)i * kSortBlocks + blockIdx.x] = s_h[i];
     bad = __reduce_add_sync(0xffffffffu, bad);
     if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&cnt->n_bad, (unsigned long long)bad);
 }
 
-// in -> out grouped by top-level bucket.  cursor[b] starts at the bucket's first position (exclusive scan of the
-// histogram) and is advanced by one atomic per (tile, bucket).
-__global__ void __launch_bounds__(kSortThreads)
-k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32_t n, Geo g, uint32_t n_lines,
-                   uint32_t shift, uint32_t* __restrict__ cursor)
+// The tile is first brought into bucket order in shared memory (ranks by shared-memory atomics, bucket offsets by a block
+// scan), then written out in that order: neighbouring lanes write neighbouring addresses of a bucket's run, so a warp's
+// store covers a few 32-byte sectors instead of 32 (ncu: 216 M store sectors for 220 M digits without the staging).
+__global__ void __launch_bounds__(kTopThreads)
+k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32_t n, uint32_t chunk, Geo g,
+                   uint32_t n_lines, uint32_t shift, const uint32_t* __restrict__ table)
 {
-    __shared__ uint32_t s_cnt[kSortTopBins];
-    __shared__ uint32_t s_base[kSortTopBins];
-    const uint32_t n_tiles = (n + kSortTileN - 1) / kSortTileN;
-    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        for (int i = threadIdx.x; i < (int)kSortTopBins; i += kSortThreads) s_cnt[i] = 0u;
-        __syncthreads();
+    extern __shared__ __align__(16) uint2 s_tile[];              // kTopTileN digits in bucket order
+    __shared__ uint32_t s_cnt[kSortTopBins];                     // digits of the tile per bucket
+    __shared__ uint32_t s_off[kSortTopBins];                     // first position of the bucket inside the tile
+    __shared__ uint32_t s_cur[kSortTopBins];                     // output position of the bucket's next digit (this block)
+    __shared__ uint32_t s_warp[32];
+    static_assert(kTopThreads == (int)kSortTopBins, "one thread per bucket in the block scan");
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    s_cur[tid] = table[(size_t)tid * kSortBlocks + blockIdx.x];
+    s_cnt[tid] = 0u;
+    __syncthreads();
+    const uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
+    for (uint64_t t0 = lo; t0 < hi; t0 += kTopTileN) {
+        const uint32_t m = (uint32_t)min((uint64_t)kTopTileN, hi - t0);     // digits in this tile
         uint2 d[kSortPerThread];
         uint32_t bin[kSortPerThread], rk[kSortPerThread];
-        const uint64_t base = (uint64_t)tile * kSortTileN + threadIdx.x;
 #pragma unroll
         for (int j = 0; j < kSortPerThread; ++j) {
-            const uint64_t i = base + (uint64_t)j * kSortThreads;
+            const uint32_t i = (uint32_t)j * kTopThreads + tid;
             bin[j] = 0xffffffffu;
-            if (i < n) {
-                d[j] = __ldg(in + i);
+            if (i < m) {
+                d[j] = __ldg(in + t0 + i);
                 bin[j] = sort_line_of(g, d[j].x, d[j].y, n_lines) >> shift;
                 rk[j] = atomicAdd(&s_cnt[bin[j]], 1u);
             }
         }
         __syncthreads();
-        for (int i = threadIdx.x; i < (int)kSortTopBins; i += kSortThreads)
-            if (s_cnt[i]) s_base[i] = atomicAdd(&cursor[i], s_cnt[i]);
+        {   // exclusive scan of the 1024 bucket counts, one per thread
+            const uint32_t c = s_cnt[tid];
+            uint32_t inc = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t up = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += up;
+            }
+            if (lane == 31) s_warp[warp] = inc;
+            __syncthreads();
+            if (warp == 0) {
+                const uint32_t w = s_warp[lane];
+                uint32_t winc = w;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t up = __shfl_up_sync(0xffffffffu, winc, o);
+                    if (lane >= o) winc += up;
+                }
+                s_warp[lane] = winc - w;
+            }
+            __syncthreads();
+            s_off[tid] = s_warp[warp] + inc - c;
+        }
         __syncthreads();
 #pragma unroll
         for (int j = 0; j < kSortPerThread; ++j)
-            if (bin[j] != 0xffffffffu) out[s_base[bin[j]] + rk[j]] = d[j];
+            if (bin[j] != 0xffffffffu) s_tile[s_off[bin[j]] + rk[j]] = d[j];
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < kSortPerThread; ++j) {
+            const uint32_t i = (uint32_t)j * kTopThreads + tid;
+            if (i < m) {
+                const uint2 e = s_tile[i];
+                const uint32_t b2 = sort_line_of(g, e.x, e.y, n_lines) >> shift;
+                out[s_cur[b2] + (i - s_off[b2])] = e;
+            }
+        }
+        __syncthreads();
+        s_cur[tid] += s_cnt[tid];
+        s_cnt[tid] = 0u;
         __syncthreads();
     }
 }
@@ -102,15 +155,55 @@ k_sort_count_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t
     }
 }
 
-// cursor[l] starts at line_start[l]
-__global__ void __launch_bounds__(kSortThreads)
+// Line level: cursor[l] starts at line_start[l].  The input is grouped by top-level bucket, so a tile of 8192 digits spans
+// few buckets: its digits are ranked per line in shared memory and ONE global atomic per (tile, line) reserves the range
+// (a tile spanning more than kLineBins lines — sparse data — takes one atomic per digit instead).
+__global__ void __launch_bounds__(kLineThreads)
 k_sort_scatter_line(const uint2* __restrict__ in, uint2* __restrict__ out, uint32_t n, Geo g, uint32_t n_lines,
-                    uint32_t* __restrict__ cursor)
+                    uint32_t shift, uint32_t* __restrict__ cursor)
 {
-    for (uint64_t i = (uint64_t)blockIdx.x * kSortThreads + threadIdx.x; i < n; i += (uint64_t)gridDim.x * kSortThreads) {
-        const uint2 d = __ldg(in + i);
-        const uint32_t pos = atomicAdd(&cursor[sort_line_of(g, d.x, d.y, n_lines)], 1u);
-        out[pos] = d;
+    __shared__ uint32_t s_cnt[kLineBins];
+    __shared__ uint32_t s_base[kLineBins];
+    __shared__ uint32_t s_l0, s_l1;
+    const uint32_t n_tiles = (uint32_t)(((uint64_t)n + kLineTileN - 1) / kLineTileN);
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const uint64_t t0 = (uint64_t)tile * kLineTileN, t1 = min((uint64_t)n, t0 + kLineTileN);
+        if (threadIdx.x == 0) {
+            const uint2 a = __ldg(in + t0), z = __ldg(in + (t1 - 1));
+            s_l0 = (sort_line_of(g, a.x, a.y, n_lines) >> shift) << shift;
+            s_l1 = min(n_lines + 1u, ((sort_line_of(g, z.x, z.y, n_lines) >> shift) + 1u) << shift);
+        }
+        __syncthreads();
+        const uint32_t l0 = s_l0, span = s_l1 - l0;
+        if (span <= kLineBins) {
+            for (uint32_t i = threadIdx.x; i < span; i += kLineThreads) s_cnt[i] = 0u;
+            __syncthreads();
+            uint2 d[kSortPerThread];
+            uint32_t bin[kSortPerThread], rk[kSortPerThread];
+#pragma unroll
+            for (int j = 0; j < kSortPerThread; ++j) {
+                const uint64_t i = t0 + (uint64_t)j * kLineThreads + threadIdx.x;
+                bin[j] = 0xffffffffu;
+                if (i < t1) {
+                    d[j] = __ldg(in + i);
+                    bin[j] = sort_line_of(g, d[j].x, d[j].y, n_lines) - l0;
+                    rk[j] = atomicAdd(&s_cnt[bin[j]], 1u);
+                }
+            }
+            __syncthreads();
+            for (uint32_t i = threadIdx.x; i < span; i += kLineThreads)
+                if (s_cnt[i]) s_base[i] = atomicAdd(&cursor[l0 + i], s_cnt[i]);
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < kSortPerThread; ++j)
+                if (bin[j] != 0xffffffffu) out[s_base[bin[j]] + rk[j]] = d[j];
+        } else {
+            for (uint64_t i = t0 + threadIdx.x; i < t1; i += kLineThreads) {
+                const uint2 d = __ldg(in + i);
+                out[atomicAdd(&cursor[sort_line_of(g, d.x, d.y, n_lines)], 1u)] = d;
+            }
+        }
+        __syncthreads();
     }
 }
 
@@ -185,6 +278,8 @@ static uint32_t sort_rank_smem(const Geo& g, uint32_t* words_out)
 
 cudaError_t sort_set_attributes()
 {
+    cudaError_t e = cudaFuncSetAttribute(k_sort_scatter_top, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kTopTileN * sizeof(uint2)));
+    if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(k_sort_rank_lines, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
 }
 
@@ -200,16 +295,18 @@ int launch_sort_digits(const Geo& g, const Workspace& ws, const tpc_digit* digit
     uint2* tmp2 = (uint2*)ws.stage;                                 // the cluster staging area is idle until the fused kernel
     const int grid = 148 * 8;
     int k = 0;
-    cudaMemsetAsync(ws.sort_top, 0, (kSortTopBins + 1) * 4, st);
+    // top level: contiguous range per block, a multiple of the tile
+    const uint32_t chunk = (uint32_t)(ceil_div_u64(ceil_div_u64(n, kSortBlocks), kTopTileN) * kTopTileN);
+    const uint64_t table_n = (uint64_t)kSortTopBins * kSortBlocks;
     cudaMemsetAsync(ws.line_cnt, 0, ((size_t)n_lines + 2) * 4, st);
-    k_sort_hist<<<grid, kSortThreads, 0, st>>>(in, (uint32_t)n, g, n_lines, shift, ws.sort_top, ws.counters);
-    k += 1 + launch_scan_u32(ws.sort_top, ws.sort_top, kSortTopBins + 1, ws.sort_part, nullptr, st);
-    k_sort_scatter_top<<<grid, kSortThreads, 0, st>>>(in, tmp, (uint32_t)n, g, n_lines, shift, ws.sort_top);
+    k_sort_hist<<<kSortBlocks, kTopThreads, 0, st>>>(in, (uint32_t)n, chunk, g, n_lines, shift, ws.sort_top, ws.counters);
+    k += 1 + launch_scan_u32(ws.sort_top, ws.sort_top, table_n, ws.sort_part, nullptr, st);
+    k_sort_scatter_top<<<kSortBlocks, kTopThreads, kTopTileN * sizeof(uint2), st>>>(in, tmp, (uint32_t)n, chunk, g, n_lines, shift, ws.sort_top);
     k_sort_count_lines<<<grid, kSortThreads, 0, st>>>(tmp, (uint32_t)n, g, n_lines, ws.line_cnt);
     k += 2 + launch_scan_u32(ws.line_cnt, ws.line_start, (uint64_t)n_lines + 1, ws.sort_part, nullptr, st);
     // the fused kernels read line_start[n_lines] as the end of the last plane: the overflow bin (invalid digits) starts there
     cudaMemcpyAsync(ws.line_cnt, ws.line_start, ((size_t)n_lines + 1) * 4, cudaMemcpyDeviceToDevice, st);
-    k_sort_scatter_line<<<grid, kSortThreads, 0, st>>>(tmp, tmp2, (uint32_t)n, g, n_lines, ws.line_cnt);
+    k_sort_scatter_line<<<148 * 2, kLineThreads, 0, st>>>(tmp, tmp2, (uint32_t)n, g, n_lines, shift, ws.line_cnt);
     uint32_t words;
     const uint32_t smem = sort_rank_smem(g, &words);
     k_sort_rank_lines<<<grid, kSortThreads, smem, st>>>(tmp2, tmp, ws.line_start, n_lines, g.n_time, words, ws.line_cnt,
