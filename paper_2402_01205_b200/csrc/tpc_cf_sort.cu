@@ -162,13 +162,20 @@ __global__ void __launch_bounds__(kLineThreads)
 k_sort_scatter_line(const uint2* __restrict__ in, uint2* __restrict__ out, uint32_t n, Geo g, uint32_t n_lines,
                     uint32_t shift, uint32_t* __restrict__ cursor)
 {
-    __shared__ uint32_t s_cnt[kLineBins];
-    __shared__ uint32_t s_base[kLineBins];
+    extern __shared__ __align__(16) uint2 s_dyn[];
+    uint2* s_tile = s_dyn;                                        // kLineTileN digits in line order
+    uint32_t* s_cnt = (uint32_t*)(s_dyn + kLineTileN);            // [kLineBins] digits of the tile per line
+    uint32_t* s_off = s_cnt + kLineBins;                          // first position of the line inside the tile
+    uint32_t* s_base = s_off + kLineBins;                         // output position of the line's run (global atomic)
+    __shared__ uint32_t s_warp[32];
     __shared__ uint32_t s_l0, s_l1;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr uint32_t kPer = kLineBins / kLineThreads;           // bins per thread in the block scan
     const uint32_t n_tiles = (uint32_t)(((uint64_t)n + kLineTileN - 1) / kLineTileN);
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const uint64_t t0 = (uint64_t)tile * kLineTileN, t1 = min((uint64_t)n, t0 + kLineTileN);
-        if (threadIdx.x == 0) {
+        const uint32_t m = (uint32_t)(t1 - t0);
+        if (tid == 0) {
             const uint2 a = __ldg(in + t0), z = __ldg(in + (t1 - 1));
             s_l0 = (sort_line_of(g, a.x, a.y, n_lines) >> shift) << shift;
             s_l1 = min(n_lines + 1u, ((sort_line_of(g, z.x, z.y, n_lines) >> shift) + 1u) << shift);
@@ -176,29 +183,69 @@ k_sort_scatter_line(const uint2* __restrict__ in, uint2* __restrict__ out, uint3
         __syncthreads();
         const uint32_t l0 = s_l0, span = s_l1 - l0;
         if (span <= kLineBins) {
-            for (uint32_t i = threadIdx.x; i < span; i += kLineThreads) s_cnt[i] = 0u;
+            for (uint32_t i = tid; i < kLineBins; i += kLineThreads) s_cnt[i] = 0u;
             __syncthreads();
             uint2 d[kSortPerThread];
             uint32_t bin[kSortPerThread], rk[kSortPerThread];
 #pragma unroll
             for (int j = 0; j < kSortPerThread; ++j) {
-                const uint64_t i = t0 + (uint64_t)j * kLineThreads + threadIdx.x;
+                const uint32_t i = (uint32_t)j * kLineThreads + tid;
                 bin[j] = 0xffffffffu;
-                if (i < t1) {
-                    d[j] = __ldg(in + i);
+                if (i < m) {
+                    d[j] = __ldg(in + t0 + i);
                     bin[j] = sort_line_of(g, d[j].x, d[j].y, n_lines) - l0;
                     rk[j] = atomicAdd(&s_cnt[bin[j]], 1u);
                 }
             }
             __syncthreads();
-            for (uint32_t i = threadIdx.x; i < span; i += kLineThreads)
-                if (s_cnt[i]) s_base[i] = atomicAdd(&cursor[l0 + i], s_cnt[i]);
+            {   // exclusive scan of the line counts (kPer consecutive bins per thread) + the runs' output positions
+                uint32_t c[kPer], sum = 0u;
+#pragma unroll
+                for (uint32_t q = 0; q < kPer; ++q) { c[q] = s_cnt[tid * kPer + q]; sum += c[q]; }
+                uint32_t inc = sum;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t up = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += up;
+                }
+                if (lane == 31) s_warp[warp] = inc;
+                __syncthreads();
+                if (warp == 0) {
+                    const uint32_t w = s_warp[lane];
+                    uint32_t winc = w;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const uint32_t up = __shfl_up_sync(0xffffffffu, winc, o);
+                        if (lane >= o) winc += up;
+                    }
+                    s_warp[lane] = winc - w;
+                }
+                __syncthreads();
+                uint32_t run = s_warp[warp] + inc - sum;
+#pragma unroll
+                for (uint32_t q = 0; q < kPer; ++q) {
+                    const uint32_t b = tid * kPer + q;
+                    s_off[b] = run;
+                    run += c[q];
+                    if (c[q]) s_base[b] = atomicAdd(&cursor[l0 + b], c[q]);
+                }
+            }
             __syncthreads();
 #pragma unroll
             for (int j = 0; j < kSortPerThread; ++j)
-                if (bin[j] != 0xffffffffu) out[s_base[bin[j]] + rk[j]] = d[j];
+                if (bin[j] != 0xffffffffu) s_tile[s_off[bin[j]] + rk[j]] = d[j];
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < kSortPerThread; ++j) {
+                const uint32_t i = (uint32_t)j * kLineThreads + tid;
+                if (i < m) {
+                    const uint2 e = s_tile[i];
+                    const uint32_t b2 = sort_line_of(g, e.x, e.y, n_lines) - l0;
+                    out[s_base[b2] + (i - s_off[b2])] = e;
+                }
+            }
         } else {
-            for (uint64_t i = t0 + threadIdx.x; i < t1; i += kLineThreads) {
+            for (uint64_t i = t0 + tid; i < t1; i += kLineThreads) {
                 const uint2 d = __ldg(in + i);
                 out[atomicAdd(&cursor[sort_line_of(g, d.x, d.y, n_lines)], 1u)] = d;
             }
@@ -280,6 +327,8 @@ cudaError_t sort_set_attributes()
 {
     cudaError_t e = cudaFuncSetAttribute(k_sort_scatter_top, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kTopTileN * sizeof(uint2)));
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_sort_scatter_line, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kLineTileN * sizeof(uint2) + 3 * kLineBins * 4));
+    if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(k_sort_rank_lines, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
 }
 
@@ -306,7 +355,7 @@ int launch_sort_digits(const Geo& g, const Workspace& ws, const tpc_digit* digit
     k += 2 + launch_scan_u32(ws.line_cnt, ws.line_start, (uint64_t)n_lines + 1, ws.sort_part, nullptr, st);
     // the fused kernels read line_start[n_lines] as the end of the last plane: the overflow bin (invalid digits) starts there
     cudaMemcpyAsync(ws.line_cnt, ws.line_start, ((size_t)n_lines + 1) * 4, cudaMemcpyDeviceToDevice, st);
-    k_sort_scatter_line<<<148 * 2, kLineThreads, 0, st>>>(tmp, tmp2, (uint32_t)n, g, n_lines, shift, ws.line_cnt);
+    k_sort_scatter_line<<<148 * 2, kLineThreads, kLineTileN * sizeof(uint2) + 3 * kLineBins * 4, st>>>(tmp, tmp2, (uint32_t)n, g, n_lines, shift, ws.line_cnt);
     uint32_t words;
     const uint32_t smem = sort_rank_smem(g, &words);
     k_sort_rank_lines<<<grid, kSortThreads, smem, st>>>(tmp2, tmp, ws.line_start, n_lines, g.n_time, words, ws.line_cnt,
