@@ -103,8 +103,8 @@ static size_t carve(const Geo& g, uint64_t max_digits, uint64_t max_clusters, ui
     w.line_desc = (unsigned long long*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 64) + 1) * 8);
     w.group_status = (tpc_cf_status*)take(sizeof(tpc_cf_status) * 32);
     w.sort_tmp = (tpc_digit*)take(sorted_only ? 0 : (size_t)max_digits * sizeof(tpc_digit));
-    w.sort_top = (uint32_t*)take(sorted_only ? 0 : ((size_t)1024 * 148 * 8 + 8) * 4);     // (bucket x block) table of the digit sort
-    w.sort_part = (uint32_t*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 1024) + 1200 + 4) * 4);
+    w.sort_top = (uint32_t*)take(1032 * 4);               // cursors of the digit sort's top-level buckets
+    w.sort_part = (uint32_t*)take((ceil_div_u64((uint64_t)g.n_planes * g.LS + 2, 1024) + 4) * 4);
     if (ws) *ws = w;
     if (n_sort_tiles) *n_sort_tiles = (uint32_t)tiles;
     if (map_bytes) *map_bytes = mapb;

@@ -8,15 +8,13 @@
 // unique inside a line (R11: one digit per cell).  So: an UNSTABLE two-level partition of the digits by pad line (order
 // inside a line does not matter yet), then one warp per line ranks its digits by time with a bitmap (rank = set bits
 // below).  No comparison sort, no stable radix pass:
-//   k_sort_hist        per block (a contiguous digit range): 1024-bin histogram of the line index's top bits -> table
-//                      (+ invalid digits counted, R11)
-//   scan (table)       -> where each block's digits of each top-level bucket go: no atomics, deterministic
-//   k_sort_scatter_top tile of 2048 digits: ranks inside the tile by shared-memory atomics, block-private cursors ->
-//                      digits grouped by bucket in ws.sort_tmp
-//   k_sort_count_lines digits per pad line (no-return atomics; a bucket's 1024 counters are L2-resident)
-//   scan (n_lines + 1) -> line_start: THE LINE INDEX OF THE FUSED PATH (k_plane_index / k_line_index are not needed)
-//   k_sort_scatter_line tile of 8192 digits (few buckets): ranks per line in shared memory, one global atomic per
-//                      (tile, line) -> digits grouped by line in the cluster staging area (idle here)
+//   k_sort_count_lines digits per pad line, on the input as it comes (no-return atomics on a 3 MB table)
+//   scan (n_lines + 1) -> line_start: THE LINE INDEX OF THE FUSED PATH (k_plane_index / k_line_index are not needed);
+//                      a top-level bucket (1024 consecutive lines) starts at line_start of its first line
+//   k_sort_scatter_top tile of 8192 digits: ranks per bucket by shared-memory atomics, the tile staged in bucket order,
+//                      one global atomic per (tile, bucket) reserves the run -> digits grouped by bucket in ws.sort_tmp
+//   k_sort_scatter_line tile of 8192 digits (few buckets): the same per line -> digits grouped by line in the cluster
+//                      staging area (idle here)
 //   k_sort_rank_lines  one warp per line: time bitmap + rank directory in shared memory -> sorted digits in ws.sort_tmp
 // Invalid digits (R11: out-of-range sector / row / pad / time, zero charge) go to an overflow bin behind the last line:
 // counted, never seen by the fused kernel.  A duplicate cell shows up as a bit already set in a line's bitmap: reported
@@ -44,51 +42,37 @@ static constexpr int kLineThreads = 1024;                            // line-lev
 static constexpr int kLineTileN = kLineThreads * kSortPerThread;
 static constexpr uint32_t kLineBins = 4096;                          // lines a tile may span for the aggregated path
 
-// Top level, deterministic and without global atomics: block b owns the contiguous digit range [b * chunk, (b + 1) *
-// chunk); k_sort_hist writes its bucket counts to table[bucket * kSortBlocks + b]; an exclusive scan of the table (bucket
-// major) turns the entry into the position where block b's digits of that bucket start; k_sort_scatter_top keeps the 1024
-// cursors of its block in shared memory and advances them tile by tile.
-__global__ void __launch_bounds__(kTopThreads)
-k_sort_hist(const uint2* __restrict__ digits, uint32_t n, uint32_t chunk, Geo g, uint32_t n_lines, uint32_t shift,
-            uint32_t* __restrict__ table, Counters* cnt)
+// first position of every top-level bucket = line_start of its first line (the overflow bin ends at n)
+__global__ void k_sort_top_cursors(const uint32_t* __restrict__ line_start, uint32_t n_lines, uint32_t shift, uint32_t n,
+                                   uint32_t* __restrict__ top_cur)
 {
-    __shared__ uint32_t s_h[kSortTopBins];
-    for (int i = threadIdx.x; i < (int)kSortTopBins; i += kTopThreads) s_h[i] = 0u;
-    __syncthreads();
-    uint32_t bad = 0u;
-    const uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
-    for (uint64_t i = lo + threadIdx.x; i < hi; i += kTopThreads) {
-        const uint2 d = __ldg(digits + i);
-        const uint32_t l = sort_line_of(g, d.x, d.y, n_lines);
-        bad += l == n_lines ? 1u : 0u;
-        atomicAdd(&s_h[l >> shift], 1u);
-    }
-    __syncthreads();
-    for (int i = threadIdx.x; i < (int)kSortTopBins; i += kTopThreads) table[(size_t)i * kSortBlocks + blockIdx.x] = s_h[i];
-    bad = __reduce_add_sync(0xffffffffu, bad);
-    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&cnt->n_bad, (unsigned long long)bad);
+    const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= kSortTopBins) return;
+    const uint64_t l = (uint64_t)b << shift;
+    top_cur[b] = l <= n_lines ? line_start[l] : n;
 }
 
+// Top level: a tile of 8192 digits; the (tile, bucket) run is reserved by one global atomic on the bucket's cursor.
 // The tile is first brought into bucket order in shared memory (ranks by shared-memory atomics, bucket offsets by a block
 // scan), then written out in that order: neighbouring lanes write neighbouring addresses of a bucket's run, so a warp's
 // store covers a few 32-byte sectors instead of 32 (ncu: 216 M store sectors for 220 M digits without the staging).
 __global__ void __launch_bounds__(kTopThreads)
-k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32_t n, uint32_t chunk, Geo g,
-                   uint32_t n_lines, uint32_t shift, const uint32_t* __restrict__ table)
+k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32_t n, Geo g,
+                   uint32_t n_lines, uint32_t shift, uint32_t* __restrict__ top_cur)
 {
     extern __shared__ __align__(16) uint2 s_tile[];              // kTopTileN digits in bucket order
     __shared__ uint32_t s_cnt[kSortTopBins];                     // digits of the tile per bucket
     __shared__ uint32_t s_off[kSortTopBins];                     // first position of the bucket inside the tile
-    __shared__ uint32_t s_cur[kSortTopBins];                     // output position of the bucket's next digit (this block)
+    __shared__ uint32_t s_cur[kSortTopBins];                     // output position of the bucket's run of this tile
     __shared__ uint32_t s_warp[32];
     static_assert(kTopThreads == (int)kSortTopBins, "one thread per bucket in the block scan");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    s_cur[tid] = table[(size_t)tid * kSortBlocks + blockIdx.x];
     s_cnt[tid] = 0u;
     __syncthreads();
-    const uint64_t lo = (uint64_t)blockIdx.x * chunk, hi = min((uint64_t)n, lo + chunk);
-    for (uint64_t t0 = lo; t0 < hi; t0 += kTopTileN) {
-        const uint32_t m = (uint32_t)min((uint64_t)kTopTileN, hi - t0);     // digits in this tile
+    const uint32_t n_tiles = (uint32_t)(((uint64_t)n + kTopTileN - 1) / kTopTileN);
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const uint64_t t0 = (uint64_t)tile * kTopTileN;
+        const uint32_t m = (uint32_t)min((uint64_t)kTopTileN, (uint64_t)n - t0);     // digits in this tile
         uint2 d[kSortPerThread];
         uint32_t bin[kSortPerThread], rk[kSortPerThread];
 #pragma unroll
@@ -124,6 +108,7 @@ k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32
             }
             __syncthreads();
             s_off[tid] = s_warp[warp] + inc - c;
+            if (c) s_cur[tid] = atomicAdd(&top_cur[tid], c);      // one reservation per (tile, bucket)
         }
         __syncthreads();
 #pragma unroll
@@ -140,7 +125,6 @@ k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32
             }
         }
         __syncthreads();
-        s_cur[tid] += s_cnt[tid];
         s_cnt[tid] = 0u;
         __syncthreads();
     }
@@ -312,7 +296,13 @@ k_sort_rank_lines(const uint2* __restrict__ in, uint2* __restrict__ out, const u
         for (uint32_t w = w0; w < w1; ++w) bm[w] = 0u;
         __syncwarp();
     }
-    if (lane == 0 && blockIdx.x == 0 && warp == 0) { line_cnt[n_lines] = 0u; line_desc[(n_lines >> 6) + 1u] = 0ull; }
+    if (lane == 0 && blockIdx.x == 0 && warp == 0) {
+        // the overflow bin behind the last line holds the invalid digits (R11): line_cnt was the line-level cursor
+        const uint32_t n_bad = line_cnt[n_lines] - line_start[n_lines];
+        if (n_bad) atomicAdd(&cnt->n_bad, (unsigned long long)n_bad);
+        line_cnt[n_lines] = 0u;
+        line_desc[(n_lines >> 6) + 1u] = 0ull;
+    }
     if (__any_sync(0xffffffffu, dup != 0u) && lane == 0) atomicOr(&cnt->unsorted, 1u);
 }
 
@@ -344,15 +334,12 @@ int launch_sort_digits(const Geo& g, const Workspace& ws, const tpc_digit* digit
     uint2* tmp2 = (uint2*)ws.stage;                                 // the cluster staging area is idle until the fused kernel
     const int grid = 148 * 8;
     int k = 0;
-    // top level: contiguous range per block, a multiple of the tile
-    const uint32_t chunk = (uint32_t)(ceil_div_u64(ceil_div_u64(n, kSortBlocks), kTopTileN) * kTopTileN);
-    const uint64_t table_n = (uint64_t)kSortTopBins * kSortBlocks;
     cudaMemsetAsync(ws.line_cnt, 0, ((size_t)n_lines + 2) * 4, st);
-    k_sort_hist<<<kSortBlocks, kTopThreads, 0, st>>>(in, (uint32_t)n, chunk, g, n_lines, shift, ws.sort_top, ws.counters);
-    k += 1 + launch_scan_u32(ws.sort_top, ws.sort_top, table_n, ws.sort_part, nullptr, st);
-    k_sort_scatter_top<<<kSortBlocks, kTopThreads, kTopTileN * sizeof(uint2), st>>>(in, tmp, (uint32_t)n, chunk, g, n_lines, shift, ws.sort_top);
-    k_sort_count_lines<<<grid, kSortThreads, 0, st>>>(tmp, (uint32_t)n, g, n_lines, ws.line_cnt);
-    k += 2 + launch_scan_u32(ws.line_cnt, ws.line_start, (uint64_t)n_lines + 1, ws.sort_part, nullptr, st);
+    k_sort_count_lines<<<grid, kSortThreads, 0, st>>>(in, (uint32_t)n, g, n_lines, ws.line_cnt);
+    k += 1 + launch_scan_u32(ws.line_cnt, ws.line_start, (uint64_t)n_lines + 1, ws.sort_part, nullptr, st);
+    k_sort_top_cursors<<<kSortTopBins / 256, 256, 0, st>>>(ws.line_start, n_lines, shift, (uint32_t)n, ws.sort_top);
+    k_sort_scatter_top<<<kSortBlocks, kTopThreads, kTopTileN * sizeof(uint2), st>>>(in, tmp, (uint32_t)n, g, n_lines, shift, ws.sort_top);
+    k += 2;
     // the fused kernels read line_start[n_lines] as the end of the last plane: the overflow bin (invalid digits) starts there
     cudaMemcpyAsync(ws.line_cnt, ws.line_start, ((size_t)n_lines + 1) * 4, cudaMemcpyDeviceToDevice, st);
     k_sort_scatter_line<<<148 * 2, kLineThreads, kLineTileN * sizeof(uint2) + 3 * kLineBins * 4, st>>>(tmp, tmp2, (uint32_t)n, g, n_lines, shift, ws.line_cnt);
