@@ -57,7 +57,10 @@ enum {
                                    free; if it is false nothing is output and status.path = 0, n_clusters = 0
                                    (rerun without the flag; tpc_cf_run_host does that by itself).  A wrong result
                                    is never returned silently. */
-    TPC_CF_FORCE_GENERAL = 2u,  /* always run the general (map in HBM, "T1") path, whatever the order */
+    TPC_CF_FORCE_GENERAL = 2u,  /* always run the general (map in HBM, "T1") path, whatever the order.  Without this flag
+                                   and without the promise above, the digits are sorted on the device into a workspace
+                                   buffer and the fused path runs on the sorted copy (status.path = 2): same result
+                                   array (R12), several times faster on unordered input */
     /* Cluster-finder variants.  The paper only says that "different cuts" are used in the
      * synchronous phase and names none; these definitions are this library's (DESIGN.md §3 V1..V3).
      * Peaks are always found by the same rule (R1): a cut never changes which cells are peaks (V3). */
