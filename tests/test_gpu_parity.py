@@ -696,3 +696,56 @@ def test_duplicate_cell_in_unsorted_input_is_reported():
     assert st["path"] == 0 and st["n_clusters"] == 0
     cl, st = gpu_run(dup, geom, PATHS["general"])
     assert st["path"] == 1 and st["n_clusters"] > 3000
+
+
+@pytest.mark.parametrize("seed", list(range(12)))
+def test_random_geometries_every_route(seed):
+    """Randomised cross-check: random geometry (sectors, rows, pads per row, time bins — including sizes that are no
+    multiple of any tile), random clustered digits with invalid ones mixed in (R11), in random order for the routes that
+    take any order; every route against the oracle, counts of invalid digits included."""
+    rng = np.random.default_rng(1000 + seed)
+    n_sectors, n_rows = int(rng.integers(1, 4)), int(rng.integers(1, 7))
+    max_pads = int(rng.integers(3, 40))
+    n_time = int(rng.choice([17, 64, 100, 513, 2000, 14336]))
+    npads = rng.integers(max(1, max_pads // 2), max_pads + 1, size=n_rows).astype(np.uint16)
+    npads[int(rng.integers(0, n_rows))] = max_pads
+    cells = {}
+    for s in range(n_sectors):
+        for r in range(n_rows):
+            for _ in range(int(rng.integers(0, 1 + max(1, int(npads[r]) * n_time // 40)))):
+                p0, t0 = int(rng.integers(0, npads[r])), int(rng.integers(0, n_time))
+                for dp in range(-1, 2):
+                    for dt in range(-2, 3):
+                        p, t = p0 + dp, t0 + dt
+                        if 0 <= p < npads[r] and 0 <= t < n_time and rng.random() < 0.75:
+                            cells[(s, r, p, t)] = int(rng.choice([1, 2, 3, 4, 5, 7, 20, 300, 65535]))
+    rows = [(s, r, p, 0, t, q) for (s, r, p, t), q in cells.items()]
+    n_bad = int(rng.integers(0, 6))
+    for _ in range(n_bad):                                  # invalid digits, each unique so that nothing is a duplicate cell
+        kind = int(rng.integers(0, 5))
+        s, r = int(rng.integers(0, n_sectors)), int(rng.integers(0, n_rows))
+        if kind == 0:
+            rows.append((n_sectors + int(rng.integers(0, 3)), r, 0, 0, len(rows) % n_time, 9))
+        elif kind == 1:
+            rows.append((s, n_rows + int(rng.integers(0, 3)), 0, 0, len(rows) % n_time, 9))
+        elif kind == 2:
+            rows.append((s, r, int(npads[r]) + int(rng.integers(0, 3)), 0, len(rows) % n_time, 9))
+        elif kind == 3:
+            rows.append((s, r, 0, 0, n_time + len(rows) % 50, 9))
+        else:
+            free = [(p, t) for p in range(int(npads[r])) for t in range(min(n_time, 40)) if (s, r, p, t) not in cells]
+            p, t = free[int(rng.integers(0, len(free)))]
+            cells[(s, r, p, t)] = 0
+            rows.append((s, r, p, 0, t, 0))               # zero charge
+    digits = np.array(rows, dtype=orc.DIGIT) if rows else np.zeros(0, dtype=orc.DIGIT)
+    geom = (n_sectors, n_rows, max_pads, n_time, npads)
+    ora, ost = orc.run(digits, *geom[:4], npads=npads)
+    assert ost["n_bad_digits"] == n_bad
+    srt = sort_digits(digits)
+    shuffled = digits[rng.permutation(digits.shape[0])]
+    for route, data in (("sorted_on_device", shuffled), ("general", shuffled), ("fused", srt), ("fused_pairs", srt),
+                        ("fused_blocks", srt), ("fused_lines", srt), ("general_hint", srt)):
+        cl, st = gpu_run(data, geom, PATHS[route], tuning=TUNING.get(route, {}))
+        assert st["path"] == EXPECT_PATH.get(route, 3), (route, st)
+        assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == n_bad, (route, st, ost)
+        assert_clusters_equal(cl, ora, "random geometry %d/%s" % (seed, route))
