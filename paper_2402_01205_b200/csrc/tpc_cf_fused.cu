@@ -81,19 +81,27 @@ k_plane_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __r
 // level 2: the lines of a plane, searched inside the plane's own range
 __global__ void __launch_bounds__(256)
 k_line_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start,
-             uint32_t* __restrict__ line_cnt, unsigned long long* __restrict__ line_desc)
+             uint32_t* __restrict__ line_cnt, unsigned long long* __restrict__ line_desc, Counters* cnt)
 {
+    // cnt != NULL: small input, no k_plane_index in front: every line is searched in the whole array (as many probes as
+    // the two-level search for small n, one launch less), and this kernel zeroes the run's counters as well
+    const bool direct = cnt != nullptr;
     const uint32_t total = g.n_planes * g.LS;
     const uint32_t e = blockIdx.x * 256 + threadIdx.x;
+    if (direct && e == 0) { cnt->n_bad = 0ull; cnt->n_used = 0ull; cnt->n_clusters = 0ull; cnt->unsorted = 0u; cnt->rsv = 0u; }
+    if (direct && e == total) line_start[total] = n;
     // per-run state of the compaction: peak counts (pads beyond npads[row] stay 0) and scan descriptors
     if (e <= total) line_cnt[e] = 0u;
     if (e <= (total + 63u) / 64u) line_desc[e] = 0ull;
     if (e >= total) return;
     const uint32_t plane = e / g.LS, p = e % g.LS;
-    if (p == 0) return;                                   // written by k_plane_index
+    if (p == 0 && !direct) return;                        // written by k_plane_index
     const uint32_t s = plane / g.n_rows, r = plane % g.n_rows;
-    uint32_t lo = line_start[(size_t)plane * g.LS], hi = line_start[(size_t)(plane + 1) * g.LS];
-    if (hi < lo || hi > n) { lo = 0; hi = n; }            // unsorted input: stay in bounds, the fused kernel reports it
+    uint32_t lo = 0, hi = n;
+    if (!direct) {
+        lo = line_start[(size_t)plane * g.LS]; hi = line_start[(size_t)(plane + 1) * g.LS];
+        if (hi < lo || hi > n) { lo = 0; hi = n; }        // unsorted input: stay in bounds, the fused kernel reports it
+    }
     line_start[e] = lower_bound_key(digits, lo, hi, (s << 16) | (r << 8) | p);   // (8-ary measured slower here: 122 vs 100 us — request-bound, not latency-bound)
 }
 
@@ -496,11 +504,15 @@ int launch_fused_sorted(const Geo& g, const Workspace& ws, const tpc_digit* digi
     }
     int k = 0;
     if (!have_index) {
-        k_plane_index<<<(g.n_planes + 1 + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
-                                                                     ws.counters);
+        const bool direct = n < (1u << 20);             // small input: one index launch instead of two
+        if (!direct) {
+            k_plane_index<<<(g.n_planes + 1 + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
+                                                                         ws.counters);
+            ++k;
+        }
         k_line_index<<<(entries + 255) / 256, 256, 0, st>>>((const uint2*)digits, (uint32_t)n, g, ws.line_start,
-                                                            ws.line_cnt, ws.line_desc);
-        k += 2;
+                                                            ws.line_cnt, ws.line_desc, direct ? ws.counters : nullptr);
+        ++k;
     }
 
     // Kernel choice.  Block-sparse line slots when the mean line fits their pool (k_fused_pairs, tpc_cf_pairs.cu; its
