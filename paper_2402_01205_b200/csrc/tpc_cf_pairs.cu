@@ -460,7 +460,7 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             const unsigned hma = __ballot_sync(0xffffffffu, head_a), hmb = __ballot_sync(0xffffffffu, head_b);
             const uint32_t idx_a = nblk + (uint32_t)__popc(hma & le_mask) + (uint32_t)__popc(hmb & lt_mask);   // 1-based
             const uint32_t idx_b = idx_a + (head_b ? 1u : 0u);
-            nblk = __shfl_sync(0xffffffffu, idx_b, 31);     // blocks opened so far
+            nblk += (uint32_t)__popc(hma) + (uint32_t)__popc(hmb);     // blocks opened so far (warp-uniform arithmetic)
             if (nblk < pcap) {                              // (warp-uniform) every block so far is in the pool
                 if (head_a) p_sts8(a_dir1 + (ta >> 3), idx_a);
                 if (head_b) p_sts8(a_dir1 + (tb >> 3), idx_b);
@@ -484,7 +484,7 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             const unsigned sma = __ballot_sync(0xffffffffu, surv_a), smb = __ballot_sync(0xffffffffu, surv_b);
             const uint32_t pos_a = nsurv + (uint32_t)__popc(sma & lt_mask) + (uint32_t)__popc(smb & lt_mask);
             const uint32_t pos_b = pos_a + (surv_a ? 1u : 0u);
-            nsurv = __shfl_sync(0xffffffffu, pos_b + (surv_b ? 1u : 0u), 31);   // survivors so far
+            nsurv += (uint32_t)__popc(sma) + (uint32_t)__popc(smb);   // survivors so far
             if (nsurv <= scap) {                            // (warp-uniform) the list holds every survivor so far
                 if (surv_a) p_sts32(a_surv + (pos_a << 2), ya);
                 if (surv_b) p_sts32(a_surv + (pos_b << 2), yb);
