@@ -454,13 +454,28 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
             const bool own_a = MULTI ? (ta - tlo) < own_span : inb_a;     // a cell this pass decides
             const bool own_b = MULTI ? (tb - tlo) < own_span : inb_b;
             ymin = min(ymin, min(ya, yb));                  // R11: zero charges are looked for here, counted below
+            // All four ballots and their bit counts come first (independent of each other: the builder warps are bound by
+            // the latency of dependent chains, not by issue slots), the stores after.
             // K1: blocks are allocated in time order: a digit opens a block iff the digit before it is in another one
             const bool head_a = inb_a && (ta ^ tp) > 7u;
             const bool head_b = inb_b && (tb ^ ta) > 7u;
+            // K2 stage A (R1, own line).  (0,-1) is earlier: the digit loses to an adjacent previous charge >= its
+            // own; (0,+1) is later: it loses to an adjacent next charge > its own (cells at time >= T read 0).
+            // With qe = charge of the adjacent cell (0 if there is no digit there): survive iff q >= max(q_peak_min,
+            // qe(previous) + 1, qe(next)).
+            const bool adj_ab = d_ab == 0u && tb < T;
+            const uint32_t qpe_a = d_pa == 0u ? qp + 1u : 0u, qne_a = adj_ab ? qb : 0u;
+            const uint32_t qpe_b = adj_ab ? qa + 1u : 0u, qne_b = (d_bn == 0u && tn < T) ? qn : 0u;
+            const bool surv_a = own_a && qa >= max(max(qpe_a, qne_a), q_peak_min);
+            const bool surv_b = own_b && qb >= max(max(qpe_b, qne_b), q_peak_min);
             const unsigned hma = __ballot_sync(0xffffffffu, head_a), hmb = __ballot_sync(0xffffffffu, head_b);
+            const unsigned sma = __ballot_sync(0xffffffffu, surv_a), smb = __ballot_sync(0xffffffffu, surv_b);
             const uint32_t idx_a = nblk + (uint32_t)__popc(hma & le_mask) + (uint32_t)__popc(hmb & lt_mask);   // 1-based
             const uint32_t idx_b = idx_a + (head_b ? 1u : 0u);
+            const uint32_t pos_a = nsurv + (uint32_t)__popc(sma & lt_mask) + (uint32_t)__popc(smb & lt_mask);
+            const uint32_t pos_b = pos_a + (surv_a ? 1u : 0u);
             nblk += (uint32_t)__popc(hma) + (uint32_t)__popc(hmb);     // blocks opened so far (warp-uniform arithmetic)
+            nsurv += (uint32_t)__popc(sma) + (uint32_t)__popc(smb);    // survivors so far
             if (nblk < pcap) {                              // (warp-uniform) every block so far is in the pool
                 if (head_a) p_sts8(a_dir1 + (ta >> 3), idx_a);
                 if (head_b) p_sts8(a_dir1 + (tb >> 3), idx_b);
@@ -472,19 +487,6 @@ k_fused_pairs(const uint2* __restrict__ digits, uint32_t n, Geo g, const uint32_
                 if (inb_a && idx_a < pcap) p_sts16(a_pool + (idx_a << 4) + ((ta & 7u) << 1), qa);
                 if (inb_b && idx_b < pcap) p_sts16(a_pool + (idx_b << 4) + ((tb & 7u) << 1), qb);
             }
-            // K2 stage A (R1, own line).  (0,-1) is earlier: the digit loses to an adjacent previous charge >= its
-            // own; (0,+1) is later: it loses to an adjacent next charge > its own (cells at time >= T read 0).
-            // With qe = charge of the adjacent cell (0 if there is no digit there): survive iff q >= max(q_peak_min,
-            // qe(previous) + 1, qe(next)).
-            const bool adj_ab = d_ab == 0u && tb < T;
-            const uint32_t qpe_a = d_pa == 0u ? qp + 1u : 0u, qne_a = adj_ab ? qb : 0u;
-            const uint32_t qpe_b = adj_ab ? qa + 1u : 0u, qne_b = (d_bn == 0u && tn < T) ? qn : 0u;
-            const bool surv_a = own_a && qa >= max(max(qpe_a, qne_a), q_peak_min);
-            const bool surv_b = own_b && qb >= max(max(qpe_b, qne_b), q_peak_min);
-            const unsigned sma = __ballot_sync(0xffffffffu, surv_a), smb = __ballot_sync(0xffffffffu, surv_b);
-            const uint32_t pos_a = nsurv + (uint32_t)__popc(sma & lt_mask) + (uint32_t)__popc(smb & lt_mask);
-            const uint32_t pos_b = pos_a + (surv_a ? 1u : 0u);
-            nsurv += (uint32_t)__popc(sma) + (uint32_t)__popc(smb);   // survivors so far
             if (nsurv <= scap) {                            // (warp-uniform) the list holds every survivor so far
                 if (surv_a) p_sts32(a_surv + (pos_a << 2), ya);
                 if (surv_b) p_sts32(a_surv + (pos_b << 2), yb);
