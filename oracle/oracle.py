@@ -36,8 +36,8 @@ class _Params(ctypes.Structure):
 
 
 # variant bits of params.flags (restated from tpc_cf_oracle.h) and cluster flag bits (V1)
-CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME = 4, 8, 16
-F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED = 1, 2, 4, 8, 16
+CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME, SHARE_CHARGE = 4, 8, 16, 32
+F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED, F_SHARED = 1, 2, 4, 8, 16, 32
 
 
 class _Status(ctypes.Structure):

@@ -49,7 +49,7 @@ typedef struct {
 } orc_geometry;
 
 /* Cluster-finder variants ("different cuts" in PAPER.md:21 — the paper names none,
- * the definitions are this repository's, DESIGN.md §3 V1..V3).  Peaks are found exactly as before; then
+ * the definitions are this repository's, DESIGN.md §3 V1..V4).  Peaks are found exactly as before; then
  *   V1 flags (written iff ORC_CLUSTER_FLAGS, else 0), from the peak cell and the sums of the accepted cells:
  *        1 EDGE_PAD     pad < 2 or pad + 2 >= npads[row]      (the 5x5 window is clipped by the plane in pad)
  *        2 EDGE_TIME    time < 2 or time + 2 >= n_time
@@ -58,9 +58,22 @@ typedef struct {
  *       16 SATURATED    q_saturation != 0 and qMax >= q_saturation
  *   V2 cuts: a peak whose cluster has qTot < q_tot_min, or is SINGLE_PAD / SINGLE_TIME while the matching
  *        ORC_CUT_* bit is set, yields no cluster and is not counted in n_clusters.
- *   V3 a cut never changes which cells are peaks. */
-enum { ORC_CLUSTER_FLAGS = 4u, ORC_CUT_SINGLE_PAD = 8u, ORC_CUT_SINGLE_TIME = 16u };
-enum { ORC_F_EDGE_PAD = 1, ORC_F_EDGE_TIME = 2, ORC_F_SINGLE_PAD = 4, ORC_F_SINGLE_TIME = 8, ORC_F_SATURATED = 16 };
+ *   V3 a cut never changes which cells are peaks.
+ *   V4 charge sharing between overlapping clusters (ORC_SHARE_CHARGE), in place of the double counting of R5.  The
+ *        clusters of the run are found, cut and flagged exactly as above, on the unshared sums.  Let A(x) = qMax of
+ *        the cluster whose peak is cell x (0 if x is no cluster's peak) and D(x) = sum of A over the 5x5 cells around
+ *        x in the same plane = the summed peak charges of the clusters whose window contains x.  For the cluster with
+ *        peak z, every cell x that enters its sums (R3 / R4 unchanged, decided on the raw charges) enters with
+ *            c'(x) = floor(64 * Q(x) * A(z) / D(x))
+ *        in place of Q(x): its charge in units of 1/64 ADC count, split among the windows that contain it in proportion
+ *        to their peak charges (a window that contains x but gates it out keeps its share: that part is dropped).
+ *        From the sums S' over c': qtot = floor((S0' + 32) / 64); centroids and sigmas by the same formulas on S'
+ *        (S0' = 0, possible only if every share rounds to 0: the peak's position, sigmas 0).  sector..time, qmax and
+ *        flags 1..16 are those of the unshared cluster; flag 32 SHARED iff D(x) != A(z) for some cell x with charge
+ *        that entered.  A cluster no other window touches comes out bit-identical to the unshared run. */
+enum { ORC_CLUSTER_FLAGS = 4u, ORC_CUT_SINGLE_PAD = 8u, ORC_CUT_SINGLE_TIME = 16u, ORC_SHARE_CHARGE = 32u };
+enum { ORC_F_EDGE_PAD = 1, ORC_F_EDGE_TIME = 2, ORC_F_SINGLE_PAD = 4, ORC_F_SINGLE_TIME = 8, ORC_F_SATURATED = 16,
+       ORC_F_SHARED = 32 };
 
 typedef struct {
     uint16_t q_peak_min;        /* R6: peak threshold, default 4 */

@@ -141,3 +141,38 @@ def find_clusters_variants(cells, P, T, q_peak_min=4, q_inner_gate=2, q_tot_min=
             continue
         out.append(c + (fl,))
     return out
+
+
+# ---- V4 charge sharing (DESIGN.md §3 V4), formulated differently from the oracle ------------------------------------
+F_SHARED = 32
+
+
+def find_clusters_shared(cells, P, T, q_peak_min=4, q_inner_gate=2, q_tot_min=0, q_saturation=0,
+                         cut_single_pad=False, cut_single_time=False):
+    """V4 by enumeration of the cluster list (no peak-charge map, no box sum): the weight of cluster k on a cell is
+    qmax_k over the summed qmax of the listed clusters whose peak lies within Chebyshev distance 2 of the cell; the
+    share is the floor of an exact Fraction.  Entries: (pad, time, qmax, qtot, S0', S1p', S1t', S2p', S2t', flags)."""
+    base = find_clusters_variants(cells, P, T, q_peak_min, q_inner_gate, q_tot_min, q_saturation,
+                                  cut_single_pad, cut_single_time)
+    out = []
+    for (p, t, qmax, _S0, _a, _b, _c, _d, fl) in base:
+        sums = [0, 0, 0, 0, 0]
+        shared = False
+        for dp, dt, c in counted_cells(cells, P, T, p, t, q_inner_gate):
+            x = (p + dp, t + dt)
+            claim = sum(k[2] for k in base if max(abs(k[0] - x[0]), abs(k[1] - x[1])) <= 2)
+            if c > 0 and claim != qmax:
+                shared = True
+            share = math.floor(Fraction(64 * c * qmax, claim))
+            for i, w in enumerate((1, dp, dt, dp * dp, dt * dt)):
+                sums[i] += share * w
+        qtot = math.floor(Fraction(sums[0], 64) + Fraction(1, 2))
+        out.append((p, t, qmax, qtot) + tuple(sums) + (fl | (F_SHARED if shared else 0),))
+    return out
+
+
+def moments_from_shared_sums(p, t, S0, S1p, S1t, S2p, S2t):
+    """moments_from_sums with V4's degenerate case: all shares rounded to zero -> the peak's position, sigmas 0."""
+    if S0 == 0:
+        return float(p), float(t), 0.0, 0.0
+    return moments_from_sums(p, t, S0, S1p, S1t, S2p, S2t)
