@@ -637,9 +637,10 @@ def main():
     ap.add_argument("--no-per-config", dest="per_config", action="store_false",
                     help="only the headline config (default: the other four configs of BASELINE.json are measured and "
                          "compared with the oracle too, in a per_config block of the same JSON line)")
-    ap.add_argument("--variant", default="none", choices=["none", "flags", "cuts"],
+    ap.add_argument("--variant", default="none", choices=["none", "flags", "cuts", "share"],
                     help="cluster-finder variants (SURVEY.md §8(f) NEXT #1): 'flags' = per-cluster flags, 'cuts' = "
-                         "flags + q_tot_min 40 + single-pad cut; the default run has none")
+                         "flags + q_tot_min 40 + single-pad cut, 'share' = flags + charge sharing between overlapping "
+                         "clusters (V4, the K6 post-pass); the default run has none")
     ap.add_argument("--stage", default="cf", choices=["cf", "ec", "fe", "chain"],
                     help="'cf' = the cluster finder (the headline path); 'ec' = the entropy coder of the cluster stream "
                          "(SURVEY.md §8(f) NEXT #2): encode and decode of the frame's clusters, one JSON line; 'fe' = the "
@@ -715,10 +716,11 @@ def measure_config(cf, torch, cfg_id, steps, warmup, path, variant, dev, frame_o
     n_digits = [int(f.shape[0]) for f in frames]
     nmax = max(n_digits)
     max_clusters = nmax // 10 + 1024
-    vflags = {"none": 0, "flags": cf.CLUSTER_FLAGS, "cuts": cf.CLUSTER_FLAGS | cf.CUT_SINGLE_PAD}[variant]
+    vflags = {"none": 0, "flags": cf.CLUSTER_FLAGS, "cuts": cf.CLUSTER_FLAGS | cf.CUT_SINGLE_PAD,
+              "share": cf.CLUSTER_FLAGS | cf.SHARE_CHARGE}[variant]
+    q_tot_min, q_saturation = (40 if variant == "cuts" else 0), (1000 if variant in ("flags", "cuts") else 0)
     finder = cf.ClusterFinder(*geom[:4], npads=geom[4], max_digits=nmax, max_clusters=max_clusters, device=dev,
-                              q_tot_min=40 if variant == "cuts" else 0,
-                              q_saturation=1000 if variant != "none" else 0)
+                              q_tot_min=q_tot_min, q_saturation=q_saturation)
     flags = (cf.DIGITS_SORTED if path == "fused" else (cf.DIGITS_SORTED | cf.FORCE_GENERAL)) | vflags
     pinned = [torch.from_numpy(f.view(np.uint8)).pin_memory() for f in frames] if keep else None
     dev_digits = [(p if p is not None else torch.from_numpy(f.view(np.uint8))).to(dev, non_blocking=True)
@@ -793,7 +795,9 @@ def measure_config(cf, torch, cfg_id, steps, warmup, path, variant, dev, frame_o
         for f, o, s in zip(frames, outs, stats):
             cl, st = finder.result(clusters=o, status=s)
             t0 = time.perf_counter()
-            ora, ost, nthr = orc.run_parallel(f, *geom[:4], npads=geom[4])
+            # (the variant bits have the same values on both sides: include/tpc_cf.h and oracle/tpc_cf_oracle.h)
+            ora, ost, nthr = orc.run_parallel(f, *geom[:4], npads=geom[4], flags=vflags, q_tot_min=q_tot_min,
+                                              q_saturation=q_saturation)
             t_or += time.perf_counter() - t0
             c = compare_clusters(cl, ora)
             if st["n_bad_digits"] != ost["n_bad_digits"]:
@@ -852,7 +856,7 @@ def run_cf(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
     peak, peak_src = load_peaks()
-    do_parity = not args.no_cpu_baseline and not args.no_parity and rank == 0 and args.variant == "none"
+    do_parity = not args.no_cpu_baseline and not args.no_parity and rank == 0
 
     # ---- headline config: K timed steps, device-resident inputs --------------------------------------------------------
     cfg = gen.CONFIGS[args.config]

@@ -62,11 +62,26 @@ enum {
                                    buffer and the fused path runs on the sorted copy (status.path = 2): same result
                                    array (R12), several times faster on unordered input */
     /* Cluster-finder variants.  The paper only says that "different cuts" are used in the
-     * synchronous phase and names none; these definitions are this library's (DESIGN.md §3 V1..V3).
+     * synchronous phase and names none; these definitions are this library's (DESIGN.md §3 V1..V4).
      * Peaks are always found by the same rule (R1): a cut never changes which cells are peaks (V3). */
     TPC_CF_CLUSTER_FLAGS = 4u,    /* V1: fill tpc_cluster.flags with the TPC_CF_F_* bits below (else the byte is 0) */
     TPC_CF_CUT_SINGLE_PAD = 8u,   /* V2: a SINGLE_PAD cluster is not output and not counted */
-    TPC_CF_CUT_SINGLE_TIME = 16u  /* V2: same for SINGLE_TIME */
+    TPC_CF_CUT_SINGLE_TIME = 16u, /* V2: same for SINGLE_TIME */
+    TPC_CF_SHARE_CHARGE = 32u     /* V4: charge sharing between overlapping clusters in place of the double counting of R5.
+                                     The clusters of the run are found, cut and flagged exactly as without this bit, on the
+                                     unshared sums.  Let A(x) = qMax of the cluster whose peak is cell x (0 if none) and
+                                     D(x) = sum of A over the 5x5 cells around x in the same plane (the summed peak charges
+                                     of the clusters whose window holds x).  For the cluster with peak z every cell x that
+                                     enters its sums (R3 / R4 unchanged, on raw charges) enters with
+                                         c'(x) = floor(64 * Q(x) * A(z) / D(x))
+                                     in place of Q(x): its charge in 1/64 ADC counts, split among the windows that hold it
+                                     in proportion to their peak charges.  From the sums S' over c':
+                                     qtot = floor((S0' + 32) / 64), centroids and sigmas by the same formulas (S0' = 0: the
+                                     peak's position, sigmas 0).  sector..time, qmax and flags 1..16 stay those of the
+                                     unshared cluster; a cluster no other window touches comes out bit-identical.
+                                     Runs as a post-pass (K6) over the ordered output of whichever path produced it.
+                                     With status.overflow = 1 the clusters written near the cut may miss neighbours that
+                                     were not written: their shared values are unspecified. */
 };
 
 /* V1: bits of tpc_cluster.flags, from the peak cell and the cells that entered qTot. */
@@ -75,7 +90,9 @@ enum {
     TPC_CF_F_EDGE_TIME = 2u,    /* time < 2 or time + 2 >= n_time */
     TPC_CF_F_SINGLE_PAD = 4u,   /* no charge outside the peak's pad line entered qTot (sigma_pad == 0) */
     TPC_CF_F_SINGLE_TIME = 8u,  /* no charge outside the peak's time bin entered qTot (sigma_time == 0) */
-    TPC_CF_F_SATURATED = 16u    /* q_saturation != 0 and qMax >= q_saturation */
+    TPC_CF_F_SATURATED = 16u,   /* q_saturation != 0 and qMax >= q_saturation */
+    TPC_CF_F_SHARED = 32u       /* V4 only: some cell with charge that entered this cluster lies in another cluster's window
+                                   too (its charge was split) */
 };
 
 typedef struct {

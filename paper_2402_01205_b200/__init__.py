@@ -4,7 +4,7 @@
 The CUDA library (libtpc_cf.so) is loaded on first use; there is no CPU fallback.
 """
 from .binding import (CLUSTER, CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME, DIGIT, DIGITS_SORTED, EXPORTS,
-                      F_EDGE_PAD, F_EDGE_TIME, F_SATURATED, F_SINGLE_PAD, F_SINGLE_TIME, FORCE_GENERAL, STATUS, ClusterFinder, Geometry, Out,
+                      F_EDGE_PAD, F_EDGE_TIME, F_SATURATED, F_SHARED, F_SINGLE_PAD, F_SINGLE_TIME, FORCE_GENERAL, SHARE_CHARGE, STATUS, ClusterFinder, Geometry, Out,
                       Params, TpcCfError, load, make_geometry, scan_u32_static, to_device, tpc_cf_create,
                       tpc_cf_destroy, tpc_cf_run, tpc_cf_workspace_bytes)
 
@@ -23,6 +23,6 @@ __all__ = ["ShardedClusterFinder", "gather_records", "plane_counts", "plane_part
            "ClusterCoder", "clusters_to_device", "tpc_ec_create", "tpc_ec_decode", "tpc_ec_destroy", "tpc_ec_encode",
            "tpc_ec_max_encoded_bytes", "tpc_ec_workspace_bytes",
            "CLUSTER", "DIGIT", "STATUS", "DIGITS_SORTED", "FORCE_GENERAL", "CLUSTER_FLAGS", "CUT_SINGLE_PAD",
-           "CUT_SINGLE_TIME", "F_EDGE_PAD", "F_EDGE_TIME", "F_SINGLE_PAD", "F_SINGLE_TIME", "F_SATURATED", "EXPORTS", "ClusterFinder", "Geometry",
+           "CUT_SINGLE_TIME", "F_EDGE_PAD", "F_EDGE_TIME", "F_SINGLE_PAD", "F_SINGLE_TIME", "F_SATURATED", "F_SHARED", "SHARE_CHARGE", "EXPORTS", "ClusterFinder", "Geometry",
            "Out", "Params", "TpcCfError", "load", "make_geometry", "scan_u32_static", "to_device", "tpc_cf_create", "tpc_cf_destroy",
            "tpc_cf_run", "tpc_cf_workspace_bytes"]

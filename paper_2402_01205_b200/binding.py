@@ -25,8 +25,8 @@ DIGITS_SORTED = 1
 FORCE_GENERAL = 2
 WS_SORTED_ONLY = 1      # tpc_cf_create_ex / tpc_cf_workspace_bytes_ex
 # cluster-finder variants (include/tpc_cf.h V1..V3): params.flags bits and tpc_cluster.flags bits
-CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME = 4, 8, 16
-F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED = 1, 2, 4, 8, 16
+CLUSTER_FLAGS, CUT_SINGLE_PAD, CUT_SINGLE_TIME, SHARE_CHARGE = 4, 8, 16, 32
+F_EDGE_PAD, F_EDGE_TIME, F_SINGLE_PAD, F_SINGLE_TIME, F_SATURATED, F_SHARED = 1, 2, 4, 8, 16, 32
 
 # tpc_cf_debug_set keys and the values of "fused_kernel" (include/tpc_cf.h)
 DEBUG_KEYS = {"fused_kernel": 1, "passes": 2, "block_pool": 3, "surv_cap": 4, "pads_per_unit": 5, "ctas_per_sm": 6}

@@ -11,7 +11,7 @@ SO = os.path.join(_HERE, "libtpc_cf.so")
 import glob
 
 SOURCES = ["tpc_cf_api.cu", "tpc_cf_general.cu", "tpc_cf_fused.cu", "tpc_cf_blocks.cu", "tpc_cf_pairs.cu", "tpc_cf_sort.cu",
-           "tpc_cf_compact.cu", "tpc_ec.cu", "tpc_fe.cu"]
+           "tpc_cf_compact.cu", "tpc_cf_share.cu", "tpc_ec.cu", "tpc_fe.cu"]
 HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh")) +
                  glob.glob(os.path.join(os.path.dirname(_HERE), "include", "*.h")))
 EXTRA = os.environ.get("TPC_CF_NVCC_EXTRA", "").split()

@@ -188,7 +188,7 @@ static int check_run_args(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     if (n > h->max_digits) return TPC_CF_E_CAPACITY;
     if (params->q_peak_min == 0) return TPC_CF_E_PARAMS;
     if (params->flags & ~(uint32_t)(TPC_CF_DIGITS_SORTED | TPC_CF_FORCE_GENERAL | TPC_CF_CLUSTER_FLAGS |
-                                    TPC_CF_CUT_SINGLE_PAD | TPC_CF_CUT_SINGLE_TIME)) return TPC_CF_E_PARAMS;
+                                    TPC_CF_CUT_SINGLE_PAD | TPC_CF_CUT_SINGLE_TIME | TPC_CF_SHARE_CHARGE)) return TPC_CF_E_PARAMS;
     if (((uintptr_t)digits & 7u) != 0) return TPC_CF_E_NULL;
     return TPC_CF_OK;
 }
@@ -215,6 +215,7 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
     var.q_saturation = params->q_saturation;
     var.vflags = params->flags & (TPC_CF_CLUSTER_FLAGS | TPC_CF_CUT_SINGLE_PAD | TPC_CF_CUT_SINGLE_TIME);
     var.active = (var.q_tot_min != 0u || var.vflags != 0u) ? 1u : 0u;
+    const bool share = (params->flags & TPC_CF_SHARE_CHARGE) != 0;
 
     (void)cudaGetLastError();
     if (prof) cudaEventRecord(ev[0], st);
@@ -243,6 +244,11 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
         k += r;
         NvtxRange nv("K3 K5: scan + ordered copy + status");
         k += launch_compact_lines(h->geo, h->ws, out->clusters, out->capacity, out->status, n, sortfuse ? 2u : 3u, st);
+        if (share) {
+            NvtxRange nv6("K6: charge sharing between overlapping clusters (V4)");
+            k += launch_share_charge(h->geo, h->ws, src, out->clusters, out->capacity, out->status, params->q_inner_gate,
+                                     var.vflags, h->max_digits, st);
+        }
     } else {
         // T1: K1 scatter -> K2+K4 digit-centric peaks + moments on the HBM map -> K3 compaction -> (K5 key sort)
         //     -> K0 un-scatter
@@ -252,8 +258,13 @@ extern "C" int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n, const 
         { NvtxRange nv("K3: compaction");
           k += launch_compact(h->ws, n, out->clusters, out->capacity, h->max_clusters, hint ? 0 : 1, st); }
         if (!hint) { NvtxRange nv("K5: key sort"); k += launch_key_sort(h->ws, h->max_clusters, h->n_sort_tiles, out->clusters, out->capacity, st); }
-        { NvtxRange nv("K0: un-scatter"); k += launch_unscatter(h->geo, h->ws, digits, n, st); }
         k += launch_finalize(h->ws, out->status, out->capacity, 1u, hint ? 1 : 0, n, h->max_clusters, st);
+        if (share) {                  // (reads the map: ahead of the un-scatter)
+            NvtxRange nv6("K6: charge sharing between overlapping clusters (V4)");
+            k += launch_share_charge(h->geo, h->ws, nullptr, out->clusters, out->capacity, out->status,
+                                     params->q_inner_gate, var.vflags, h->max_digits, st);
+        }
+        { NvtxRange nv("K0: un-scatter"); k += launch_unscatter(h->geo, h->ws, digits, n, st); }
     }
     if (prof) { cudaEventRecord(ev[3], st); ++h->run_index; }
     e = cudaGetLastError();

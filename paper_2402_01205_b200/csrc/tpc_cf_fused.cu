@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(256)
 k_plane_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __restrict__ line_start, Counters* cnt)
 {
     const uint32_t plane = blockIdx.x * 256 + threadIdx.x;
-    if (plane == 0) { cnt->n_bad = 0ull; cnt->n_used = 0ull; cnt->n_clusters = 0ull; cnt->unsorted = 0u; cnt->rsv = 0u; }
+    if (plane == 0) { cnt->n_bad = 0ull; cnt->n_used = 0ull; cnt->n_clusters = 0ull; cnt->unsorted = 0u; cnt->n_share = 0u; }
     if (plane > g.n_planes) return;
     if (plane == g.n_planes) { line_start[(size_t)g.n_planes * g.LS] = n; return; }
     const uint32_t s = plane / g.n_rows, r = plane % g.n_rows;
@@ -88,7 +88,7 @@ k_line_index(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t* __re
     const bool direct = cnt != nullptr;
     const uint32_t total = g.n_planes * g.LS;
     const uint32_t e = blockIdx.x * 256 + threadIdx.x;
-    if (direct && e == 0) { cnt->n_bad = 0ull; cnt->n_used = 0ull; cnt->n_clusters = 0ull; cnt->unsorted = 0u; cnt->rsv = 0u; }
+    if (direct && e == 0) { cnt->n_bad = 0ull; cnt->n_used = 0ull; cnt->n_clusters = 0ull; cnt->unsorted = 0u; cnt->n_share = 0u; }
     if (direct && e == total) line_start[total] = n;
     // per-run state of the compaction: peak counts (pads beyond npads[row] stay 0) and scan descriptors
     if (e <= total) line_cnt[e] = 0u;

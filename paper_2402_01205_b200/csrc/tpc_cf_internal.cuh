@@ -26,7 +26,7 @@ struct Counters {
     unsigned long long n_used;
     unsigned long long n_clusters;  // total peaks
     unsigned int unsorted;          // 1 if digits[i-1] > digits[i] for some i (key = sector,row,pad,time)
-    unsigned int rsv;
+    unsigned int n_share;           // V4: clusters queued for the sharing pass (tpc_cf_share.cu)
 };
 
 // Pointers into the caller-owned workspace.
@@ -252,6 +252,12 @@ int launch_key_sort(const Workspace& ws, uint64_t max_clusters, uint32_t n_sort_
                     uint64_t capacity, cudaStream_t st);
 int launch_finalize(const Workspace& ws, tpc_cf_status* status, uint64_t capacity, uint32_t path,
                     int hint_sorted, uint64_t n, uint64_t max_clusters, cudaStream_t st);
+
+// V4 (TPC_CF_SHARE_CHARGE): post-pass over the ordered records in `out` once `status` is written (tpc_cf_share.cu).
+// digits != nullptr: the sorted digits the fused path ran on (+ ws.line_start); nullptr: the general path's charge map,
+// which must still be filled.  Scratch: ws.line_cnt, ws.stage (8 bytes per digit of it), counters->n_share.
+int launch_share_charge(const Geo& g, const Workspace& ws, const tpc_digit* digits, tpc_cluster* out, uint64_t capacity,
+                        const tpc_cf_status* status, uint32_t q_gate, uint32_t vflags, uint64_t max_digits, cudaStream_t st);
 
 // exclusive scan of n uint32 (in -> out, may alias); total (optional) receives the sum as 64-bit.
 int launch_scan_u32(const uint32_t* in, uint32_t* out, uint64_t n, uint32_t* partials,
