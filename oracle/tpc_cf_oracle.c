@@ -129,6 +129,7 @@ static int64_t scan_plane(const uint16_t* Q, uint16_t* A, uint32_t P, uint32_t T
         memset(A, 0, ((size_t)P + 2 * ABORDER) * WA * sizeof(uint16_t));
         for (int p = 0; p < (int)P; ++p)
             for (int t = 0; t < (int)T; ++t) {
+                if (QAT(p, t) < prm->q_peak_min) continue;    /* R6 (most cells are empty) */
                 if (!is_peak(Q, W, p, t, prm)) continue;
                 const orc_sums m = window_sums(Q, W, NULL, 0, p, t, prm, NULL);
                 unsigned fl;
@@ -138,8 +139,9 @@ static int64_t scan_plane(const uint16_t* Q, uint16_t* A, uint32_t P, uint32_t T
 
     for (int p = 0; p < (int)P; ++p) {                       /* pad-major, time-minor (R10) */
         for (int t = 0; t < (int)T; ++t) {
-            if (!is_peak(Q, W, p, t, prm)) continue;
             const uint16_t q = QAT(p, t);
+            if (q < prm->q_peak_min) continue;                /* R6 (most cells are empty) */
+            if (!is_peak(Q, W, p, t, prm)) continue;
             orc_sums m = window_sums(Q, W, NULL, 0, p, t, prm, NULL);
             /* P5 / R8: every sum is an integer below 2^24, so fp32 accumulation is exact. */
             if (m.S0 >= (1 << 24) || llabs(m.S1p) >= (1 << 24) || llabs(m.S1t) >= (1 << 24) ||

@@ -161,6 +161,27 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(cf.Geometry) == 24 and ctypes.sizeof(cf.Params) == 16 and ctypes.sizeof(cf.Out) == 32
 
 
+def test_variant_bits_agree_between_header_binding_and_oracle_header():
+    """bench.py and the GPU tests pass the same flag word to the library and to the oracle: the enumerators of
+    include/tpc_cf.h, the constants of the binding and the (independently written) oracle header must agree."""
+    import re
+    root = os.path.join(os.path.dirname(__file__), "..")
+    hdr = open(os.path.join(root, "include", "tpc_cf.h")).read()
+    orc_hdr = open(os.path.join(root, "oracle", "tpc_cf_oracle.h")).read()
+
+    def enum(text, name):
+        m = re.search(r"\b%s\s*=\s*(\d+)u?" % name, text)
+        assert m, name
+        return int(m.group(1))
+    from paper_2402_01205_b200 import binding
+    from oracle import oracle as orc
+    for name in ("CLUSTER_FLAGS", "CUT_SINGLE_PAD", "CUT_SINGLE_TIME", "SHARE_CHARGE"):
+        assert enum(hdr, "TPC_CF_" + name) == getattr(binding, name) == getattr(orc, name) == enum(orc_hdr, "ORC_" + name)
+    for name in ("EDGE_PAD", "EDGE_TIME", "SINGLE_PAD", "SINGLE_TIME", "SATURATED", "SHARED"):
+        assert (enum(hdr, "TPC_CF_F_" + name) == getattr(binding, "F_" + name) == getattr(orc, "F_" + name)
+                == enum(orc_hdr, "ORC_F_" + name))
+
+
 def test_workspace_bytes_and_geometry_limits():
     import paper_2402_01205_b200 as cf
     g, _ = cf.make_geometry(36, 152, 138, 14336)
