@@ -165,7 +165,9 @@ int tpc_cf_create(tpc_cf** h, const tpc_cf_geometry* geom, uint64_t max_digits, 
  * synchronising.  digits: DEVICE pointer, 8-byte aligned, any order, at most one digit per cell (R11), must
  * stay alive until the stream has passed the run.  geom must equal the geometry given to create.
  * Synchronous errors (nothing enqueued): negative return.  Asynchronous conditions are in out->status.
- * One handle serves one stream at a time. */
+ * One handle serves one stream at a time.  The call only enqueues kernels, memsets and device-to-device copies on that
+ * stream (no allocation, no synchronisation, no host read), so it may be captured in a CUDA graph (with profiling off)
+ * and replayed on the same buffers; launch-bound small frames gain from that. */
 int tpc_cf_run(tpc_cf* h, const tpc_digit* digits, uint64_t n,
                const tpc_cf_geometry* geom, const tpc_cf_params* params, tpc_cf_out* out);
 

@@ -749,3 +749,36 @@ def test_random_geometries_every_route(seed):
         assert st["path"] == EXPECT_PATH.get(route, 3), (route, st)
         assert st["n_clusters"] == ost["n_clusters"] and st["n_bad_digits"] == n_bad, (route, st, ost)
         assert_clusters_equal(cl, ora, "random geometry %d/%s" % (seed, route))
+
+
+@pytest.mark.parametrize("route", ["fused", "sorted_on_device", "general", "fused+share"])
+def test_run_is_capturable_in_a_cuda_graph(route):
+    """tpc_cf_run only enqueues work on the caller's stream (no allocation, no synchronisation, no host read): the whole
+    call can be captured in a CUDA graph and replayed — the launch-bound small frames (config 1: 3 launches, 64 us) are
+    the case that wants it.  The replay must recompute from the buffers' present contents."""
+    import torch
+    cf = _cf()
+    digits, geom = gen.generate(1), gen.geometry(1)
+    n = digits.shape[0]
+    share = route.endswith("+share")
+    flags = PATHS[route.split("+")[0]] | (cf.SHARE_CHARGE if share else 0)
+    ora, ost = orc.run(digits, *geom[:4], flags=orc.SHARE_CHARGE if share else 0)
+    f = cf.ClusterFinder(*geom[:4], max_digits=n, max_clusters=ost["n_clusters"] + 64)
+    buf = cf.to_device(digits).clone()
+    f.run(buf, n, flags=flags)                    # warm-up outside the capture (module load, attributes)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        f.run(buf, n, flags=flags)
+    for rep in range(3):
+        if rep and not (flags & cf.DIGITS_SORTED):
+            # another order of the same digits in the same buffer: the result must be the same array (R12)
+            perm = torch.from_numpy(np.random.default_rng(rep).permutation(n)).cuda()
+            buf.view(torch.int64).copy_(cf.to_device(digits).view(torch.int64)[perm])
+        f.clusters.zero_(); f.status.zero_()
+        g.replay()
+        cl, st = f.result()
+        assert st["n_clusters"] == ost["n_clusters"] and st["path"] == EXPECT_PATH.get(route.split("+")[0], 3)
+        assert_clusters_equal(cl, ora, "graph replay %d/%s" % (rep, route))
+    del g
+    f.close()
