@@ -12,8 +12,9 @@
  * (readings R1..R19, restated in DESIGN.md §3).  The oracle is that definition executed
  * literally, one (sector,row) plane at a time, single-threaded, sums in int64, moments in double.
  *
- * Parity pins (tests/test_oracle_*.py): hand-evaluated grids tests/golden/E*.txt, brute-force
- * sparse-dict checker, numpy argmax / box-filter special cases, closed-form moments, invariants.
+ * Parity pins (tests/test_oracle_*.py): hand-evaluated grids under tests/golden/ (worked_examples.txt E1..E15,
+ * variant_examples.txt V1..V10, sharing_examples.txt S1..S7), brute-force sparse-dict checker (tests/brute.py),
+ * numpy argmax / box-filter special cases, closed-form moments, invariants.
  * No function in this file is "parity unpinned".
  */
 #ifndef TPC_CF_ORACLE_H
