@@ -174,3 +174,30 @@ def test_capacity_overflow_with_sharing_reports_and_does_not_crash():
         assert st["overflow"] == 1 and st["n_clusters"] == ost["n_clusters"]
         # records far from the cut have all their neighbours: identical to the full run
         assert_clusters_equal(cl[:50], ora[:50], "overflow with sharing/" + path)
+
+
+@pytest.mark.parametrize("path", ["fused", "sorted_on_device", "general"])
+def test_sharing_at_the_limits_of_the_geometry(path):
+    """The largest plane the record fields allow (255 pads x 65535 time bins: the digit searches of K6 run on 16-bit
+    times up to 65534 and the fused path there is k_fused_blocks), tiny planes (fewer pads / time bins than a 5x5 window
+    and than the +-4 neighbour search), and overlapping clusters pressed into the corners."""
+    rng = np.random.default_rng(77)
+    for (P, T, ncl) in ((255, 65535, 3000), (3, 4, 3), (2, 300, 20), (200, 3, 30), (1, 1, 1), (9, 257, 60)):
+        cells = {}
+        for _ in range(ncl):
+            p0, t0 = int(rng.integers(0, P)), int(rng.integers(0, T))
+            for (a, b) in ((0, 0), (0, 3), (2, 1)):                 # three peaks whose windows overlap
+                for dp in range(-1, 2):
+                    for dt in range(-1, 2):
+                        p, t = p0 + a + dp, t0 + b + dt
+                        if 0 <= p < P and 0 <= t < T and rng.random() < 0.8:
+                            cells[(p, t)] = int(rng.integers(1, 400))
+        for p, t in ((P - 1, T - 1), (0, 0), (0, T - 1), (P - 1, 0)):
+            cells[(p, t)] = int(rng.integers(4, 65535))
+        digits = sort_digits(orc.make_digits([(p, t, q) for (p, t), q in cells.items()]))
+        geom = (1, 1, P, T, None)
+        ora, ost = orc.run(digits, *geom[:4], flags=SHARE | 4)
+        data = digits if PATHS[path] & 1 else digits[rng.permutation(digits.shape[0])]
+        cl, st = gpu_run(data, geom, PATHS[path] | SHARE | 4, max_clusters=ost["n_clusters"] + 8, tuning={})
+        assert st["n_clusters"] == ost["n_clusters"]
+        assert_clusters_equal(cl, ora, "sharing at the limits %dx%d/%s" % (P, T, path))
