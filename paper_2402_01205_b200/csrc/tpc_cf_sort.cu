@@ -243,6 +243,8 @@ k_sort_scatter_line(const uint2* __restrict__ in, uint2* __restrict__ out, uint3
 // bitmap word (pre).  rank(t) = pre[t / 32] + popc(bm[t / 32] below bit t): the digit's place in the sorted line.
 // A bit found already set is a duplicate cell (R11 contract violation): raised as Counters::unsorted.
 // The zeroing of line_cnt / line_desc for the fused kernels that follow rides along (line_cnt was the scatter cursor).
+static constexpr int kRankRegs = 16;                                 // digits per lane kept in registers: lines up to 512 digits
+
 __global__ void __launch_bounds__(kSortThreads)
 k_sort_rank_lines(const uint2* __restrict__ in, uint2* __restrict__ out, const uint32_t* __restrict__ line_start,
                   uint32_t n_lines, uint32_t n_time, uint32_t words, uint32_t* __restrict__ line_cnt,
@@ -263,11 +265,32 @@ k_sort_rank_lines(const uint2* __restrict__ in, uint2* __restrict__ out, const u
         if (len == 0u) continue;
         if (len == 1u) { if (lane == 0) out[ls] = in[ls]; continue; }
         uint32_t wlo = 0xffffffffu, whi = 0u;               // words this line touches
-        for (uint32_t i = lane; i < len; i += 32) {
-            const uint32_t t = __ldg(&in[ls + i].y) & 0xffffu;   // (valid digits only: t < n_time)
-            const uint32_t old = atomicOr(&bm[t >> 5], 1u << (t & 31u));
-            dup |= (old >> (t & 31u)) & 1u;
-            wlo = min(wlo, t >> 5); whi = max(whi, t >> 5);
+        // a line of up to 32 * kRankRegs digits is read ONCE, all loads in flight together, and kept in registers
+        // between the two phases; longer lines are read twice
+        const bool in_regs = len <= 32u * (uint32_t)kRankRegs;
+        uint2 d[kRankRegs];
+        if (in_regs) {
+#pragma unroll
+            for (int k = 0; k < kRankRegs; ++k) {
+                const uint32_t i = (uint32_t)lane + 32u * (uint32_t)k;
+                d[k] = i < len ? __ldg(in + ls + i) : make_uint2(0u, 0u);
+            }
+#pragma unroll
+            for (int k = 0; k < kRankRegs; ++k) {
+                if ((uint32_t)lane + 32u * (uint32_t)k < len) {
+                    const uint32_t t = d[k].y & 0xffffu;             // (valid digits only: t < n_time)
+                    const uint32_t old = atomicOr(&bm[t >> 5], 1u << (t & 31u));
+                    dup |= (old >> (t & 31u)) & 1u;
+                    wlo = min(wlo, t >> 5); whi = max(whi, t >> 5);
+                }
+            }
+        } else {
+            for (uint32_t i = lane; i < len; i += 32) {
+                const uint32_t t = __ldg(&in[ls + i].y) & 0xffffu;
+                const uint32_t old = atomicOr(&bm[t >> 5], 1u << (t & 31u));
+                dup |= (old >> (t & 31u)) & 1u;
+                wlo = min(wlo, t >> 5); whi = max(whi, t >> 5);
+            }
         }
         wlo = __reduce_min_sync(0xffffffffu, wlo);
         whi = __reduce_max_sync(0xffffffffu, whi);
@@ -286,11 +309,22 @@ k_sort_rank_lines(const uint2* __restrict__ in, uint2* __restrict__ out, const u
         uint32_t run = inc - mine;
         for (uint32_t w = w0; w < w1; ++w) { pre[w] = (uint16_t)run; run += (uint32_t)__popc(bm[w]); }
         __syncwarp();
-        for (uint32_t i = lane; i < len; i += 32) {
-            const uint2 d = __ldg(in + ls + i);
-            const uint32_t t = d.y & 0xffffu;
-            const uint32_t rank = (uint32_t)pre[t >> 5] + (uint32_t)__popc(bm[t >> 5] & ((1u << (t & 31u)) - 1u));
-            out[ls + min(rank, len - 1u)] = d;              // (min: stays inside the line if a duplicate broke the ranks)
+        if (in_regs) {
+#pragma unroll
+            for (int k = 0; k < kRankRegs; ++k) {
+                if ((uint32_t)lane + 32u * (uint32_t)k < len) {
+                    const uint32_t t = d[k].y & 0xffffu;
+                    const uint32_t rank = (uint32_t)pre[t >> 5] + (uint32_t)__popc(bm[t >> 5] & ((1u << (t & 31u)) - 1u));
+                    out[ls + min(rank, len - 1u)] = d[k];      // (min: stays inside the line if a duplicate broke the ranks)
+                }
+            }
+        } else {
+            for (uint32_t i = lane; i < len; i += 32) {
+                const uint2 e = __ldg(in + ls + i);
+                const uint32_t t = e.y & 0xffffu;
+                const uint32_t rank = (uint32_t)pre[t >> 5] + (uint32_t)__popc(bm[t >> 5] & ((1u << (t & 31u)) - 1u));
+                out[ls + min(rank, len - 1u)] = e;
+            }
         }
         __syncwarp();
         for (uint32_t w = w0; w < w1; ++w) bm[w] = 0u;
