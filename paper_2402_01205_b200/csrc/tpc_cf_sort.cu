@@ -38,9 +38,9 @@ __device__ __forceinline__ uint32_t sort_line_of(const Geo& g, uint32_t w0, uint
 static constexpr int kTopThreads = 1024;                             // top-level pass: tiles of 8192 digits, so that a
 static constexpr int kTopTileN = kTopThreads * kSortPerThread;       //   (tile, bucket) run is ~11 digits, not ~3
 static constexpr int kSortBlocks = 148 * 2;                          // persistent blocks of the top-level pass
-static constexpr int kLineThreads = 1024;                            // line-level scatter: tiles of 8192 digits
+static constexpr int kLineThreads = 512;                             // line-level scatter: tiles of 4096 digits, 4 blocks per SM
 static constexpr int kLineTileN = kLineThreads * kSortPerThread;
-static constexpr uint32_t kLineBins = 4096;                          // lines a tile may span for the aggregated path
+static constexpr uint32_t kLineBins = 1024;                          // lines a tile may span for the aggregated path (one top-level bucket)
 
 // first position of every top-level bucket = line_start of its first line (the overflow bin ends at n)
 __global__ void k_sort_top_cursors(const uint32_t* __restrict__ line_start, uint32_t n_lines, uint32_t shift, uint32_t n,
@@ -139,8 +139,8 @@ k_sort_count_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t
     }
 }
 
-// Line level: cursor[l] starts at line_start[l].  The input is grouped by top-level bucket, so a tile of 8192 digits spans
-// few buckets: its digits are ranked per line in shared memory and ONE global atomic per (tile, line) reserves the range
+// Line level: cursor[l] starts at line_start[l].  The input is grouped by top-level bucket, so a tile of 4096 digits spans
+// few lines: its digits are ranked per line in shared memory and ONE global atomic per (tile, line) reserves the range
 // (a tile spanning more than kLineBins lines — sparse data — takes one atomic per digit instead).
 __global__ void __launch_bounds__(kLineThreads)
 k_sort_scatter_line(const uint2* __restrict__ in, uint2* __restrict__ out, uint32_t n, Geo g, uint32_t n_lines,
@@ -159,25 +159,34 @@ k_sort_scatter_line(const uint2* __restrict__ in, uint2* __restrict__ out, uint3
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const uint64_t t0 = (uint64_t)tile * kLineTileN, t1 = min((uint64_t)n, t0 + kLineTileN);
         const uint32_t m = (uint32_t)(t1 - t0);
-        if (tid == 0) {
-            const uint2 a = __ldg(in + t0), z = __ldg(in + (t1 - 1));
-            s_l0 = (sort_line_of(g, a.x, a.y, n_lines) >> shift) << shift;
-            s_l1 = min(n_lines + 1u, ((sort_line_of(g, z.x, z.y, n_lines) >> shift) + 1u) << shift);
+        // the tile's digits first (all loads in flight), then the range of lines it spans: the input is grouped by
+        // top-level bucket, so the range is one bucket (rarely two)
+        uint2 d[kSortPerThread];
+        uint32_t bin[kSortPerThread], rk[kSortPerThread];
+        uint32_t lmin = 0xffffffffu, lmax = 0u;
+        if (tid == 0) { s_l0 = 0xffffffffu; s_l1 = 0u; }
+        for (uint32_t i = tid; i < kLineBins; i += kLineThreads) s_cnt[i] = 0u;
+#pragma unroll
+        for (int j = 0; j < kSortPerThread; ++j) {
+            const uint32_t i = (uint32_t)j * kLineThreads + tid;
+            bin[j] = 0xffffffffu;
+            if (i < m) {
+                d[j] = __ldg(in + t0 + i);
+                bin[j] = sort_line_of(g, d[j].x, d[j].y, n_lines);
+                lmin = min(lmin, bin[j]); lmax = max(lmax, bin[j]);
+            }
         }
         __syncthreads();
-        const uint32_t l0 = s_l0, span = s_l1 - l0;
+        lmin = __reduce_min_sync(0xffffffffu, lmin);
+        lmax = __reduce_max_sync(0xffffffffu, lmax);
+        if (lane == 0) { atomicMin(&s_l0, lmin); atomicMax(&s_l1, lmax); }
+        __syncthreads();
+        const uint32_t l0 = s_l0, span = s_l1 - l0 + 1u;
         if (span <= kLineBins) {
-            for (uint32_t i = tid; i < kLineBins; i += kLineThreads) s_cnt[i] = 0u;
-            __syncthreads();
-            uint2 d[kSortPerThread];
-            uint32_t bin[kSortPerThread], rk[kSortPerThread];
 #pragma unroll
             for (int j = 0; j < kSortPerThread; ++j) {
-                const uint32_t i = (uint32_t)j * kLineThreads + tid;
-                bin[j] = 0xffffffffu;
-                if (i < m) {
-                    d[j] = __ldg(in + t0 + i);
-                    bin[j] = sort_line_of(g, d[j].x, d[j].y, n_lines) - l0;
+                if (bin[j] != 0xffffffffu) {
+                    bin[j] -= l0;
                     rk[j] = atomicAdd(&s_cnt[bin[j]], 1u);
                 }
             }
@@ -195,7 +204,7 @@ k_sort_scatter_line(const uint2* __restrict__ in, uint2* __restrict__ out, uint3
                 if (lane == 31) s_warp[warp] = inc;
                 __syncthreads();
                 if (warp == 0) {
-                    const uint32_t w = s_warp[lane];
+                    const uint32_t w = lane < kLineThreads / 32 ? s_warp[lane] : 0u;
                     uint32_t winc = w;
 #pragma unroll
                     for (int o = 1; o < 32; o <<= 1) {
@@ -376,7 +385,7 @@ int launch_sort_digits(const Geo& g, const Workspace& ws, const tpc_digit* digit
     k += 2;
     // the fused kernels read line_start[n_lines] as the end of the last plane: the overflow bin (invalid digits) starts there
     cudaMemcpyAsync(ws.line_cnt, ws.line_start, ((size_t)n_lines + 1) * 4, cudaMemcpyDeviceToDevice, st);
-    k_sort_scatter_line<<<148 * 2, kLineThreads, kLineTileN * sizeof(uint2) + 3 * kLineBins * 4, st>>>(tmp, tmp2, (uint32_t)n, g, n_lines, shift, ws.line_cnt);
+    k_sort_scatter_line<<<148 * 4, kLineThreads, kLineTileN * sizeof(uint2) + 3 * kLineBins * 4, st>>>(tmp, tmp2, (uint32_t)n, g, n_lines, shift, ws.line_cnt);
     uint32_t words;
     const uint32_t smem = sort_rank_smem(g, &words);
     k_sort_rank_lines<<<grid, kSortThreads, smem, st>>>(tmp2, tmp, ws.line_start, n_lines, g.n_time, words, ws.line_cnt,
