@@ -70,17 +70,31 @@ k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32
     s_cnt[tid] = 0u;
     __syncthreads();
     const uint32_t n_tiles = (uint32_t)(((uint64_t)n + kTopTileN - 1) / kTopTileN);
+    // the digits of the block's next tile are loaded while the present one is ranked, staged and written
+    uint2 dn[kSortPerThread];
+    auto load_tile = [&](uint32_t tile) {
+        const uint64_t t0 = (uint64_t)tile * kTopTileN;
+        const uint32_t m = tile < n_tiles ? (uint32_t)min((uint64_t)kTopTileN, (uint64_t)n - t0) : 0u;
+#pragma unroll
+        for (int j = 0; j < kSortPerThread; ++j) {
+            const uint32_t i = (uint32_t)j * kTopThreads + tid;
+            if (i < m) dn[j] = __ldg(in + t0 + i);
+        }
+    };
+    load_tile(blockIdx.x);
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const uint64_t t0 = (uint64_t)tile * kTopTileN;
         const uint32_t m = (uint32_t)min((uint64_t)kTopTileN, (uint64_t)n - t0);     // digits in this tile
         uint2 d[kSortPerThread];
         uint32_t bin[kSortPerThread], rk[kSortPerThread];
 #pragma unroll
+        for (int j = 0; j < kSortPerThread; ++j) d[j] = dn[j];
+        load_tile(tile + gridDim.x);
+#pragma unroll
         for (int j = 0; j < kSortPerThread; ++j) {
             const uint32_t i = (uint32_t)j * kTopThreads + tid;
             bin[j] = 0xffffffffu;
             if (i < m) {
-                d[j] = __ldg(in + t0 + i);
                 bin[j] = sort_line_of(g, d[j].x, d[j].y, n_lines) >> shift;
                 rk[j] = atomicAdd(&s_cnt[bin[j]], 1u);
             }
@@ -156,22 +170,36 @@ k_sort_scatter_line(const uint2* __restrict__ in, uint2* __restrict__ out, uint3
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr uint32_t kPer = kLineBins / kLineThreads;           // bins per thread in the block scan
     const uint32_t n_tiles = (uint32_t)(((uint64_t)n + kLineTileN - 1) / kLineTileN);
+    // the digits of the block's next tile are loaded while the present one is ranked, staged and written
+    uint2 dn[kSortPerThread];
+    auto load_tile = [&](uint32_t tile) {
+        const uint64_t t0 = (uint64_t)tile * kLineTileN;
+        const uint32_t m = tile < n_tiles ? (uint32_t)min((uint64_t)kLineTileN, (uint64_t)n - t0) : 0u;
+#pragma unroll
+        for (int j = 0; j < kSortPerThread; ++j) {
+            const uint32_t i = (uint32_t)j * kLineThreads + tid;
+            if (i < m) dn[j] = __ldg(in + t0 + i);
+        }
+    };
+    load_tile(blockIdx.x);
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const uint64_t t0 = (uint64_t)tile * kLineTileN, t1 = min((uint64_t)n, t0 + kLineTileN);
         const uint32_t m = (uint32_t)(t1 - t0);
-        // the tile's digits first (all loads in flight), then the range of lines it spans: the input is grouped by
-        // top-level bucket, so the range is one bucket (rarely two)
+        // the range of lines the tile spans comes from its digits: the input is grouped by top-level bucket, so the
+        // range is one bucket (rarely parts of two)
         uint2 d[kSortPerThread];
         uint32_t bin[kSortPerThread], rk[kSortPerThread];
         uint32_t lmin = 0xffffffffu, lmax = 0u;
         if (tid == 0) { s_l0 = 0xffffffffu; s_l1 = 0u; }
         for (uint32_t i = tid; i < kLineBins; i += kLineThreads) s_cnt[i] = 0u;
 #pragma unroll
+        for (int j = 0; j < kSortPerThread; ++j) d[j] = dn[j];
+        load_tile(tile + gridDim.x);
+#pragma unroll
         for (int j = 0; j < kSortPerThread; ++j) {
             const uint32_t i = (uint32_t)j * kLineThreads + tid;
             bin[j] = 0xffffffffu;
             if (i < m) {
-                d[j] = __ldg(in + t0 + i);
                 bin[j] = sort_line_of(g, d[j].x, d[j].y, n_lines);
                 lmin = min(lmin, bin[j]); lmax = max(lmax, bin[j]);
             }
