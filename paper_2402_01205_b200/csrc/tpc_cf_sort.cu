@@ -35,6 +35,18 @@ __device__ __forceinline__ uint32_t sort_line_of(const Geo& g, uint32_t w0, uint
     return digit_valid(g, w0, w1) ? (s * g.n_rows + r) * g.LS + p : n_lines;
 }
 
+// The same with the pads-per-row table in SHARED memory: g.npads[] lives in the kernel's parameter space, and a load
+// from there with a per-lane index (the rows of unordered digits differ from lane to lane) is replayed once per distinct
+// row of the warp.
+__device__ __forceinline__ uint32_t sort_line_of_s(const Geo& g, const uint8_t* s_np, uint32_t w0, uint32_t w1,
+                                                   uint32_t n_lines)
+{
+    const uint32_t s = w0 & 0xffu, r = (w0 >> 8) & 0xffu, p = (w0 >> 16) & 0xffu;
+    const uint32_t t = w1 & 0xffffu, q = w1 >> 16;
+    const bool ok = s < g.n_sectors && r < g.n_rows && p < (uint32_t)s_np[r] && t < g.n_time && q != 0u;
+    return ok ? (s * g.n_rows + r) * g.LS + p : n_lines;
+}
+
 static constexpr int kTopThreads = 1024;                             // top-level pass: tiles of 8192 digits, so that a
 static constexpr int kTopTileN = kTopThreads * kSortPerThread;       //   (tile, bucket) run is ~11 digits, not ~3
 static constexpr int kSortBlocks = 148 * 2;                          // persistent blocks of the top-level pass
@@ -65,9 +77,11 @@ k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32
     __shared__ uint32_t s_off[kSortTopBins];                     // first position of the bucket inside the tile
     __shared__ uint32_t s_cur[kSortTopBins];                     // output position of the bucket's run of this tile
     __shared__ uint32_t s_warp[32];
+    __shared__ uint8_t s_np[256];                                // pads per row (see sort_line_of_s)
     static_assert(kTopThreads == (int)kSortTopBins, "one thread per bucket in the block scan");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     s_cnt[tid] = 0u;
+    if (tid < 256) s_np[tid] = g.npads[tid];
     __syncthreads();
     const uint32_t n_tiles = (uint32_t)(((uint64_t)n + kTopTileN - 1) / kTopTileN);
     // the digits of the block's next tile are loaded while the present one is ranked, staged and written
@@ -95,7 +109,7 @@ k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32
             const uint32_t i = (uint32_t)j * kTopThreads + tid;
             bin[j] = 0xffffffffu;
             if (i < m) {
-                bin[j] = sort_line_of(g, d[j].x, d[j].y, n_lines) >> shift;
+                bin[j] = sort_line_of_s(g, s_np, d[j].x, d[j].y, n_lines) >> shift;
                 rk[j] = atomicAdd(&s_cnt[bin[j]], 1u);
             }
         }
@@ -134,7 +148,7 @@ k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32
             const uint32_t i = (uint32_t)j * kTopThreads + tid;
             if (i < m) {
                 const uint2 e = s_tile[i];
-                const uint32_t b2 = sort_line_of(g, e.x, e.y, n_lines) >> shift;
+                const uint32_t b2 = sort_line_of_s(g, s_np, e.x, e.y, n_lines) >> shift;
                 out[s_cur[b2] + (i - s_off[b2])] = e;
             }
         }
@@ -147,9 +161,12 @@ k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32
 __global__ void __launch_bounds__(kSortThreads)
 k_sort_count_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t n_lines, uint32_t* __restrict__ line_cnt)
 {
+    __shared__ uint8_t s_np[256];
+    s_np[threadIdx.x] = g.npads[threadIdx.x];
+    __syncthreads();
     for (uint64_t i = (uint64_t)blockIdx.x * kSortThreads + threadIdx.x; i < n; i += (uint64_t)gridDim.x * kSortThreads) {
         const uint2 d = __ldg(digits + i);
-        atomicAdd(&line_cnt[sort_line_of(g, d.x, d.y, n_lines)], 1u);
+        atomicAdd(&line_cnt[sort_line_of_s(g, s_np, d.x, d.y, n_lines)], 1u);
     }
 }
 
