@@ -8,12 +8,14 @@
 // unique inside a line (R11: one digit per cell).  So: an UNSTABLE two-level partition of the digits by pad line (order
 // inside a line does not matter yet), then one warp per line ranks its digits by time with a bitmap (rank = set bits
 // below).  No comparison sort, no stable radix pass:
-//   k_sort_count_lines digits per pad line, on the input as it comes (no-return atomics on a 3 MB table)
-//   scan (n_lines + 1) -> line_start: THE LINE INDEX OF THE FUSED PATH (k_plane_index / k_line_index are not needed);
-//                      a top-level bucket (1024 consecutive lines) starts at line_start of its first line
+//   k_sort_count_top   digits per top-level bucket (<= 1024 buckets of 2^shift consecutive lines): a shared-memory
+//                      histogram per block; k_sort_top_scan turns the counts into the buckets' first positions
 //   k_sort_scatter_top tile of 8192 digits: ranks per bucket by shared-memory atomics, the tile staged in bucket order,
 //                      one global atomic per (tile, bucket) reserves the run -> digits grouped by bucket in ws.sort_tmp
-//   k_sort_scatter_line tile of 8192 digits (few buckets): the same per line -> digits grouped by line in the cluster
+//   k_sort_count_grouped digits per pad line, counted on the grouped digits: two blocks per bucket, shared-memory
+//                      histogram of the bucket's lines, one global atomic per line
+//   scan (n_lines + 1) -> line_start: THE LINE INDEX OF THE FUSED PATH (k_plane_index / k_line_index are not needed)
+//   k_sort_scatter_line tile of 4096 digits (one bucket, rarely two): the same per line -> digits grouped by line in the cluster
 //                      staging area (idle here)
 //   k_sort_rank_lines  one warp per line: time bitmap + rank directory in shared memory -> sorted digits in ws.sort_tmp
 // Invalid digits (R11: out-of-range sector / row / pad / time, zero charge) go to an overflow bin behind the last line:
@@ -54,14 +56,84 @@ static constexpr int kLineThreads = 512;                             // line-lev
 static constexpr int kLineTileN = kLineThreads * kSortPerThread;
 static constexpr uint32_t kLineBins = 1024;                          // lines a tile may span for the aggregated path (one top-level bucket)
 
-// first position of every top-level bucket = line_start of its first line (the overflow bin ends at n)
-__global__ void k_sort_top_cursors(const uint32_t* __restrict__ line_start, uint32_t n_lines, uint32_t shift, uint32_t n,
-                                   uint32_t* __restrict__ top_cur)
+// digits per top-level bucket: a histogram per block in shared memory, one global atomic per (block, bucket)
+__global__ void __launch_bounds__(1024)
+k_sort_count_top(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t n_lines, uint32_t shift,
+                 uint32_t* __restrict__ top_cnt)
 {
-    const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= kSortTopBins) return;
-    const uint64_t l = (uint64_t)b << shift;
-    top_cur[b] = l <= n_lines ? line_start[l] : n;
+    __shared__ uint32_t s_h[kSortTopBins];
+    __shared__ uint8_t s_np[256];
+    s_h[threadIdx.x] = 0u;
+    if (threadIdx.x < 256) s_np[threadIdx.x] = g.npads[threadIdx.x];
+    __syncthreads();
+    for (uint64_t i = (uint64_t)blockIdx.x * 1024u + threadIdx.x; i < n; i += (uint64_t)gridDim.x * 1024u) {
+        const uint2 d = __ldg(digits + i);
+        atomicAdd(&s_h[sort_line_of_s(g, s_np, d.x, d.y, n_lines) >> shift], 1u);
+    }
+    __syncthreads();
+    if (s_h[threadIdx.x]) atomicAdd(&top_cnt[threadIdx.x], s_h[threadIdx.x]);
+}
+
+// counts -> first position of every top-level bucket (exclusive scan of 1024 values, one block); a copy stays in
+// top_start for the line count
+__global__ void __launch_bounds__(1024)
+k_sort_top_scan(uint32_t* __restrict__ top_cur)
+{
+    __shared__ uint32_t s_w[32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t c = top_cur[tid];
+    uint32_t inc = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t up = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += up;
+    }
+    if (lane == 31) s_w[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        const uint32_t w = s_w[lane];
+        uint32_t winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t up = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += up;
+        }
+        s_w[lane] = winc - w;
+    }
+    __syncthreads();
+    top_cur[tid] = s_w[warp] + inc - c;
+}
+
+// digits per pad line, counted on the digits GROUPED BY BUCKET (after the top-level pass top_cur[b] is the END of bucket
+// b): kCountSplit blocks per bucket count their share of the bucket in shared memory (a bucket is 2^shift <= kCountBins
+// consecutive lines) and flush with one global atomic per line — 2 M atomics instead of one per digit.  Buckets of more
+// lines than the histogram holds (geometries far beyond the TPC's) are counted with one global atomic per digit.
+static constexpr uint32_t kCountBins = 2048, kCountSplit = 2, kCountThreads = 512;
+__global__ void __launch_bounds__(kCountThreads)
+k_sort_count_grouped(const uint2* __restrict__ digits, Geo g, uint32_t n_lines, uint32_t shift,
+                     const uint32_t* __restrict__ top_end, uint32_t* __restrict__ line_cnt)
+{
+    __shared__ uint32_t s_h[kCountBins];
+    __shared__ uint8_t s_np[256];                                 // pads per row (see sort_line_of_s)
+    if (threadIdx.x < 256) s_np[threadIdx.x] = g.npads[threadIdx.x];
+    const uint32_t b = blockIdx.x / kCountSplit, part = blockIdx.x % kCountSplit;
+    const uint32_t beg = b ? top_end[b - 1u] : 0u, end = top_end[b];
+    if (end <= beg) return;
+    const uint32_t len = end - beg, per = (len + kCountSplit - 1u) / kCountSplit;
+    const uint32_t lo = beg + part * per, hi = min(end, lo + per);
+    const uint32_t l0 = b << shift;
+    const bool fits = (1u << shift) <= kCountBins;
+    for (uint32_t i = threadIdx.x; i < kCountBins; i += kCountThreads) s_h[i] = 0u;
+    __syncthreads();
+    for (uint32_t i = lo + threadIdx.x; i < hi; i += kCountThreads) {
+        const uint2 d = __ldg(digits + i);
+        const uint32_t line = sort_line_of_s(g, s_np, d.x, d.y, n_lines);
+        if (fits) atomicAdd(&s_h[line - l0], 1u); else atomicAdd(&line_cnt[line], 1u);
+    }
+    __syncthreads();
+    if (fits)
+        for (uint32_t i = threadIdx.x; i < kCountBins; i += kCountThreads)
+            if (s_h[i]) atomicAdd(&line_cnt[l0 + i], s_h[i]);
 }
 
 // Top level: a tile of 8192 digits; the (tile, bucket) run is reserved by one global atomic on the bucket's cursor.
@@ -155,18 +227,6 @@ k_sort_scatter_top(const uint2* __restrict__ in, uint2* __restrict__ out, uint32
         __syncthreads();
         s_cnt[tid] = 0u;
         __syncthreads();
-    }
-}
-
-__global__ void __launch_bounds__(kSortThreads)
-k_sort_count_lines(const uint2* __restrict__ digits, uint32_t n, Geo g, uint32_t n_lines, uint32_t* __restrict__ line_cnt)
-{
-    __shared__ uint8_t s_np[256];
-    s_np[threadIdx.x] = g.npads[threadIdx.x];
-    __syncthreads();
-    for (uint64_t i = (uint64_t)blockIdx.x * kSortThreads + threadIdx.x; i < n; i += (uint64_t)gridDim.x * kSortThreads) {
-        const uint2 d = __ldg(digits + i);
-        atomicAdd(&line_cnt[sort_line_of_s(g, s_np, d.x, d.y, n_lines)], 1u);
     }
 }
 
@@ -423,11 +483,12 @@ int launch_sort_digits(const Geo& g, const Workspace& ws, const tpc_digit* digit
     const int grid = 148 * 8;
     int k = 0;
     cudaMemsetAsync(ws.line_cnt, 0, ((size_t)n_lines + 2) * 4, st);
-    k_sort_count_lines<<<grid, kSortThreads, 0, st>>>(in, (uint32_t)n, g, n_lines, ws.line_cnt);
-    k += 1 + launch_scan_u32(ws.line_cnt, ws.line_start, (uint64_t)n_lines + 1, ws.sort_part, nullptr, st);
-    k_sort_top_cursors<<<kSortTopBins / 256, 256, 0, st>>>(ws.line_start, n_lines, shift, (uint32_t)n, ws.sort_top);
+    cudaMemsetAsync(ws.sort_top, 0, (size_t)kSortTopBins * 4, st);
+    k_sort_count_top<<<kSortBlocks, 1024, 0, st>>>(in, (uint32_t)n, g, n_lines, shift, ws.sort_top);
+    k_sort_top_scan<<<1, 1024, 0, st>>>(ws.sort_top);
     k_sort_scatter_top<<<kSortBlocks, kTopThreads, kTopTileN * sizeof(uint2), st>>>(in, tmp, (uint32_t)n, g, n_lines, shift, ws.sort_top);
-    k += 2;
+    k_sort_count_grouped<<<kSortTopBins * kCountSplit, kCountThreads, 0, st>>>(tmp, g, n_lines, shift, ws.sort_top, ws.line_cnt);
+    k += 4 + launch_scan_u32(ws.line_cnt, ws.line_start, (uint64_t)n_lines + 1, ws.sort_part, nullptr, st);
     // the fused kernels read line_start[n_lines] as the end of the last plane: the overflow bin (invalid digits) starts there
     cudaMemcpyAsync(ws.line_cnt, ws.line_start, ((size_t)n_lines + 1) * 4, cudaMemcpyDeviceToDevice, st);
     k_sort_scatter_line<<<148 * 4, kLineThreads, kLineTileN * sizeof(uint2) + 3 * kLineBins * 4, st>>>(tmp, tmp2, (uint32_t)n, g, n_lines, shift, ws.line_cnt);
